@@ -1,0 +1,150 @@
+/*
+ * cs.h -- C ABI of libcs: batched parametric spectral likelihood for CMB component separation on NVIDIA B200.
+ *
+ * The hot path of arxiv 2604.08463: for every batch entry e = (clustering configuration, data set,
+ * parameter vector) and every unmasked pixel p
+ *
+ *     A_p      = [1, a_d(nu; beta_d[k0], T_d[k1]), a_s(nu; beta_s[k2])]        Eq. 2
+ *     M_p      = A^T N^-1 A ,  b_S = A^T N^-1 d_S   (S = Q, U)                 L233, Eq. 5 (L76)
+ *     s_S      = M^-1 b_S                                                       Eq. 5 / 8 (L76, L128)
+ *     nll      = -1/2 sum_p sum_S b_S . s_S                                     Eq. 6 negated, const 0 (L80)
+ *     grad[k]  = - sum_{p in k} sum_S (N^-1 (d_S - A s_S))^T (dA/dtheta_k) s_S  Eq. 17 (L241), factor 1 for this nll
+ *
+ * with k0,k1,k2 the pixel's cluster ids in three independent cluster maps (patch model, L93-L98).
+ * Everything runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *   - frequencies in GHz, maps in uK_CMB, HEALPix RING order is whatever order the caller uses: the library only
+ *     needs d, cluster maps and region_idx to share one pixel order.
+ *   - "dev" = pointer to device memory on the current CUDA device; "host" = host memory; "any" = either (copied
+ *     with cudaMemcpyDefault during the call).  Borrowed pointers must stay valid and unchanged until replaced.
+ *   - every function returns CS_OK (0) or a negative CS_E* code; nothing throws; no global state; a context is
+ *     bound to the CUDA device current at cs_create and must be used from one stream at a time.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Hot-path calls are
+ *     asynchronous on it and allocate nothing.
+ *
+ * Parameter layout: entry e owns params[off[e] .. off[e+1]) = [beta_d x K0 ; T_d x K1 ; beta_s x K2] where
+ * (K0,K1,K2) are the cluster counts of the three maps of its configuration; off[] = cs_param_offsets().
+ * grad has the same layout.  nll is [batch, nregion].
+ */
+#ifndef CS_H
+#define CS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CS_OK          0
+#define CS_EINVAL     -1   /* bad argument / call order */
+#define CS_EINDEX     -2   /* a cluster id or region id is out of range (checked bit-exactly, nothing computed) */
+#define CS_EDOMAIN    -3   /* device error bit: T_d <= 0 or a non-finite parameter seen by cs_build_sed_tables */
+#define CS_ESINGULAR  -4   /* device error bit: a pixel's M = A^T N^-1 A had a non-positive pivot; that nll = +inf */
+#define CS_ECUDA      -5   /* a CUDA runtime call failed */
+#define CS_ENOMEM     -6   /* allocation failed */
+
+#define CS_UNITS_KCMB    0 /* dust/synchrotron columns carry the K_RJ -> K_CMB factor u(nu)/u(nu0) (default) */
+#define CS_UNITS_LITERAL 1 /* Eq. 2 as printed (brightness-temperature units), no unit factor */
+
+#define CS_MAX_NFREQ 16
+
+#if defined(__GNUC__)
+#define CS_API __attribute__((visibility("default")))
+#else
+#define CS_API
+#endif
+
+typedef struct cs_ctx cs_ctx;
+
+/* Sky / instrument model (Eq. 2).  3 components: CMB (column of ones), dust modified black
+ * body normalised at nu0_dust, synchrotron power law normalised at nu0_sync. */
+typedef struct cs_model {
+    int32_t nfreq;            /* 3 .. CS_MAX_NFREQ */
+    const double *freqs_ghz;  /* host [nfreq] */
+    double nu0_dust_ghz;      /* 353 in the paper's setup */
+    double nu0_sync_ghz;      /* 23 */
+    double t_cmb_k;           /* 2.7255 */
+    int32_t units;            /* CS_UNITS_* */
+    int64_t npix;             /* pixels per map */
+} cs_model;
+
+/* Fixed-budget optimizer options (AdaTopK, App. A, Alg. 1; hyper-parameters: DESIGN.md R13). */
+typedef struct cs_opt {
+    int32_t iters;      /* number of iterations (no convergence test) */
+    int32_t ls_max;     /* backtracking trials per iteration (value-only evaluations) */
+    double lr;          /* AdaBelief step size in [0,1] units */
+    double beta1, beta2, eps;
+    double ls_c1;       /* Armijo constant */
+    double safe_lo, safe_hi; /* dynamic rescale range for |g_proj| (A4, L541) */
+} cs_opt;
+
+/* Create a context for `model`.  Allocates only small constant tables.  *out is NULL on failure. */
+CS_API int cs_create(cs_ctx **out, const cs_model *model);
+CS_API int cs_destroy(cs_ctx *ctx);
+
+/* Patch model: `maps` holds nmap cluster maps [nmap, npix] int32 (any); Kmap[nmap] (host) their
+ * cluster counts; a clustering configuration c is a triple cfg_maps[c] = (map for beta_d, map for T_d, map for
+ * beta_s) (host [ncfg,3]).  A cluster id of -1 in any of a configuration's three maps masks the pixel for that
+ * configuration (L211).  region_idx (any, [npix], values < nregion) or NULL with nregion = 1 splits nll by sky
+ * region (L269).  Validates -1 <= id < K bit-exactly (CS_EINDEX otherwise, context unchanged), copies the maps
+ * (the caller may free them) and builds the per-tile segment plan of the ordered cluster reduction. */
+CS_API int cs_set_clusters(cs_ctx *ctx, int32_t nmap, const int32_t *maps, const int32_t *Kmap,
+                    int32_t ncfg, const int32_t *cfg_maps, const uint8_t *region_idx, int32_t nregion);
+
+/* Data (Eq. 1): d dev [ndata, nfreq, 2, npix] fp32 (Q then U per band, pixel fastest), borrowed;
+ * ninv any [nfreq] fp32 = 1/sigma_f^2, the same for Q, U and every pixel (L219), copied. */
+CS_API int cs_set_data(cs_ctx *ctx, int32_t ndata, const float *d, const float *ninv);
+
+/* Batch: entry e evaluates configuration cfg_of[e] on data set data_of[e] (both host [batch]).  Allocates the
+ * SED tables and the reduction workspace for this batch (the only allocation outside cs_create/cs_set_clusters). */
+CS_API int cs_set_batch(cs_ctx *ctx, int32_t batch, const int32_t *cfg_of, const int32_t *data_of);
+
+/* off host [batch+1] int64: parameter offsets of the current batch. */
+CS_API int cs_param_offsets(cs_ctx *ctx, int64_t *off);
+
+/* a1 (Eq. 2): per entry, cluster and band the separable SED factors cd*(nu/nu0d)^beta_d, the Planck ratio
+ * B-factor G(nu,T_d), its log-derivative dlnG/dT_d and cs*(nu/nu0s)^beta_s, evaluated in fp64 and stored fp32.
+ * params dev fp64 (layout above).  Sets the sticky device bit CS_EDOMAIN on T_d <= 0 / non-finite input. */
+CS_API int cs_build_sed_tables(cs_ctx *ctx, const double *params, void *stream);
+
+/* a2+a3: fused per-pixel likelihood / gradient and the ordered fp64 reduction onto clusters, for the tables last
+ * built.  nll dev [batch*nregion] fp64; grad dev fp64 (parameter layout) or NULL for value only.
+ * Results are bitwise reproducible and independent of how entries are grouped into batches. */
+CS_API int cs_spectral_like_grad(cs_ctx *ctx, double *nll, double *grad, void *stream);
+
+/* a4 (Eq. 5/8): GLS component maps s dev [nsel, 3, 2, npix] fp32 (cmb, dust@nu0d, sync@nu0s; Q,U) for entries
+ * `entries` (host [nsel]) or all entries in order when entries == NULL (then nsel must equal batch).  Masked
+ * pixels are written as 0. */
+CS_API int cs_component_maps(cs_ctx *ctx, int32_t nsel, const int32_t *entries, float *s, void *stream);
+
+/* f1 (Eq. 10): per entry and region, variance over unmasked pixels of the reconstructed CMB map, Q and U
+ * summed: var dev [batch*nregion] fp64, computed without writing the maps. */
+CS_API int cs_cmb_variance(cs_ctx *ctx, double *var, void *stream);
+
+/* a5: device-resident fixed-budget AdaTopK (Alg. 1) on every entry independently; calls only
+ * cs_build_sed_tables and cs_spectral_like_grad.  params dev in: start, out: result; lower/upper dev, same layout;
+ * nll_final dev [batch] (summed over regions) or NULL.  No host synchronisation. */
+CS_API int cs_optimize(cs_ctx *ctx, double *params, const double *lower, const double *upper, const cs_opt *opt,
+                double *nll_final, void *stream);
+CS_API void cs_opt_defaults(cs_opt *opt);
+
+/* Convenience for end-to-end use from host memory: uploads d_host [ndata,nfreq,2,npix] (pinned or pageable) in
+ * chunks overlapped with compute, evaluates the current batch and returns nll / grad in host memory.
+ * Requires data_of to be non-decreasing over the batch.  Synchronous. */
+CS_API int cs_eval_host(cs_ctx *ctx, int32_t ndata, const float *d_host, const float *ninv_host, const double *params_host,
+                 double *nll_host, double *grad_host);
+
+/* Synchronises `stream`, returns and clears the sticky device error bits: CS_OK, CS_EDOMAIN or CS_ESINGULAR. */
+CS_API int cs_check(cs_ctx *ctx, void *stream);
+CS_API const char *cs_strerror(int code);
+
+/* Introspection used by the bench and the tests. */
+CS_API int64_t cs_workspace_bytes(cs_ctx *ctx);      /* device bytes currently held by the context */
+CS_API int64_t cs_kernel_launches(cs_ctx *ctx);      /* kernels launched by this context so far */
+CS_API int cs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CS_H */

@@ -1,0 +1,9 @@
+"""B200-native batched parametric spectral likelihood for CMB component separation (arxiv 2604.08463).
+
+The product is the CUDA library `libcs.so` (C ABI: include/cs.h, sources: csrc/).  This package is its thin
+Python binding; see DESIGN.md.
+"""
+from .binding import (  # noqa: F401
+    Context, CsError, CsOpt, opt_defaults, lib, strerror, EXPORTS,
+    OK, EINVAL, EINDEX, EDOMAIN, ESINGULAR, ECUDA, ENOMEM, UNITS_KCMB, UNITS_LITERAL,
+)

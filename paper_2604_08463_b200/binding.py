@@ -1,0 +1,216 @@
+"""Thin ctypes binding of libcs (include/cs.h): argument marshalling only, same names as the C ABI.
+
+PyTorch supplies device memory and streams; every step of the hot path runs in the CUDA kernels of
+csrc/.  There is no CPU fallback: loading fails loudly when libcs.so is missing and cannot be built.
+"""
+import ctypes as C
+import os
+import numpy as np
+
+from . import build as _build
+
+OK, EINVAL, EINDEX, EDOMAIN, ESINGULAR, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5, -6
+UNITS_KCMB, UNITS_LITERAL = 0, 1
+
+EXPORTS = ["cs_create", "cs_destroy", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
+           "cs_build_sed_tables", "cs_spectral_like_grad", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
+           "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
+           "cs_version"]
+
+
+class CsModel(C.Structure):
+    _fields_ = [("nfreq", C.c_int32), ("freqs_ghz", C.POINTER(C.c_double)), ("nu0_dust_ghz", C.c_double),
+                ("nu0_sync_ghz", C.c_double), ("t_cmb_k", C.c_double), ("units", C.c_int32), ("npix", C.c_int64)]
+
+
+class CsOpt(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("ls_max", C.c_int32), ("lr", C.c_double), ("beta1", C.c_double),
+                ("beta2", C.c_double), ("eps", C.c_double), ("ls_c1", C.c_double), ("safe_lo", C.c_double),
+                ("safe_hi", C.c_double)]
+
+
+class CsError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} ({code})")
+
+
+_lib = None
+
+
+def lib():
+    """Loads (building first if stale and nvcc is present) libcs.so; raises if it cannot."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.stale():
+        try:
+            path = _build.build()
+        except Exception as exc:  # no nvcc on the box: use the shipped .so if there is one
+            if not os.path.exists(path):
+                raise RuntimeError(f"libcs.so is missing and could not be built: {exc}") from exc
+    L = C.CDLL(path)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    sig = {
+        "cs_create": (C.c_int, [C.POINTER(vp), C.POINTER(CsModel)]),
+        "cs_destroy": (C.c_int, [vp]),
+        "cs_set_clusters": (C.c_int, [vp, i32, vp, vp, i32, vp, vp, i32]),
+        "cs_set_data": (C.c_int, [vp, i32, vp, vp]),
+        "cs_set_batch": (C.c_int, [vp, i32, vp, vp]),
+        "cs_param_offsets": (C.c_int, [vp, vp]),
+        "cs_build_sed_tables": (C.c_int, [vp, vp, vp]),
+        "cs_spectral_like_grad": (C.c_int, [vp, vp, vp, vp]),
+        "cs_component_maps": (C.c_int, [vp, i32, vp, vp, vp]),
+        "cs_cmb_variance": (C.c_int, [vp, vp, vp]),
+        "cs_optimize": (C.c_int, [vp, vp, vp, vp, C.POINTER(CsOpt), vp, vp]),
+        "cs_opt_defaults": (None, [C.POINTER(CsOpt)]),
+        "cs_eval_host": (C.c_int, [vp, i32, vp, vp, vp, vp, vp]),
+        "cs_check": (C.c_int, [vp, vp]),
+        "cs_strerror": (C.c_char_p, [C.c_int]),
+        "cs_workspace_bytes": (i64, [vp]),
+        "cs_kernel_launches": (i64, [vp]),
+        "cs_version": (C.c_int, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = L
+    return L
+
+
+def strerror(code: int) -> str:
+    return lib().cs_strerror(int(code)).decode()
+
+
+def _chk(code, where):
+    if code != OK:
+        raise CsError(code, where)
+
+
+def _hp(a):
+    """Host pointer of a contiguous numpy array (or None)."""
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _ptr(t):
+    """Raw pointer of a torch tensor (device or host), a numpy array, an int, or None."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data_as(C.c_void_p)
+    if isinstance(t, int):
+        return C.c_void_p(t)
+    assert t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return C.c_void_p(stream)
+    return C.c_void_p(stream.cuda_stream)
+
+
+def opt_defaults(**kw) -> CsOpt:
+    o = CsOpt()
+    lib().cs_opt_defaults(C.byref(o))
+    for k, v in kw.items():
+        setattr(o, k, v)
+    return o
+
+
+class Context:
+    """Owns a cs_ctx*.  Methods mirror the C calls one to one (cs_<name> -> <name>)."""
+
+    def __init__(self, freqs_ghz, npix, nu0_dust=353.0, nu0_sync=23.0, t_cmb=2.7255, units=UNITS_KCMB):
+        self._freqs = np.ascontiguousarray(freqs_ghz, dtype=np.float64)
+        m = CsModel(len(self._freqs), self._freqs.ctypes.data_as(C.POINTER(C.c_double)), float(nu0_dust),
+                    float(nu0_sync), float(t_cmb), int(units), int(npix))
+        self._h = C.c_void_p()
+        self.nfreq, self.npix = len(self._freqs), int(npix)
+        self.batch = 0
+        self.nregion = 1
+        self._keep = {}
+        _chk(lib().cs_create(C.byref(self._h), C.byref(m)), "cs_create")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().cs_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_clusters(self, maps, Kmap, cfg_maps, region_idx=None, nregion=1):
+        """maps: int32 [nmap,npix] (torch device tensor or numpy); Kmap, cfg_maps: host arrays."""
+        Kmap = np.ascontiguousarray(Kmap, dtype=np.int32)
+        cfg_maps = np.ascontiguousarray(cfg_maps, dtype=np.int32).reshape(-1, 3)
+        nmap = int(Kmap.shape[0])
+        _chk(lib().cs_set_clusters(self._h, nmap, _ptr(maps), _hp(Kmap), int(cfg_maps.shape[0]), _hp(cfg_maps),
+                                   _ptr(region_idx), int(nregion)), "cs_set_clusters")
+        self.nregion = int(nregion)
+        self.batch = 0
+
+    def set_data(self, d, ninv):
+        """d: float32 device tensor [ndata,nfreq,2,npix] (borrowed: kept alive here); ninv: [nfreq] float32."""
+        ndata = int(d.shape[0])
+        if isinstance(ninv, np.ndarray):
+            ninv = np.ascontiguousarray(ninv, dtype=np.float32)
+        _chk(lib().cs_set_data(self._h, ndata, _ptr(d), _ptr(ninv)), "cs_set_data")
+        self._keep["d"] = d
+
+    def set_batch(self, cfg_of, data_of):
+        cfg_of = np.ascontiguousarray(cfg_of, dtype=np.int32)
+        data_of = np.ascontiguousarray(data_of, dtype=np.int32)
+        _chk(lib().cs_set_batch(self._h, int(cfg_of.shape[0]), _hp(cfg_of), _hp(data_of)), "cs_set_batch")
+        self.batch = int(cfg_of.shape[0])
+
+    def param_offsets(self):
+        off = np.empty(self.batch + 1, dtype=np.int64)
+        _chk(lib().cs_param_offsets(self._h, _hp(off)), "cs_param_offsets")
+        return off
+
+    def build_sed_tables(self, params, stream=None):
+        _chk(lib().cs_build_sed_tables(self._h, _ptr(params), _stream(stream)), "cs_build_sed_tables")
+
+    def spectral_like_grad(self, nll, grad=None, stream=None):
+        _chk(lib().cs_spectral_like_grad(self._h, _ptr(nll), _ptr(grad), _stream(stream)), "cs_spectral_like_grad")
+
+    def component_maps(self, s, entries=None, stream=None):
+        if entries is None:
+            nsel, ep = self.batch, None
+        else:
+            entries = np.ascontiguousarray(entries, dtype=np.int32)
+            nsel, ep = int(entries.shape[0]), _hp(entries)
+        _chk(lib().cs_component_maps(self._h, nsel, ep, _ptr(s), _stream(stream)), "cs_component_maps")
+
+    def cmb_variance(self, var, stream=None):
+        _chk(lib().cs_cmb_variance(self._h, _ptr(var), _stream(stream)), "cs_cmb_variance")
+
+    def optimize(self, params, lower, upper, opt=None, nll_final=None, stream=None):
+        opt = opt or opt_defaults()
+        _chk(lib().cs_optimize(self._h, _ptr(params), _ptr(lower), _ptr(upper), C.byref(opt), _ptr(nll_final),
+                               _stream(stream)), "cs_optimize")
+
+    def eval_host(self, d_host, ninv_host, params_host, nll_host, grad_host=None):
+        """Host buffers in, host buffers out (numpy arrays or pinned torch CPU tensors)."""
+        ndata = int(d_host.shape[0])
+        _chk(lib().cs_eval_host(self._h, ndata, _ptr(d_host), _ptr(ninv_host), _ptr(params_host), _ptr(nll_host),
+                                _ptr(grad_host)), "cs_eval_host")
+
+    def check(self, stream=None):
+        return lib().cs_check(self._h, _stream(stream))
+
+    def workspace_bytes(self):
+        return int(lib().cs_workspace_bytes(self._h))
+
+    def kernel_launches(self):
+        return int(lib().cs_kernel_launches(self._h))

@@ -1,0 +1,443 @@
+// cs_kernels.cuh -- the CUDA kernels of libcs (sm_100a).
+//
+//   k_tables   a1  SED factor tables, fp64 math -> fp32 rows                     (Eq. 2)
+//   k_like     a2  fused per-pixel gather / assemble A / 3x3 solve / likelihood and gradient terms, data streamed
+//                  through a cp.async.bulk (TMA) + mbarrier ring, followed in the same CTA by the first level of
+//              a3  the ordered fp64 segmented reduction (per-tile segments)        (Eq. 5, 6, 17)
+//              a4  (MODE_MAPS) GLS component maps                                 (Eq. 5 / 8)
+//   k_merge    a3  second level: fixed-order sum of per-tile partials onto clusters and regions
+//
+// One thread owns one pixel of a 256-pixel tile and walks over the entries of its group (same clustering
+// configuration, different data sets / parameters), so cluster ids, slot ids and the reduction plan are loaded
+// once per CTA.
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include "cs_internal.h"
+
+namespace cs {
+
+constexpr int MODE_VALUE = 0;   // ll only (line search)
+constexpr int MODE_GRAD = 1;    // ll + three gradient terms
+constexpr int MODE_MAPS = 2;    // component maps
+constexpr int MODE_CMBVAR = 3;  // sums for the CMB-variance metric (Eq. 10)
+
+constexpr int NST = 3;   // stages of the data ring
+constexpr int EC = 4;    // entries buffered between reduce phases
+
+struct LikeParams {
+    const float *d;
+    int64_t npix;
+    int32_t nfreq;
+    int32_t use_bulk;          // 1: rows are 16-byte aligned -> cp.async.bulk; 0: plain loads
+    const MapDev *maps;
+    const CfgDev *cfgs;
+    const Group *groups;
+    const int32_t *elist;
+    const int32_t *data_of;
+    const int64_t *tab_off;    // [batch] first table row of entry
+    const float *tab;
+    double *partial;
+    int64_t PS;                // doubles per partial row
+    float *maps_out;           // MODE_MAPS: [nsel,3,2,npix], slot = position in elist
+    int32_t *err;
+    KConst kc;
+};
+
+// ----------------------------------------------------------------------------------------------------------
+// mbarrier / bulk-copy helpers (PTX ISA: mbarrier, cp.async.bulk)
+// ----------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy completing on an mbarrier; dst/src/bytes 16-byte aligned; evict-first L2 policy.
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_normal() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+// ----------------------------------------------------------------------------------------------------------
+// a1: SED factor tables.  One thread per (entry, parameter, band).  fp64 -> fp32.
+// ----------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const int64_t *__restrict__ param_off,
+                                                const int64_t *__restrict__ tab_off, const int32_t *__restrict__ cfg_of,
+                                                const CfgDev *__restrict__ cfgs, float *__restrict__ tab, int32_t batch,
+                                                int32_t *err, const TConst tc) {
+    const int f = threadIdx.x;   // 0..15
+    for (int e = blockIdx.y; e < batch; e += gridDim.y) {
+        const CfgDev c = cfgs[cfg_of[e]];
+        const int j = blockIdx.x * blockDim.y + threadIdx.y;
+        if (j >= c.ktot) continue;
+        const double x = params[param_off[e] + j];
+        float *row0 = tab + (tab_off[e]) * NROW;
+        const bool live = f < tc.nfreq;
+        bool bad = !isfinite(x);
+        if (j < c.K[0]) {
+            // dust power-law factor with the band constant folded in: cd[f] * (nu_f/nu0d)^beta_d
+            float v = live ? (float)(tc.cd[f] * exp(x * tc.lnd[f])) : 0.f;
+            row0[(int64_t)j * NROW + f] = v;
+        } else if (j < c.K[0] + c.K[1]) {
+            // Planck ratio G = expm1(x0)/expm1(x) and d ln G / dT = (1/T) [ x/(1-e^-x) - x0/(1-e^-x0) ]
+            bad = bad || !(x > 0.0);
+            const int k = j - c.K[0];
+            float g = 0.f, dg = 0.f;
+            if (live) {
+                const double xf = tc.hk * tc.nu[f] / x, x0 = tc.hk * tc.nu0d / x;
+                g = (float)(expm1(x0) / expm1(xf));
+                dg = (float)((xf / (-expm1(-xf)) - x0 / (-expm1(-x0))) / x);
+            }
+            row0[(int64_t)(c.K[0] + k) * NROW + f] = g;
+            row0[(int64_t)(c.K[0] + c.K[1] + k) * NROW + f] = dg;
+        } else {
+            const int k = j - c.K[0] - c.K[1];
+            float v = live ? (float)(tc.cs[f] * exp(x * tc.lns[f])) : 0.f;
+            row0[(int64_t)(c.K[0] + 2 * c.K[1] + k) * NROW + f] = v;
+        }
+        if (bad && f == 0) atomicOr(err, ERR_DOMAIN);
+    }
+}
+
+// ----------------------------------------------------------------------------------------------------------
+// a2: per-pixel arithmetic.  NF = number of bands looped over (15 fast path, 16 generic with zero weights).
+// ----------------------------------------------------------------------------------------------------------
+template <int NF>
+struct PixelIn {
+    float dq[NF], du[NF];
+};
+
+__device__ __forceinline__ void load_row(const float *__restrict__ row, float (&out)[NROW]) {
+    const float4 *r4 = reinterpret_cast<const float4 *>(row);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float4 v = __ldg(r4 + i);
+        out[4 * i + 0] = v.x; out[4 * i + 1] = v.y; out[4 * i + 2] = v.z; out[4 * i + 3] = v.w;
+    }
+}
+
+// Forward part shared by all modes: builds a_d, a_s, M, b, solves; returns s (component amplitudes) and ll.
+template <int NF>
+__device__ __forceinline__ bool pixel_forward(const PixelIn<NF> &in, const float (&Fd)[NROW], const float (&G)[NROW],
+                                              const float (&Fs)[NROW], const KConst &kc, float (&ad)[NF],
+                                              float (&sq)[3], float (&su)[3], float &ll) {
+    float m01 = 0.f, m02 = 0.f, m11 = 0.f, m12 = 0.f, m22 = 0.f;
+    float bq0 = 0.f, bq1 = 0.f, bq2 = 0.f, bu0 = 0.f, bu1 = 0.f, bu2 = 0.f;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        const float a = Fd[f] * G[f];     // a_d = cd (nu/nu0)^beta_d * Planck ratio     (Eq. 2)
+        const float s = Fs[f];            // a_s = cs (nu/nu0)^beta_s
+        ad[f] = a;
+        const float wd = kc.w[f] * a, ws = kc.w[f] * s;
+        m01 += wd; m02 += ws;
+        m11 = fmaf(wd, a, m11); m12 = fmaf(wd, s, m12); m22 = fmaf(ws, s, m22);
+        bq0 = fmaf(kc.w[f], in.dq[f], bq0); bq1 = fmaf(wd, in.dq[f], bq1); bq2 = fmaf(ws, in.dq[f], bq2);
+        bu0 = fmaf(kc.w[f], in.du[f], bu0); bu1 = fmaf(wd, in.du[f], bu1); bu2 = fmaf(ws, in.du[f], bu2);
+    }
+    // LDL^T of the 3x3 SPD matrix M = A^T N^-1 A (m00 = sum w is a constant)
+    const float l10 = m01 * kc.inv_m00, l20 = m02 * kc.inv_m00;
+    const float d1 = fmaf(-l10, m01, m11);
+    const float t12 = fmaf(-l10, m02, m12);
+    const float id1 = __frcp_rn(d1);
+    const float l21 = t12 * id1;
+    const float d2 = fmaf(-l21, t12, fmaf(-l20, m02, m22));
+    const float id2 = __frcp_rn(d2);
+    const bool ok = (d1 > 0.f) && (d2 > 0.f);
+    {
+        const float y0 = bq0, y1 = fmaf(-l10, bq0, bq1);
+        const float y2 = fmaf(-l21, y1, fmaf(-l20, bq0, bq2));
+        const float z0 = y0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
+        sq[2] = z2; sq[1] = fmaf(-l21, z2, z1); sq[0] = fmaf(-l20, sq[2], fmaf(-l10, sq[1], z0));
+        ll = fmaf(y0, z0, fmaf(y1, z1, y2 * z2));
+    }
+    {
+        const float y0 = bu0, y1 = fmaf(-l10, bu0, bu1);
+        const float y2 = fmaf(-l21, y1, fmaf(-l20, bu0, bu2));
+        const float z0 = y0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
+        su[2] = z2; su[1] = fmaf(-l21, z2, z1); su[0] = fmaf(-l20, su[2], fmaf(-l10, su[1], z0));
+        ll += fmaf(y0, z0, fmaf(y1, z1, y2 * z2));
+    }
+    ll *= -0.5f;                          // -1/2 sum_S b_S . s_S                        (Eq. 6)
+    return ok;
+}
+
+// Gradient terms (Eq. 17 with s held fixed): g_theta = - sum_f w_f (da_f/dtheta) sum_S s_{S,c} r_{S,f}.
+template <int NF>
+__device__ __forceinline__ void pixel_grad(const PixelIn<NF> &in, const float (&ad)[NF], const float (&Fs)[NROW],
+                                           const float (&dG)[NROW], const KConst &kc, const float (&sq)[3],
+                                           const float (&su)[3], float &g_bd, float &g_td, float &g_bs) {
+    // q_f  = sum_S s_{S,dust} r_{S,f},  qs_f = sum_S s_{S,sync} r_{S,f},  r = d - A s, expanded so that the
+    // residual itself is never stored.
+    const float c0 = fmaf(sq[1], sq[0], su[1] * su[0]);
+    const float c1 = fmaf(sq[1], sq[1], su[1] * su[1]);
+    const float c2 = fmaf(sq[1], sq[2], su[1] * su[2]);
+    const float e0 = fmaf(sq[2], sq[0], su[2] * su[0]);
+    const float e2 = fmaf(sq[2], sq[2], su[2] * su[2]);
+    float g1 = 0.f, g2 = 0.f, g3 = 0.f;
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        const float a = ad[f], s = Fs[f];
+        float q = fmaf(sq[1], in.dq[f], -c0);
+        q = fmaf(su[1], in.du[f], q);
+        q = fmaf(-c1, a, q);
+        q = fmaf(-c2, s, q);
+        float qs = fmaf(sq[2], in.dq[f], -e0);
+        qs = fmaf(su[2], in.du[f], qs);
+        qs = fmaf(-c2, a, qs);
+        qs = fmaf(-e2, s, qs);
+        const float t = kc.w[f] * (a * q);
+        g1 = fmaf(kc.lnd[f], t, g1);          // d a_d / d beta_d = ln(nu/nu0d) a_d
+        g2 = fmaf(dG[f], t, g2);              // d a_d / d T_d    = (d ln G / dT) a_d
+        g3 = fmaf(kc.lnsw[f], s * qs, g3);    // d a_s / d beta_s = ln(nu/nu0s) a_s
+    }
+    g_bd = -g1; g_td = -g2; g_bs = -g3;
+}
+
+// ----------------------------------------------------------------------------------------------------------
+// a2 + first level of a3: the fused kernel.  grid = (ntile, ngroup), block = TP threads.
+// shared memory: data ring [NST][2*NF][TP] fp32 | terms [EC][4][TP] fp32 | members [4][TP] u8 | barriers | meta
+// ----------------------------------------------------------------------------------------------------------
+template <int NF>
+constexpr size_t like_smem_bytes() {
+    return (size_t)NST * 2 * NF * TP * 4 + (size_t)EC * 4 * TP * 4 + 4 * TP + NST * 8 + 64 * 4;
+}
+
+template <int NF, int MODE>
+__global__ void __launch_bounds__(TP, 2) k_like(const LikeParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float *sd = reinterpret_cast<float *>(smem_raw);
+    float *sterm = sd + NST * 2 * NF * TP;
+    uint8_t *smem_members = reinterpret_cast<uint8_t *>(sterm + EC * 4 * TP);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_members + 4 * TP);
+    int32_t *meta = reinterpret_cast<int32_t *>(full + NST);   // [0..3] nseg, [4..7] first seg, [8..11] segbase
+
+    const int tid = threadIdx.x;
+    const int tile = blockIdx.x;
+    const Group grp = P.groups[blockIdx.y];
+    const CfgDev cfg = P.cfgs[grp.cfg];
+    const int64_t p = (int64_t)tile * TP + tid;
+    const int64_t npix = P.npix;
+    const int nrows = 2 * P.nfreq;
+    const int nvalid = (int)min((int64_t)TP, npix - (int64_t)tile * TP);
+    constexpr bool kReduce = (MODE != MODE_MAPS);
+    // which map reduces which term: value -> region only; grad -> three cluster maps + region; cmbvar -> region x4
+    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;
+
+    int k0 = -1, k1 = -1, k2 = -1;
+    if (p < npix) {
+        k0 = P.maps[cfg.map[0]].idx[p];
+        k1 = P.maps[cfg.map[1]].idx[p];
+        k2 = P.maps[cfg.map[2]].idx[p];
+    }
+    const bool live = (k0 >= 0) && (k1 >= 0) && (k2 >= 0);
+
+    if (kReduce) {
+#pragma unroll
+        for (int t = T0; t < 4; ++t) {
+            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+            smem_members[t * TP + tid] = P.maps[mi].members[(int64_t)tile * TP + tid];
+        }
+        if (tid < 4) {
+            const int t = tid;
+            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+            const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
+            meta[t] = (t >= T0) ? (s1 - s0) : 0;
+            meta[4 + t] = s0;
+            meta[8 + t] = (MODE == MODE_CMBVAR) ? t * P.maps[mi].nseg : cfg.segbase[t];
+        }
+    }
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (NF > 15 && P.nfreq < NF) {
+        // generic path: rows beyond nfreq are never copied; they must read as zero
+        for (int s = 0; s < NST; ++s)
+            for (int r = nrows; r < 2 * NF; ++r) sd[(s * 2 * NF + r) * TP + tid] = 0.f;
+    }
+    __syncthreads();
+
+    const uint32_t row_bytes = (uint32_t)nvalid * 4u;
+    uint64_t policy = 0;
+    if (P.use_bulk) policy = policy_evict_first();
+
+    auto issue = [&](int i) {
+        // warp 0: lane 0 arms the barrier, then lanes 0..nrows-1 copy one band/Stokes row each
+        const int e = P.elist[grp.start + i];
+        const int64_t n = P.data_of[e];
+        const int s = i % NST;
+        const int lane = tid;
+        if (lane == 0) mbar_expect_tx(&full[s], row_bytes * (uint32_t)nrows);
+        __syncwarp();
+        for (int r = lane; r < nrows; r += 32) {
+            const float *src = P.d + ((n * nrows + r) * npix + (int64_t)tile * TP);
+            bulk_g2s(sd + (s * 2 * NF + r) * TP, src, row_bytes, &full[s], policy);
+        }
+    };
+
+    if (P.use_bulk && tid < 32) {
+        for (int i = 0; i < NST - 1 && i < grp.count; ++i) issue(i);
+    }
+
+    for (int i = 0; i < grp.count; ++i) {
+        const int s = i % NST;
+        const int e = P.elist[grp.start + i];
+        if (P.use_bulk) {
+            if (tid < 32 && i + NST - 1 < grp.count) issue(i + NST - 1);
+            mbar_wait(&full[s], (uint32_t)((i / NST) & 1));
+        } else {
+            const int64_t n = P.data_of[e];
+            for (int r = 0; r < nrows; ++r)
+                sd[(s * 2 * NF + r) * TP + tid] = (p < npix) ? P.d[(n * nrows + r) * npix + p] : 0.f;
+        }
+        PixelIn<NF> in;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            in.dq[f] = sd[(s * 2 * NF + 2 * f + 0) * TP + tid];
+            in.du[f] = sd[(s * 2 * NF + 2 * f + 1) * TP + tid];
+        }
+        __syncthreads();   // every thread holds its data in registers: stage s may be refilled
+
+        float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
+        if (live) {
+            const float *tb = P.tab + P.tab_off[e] * NROW;
+            float Fd[NROW], G[NROW], Fs[NROW];
+            load_row(tb + (int64_t)k0 * NROW, Fd);
+            load_row(tb + (int64_t)(cfg.K[0] + k1) * NROW, G);
+            load_row(tb + (int64_t)(cfg.K[0] + 2 * cfg.K[1] + k2) * NROW, Fs);
+            float ad[NF], sq[3], su[3], ll;
+            const bool ok = pixel_forward<NF>(in, Fd, G, Fs, P.kc, ad, sq, su, ll);
+            if (!ok) {
+                atomicOr(P.err, ERR_SINGULAR);
+                ll = CUDART_INF_F;
+            }
+            if (MODE == MODE_VALUE) {
+                t3 = ll;
+            } else if (MODE == MODE_GRAD) {
+                float dG[NROW];
+                load_row(tb + (int64_t)(cfg.K[0] + cfg.K[1] + k1) * NROW, dG);
+                pixel_grad<NF>(in, ad, Fs, dG, P.kc, sq, su, t0, t1, t2);
+                t3 = ll;
+            } else if (MODE == MODE_CMBVAR) {
+                t0 = sq[0]; t1 = su[0]; t2 = sq[0] * sq[0]; t3 = su[0] * su[0];
+            } else {
+                t0 = sq[0]; t1 = su[0]; t2 = sq[1]; t3 = su[1];
+                float *o = P.maps_out + (int64_t)(grp.start + i) * 6 * npix + p;
+                o[0] = sq[0]; o[npix] = su[0]; o[2 * npix] = sq[1]; o[3 * npix] = su[1];
+                o[4 * npix] = sq[2]; o[5 * npix] = su[2];
+            }
+        } else if (MODE == MODE_MAPS && p < npix) {
+            float *o = P.maps_out + (int64_t)(grp.start + i) * 6 * npix + p;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) o[c * npix] = 0.f;
+        }
+        if (kReduce) {
+            float *tm = sterm + (i % EC) * 4 * TP;
+            if (MODE != MODE_VALUE) { tm[0 * TP + tid] = t0; tm[1 * TP + tid] = t1; tm[2 * TP + tid] = t2; }
+            tm[3 * TP + tid] = t3;
+            if ((i % EC) == EC - 1 || i == grp.count - 1) {
+                __syncthreads();
+                // first level of the ordered reduction: one thread per (entry, term, segment); members of a
+                // segment are summed in ascending pixel order in fp64.
+                const int i0 = i - (i % EC), nent = (i % EC) + 1;
+                const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
+                const int c1 = n0, c2 = n0 + n1, c3 = n0 + n1 + n2, tot = c3 + n3;
+                for (int w = tid; w < nent * tot; w += TP) {
+                    const int ent = w / tot, r = w - ent * tot;
+                    const int t = (r >= c1) + (r >= c2) + (r >= c3);
+                    const int ls = r - (t == 0 ? 0 : (t == 1 ? c1 : (t == 2 ? c2 : c3)));
+                    const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+                    const int gseg = meta[4 + t] + ls;
+                    const uint32_t desc = P.maps[mi].segdesc[gseg];
+                    const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
+                    const uint8_t *mem = smem_members + t * TP + start;
+                    const float *term = sterm + (ent * 4 + t) * TP;
+                    double acc = 0.0;
+                    for (int j = 0; j < len; ++j) acc += (double)term[mem[j]];
+                    const int ee = P.elist[grp.start + i0 + ent];
+                    P.partial[(int64_t)ee * P.PS + meta[8 + t] + gseg] = acc;
+                }
+                __syncthreads();
+            }
+        }
+    }
+    (void)nvalid;
+}
+
+// ----------------------------------------------------------------------------------------------------------
+// a3 second level: grad[e][j] / nll[e][r] = fixed-order sum over the segments of cluster j / region r.
+// grid = (ceil(nout_max/256), batch).  want_grad = 0: only the region outputs.
+// ----------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
+                                               const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
+                                               const int64_t *__restrict__ param_off, int32_t nregion, int32_t want_grad,
+                                               double *__restrict__ nll, double *__restrict__ grad) {
+    const int e = blockIdx.y;
+    const CfgDev c = cfgs[cfg_of[e]];
+    const int nout = (want_grad ? c.ktot : 0) + nregion;
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= nout) return;
+    int t, k;
+    if (!want_grad) { t = 3; k = j; }
+    else if (j < c.K[0]) { t = 0; k = j; }
+    else if (j < c.K[0] + c.K[1]) { t = 1; k = j - c.K[0]; }
+    else if (j < c.ktot) { t = 2; k = j - c.K[0] - c.K[1]; }
+    else { t = 3; k = j - c.ktot; }
+    const MapDev m = maps[c.map[t]];
+    const double *row = partial + (int64_t)e * PS + c.segbase[t];
+    double acc = 0.0;
+    const int a = m.ksegptr[k], b = m.ksegptr[k + 1];
+    for (int q = a; q < b; ++q) acc += row[m.kseglist[q]];
+    if (t == 3) nll[(int64_t)e * nregion + k] = acc;
+    else grad[param_off[e] + j] = acc;
+}
+
+// f1 (Eq. 10): variance of the CMB map per entry and region from the four region-reduced sums.
+__global__ void __launch_bounds__(128) k_cmbvar(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
+                                                const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
+                                                const int32_t *__restrict__ npix_live, int32_t nregion, int32_t batch,
+                                                double *__restrict__ var) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= batch * nregion) return;
+    const int e = i / nregion, r = i - e * nregion;
+    const CfgDev c = cfgs[cfg_of[e]];
+    const MapDev m = maps[c.map[3]];
+    double s[4];
+    for (int t = 0; t < 4; ++t) {
+        const double *row = partial + (int64_t)e * PS + (int64_t)t * m.nseg;
+        double acc = 0.0;
+        for (int q = m.ksegptr[r]; q < m.ksegptr[r + 1]; ++q) acc += row[m.kseglist[q]];
+        s[t] = acc;
+    }
+    const double n = (double)npix_live[cfg_of[e] * nregion + r];
+    var[i] = n > 0 ? (s[2] / n - (s[0] / n) * (s[0] / n)) + (s[3] / n - (s[1] / n) * (s[1] / n)) : 0.0;
+}
+
+}  // namespace cs

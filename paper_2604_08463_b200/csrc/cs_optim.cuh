@@ -1,0 +1,272 @@
+// cs_optim.cuh -- a5: device-resident fixed-budget AdaTopK (App. A, Alg. 1; readings R13/R14 of
+// DESIGN.md).  Every batch entry is an independent bounded minimisation over its own parameter block.  All state
+// lives on the device in fp64; the host only enqueues kernels (no synchronisation, no data-dependent launches).
+//
+// One iteration (Alg. 1):
+//   y = (x - l)/(u - l), g_int = g * (u - l)                                   A1, L509-L513, Alg. 1 line 3
+//   release the single bound parameter pushed hardest into the feasible region  A2, L519-L525 with K = 0 (L249)
+//   g_proj = g_int * (p == 0)                                                    line 8
+//   if |g_proj| outside [safe_lo, safe_hi]: f = 1/|g_proj|; L,g_proj *= f; m *= f; v *= f^2     A4, L541-L546
+//   AdaBelief direction (Zhuang et al. 2020), masked by p == 0                   lines 14-16
+//   alpha_max = distance to the nearest bound along the direction                line 17
+//   backtracking line search on alpha in (0, min(1, alpha_max)]                  line 18, L263
+//   y += alpha d; pin the limiting parameter when alpha == alpha_max             lines 19-25
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cs {
+
+struct OptWork {
+    double *y = nullptr, *x = nullptr, *xt = nullptr, *dir = nullptr, *m = nullptr, *v = nullptr, *grad = nullptr;
+    const double *lo = nullptr, *hi = nullptr;
+    int8_t *pivot = nullptr;
+    double *nll_reg = nullptr, *nll_reg_t = nullptr;
+    double *L0 = nullptr, *gd = nullptr, *amax = nullptr, *alpha = nullptr, *alpha_acc = nullptr, *cscale = nullptr;
+    long long *ilim = nullptr;
+    int32_t *accepted = nullptr;
+};
+
+struct OptShape {
+    int64_t nparam;
+    int32_t batch, nregion, ktot_max;
+    const int64_t *param_off;
+};
+
+struct OptHyper {
+    double lr, beta1, beta2, eps, c1, safe_lo, safe_hi;
+    int32_t ls_max;
+};
+
+inline void opt_free(OptWork &w) {
+    cudaFree(w.y); cudaFree(w.x); cudaFree(w.xt); cudaFree(w.dir); cudaFree(w.m); cudaFree(w.v); cudaFree(w.grad);
+    cudaFree(w.pivot); cudaFree(w.nll_reg); cudaFree(w.nll_reg_t); cudaFree(w.L0); cudaFree(w.gd); cudaFree(w.amax);
+    cudaFree(w.alpha); cudaFree(w.alpha_acc); cudaFree(w.cscale); cudaFree(w.ilim); cudaFree(w.accepted);
+    w = OptWork();
+}
+
+// returns 0 ok, 1 out of memory
+inline int opt_alloc(OptWork &w, int64_t nparam, int32_t batch, int32_t nregion, int64_t *bytes) {
+    const size_t np = (size_t)(nparam > 0 ? nparam : 1) * sizeof(double), nb = (size_t)batch * sizeof(double);
+    bool ok = true;
+    ok &= cudaMalloc((void **)&w.y, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.x, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.xt, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.dir, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.m, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.v, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.grad, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.pivot, (size_t)(nparam > 0 ? nparam : 1)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.nll_reg, nb * nregion) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.nll_reg_t, nb * nregion) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.L0, nb) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.gd, nb) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.amax, nb) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.alpha, nb) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.alpha_acc, nb) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.cscale, nb) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.ilim, (size_t)batch * sizeof(long long)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.accepted, (size_t)batch * sizeof(int32_t)) == cudaSuccess;
+    if (!ok) { opt_free(w); return 1; }
+    *bytes = (int64_t)(7 * np + nparam + 2 * nb * nregion + 7 * nb + (size_t)batch * 4);
+    return 0;
+}
+
+constexpr int OPT_THREADS = 256;
+
+// block-wide reductions over OPT_THREADS threads, deterministic (fixed tree)
+__device__ __forceinline__ double block_sum(double v, double *sh) {
+    const int tid = threadIdx.x;
+    sh[tid] = v;
+    __syncthreads();
+    for (int s = OPT_THREADS / 2; s > 0; s >>= 1) {
+        if (tid < s) sh[tid] += sh[tid + s];
+        __syncthreads();
+    }
+    const double r = sh[0];
+    __syncthreads();
+    return r;
+}
+// max with lowest-index tie break (want_min: min with lowest index)
+__device__ __forceinline__ void block_argbest(double &val, long long &idx, bool want_min, double *shv, long long *shi) {
+    const int tid = threadIdx.x;
+    shv[tid] = val; shi[tid] = idx;
+    __syncthreads();
+    for (int s = OPT_THREADS / 2; s > 0; s >>= 1) {
+        if (tid < s) {
+            const double a = shv[tid], b = shv[tid + s];
+            const long long ia = shi[tid], ib = shi[tid + s];
+            const bool take_b = (ib >= 0) && (ia < 0 || (want_min ? (b < a) : (b > a)) || (b == a && ib < ia));
+            if (take_b) { shv[tid] = b; shi[tid] = ib; }
+        }
+        __syncthreads();
+    }
+    val = shv[0]; idx = shi[0];
+    __syncthreads();
+}
+
+// A1 (L509-L513): map the start into [0,1], set the pivots, clear the AdaBelief moments.
+__global__ void k_opt_init(OptWork w, int64_t nparam, const double *params, int32_t batch) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < batch) w.cscale[i] = 1.0;
+    if (i >= nparam) return;
+    const double l = w.lo[i], u = w.hi[i];
+    double y = (params[i] - l) / (u - l);
+    y = fmin(fmax(y, 0.0), 1.0);
+    w.y[i] = y;
+    w.pivot[i] = y <= 0.0 ? -1 : (y >= 1.0 ? 1 : 0);
+    w.m[i] = 0.0; w.v[i] = 0.0; w.dir[i] = 0.0;
+    w.x[i] = l + y * (u - l);
+}
+
+// Alg. 1 lines 3-17 for one entry per CTA.
+__global__ void __launch_bounds__(OPT_THREADS) k_opt_direction(OptWork w, OptShape sh, OptHyper hy, int32_t iter) {
+    __shared__ double shv[OPT_THREADS];
+    __shared__ long long shi[OPT_THREADS];
+    const int e = blockIdx.x, tid = threadIdx.x;
+    const int64_t o0 = sh.param_off[e], o1 = sh.param_off[e + 1];
+    double cscale = w.cscale[e];
+    double L = 0.0;
+    for (int r = 0; r < sh.nregion; ++r) L += w.nll_reg[(int64_t)e * sh.nregion + r];
+    L *= cscale;
+    // release (A2, K = 0): the bound parameter whose descent direction -g points furthest into the interior
+    double best = 0.0;
+    long long bi = -1;
+    for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) {
+        const int8_t p = w.pivot[i];
+        if (p != 0) {
+            const double gint = cscale * w.grad[i] * (w.hi[i] - w.lo[i]);
+            const double score = (p < 0) ? -gint : gint;
+            if (score > 0.0 && (bi < 0 || score > best)) { best = score; bi = i; }
+        }
+    }
+    block_argbest(best, bi, false, shv, shi);
+    if (tid == 0 && bi >= 0) w.pivot[bi] = 0;
+    __syncthreads();
+    // projected gradient norm and dynamic rescale (A4)
+    double n2 = 0.0;
+    for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS)
+        if (w.pivot[i] == 0) {
+            const double gint = cscale * w.grad[i] * (w.hi[i] - w.lo[i]);
+            n2 += gint * gint;
+        }
+    n2 = block_sum(n2, shv);
+    const double nrm = sqrt(n2);
+    double f = 1.0;
+    if (nrm > 0.0 && (nrm < hy.safe_lo || nrm > hy.safe_hi)) f = 1.0 / nrm;
+    cscale *= f;
+    L *= f;
+    // AdaBelief direction, masked; directional derivative; distance to the nearest bound
+    const double t = (double)(iter + 1);
+    const double bc1 = 1.0 - pow(hy.beta1, t), bc2 = 1.0 - pow(hy.beta2, t);
+    double gd = 0.0, amax = CUDART_INF;
+    long long il = -1;
+    for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) {
+        const bool free_i = w.pivot[i] == 0;
+        const double g = free_i ? cscale * w.grad[i] * (w.hi[i] - w.lo[i]) : 0.0;
+        double m = w.m[i] * f, v = w.v[i] * f * f;
+        m = hy.beta1 * m + (1.0 - hy.beta1) * g;
+        const double dgm = g - m;
+        v = hy.beta2 * v + (1.0 - hy.beta2) * dgm * dgm + hy.eps;
+        w.m[i] = m; w.v[i] = v;
+        double d = free_i ? -hy.lr * (m / bc1) / (sqrt(v / bc2) + hy.eps) : 0.0;
+        w.dir[i] = d;
+        gd += g * d;
+        if (d != 0.0) {
+            const double y = w.y[i];
+            const double a = d > 0.0 ? (1.0 - y) / d : y / (-d);
+            if (il < 0 || a < amax) { amax = a; il = i; }
+        }
+    }
+    gd = block_sum(gd, shv);
+    block_argbest(amax, il, true, shv, shi);
+    if (tid == 0) {
+        w.cscale[e] = cscale;
+        w.L0[e] = L;
+        w.gd[e] = gd;
+        w.amax[e] = (il >= 0) ? amax : CUDART_INF;
+        w.ilim[e] = il;
+        w.alpha[e] = (il >= 0) ? fmin(1.0, amax) : 1.0;
+        w.alpha_acc[e] = 0.0;
+        w.accepted[e] = 0;
+    }
+}
+
+// trial point x_t = l + clamp(y + alpha d)(u - l); grid = (ceil(ktot_max/256), batch)
+__global__ void k_opt_trial(OptWork w, OptShape sh) {
+    const int e = blockIdx.y;
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= sh.param_off[e + 1]) return;
+    const double a = w.accepted[e] ? w.alpha_acc[e] : w.alpha[e];
+    const double y = fmin(fmax(w.y[i] + a * w.dir[i], 0.0), 1.0);
+    w.xt[i] = w.lo[i] + y * (w.hi[i] - w.lo[i]);
+}
+
+// Armijo test per entry (L263: every accepted step decreases the objective)
+__global__ void k_opt_ls(OptWork w, OptShape sh, OptHyper hy) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= sh.batch || w.accepted[e]) return;
+    double Lt = 0.0;
+    for (int r = 0; r < sh.nregion; ++r) Lt += w.nll_reg_t[(int64_t)e * sh.nregion + r];
+    Lt *= w.cscale[e];
+    const double a = w.alpha[e];
+    if (Lt <= w.L0[e] + hy.c1 * a * w.gd[e]) {   // false for NaN / +inf
+        w.accepted[e] = 1;
+        w.alpha_acc[e] = a;
+    } else {
+        w.alpha[e] = 0.5 * a;
+    }
+}
+
+// lines 19-25: move, pin the limiting parameter if the step reached alpha_max
+__global__ void k_opt_commit(OptWork w, OptShape sh) {
+    const int e = blockIdx.y;
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= sh.param_off[e + 1]) return;
+    const double a = w.accepted[e] ? w.alpha_acc[e] : 0.0;
+    double y = fmin(fmax(w.y[i] + a * w.dir[i], 0.0), 1.0);
+    if (a > 0.0 && a == w.amax[e] && i == w.ilim[e]) {
+        y = w.dir[i] > 0.0 ? 1.0 : 0.0;
+        w.pivot[i] = w.dir[i] > 0.0 ? 1 : -1;
+    } else if (w.pivot[i] == 0 && a > 0.0 && (y <= 0.0 || y >= 1.0)) {
+        w.pivot[i] = y <= 0.0 ? -1 : 1;
+    }
+    w.y[i] = y;
+    w.x[i] = w.lo[i] + y * (w.hi[i] - w.lo[i]);
+}
+
+__global__ void k_opt_finish(OptWork w, OptShape sh, double *params, double *nll_final) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < sh.nparam) params[i] = w.x[i];
+    if (nll_final && i < sh.batch) {
+        double L = 0.0;
+        for (int r = 0; r < sh.nregion; ++r) L += w.nll_reg[i * sh.nregion + r];
+        nll_final[i] = L;
+    }
+}
+
+inline void opt_init(OptWork &w, const OptShape &sh, const double *params, const double *lo, const double *hi, cudaStream_t st) {
+    w.lo = lo; w.hi = hi;
+    const int64_t n = sh.nparam > sh.batch ? sh.nparam : sh.batch;
+    k_opt_init<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w, sh.nparam, params, sh.batch);
+}
+inline void opt_direction(OptWork &w, const OptShape &sh, const OptHyper &hy, int iter, cudaStream_t st) {
+    k_opt_direction<<<sh.batch, OPT_THREADS, 0, st>>>(w, sh, hy, iter);
+}
+inline void opt_trial_point(OptWork &w, const OptShape &sh, cudaStream_t st) {
+    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    k_opt_trial<<<grid, 256, 0, st>>>(w, sh);
+}
+inline void opt_ls_update(OptWork &w, const OptShape &sh, const OptHyper &hy, cudaStream_t st) {
+    k_opt_ls<<<(sh.batch + 127) / 128, 128, 0, st>>>(w, sh, hy);
+}
+inline void opt_commit(OptWork &w, const OptShape &sh, cudaStream_t st) {
+    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    k_opt_commit<<<grid, 256, 0, st>>>(w, sh);
+}
+inline void opt_finish(OptWork &w, const OptShape &sh, double *params, double *nll_final, cudaStream_t st) {
+    const int64_t n = sh.nparam > sh.batch ? sh.nparam : sh.batch;
+    k_opt_finish<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w, sh, params, nll_final);
+}
+
+}  // namespace cs
