@@ -139,6 +139,12 @@ CS_API int cs_eval_host(cs_ctx *ctx, int32_t ndata, const float *d_host, const f
 CS_API int cs_check(cs_ctx *ctx, void *stream);
 CS_API const char *cs_strerror(int code);
 
+/* Optional device timing of the fused kernel: when enabled, every gradient-mode launch of the fused per-pixel kernel
+ * is bracketed by CUDA events on its own stream (ring of 512 launches).  cs_profile_read synchronises the device and
+ * returns the summed duration [ms] and the number of launches measured since cs_profile(ctx, 1). */
+CS_API int cs_profile(cs_ctx *ctx, int enable);
+CS_API int cs_profile_read(cs_ctx *ctx, double *total_ms, int64_t *count);
+
 /* Introspection used by the bench and the tests. */
 CS_API int64_t cs_workspace_bytes(cs_ctx *ctx);      /* device bytes currently held by the context */
 CS_API int64_t cs_kernel_launches(cs_ctx *ctx);      /* kernels launched by this context so far */

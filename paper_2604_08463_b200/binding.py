@@ -14,7 +14,7 @@ UNITS_KCMB, UNITS_LITERAL = 0, 1
 
 EXPORTS = ["cs_create", "cs_destroy", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
            "cs_build_sed_tables", "cs_spectral_like_grad", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
-           "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
+           "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
 
 
@@ -67,6 +67,8 @@ def lib():
         "cs_opt_defaults": (None, [C.POINTER(CsOpt)]),
         "cs_eval_host": (C.c_int, [vp, i32, vp, vp, vp, vp, vp]),
         "cs_check": (C.c_int, [vp, vp]),
+        "cs_profile": (C.c_int, [vp, C.c_int]),
+        "cs_profile_read": (C.c_int, [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
         "cs_strerror": (C.c_char_p, [C.c_int]),
         "cs_workspace_bytes": (i64, [vp]),
         "cs_kernel_launches": (i64, [vp]),
@@ -208,6 +210,15 @@ class Context:
 
     def check(self, stream=None):
         return lib().cs_check(self._h, _stream(stream))
+
+    def profile(self, enable=True):
+        _chk(lib().cs_profile(self._h, 1 if enable else 0), "cs_profile")
+
+    def profile_read(self):
+        """(total ms, launches) of the fused gradient kernel since profile(True)."""
+        ms, n = C.c_double(), C.c_int64()
+        _chk(lib().cs_profile_read(self._h, C.byref(ms), C.byref(n)), "cs_profile_read")
+        return ms.value, n.value
 
     def workspace_bytes(self):
         return int(lib().cs_workspace_bytes(self._h))

@@ -87,6 +87,11 @@ struct cs_ctx {
     double *d_hparams = nullptr, *d_hnll = nullptr, *d_hgrad = nullptr;
     int64_t hbuf_bytes = 0;
     cudaStream_t copy_stream = nullptr, comp_stream = nullptr;
+    // optional timing of the fused kernel (cs_profile): ring of event pairs recorded around every k_like launch
+    static constexpr int PROF_RING = 512;
+    bool prof_on = false;
+    std::vector<cudaEvent_t> prof_ev;   // 2*PROF_RING
+    int64_t prof_n = 0;
     // misc
     int32_t *d_err = nullptr;
     int64_t launches = 0;
@@ -196,7 +201,10 @@ int launch_like_t(cs_ctx *c, const LikeParams &P, int ngroup, cudaStream_t st) {
         LikeParams Q = P;
         Q.groups = P.groups + g0;
         dim3 grid(c->ntile, std::min(65535, ngroup - g0));
+        const bool prof = c->prof_on && MODE == MODE_GRAD;
+        if (prof) cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING)], st);
         k_like<NF, MODE><<<grid, TP, smem, st>>>(Q);
+        if (prof) { cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING) + 1], st); c->prof_n++; }
         c->launches++;
     }
     CK(cudaGetLastError());
@@ -303,6 +311,7 @@ int cs_destroy(cs_ctx *c) {
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->comp_stream) cudaStreamDestroy(c->comp_stream);
     cudaFree(c->d_err);
+    for (auto &e : c->prof_ev) cudaEventDestroy(e);
     delete c;
     return CS_OK;
 }
@@ -663,6 +672,31 @@ int cs_check(cs_ctx *c, void *stream) {
     CK(cudaMemset(c->d_err, 0, sizeof(e)));
     if (e & ERR_DOMAIN) return CS_EDOMAIN;
     if (e & ERR_SINGULAR) return CS_ESINGULAR;
+    return CS_OK;
+}
+
+int cs_profile(cs_ctx *c, int enable) {
+    if (!c) return CS_EINVAL;
+    if (enable && c->prof_ev.empty()) {
+        c->prof_ev.resize(2 * cs_ctx::PROF_RING);
+        for (auto &e : c->prof_ev) CK(cudaEventCreate(&e));
+    }
+    c->prof_on = enable != 0;
+    c->prof_n = 0;
+    return CS_OK;
+}
+
+int cs_profile_read(cs_ctx *c, double *total_ms, int64_t *count) {
+    if (!c || !total_ms || !count) return CS_EINVAL;
+    CK(cudaDeviceSynchronize());
+    const int64_t n = std::min<int64_t>(c->prof_n, cs_ctx::PROF_RING);
+    double tot = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+        tot += ms;
+    }
+    *total_ms = tot; *count = n;
     return CS_OK;
 }
 
