@@ -8,7 +8,7 @@
 //              rows [K0+K1,K0+2K1)    dlnG[k][f] = d ln G / d T_d
 //              rows [K0+2K1, ..+K2)   Fs'[k][f] = cs[f] * (nu_f/nu0s)^beta_s[k]
 //   partial  [batch][PS] fp64   per-tile, per-segment ordered partial sums (written by k_like, read by k_merge)
-//   plan     per cluster map: idx int32[npix], members u8[ntile*TP], segptr int32[ntile+1], segdesc u16[nseg],
+//   plan     per cluster map: idx int32[npix], rank u8[ntile*TP], segptr int32[ntile+1], segdesc u16[nseg],
 //            ksegptr int32[K+1], kseglist int32[nseg]
 #pragma once
 #include <stdint.h>
@@ -26,7 +26,7 @@ constexpr int ERR_SINGULAR = 2;
 // One cluster map (or the region pseudo-map) as the kernels see it.
 struct MapDev {
     const int32_t *idx;       // [npix] cluster id, -1 = masked
-    const uint8_t *members;   // [ntile*TP] per tile: in-tile pixel ids sorted by (cluster id, pixel)
+    const uint8_t *rank;      // [ntile*TP] position of the pixel in its tile's (cluster id, pixel) order
     const int32_t *segptr;    // [ntile+1] first segment of each tile (map-local numbering)
     const uint16_t *segdesc;  // [nseg] start (8 bits) | (len-1) << 8
     const int32_t *ksegptr;   // [K+1] CSR cluster -> segments

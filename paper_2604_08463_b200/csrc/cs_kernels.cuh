@@ -11,6 +11,7 @@
 // configuration, different data sets / parameters), so cluster ids, slot ids and the reduction plan are loaded
 // once per CTA.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include "cs_internal.h"
@@ -22,14 +23,15 @@ constexpr int MODE_GRAD = 1;    // ll + three gradient terms
 constexpr int MODE_MAPS = 2;    // component maps
 constexpr int MODE_CMBVAR = 3;  // sums for the CMB-variance metric (Eq. 10)
 
-constexpr int NST = 3;   // stages of the data ring
+constexpr int NST = 2;   // stages of each warp's data ring (both in flight while the warp computes)
 constexpr int EC = 4;    // entries buffered between reduce phases
 
 struct LikeParams {
     const float *d;
     int64_t npix;
     int32_t nfreq;
-    int32_t use_bulk;          // 1: rows are 16-byte aligned -> cp.async.bulk; 0: plain loads
+    int32_t use_bulk;          // 1: d is TMA-addressable (16-byte aligned rows) -> tensor-map loads; 0: plain loads
+    int32_t evict_first;       // 1: d is much larger than L2 and streamed once -> L2 evict-first policy
     const MapDev *maps;
     const CfgDev *cfgs;
     const Group *groups;
@@ -220,110 +222,125 @@ __device__ __forceinline__ void pixel_grad(const PixelIn<NF> &in, const float (&
 }
 
 // ----------------------------------------------------------------------------------------------------------
-// a2 + first level of a3: the fused kernel.  grid = (ntile, ngroup), block = TP threads.
-// shared memory: data ring [NST][2*NF][TP] fp32 | terms [EC][4][TP] fp32 | members [4][TP] u8 | barriers | meta
+// a2 + first level of a3: the fused kernel.  grid = (ntile, ngroup), block = TP threads = 8 warps.
+//
+// Data path: every warp owns the 32 pixels [tile*256 + 32*warp, +32) and streams its own [2*nfreq x 32] box of d
+// per entry through a private NST-stage ring filled by TMA (cp.async.bulk.tensor.2d, one instruction per warp and
+// entry, completion on the warp's own mbarrier).  Warps never synchronise with each other on the data path.
+// Reduction: each thread stores its four terms at the rank its pixel has in the tile's (cluster, pixel) order, so
+// that every segment is a contiguous run in shared memory; every EC entries the CTA sums the segments (one thread
+// per (entry, term, segment), ascending pixel order, fp64) into the partial buffer.  The term buffer is double
+// buffered: one __syncthreads per EC entries.
+// shared memory: ring [8 warps][NST][2*NF][32] fp32 | terms [2][EC][4][TP] fp32 | barriers [8][NST] | meta
 // ----------------------------------------------------------------------------------------------------------
+constexpr int NWARP = TP / 32;
+
 template <int NF>
 constexpr size_t like_smem_bytes() {
-    return (size_t)NST * 2 * NF * TP * 4 + (size_t)EC * 4 * TP * 4 + 4 * TP + NST * 8 + 64 * 4;
+    return (size_t)NWARP * NST * 2 * NF * 32 * 4 + (size_t)2 * EC * 4 * TP * 4 + NWARP * NST * 8 + 64 * 4;
+}
+
+__device__ __forceinline__ void tma_box_g2s(void *dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
 }
 
 template <int NF, int MODE>
-__global__ void __launch_bounds__(TP, 2) k_like(const LikeParams P) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    float *sd = reinterpret_cast<float *>(smem_raw);
-    float *sterm = sd + NST * 2 * NF * TP;
-    uint8_t *smem_members = reinterpret_cast<uint8_t *>(sterm + EC * 4 * TP);
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_members + 4 * TP);
-    int32_t *meta = reinterpret_cast<int32_t *>(full + NST);   // [0..3] nseg, [4..7] first seg, [8..11] segbase
+__global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensorMap tmap, const LikeParams P) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    float *ring = reinterpret_cast<float *>(smem_raw);
+    float *sterm = ring + NWARP * NST * 2 * NF * 32;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sterm + 2 * EC * 4 * TP);
+    int32_t *meta = reinterpret_cast<int32_t *>(bars + NWARP * NST);   // [0..3] nseg, [4..7] first seg, [8..11] segbase
 
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int tile = blockIdx.x;
     const Group grp = P.groups[blockIdx.y];
     const CfgDev cfg = P.cfgs[grp.cfg];
-    const int64_t p = (int64_t)tile * TP + tid;
     const int64_t npix = P.npix;
+    const int64_t p = (int64_t)tile * TP + tid;
     const int nrows = 2 * P.nfreq;
-    const int nvalid = (int)min((int64_t)TP, npix - (int64_t)tile * TP);
     constexpr bool kReduce = (MODE != MODE_MAPS);
-    // which map reduces which term: value -> region only; grad -> three cluster maps + region; cmbvar -> region x4
-    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;
+    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;   // value-only: only the ll / region term is reduced
 
     int k0 = -1, k1 = -1, k2 = -1;
+    uint32_t rank4 = 0;   // rank of this pixel in the tile order of the four reducing maps, 8 bits each
     if (p < npix) {
         k0 = P.maps[cfg.map[0]].idx[p];
         k1 = P.maps[cfg.map[1]].idx[p];
         k2 = P.maps[cfg.map[2]].idx[p];
+        if (kReduce) {
+#pragma unroll
+            for (int t = T0; t < 4; ++t) {
+                const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+                rank4 |= (uint32_t)P.maps[mi].rank[p] << (8 * t);
+            }
+        }
     }
     const bool live = (k0 >= 0) && (k1 >= 0) && (k2 >= 0);
-
-    if (kReduce) {
-#pragma unroll
-        for (int t = T0; t < 4; ++t) {
-            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
-            smem_members[t * TP + tid] = P.maps[mi].members[(int64_t)tile * TP + tid];
-        }
-        if (tid < 4) {
-            const int t = tid;
-            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
-            const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
-            meta[t] = (t >= T0) ? (s1 - s0) : 0;
-            meta[4 + t] = s0;
-            meta[8 + t] = (MODE == MODE_CMBVAR) ? t * P.maps[mi].nseg : cfg.segbase[t];
-        }
+    if (kReduce && tid < 4) {
+        const int t = tid;
+        const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+        const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
+        meta[t] = (t >= T0) ? (s1 - s0) : 0;
+        meta[4 + t] = s0;
+        meta[8 + t] = (MODE == MODE_CMBVAR) ? t * P.maps[mi].nseg : cfg.segbase[t];
     }
-    if (tid == 0) {
+    float *wring = ring + warp * NST * 2 * NF * 32;
+    uint64_t *wbar = bars + warp * NST;
+    if (lane == 0) {
 #pragma unroll
-        for (int s = 0; s < NST; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < NST; ++s) mbar_init(&wbar[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (NF > 15 && P.nfreq < NF) {
         // generic path: rows beyond nfreq are never copied; they must read as zero
         for (int s = 0; s < NST; ++s)
-            for (int r = nrows; r < 2 * NF; ++r) sd[(s * 2 * NF + r) * TP + tid] = 0.f;
+            for (int r = nrows; r < 2 * NF; ++r) wring[(s * 2 * NF + r) * 32 + lane] = 0.f;
     }
     __syncthreads();
 
-    const uint32_t row_bytes = (uint32_t)nvalid * 4u;
+    const int px0 = tile * TP + warp * 32;   // first pixel of this warp
+    const bool warp_has_pixels = (int64_t)px0 < npix;
+    const uint32_t box_bytes = (uint32_t)nrows * 32u * 4u;
     uint64_t policy = 0;
-    if (P.use_bulk) policy = policy_evict_first();
+    if (P.use_bulk) policy = P.evict_first ? policy_evict_first() : policy_evict_normal();
 
-    auto issue = [&](int i) {
-        // warp 0: lane 0 arms the barrier, then lanes 0..nrows-1 copy one band/Stokes row each
+    auto issue = [&](int i) {   // lane 0 only
         const int e = P.elist[grp.start + i];
-        const int64_t n = P.data_of[e];
+        const int n = P.data_of[e];
         const int s = i % NST;
-        const int lane = tid;
-        if (lane == 0) mbar_expect_tx(&full[s], row_bytes * (uint32_t)nrows);
-        __syncwarp();
-        for (int r = lane; r < nrows; r += 32) {
-            const float *src = P.d + ((n * nrows + r) * npix + (int64_t)tile * TP);
-            bulk_g2s(sd + (s * 2 * NF + r) * TP, src, row_bytes, &full[s], policy);
-        }
+        mbar_expect_tx(&wbar[s], box_bytes);
+        tma_box_g2s(wring + s * 2 * NF * 32, &tmap, px0, n * nrows, &wbar[s], policy);
     };
-
-    if (P.use_bulk && tid < 32) {
-        for (int i = 0; i < NST - 1 && i < grp.count; ++i) issue(i);
-    }
+    if (P.use_bulk && warp_has_pixels && lane == 0)
+        for (int i = 0; i < NST && i < grp.count; ++i) issue(i);
 
     for (int i = 0; i < grp.count; ++i) {
         const int s = i % NST;
         const int e = P.elist[grp.start + i];
-        if (P.use_bulk) {
-            if (tid < 32 && i + NST - 1 < grp.count) issue(i + NST - 1);
-            mbar_wait(&full[s], (uint32_t)((i / NST) & 1));
-        } else {
-            const int64_t n = P.data_of[e];
-            for (int r = 0; r < nrows; ++r)
-                sd[(s * 2 * NF + r) * TP + tid] = (p < npix) ? P.d[(n * nrows + r) * npix + p] : 0.f;
-        }
         PixelIn<NF> in;
+        if (warp_has_pixels) {
+            const float *st = wring + s * 2 * NF * 32;
+            if (P.use_bulk) {
+                mbar_wait(&wbar[s], (uint32_t)((i / NST) & 1));
+            } else {
+                const int64_t n = P.data_of[e];
+                for (int r = 0; r < nrows; ++r)
+                    wring[(s * 2 * NF + r) * 32 + lane] = (p < npix) ? P.d[(n * nrows + r) * npix + p] : 0.f;
+                __syncwarp();
+            }
 #pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            in.dq[f] = sd[(s * 2 * NF + 2 * f + 0) * TP + tid];
-            in.du[f] = sd[(s * 2 * NF + 2 * f + 1) * TP + tid];
+            for (int f = 0; f < NF; ++f) {
+                in.dq[f] = st[(2 * f + 0) * 32 + lane];
+                in.du[f] = st[(2 * f + 1) * 32 + lane];
+            }
+            __syncwarp();   // the whole warp holds its data in registers: the stage may be refilled
+            if (P.use_bulk && lane == 0 && i + NST < grp.count) issue(i + NST);
         }
-        __syncthreads();   // every thread holds its data in registers: stage s may be refilled
 
         float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
         if (live) {
@@ -348,7 +365,6 @@ __global__ void __launch_bounds__(TP, 2) k_like(const LikeParams P) {
             } else if (MODE == MODE_CMBVAR) {
                 t0 = sq[0]; t1 = su[0]; t2 = sq[0] * sq[0]; t3 = su[0] * su[0];
             } else {
-                t0 = sq[0]; t1 = su[0]; t2 = sq[1]; t3 = su[1];
                 float *o = P.maps_out + (int64_t)(grp.start + i) * 6 * npix + p;
                 o[0] = sq[0]; o[npix] = su[0]; o[2 * npix] = sq[1]; o[3 * npix] = su[1];
                 o[4 * npix] = sq[2]; o[5 * npix] = su[2];
@@ -359,14 +375,23 @@ __global__ void __launch_bounds__(TP, 2) k_like(const LikeParams P) {
             for (int c = 0; c < 6; ++c) o[c * npix] = 0.f;
         }
         if (kReduce) {
-            float *tm = sterm + (i % EC) * 4 * TP;
-            if (MODE != MODE_VALUE) { tm[0 * TP + tid] = t0; tm[1 * TP + tid] = t1; tm[2 * TP + tid] = t2; }
-            tm[3 * TP + tid] = t3;
+            // terms at the pixel's rank in each reducing map's (cluster, pixel) order; pixels without a cluster in
+            // map t have no rank there (and are not live), live == false elsewhere contributes an explicit zero
+            float *tm = sterm + (((i / EC) & 1) * EC + (i % EC)) * 4 * TP;
+            if (p < npix) {
+                if (MODE != MODE_VALUE) {
+                    if (k0 >= 0 || MODE == MODE_CMBVAR) tm[0 * TP + (rank4 & 0xff)] = t0;
+                    if (k1 >= 0 || MODE == MODE_CMBVAR) tm[1 * TP + ((rank4 >> 8) & 0xff)] = t1;
+                    if (k2 >= 0 || MODE == MODE_CMBVAR) tm[2 * TP + ((rank4 >> 16) & 0xff)] = t2;
+                }
+                tm[3 * TP + (rank4 >> 24)] = t3;
+            }
             if ((i % EC) == EC - 1 || i == grp.count - 1) {
                 __syncthreads();
-                // first level of the ordered reduction: one thread per (entry, term, segment); members of a
-                // segment are summed in ascending pixel order in fp64.
+                // first level of the ordered reduction: one thread per (entry, term, segment); a segment is a
+                // contiguous run of the rank-ordered terms, summed in ascending pixel order in fp64.
                 const int i0 = i - (i % EC), nent = (i % EC) + 1;
+                const float *tbuf = sterm + ((i / EC) & 1) * EC * 4 * TP;
                 const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
                 const int c1 = n0, c2 = n0 + n1, c3 = n0 + n1 + n2, tot = c3 + n3;
                 for (int w = tid; w < nent * tot; w += TP) {
@@ -377,18 +402,16 @@ __global__ void __launch_bounds__(TP, 2) k_like(const LikeParams P) {
                     const int gseg = meta[4 + t] + ls;
                     const uint32_t desc = P.maps[mi].segdesc[gseg];
                     const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
-                    const uint8_t *mem = smem_members + t * TP + start;
-                    const float *term = sterm + (ent * 4 + t) * TP;
+                    const float *term = tbuf + (ent * 4 + t) * TP + start;
                     double acc = 0.0;
-                    for (int j = 0; j < len; ++j) acc += (double)term[mem[j]];
+#pragma unroll 4
+                    for (int j = 0; j < len; ++j) acc += (double)term[j];
                     const int ee = P.elist[grp.start + i0 + ent];
                     P.partial[(int64_t)ee * P.PS + meta[8 + t] + gseg] = acc;
                 }
-                __syncthreads();
             }
         }
     }
-    (void)nvalid;
 }
 
 // ----------------------------------------------------------------------------------------------------------

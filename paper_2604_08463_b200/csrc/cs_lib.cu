@@ -25,7 +25,7 @@ namespace {
 struct MapHost {
     int32_t K = 0, nseg = 0;
     int32_t *idx = nullptr;
-    uint8_t *members = nullptr;
+    uint8_t *rank = nullptr;
     int32_t *segptr = nullptr;
     uint16_t *segdesc = nullptr;
     int32_t *ksegptr = nullptr;
@@ -67,6 +67,8 @@ struct cs_ctx {
     // data
     const float *d = nullptr;
     int32_t ndata = 0;
+    CUtensorMap tmap;                   // d as [ndata*2*nfreq, npix], box [2*nfreq, 32]
+    bool have_tmap = false;
     // batch
     int32_t batch = 0, ngroup = 0, ktot_max = 0;
     int64_t nparam = 0, nrows = 0, PS = 0;
@@ -102,7 +104,7 @@ namespace {
 
 void free_clusters(cs_ctx *c) {
     for (auto &m : c->maps) {
-        cudaFree(m.idx); cudaFree(m.members); cudaFree(m.segptr); cudaFree(m.segdesc); cudaFree(m.ksegptr); cudaFree(m.kseglist);
+        cudaFree(m.idx); cudaFree(m.rank); cudaFree(m.segptr); cudaFree(m.segdesc); cudaFree(m.ksegptr); cudaFree(m.kseglist);
     }
     c->maps.clear();
     cudaFree(c->d_maps); cudaFree(c->d_cfgs); cudaFree(c->d_npix_live);
@@ -140,10 +142,10 @@ double krj2kcmb(double nu_ghz, double tcmb, double hk) {
     return em1 * em1 / (x * x * std::exp(x));
 }
 
-// Reduction plan of one cluster map: per tile the member permutation sorted by (cluster, pixel), cut into
-// segments of <= SEG_MAX pixels of one cluster, plus the CSR cluster -> segments.
+// Reduction plan of one cluster map: per tile the rank of every pixel in the (cluster, pixel) order, that order cut
+// into segments of <= SEG_MAX pixels of one cluster, plus the CSR cluster -> segments.
 int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, MapHost *out, int64_t *bytes) {
-    std::vector<uint8_t> members((size_t)ntile * TP, 0);
+    std::vector<uint8_t> rank((size_t)ntile * TP, 0);
     std::vector<int32_t> segptr(ntile + 1, 0);
     std::vector<uint16_t> segdesc;
     std::vector<int32_t> segcluster;
@@ -167,7 +169,7 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
             segcluster.push_back(tmp[i].first);
             i = j;
         }
-        for (size_t q = 0; q < tmp.size(); ++q) members[p0 + q] = (uint8_t)tmp[q].second;
+        for (size_t q = 0; q < tmp.size(); ++q) rank[p0 + tmp[q].second] = (uint8_t)q;
     }
     segptr[ntile] = (int32_t)segdesc.size();
     const int32_t nseg = (int32_t)segdesc.size();
@@ -180,11 +182,38 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     out->K = K; out->nseg = nseg;
     int rc;
     if ((rc = dev_upload(&out->idx, idxv, bytes))) return rc;
-    if ((rc = dev_upload(&out->members, members, bytes))) return rc;
+    if ((rc = dev_upload(&out->rank, rank, bytes))) return rc;
     if ((rc = dev_upload(&out->segptr, segptr, bytes))) return rc;
     if ((rc = dev_upload(&out->segdesc, segdesc, bytes))) return rc;
     if ((rc = dev_upload(&out->ksegptr, ksegptr, bytes))) return rc;
     if ((rc = dev_upload(&out->kseglist, kseglist, bytes))) return rc;
+    return CS_OK;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// TMA descriptor of d viewed as a 2-D fp32 tensor [ndata*2*nfreq rows, npix]; one box = all rows of one data set for
+// 32 consecutive pixels.  Only possible when rows are 16-byte aligned; otherwise the kernels use plain loads.
+int make_tmap(cs_ctx *c) {
+    c->have_tmap = false;
+    std::memset(&c->tmap, 0, sizeof(c->tmap));
+    if ((c->npix % 4) != 0 || (((uintptr_t)c->d) % 16) != 0) return CS_OK;
+    static EncodeTiledFn enc = nullptr;
+    if (!enc) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return CS_ECUDA;
+        enc = (EncodeTiledFn)fn;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)c->npix, (cuuint64_t)c->ndata * 2 * c->nfreq};
+    const cuuint64_t strides[1] = {(cuuint64_t)c->npix * 4};
+    const cuuint32_t box[2] = {32, (cuuint32_t)(2 * c->nfreq)}, es[2] = {1, 1};
+    if (enc(&c->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)c->d, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return CS_ECUDA;
+    c->have_tmap = true;
     return CS_OK;
 }
 
@@ -203,7 +232,7 @@ int launch_like_t(cs_ctx *c, const LikeParams &P, int ngroup, cudaStream_t st) {
         dim3 grid(c->ntile, std::min(65535, ngroup - g0));
         const bool prof = c->prof_on && MODE == MODE_GRAD;
         if (prof) cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING)], st);
-        k_like<NF, MODE><<<grid, TP, smem, st>>>(Q);
+        k_like<NF, MODE><<<grid, TP, smem, st>>>(c->tmap, Q);
         if (prof) { cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING) + 1], st); c->prof_n++; }
         c->launches++;
     }
@@ -222,7 +251,8 @@ LikeParams base_params(cs_ctx *c) {
     P.d = c->d;
     P.npix = c->npix;
     P.nfreq = c->nfreq;
-    P.use_bulk = ((c->npix % 4) == 0 && (((uintptr_t)c->d) % 16) == 0) ? 1 : 0;
+    P.use_bulk = c->have_tmap ? 1 : 0;
+    P.evict_first = ((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4 > (int64_t)96 << 20) ? 1 : 0;
     P.maps = c->d_maps;
     P.cfgs = c->d_cfgs;
     P.groups = c->d_groups;
@@ -362,7 +392,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     std::vector<MapDev> md(nmap + 1);
     for (int32_t m = 0; m <= nmap; ++m) {
         const MapHost &s = c->maps[m];
-        md[m] = MapDev{s.idx, s.members, s.segptr, s.segdesc, s.ksegptr, s.kseglist, s.K, s.nseg};
+        md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.ksegptr, s.kseglist, s.K, s.nseg};
     }
     c->cfgs.resize(ncfg);
     c->npix_live.assign((size_t)ncfg * nregion, 0);
@@ -412,6 +442,8 @@ int cs_set_data(cs_ctx *c, int32_t ndata, const float *d, const float *ninv) {
     c->d = d;
     c->ndata = ndata;
     c->have_ninv = true;
+    int rc = make_tmap(c);
+    if (rc) return rc;
     for (int e = 0; e < c->batch; ++e)
         if (c->data_of[e] >= ndata) return CS_EINVAL;
     return CS_OK;
