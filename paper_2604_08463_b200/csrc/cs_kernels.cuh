@@ -128,62 +128,92 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
 }
 
 // ----------------------------------------------------------------------------------------------------------
-// a2: per-pixel arithmetic.  NF = number of bands looped over (15 fast path, 16 generic with zero weights).
+// a2: per-pixel arithmetic in packed fp32x2 (FFMA2 / FMUL2 / FADD2 on sm_100): the two lanes of every packed
+// operation are two consecutive bands (f, f+1), so table rows (float4 loads), constants and data pair up without
+// any broadcast; the 16th band is a zero pad.  Accumulators are reduced lane-to-scalar once per pixel.
 // ----------------------------------------------------------------------------------------------------------
+constexpr int NPAIR = NROW / 2;
+
+// The pixel's data in the warp's shared-memory stage: rows are (band, Stokes), 32 pixels per row.  Both passes
+// (forward and gradient) read it from there instead of keeping 30 values in registers.
 template <int NF>
 struct PixelIn {
-    float dq[NF], du[NF];
+    const float *st;   // stage base + lane
+    __device__ __forceinline__ float2 dq(int j) const {
+        return make_float2(st[(4 * j + 0) * 32], (2 * j + 1 < NF) ? st[(4 * j + 2) * 32] : 0.f);
+    }
+    __device__ __forceinline__ float2 du(int j) const {
+        return make_float2(st[(4 * j + 1) * 32], (2 * j + 1 < NF) ? st[(4 * j + 3) * 32] : 0.f);
+    }
 };
 
-__device__ __forceinline__ void load_row(const float *__restrict__ row, float (&out)[NROW]) {
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 dup2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float hsum(float2 a) { return a.x + a.y; }
+
+__device__ __forceinline__ void load_row(const float *__restrict__ row, float2 (&out)[NPAIR]) {
     const float4 *r4 = reinterpret_cast<const float4 *>(row);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const float4 v = __ldg(r4 + i);
-        out[4 * i + 0] = v.x; out[4 * i + 1] = v.y; out[4 * i + 2] = v.z; out[4 * i + 3] = v.w;
+        out[2 * i] = make_float2(v.x, v.y);
+        out[2 * i + 1] = make_float2(v.z, v.w);
     }
 }
 
-// Forward part shared by all modes: builds a_d, a_s, M, b, solves; returns s (component amplitudes) and ll.
+// 1/x for x > 0 in normal range: MUFU.RCP plus one Newton step (error below 1 ulp; no slow-path branch).
+__device__ __forceinline__ float fast_rcp(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return fmaf(r, fmaf(-x, r, 1.0f), r);
+}
+
+// Forward part shared by all modes: M = A^T N^-1 A, b = A^T N^-1 d, LDL^T solve; returns s and ll.
 template <int NF>
-__device__ __forceinline__ bool pixel_forward(const PixelIn<NF> &in, const float (&Fd)[NROW], const float (&G)[NROW],
-                                              const float (&Fs)[NROW], const KConst &kc, float (&ad)[NF],
-                                              float (&sq)[3], float (&su)[3], float &ll) {
-    float m01 = 0.f, m02 = 0.f, m11 = 0.f, m12 = 0.f, m22 = 0.f;
-    float bq0 = 0.f, bq1 = 0.f, bq2 = 0.f, bu0 = 0.f, bu1 = 0.f, bu2 = 0.f;
+__device__ __forceinline__ bool pixel_forward(const PixelIn<NF> &in, const float2 (&ad)[NPAIR], const float2 (&as)[NPAIR],
+                                              const KConst &kc, float (&sq)[3], float (&su)[3], float &ll) {
+    const float2 *w2 = reinterpret_cast<const float2 *>(kc.w);
+    const float2 z = make_float2(0.f, 0.f);
+    float2 m01 = z, m02 = z, m11 = z, m12 = z, m22 = z;
+    float2 bq0 = z, bq1 = z, bq2 = z, bu0 = z, bu1 = z, bu2 = z;
 #pragma unroll
-    for (int f = 0; f < NF; ++f) {
-        const float a = Fd[f] * G[f];     // a_d = cd (nu/nu0)^beta_d * Planck ratio     (Eq. 2)
-        const float s = Fs[f];            // a_s = cs (nu/nu0)^beta_s
-        ad[f] = a;
-        const float wd = kc.w[f] * a, ws = kc.w[f] * s;
-        m01 += wd; m02 += ws;
-        m11 = fmaf(wd, a, m11); m12 = fmaf(wd, s, m12); m22 = fmaf(ws, s, m22);
-        bq0 = fmaf(kc.w[f], in.dq[f], bq0); bq1 = fmaf(wd, in.dq[f], bq1); bq2 = fmaf(ws, in.dq[f], bq2);
-        bu0 = fmaf(kc.w[f], in.du[f], bu0); bu1 = fmaf(wd, in.du[f], bu1); bu2 = fmaf(ws, in.du[f], bu2);
+    for (int j = 0; j < NPAIR; ++j) {
+        const float2 a = ad[j];            // a_d = cd (nu/nu0)^beta_d * Planck ratio     (Eq. 2)
+        const float2 s = as[j];            // a_s = cs (nu/nu0)^beta_s
+        const float2 wd = mul2(w2[j], a), ws = mul2(w2[j], s);
+        m01 = add2(m01, wd); m02 = add2(m02, ws);
+        m11 = fma2(wd, a, m11); m12 = fma2(wd, s, m12); m22 = fma2(ws, s, m22);
+        const float2 dq = in.dq(j), du = in.du(j);
+        bq0 = fma2(w2[j], dq, bq0); bq1 = fma2(wd, dq, bq1); bq2 = fma2(ws, dq, bq2);
+        bu0 = fma2(w2[j], du, bu0); bu1 = fma2(wd, du, bu1); bu2 = fma2(ws, du, bu2);
     }
     // LDL^T of the 3x3 SPD matrix M = A^T N^-1 A (m00 = sum w is a constant)
-    const float l10 = m01 * kc.inv_m00, l20 = m02 * kc.inv_m00;
-    const float d1 = fmaf(-l10, m01, m11);
-    const float t12 = fmaf(-l10, m02, m12);
-    const float id1 = __frcp_rn(d1);
+    const float M01 = hsum(m01), M02 = hsum(m02), M11 = hsum(m11), M12 = hsum(m12), M22 = hsum(m22);
+    const float l10 = M01 * kc.inv_m00, l20 = M02 * kc.inv_m00;
+    const float d1 = fmaf(-l10, M01, M11);
+    const float t12 = fmaf(-l10, M02, M12);
+    const float id1 = fast_rcp(d1);
     const float l21 = t12 * id1;
-    const float d2 = fmaf(-l21, t12, fmaf(-l20, m02, m22));
-    const float id2 = __frcp_rn(d2);
+    const float d2 = fmaf(-l21, t12, fmaf(-l20, M02, M22));
+    const float id2 = fast_rcp(d2);
     const bool ok = (d1 > 0.f) && (d2 > 0.f);
     {
-        const float y0 = bq0, y1 = fmaf(-l10, bq0, bq1);
-        const float y2 = fmaf(-l21, y1, fmaf(-l20, bq0, bq2));
-        const float z0 = y0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
+        const float b0 = hsum(bq0), b1 = hsum(bq1), b2 = hsum(bq2);
+        const float y1 = fmaf(-l10, b0, b1);
+        const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
+        const float z0 = b0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
         sq[2] = z2; sq[1] = fmaf(-l21, z2, z1); sq[0] = fmaf(-l20, sq[2], fmaf(-l10, sq[1], z0));
-        ll = fmaf(y0, z0, fmaf(y1, z1, y2 * z2));
+        ll = fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
     }
     {
-        const float y0 = bu0, y1 = fmaf(-l10, bu0, bu1);
-        const float y2 = fmaf(-l21, y1, fmaf(-l20, bu0, bu2));
-        const float z0 = y0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
+        const float b0 = hsum(bu0), b1 = hsum(bu1), b2 = hsum(bu2);
+        const float y1 = fmaf(-l10, b0, b1);
+        const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
+        const float z0 = b0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
         su[2] = z2; su[1] = fmaf(-l21, z2, z1); su[0] = fmaf(-l20, su[2], fmaf(-l10, su[1], z0));
-        ll += fmaf(y0, z0, fmaf(y1, z1, y2 * z2));
+        ll += fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
     }
     ll *= -0.5f;                          // -1/2 sum_S b_S . s_S                        (Eq. 6)
     return ok;
@@ -191,34 +221,40 @@ __device__ __forceinline__ bool pixel_forward(const PixelIn<NF> &in, const float
 
 // Gradient terms (Eq. 17 with s held fixed): g_theta = - sum_f w_f (da_f/dtheta) sum_S s_{S,c} r_{S,f}.
 template <int NF>
-__device__ __forceinline__ void pixel_grad(const PixelIn<NF> &in, const float (&ad)[NF], const float (&Fs)[NROW],
-                                           const float (&dG)[NROW], const KConst &kc, const float (&sq)[3],
+__device__ __forceinline__ void pixel_grad(const PixelIn<NF> &in, const float2 (&ad)[NPAIR], const float2 (&as)[NPAIR],
+                                           const float2 (&dG)[NPAIR], const KConst &kc, const float (&sq)[3],
                                            const float (&su)[3], float &g_bd, float &g_td, float &g_bs) {
     // q_f  = sum_S s_{S,dust} r_{S,f},  qs_f = sum_S s_{S,sync} r_{S,f},  r = d - A s, expanded so that the
     // residual itself is never stored.
-    const float c0 = fmaf(sq[1], sq[0], su[1] * su[0]);
-    const float c1 = fmaf(sq[1], sq[1], su[1] * su[1]);
-    const float c2 = fmaf(sq[1], sq[2], su[1] * su[2]);
-    const float e0 = fmaf(sq[2], sq[0], su[2] * su[0]);
-    const float e2 = fmaf(sq[2], sq[2], su[2] * su[2]);
-    float g1 = 0.f, g2 = 0.f, g3 = 0.f;
+    const float2 *w2 = reinterpret_cast<const float2 *>(kc.w);
+    const float2 *lnd2 = reinterpret_cast<const float2 *>(kc.lnd);
+    const float2 *lnsw2 = reinterpret_cast<const float2 *>(kc.lnsw);
+    const float2 sqd = dup2(sq[1]), sud = dup2(su[1]), sqs = dup2(sq[2]), sus = dup2(su[2]);
+    const float2 nc0 = dup2(-fmaf(sq[1], sq[0], su[1] * su[0]));
+    const float2 nc1 = dup2(-fmaf(sq[1], sq[1], su[1] * su[1]));
+    const float2 nc2 = dup2(-fmaf(sq[1], sq[2], su[1] * su[2]));
+    const float2 ne0 = dup2(-fmaf(sq[2], sq[0], su[2] * su[0]));
+    const float2 ne2 = dup2(-fmaf(sq[2], sq[2], su[2] * su[2]));
+    const float2 z = make_float2(0.f, 0.f);
+    float2 g1 = z, g2 = z, g3 = z;
 #pragma unroll
-    for (int f = 0; f < NF; ++f) {
-        const float a = ad[f], s = Fs[f];
-        float q = fmaf(sq[1], in.dq[f], -c0);
-        q = fmaf(su[1], in.du[f], q);
-        q = fmaf(-c1, a, q);
-        q = fmaf(-c2, s, q);
-        float qs = fmaf(sq[2], in.dq[f], -e0);
-        qs = fmaf(su[2], in.du[f], qs);
-        qs = fmaf(-c2, a, qs);
-        qs = fmaf(-e2, s, qs);
-        const float t = kc.w[f] * (a * q);
-        g1 = fmaf(kc.lnd[f], t, g1);          // d a_d / d beta_d = ln(nu/nu0d) a_d
-        g2 = fmaf(dG[f], t, g2);              // d a_d / d T_d    = (d ln G / dT) a_d
-        g3 = fmaf(kc.lnsw[f], s * qs, g3);    // d a_s / d beta_s = ln(nu/nu0s) a_s
+    for (int j = 0; j < NPAIR; ++j) {
+        const float2 a = ad[j], s = as[j];
+        const float2 dq = in.dq(j), du = in.du(j);
+        float2 q = fma2(sqd, dq, nc0);
+        q = fma2(sud, du, q);
+        q = fma2(nc1, a, q);
+        q = fma2(nc2, s, q);
+        float2 qs = fma2(sqs, dq, ne0);
+        qs = fma2(sus, du, qs);
+        qs = fma2(nc2, a, qs);
+        qs = fma2(ne2, s, qs);
+        const float2 t = mul2(w2[j], mul2(a, q));
+        g1 = fma2(lnd2[j], t, g1);               // d a_d / d beta_d = ln(nu/nu0d) a_d
+        g2 = fma2(dG[j], t, g2);                 // d a_d / d T_d    = (d ln G / dT) a_d
+        g3 = fma2(lnsw2[j], mul2(s, qs), g3);    // d a_s / d beta_s = ln(nu/nu0s) a_s
     }
-    g_bd = -g1; g_td = -g2; g_bs = -g3;
+    g_bd = -hsum(g1); g_td = -hsum(g2); g_bs = -hsum(g3);
 }
 
 // ----------------------------------------------------------------------------------------------------------
@@ -234,10 +270,16 @@ __device__ __forceinline__ void pixel_grad(const PixelIn<NF> &in, const float (&
 // shared memory: ring [8 warps][NST][2*NF][32] fp32 | terms [2][EC][4][TP] fp32 | barriers [8][NST] | meta
 // ----------------------------------------------------------------------------------------------------------
 constexpr int NWARP = TP / 32;
+constexpr int TROW = TP + 4;   // floats per term row: TP ranks + a dump slot for pixels without a rank
 
 template <int NF>
 constexpr size_t like_smem_bytes() {
-    return (size_t)NWARP * NST * 2 * NF * 32 * 4 + (size_t)2 * EC * 4 * TP * 4 + NWARP * NST * 8 + 64 * 4;
+    return (size_t)NWARP * NST * 2 * NF * 32 * 4      // data ring
+           + (size_t)2 * EC * 4 * TROW * 4            // double-buffered terms
+           + NWARP * NST * 8                          // mbarriers
+           + GROUP_MAX * 16                           // per-entry table base (8 B), data row (4 B), entry id (4 B)
+           + 4 * TP * 2                               // segment descriptors of the tile, four maps
+           + 16 * 4;                                  // meta
 }
 
 __device__ __forceinline__ void tma_box_g2s(void *dst, const CUtensorMap *map, int x, int y, uint64_t *bar, uint64_t policy) {
@@ -253,8 +295,12 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     float *ring = reinterpret_cast<float *>(smem_raw);
     float *sterm = ring + NWARP * NST * 2 * NF * 32;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(sterm + 2 * EC * 4 * TP);
-    int32_t *meta = reinterpret_cast<int32_t *>(bars + NWARP * NST);   // [0..3] nseg, [4..7] first seg, [8..11] segbase
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sterm + 2 * EC * 4 * TROW);
+    const float **s_tab = reinterpret_cast<const float **>(bars + NWARP * NST);   // [GROUP_MAX] table base of entry
+    int32_t *s_drow = reinterpret_cast<int32_t *>(s_tab + GROUP_MAX);             // [GROUP_MAX] first d row of entry
+    int32_t *s_ent = s_drow + GROUP_MAX;                                          // [GROUP_MAX] entry id
+    uint16_t *s_desc = reinterpret_cast<uint16_t *>(s_ent + GROUP_MAX);           // [4][TP] segment descriptors
+    int32_t *meta = reinterpret_cast<int32_t *>(s_desc + 4 * TP);                 // [0..3] nseg, [4..7] first seg, [8..11] segbase
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int tile = blockIdx.x;
@@ -267,27 +313,50 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
     constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;   // value-only: only the ll / region term is reduced
 
     int k0 = -1, k1 = -1, k2 = -1;
-    uint32_t rank4 = 0;   // rank of this pixel in the tile order of the four reducing maps, 8 bits each
+    // float offset of this pixel's slot in each term row: its rank in the tile's (cluster, pixel) order of the
+    // reducing map, or the dump slot TP when the pixel has no cluster there
+    int so0 = 0 * TROW + TP, so1 = 1 * TROW + TP, so2 = 2 * TROW + TP, so3 = 3 * TROW + TP;
     if (p < npix) {
         k0 = P.maps[cfg.map[0]].idx[p];
         k1 = P.maps[cfg.map[1]].idx[p];
         k2 = P.maps[cfg.map[2]].idx[p];
         if (kReduce) {
-#pragma unroll
-            for (int t = T0; t < 4; ++t) {
-                const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
-                rank4 |= (uint32_t)P.maps[mi].rank[p] << (8 * t);
+            const int m3 = cfg.map[3];
+            if (MODE == MODE_CMBVAR) {
+                const int r = P.maps[m3].rank[p];
+                so0 = 0 * TROW + r; so1 = 1 * TROW + r; so2 = 2 * TROW + r; so3 = 3 * TROW + r;
+            } else {
+                if (MODE != MODE_VALUE) {
+                    if (k0 >= 0) so0 = 0 * TROW + P.maps[cfg.map[0]].rank[p];
+                    if (k1 >= 0) so1 = 1 * TROW + P.maps[cfg.map[1]].rank[p];
+                    if (k2 >= 0) so2 = 2 * TROW + P.maps[cfg.map[2]].rank[p];
+                }
+                so3 = 3 * TROW + P.maps[m3].rank[p];
             }
         }
     }
     const bool live = (k0 >= 0) && (k1 >= 0) && (k2 >= 0);
-    if (kReduce && tid < 4) {
-        const int t = tid;
-        const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
-        const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
-        meta[t] = (t >= T0) ? (s1 - s0) : 0;
-        meta[4 + t] = s0;
-        meta[8 + t] = (MODE == MODE_CMBVAR) ? t * P.maps[mi].nseg : cfg.segbase[t];
+    if (kReduce) {
+        if (tid < 4) {
+            const int t = tid;
+            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+            const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
+            meta[t] = (t >= T0) ? (s1 - s0) : 0;
+            meta[4 + t] = s0;
+            meta[8 + t] = (MODE == MODE_CMBVAR) ? t * P.maps[mi].nseg : cfg.segbase[t];
+        }
+#pragma unroll
+        for (int t = T0; t < 4; ++t) {
+            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+            const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
+            if (tid < s1 - s0) s_desc[t * TP + tid] = P.maps[mi].segdesc[s0 + tid];
+        }
+    }
+    if (tid < grp.count) {
+        const int e = P.elist[grp.start + tid];
+        s_ent[tid] = e;
+        s_drow[tid] = P.data_of[e] * nrows;
+        s_tab[tid] = P.tab + P.tab_off[e] * NROW;
     }
     float *wring = ring + warp * NST * 2 * NF * 32;
     uint64_t *wbar = bars + warp * NST;
@@ -310,47 +379,46 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
     if (P.use_bulk) policy = P.evict_first ? policy_evict_first() : policy_evict_normal();
 
     auto issue = [&](int i) {   // lane 0 only
-        const int e = P.elist[grp.start + i];
-        const int n = P.data_of[e];
         const int s = i % NST;
         mbar_expect_tx(&wbar[s], box_bytes);
-        tma_box_g2s(wring + s * 2 * NF * 32, &tmap, px0, n * nrows, &wbar[s], policy);
+        tma_box_g2s(wring + s * 2 * NF * 32, &tmap, px0, s_drow[i], &wbar[s], policy);
     };
     if (P.use_bulk && warp_has_pixels && lane == 0)
         for (int i = 0; i < NST && i < grp.count; ++i) issue(i);
 
+    // row offsets (in floats) of this pixel's table rows inside an entry's table block
+    const int r_fd = k0 * NROW, r_g = (cfg.K[0] + k1) * NROW, r_dg = (cfg.K[0] + cfg.K[1] + k1) * NROW,
+              r_fs = (cfg.K[0] + 2 * cfg.K[1] + k2) * NROW;
+
     for (int i = 0; i < grp.count; ++i) {
         const int s = i % NST;
-        const int e = P.elist[grp.start + i];
+        const float *tb = s_tab[i];
+        float2 ad[NPAIR], Fs[NPAIR];
+        if (live) {   // table rows first: their latency overlaps the wait for the data box
+            float2 Fd[NPAIR], G[NPAIR];
+            load_row(tb + r_fd, Fd);
+            load_row(tb + r_g, G);
+            load_row(tb + r_fs, Fs);
+#pragma unroll
+            for (int j = 0; j < NPAIR; ++j) ad[j] = mul2(Fd[j], G[j]);
+        }
         PixelIn<NF> in;
+        in.st = wring + s * 2 * NF * 32 + lane;
         if (warp_has_pixels) {
-            const float *st = wring + s * 2 * NF * 32;
             if (P.use_bulk) {
                 mbar_wait(&wbar[s], (uint32_t)((i / NST) & 1));
             } else {
-                const int64_t n = P.data_of[e];
+                const int64_t row0 = s_drow[i];
                 for (int r = 0; r < nrows; ++r)
-                    wring[(s * 2 * NF + r) * 32 + lane] = (p < npix) ? P.d[(n * nrows + r) * npix + p] : 0.f;
+                    wring[(s * 2 * NF + r) * 32 + lane] = (p < npix) ? P.d[(row0 + r) * npix + p] : 0.f;
                 __syncwarp();
             }
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-                in.dq[f] = st[(2 * f + 0) * 32 + lane];
-                in.du[f] = st[(2 * f + 1) * 32 + lane];
-            }
-            __syncwarp();   // the whole warp holds its data in registers: the stage may be refilled
-            if (P.use_bulk && lane == 0 && i + NST < grp.count) issue(i + NST);
         }
 
         float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
         if (live) {
-            const float *tb = P.tab + P.tab_off[e] * NROW;
-            float Fd[NROW], G[NROW], Fs[NROW];
-            load_row(tb + (int64_t)k0 * NROW, Fd);
-            load_row(tb + (int64_t)(cfg.K[0] + k1) * NROW, G);
-            load_row(tb + (int64_t)(cfg.K[0] + 2 * cfg.K[1] + k2) * NROW, Fs);
-            float ad[NF], sq[3], su[3], ll;
-            const bool ok = pixel_forward<NF>(in, Fd, G, Fs, P.kc, ad, sq, su, ll);
+            float sq[3], su[3], ll;
+            const bool ok = pixel_forward<NF>(in, ad, Fs, P.kc, sq, su, ll);
             if (!ok) {
                 atomicOr(P.err, ERR_SINGULAR);
                 ll = CUDART_INF_F;
@@ -358,8 +426,8 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
             if (MODE == MODE_VALUE) {
                 t3 = ll;
             } else if (MODE == MODE_GRAD) {
-                float dG[NROW];
-                load_row(tb + (int64_t)(cfg.K[0] + cfg.K[1] + k1) * NROW, dG);
+                float2 dG[NPAIR];
+                load_row(tb + r_dg, dG);
                 pixel_grad<NF>(in, ad, Fs, dG, P.kc, sq, su, t0, t1, t2);
                 t3 = ll;
             } else if (MODE == MODE_CMBVAR) {
@@ -374,40 +442,34 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
 #pragma unroll
             for (int c = 0; c < 6; ++c) o[c * npix] = 0.f;
         }
+        if (warp_has_pixels && P.use_bulk) {
+            __syncwarp();   // every lane is done reading stage s: refill it with the entry NST ahead
+            if (lane == 0 && i + NST < grp.count) issue(i + NST);
+        }
         if (kReduce) {
-            // terms at the pixel's rank in each reducing map's (cluster, pixel) order; pixels without a cluster in
-            // map t have no rank there (and are not live), live == false elsewhere contributes an explicit zero
-            float *tm = sterm + (((i / EC) & 1) * EC + (i % EC)) * 4 * TP;
-            if (p < npix) {
-                if (MODE != MODE_VALUE) {
-                    if (k0 >= 0 || MODE == MODE_CMBVAR) tm[0 * TP + (rank4 & 0xff)] = t0;
-                    if (k1 >= 0 || MODE == MODE_CMBVAR) tm[1 * TP + ((rank4 >> 8) & 0xff)] = t1;
-                    if (k2 >= 0 || MODE == MODE_CMBVAR) tm[2 * TP + ((rank4 >> 16) & 0xff)] = t2;
-                }
-                tm[3 * TP + (rank4 >> 24)] = t3;
-            }
+            float *tm = sterm + (((i / EC) & 1) * EC + (i % EC)) * 4 * TROW;
+            if (MODE != MODE_VALUE) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
+            tm[so3] = t3;
             if ((i % EC) == EC - 1 || i == grp.count - 1) {
                 __syncthreads();
                 // first level of the ordered reduction: one thread per (entry, term, segment); a segment is a
                 // contiguous run of the rank-ordered terms, summed in ascending pixel order in fp64.
                 const int i0 = i - (i % EC), nent = (i % EC) + 1;
-                const float *tbuf = sterm + ((i / EC) & 1) * EC * 4 * TP;
+                const float *tbuf = sterm + ((i / EC) & 1) * EC * 4 * TROW;
                 const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
                 const int c1 = n0, c2 = n0 + n1, c3 = n0 + n1 + n2, tot = c3 + n3;
+                const float inv_tot = 1.0f / (float)tot;
                 for (int w = tid; w < nent * tot; w += TP) {
-                    const int ent = w / tot, r = w - ent * tot;
+                    const int ent = (int)(((float)w + 0.5f) * inv_tot), r = w - ent * tot;
                     const int t = (r >= c1) + (r >= c2) + (r >= c3);
                     const int ls = r - (t == 0 ? 0 : (t == 1 ? c1 : (t == 2 ? c2 : c3)));
-                    const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
-                    const int gseg = meta[4 + t] + ls;
-                    const uint32_t desc = P.maps[mi].segdesc[gseg];
+                    const uint32_t desc = s_desc[t * TP + ls];
                     const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
-                    const float *term = tbuf + (ent * 4 + t) * TP + start;
+                    const float *term = tbuf + (ent * 4 + t) * TROW + start;
                     double acc = 0.0;
 #pragma unroll 4
                     for (int j = 0; j < len; ++j) acc += (double)term[j];
-                    const int ee = P.elist[grp.start + i0 + ent];
-                    P.partial[(int64_t)ee * P.PS + meta[8 + t] + gseg] = acc;
+                    P.partial[(int64_t)s_ent[i0 + ent] * P.PS + meta[8 + t] + meta[4 + t] + ls] = acc;
                 }
             }
         }
