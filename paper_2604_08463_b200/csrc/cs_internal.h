@@ -8,8 +8,13 @@
 //              rows [K0+K1,K0+2K1)    dlnG[k][f] = d ln G / d T_d
 //              rows [K0+2K1, ..+K2)   Fs'[k][f] = cs[f] * (nu_f/nu0s)^beta_s[k]
 //   partial  [batch][PS] fp64   per-tile, per-segment ordered partial sums (written by k_like, read by k_merge)
+//            The slot of a segment inside its term's block is cluster-major (all segments of cluster 0 in ascending
+//            tile order, then cluster 1, ...), so that the merge reads every cluster's partials contiguously.
 //   plan     per cluster map: idx int32[npix], rank u8[ntile*TP], segptr int32[ntile+1], segdesc u16[nseg],
-//            ksegptr int32[K+1], kseglist int32[nseg]
+//            segslot int32[nseg], ksegptr int32[K+1]
+//   cells    per clustering configuration (cell path only): the distinct (k0,k1,k2) triples of every tile in order of
+//            first appearance: cellid u8[ntile*TP] (0xFF = masked pixel), cellptr int32[ntile+1],
+//            cellrows int32[ncell][4] = table rows (Fd', G, dlnG, Fs') of the cell
 #pragma once
 #include <stdint.h>
 
@@ -18,7 +23,13 @@ namespace cs {
 constexpr int TP = 256;        // pixels per tile == threads per CTA of the fused kernel
 constexpr int SEG_MAX = 32;    // longest ordered chain summed by one thread in the reduce phase
 constexpr int NROW = 16;       // floats per table row (nfreq padded to 16 -> 64-byte rows)
-constexpr int GROUP_MAX = 32;  // entries of one configuration handled by one CTA (per tile)
+constexpr int GROUP_MAX = 64;  // entries of one configuration handled by one CTA (per tile)
+constexpr int CELL_CAP = 96;   // cell path: most distinct cluster triples a tile may hold (else the direct kernel runs)
+constexpr int CSTRIDE = 68;    // floats per cell row in shared memory: 48 column values + 16 scalars + 4 pad (= 4 mod 32 banks)
+
+// A pivot of the LDL^T factorisation of M = A^T N^-1 A counts as non-positive (CS_ESINGULAR) when it is below this
+// fraction of its diagonal entry: below it an fp32 solve carries no correct digit (R11).
+constexpr float PIVOT_RTOL = 1e-6f;
 
 constexpr int ERR_DOMAIN = 1;
 constexpr int ERR_SINGULAR = 2;
@@ -29,8 +40,8 @@ struct MapDev {
     const uint8_t *rank;      // [ntile*TP] position of the pixel in its tile's (cluster id, pixel) order
     const int32_t *segptr;    // [ntile+1] first segment of each tile (map-local numbering)
     const uint16_t *segdesc;  // [nseg] start (8 bits) | (len-1) << 8
-    const int32_t *ksegptr;   // [K+1] CSR cluster -> segments
-    const int32_t *kseglist;  // [nseg] segment ids in ascending (tile, chunk) order per cluster
+    const int32_t *segslot;   // [nseg] cluster-major slot of the segment inside its term's block of a partial row
+    const int32_t *ksegptr;   // [K+1] CSR cluster -> slots [ksegptr[k], ksegptr[k+1])
     int32_t K;
     int32_t nseg;
 };
@@ -41,6 +52,12 @@ struct CfgDev {
     int32_t segbase[4];   // offset of term t inside a partial row (t = 0,1,2 gradient terms, 3 = ll / region)
     int32_t K[3];
     int32_t ktot;
+    // cell plan (null / 0 when the configuration runs on the direct kernel)
+    const uint8_t *cellid;     // [ntile*TP]
+    const int32_t *cellptr;    // [ntile+1]
+    const int32_t *cellrows;   // [ncell][4]
+    int32_t ncell_max;         // most cells in one tile; 0 = direct path
+    int32_t pad;
 };
 
 struct Group {
@@ -55,6 +72,7 @@ struct KConst {
     float w[NROW];     // Ninv per band, 0 beyond nfreq
     float lnd[NROW];   // ln(nu_f/nu0d)
     float lnsw[NROW];  // ln(nu_f/nu0s) * w_f
+    float lns[NROW];   // ln(nu_f/nu0s)
     float inv_m00;     // 1 / sum_f w_f
     float m00;
 };

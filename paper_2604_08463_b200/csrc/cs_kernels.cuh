@@ -67,6 +67,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
         "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
 }
+// Wait used by producer roles (loader, builders): they are ahead of the consumers most of the time, so the poll
+// backs off (suspend hint + nanosleep) instead of burning issue slots the consumers need.
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity) {
+    uint32_t done = 0;
+    while (true) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity), "r"(500u)
+            : "memory");
+        if (done) break;
+        __nanosleep(40);
+    }
+}
 // global -> shared bulk copy completing on an mbarrier; dst/src/bytes 16-byte aligned; evict-first L2 policy.
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t policy) {
     asm volatile(
@@ -198,7 +214,7 @@ __device__ __forceinline__ bool pixel_forward(const PixelIn<NF> &in, const float
     const float l21 = t12 * id1;
     const float d2 = fmaf(-l21, t12, fmaf(-l20, M02, M22));
     const float id2 = fast_rcp(d2);
-    const bool ok = (d1 > 0.f) && (d2 > 0.f);
+    const bool ok = (d1 > PIVOT_RTOL * M11) && (d2 > PIVOT_RTOL * M22);
     {
         const float b0 = hsum(bq0), b1 = hsum(bq1), b2 = hsum(bq2);
         const float y1 = fmaf(-l10, b0, b1);
@@ -268,9 +284,54 @@ __device__ __forceinline__ void pixel_grad(const PixelIn<NF> &in, const float2 (
 // per (entry, term, segment), ascending pixel order, fp64) into the partial buffer.  The term buffer is double
 // buffered: one __syncthreads per EC entries.
 // shared memory: ring [8 warps][NST][2*NF][32] fp32 | terms [2][EC][4][TP] fp32 | barriers [8][NST] | meta
+// (configurations whose tiles hold few distinct cluster triples run on k_like_cell, cs_like_cell.cuh, instead)
 // ----------------------------------------------------------------------------------------------------------
 constexpr int NWARP = TP / 32;
 constexpr int TROW = TP + 4;   // floats per term row: TP ranks + a dump slot for pixels without a rank
+
+// Loads the tile's segment descriptors and output slots of the four reducing maps into shared memory.
+// meta[t] = number of segments of term t in this tile (0 for terms below T0).
+template <int MODE>
+__device__ __forceinline__ void load_tile_plan(const MapDev *__restrict__ maps, const CfgDev &cfg, int tile, int tid,
+                                               uint16_t *s_desc, int32_t *s_slot, int32_t *meta) {
+    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;
+    if (tid < 4) {
+        const int t = tid;
+        const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+        meta[t] = (t >= T0) ? (maps[mi].segptr[tile + 1] - maps[mi].segptr[tile]) : 0;
+    }
+#pragma unroll
+    for (int t = T0; t < 4; ++t) {
+        const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
+        const int s0 = maps[mi].segptr[tile], s1 = maps[mi].segptr[tile + 1];
+        if (tid < s1 - s0) {
+            s_desc[t * TP + tid] = maps[mi].segdesc[s0 + tid];
+            s_slot[t * TP + tid] = ((MODE == MODE_CMBVAR) ? t * maps[mi].nseg : cfg.segbase[t]) + maps[mi].segslot[s0 + tid];
+        }
+    }
+}
+
+// First level of the ordered reduction (a3) for `nent` buffered entries: one thread per (entry, term, segment); a
+// segment is a contiguous run of the rank-ordered terms of one cluster, summed in ascending pixel order in fp64 and
+// stored at the segment's cluster-major slot of the entry's partial row.
+__device__ __forceinline__ void reduce_terms(const float *tbuf, int nent, int tid, const int32_t *meta, const uint16_t *s_desc,
+                                             const int32_t *s_slot, const int32_t *s_ent, double *__restrict__ partial, int64_t PS) {
+    const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
+    const int c1 = n0, c2 = n0 + n1, c3 = n0 + n1 + n2, tot = c3 + n3;
+    const float inv_tot = 1.0f / (float)tot;
+    for (int w = tid; w < nent * tot; w += TP) {
+        const int ent = (int)(((float)w + 0.5f) * inv_tot), r = w - ent * tot;
+        const int t = (r >= c1) + (r >= c2) + (r >= c3);
+        const int ls = r - (t == 0 ? 0 : (t == 1 ? c1 : (t == 2 ? c2 : c3)));
+        const uint32_t desc = s_desc[t * TP + ls];
+        const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
+        const float *term = tbuf + (ent * 4 + t) * TROW + start;
+        double acc = 0.0;
+#pragma unroll 4
+        for (int j = 0; j < len; ++j) acc += (double)term[j];
+        partial[(int64_t)s_ent[ent] * PS + s_slot[t * TP + ls]] = acc;
+    }
+}
 
 template <int NF>
 constexpr size_t like_smem_bytes() {
@@ -279,6 +340,7 @@ constexpr size_t like_smem_bytes() {
            + NWARP * NST * 8                          // mbarriers
            + GROUP_MAX * 16                           // per-entry table base (8 B), data row (4 B), entry id (4 B)
            + 4 * TP * 2                               // segment descriptors of the tile, four maps
+           + 4 * TP * 4                               // output slots of those segments
            + 16 * 4;                                  // meta
 }
 
@@ -300,7 +362,8 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
     int32_t *s_drow = reinterpret_cast<int32_t *>(s_tab + GROUP_MAX);             // [GROUP_MAX] first d row of entry
     int32_t *s_ent = s_drow + GROUP_MAX;                                          // [GROUP_MAX] entry id
     uint16_t *s_desc = reinterpret_cast<uint16_t *>(s_ent + GROUP_MAX);           // [4][TP] segment descriptors
-    int32_t *meta = reinterpret_cast<int32_t *>(s_desc + 4 * TP);                 // [0..3] nseg, [4..7] first seg, [8..11] segbase
+    int32_t *s_slot = reinterpret_cast<int32_t *>(s_desc + 4 * TP);               // [4][TP] output slots
+    int32_t *meta = s_slot + 4 * TP;                                              // [0..3] segments per term
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int tile = blockIdx.x;
@@ -336,22 +399,7 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
         }
     }
     const bool live = (k0 >= 0) && (k1 >= 0) && (k2 >= 0);
-    if (kReduce) {
-        if (tid < 4) {
-            const int t = tid;
-            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
-            const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
-            meta[t] = (t >= T0) ? (s1 - s0) : 0;
-            meta[4 + t] = s0;
-            meta[8 + t] = (MODE == MODE_CMBVAR) ? t * P.maps[mi].nseg : cfg.segbase[t];
-        }
-#pragma unroll
-        for (int t = T0; t < 4; ++t) {
-            const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
-            const int s0 = P.maps[mi].segptr[tile], s1 = P.maps[mi].segptr[tile + 1];
-            if (tid < s1 - s0) s_desc[t * TP + tid] = P.maps[mi].segdesc[s0 + tid];
-        }
-    }
+    if (kReduce) load_tile_plan<MODE>(P.maps, cfg, tile, tid, s_desc, s_slot, meta);
     if (tid < grp.count) {
         const int e = P.elist[grp.start + tid];
         s_ent[tid] = e;
@@ -452,32 +500,16 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
             tm[so3] = t3;
             if ((i % EC) == EC - 1 || i == grp.count - 1) {
                 __syncthreads();
-                // first level of the ordered reduction: one thread per (entry, term, segment); a segment is a
-                // contiguous run of the rank-ordered terms, summed in ascending pixel order in fp64.
                 const int i0 = i - (i % EC), nent = (i % EC) + 1;
-                const float *tbuf = sterm + ((i / EC) & 1) * EC * 4 * TROW;
-                const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
-                const int c1 = n0, c2 = n0 + n1, c3 = n0 + n1 + n2, tot = c3 + n3;
-                const float inv_tot = 1.0f / (float)tot;
-                for (int w = tid; w < nent * tot; w += TP) {
-                    const int ent = (int)(((float)w + 0.5f) * inv_tot), r = w - ent * tot;
-                    const int t = (r >= c1) + (r >= c2) + (r >= c3);
-                    const int ls = r - (t == 0 ? 0 : (t == 1 ? c1 : (t == 2 ? c2 : c3)));
-                    const uint32_t desc = s_desc[t * TP + ls];
-                    const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
-                    const float *term = tbuf + (ent * 4 + t) * TROW + start;
-                    double acc = 0.0;
-#pragma unroll 4
-                    for (int j = 0; j < len; ++j) acc += (double)term[j];
-                    P.partial[(int64_t)s_ent[i0 + ent] * P.PS + meta[8 + t] + meta[4 + t] + ls] = acc;
-                }
+                reduce_terms(sterm + ((i / EC) & 1) * EC * 4 * TROW, nent, tid, meta, s_desc, s_slot, s_ent + i0, P.partial, P.PS);
             }
         }
     }
 }
 
 // ----------------------------------------------------------------------------------------------------------
-// a3 second level: grad[e][j] / nll[e][r] = fixed-order sum over the segments of cluster j / region r.
+// a3 second level: grad[e][j] / nll[e][r] = fixed-order (ascending tile) sum over the segments of cluster j / region r,
+// which are contiguous in the partial row.
 // grid = (ceil(nout_max/256), batch).  want_grad = 0: only the region outputs.
 // ----------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
@@ -499,7 +531,7 @@ __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partia
     const double *row = partial + (int64_t)e * PS + c.segbase[t];
     double acc = 0.0;
     const int a = m.ksegptr[k], b = m.ksegptr[k + 1];
-    for (int q = a; q < b; ++q) acc += row[m.kseglist[q]];
+    for (int q = a; q < b; ++q) acc += row[q];
     if (t == 3) nll[(int64_t)e * nregion + k] = acc;
     else grad[param_off[e] + j] = acc;
 }
@@ -518,7 +550,7 @@ __global__ void __launch_bounds__(128) k_cmbvar(const double *__restrict__ parti
     for (int t = 0; t < 4; ++t) {
         const double *row = partial + (int64_t)e * PS + (int64_t)t * m.nseg;
         double acc = 0.0;
-        for (int q = m.ksegptr[r]; q < m.ksegptr[r + 1]; ++q) acc += row[m.kseglist[q]];
+        for (int q = m.ksegptr[r]; q < m.ksegptr[r + 1]; ++q) acc += row[q];
         s[t] = acc;
     }
     const double n = (double)npix_live[cfg_of[e] * nregion + r];

@@ -4,12 +4,14 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
 #include "../../include/cs.h"
 #include "cs_kernels.cuh"
+#include "cs_like_cell.cuh"
 #include "cs_optim.cuh"
 
 using namespace cs;
@@ -28,8 +30,15 @@ struct MapHost {
     uint8_t *rank = nullptr;
     int32_t *segptr = nullptr;
     uint16_t *segdesc = nullptr;
+    int32_t *segslot = nullptr;
     int32_t *ksegptr = nullptr;
-    int32_t *kseglist = nullptr;
+};
+
+// Device arrays of one configuration's cell plan (empty when it runs on the direct kernel).
+struct CellHost {
+    uint8_t *cellid = nullptr;
+    int32_t *cellptr = nullptr;
+    int32_t *cellrows = nullptr;
 };
 
 template <typename T>
@@ -59,6 +68,7 @@ struct cs_ctx {
     int32_t nmap = 0, ncfg = 0, nregion = 1;
     std::vector<MapHost> maps;          // nmap + 1 (last = region pseudo-map)
     std::vector<CfgDev> cfgs;
+    std::vector<CellHost> cellplans;    // ncfg
     std::vector<int32_t> npix_live;     // [ncfg*nregion]
     MapDev *d_maps = nullptr;
     CfgDev *d_cfgs = nullptr;
@@ -67,10 +77,11 @@ struct cs_ctx {
     // data
     const float *d = nullptr;
     int32_t ndata = 0;
-    CUtensorMap tmap;                   // d as [ndata*2*nfreq, npix], box [2*nfreq, 32]
+    CUtensorMap tmap;                   // d as [ndata*2*nfreq, npix], box [2*nfreq, 32]   (direct kernel: one box per warp)
+    CUtensorMap tmap_cta;               // same tensor, box [2*nfreq, TP]                  (cell kernel: one box per CTA)
     bool have_tmap = false;
     // batch
-    int32_t batch = 0, ngroup = 0, ktot_max = 0;
+    int32_t batch = 0, ngroup = 0, ngroup_cell = 0, ktot_max = 0;   // groups [0, ngroup_cell) run on the cell kernel
     int64_t nparam = 0, nrows = 0, PS = 0;
     std::vector<int32_t> cfg_of, data_of;
     std::vector<int64_t> param_off;
@@ -98,15 +109,18 @@ struct cs_ctx {
     int32_t *d_err = nullptr;
     int64_t launches = 0;
     bool tables_built = false;
+    bool force_direct = false;          // CS_FORCE_DIRECT=1 in the environment at cs_create: never use the cell kernel (tests)
 };
 
 namespace {
 
 void free_clusters(cs_ctx *c) {
     for (auto &m : c->maps) {
-        cudaFree(m.idx); cudaFree(m.rank); cudaFree(m.segptr); cudaFree(m.segdesc); cudaFree(m.ksegptr); cudaFree(m.kseglist);
+        cudaFree(m.idx); cudaFree(m.rank); cudaFree(m.segptr); cudaFree(m.segdesc); cudaFree(m.segslot); cudaFree(m.ksegptr);
     }
     c->maps.clear();
+    for (auto &p : c->cellplans) { cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); }
+    c->cellplans.clear();
     cudaFree(c->d_maps); cudaFree(c->d_cfgs); cudaFree(c->d_npix_live);
     c->d_maps = nullptr; c->d_cfgs = nullptr; c->d_npix_live = nullptr;
     c->cfgs.clear();
@@ -152,6 +166,7 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     segdesc.reserve((size_t)ntile * 16);
     segcluster.reserve((size_t)ntile * 16);
     std::vector<std::pair<int32_t, int32_t>> tmp;
+    std::vector<std::pair<uint16_t, int32_t>> tseg;   // (descriptor, cluster)
     tmp.reserve(TP);
     for (int32_t t = 0; t < ntile; ++t) {
         tmp.clear();
@@ -161,23 +176,29 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
             if (idx[p0 + j] >= 0) tmp.emplace_back(idx[p0 + j], j);
         std::sort(tmp.begin(), tmp.end());
         segptr[t] = (int32_t)segdesc.size();
+        // segments of this tile, longest first: the lanes of a warp of the reduce phase then walk runs of similar length
+        tseg.clear();
         size_t i = 0;
         while (i < tmp.size()) {
             size_t j = i;
             while (j < tmp.size() && tmp[j].first == tmp[i].first && j - i < (size_t)SEG_MAX) ++j;
-            segdesc.push_back((uint16_t)(i | ((j - i - 1) << 8)));
-            segcluster.push_back(tmp[i].first);
+            tseg.push_back({(uint16_t)(i | ((j - i - 1) << 8)), tmp[i].first});
             i = j;
         }
+        std::stable_sort(tseg.begin(), tseg.end(), [](const std::pair<uint16_t, int32_t> &a, const std::pair<uint16_t, int32_t> &b) {
+            return (a.first >> 8) > (b.first >> 8);
+        });
+        for (auto &sg : tseg) { segdesc.push_back(sg.first); segcluster.push_back(sg.second); }
         for (size_t q = 0; q < tmp.size(); ++q) rank[p0 + tmp[q].second] = (uint8_t)q;
     }
     segptr[ntile] = (int32_t)segdesc.size();
     const int32_t nseg = (int32_t)segdesc.size();
-    std::vector<int32_t> ksegptr(K + 1, 0), kseglist(nseg);
+    // cluster-major slots: the segments of cluster k occupy [ksegptr[k], ksegptr[k+1]) in ascending (tile, chunk) order
+    std::vector<int32_t> ksegptr(K + 1, 0), segslot(nseg);
     for (int32_t s = 0; s < nseg; ++s) ksegptr[segcluster[s] + 1]++;
     for (int32_t k = 0; k < K; ++k) ksegptr[k + 1] += ksegptr[k];
     std::vector<int32_t> fill(ksegptr.begin(), ksegptr.end() - 1);
-    for (int32_t s = 0; s < nseg; ++s) kseglist[fill[segcluster[s]]++] = s;   // ascending s == ascending (tile, chunk)
+    for (int32_t s = 0; s < nseg; ++s) segslot[s] = fill[segcluster[s]]++;
     std::vector<int32_t> idxv(idx, idx + npix);
     out->K = K; out->nseg = nseg;
     int rc;
@@ -185,8 +206,54 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     if ((rc = dev_upload(&out->rank, rank, bytes))) return rc;
     if ((rc = dev_upload(&out->segptr, segptr, bytes))) return rc;
     if ((rc = dev_upload(&out->segdesc, segdesc, bytes))) return rc;
+    if ((rc = dev_upload(&out->segslot, segslot, bytes))) return rc;
     if ((rc = dev_upload(&out->ksegptr, ksegptr, bytes))) return rc;
-    if ((rc = dev_upload(&out->kseglist, kseglist, bytes))) return rc;
+    return CS_OK;
+}
+
+// Cell plan of one configuration: per tile the distinct (k0,k1,k2) triples in order of first appearance, as table-row
+// indices of an entry's table block.  Returns 1 (and uploads nothing) when some tile holds more than CELL_CAP cells:
+// that configuration then runs on the direct kernel.
+int build_cell_plan(const int32_t *i0, const int32_t *i1, const int32_t *i2, const int32_t K[3], int64_t npix, int32_t ntile,
+                    CellHost *out, int32_t *ncell_max, int64_t *bytes) {
+    std::vector<uint8_t> cellid((size_t)ntile * TP, 0xFF);
+    std::vector<int32_t> cellptr(ntile + 1, 0);
+    std::vector<int32_t> rows;
+    rows.reserve((size_t)ntile * 64 * 4);
+    int32_t mx = 0;
+    for (int32_t t = 0; t < ntile; ++t) {
+        const int64_t p0 = (int64_t)t * TP;
+        const int nv = (int)std::min<int64_t>(TP, npix - p0);
+        const size_t base = rows.size() / 4;
+        cellptr[t] = (int32_t)base;
+        int n = 0, last = -1;
+        for (int j = 0; j < nv; ++j) {
+            const int32_t a = i0[p0 + j], b = i1[p0 + j], d = i2[p0 + j];
+            if (a < 0 || b < 0 || d < 0) continue;
+            const int32_t r0 = a, r1 = K[0] + b, r3 = K[0] + 2 * K[1] + d;
+            int id = -1;
+            if (last >= 0 && rows[4 * (base + last)] == r0 && rows[4 * (base + last) + 1] == r1 && rows[4 * (base + last) + 3] == r3) {
+                id = last;   // consecutive pixels mostly share their cell
+            } else {
+                for (int q = n - 1; q >= 0; --q)
+                    if (rows[4 * (base + q)] == r0 && rows[4 * (base + q) + 1] == r1 && rows[4 * (base + q) + 3] == r3) { id = q; break; }
+            }
+            if (id < 0) {
+                if (n == CELL_CAP) return 1;
+                id = n++;
+                rows.push_back(r0); rows.push_back(r1); rows.push_back(K[0] + K[1] + b); rows.push_back(r3);
+            }
+            cellid[p0 + j] = (uint8_t)id;
+            last = id;
+        }
+        mx = std::max(mx, n);
+    }
+    cellptr[ntile] = (int32_t)(rows.size() / 4);
+    *ncell_max = mx;
+    int rc;
+    if ((rc = dev_upload(&out->cellid, cellid, bytes))) return rc;
+    if ((rc = dev_upload(&out->cellptr, cellptr, bytes))) return rc;
+    if ((rc = dev_upload(&out->cellrows, rows, bytes))) return rc;
     return CS_OK;
 }
 
@@ -199,6 +266,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 int make_tmap(cs_ctx *c) {
     c->have_tmap = false;
     std::memset(&c->tmap, 0, sizeof(c->tmap));
+    std::memset(&c->tmap_cta, 0, sizeof(c->tmap_cta));
     if ((c->npix % 4) != 0 || (((uintptr_t)c->d) % 16) != 0) return CS_OK;
     static EncodeTiledFn enc = nullptr;
     if (!enc) {
@@ -213,37 +281,47 @@ int make_tmap(cs_ctx *c) {
     if (enc(&c->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)c->d, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return CS_ECUDA;
+    const cuuint32_t box_cta[2] = {(cuuint32_t)TP, (cuuint32_t)(2 * c->nfreq)};
+    if (enc(&c->tmap_cta, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)c->d, dims, strides, box_cta, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return CS_ECUDA;
     c->have_tmap = true;
     return CS_OK;
 }
 
+// Launches the fused kernel over the groups [g0, g1) of P.groups; groups below `ncell` (cell path) run on
+// k_like_cell, the rest on the direct kernel k_like.  grid.y is limited to 65535: launch in slabs of groups.
 template <int NF, int MODE>
-int launch_like_t(cs_ctx *c, const LikeParams &P, int ngroup, cudaStream_t st) {
+int launch_like_t(cs_ctx *c, const LikeParams &P, int g0, int g1, int ncell, cudaStream_t st) {
     static bool configured = false;
-    constexpr size_t smem = like_smem_bytes<NF>();
+    constexpr size_t smem = like_smem_bytes<NF>(), smem_cell = cell_smem_bytes<NF>();
     if (!configured) {
         CK(cudaFuncSetAttribute(k_like<NF, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(cudaFuncSetAttribute(k_like_cell<NF, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cell));
         configured = true;
     }
-    // grid.y is limited to 65535: launch in slabs of groups
-    for (int g0 = 0; g0 < ngroup; g0 += 65535) {
-        LikeParams Q = P;
-        Q.groups = P.groups + g0;
-        dim3 grid(c->ntile, std::min(65535, ngroup - g0));
-        const bool prof = c->prof_on && MODE == MODE_GRAD;
-        if (prof) cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING)], st);
-        k_like<NF, MODE><<<grid, TP, smem, st>>>(c->tmap, Q);
-        if (prof) { cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING) + 1], st); c->prof_n++; }
-        c->launches++;
+    const bool prof = c->prof_on && MODE == MODE_GRAD;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int a = pass == 0 ? g0 : std::max(g0, ncell), b = pass == 0 ? std::min(g1, ncell) : g1;
+        for (int g = a; g < b; g += 65535) {
+            LikeParams Q = P;
+            Q.groups = P.groups + g;
+            dim3 grid(c->ntile, std::min(65535, b - g));
+            if (prof) cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING)], st);
+            if (pass == 0) k_like_cell<NF, MODE><<<grid, CELL_THREADS, smem_cell, st>>>(c->tmap_cta, Q);
+            else k_like<NF, MODE><<<grid, TP, smem, st>>>(c->tmap, Q);
+            if (prof) { cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING) + 1], st); c->prof_n++; }
+            c->launches++;
+        }
     }
     CK(cudaGetLastError());
     return CS_OK;
 }
 
 template <int MODE>
-int launch_like(cs_ctx *c, const LikeParams &P, int ngroup, cudaStream_t st) {
-    if (c->nfreq == 15) return launch_like_t<15, MODE>(c, P, ngroup, st);
-    return launch_like_t<16, MODE>(c, P, ngroup, st);
+int launch_like(cs_ctx *c, const LikeParams &P, int g0, int g1, int ncell, cudaStream_t st) {
+    if (c->nfreq == 15) return launch_like_t<15, MODE>(c, P, g0, g1, ncell, st);
+    return launch_like_t<16, MODE>(c, P, g0, g1, ncell, st);
 }
 
 LikeParams base_params(cs_ctx *c) {
@@ -328,6 +406,8 @@ int cs_create(cs_ctx **out, const cs_model *m) {
         delete c;
         return CS_ECUDA;
     }
+    const char *fd = std::getenv("CS_FORCE_DIRECT");
+    c->force_direct = fd && fd[0] == '1';
     *out = c;
     return CS_OK;
 }
@@ -392,9 +472,10 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     std::vector<MapDev> md(nmap + 1);
     for (int32_t m = 0; m <= nmap; ++m) {
         const MapHost &s = c->maps[m];
-        md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.ksegptr, s.kseglist, s.K, s.nseg};
+        md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.segslot, s.ksegptr, s.K, s.nseg};
     }
     c->cfgs.resize(ncfg);
+    c->cellplans.resize(ncfg);
     c->npix_live.assign((size_t)ncfg * nregion, 0);
     for (int32_t i = 0; i < ncfg; ++i) {
         CfgDev &cf = c->cfgs[i];
@@ -410,6 +491,17 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
                       *d = h.data() + (size_t)cf.map[2] * npix;
         for (int64_t p = 0; p < npix; ++p)
             if (a[p] >= 0 && b[p] >= 0 && d[p] >= 0) c->npix_live[(size_t)i * nregion + reg[p]]++;
+        // cell plan; a configuration with a tile of more than CELL_CAP distinct triples stays on the direct kernel
+        cf.cellid = nullptr; cf.cellptr = nullptr; cf.cellrows = nullptr; cf.ncell_max = 0; cf.pad = 0;
+        if (!c->force_direct) {
+            int32_t mx = 0;
+            rc = build_cell_plan(a, b, d, cf.K, npix, c->ntile, &c->cellplans[i], &mx, &c->cluster_bytes);
+            if (rc < 0) { free_clusters(c); return rc; }
+            if (rc == 0) {
+                cf.cellid = c->cellplans[i].cellid; cf.cellptr = c->cellplans[i].cellptr; cf.cellrows = c->cellplans[i].cellrows;
+                cf.ncell_max = std::max(mx, 1);
+            }
+        }
     }
     if ((rc = dev_upload(&c->d_maps, md, &c->cluster_bytes)) || (rc = dev_upload(&c->d_cfgs, c->cfgs, &c->cluster_bytes)) ||
         (rc = dev_upload(&c->d_npix_live, c->npix_live, &c->cluster_bytes))) {
@@ -434,6 +526,7 @@ int cs_set_data(cs_ctx *c, int32_t ndata, const float *d, const float *ninv) {
         c->kc.w[f] = w[f];
         c->kc.lnd[f] = (float)c->tc.lnd[f];
         c->kc.lnsw[f] = (float)(c->tc.lns[f] * (double)w[f]);
+        c->kc.lns[f] = (float)c->tc.lns[f];
         m00f += w[f];
     }
     (void)m00f;
@@ -476,12 +569,16 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     // entries grouped by configuration (stable), cut into groups of <= GROUP_MAX
     std::vector<int32_t> elist(batch);
     for (int32_t e = 0; e < batch; ++e) elist[e] = e;
-    std::stable_sort(elist.begin(), elist.end(), [&](int32_t a, int32_t b) { return cfg_of[a] < cfg_of[b]; });
+    // cell-path configurations first, then the direct ones; stable inside a configuration
+    auto key = [&](int32_t e) { return ((int64_t)(c->cfgs[cfg_of[e]].ncell_max > 0 ? 0 : 1) << 32) | (int64_t)cfg_of[e]; };
+    std::stable_sort(elist.begin(), elist.end(), [&](int32_t a, int32_t b) { return key(a) < key(b); });
     std::vector<Group> groups;
+    c->ngroup_cell = 0;
     for (int32_t i = 0; i < batch;) {
         int32_t j = i;
         while (j < batch && cfg_of[elist[j]] == cfg_of[elist[i]] && j - i < GROUP_MAX) ++j;
         groups.push_back(Group{cfg_of[elist[i]], i, j - i, 0});
+        if (c->cfgs[cfg_of[elist[i]]].ncell_max > 0) c->ngroup_cell = (int32_t)groups.size();
         i = j;
     }
     c->ngroup = (int32_t)groups.size();
@@ -542,7 +639,7 @@ int cs_spectral_like_grad(cs_ctx *c, double *nll, double *grad, void *stream) {
     if (!nll || !c->tables_built) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     LikeParams P = base_params(c);
-    rc = grad ? launch_like<MODE_GRAD>(c, P, c->ngroup, st) : launch_like<MODE_VALUE>(c, P, c->ngroup, st);
+    rc = grad ? launch_like<MODE_GRAD>(c, P, 0, c->ngroup, c->ngroup_cell, st) : launch_like<MODE_VALUE>(c, P, 0, c->ngroup, c->ngroup_cell, st);
     if (rc) return rc;
     return merge_launch(c, nll, grad, st);
 }
@@ -554,13 +651,21 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
     if (!entries && nsel != c->batch) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     std::vector<int32_t> el(nsel);
-    std::vector<Group> gr(nsel);
+    std::vector<Group> gr;
+    gr.reserve(nsel);
     for (int32_t i = 0; i < nsel; ++i) {
         const int32_t e = entries ? entries[i] : i;
         if (e < 0 || e >= c->batch) return CS_EINVAL;
         el[i] = e;
-        gr[i] = Group{c->cfg_of[e], i, 1, 0};
     }
+    // one group per selected entry (its start is the output slot); cell-path groups first
+    int32_t ncell = 0;
+    for (int pass = 0; pass < 2; ++pass)
+        for (int32_t i = 0; i < nsel; ++i) {
+            const bool cellp = c->cfgs[c->cfg_of[el[i]]].ncell_max > 0;
+            if (cellp == (pass == 0)) gr.push_back(Group{c->cfg_of[el[i]], i, 1, 0});
+            if (pass == 0 && cellp) ++ncell;
+        }
     // small synchronous uploads: map output is not on the optimizer's hot path
     CK(cudaStreamSynchronize(st));
     CK(cudaMemcpy(c->d_sel_elist, el.data(), sizeof(int32_t) * nsel, cudaMemcpyHostToDevice));
@@ -569,7 +674,7 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
     P.groups = c->d_sel_groups;
     P.elist = c->d_sel_elist;
     P.maps_out = s;
-    return launch_like<MODE_MAPS>(c, P, nsel, st);
+    return launch_like<MODE_MAPS>(c, P, 0, nsel, ncell, st);
 }
 
 int cs_cmb_variance(cs_ctx *c, double *var, void *stream) {
@@ -578,7 +683,7 @@ int cs_cmb_variance(cs_ctx *c, double *var, void *stream) {
     if (!var || !c->tables_built) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     LikeParams P = base_params(c);
-    if ((rc = launch_like<MODE_CMBVAR>(c, P, c->ngroup, st))) return rc;
+    if ((rc = launch_like<MODE_CMBVAR>(c, P, 0, c->ngroup, c->ngroup_cell, st))) return rc;
     const int n = c->batch * c->nregion;
     k_cmbvar<<<(n + 127) / 128, 128, 0, st>>>(c->d_partial, c->PS, c->d_maps, c->d_cfgs, c->d_cfg_of, c->d_npix_live,
                                              c->nregion, c->batch, var);
@@ -682,9 +787,7 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
             if (done[g] || gmax[g] >= n1) { ++g; continue; }
             int h = g;
             while (h < c->ngroup && !done[h] && gmax[h] < n1) { done[h] = 1; ++h; }
-            LikeParams Q = P;
-            Q.groups = c->d_groups + g;
-            rc = grad_host ? launch_like<MODE_GRAD>(c, Q, h - g, cm) : launch_like<MODE_VALUE>(c, Q, h - g, cm);
+            rc = grad_host ? launch_like<MODE_GRAD>(c, P, g, h, c->ngroup_cell, cm) : launch_like<MODE_VALUE>(c, P, g, h, c->ngroup_cell, cm);
             g = h;
         }
     }

@@ -1,0 +1,395 @@
+// cs_like_cell.cuh -- k_like_cell: the fused per-pixel kernel (a2 + first level of a3, a4, f1) in its "cell" form.
+//
+// Everything in Eq. 5/6/17 that depends only on the pixel's cluster triple (k0,k1,k2) -- the weighted columns
+// N^-1 a_d, N^-1 a_s, N^-1 da_d/dT, the matrix M = A^T N^-1 A, its LDL^T factors and the nine
+// contractions P_{theta,c} = sum_f w_f (da_f/dtheta) A_{f,c} -- is the same for all pixels of a tile that share the
+// triple (a "cell").  It is hoisted out of the pixel loop: per entry, builder warps evaluate it once per cell of
+// the tile into shared memory, and a pixel-eval is left with 12 dot products of length nfreq between its data
+// (Q, U) and six weighted columns, two 3x3 triangular solves and a handful of FMAs:
+//
+//     b_S  = A^T N^-1 d_S                        (3 dots per Stokes)            Eq. 5
+//     c_S  = (dA/dtheta)^T N^-1 d_S              (3 dots per Stokes)
+//     s_S  = M^-1 b_S  via the cell's LDL^T ;   ll = -1/2 sum_S b_S . s_S       Eq. 5, 6
+//     g_th = - sum_S s_{S,c(th)} ( c_{S,th} - sum_c P_{th,c} s_{S,c} )          Eq. 17 with r = d - A s expanded
+//
+// CTA = 16 warps, one CTA per SM, warp-specialised:
+//   warps 0-7    consumers: one pixel of the 256-pixel tile per thread, loop over the group's entries
+//   warps 8-10   builders : one cell per thread, fill the cell table of a later entry while earlier ones are consumed
+//   warps 11-14  reducers : first level of the ordered fp64 reduction (a3) of the terms the consumers leave behind,
+//                           one warp per entry in flight
+//   warp  15     loader   : one lane issues the TMA box [2*nfreq rows x 256 pixels] of every entry into a 4-deep ring
+// Every hand-over is an mbarrier pair (full/empty per ring slot): data ring, cell-table ring, term ring.  No role
+// ever waits at a CTA-wide barrier after the prologue.
+// shared memory: data ring [ND][2*NF][256] | cell tables [NC][CELL_CAP][CSTRIDE] | term ring [NT][4][TROW] |
+//                barriers | per-entry meta | segment plan
+#pragma once
+#include "cs_kernels.cuh"
+
+namespace cs {
+
+constexpr int ND = 3;        // data ring depth (entries in flight)
+constexpr int NBG = 2;       // builder groups: group g builds the entries i = g (mod NBG)
+constexpr int NC = 4;        // cell-table ring depth (a multiple of NBG)
+constexpr int NT = 4;        // term ring depth
+constexpr int NBUILD = NBG * CELL_CAP;           // builder threads (one per cell and group)
+constexpr int NRED = 128;                        // reducer threads
+constexpr int CELL_THREADS = TP + NBUILD + NRED + 32;   // 512
+static_assert(CELL_CAP % 32 == 0 && NC % NBG == 0, "builder warps / ring slots per group");
+
+// cell row layout (floats): for quad q = 0..3 (bands 4q..4q+3): [12q+0..3] w a_d, [12q+4..7] w a_s, [12q+8..11] w a_d dlnG
+// [48..63] scalars:
+constexpr int CS_L10 = 48, CS_L20 = 49, CS_L21 = 50, CS_ID1 = 51, CS_ID2 = 52, CS_P10 = 53, CS_P11 = 54, CS_P12 = 55,
+              CS_P20 = 56, CS_P21 = 57, CS_P22 = 58, CS_P30 = 59, CS_P31 = 60, CS_P32 = 61, CS_BAD = 62;
+
+template <int NF>
+constexpr size_t cell_smem_bytes() {
+    return (size_t)ND * 2 * NF * TP * 4               // data ring
+           + (size_t)NC * CELL_CAP * CSTRIDE * 4      // cell tables
+           + (size_t)NT * 4 * TROW * 4                // term ring
+           + (2 * ND + 2 * NC + 2 * NT) * 8           // mbarriers
+           + GROUP_MAX * 16                           // per-entry table base, data row, entry id
+           + 4 * TP * 2 + 4 * TP * 4                  // segment descriptors and output slots
+           + 16 * 4;                                  // meta
+}
+
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// First level of the ordered reduction (a3) of one entry by one reducer warp: one lane per (term, segment); a
+// segment is a contiguous run of <= SEG_MAX rank-ordered terms of one cluster.  It is summed in fp64 in a fixed
+// order -- four interleaved chains (elements j = 0,1,2,3 mod 4, ascending pixel order inside each) combined as
+// (a0 + a1) + (a2 + a3) -- and stored at the segment's cluster-major slot of the entry's partial row.
+__device__ __forceinline__ void reduce_entry(const float *tbuf, int lane, const int32_t *meta, const uint16_t *s_desc,
+                                             const int32_t *s_slot, double *__restrict__ prow) {
+    const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
+    const int c1 = n0, c2 = n0 + n1, c3 = n0 + n1 + n2, tot = c3 + n3;
+    for (int r = lane; r < tot; r += 32) {
+        const int t = (r >= c1) + (r >= c2) + (r >= c3);
+        const int ls = r - (t == 0 ? 0 : (t == 1 ? c1 : (t == 2 ? c2 : c3)));
+        const uint32_t desc = s_desc[t * TP + ls];
+        const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
+        const float *term = tbuf + t * TROW + start;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        int j = 0;
+        for (; j + 4 <= len; j += 4) {
+            a0 += (double)term[j]; a1 += (double)term[j + 1]; a2 += (double)term[j + 2]; a3 += (double)term[j + 3];
+        }
+        if (j < len) a0 += (double)term[j];
+        if (j + 1 < len) a1 += (double)term[j + 1];
+        if (j + 2 < len) a2 += (double)term[j + 2];
+        prow[s_slot[t * TP + ls]] = (a0 + a1) + (a2 + a3);
+    }
+}
+
+// The four table rows of a cell (Fd', G, dlnG, Fs'), loaded one entry ahead of their use.
+struct CellRows {
+    float4 Fd[4], G[4], dG[4], Fs[4];
+};
+template <bool GRAD>
+__device__ __forceinline__ void load_cell_rows(const float *__restrict__ tb, const int4 rows, CellRows &R) {
+    const float4 *rFd = reinterpret_cast<const float4 *>(tb + (int64_t)rows.x * NROW);
+    const float4 *rG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.y * NROW);
+    const float4 *rdG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.z * NROW);
+    const float4 *rFs = reinterpret_cast<const float4 *>(tb + (int64_t)rows.w * NROW);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        R.Fd[q] = __ldg(rFd + q); R.G[q] = __ldg(rG + q); R.Fs[q] = __ldg(rFs + q);
+        R.dG[q] = GRAD ? __ldg(rdG + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+// One cell (Eq. 2 columns -> weighted columns, M, LDL^T, P) from the entry's four table rows.
+template <bool GRAD>
+__device__ __forceinline__ void build_cell(const CellRows &R, const KConst &kc, float *__restrict__ out, int32_t *err) {
+    const float2 *w2 = reinterpret_cast<const float2 *>(kc.w);
+    const float2 *lnd2 = reinterpret_cast<const float2 *>(kc.lnd);
+    const float2 *lns2 = reinterpret_cast<const float2 *>(kc.lns);
+    const float4 *vFd = R.Fd, *vG = R.G, *vdG = R.dG, *vFs = R.Fs;
+    const float2 z = make_float2(0.f, 0.f);
+    float2 m01 = z, m02 = z, m11 = z, m12 = z, m22 = z;
+    float2 p10 = z, p11 = z, p12 = z, p20 = z, p21 = z, p22 = z, p30 = z, p31 = z, p32 = z;
+    float4 *o4 = reinterpret_cast<float4 *>(out);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        float2 wd[2], ws[2], u2[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int j = 2 * q + h;
+            const float2 Fd = h ? make_float2(vFd[q].z, vFd[q].w) : make_float2(vFd[q].x, vFd[q].y);
+            const float2 G = h ? make_float2(vG[q].z, vG[q].w) : make_float2(vG[q].x, vG[q].y);
+            const float2 dG = h ? make_float2(vdG[q].z, vdG[q].w) : make_float2(vdG[q].x, vdG[q].y);
+            const float2 as = h ? make_float2(vFs[q].z, vFs[q].w) : make_float2(vFs[q].x, vFs[q].y);
+            const float2 ad = mul2(Fd, G);                   // a_d = cd (nu/nu0)^beta_d * Planck ratio   (Eq. 2)
+            wd[h] = mul2(w2[j], ad);
+            ws[h] = mul2(w2[j], as);
+            m01 = add2(m01, wd[h]); m02 = add2(m02, ws[h]);
+            m11 = fma2(wd[h], ad, m11); m12 = fma2(wd[h], as, m12); m22 = fma2(ws[h], as, m22);
+            u2[h] = z;
+            if (GRAD) {
+                const float2 u1 = mul2(lnd2[j], wd[h]);      // w da_d/dbeta_d
+                u2[h] = mul2(dG, wd[h]);                     // w da_d/dT_d
+                const float2 u3 = mul2(lns2[j], ws[h]);      // w da_s/dbeta_s
+                p10 = add2(p10, u1); p11 = fma2(u1, ad, p11); p12 = fma2(u1, as, p12);
+                p20 = add2(p20, u2[h]); p21 = fma2(u2[h], ad, p21); p22 = fma2(u2[h], as, p22);
+                p30 = add2(p30, u3); p31 = fma2(u3, ad, p31); p32 = fma2(u3, as, p32);
+            }
+        }
+        o4[3 * q + 0] = make_float4(wd[0].x, wd[0].y, wd[1].x, wd[1].y);
+        o4[3 * q + 1] = make_float4(ws[0].x, ws[0].y, ws[1].x, ws[1].y);
+        if (GRAD) o4[3 * q + 2] = make_float4(u2[0].x, u2[0].y, u2[1].x, u2[1].y);
+    }
+    // LDL^T of M (m00 = sum_f w_f is a constant of the data set)
+    const float M01 = hsum(m01), M02 = hsum(m02), M11 = hsum(m11), M12 = hsum(m12), M22 = hsum(m22);
+    const float l10 = M01 * kc.inv_m00, l20 = M02 * kc.inv_m00;
+    const float d1 = fmaf(-l10, M01, M11);
+    const float t12 = fmaf(-l10, M02, M12);
+    const float id1 = fast_rcp(d1);
+    const float l21 = t12 * id1;
+    const float d2 = fmaf(-l21, t12, fmaf(-l20, M02, M22));
+    const float id2 = fast_rcp(d2);
+    const bool ok = (d1 > PIVOT_RTOL * M11) && (d2 > PIVOT_RTOL * M22);
+    if (!ok) atomicOr(err, ERR_SINGULAR);
+    o4[12] = make_float4(l10, l20, l21, id1);
+    o4[13] = make_float4(id2, hsum(p10), hsum(p11), hsum(p12));
+    o4[14] = make_float4(hsum(p20), hsum(p21), hsum(p22), hsum(p30));
+    o4[15] = make_float4(hsum(p31), hsum(p32), ok ? 0.f : 1.f, 0.f);
+}
+
+template <int NF, int MODE>
+__global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_constant__ CUtensorMap tmap, const LikeParams P) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int STAGE = 2 * NF * TP;   // floats per data stage
+    float *ring = reinterpret_cast<float *>(smem_raw);
+    float *cells = ring + ND * STAGE;
+    float *sterm = cells + NC * CELL_CAP * CSTRIDE;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sterm + NT * 4 * TROW);
+    uint64_t *full_d = bars, *empty_d = bars + ND, *full_c = bars + 2 * ND, *empty_c = bars + 2 * ND + NC;
+    uint64_t *full_t = bars + 2 * ND + 2 * NC, *empty_t = full_t + NT;
+    const float **s_tab = reinterpret_cast<const float **>(bars + 2 * ND + 2 * NC + 2 * NT);
+    int32_t *s_drow = reinterpret_cast<int32_t *>(s_tab + GROUP_MAX);
+    int32_t *s_ent = s_drow + GROUP_MAX;
+    uint16_t *s_desc = reinterpret_cast<uint16_t *>(s_ent + GROUP_MAX);
+    int32_t *s_slot = reinterpret_cast<int32_t *>(s_desc + 4 * TP);
+    int32_t *meta = s_slot + 4 * TP;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int tile = blockIdx.x;
+    const Group grp = P.groups[blockIdx.y];
+    const CfgDev cfg = P.cfgs[grp.cfg];
+    const int64_t npix = P.npix;
+    const int nrows = 2 * P.nfreq;
+    constexpr bool kReduce = (MODE != MODE_MAPS);
+    constexpr bool kGrad = (MODE == MODE_GRAD);
+
+    // ---------------- prologue (all threads) ----------------
+    if (tid == 0) {
+        for (int s = 0; s < ND; ++s) { mbar_init(&full_d[s], 1); mbar_init(&empty_d[s], TP / 32); }
+        for (int s = 0; s < NC; ++s) { mbar_init(&full_c[s], CELL_CAP / 32); mbar_init(&empty_c[s], TP / 32); }
+        for (int s = 0; s < NT; ++s) { mbar_init(&full_t[s], TP / 32); mbar_init(&empty_t[s], 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (tid < grp.count) {
+        const int e = P.elist[grp.start + tid];
+        s_ent[tid] = e;
+        s_drow[tid] = P.data_of[e] * nrows;
+        s_tab[tid] = P.tab + P.tab_off[e] * NROW;
+    }
+    if (kReduce && tid < TP) load_tile_plan<MODE>(P.maps, cfg, tile, tid, s_desc, s_slot, meta);
+    if (NF > 15 && P.nfreq < NF) {   // generic path: rows beyond nfreq are never copied; they must read as zero
+        for (int s = 0; s < ND; ++s)
+            for (int r = nrows * TP + tid; r < STAGE; r += CELL_THREADS) ring[s * STAGE + r] = 0.f;
+    }
+    __syncthreads();
+
+    if (warp == CELL_THREADS / 32 - 1) {
+        // ---------------- loader warp ----------------
+        const uint32_t box_bytes = (uint32_t)nrows * TP * 4u;
+        if (P.use_bulk) {
+            if (lane == 0) {
+                const uint64_t policy = P.evict_first ? policy_evict_first() : policy_evict_normal();
+                for (int i = 0; i < grp.count; ++i) {
+                    const int s = i % ND;
+                    mbar_wait_relaxed(&empty_d[s], (uint32_t)(((i / ND) & 1) ^ 1));
+                    mbar_expect_tx(&full_d[s], box_bytes);
+                    tma_box_g2s(ring + s * STAGE, &tmap, tile * TP, s_drow[i], &full_d[s], policy);
+                }
+            }
+        } else {   // rows not 16-byte aligned: plain loads by the whole warp
+            for (int i = 0; i < grp.count; ++i) {
+                const int s = i % ND;
+                mbar_wait_relaxed(&empty_d[s], (uint32_t)(((i / ND) & 1) ^ 1));
+                const int64_t row0 = s_drow[i];
+                for (int r = 0; r < nrows; ++r)
+                    for (int x = lane; x < TP; x += 32) {
+                        const int64_t px = (int64_t)tile * TP + x;
+                        ring[s * STAGE + r * TP + x] = (px < npix) ? P.d[(row0 + r) * npix + px] : 0.f;
+                    }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&full_d[s]);
+            }
+        }
+        return;
+    }
+    if (warp >= (TP + NBUILD) / 32) {
+        // ---------------- reducer warps: first level of a3, one entry behind the consumers ----------------
+        if (!kReduce) return;
+        // reducer warp r owns term-ring slot r and the entries i = r (mod NT)
+        static_assert(NRED / 32 == NT, "one reducer warp per term-ring slot");
+        const int s = warp - (TP + NBUILD) / 32;
+        for (int i = s; i < grp.count; i += NT) {
+            mbar_wait_relaxed(&full_t[s], (uint32_t)((i / NT) & 1));
+            reduce_entry(sterm + s * 4 * TROW, lane, meta, s_desc, s_slot, P.partial + (int64_t)s_ent[i] * P.PS);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_t[s]);
+        }
+        return;
+    }
+    if (warp >= TP / 32) {
+        // ---------------- builder warps: thread c builds cell c of this tile for every entry ----------------
+        const int g = (tid - TP) / CELL_CAP, c = (tid - TP) % CELL_CAP;
+        const int c0 = cfg.cellptr[tile], ncell = cfg.cellptr[tile + 1] - c0;
+        int4 rows = make_int4(0, 0, 0, 0);
+        if (c < ncell) rows = *reinterpret_cast<const int4 *>(cfg.cellrows + 4 * (int64_t)(c0 + c));
+        CellRows R;
+        if (c < ncell && g < grp.count) load_cell_rows<kGrad>(s_tab[g], rows, R);
+        for (int i = g; i < grp.count; i += NBG) {
+            const int s = i % NC;
+            mbar_wait_relaxed(&empty_c[s], (uint32_t)(((i / NC) & 1) ^ 1));
+            if (c < ncell) build_cell<kGrad>(R, P.kc, cells + (s * CELL_CAP + c) * CSTRIDE, P.err);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&full_c[s]);
+            if (c < ncell && i + NBG < grp.count) load_cell_rows<kGrad>(s_tab[i + NBG], rows, R);   // in flight during the next wait
+        }
+        return;
+    }
+
+    // ---------------- consumers ----------------
+    const int64_t p = (int64_t)tile * TP + tid;
+    int so0 = 0 * TROW + TP, so1 = 1 * TROW + TP, so2 = 2 * TROW + TP, so3 = 3 * TROW + TP;
+    int cid = 0xFF;
+    if (p < npix) {
+        cid = cfg.cellid[p];
+        if (kReduce) {
+            const int m3 = cfg.map[3];
+            if (MODE == MODE_CMBVAR) {
+                const int r = P.maps[m3].rank[p];
+                so0 = 0 * TROW + r; so1 = 1 * TROW + r; so2 = 2 * TROW + r; so3 = 3 * TROW + r;
+            } else {
+                if (kGrad) {   // a pixel masked in another map still owns a rank here: its slot must read 0
+                    if (P.maps[cfg.map[0]].idx[p] >= 0) so0 = 0 * TROW + P.maps[cfg.map[0]].rank[p];
+                    if (P.maps[cfg.map[1]].idx[p] >= 0) so1 = 1 * TROW + P.maps[cfg.map[1]].rank[p];
+                    if (P.maps[cfg.map[2]].idx[p] >= 0) so2 = 2 * TROW + P.maps[cfg.map[2]].rank[p];
+                }
+                so3 = 3 * TROW + P.maps[m3].rank[p];
+            }
+        }
+    }
+    const bool live = cid != 0xFF;
+    const float2 *w2 = reinterpret_cast<const float2 *>(P.kc.w);
+    const float2 *lnd2 = reinterpret_cast<const float2 *>(P.kc.lnd);
+    const float2 *lns2 = reinterpret_cast<const float2 *>(P.kc.lns);
+    const float inv_m00 = P.kc.inv_m00;
+
+    for (int i = 0; i < grp.count; ++i) {
+        const int sd = i % ND, sc = i % NC;
+        mbar_wait(&full_c[sc], (uint32_t)((i / NC) & 1));
+        mbar_wait(&full_d[sd], (uint32_t)((i / ND) & 1));
+        const float2 z = make_float2(0.f, 0.f);
+        float2 bq0 = z, bq1 = z, bq2 = z, bu0 = z, bu1 = z, bu2 = z;
+        float2 cq1 = z, cq2 = z, cq3 = z, cu1 = z, cu2 = z, cu3 = z;
+        float4 S0 = make_float4(0.f, 0.f, 0.f, 0.f), S1 = S0, S2 = S0, S3 = S0;
+        if (live) {
+            const float *st = ring + sd * STAGE + tid;
+            const float4 *cell = reinterpret_cast<const float4 *>(cells + (sc * CELL_CAP + cid) * CSTRIDE);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 WD = cell[3 * q], WS = cell[3 * q + 1];
+                float4 U2 = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (kGrad) U2 = cell[3 * q + 2];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int j = 2 * q + h;
+                    const float2 dq = make_float2(st[(4 * j + 0) * TP], (2 * j + 1 < NF) ? st[(4 * j + 2) * TP] : 0.f);
+                    const float2 du = make_float2(st[(4 * j + 1) * TP], (2 * j + 1 < NF) ? st[(4 * j + 3) * TP] : 0.f);
+                    const float2 wd = h ? make_float2(WD.z, WD.w) : make_float2(WD.x, WD.y);
+                    const float2 ws = h ? make_float2(WS.z, WS.w) : make_float2(WS.x, WS.y);
+                    bq0 = fma2(w2[j], dq, bq0); bq1 = fma2(wd, dq, bq1); bq2 = fma2(ws, dq, bq2);
+                    bu0 = fma2(w2[j], du, bu0); bu1 = fma2(wd, du, bu1); bu2 = fma2(ws, du, bu2);
+                    if (kGrad) {
+                        const float2 u2 = h ? make_float2(U2.z, U2.w) : make_float2(U2.x, U2.y);
+                        const float2 u1 = mul2(lnd2[j], wd), u3 = mul2(lns2[j], ws);
+                        cq1 = fma2(u1, dq, cq1); cq2 = fma2(u2, dq, cq2); cq3 = fma2(u3, dq, cq3);
+                        cu1 = fma2(u1, du, cu1); cu2 = fma2(u2, du, cu2); cu3 = fma2(u3, du, cu3);
+                    }
+                }
+            }
+            S0 = cell[12]; S1 = cell[13];
+            if (kGrad) S2 = cell[14];
+            S3 = cell[15];
+        }
+        __syncwarp();   // every lane has read its data and cell rows: hand both slots back
+        if (lane == 0) { mbar_arrive(&empty_d[sd]); mbar_arrive(&empty_c[sc]); }
+
+        float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
+        if (live) {
+            const float l10 = S0.x, l20 = S0.y, l21 = S0.z, id1 = S0.w, id2 = S1.x;
+            float sq[3], su[3], ll;
+            {
+                const float b0 = hsum(bq0), b1 = hsum(bq1), b2 = hsum(bq2);
+                const float y1 = fmaf(-l10, b0, b1);
+                const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
+                const float z0 = b0 * inv_m00, z1 = y1 * id1, z2 = y2 * id2;
+                sq[2] = z2; sq[1] = fmaf(-l21, z2, z1); sq[0] = fmaf(-l20, sq[2], fmaf(-l10, sq[1], z0));
+                ll = fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
+            }
+            {
+                const float b0 = hsum(bu0), b1 = hsum(bu1), b2 = hsum(bu2);
+                const float y1 = fmaf(-l10, b0, b1);
+                const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
+                const float z0 = b0 * inv_m00, z1 = y1 * id1, z2 = y2 * id2;
+                su[2] = z2; su[1] = fmaf(-l21, z2, z1); su[0] = fmaf(-l20, su[2], fmaf(-l10, su[1], z0));
+                ll += fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
+            }
+            ll *= -0.5f;                              // -1/2 sum_S b_S . s_S                    (Eq. 6)
+            if (S3.z != 0.f) ll = CUDART_INF_F;       // non-positive pivot in this cell's M
+            if (MODE == MODE_VALUE) {
+                t3 = ll;
+            } else if (MODE == MODE_GRAD) {
+                // g_theta = - sum_S s_{S,c} ( c_{S,theta} - P_theta . s_S )                      (Eq. 17)
+                const float P10 = S1.y, P11 = S1.z, P12 = S1.w, P20 = S2.x, P21 = S2.y, P22 = S2.z, P30 = S2.w, P31 = S3.x, P32 = S3.y;
+                const float eq1 = fmaf(-P12, sq[2], fmaf(-P11, sq[1], fmaf(-P10, sq[0], hsum(cq1))));
+                const float eu1 = fmaf(-P12, su[2], fmaf(-P11, su[1], fmaf(-P10, su[0], hsum(cu1))));
+                const float eq2 = fmaf(-P22, sq[2], fmaf(-P21, sq[1], fmaf(-P20, sq[0], hsum(cq2))));
+                const float eu2 = fmaf(-P22, su[2], fmaf(-P21, su[1], fmaf(-P20, su[0], hsum(cu2))));
+                const float eq3 = fmaf(-P32, sq[2], fmaf(-P31, sq[1], fmaf(-P30, sq[0], hsum(cq3))));
+                const float eu3 = fmaf(-P32, su[2], fmaf(-P31, su[1], fmaf(-P30, su[0], hsum(cu3))));
+                t0 = -fmaf(sq[1], eq1, su[1] * eu1);
+                t1 = -fmaf(sq[1], eq2, su[1] * eu2);
+                t2 = -fmaf(sq[2], eq3, su[2] * eu3);
+                t3 = ll;
+            } else if (MODE == MODE_CMBVAR) {
+                t0 = sq[0]; t1 = su[0]; t2 = sq[0] * sq[0]; t3 = su[0] * su[0];
+            } else {
+                float *o = P.maps_out + (int64_t)(grp.start + i) * 6 * npix + p;
+                o[0] = sq[0]; o[npix] = su[0]; o[2 * npix] = sq[1]; o[3 * npix] = su[1];
+                o[4 * npix] = sq[2]; o[5 * npix] = su[2];
+            }
+        } else if (MODE == MODE_MAPS && p < npix) {
+            float *o = P.maps_out + (int64_t)(grp.start + i) * 6 * npix + p;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) o[c * npix] = 0.f;
+        }
+        if (kReduce) {
+            const int st = i % NT;
+            mbar_wait(&empty_t[st], (uint32_t)(((i / NT) & 1) ^ 1));
+            float *tm = sterm + st * 4 * TROW;
+            if (MODE != MODE_VALUE) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
+            tm[so3] = t3;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&full_t[st]);
+        }
+    }
+}
+
+}  // namespace cs
