@@ -14,7 +14,8 @@
 //            segslot int32[nseg], ksegptr int32[K+1]
 //   cells    per clustering configuration (cell path only): the distinct (k0,k1,k2) triples of every tile in order of
 //            first appearance: cellid u8[ntile*TP] (0xFF = masked pixel), cellptr int32[ntile+1],
-//            cellrows int32[ncell][4] = table rows (Fd', G, dlnG, Fs') of the cell
+//            rowlist int32[nrow] = the distinct table rows a tile's cells read (rowptr int32[ntile+1]),
+//            cellrows int32[ncell][4] = slots of the cell's rows (Fd', G, dlnG, Fs') in its tile's row list
 #pragma once
 #include <stdint.h>
 
@@ -25,6 +26,9 @@ constexpr int SEG_MAX = 32;    // longest ordered chain summed by one thread in 
 constexpr int NROW = 16;       // floats per table row (nfreq padded to 16 -> 64-byte rows)
 constexpr int GROUP_MAX = 64;  // entries of one configuration handled by one CTA (per tile)
 constexpr int CELL_CAP = 96;   // cell path: most distinct cluster triples a tile may hold (else the direct kernel runs)
+constexpr int CHUNK_LEN = 8;   // cell kernel reduce: ranks summed by one lane in one step (SEG_MAX / CHUNK_LEN <= 4)
+constexpr int CHUNK_CAP = 416; // cell kernel reduce: most chunks (and segments) of the four terms of one tile
+constexpr int ROW_CAP = 128;   // cell path: most distinct table rows the cells of one tile may read
 constexpr int CSTRIDE = 68;    // floats per cell row in shared memory: 48 column values + 16 scalars + 4 pad (= 4 mod 32 banks)
 
 // A pivot of the LDL^T factorisation of M = A^T N^-1 A counts as non-positive (CS_ESINGULAR) when it is below this
@@ -42,6 +46,8 @@ struct MapDev {
     const uint16_t *segdesc;  // [nseg] start (8 bits) | (len-1) << 8
     const int32_t *segslot;   // [nseg] cluster-major slot of the segment inside its term's block of a partial row
     const int32_t *ksegptr;   // [K+1] CSR cluster -> slots [ksegptr[k], ksegptr[k+1])
+    const int32_t *chunkptr;  // [ntile+1] running count of <= CHUNK_LEN-rank chunks (each segment is cut into 1..4 of them)
+    const uint16_t *segcfirst;// [nseg] index of the segment's first chunk inside its tile's chunk list
     int32_t K;
     int32_t nseg;
 };
@@ -55,7 +61,9 @@ struct CfgDev {
     // cell plan (null / 0 when the configuration runs on the direct kernel)
     const uint8_t *cellid;     // [ntile*TP]
     const int32_t *cellptr;    // [ntile+1]
-    const int32_t *cellrows;   // [ncell][4]
+    const int32_t *cellrows;   // [ncell][4] tile-local row slots (Fd', G, dlnG, Fs') into the tile's row list
+    const int32_t *rowptr;     // [ntile+1]
+    const int32_t *rowlist;    // [nrow] distinct table rows (of an entry's table block) the tile's cells read
     int32_t ncell_max;         // most cells in one tile; 0 = direct path
     int32_t pad;
 };

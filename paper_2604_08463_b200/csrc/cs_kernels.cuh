@@ -69,7 +69,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
 }
 // Wait used by producer roles (loader, builders): they are ahead of the consumers most of the time, so the poll
 // backs off (suspend hint + nanosleep) instead of burning issue slots the consumers need.
-__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity, unsigned sleep_ns = 40) {
     uint32_t done = 0;
     while (true) {
         asm volatile(
@@ -80,7 +80,7 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity
             : "r"(smem_u32(bar)), "r"(parity), "r"(500u)
             : "memory");
         if (done) break;
-        __nanosleep(40);
+        __nanosleep(sleep_ns);
     }
 }
 // global -> shared bulk copy completing on an mbarrier; dst/src/bytes 16-byte aligned; evict-first L2 policy.
@@ -90,6 +90,11 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
             smem_u32(dst)),
         "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
         : "memory");
+}
+// Pulls the 64-byte table row at p towards L1 (no register is tied up while it is in flight).
+__device__ __forceinline__ void prefetch_row(const float *p) {
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p + 8));
 }
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
@@ -449,6 +454,11 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
             load_row(tb + r_fs, Fs);
 #pragma unroll
             for (int j = 0; j < NPAIR; ++j) ad[j] = mul2(Fd[j], G[j]);
+            if (i + 1 < grp.count) {   // next entry's rows on their way to L1 while this entry is computed
+                const float *tn = s_tab[i + 1];
+                prefetch_row(tn + r_fd); prefetch_row(tn + r_g); prefetch_row(tn + r_fs);
+                if (MODE == MODE_GRAD) prefetch_row(tn + r_dg);
+            }
         }
         PixelIn<NF> in;
         in.st = wring + s * 2 * NF * 32 + lane;

@@ -32,6 +32,9 @@ struct MapHost {
     uint16_t *segdesc = nullptr;
     int32_t *segslot = nullptr;
     int32_t *ksegptr = nullptr;
+    int32_t *chunkptr = nullptr;
+    uint16_t *segcfirst = nullptr;
+    std::vector<int32_t> h_chunkptr, h_segptr;   // host copies: per-tile counts decide a configuration's kernel
 };
 
 // Device arrays of one configuration's cell plan (empty when it runs on the direct kernel).
@@ -39,6 +42,8 @@ struct CellHost {
     uint8_t *cellid = nullptr;
     int32_t *cellptr = nullptr;
     int32_t *cellrows = nullptr;
+    int32_t *rowptr = nullptr;
+    int32_t *rowlist = nullptr;
 };
 
 template <typename T>
@@ -117,9 +122,10 @@ namespace {
 void free_clusters(cs_ctx *c) {
     for (auto &m : c->maps) {
         cudaFree(m.idx); cudaFree(m.rank); cudaFree(m.segptr); cudaFree(m.segdesc); cudaFree(m.segslot); cudaFree(m.ksegptr);
+        cudaFree(m.chunkptr); cudaFree(m.segcfirst);
     }
     c->maps.clear();
-    for (auto &p : c->cellplans) { cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); }
+    for (auto &p : c->cellplans) { cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); cudaFree(p.rowptr); cudaFree(p.rowlist); }
     c->cellplans.clear();
     cudaFree(c->d_maps); cudaFree(c->d_cfgs); cudaFree(c->d_npix_live);
     c->d_maps = nullptr; c->d_cfgs = nullptr; c->d_npix_live = nullptr;
@@ -167,6 +173,9 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     segcluster.reserve((size_t)ntile * 16);
     std::vector<std::pair<int32_t, int32_t>> tmp;
     std::vector<std::pair<uint16_t, int32_t>> tseg;   // (descriptor, cluster)
+    std::vector<int32_t> chunkptr(ntile + 1, 0);
+    std::vector<uint16_t> segcfirst;
+    int32_t nchunk = 0;
     tmp.reserve(TP);
     for (int32_t t = 0; t < ntile; ++t) {
         tmp.clear();
@@ -188,10 +197,18 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
         std::stable_sort(tseg.begin(), tseg.end(), [](const std::pair<uint16_t, int32_t> &a, const std::pair<uint16_t, int32_t> &b) {
             return (a.first >> 8) > (b.first >> 8);
         });
-        for (auto &sg : tseg) { segdesc.push_back(sg.first); segcluster.push_back(sg.second); }
+        chunkptr[t] = nchunk;
+        int32_t local = 0;
+        for (auto &sg : tseg) {
+            segdesc.push_back(sg.first); segcluster.push_back(sg.second);
+            segcfirst.push_back((uint16_t)local);
+            local += ((sg.first >> 8) + 1 + CHUNK_LEN - 1) / CHUNK_LEN;
+        }
+        nchunk += local;
         for (size_t q = 0; q < tmp.size(); ++q) rank[p0 + tmp[q].second] = (uint8_t)q;
     }
     segptr[ntile] = (int32_t)segdesc.size();
+    chunkptr[ntile] = nchunk;
     const int32_t nseg = (int32_t)segdesc.size();
     // cluster-major slots: the segments of cluster k occupy [ksegptr[k], ksegptr[k+1]) in ascending (tile, chunk) order
     std::vector<int32_t> ksegptr(K + 1, 0), segslot(nseg);
@@ -208,6 +225,9 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     if ((rc = dev_upload(&out->segdesc, segdesc, bytes))) return rc;
     if ((rc = dev_upload(&out->segslot, segslot, bytes))) return rc;
     if ((rc = dev_upload(&out->ksegptr, ksegptr, bytes))) return rc;
+    if ((rc = dev_upload(&out->chunkptr, chunkptr, bytes))) return rc;
+    if ((rc = dev_upload(&out->segcfirst, segcfirst, bytes))) return rc;
+    out->h_chunkptr = chunkptr; out->h_segptr = segptr;
     return CS_OK;
 }
 
@@ -218,7 +238,7 @@ int build_cell_plan(const int32_t *i0, const int32_t *i1, const int32_t *i2, con
                     CellHost *out, int32_t *ncell_max, int64_t *bytes) {
     std::vector<uint8_t> cellid((size_t)ntile * TP, 0xFF);
     std::vector<int32_t> cellptr(ntile + 1, 0);
-    std::vector<int32_t> rows;
+    std::vector<int32_t> rows, rowlist, rowptr(ntile + 1, 0);
     rows.reserve((size_t)ntile * 64 * 4);
     int32_t mx = 0;
     for (int32_t t = 0; t < ntile; ++t) {
@@ -247,13 +267,28 @@ int build_cell_plan(const int32_t *i0, const int32_t *i1, const int32_t *i2, con
             last = id;
         }
         mx = std::max(mx, n);
+        // the tile's distinct table rows; cells keep slots into this list (the loader stages the list per entry)
+        rowptr[t] = (int32_t)rowlist.size();
+        const size_t r0 = rowlist.size();
+        for (size_t q = 4 * base; q < rows.size(); ++q) {
+            size_t f = r0;
+            while (f < rowlist.size() && rowlist[f] != rows[q]) ++f;
+            if (f == rowlist.size()) {
+                if (rowlist.size() - r0 == (size_t)ROW_CAP) return 1;
+                rowlist.push_back(rows[q]);
+            }
+            rows[q] = (int32_t)(f - r0);
+        }
     }
+    rowptr[ntile] = (int32_t)rowlist.size();
     cellptr[ntile] = (int32_t)(rows.size() / 4);
     *ncell_max = mx;
     int rc;
     if ((rc = dev_upload(&out->cellid, cellid, bytes))) return rc;
     if ((rc = dev_upload(&out->cellptr, cellptr, bytes))) return rc;
     if ((rc = dev_upload(&out->cellrows, rows, bytes))) return rc;
+    if ((rc = dev_upload(&out->rowptr, rowptr, bytes))) return rc;
+    if ((rc = dev_upload(&out->rowlist, rowlist, bytes))) return rc;
     return CS_OK;
 }
 
@@ -472,7 +507,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     std::vector<MapDev> md(nmap + 1);
     for (int32_t m = 0; m <= nmap; ++m) {
         const MapHost &s = c->maps[m];
-        md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.segslot, s.ksegptr, s.K, s.nseg};
+        md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.segslot, s.ksegptr, s.chunkptr, s.segcfirst, s.K, s.nseg};
     }
     c->cfgs.resize(ncfg);
     c->cellplans.resize(ncfg);
@@ -492,13 +527,34 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
         for (int64_t p = 0; p < npix; ++p)
             if (a[p] >= 0 && b[p] >= 0 && d[p] >= 0) c->npix_live[(size_t)i * nregion + reg[p]]++;
         // cell plan; a configuration with a tile of more than CELL_CAP distinct triples stays on the direct kernel
-        cf.cellid = nullptr; cf.cellptr = nullptr; cf.cellrows = nullptr; cf.ncell_max = 0; cf.pad = 0;
+        cf.cellid = nullptr; cf.cellptr = nullptr; cf.cellrows = nullptr; cf.rowptr = nullptr; cf.rowlist = nullptr;
+        cf.ncell_max = 0; cf.pad = 0;
         if (!c->force_direct) {
             int32_t mx = 0;
             rc = build_cell_plan(a, b, d, cf.K, npix, c->ntile, &c->cellplans[i], &mx, &c->cluster_bytes);
             if (rc < 0) { free_clusters(c); return rc; }
+            if (rc == 0) {   // the reducer warps' plan must fit too
+                for (int32_t t = 0; t < c->ntile && rc == 0; ++t) {
+                    int32_t nc = 0, ns = 0;
+                    for (int q = 0; q < 4; ++q) {
+                        const MapHost &mh = c->maps[cf.map[q]];
+                        nc += mh.h_chunkptr[t + 1] - mh.h_chunkptr[t];
+                        ns += mh.h_segptr[t + 1] - mh.h_segptr[t];
+                    }
+                    // CMBVAR reduces all four terms over the region map
+                    const MapHost &mr = c->maps[cf.map[3]];
+                    nc = std::max(nc, 4 * (mr.h_chunkptr[t + 1] - mr.h_chunkptr[t]));
+                    if (nc > CHUNK_CAP || ns > CHUNK_CAP) rc = 1;
+                }
+                if (rc == 1) {
+                    cudaFree(c->cellplans[i].cellid); cudaFree(c->cellplans[i].cellptr); cudaFree(c->cellplans[i].cellrows);
+                    cudaFree(c->cellplans[i].rowptr); cudaFree(c->cellplans[i].rowlist);
+                    c->cellplans[i] = CellHost();
+                }
+            }
             if (rc == 0) {
                 cf.cellid = c->cellplans[i].cellid; cf.cellptr = c->cellplans[i].cellptr; cf.cellrows = c->cellplans[i].cellrows;
+                cf.rowptr = c->cellplans[i].rowptr; cf.rowlist = c->cellplans[i].rowlist;
                 cf.ncell_max = std::max(mx, 1);
             }
         }

@@ -17,7 +17,8 @@
 //   warps 8-10   builders : one cell per thread, fill the cell table of a later entry while earlier ones are consumed
 //   warps 11-14  reducers : first level of the ordered fp64 reduction (a3) of the terms the consumers leave behind,
 //                           one warp per entry in flight
-//   warp  15     loader   : one lane issues the TMA box [2*nfreq rows x 256 pixels] of every entry into a 4-deep ring
+//   warp  15     loader   : per entry, one TMA box [2*nfreq rows x 256 pixels] into the data ring and the distinct table
+//                           rows of the tile's cells (plain loads, one entry ahead) into the row ring
 // Every hand-over is an mbarrier pair (full/empty per ring slot): data ring, cell-table ring, term ring.  No role
 // ever waits at a CTA-wide barrier after the prologue.
 // shared memory: data ring [ND][2*NF][256] | cell tables [NC][CELL_CAP][CSTRIDE] | term ring [NT][4][TROW] |
@@ -27,14 +28,16 @@
 
 namespace cs {
 
-constexpr int ND = 3;        // data ring depth (entries in flight)
-constexpr int NBG = 2;       // builder groups: group g builds the entries i = g (mod NBG)
-constexpr int NC = 4;        // cell-table ring depth (a multiple of NBG)
+constexpr int NR = 3;        // table-row ring depth
+template <int NF>
+struct DataDepth { static constexpr int value = (NF == 15) ? 3 : 2; };   // data ring depth (entries in flight)
+constexpr int NBG = 1;       // builder groups: group g builds the entries i = g (mod NBG)
+constexpr int NC = 3;        // cell-table ring depth (a multiple of NBG)
 constexpr int NT = 4;        // term ring depth
 constexpr int NBUILD = NBG * CELL_CAP;           // builder threads (one per cell and group)
 constexpr int NRED = 128;                        // reducer threads
 constexpr int CELL_THREADS = TP + NBUILD + NRED + 32;   // 512
-static_assert(CELL_CAP % 32 == 0 && NC % NBG == 0, "builder warps / ring slots per group");
+static_assert(SEG_MAX <= 4 * CHUNK_LEN && CELL_CAP % 32 == 0 && NC % NBG == 0, "builder warps / ring slots per group");
 
 // cell row layout (floats): for quad q = 0..3 (bands 4q..4q+3): [12q+0..3] w a_d, [12q+4..7] w a_s, [12q+8..11] w a_d dlnG
 // [48..63] scalars:
@@ -43,12 +46,15 @@ constexpr int CS_L10 = 48, CS_L20 = 49, CS_L21 = 50, CS_ID1 = 51, CS_ID2 = 52, C
 
 template <int NF>
 constexpr size_t cell_smem_bytes() {
+    constexpr int ND = DataDepth<NF>::value;
     return (size_t)ND * 2 * NF * TP * 4               // data ring
+           + (size_t)NR * ROW_CAP * NROW * 4          // table rows of the tile's cells, staged per entry
            + (size_t)NC * CELL_CAP * CSTRIDE * 4      // cell tables
            + (size_t)NT * 4 * TROW * 4                // term ring
-           + (2 * ND + 2 * NC + 2 * NT) * 8           // mbarriers
+           + (size_t)NT * CHUNK_CAP * 8               // chunk sums of the reducer warps (fp64)
+           + (2 * ND + 2 * NC + 2 * NT + 2 * NR) * 8  // mbarriers
            + GROUP_MAX * 16                           // per-entry table base, data row, entry id
-           + 4 * TP * 2 + 4 * TP * 4                  // segment descriptors and output slots
+           + CHUNK_CAP * (2 + 2 + 4)                  // chunk descriptors, segment descriptors, output slots
            + 16 * 4;                                  // meta
 }
 
@@ -56,30 +62,65 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-// First level of the ordered reduction (a3) of one entry by one reducer warp: one lane per (term, segment); a
-// segment is a contiguous run of <= SEG_MAX rank-ordered terms of one cluster.  It is summed in fp64 in a fixed
-// order -- four interleaved chains (elements j = 0,1,2,3 mod 4, ascending pixel order inside each) combined as
-// (a0 + a1) + (a2 + a3) -- and stored at the segment's cluster-major slot of the entry's partial row.
-__device__ __forceinline__ void reduce_entry(const float *tbuf, int lane, const int32_t *meta, const uint16_t *s_desc,
-                                             const int32_t *s_slot, double *__restrict__ prow) {
-    const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
-    const int c1 = n0, c2 = n0 + n1, c3 = n0 + n1 + n2, tot = c3 + n3;
-    for (int r = lane; r < tot; r += 32) {
-        const int t = (r >= c1) + (r >= c2) + (r >= c3);
-        const int ls = r - (t == 0 ? 0 : (t == 1 ? c1 : (t == 2 ? c2 : c3)));
-        const uint32_t desc = s_desc[t * TP + ls];
-        const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
-        const float *term = tbuf + t * TROW + start;
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        int j = 0;
-        for (; j + 4 <= len; j += 4) {
-            a0 += (double)term[j]; a1 += (double)term[j + 1]; a2 += (double)term[j + 2]; a3 += (double)term[j + 3];
+// Reducer plan of a tile in shared memory: every (term, cluster) segment of <= SEG_MAX rank-ordered terms is cut into
+// 1..4 chunks of <= CHUNK_LEN ranks.  s_cdesc[chunk] = start | (len-1) << 8 | term << 11;
+// s_sdesc[segment] = first chunk | (chunks-1) << 12; s_slot[segment] = cluster-major slot in the entry's partial row.
+template <int MODE>
+__device__ __forceinline__ void load_chunk_plan(const MapDev *__restrict__ maps, const CfgDev &cfg, int tile, int tid,
+                                                uint16_t *s_cdesc, uint16_t *s_sdesc, int32_t *s_slot, int32_t *meta) {
+    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;
+    int sbase = 0, cbase = 0;
+#pragma unroll
+    for (int t = T0; t < 4; ++t) {
+        const MapDev m = maps[(MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t]];
+        const int s0 = m.segptr[tile], ns = m.segptr[tile + 1] - s0;
+        const int nc = m.chunkptr[tile + 1] - m.chunkptr[tile];
+        if (tid < ns) {
+            const uint32_t desc = m.segdesc[s0 + tid];
+            const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
+            const int first = cbase + m.segcfirst[s0 + tid], cnt = (len + CHUNK_LEN - 1) / CHUNK_LEN;
+            s_sdesc[sbase + tid] = (uint16_t)(first | ((cnt - 1) << 12));
+            s_slot[sbase + tid] = ((MODE == MODE_CMBVAR) ? t * m.nseg : cfg.segbase[t]) + m.segslot[s0 + tid];
+            for (int q = 0; q < cnt; ++q) {
+                const int l = min(CHUNK_LEN, len - CHUNK_LEN * q);
+                s_cdesc[first + q] = (uint16_t)((start + CHUNK_LEN * q) | ((l - 1) << 8) | (t << 11));
+            }
         }
-        if (j < len) a0 += (double)term[j];
-        if (j + 1 < len) a1 += (double)term[j + 1];
-        if (j + 2 < len) a2 += (double)term[j + 2];
-        prow[s_slot[t * TP + ls]] = (a0 + a1) + (a2 + a3);
+        sbase += ns; cbase += nc;
     }
+    if (tid == 0) { meta[0] = cbase; meta[1] = sbase; }
+}
+
+// First level of the ordered reduction (a3) of one entry by one reducer warp, in fp64 and in a fixed order:
+// step 1, one lane per chunk: (x0 + x4) + (x1 + x5) paired with (x2 + x6) + (x3 + x7) over the chunk's <= 8 ranks
+// (ascending pixel order), straight-line so that the lanes do not diverge; step 2, one lane per segment: the
+// segment's chunk sums left to right, stored at the segment's cluster-major slot of the entry's partial row.
+__device__ __forceinline__ void reduce_entry(const float *tbuf, int lane, const int32_t *meta, const uint16_t *s_cdesc,
+                                             const uint16_t *s_sdesc, const int32_t *s_slot, double *csum,
+                                             double *__restrict__ prow) {
+    const int nchunk = meta[0], nseg = meta[1];
+    for (int r = lane; r < nchunk; r += 32) {
+        const uint32_t d = s_cdesc[r];
+        const int start = d & 0xff, len = (int)((d >> 8) & 7) + 1, t = (int)(d >> 11);
+        const float *term = tbuf + t * TROW + start;
+        float x[CHUNK_LEN];
+#pragma unroll
+        for (int j = 0; j < CHUNK_LEN; ++j) x[j] = (j < len) ? term[j] : 0.f;
+        const double a0 = (double)x[0] + (double)x[4], a1 = (double)x[1] + (double)x[5];
+        const double a2 = (double)x[2] + (double)x[6], a3 = (double)x[3] + (double)x[7];
+        csum[r] = (a0 + a1) + (a2 + a3);
+    }
+    __syncwarp();
+    for (int r = lane; r < nseg; r += 32) {
+        const uint32_t d = s_sdesc[r];
+        const int first = d & 0xfff, cnt = (int)(d >> 12) + 1;
+        double acc = csum[first];
+        if (cnt > 1) acc += csum[first + 1];
+        if (cnt > 2) acc += csum[first + 2];
+        if (cnt > 3) acc += csum[first + 3];
+        prow[s_slot[r]] = acc;
+    }
+    __syncwarp();
 }
 
 // The four table rows of a cell (Fd', G, dlnG, Fs'), loaded one entry ahead of their use.
@@ -87,15 +128,15 @@ struct CellRows {
     float4 Fd[4], G[4], dG[4], Fs[4];
 };
 template <bool GRAD>
-__device__ __forceinline__ void load_cell_rows(const float *__restrict__ tb, const int4 rows, CellRows &R) {
-    const float4 *rFd = reinterpret_cast<const float4 *>(tb + (int64_t)rows.x * NROW);
-    const float4 *rG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.y * NROW);
-    const float4 *rdG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.z * NROW);
-    const float4 *rFs = reinterpret_cast<const float4 *>(tb + (int64_t)rows.w * NROW);
+__device__ __forceinline__ void load_cell_rows(const float *tb, const int4 rows, CellRows &R) {   // tb: staged rows (smem)
+    const float4 *rFd = reinterpret_cast<const float4 *>(tb + rows.x * NROW);
+    const float4 *rG = reinterpret_cast<const float4 *>(tb + rows.y * NROW);
+    const float4 *rdG = reinterpret_cast<const float4 *>(tb + rows.z * NROW);
+    const float4 *rFs = reinterpret_cast<const float4 *>(tb + rows.w * NROW);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-        R.Fd[q] = __ldg(rFd + q); R.G[q] = __ldg(rG + q); R.Fs[q] = __ldg(rFs + q);
-        R.dG[q] = GRAD ? __ldg(rdG + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+        R.Fd[q] = rFd[q]; R.G[q] = rG[q]; R.Fs[q] = rFs[q];
+        R.dG[q] = GRAD ? rdG[q] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
 
@@ -160,18 +201,23 @@ template <int NF, int MODE>
 __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_constant__ CUtensorMap tmap, const LikeParams P) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     constexpr int STAGE = 2 * NF * TP;   // floats per data stage
+    constexpr int ND = DataDepth<NF>::value;
     float *ring = reinterpret_cast<float *>(smem_raw);
-    float *cells = ring + ND * STAGE;
+    float *rowbuf = ring + ND * STAGE;
+    float *cells = rowbuf + NR * ROW_CAP * NROW;
     float *sterm = cells + NC * CELL_CAP * CSTRIDE;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(sterm + NT * 4 * TROW);
+    double *csum = reinterpret_cast<double *>(sterm + NT * 4 * TROW);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(csum + NT * CHUNK_CAP);
     uint64_t *full_d = bars, *empty_d = bars + ND, *full_c = bars + 2 * ND, *empty_c = bars + 2 * ND + NC;
     uint64_t *full_t = bars + 2 * ND + 2 * NC, *empty_t = full_t + NT;
-    const float **s_tab = reinterpret_cast<const float **>(bars + 2 * ND + 2 * NC + 2 * NT);
+    uint64_t *full_r = empty_t + NT, *empty_r = full_r + NR;
+    const float **s_tab = reinterpret_cast<const float **>(empty_r + NR);
     int32_t *s_drow = reinterpret_cast<int32_t *>(s_tab + GROUP_MAX);
     int32_t *s_ent = s_drow + GROUP_MAX;
-    uint16_t *s_desc = reinterpret_cast<uint16_t *>(s_ent + GROUP_MAX);
-    int32_t *s_slot = reinterpret_cast<int32_t *>(s_desc + 4 * TP);
-    int32_t *meta = s_slot + 4 * TP;
+    int32_t *s_slot = s_ent + GROUP_MAX;
+    int32_t *meta = s_slot + CHUNK_CAP;
+    uint16_t *s_cdesc = reinterpret_cast<uint16_t *>(meta + 16);
+    uint16_t *s_sdesc = s_cdesc + CHUNK_CAP;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int tile = blockIdx.x;
@@ -187,6 +233,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         for (int s = 0; s < ND; ++s) { mbar_init(&full_d[s], 1); mbar_init(&empty_d[s], TP / 32); }
         for (int s = 0; s < NC; ++s) { mbar_init(&full_c[s], CELL_CAP / 32); mbar_init(&empty_c[s], TP / 32); }
         for (int s = 0; s < NT; ++s) { mbar_init(&full_t[s], TP / 32); mbar_init(&empty_t[s], 1); }
+        for (int s = 0; s < NR; ++s) { mbar_init(&full_r[s], 1); mbar_init(&empty_r[s], NBUILD / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid < grp.count) {
@@ -195,7 +242,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         s_drow[tid] = P.data_of[e] * nrows;
         s_tab[tid] = P.tab + P.tab_off[e] * NROW;
     }
-    if (kReduce && tid < TP) load_tile_plan<MODE>(P.maps, cfg, tile, tid, s_desc, s_slot, meta);
+    if (kReduce && tid < TP) load_chunk_plan<MODE>(P.maps, cfg, tile, tid, s_cdesc, s_sdesc, s_slot, meta);
     if (NF > 15 && P.nfreq < NF) {   // generic path: rows beyond nfreq are never copied; they must read as zero
         for (int s = 0; s < ND; ++s)
             for (int r = nrows * TP + tid; r < STAGE; r += CELL_THREADS) ring[s * STAGE + r] = 0.f;
@@ -204,21 +251,45 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
 
     if (warp == CELL_THREADS / 32 - 1) {
         // ---------------- loader warp ----------------
+        // per entry: (1) the distinct table rows this tile's cells read, loaded one entry ahead by all lanes, into the
+        // row ring; (2) the data box into the data ring (one TMA by lane 0, or plain loads when rows of d are not
+        // 16-byte aligned)
         const uint32_t box_bytes = (uint32_t)nrows * TP * 4u;
-        if (P.use_bulk) {
-            if (lane == 0) {
-                const uint64_t policy = P.evict_first ? policy_evict_first() : policy_evict_normal();
-                for (int i = 0; i < grp.count; ++i) {
-                    const int s = i % ND;
-                    mbar_wait_relaxed(&empty_d[s], (uint32_t)(((i / ND) & 1) ^ 1));
+        const int r0 = cfg.rowptr[tile], nrow = cfg.rowptr[tile + 1] - r0;
+        constexpr int NQ = ROW_CAP * 4 / 32;   // float4 quarters of rows per lane
+        int myoff[NQ];                         // float offset of this lane's k-th quarter inside an entry's table block
+#pragma unroll
+        for (int k = 0; k < NQ; ++k) {
+            const int q = lane + 32 * k;       // quarter q = row (q >> 2), part (q & 3)
+            myoff[k] = (q < 4 * nrow) ? cfg.rowlist[r0 + (q >> 2)] * NROW + (q & 3) * 4 : -1;
+        }
+        float4 v[NQ];
+        auto fetch = [&](int i) {
+            const float *tb = s_tab[i];
+#pragma unroll
+            for (int k = 0; k < NQ; ++k)
+                if (myoff[k] >= 0) v[k] = __ldg(reinterpret_cast<const float4 *>(tb + myoff[k]));
+        };
+        const uint64_t policy = P.evict_first ? policy_evict_first() : policy_evict_normal();
+        fetch(0);
+        for (int i = 0; i < grp.count; ++i) {
+            const int sr = i % NR, s = i % ND;
+            mbar_wait_relaxed(&empty_r[sr], (uint32_t)(((i / NR) & 1) ^ 1), 250);
+            float4 *dst = reinterpret_cast<float4 *>(rowbuf + sr * ROW_CAP * NROW);
+#pragma unroll
+            for (int k = 0; k < NQ; ++k)
+                if (myoff[k] >= 0) dst[lane + 32 * k] = v[k];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&full_r[sr]);
+            if (i + 1 < grp.count) fetch(i + 1);   // in flight while lane 0 waits for a data slot
+            if (P.use_bulk) {
+                if (lane == 0) {
+                    mbar_wait_relaxed(&empty_d[s], (uint32_t)(((i / ND) & 1) ^ 1), 250);
                     mbar_expect_tx(&full_d[s], box_bytes);
                     tma_box_g2s(ring + s * STAGE, &tmap, tile * TP, s_drow[i], &full_d[s], policy);
                 }
-            }
-        } else {   // rows not 16-byte aligned: plain loads by the whole warp
-            for (int i = 0; i < grp.count; ++i) {
-                const int s = i % ND;
-                mbar_wait_relaxed(&empty_d[s], (uint32_t)(((i / ND) & 1) ^ 1));
+            } else {   // rows of d not 16-byte aligned: plain loads by the whole warp
+                mbar_wait_relaxed(&empty_d[s], (uint32_t)(((i / ND) & 1) ^ 1), 250);
                 const int64_t row0 = s_drow[i];
                 for (int r = 0; r < nrows; ++r)
                     for (int x = lane; x < TP; x += 32) {
@@ -238,8 +309,9 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         static_assert(NRED / 32 == NT, "one reducer warp per term-ring slot");
         const int s = warp - (TP + NBUILD) / 32;
         for (int i = s; i < grp.count; i += NT) {
-            mbar_wait_relaxed(&full_t[s], (uint32_t)((i / NT) & 1));
-            reduce_entry(sterm + s * 4 * TROW, lane, meta, s_desc, s_slot, P.partial + (int64_t)s_ent[i] * P.PS);
+            mbar_wait_relaxed(&full_t[s], (uint32_t)((i / NT) & 1), 150);
+            reduce_entry(sterm + s * 4 * TROW, lane, meta, s_cdesc, s_sdesc, s_slot, csum + s * CHUNK_CAP,
+                         P.partial + (int64_t)s_ent[i] * P.PS);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_t[s]);
         }
@@ -251,15 +323,17 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         const int c0 = cfg.cellptr[tile], ncell = cfg.cellptr[tile + 1] - c0;
         int4 rows = make_int4(0, 0, 0, 0);
         if (c < ncell) rows = *reinterpret_cast<const int4 *>(cfg.cellrows + 4 * (int64_t)(c0 + c));
-        CellRows R;
-        if (c < ncell && g < grp.count) load_cell_rows<kGrad>(s_tab[g], rows, R);
         for (int i = g; i < grp.count; i += NBG) {
-            const int s = i % NC;
+            const int s = i % NC, sr = i % NR;
+            CellRows R;
+            mbar_wait_relaxed(&full_r[sr], (uint32_t)((i / NR) & 1));
+            if (c < ncell) load_cell_rows<kGrad>(rowbuf + sr * ROW_CAP * NROW, rows, R);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_r[sr]);
             mbar_wait_relaxed(&empty_c[s], (uint32_t)(((i / NC) & 1) ^ 1));
             if (c < ncell) build_cell<kGrad>(R, P.kc, cells + (s * CELL_CAP + c) * CSTRIDE, P.err);
             __syncwarp();
             if (lane == 0) mbar_arrive(&full_c[s]);
-            if (c < ncell && i + NBG < grp.count) load_cell_rows<kGrad>(s_tab[i + NBG], rows, R);   // in flight during the next wait
         }
         return;
     }
