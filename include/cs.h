@@ -77,6 +77,9 @@ typedef struct cs_opt {
     double beta1, beta2, eps;
     double ls_c1;       /* Armijo constant */
     double safe_lo, safe_hi; /* dynamic rescale range for |g_proj| (A4, L541) */
+    double ls_noise;    /* Armijo slack, relative to |L|: accept when L_trial <= L + ls_c1 a g.d + ls_noise |L|.  The
+                           per-pixel likelihood is fp32, so differences of the objective below ~3e-8 |L| are evaluation
+                           noise; 0 = strict decrease of the computed objective (R13) */
 } cs_opt;
 
 /* Create a context for `model`.  Allocates only small constant tables.  *out is NULL on failure. */

@@ -116,7 +116,8 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
                                                 int32_t *err, const TConst tc) {
     const int f = threadIdx.x;   // 0..15
     for (int e = blockIdx.y; e < batch; e += gridDim.y) {
-        const CfgDev c = cfgs[cfg_of[e]];
+        const CfgDev *cp = cfgs + cfg_of[e];
+        struct { int32_t K[3]; int32_t ktot; } c = {{cp->K[0], cp->K[1], cp->K[2]}, cp->ktot};   // only these fields
         const int j = blockIdx.x * blockDim.y + threadIdx.y;
         if (j >= c.ktot) continue;
         const double x = params[param_off[e] + j];
@@ -520,30 +521,41 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
 // ----------------------------------------------------------------------------------------------------------
 // a3 second level: grad[e][j] / nll[e][r] = fixed-order (ascending tile) sum over the segments of cluster j / region r,
 // which are contiguous in the partial row.
-// grid = (ceil(nout_max/256), batch).  want_grad = 0: only the region outputs.
+// want_grad = 0: only the region outputs.
 // ----------------------------------------------------------------------------------------------------------
+// One warp per output: lane l adds the slots a+l, a+l+32, ... in ascending order, then the 32 lane sums are combined
+// by a fixed xor-shuffle tree, so the result is bitwise reproducible.  grid = (ceil(nout_max/8), batch), 256 threads.
+__device__ __forceinline__ double warp_sum_fixed(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
 __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
                                                const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
                                                const int64_t *__restrict__ param_off, int32_t nregion, int32_t want_grad,
                                                double *__restrict__ nll, double *__restrict__ grad) {
-    const int e = blockIdx.y;
-    const CfgDev c = cfgs[cfg_of[e]];
-    const int nout = (want_grad ? c.ktot : 0) + nregion;
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int e = blockIdx.y, lane = threadIdx.x & 31;
+    const CfgDev *c = cfgs + cfg_of[e];
+    const int K0 = c->K[0], K1 = c->K[1], ktot = c->ktot;
+    const int nout = (want_grad ? ktot : 0) + nregion;
+    const int j = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (j >= nout) return;
     int t, k;
     if (!want_grad) { t = 3; k = j; }
-    else if (j < c.K[0]) { t = 0; k = j; }
-    else if (j < c.K[0] + c.K[1]) { t = 1; k = j - c.K[0]; }
-    else if (j < c.ktot) { t = 2; k = j - c.K[0] - c.K[1]; }
-    else { t = 3; k = j - c.ktot; }
-    const MapDev m = maps[c.map[t]];
-    const double *row = partial + (int64_t)e * PS + c.segbase[t];
+    else if (j < K0) { t = 0; k = j; }
+    else if (j < K0 + K1) { t = 1; k = j - K0; }
+    else if (j < ktot) { t = 2; k = j - K0 - K1; }
+    else { t = 3; k = j - ktot; }
+    const int32_t *ksegptr = maps[c->map[t]].ksegptr;
+    const double *row = partial + (int64_t)e * PS + c->segbase[t];
     double acc = 0.0;
-    const int a = m.ksegptr[k], b = m.ksegptr[k + 1];
-    for (int q = a; q < b; ++q) acc += row[q];
-    if (t == 3) nll[(int64_t)e * nregion + k] = acc;
-    else grad[param_off[e] + j] = acc;
+    const int a = ksegptr[k], b = ksegptr[k + 1];
+    for (int q = a + lane; q < b; q += 32) acc += row[q];
+    acc = warp_sum_fixed(acc);
+    if (lane == 0) {
+        if (t == 3) nll[(int64_t)e * nregion + k] = acc;
+        else grad[param_off[e] + j] = acc;
+    }
 }
 
 // f1 (Eq. 10): variance of the CMB map per entry and region from the four region-reduced sums.
@@ -554,13 +566,14 @@ __global__ void __launch_bounds__(128) k_cmbvar(const double *__restrict__ parti
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= batch * nregion) return;
     const int e = i / nregion, r = i - e * nregion;
-    const CfgDev c = cfgs[cfg_of[e]];
-    const MapDev m = maps[c.map[3]];
+    const MapDev *m = maps + cfgs[cfg_of[e]].map[3];
+    const int32_t *ksegptr = m->ksegptr;
+    const int32_t nseg = m->nseg;
     double s[4];
     for (int t = 0; t < 4; ++t) {
-        const double *row = partial + (int64_t)e * PS + (int64_t)t * m.nseg;
+        const double *row = partial + (int64_t)e * PS + (int64_t)t * nseg;
         double acc = 0.0;
-        for (int q = m.ksegptr[r]; q < m.ksegptr[r + 1]; ++q) acc += row[q];
+        for (int q = ksegptr[r]; q < ksegptr[r + 1]; ++q) acc += row[q];
         s[t] = acc;
     }
     const double n = (double)npix_live[cfg_of[e] * nregion + r];

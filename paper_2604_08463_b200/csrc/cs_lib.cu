@@ -680,7 +680,7 @@ static int merge_launch(cs_ctx *c, double *nll, double *grad, cudaStream_t st) {
     for (int e0 = 0; e0 < c->batch; e0 += 65535) {
         const int nb = std::min(65535, c->batch - e0);
         const int nout = (grad ? c->ktot_max : 0) + c->nregion;
-        dim3 grid((nout + 255) / 256, nb);
+        dim3 grid((nout + 7) / 8, nb);
         k_merge<<<grid, 256, 0, st>>>(c->d_partial + (int64_t)e0 * c->PS, c->PS, c->d_maps, c->d_cfgs, c->d_cfg_of + e0,
                                      c->d_param_off + e0, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad);
         c->launches++;
@@ -752,20 +752,20 @@ void cs_opt_defaults(cs_opt *o) {
     if (!o) return;
     o->iters = 200; o->ls_max = 8;
     o->lr = 0.02; o->beta1 = 0.9; o->beta2 = 0.999; o->eps = 1e-16;
-    o->ls_c1 = 1e-4; o->safe_lo = 1e-15; o->safe_hi = 1e15;
+    o->ls_c1 = 1e-4; o->safe_lo = 1e-15; o->safe_hi = 1e15; o->ls_noise = 3e-8;
 }
 
 int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *upper, const cs_opt *opt, double *nll_final,
                 void *stream) {
     int rc = ready(c);
     if (rc) return rc;
-    if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || c->batch > 65535) return CS_EINVAL;
+    if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || !(opt->ls_noise >= 0) || c->batch > 65535) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     if (!c->opt.y) {
         if ((rc = opt_alloc(c->opt, c->nparam, c->batch, c->nregion, &c->opt_bytes))) return rc == 1 ? CS_ENOMEM : CS_ECUDA;
     }
     OptShape sh{c->nparam, c->batch, c->nregion, c->ktot_max, c->d_param_off};
-    OptHyper hy{opt->lr, opt->beta1, opt->beta2, opt->eps, opt->ls_c1, opt->safe_lo, opt->safe_hi, opt->ls_max};
+    OptHyper hy{opt->lr, opt->beta1, opt->beta2, opt->eps, opt->ls_c1, opt->safe_lo, opt->safe_hi, opt->ls_noise, opt->ls_max};
     OptWork &w = c->opt;
     opt_init(w, sh, params, lower, upper, st); c->launches += 1;
     for (int it = 0; it < opt->iters; ++it) {

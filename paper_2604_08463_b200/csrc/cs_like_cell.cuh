@@ -58,6 +58,13 @@ constexpr size_t cell_smem_bytes() {
            + 16 * 4;                                  // meta
 }
 
+// Term-ring "full" hand-over on hardware named barriers 1..NT (consumers arrive, the slot's reducer warp syncs): a
+// warp blocked in bar.sync takes no issue slots, unlike a polling mbarrier wait.
+__device__ __forceinline__ void terms_arrive(int slot) {
+    __threadfence_block();
+    asm volatile("bar.arrive %0, %1;" ::"r"(slot + 1), "n"(TP + 32) : "memory");
+}
+__device__ __forceinline__ void terms_wait(int slot) { asm volatile("bar.sync %0, %1;" ::"r"(slot + 1), "n"(TP + 32) : "memory"); }
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -309,7 +316,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         static_assert(NRED / 32 == NT, "one reducer warp per term-ring slot");
         const int s = warp - (TP + NBUILD) / 32;
         for (int i = s; i < grp.count; i += NT) {
-            mbar_wait_relaxed(&full_t[s], (uint32_t)((i / NT) & 1), 150);
+            terms_wait(s);
             reduce_entry(sterm + s * 4 * TROW, lane, meta, s_cdesc, s_sdesc, s_slot, csum + s * CHUNK_CAP,
                          P.partial + (int64_t)s_ent[i] * P.PS);
             __syncwarp();
@@ -460,8 +467,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
             float *tm = sterm + st * 4 * TROW;
             if (MODE != MODE_VALUE) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
             tm[so3] = t3;
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&full_t[st]);
+            terms_arrive(st);
         }
     }
 }

@@ -34,7 +34,7 @@ struct OptShape {
 };
 
 struct OptHyper {
-    double lr, beta1, beta2, eps, c1, safe_lo, safe_hi;
+    double lr, beta1, beta2, eps, c1, safe_lo, safe_hi, ls_noise;
     int32_t ls_max;
 };
 
@@ -210,7 +210,7 @@ __global__ void k_opt_ls(OptWork w, OptShape sh, OptHyper hy) {
     for (int r = 0; r < sh.nregion; ++r) Lt += w.nll_reg_t[(int64_t)e * sh.nregion + r];
     Lt *= w.cscale[e];
     const double a = w.alpha[e];
-    if (Lt <= w.L0[e] + hy.c1 * a * w.gd[e]) {   // false for NaN / +inf
+    if (Lt <= w.L0[e] + hy.c1 * a * w.gd[e] + hy.ls_noise * fabs(w.L0[e])) {   // false for NaN / +inf
         w.accepted[e] = 1;
         w.alpha_acc[e] = a;
     } else {
