@@ -268,7 +268,7 @@ def main():
     alg_bytes = BYTES_PER_PIXEL_EVAL * pe_step / launches_per_step
     achieved = alg_bytes / (k_avg_ms * 1e-3) / 1e9 if k_n else 0.0
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "k_like<15,GRAD>", "kernel_ms": k_avg_ms, "kernel_share_of_step": k_ms / ms if ms else None,
+                "traffic": None, "kernel": "k_like_cell<15,GRAD> (fused per-pixel kernel, cell form)", "kernel_ms": k_avg_ms, "kernel_share_of_step": k_ms / ms if ms else None,
                 "peak_source": peak_src, "frac_of_8TBps_nominal": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes}
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")

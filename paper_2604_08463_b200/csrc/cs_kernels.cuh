@@ -108,44 +108,75 @@ __device__ __forceinline__ uint64_t policy_evict_normal() {
 }
 
 // ----------------------------------------------------------------------------------------------------------
-// a1: SED factor tables.  One thread per (entry, parameter, band).  fp64 -> fp32.
+// a1: SED factor tables.  One thread per (entry, parameter, band quad).  fp64 -> fp32.
 // ----------------------------------------------------------------------------------------------------------
+// exp(y) in fp64 for the power-law rows: y = k ln2 + r, |r| <= ln2/2, degree-11 Taylor polynomial (truncation
+// 6e-15 relative, far below the fp32 rounding of the stored value), scaled by 2^k through the exponent field.
+// Arguments outside the range where 2^k is a normal number take the library routine.
+__device__ __forceinline__ double exp_pow(double y) {
+    if (!(fabs(y) < 700.0)) return exp(y);
+    const double kf = rint(y * 1.4426950408889634074);
+    double r = fma(-kf, 6.93147180369123816490e-01, y);
+    r = fma(-kf, 1.90821492927058770002e-10, r);
+    double p = 1.0 / 39916800.0;
+    p = fma(p, r, 1.0 / 3628800.0); p = fma(p, r, 1.0 / 362880.0); p = fma(p, r, 1.0 / 40320.0);
+    p = fma(p, r, 1.0 / 5040.0);    p = fma(p, r, 1.0 / 720.0);    p = fma(p, r, 1.0 / 120.0);
+    p = fma(p, r, 1.0 / 24.0);      p = fma(p, r, 1.0 / 6.0);      p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);             p = fma(p, r, 1.0);
+    return p * __hiloint2double(((int)kf + 1023) << 20, 0);
+}
+
+// One thread per (entry, parameter, band quad): four table values, one 16-byte store.  The band constants come from a
+// shared-memory copy (indexed by the thread's quad: a constant-bank read would serialise).
+// grid = (ceil(4 * ktot_max / 256), batch), block = 256.
 __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const int64_t *__restrict__ param_off,
                                                 const int64_t *__restrict__ tab_off, const int32_t *__restrict__ cfg_of,
                                                 const CfgDev *__restrict__ cfgs, float *__restrict__ tab, int32_t batch,
-                                                int32_t *err, const TConst tc) {
-    const int f = threadIdx.x;   // 0..15
+                                                int32_t *err, const TConst *__restrict__ tcg) {
+    __shared__ TConst tc;
+    for (int i = threadIdx.x; i < (int)(sizeof(TConst) / 8); i += blockDim.x)
+        reinterpret_cast<double *>(&tc)[i] = reinterpret_cast<const double *>(tcg)[i];
+    __syncthreads();
+    const int nfreq = tc.nfreq;
     for (int e = blockIdx.y; e < batch; e += gridDim.y) {
         const CfgDev *cp = cfgs + cfg_of[e];
-        struct { int32_t K[3]; int32_t ktot; } c = {{cp->K[0], cp->K[1], cp->K[2]}, cp->ktot};   // only these fields
-        const int j = blockIdx.x * blockDim.y + threadIdx.y;
-        if (j >= c.ktot) continue;
+        const int K0 = cp->K[0], K1 = cp->K[1], ktot = cp->ktot;
+        const int id = blockIdx.x * blockDim.x + threadIdx.x;
+        const int j = id >> 2, f0 = (id & 3) * 4;
+        if (j >= ktot) continue;
         const double x = params[param_off[e] + j];
-        float *row0 = tab + (tab_off[e]) * NROW;
-        const bool live = f < tc.nfreq;
+        float *row0 = tab + tab_off[e] * NROW;
         bool bad = !isfinite(x);
-        if (j < c.K[0]) {
+        float v[4];
+        if (j < K0) {
             // dust power-law factor with the band constant folded in: cd[f] * (nu_f/nu0d)^beta_d
-            float v = live ? (float)(tc.cd[f] * exp(x * tc.lnd[f])) : 0.f;
-            row0[(int64_t)j * NROW + f] = v;
-        } else if (j < c.K[0] + c.K[1]) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cd[f0 + i] * exp_pow(x * tc.lnd[f0 + i])) : 0.f;
+            *reinterpret_cast<float4 *>(row0 + (int64_t)j * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+        } else if (j < K0 + K1) {
             // Planck ratio G = expm1(x0)/expm1(x) and d ln G / dT = (1/T) [ x/(1-e^-x) - x0/(1-e^-x0) ]
             bad = bad || !(x > 0.0);
-            const int k = j - c.K[0];
-            float g = 0.f, dg = 0.f;
-            if (live) {
-                const double xf = tc.hk * tc.nu[f] / x, x0 = tc.hk * tc.nu0d / x;
-                g = (float)(expm1(x0) / expm1(xf));
-                dg = (float)((xf / (-expm1(-xf)) - x0 / (-expm1(-x0))) / x);
+            const int k = j - K0;
+            float dg[4];
+            const double x0 = tc.hk * tc.nu0d / x, e0 = expm1(x0), h0 = x0 / (-expm1(-x0));
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                v[i] = 0.f; dg[i] = 0.f;
+                if (f0 + i < nfreq) {
+                    const double xf = tc.hk * tc.nu[f0 + i] / x;
+                    v[i] = (float)(e0 / expm1(xf));
+                    dg[i] = (float)((xf / (-expm1(-xf)) - h0) / x);
+                }
             }
-            row0[(int64_t)(c.K[0] + k) * NROW + f] = g;
-            row0[(int64_t)(c.K[0] + c.K[1] + k) * NROW + f] = dg;
+            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + K1 + k) * NROW + f0) = make_float4(dg[0], dg[1], dg[2], dg[3]);
         } else {
-            const int k = j - c.K[0] - c.K[1];
-            float v = live ? (float)(tc.cs[f] * exp(x * tc.lns[f])) : 0.f;
-            row0[(int64_t)(c.K[0] + 2 * c.K[1] + k) * NROW + f] = v;
+            const int k = j - K0 - K1;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cs[f0 + i] * exp_pow(x * tc.lns[f0 + i])) : 0.f;
+            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + 2 * K1 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
         }
-        if (bad && f == 0) atomicOr(err, ERR_DOMAIN);
+        if (bad && f0 == 0) atomicOr(err, ERR_DOMAIN);
     }
 }
 
@@ -523,38 +554,43 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
 // which are contiguous in the partial row.
 // want_grad = 0: only the region outputs.
 // ----------------------------------------------------------------------------------------------------------
-// One warp per output: lane l adds the slots a+l, a+l+32, ... in ascending order, then the 32 lane sums are combined
-// by a fixed xor-shuffle tree, so the result is bitwise reproducible.  grid = (ceil(nout_max/8), batch), 256 threads.
-__device__ __forceinline__ double warp_sum_fixed(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
+// Cluster outputs (short slot ranges): one thread each, slots added in ascending order.  Region outputs (one slot per
+// tile): one warp each, lane l adds the slots a+l, a+l+32, ... in ascending order and the 32 lane sums are combined by a
+// fixed xor-shuffle tree.  Both orders are fixed, so the result is bitwise reproducible.
+// Virtual thread index v: [0, ktot) clusters, [ktot_pad + 32 r, +32) region r.  grid = (ceil(nvirt_max/256), batch).
 __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
                                                const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
                                                const int64_t *__restrict__ param_off, int32_t nregion, int32_t want_grad,
                                                double *__restrict__ nll, double *__restrict__ grad) {
     const int e = blockIdx.y, lane = threadIdx.x & 31;
     const CfgDev *c = cfgs + cfg_of[e];
-    const int K0 = c->K[0], K1 = c->K[1], ktot = c->ktot;
-    const int nout = (want_grad ? ktot : 0) + nregion;
-    const int j = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (j >= nout) return;
-    int t, k;
-    if (!want_grad) { t = 3; k = j; }
-    else if (j < K0) { t = 0; k = j; }
-    else if (j < K0 + K1) { t = 1; k = j - K0; }
-    else if (j < ktot) { t = 2; k = j - K0 - K1; }
-    else { t = 3; k = j - ktot; }
-    const int32_t *ksegptr = maps[c->map[t]].ksegptr;
-    const double *row = partial + (int64_t)e * PS + c->segbase[t];
-    double acc = 0.0;
-    const int a = ksegptr[k], b = ksegptr[k + 1];
-    for (int q = a + lane; q < b; q += 32) acc += row[q];
-    acc = warp_sum_fixed(acc);
-    if (lane == 0) {
-        if (t == 3) nll[(int64_t)e * nregion + k] = acc;
-        else grad[param_off[e] + j] = acc;
+    const int K0 = c->K[0], K1 = c->K[1], ktot = want_grad ? c->ktot : 0;
+    const int kpad = (ktot + 31) & ~31;
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    const double *erow = partial + (int64_t)e * PS;
+    if (v < ktot) {
+        int t, k;
+        if (v < K0) { t = 0; k = v; }
+        else if (v < K0 + K1) { t = 1; k = v - K0; }
+        else { t = 2; k = v - K0 - K1; }
+        const int32_t *ksegptr = maps[c->map[t]].ksegptr;
+        const double *row = erow + c->segbase[t];
+        const int a = ksegptr[k], b = ksegptr[k + 1];
+        double acc = 0.0;
+#pragma unroll 4
+        for (int q = a; q < b; ++q) acc += row[q];
+        grad[param_off[e] + v] = acc;
+    } else if (v >= kpad && (v - kpad) >> 5 < nregion) {
+        const int r = (v - kpad) >> 5;
+        const int32_t *ksegptr = maps[c->map[3]].ksegptr;
+        const double *row = erow + c->segbase[3];
+        const int a = ksegptr[r], b = ksegptr[r + 1];
+        double acc = 0.0;
+#pragma unroll 4
+        for (int q = a + lane; q < b; q += 32) acc += row[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) nll[(int64_t)e * nregion + r] = acc;
     }
 }
 

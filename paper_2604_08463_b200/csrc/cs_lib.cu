@@ -112,6 +112,7 @@ struct cs_ctx {
     int64_t prof_n = 0;
     // misc
     int32_t *d_err = nullptr;
+    TConst *d_tc = nullptr;             // device copy of tc (k_tables stages it in shared memory)
     int64_t launches = 0;
     bool tables_built = false;
     bool force_direct = false;          // CS_FORCE_DIRECT=1 in the environment at cs_create: never use the cell kernel (tests)
@@ -437,7 +438,10 @@ int cs_create(cs_ctx **out, const cs_model *m) {
         c->tc.cd[f] = (nu / c->nu0d) * ud;   // (nu/nu0)^(beta_d+1) = (nu/nu0) * (nu/nu0)^beta_d
         c->tc.cs[f] = us;
     }
-    if (cudaMalloc((void **)&c->d_err, sizeof(int32_t)) != cudaSuccess || cudaMemset(c->d_err, 0, sizeof(int32_t)) != cudaSuccess) {
+    if (cudaMalloc((void **)&c->d_err, sizeof(int32_t)) != cudaSuccess || cudaMemset(c->d_err, 0, sizeof(int32_t)) != cudaSuccess ||
+        cudaMalloc((void **)&c->d_tc, sizeof(TConst)) != cudaSuccess ||
+        cudaMemcpy(c->d_tc, &c->tc, sizeof(TConst), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaFree(c->d_err); cudaFree(c->d_tc);
         delete c;
         return CS_ECUDA;
     }
@@ -456,6 +460,7 @@ int cs_destroy(cs_ctx *c) {
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->comp_stream) cudaStreamDestroy(c->comp_stream);
     cudaFree(c->d_err);
+    cudaFree(c->d_tc);
     for (auto &e : c->prof_ev) cudaEventDestroy(e);
     delete c;
     return CS_OK;
@@ -667,9 +672,9 @@ int cs_param_offsets(cs_ctx *c, int64_t *off) {
 int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
     if (!c || c->batch <= 0 || !params) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    dim3 block(16, 16);
-    dim3 grid((c->ktot_max + 15) / 16, std::min(c->batch, 65535));
-    k_tables<<<grid, block, 0, st>>>(params, c->d_param_off, c->d_tab_off, c->d_cfg_of, c->d_cfgs, c->d_tab, c->batch, c->d_err, c->tc);
+    dim3 block(256);
+    dim3 grid((4 * c->ktot_max + 255) / 256, std::min(c->batch, 65535));
+    k_tables<<<grid, block, 0, st>>>(params, c->d_param_off, c->d_tab_off, c->d_cfg_of, c->d_cfgs, c->d_tab, c->batch, c->d_err, c->d_tc);
     c->launches++;
     CK(cudaGetLastError());
     c->tables_built = true;
@@ -679,8 +684,8 @@ int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
 static int merge_launch(cs_ctx *c, double *nll, double *grad, cudaStream_t st) {
     for (int e0 = 0; e0 < c->batch; e0 += 65535) {
         const int nb = std::min(65535, c->batch - e0);
-        const int nout = (grad ? c->ktot_max : 0) + c->nregion;
-        dim3 grid((nout + 7) / 8, nb);
+        const int nout = (grad ? ((c->ktot_max + 31) & ~31) : 0) + 32 * c->nregion;   // virtual threads, see k_merge
+        dim3 grid((nout + 255) / 256, nb);
         k_merge<<<grid, 256, 0, st>>>(c->d_partial + (int64_t)e0 * c->PS, c->PS, c->d_maps, c->d_cfgs, c->d_cfg_of + e0,
                                      c->d_param_off + e0, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad);
         c->launches++;
