@@ -29,7 +29,7 @@ constexpr int CELL_CAP = 96;   // cell path: most distinct cluster triples a til
 constexpr int CHUNK_LEN = 8;   // cell kernel reduce: ranks summed by one lane in one step (SEG_MAX / CHUNK_LEN <= 4)
 constexpr int CHUNK_CAP = 416; // cell kernel reduce: most chunks (and segments) of the four terms of one tile
 constexpr int ROW_CAP = 128;   // cell path: most distinct table rows the cells of one tile may read
-constexpr int CSTRIDE = 68;    // floats per cell row in shared memory: 48 column values + 16 scalars + 4 pad (= 4 mod 32 banks)
+constexpr int CSTRIDE = 36;    // floats per cell row in shared memory: 16 column values + 16 scalars + 4 pad (= 4 mod 32 banks)
 
 // A pivot of the LDL^T factorisation of M = A^T N^-1 A counts as non-positive (CS_ESINGULAR) when it is below this
 // fraction of its diagonal entry: below it an fp32 solve carries no correct digit (R11).

@@ -28,7 +28,8 @@
 
 namespace cs {
 
-constexpr int NR = 3;        // table-row ring depth
+constexpr int NR = 5;        // table-row ring depth: builders run up to NC entries ahead of the consumers, which read
+                             // the T_d and beta_s rows of their cell from the same stage (NR >= NC + 2)
 template <int NF>
 struct DataDepth { static constexpr int value = (NF == 15) ? 3 : 2; };   // data ring depth (entries in flight)
 constexpr int NBG = 1;       // builder groups: group g builds the entries i = g (mod NBG)
@@ -39,10 +40,9 @@ constexpr int NRED = 128;                        // reducer threads
 constexpr int CELL_THREADS = TP + NBUILD + NRED + 32;   // 512
 static_assert(SEG_MAX <= 4 * CHUNK_LEN && CELL_CAP % 32 == 0 && NC % NBG == 0, "builder warps / ring slots per group");
 
-// cell row layout (floats): for quad q = 0..3 (bands 4q..4q+3): [12q+0..3] w a_d, [12q+4..7] w a_s, [12q+8..11] w a_d dlnG
-// [48..63] scalars:
-constexpr int CS_L10 = 48, CS_L20 = 49, CS_L21 = 50, CS_ID1 = 51, CS_ID2 = 52, CS_P10 = 53, CS_P11 = 54, CS_P12 = 55,
-              CS_P20 = 56, CS_P21 = 57, CS_P22 = 58, CS_P30 = 59, CS_P31 = 60, CS_P32 = 61, CS_BAD = 62;
+// cell row layout (floats): [0..15] w a_d per band; [16..31] scalars l10 l20 l21 1/d1 | 1/d2 P10 P11 P12 | P20 P21 P22 P30 |
+// P31 P32 bad -.  The other two weighted columns depend on one cluster id only and are formed by the consumers from
+// the staged table rows, which many lanes of a warp share: w a_s = w Fs'[k2], w a_d dlnG = dlnG[k1] (w a_d).
 
 template <int NF>
 constexpr size_t cell_smem_bytes() {
@@ -183,9 +183,7 @@ __device__ __forceinline__ void build_cell(const CellRows &R, const KConst &kc, 
                 p30 = add2(p30, u3); p31 = fma2(u3, ad, p31); p32 = fma2(u3, as, p32);
             }
         }
-        o4[3 * q + 0] = make_float4(wd[0].x, wd[0].y, wd[1].x, wd[1].y);
-        o4[3 * q + 1] = make_float4(ws[0].x, ws[0].y, ws[1].x, ws[1].y);
-        if (GRAD) o4[3 * q + 2] = make_float4(u2[0].x, u2[0].y, u2[1].x, u2[1].y);
+        o4[q] = make_float4(wd[0].x, wd[0].y, wd[1].x, wd[1].y);
     }
     // LDL^T of M (m00 = sum_f w_f is a constant of the data set)
     const float M01 = hsum(m01), M02 = hsum(m02), M11 = hsum(m11), M12 = hsum(m12), M22 = hsum(m22);
@@ -198,10 +196,10 @@ __device__ __forceinline__ void build_cell(const CellRows &R, const KConst &kc, 
     const float id2 = fast_rcp(d2);
     const bool ok = (d1 > PIVOT_RTOL * M11) && (d2 > PIVOT_RTOL * M22);
     if (!ok) atomicOr(err, ERR_SINGULAR);
-    o4[12] = make_float4(l10, l20, l21, id1);
-    o4[13] = make_float4(id2, hsum(p10), hsum(p11), hsum(p12));
-    o4[14] = make_float4(hsum(p20), hsum(p21), hsum(p22), hsum(p30));
-    o4[15] = make_float4(hsum(p31), hsum(p32), ok ? 0.f : 1.f, 0.f);
+    o4[4] = make_float4(l10, l20, l21, id1);
+    o4[5] = make_float4(id2, hsum(p10), hsum(p11), hsum(p12));
+    o4[6] = make_float4(hsum(p20), hsum(p21), hsum(p22), hsum(p30));
+    o4[7] = make_float4(hsum(p31), hsum(p32), ok ? 0.f : 1.f, 0.f);
 }
 
 template <int NF, int MODE>
@@ -240,7 +238,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         for (int s = 0; s < ND; ++s) { mbar_init(&full_d[s], 1); mbar_init(&empty_d[s], TP / 32); }
         for (int s = 0; s < NC; ++s) { mbar_init(&full_c[s], CELL_CAP / 32); mbar_init(&empty_c[s], TP / 32); }
         for (int s = 0; s < NT; ++s) { mbar_init(&full_t[s], TP / 32); mbar_init(&empty_t[s], 1); }
-        for (int s = 0; s < NR; ++s) { mbar_init(&full_r[s], 1); mbar_init(&empty_r[s], NBUILD / 32); }
+        for (int s = 0; s < NR; ++s) { mbar_init(&full_r[s], 1); mbar_init(&empty_r[s], NBUILD / 32 + TP / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid < grp.count) {
@@ -367,14 +365,19 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         }
     }
     const bool live = cid != 0xFF;
+    int slot_dg = 0, slot_fs = 0;   // slots of this pixel's dlnG[k1] and Fs'[k2] rows in the tile's staged row list
+    if (live) {
+        const int32_t *cr = cfg.cellrows + 4 * (int64_t)(cfg.cellptr[tile] + cid);
+        slot_dg = cr[2] * NROW; slot_fs = cr[3] * NROW;
+    }
     const float2 *w2 = reinterpret_cast<const float2 *>(P.kc.w);
     const float2 *lnd2 = reinterpret_cast<const float2 *>(P.kc.lnd);
     const float2 *lns2 = reinterpret_cast<const float2 *>(P.kc.lns);
     const float inv_m00 = P.kc.inv_m00;
 
     for (int i = 0; i < grp.count; ++i) {
-        const int sd = i % ND, sc = i % NC;
-        mbar_wait(&full_c[sc], (uint32_t)((i / NC) & 1));
+        const int sd = i % ND, sc = i % NC, sr = i % NR;
+        mbar_wait(&full_c[sc], (uint32_t)((i / NC) & 1));   // the builders waited for full_r[sr]: the rows are there too
         mbar_wait(&full_d[sd], (uint32_t)((i / ND) & 1));
         const float2 z = make_float2(0.f, 0.f);
         float2 bq0 = z, bq1 = z, bq2 = z, bu0 = z, bu1 = z, bu2 = z;
@@ -383,34 +386,36 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         if (live) {
             const float *st = ring + sd * STAGE + tid;
             const float4 *cell = reinterpret_cast<const float4 *>(cells + (sc * CELL_CAP + cid) * CSTRIDE);
+            const float4 *rfs = reinterpret_cast<const float4 *>(rowbuf + sr * ROW_CAP * NROW + slot_fs);
+            const float4 *rdg = reinterpret_cast<const float4 *>(rowbuf + sr * ROW_CAP * NROW + slot_dg);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const float4 WD = cell[3 * q], WS = cell[3 * q + 1];
-                float4 U2 = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (kGrad) U2 = cell[3 * q + 2];
+                const float4 WD = cell[q], FS = rfs[q];
+                float4 DG = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (kGrad) DG = rdg[q];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                     const int j = 2 * q + h;
                     const float2 dq = make_float2(st[(4 * j + 0) * TP], (2 * j + 1 < NF) ? st[(4 * j + 2) * TP] : 0.f);
                     const float2 du = make_float2(st[(4 * j + 1) * TP], (2 * j + 1 < NF) ? st[(4 * j + 3) * TP] : 0.f);
                     const float2 wd = h ? make_float2(WD.z, WD.w) : make_float2(WD.x, WD.y);
-                    const float2 ws = h ? make_float2(WS.z, WS.w) : make_float2(WS.x, WS.y);
+                    const float2 ws = mul2(w2[j], h ? make_float2(FS.z, FS.w) : make_float2(FS.x, FS.y));
                     bq0 = fma2(w2[j], dq, bq0); bq1 = fma2(wd, dq, bq1); bq2 = fma2(ws, dq, bq2);
                     bu0 = fma2(w2[j], du, bu0); bu1 = fma2(wd, du, bu1); bu2 = fma2(ws, du, bu2);
                     if (kGrad) {
-                        const float2 u2 = h ? make_float2(U2.z, U2.w) : make_float2(U2.x, U2.y);
+                        const float2 u2 = mul2(h ? make_float2(DG.z, DG.w) : make_float2(DG.x, DG.y), wd);
                         const float2 u1 = mul2(lnd2[j], wd), u3 = mul2(lns2[j], ws);
                         cq1 = fma2(u1, dq, cq1); cq2 = fma2(u2, dq, cq2); cq3 = fma2(u3, dq, cq3);
                         cu1 = fma2(u1, du, cu1); cu2 = fma2(u2, du, cu2); cu3 = fma2(u3, du, cu3);
                     }
                 }
             }
-            S0 = cell[12]; S1 = cell[13];
-            if (kGrad) S2 = cell[14];
-            S3 = cell[15];
+            S0 = cell[4]; S1 = cell[5];
+            if (kGrad) S2 = cell[6];
+            S3 = cell[7];
         }
         __syncwarp();   // every lane has read its data and cell rows: hand both slots back
-        if (lane == 0) { mbar_arrive(&empty_d[sd]); mbar_arrive(&empty_c[sc]); }
+        if (lane == 0) { mbar_arrive(&empty_d[sd]); mbar_arrive(&empty_c[sc]); mbar_arrive(&empty_r[sr]); }
 
         float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
         if (live) {
