@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         for (int s = 0; s < ND; ++s) { mbar_init(&full_d[s], 1); mbar_init(&empty_d[s], TP / 32); }
         for (int s = 0; s < NC; ++s) { mbar_init(&full_c[s], CELL_CAP / 32); mbar_init(&empty_c[s], TP / 32); }
         for (int s = 0; s < NT; ++s) { mbar_init(&full_t[s], TP / 32); mbar_init(&empty_t[s], 1); }
-        for (int s = 0; s < NR; ++s) { mbar_init(&full_r[s], 1); mbar_init(&empty_r[s], NBUILD / 32 + TP / 32); }
+        for (int s = 0; s < NR; ++s) { mbar_init(&full_r[s], 1); mbar_init(&empty_r[s], CELL_CAP / 32 + TP / 32); }   // one builder group + consumers
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid < grp.count) {
