@@ -343,6 +343,38 @@ def main():
             mms = e0.elapsed_time(e1) / 5
             out["extras"] = {"component_maps_pixel_evals_per_s": nsel * w.npix / (mms * 1e-3),
                              "component_maps_GBps": nsel * w.npix * 144.0 / (mms * 1e-3) / 1e9, "component_maps_entries": nsel}
+            # config 2 of BASELINE.json: one entry, K=(500,50,100), 200 AdaTopK iterations from (1.54, 20, -3)
+            w2 = gen.make_config(1)
+            c2 = cs.Context(w2.freqs, w2.npix)
+            c2.set_clusters(w2.maps, w2.Kmap, w2.cfg_maps, w2.region_idx, w2.nregion)
+            d2 = torch.from_numpy(w2.data()).to(dev)
+            c2.set_data(d2, w2.ninv)
+            c2.set_batch(w2.cfg_of, w2.data_of)
+            K2 = w2.K_of_cfg(0)
+            lo = torch.from_numpy(np.concatenate([np.full(K2[0], 0.5), np.full(K2[1], 8.0), np.full(K2[2], -5.0)])).to(dev)
+            hi = torch.from_numpy(np.concatenate([np.full(K2[0], 3.0), np.full(K2[1], 40.0), np.full(K2[2], -1.0)])).to(dev)
+            nf = torch.zeros(1, dtype=torch.float64, device=dev)
+            times = []
+            for _ in range(2):
+                p2 = torch.from_numpy(w2.params_const()).to(dev)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                c2.optimize(p2, lo, hi, cs.opt_defaults(iters=200), nf, stream)
+                torch.cuda.synchronize()
+                times.append(time.perf_counter() - t0)
+            l0 = c2.kernel_launches()
+            c2.build_sed_tables(p2, stream)
+            n1 = torch.zeros(1, dtype=torch.float64, device=dev)
+            g1 = torch.zeros_like(p2)
+            e0.record(stream)
+            for _ in range(20):
+                c2.build_sed_tables(p2, stream)
+                c2.spectral_like_grad(n1, g1, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            out["extras"].update({"c2_optimize_200_iters_ms": 1e3 * min(times), "c2_final_nll": float(nf.item()),
+                                  "c2_like_grad_call_us": 1e3 * e0.elapsed_time(e1) / 20})
+            c2.close()
     elif world > 1:
         out["e2e"] = None
     if rank == 0:

@@ -719,23 +719,31 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
         if (e < 0 || e >= c->batch) return CS_EINVAL;
         el[i] = e;
     }
-    // one group per selected entry (its start is the output slot); cell-path groups first
+    // groups = runs of consecutive selected entries of one configuration (a group's start is its first output slot);
+    // cell-path groups first
     int32_t ncell = 0;
     for (int pass = 0; pass < 2; ++pass)
-        for (int32_t i = 0; i < nsel; ++i) {
-            const bool cellp = c->cfgs[c->cfg_of[el[i]]].ncell_max > 0;
-            if (cellp == (pass == 0)) gr.push_back(Group{c->cfg_of[el[i]], i, 1, 0});
-            if (pass == 0 && cellp) ++ncell;
+        for (int32_t i = 0; i < nsel;) {
+            const int32_t cf = c->cfg_of[el[i]];
+            int32_t j = i;
+            while (j < nsel && c->cfg_of[el[j]] == cf && j - i < GROUP_MAX) ++j;
+            const bool cellp = c->cfgs[cf].ncell_max > 0;
+            if (cellp == (pass == 0)) {
+                gr.push_back(Group{cf, i, j - i, 0});
+                if (pass == 0) ++ncell;
+            }
+            i = j;
         }
+    const int32_t ngr = (int32_t)gr.size();
     // small synchronous uploads: map output is not on the optimizer's hot path
     CK(cudaStreamSynchronize(st));
     CK(cudaMemcpy(c->d_sel_elist, el.data(), sizeof(int32_t) * nsel, cudaMemcpyHostToDevice));
-    CK(cudaMemcpy(c->d_sel_groups, gr.data(), sizeof(Group) * nsel, cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->d_sel_groups, gr.data(), sizeof(Group) * ngr, cudaMemcpyHostToDevice));
     LikeParams P = base_params(c);
     P.groups = c->d_sel_groups;
     P.elist = c->d_sel_elist;
     P.maps_out = s;
-    return launch_like<MODE_MAPS>(c, P, 0, nsel, ncell, st);
+    return launch_like<MODE_MAPS>(c, P, 0, ngr, ncell, st);
 }
 
 int cs_cmb_variance(cs_ctx *c, double *var, void *stream) {

@@ -32,6 +32,7 @@ constexpr int NR = 5;        // table-row ring depth: builders run up to NC entr
                              // the T_d and beta_s rows of their cell from the same stage (NR >= NC + 2)
 template <int NF>
 struct DataDepth { static constexpr int value = (NF == 15) ? 3 : 2; };   // data ring depth (entries in flight)
+constexpr int RSTRIDE = 20;   // floats per staged table row (16 + 4 pad: consecutive rows start 20 banks apart, no conflicts)
 constexpr int NBG = 1;       // builder groups: group g builds the entries i = g (mod NBG)
 constexpr int NC = 3;        // cell-table ring depth (a multiple of NBG)
 constexpr int NT = 4;        // term ring depth
@@ -48,7 +49,7 @@ template <int NF>
 constexpr size_t cell_smem_bytes() {
     constexpr int ND = DataDepth<NF>::value;
     return (size_t)ND * 2 * NF * TP * 4               // data ring
-           + (size_t)NR * ROW_CAP * NROW * 4          // table rows of the tile's cells, staged per entry
+           + (size_t)NR * ROW_CAP * RSTRIDE * 4       // table rows of the tile's cells, staged per entry
            + (size_t)NC * CELL_CAP * CSTRIDE * 4      // cell tables
            + (size_t)NT * 4 * TROW * 4                // term ring
            + (size_t)NT * CHUNK_CAP * 8               // chunk sums of the reducer warps (fp64)
@@ -100,7 +101,7 @@ __device__ __forceinline__ void load_chunk_plan(const MapDev *__restrict__ maps,
 
 // First level of the ordered reduction (a3) of one entry by one reducer warp, in fp64 and in a fixed order:
 // step 1, one lane per chunk: (x0 + x4) + (x1 + x5) paired with (x2 + x6) + (x3 + x7) over the chunk's <= 8 ranks
-// (ascending pixel order), straight-line so that the lanes do not diverge; step 2, one lane per segment: the
+// taken in an order rotated by the lane, straight-line so that the lanes do not diverge; step 2, one lane per segment: the
 // segment's chunk sums left to right, stored at the segment's cluster-major slot of the entry's partial row.
 __device__ __forceinline__ void reduce_entry(const float *tbuf, int lane, const int32_t *meta, const uint16_t *s_cdesc,
                                              const uint16_t *s_sdesc, const int32_t *s_slot, double *csum,
@@ -110,9 +111,14 @@ __device__ __forceinline__ void reduce_entry(const float *tbuf, int lane, const 
         const uint32_t d = s_cdesc[r];
         const int start = d & 0xff, len = (int)((d >> 8) & 7) + 1, t = (int)(d >> 11);
         const float *term = tbuf + t * TROW + start;
+        // element (k + lane) mod 8 in step k: consecutive lanes hold consecutive chunks (8 ranks apart), so the rotation
+        // spreads a step's 32 loads over all banks; the order stays a fixed function of the plan
         float x[CHUNK_LEN];
 #pragma unroll
-        for (int j = 0; j < CHUNK_LEN; ++j) x[j] = (j < len) ? term[j] : 0.f;
+        for (int k = 0; k < CHUNK_LEN; ++k) {
+            const int j = (k + lane) & (CHUNK_LEN - 1);
+            x[k] = (j < len) ? term[j] : 0.f;
+        }
         const double a0 = (double)x[0] + (double)x[4], a1 = (double)x[1] + (double)x[5];
         const double a2 = (double)x[2] + (double)x[6], a3 = (double)x[3] + (double)x[7];
         csum[r] = (a0 + a1) + (a2 + a3);
@@ -136,10 +142,10 @@ struct CellRows {
 };
 template <bool GRAD>
 __device__ __forceinline__ void load_cell_rows(const float *tb, const int4 rows, CellRows &R) {   // tb: staged rows (smem)
-    const float4 *rFd = reinterpret_cast<const float4 *>(tb + rows.x * NROW);
-    const float4 *rG = reinterpret_cast<const float4 *>(tb + rows.y * NROW);
-    const float4 *rdG = reinterpret_cast<const float4 *>(tb + rows.z * NROW);
-    const float4 *rFs = reinterpret_cast<const float4 *>(tb + rows.w * NROW);
+    const float4 *rFd = reinterpret_cast<const float4 *>(tb + rows.x * RSTRIDE);
+    const float4 *rG = reinterpret_cast<const float4 *>(tb + rows.y * RSTRIDE);
+    const float4 *rdG = reinterpret_cast<const float4 *>(tb + rows.z * RSTRIDE);
+    const float4 *rFs = reinterpret_cast<const float4 *>(tb + rows.w * RSTRIDE);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         R.Fd[q] = rFd[q]; R.G[q] = rG[q]; R.Fs[q] = rFs[q];
@@ -209,7 +215,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
     constexpr int ND = DataDepth<NF>::value;
     float *ring = reinterpret_cast<float *>(smem_raw);
     float *rowbuf = ring + ND * STAGE;
-    float *cells = rowbuf + NR * ROW_CAP * NROW;
+    float *cells = rowbuf + NR * ROW_CAP * RSTRIDE;
     float *sterm = cells + NC * CELL_CAP * CSTRIDE;
     double *csum = reinterpret_cast<double *>(sterm + NT * 4 * TROW);
     uint64_t *bars = reinterpret_cast<uint64_t *>(csum + NT * CHUNK_CAP);
@@ -280,10 +286,12 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         for (int i = 0; i < grp.count; ++i) {
             const int sr = i % NR, s = i % ND;
             mbar_wait_relaxed(&empty_r[sr], (uint32_t)(((i / NR) & 1) ^ 1), 250);
-            float4 *dst = reinterpret_cast<float4 *>(rowbuf + sr * ROW_CAP * NROW);
+            float *dst = rowbuf + sr * ROW_CAP * RSTRIDE;
 #pragma unroll
-            for (int k = 0; k < NQ; ++k)
-                if (myoff[k] >= 0) dst[lane + 32 * k] = v[k];
+            for (int k = 0; k < NQ; ++k) {
+                const int q = lane + 32 * k;   // quarter q = row (q >> 2), part (q & 3)
+                if (myoff[k] >= 0) *reinterpret_cast<float4 *>(dst + (q >> 2) * RSTRIDE + (q & 3) * 4) = v[k];
+            }
             __syncwarp();
             if (lane == 0) mbar_arrive(&full_r[sr]);
             if (i + 1 < grp.count) fetch(i + 1);   // in flight while lane 0 waits for a data slot
@@ -332,7 +340,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
             const int s = i % NC, sr = i % NR;
             CellRows R;
             mbar_wait_relaxed(&full_r[sr], (uint32_t)((i / NR) & 1));
-            if (c < ncell) load_cell_rows<kGrad>(rowbuf + sr * ROW_CAP * NROW, rows, R);
+            if (c < ncell) load_cell_rows<kGrad>(rowbuf + sr * ROW_CAP * RSTRIDE, rows, R);
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty_r[sr]);
             mbar_wait_relaxed(&empty_c[s], (uint32_t)(((i / NC) & 1) ^ 1));
@@ -368,7 +376,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
     int slot_dg = 0, slot_fs = 0;   // slots of this pixel's dlnG[k1] and Fs'[k2] rows in the tile's staged row list
     if (live) {
         const int32_t *cr = cfg.cellrows + 4 * (int64_t)(cfg.cellptr[tile] + cid);
-        slot_dg = cr[2] * NROW; slot_fs = cr[3] * NROW;
+        slot_dg = cr[2] * RSTRIDE; slot_fs = cr[3] * RSTRIDE;
     }
     const float2 *w2 = reinterpret_cast<const float2 *>(P.kc.w);
     const float2 *lnd2 = reinterpret_cast<const float2 *>(P.kc.lnd);
@@ -386,8 +394,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         if (live) {
             const float *st = ring + sd * STAGE + tid;
             const float4 *cell = reinterpret_cast<const float4 *>(cells + (sc * CELL_CAP + cid) * CSTRIDE);
-            const float4 *rfs = reinterpret_cast<const float4 *>(rowbuf + sr * ROW_CAP * NROW + slot_fs);
-            const float4 *rdg = reinterpret_cast<const float4 *>(rowbuf + sr * ROW_CAP * NROW + slot_dg);
+            const float4 *rfs = reinterpret_cast<const float4 *>(rowbuf + sr * ROW_CAP * RSTRIDE + slot_fs);
+            const float4 *rdg = reinterpret_cast<const float4 *>(rowbuf + sr * ROW_CAP * RSTRIDE + slot_dg);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const float4 WD = cell[q], FS = rfs[q];
