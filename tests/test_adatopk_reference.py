@@ -1,0 +1,64 @@
+"""Pins for oracle/adatopk.py, the fp64 reference of the fixed-budget AdaTopK driver (a5; App. A, Alg. 1,
+readings R13/R14 of DESIGN.md).  The paper publishes neither hyper-parameters nor a worked trajectory, so what is
+pinned is what it states about the algorithm: iterates stay inside the bounds, every accepted step decreases the
+objective (L263), a bound that the gradient pushes away from is released (L519-L525), a bound that the minimum lies
+beyond stays active, and on a sky whose optimum is known by construction (L287) the truth is recovered."""
+import numpy as np
+
+import gen
+import oracle
+from oracle.adatopk import adatopk
+
+
+def test_quadratic_with_active_bounds():
+    # f(x) = 1/2 sum c_i (x_i - t_i)^2 on [0,1]^n with some targets outside the box: the minimiser is clip(t, 0, 1)
+    g = gen.rng_for("misc", 77)
+    n = 12
+    c = 1.0 + 9.0 * g.random(n)
+    t = g.uniform(-0.5, 1.5, n)
+    t[0], t[1] = 1.7, -0.4                       # beyond the upper / lower bound
+
+    def fun(x, want_grad):
+        return 0.5 * float(np.sum(c * (x - t) ** 2)), (c * (x - t) if want_grad else None)
+    hist = []
+    x0 = np.full(n, 0.5)
+    x0[2] = 0.0                                  # starts ON the lower bound although its target is inside: must be released
+    t[2] = 0.6
+    x, L = adatopk(fun, x0, np.zeros(n), np.ones(n), iters=600, lr=0.05, history=hist)
+    assert np.all(x >= 0.0) and np.all(x <= 1.0)
+    assert all(b <= a for a, b in zip(hist, hist[1:]))
+    assert x[0] == 1.0 and x[1] == 0.0           # pinned exactly at the bound
+    assert np.max(np.abs(x - np.clip(t, 0.0, 1.0))) < 2e-3
+    assert L <= fun(np.clip(t, 0, 1), False)[0] + 1e-4
+
+
+def test_rescale_keeps_the_trajectory_scale_invariant():
+    # A4 (L541-L546): objectives scaled out of [1e-15, 1e15] are rescaled; the iterates must not depend on the scale
+    def make(scale):
+        def fun(x, want_grad):
+            return scale * float(np.sum((x - 0.3) ** 2)), (scale * 2 * (x - 0.3) if want_grad else None)
+        return fun
+    xs = [adatopk(make(s), np.full(4, 0.9), np.zeros(4), np.ones(4), iters=50)[0] for s in (1.0, 1e20, 1e-20)]
+    assert np.allclose(xs[0], xs[1], rtol=0, atol=1e-9) and np.allclose(xs[0], xs[2], rtol=0, atol=1e-9)
+
+
+def test_recovers_known_optimum_on_noiseless_cluster_constant_sky():
+    w = gen.make_config(0, nside=8, K=(6, 2, 3), noiseless=True, cluster_truth=True)
+    model, K = oracle.Model(w.freqs), w.K_of_cfg(0)
+    d, idx = w.data()[0], w.maps[w.cfg_maps[0]]
+
+    def fun(x, want_grad):
+        r = oracle.nll_grad(model, d, w.ninv, idx, K, x, want_grad=want_grad)
+        return r["nll"][0], r["grad"]
+    lo = np.concatenate([np.full(K[0], 0.5), np.full(K[1], 8.0), np.full(K[2], -5.0)])
+    hi = np.concatenate([np.full(K[0], 3.0), np.full(K[1], 40.0), np.full(K[2], -1.0)])
+    hist = []
+    x, L = adatopk(fun, w.params_const(), lo, hi, iters=300, history=hist)
+    truth = np.concatenate(w.truth["per_cluster"])
+    assert np.all(x >= lo) and np.all(x <= hi)
+    assert all(b <= a for a, b in zip(hist, hist[1:]))
+    err = np.abs(x - truth)
+    assert err[:K[0]].max() < 5e-3 and err[K[0]:K[0] + K[1]].max() < 0.2 and err[K[0] + K[1]:].max() < 5e-3, err
+    dd = d.astype(np.float64)
+    dNd = float(np.einsum("f,fsp,fsp->", w.ninv.astype(np.float64), dd, dd))
+    assert L + 0.5 * dNd < 1e-3 * abs(hist[0] + 0.5 * dNd)      # misfit reduced by > 1000x towards the noiseless optimum 0

@@ -440,3 +440,45 @@ def test_full_size_c3h_sampled_entries(torch_cuda):
     dNd = float(np.einsum("f,fsp,fsp->", w.ninv.astype(np.float64), d0, d0))
     assert 0 < 2 * nll[5, 0] + dNd < 4 * 2 * w.npix * (w.nfreq - 3)
     ctx.close()
+
+
+def _sampled_full_size(w, params, nsample, seed):
+    """Full-size batch in one context (the launch configuration of bench.py): finite everywhere, a seeded sample of
+    entries against the oracle (T1, T2), every other entry through batch invariance of a second sample."""
+    ctx, _ = make_ctx(w)
+    nll, grad = gpu_eval(ctx, params)
+    assert ctx.check() == 0 and np.isfinite(nll).all() and np.isfinite(grad).all()
+    off = w.param_offsets()
+    sample = sorted(set(gen.rng_for("misc", seed).integers(0, w.batch, nsample).tolist()) | {0, w.batch - 1})
+    data = w.data()
+    for e in sample:
+        ref = oracle_entry(w, params, e, data=data)
+        check_T1(nll[e], ref["nll"])
+        check_T2(grad[off[e]:off[e + 1]], ref, w.K_of_cfg(int(w.cfg_of[e])))
+    # an entry evaluated alone gives the same bits as inside the full batch
+    for e in sample[:3]:
+        ctx.set_batch(w.cfg_of[e:e + 1], w.data_of[e:e + 1])
+        n1, g1 = gpu_eval(ctx, params[off[e]:off[e + 1]])
+        assert np.array_equal(n1[0], nll[e]) and np.array_equal(g1, grad[off[e]:off[e + 1]])
+    ctx.close()
+
+
+def test_full_size_c4_regions_monte_carlo_sampled(torch_cuda):
+    """configs[3] at full size: 3 latitude regions, 64 configurations x 100 noise realisations = 6400 entries."""
+    w = gen.make_config(3)
+    assert w.batch == 6400 and w.nregion == 3 and w.ndata == 100
+    _sampled_full_size(w, w.params_jittered(seed=17), 10, 23)
+
+
+def test_full_size_c5_nside128_sampled(torch_cuda):
+    """configs[4] at full size: nside 128, K=(2000,200,400), 256 noise realisations."""
+    w = gen.make_config(4)
+    assert w.batch == 256 and w.npix == 196608
+    _sampled_full_size(w, w.params_jittered(seed=18), 6, 24)
+
+
+def test_full_size_c3_scan_sampled(torch_cuda):
+    """configs[2] at full size: the 1024-configuration clustering scan on one shared data set (32 distinct maps)."""
+    w = gen.make_config(2)
+    assert w.batch == 1024 and w.maps.shape[0] == 32
+    _sampled_full_size(w, w.params_jittered(seed=19), 10, 25)
