@@ -47,6 +47,9 @@ def make_workload(name, batch, rank=0):
         B = batch or 1024
         w = gen.make_config(2, batch=B)
         desc = f"C3: nside 64 clustering scan, {B} configurations sharing one data set (L2-resident)"
+    elif name == "c4":
+        w = gen.make_config(3, batch=batch or None)
+        desc = f"C4: nside 64, 3 latitude regions, 64 configurations x 100 noise realisations ({w.batch} entries, 100 data sets)"
     elif name == "c2":
         w = gen.make_config(1)
         desc = "C2: nside 64, K=(500,50,100), one entry"
@@ -54,6 +57,7 @@ def make_workload(name, batch, rank=0):
         raise SystemExit(f"unknown workload {name}")
     if rank:
         w.realizations = tuple(r + rank * w.ndata for r in w.realizations)
+    w.bytes_per_pixel_eval = BYTES_PER_PIXEL_EVAL
     return w, desc
 
 

@@ -25,6 +25,7 @@ constexpr int TP = 256;        // pixels per tile == threads per CTA of the fuse
 constexpr int SEG_MAX = 32;    // longest ordered chain summed by one thread in the reduce phase
 constexpr int NROW = 16;       // floats per table row (nfreq padded to 16 -> 64-byte rows)
 constexpr int GROUP_MAX = 64;  // entries of one configuration handled by one CTA (per tile)
+constexpr int CELL_MIN_GROUP = 12;   // shortest group (entries of one configuration) worth the cell kernel's set-up
 constexpr int CELL_CAP = 96;   // cell path: most distinct cluster triples a tile may hold (else the direct kernel runs)
 constexpr int CHUNK_LEN = 8;   // cell kernel reduce: ranks summed by one lane in one step (SEG_MAX / CHUNK_LEN <= 4)
 constexpr int CHUNK_CAP = 416; // cell kernel reduce: most chunks (and segments) of the four terms of one tile

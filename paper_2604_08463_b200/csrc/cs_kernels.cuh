@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include "cs_internal.h"
+#include "cs_math.cuh"
 
 namespace cs {
 
@@ -200,116 +201,6 @@ struct PixelIn {
     }
 };
 
-__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
-__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
-__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
-__device__ __forceinline__ float2 dup2(float a) { return make_float2(a, a); }
-__device__ __forceinline__ float hsum(float2 a) { return a.x + a.y; }
-
-__device__ __forceinline__ void load_row(const float *__restrict__ row, float2 (&out)[NPAIR]) {
-    const float4 *r4 = reinterpret_cast<const float4 *>(row);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const float4 v = __ldg(r4 + i);
-        out[2 * i] = make_float2(v.x, v.y);
-        out[2 * i + 1] = make_float2(v.z, v.w);
-    }
-}
-
-// 1/x for x > 0 in normal range: MUFU.RCP plus one Newton step (error below 1 ulp; no slow-path branch).
-__device__ __forceinline__ float fast_rcp(float x) {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return fmaf(r, fmaf(-x, r, 1.0f), r);
-}
-
-// Forward part shared by all modes: M = A^T N^-1 A, b = A^T N^-1 d, LDL^T solve; returns s and ll.
-template <int NF>
-__device__ __forceinline__ bool pixel_forward(const PixelIn<NF> &in, const float2 (&ad)[NPAIR], const float2 (&as)[NPAIR],
-                                              const KConst &kc, float (&sq)[3], float (&su)[3], float &ll) {
-    const float2 *w2 = reinterpret_cast<const float2 *>(kc.w);
-    const float2 z = make_float2(0.f, 0.f);
-    float2 m01 = z, m02 = z, m11 = z, m12 = z, m22 = z;
-    float2 bq0 = z, bq1 = z, bq2 = z, bu0 = z, bu1 = z, bu2 = z;
-#pragma unroll
-    for (int j = 0; j < NPAIR; ++j) {
-        const float2 a = ad[j];            // a_d = cd (nu/nu0)^beta_d * Planck ratio     (Eq. 2)
-        const float2 s = as[j];            // a_s = cs (nu/nu0)^beta_s
-        const float2 wd = mul2(w2[j], a), ws = mul2(w2[j], s);
-        m01 = add2(m01, wd); m02 = add2(m02, ws);
-        m11 = fma2(wd, a, m11); m12 = fma2(wd, s, m12); m22 = fma2(ws, s, m22);
-        const float2 dq = in.dq(j), du = in.du(j);
-        bq0 = fma2(w2[j], dq, bq0); bq1 = fma2(wd, dq, bq1); bq2 = fma2(ws, dq, bq2);
-        bu0 = fma2(w2[j], du, bu0); bu1 = fma2(wd, du, bu1); bu2 = fma2(ws, du, bu2);
-    }
-    // LDL^T of the 3x3 SPD matrix M = A^T N^-1 A (m00 = sum w is a constant)
-    const float M01 = hsum(m01), M02 = hsum(m02), M11 = hsum(m11), M12 = hsum(m12), M22 = hsum(m22);
-    const float l10 = M01 * kc.inv_m00, l20 = M02 * kc.inv_m00;
-    const float d1 = fmaf(-l10, M01, M11);
-    const float t12 = fmaf(-l10, M02, M12);
-    const float id1 = fast_rcp(d1);
-    const float l21 = t12 * id1;
-    const float d2 = fmaf(-l21, t12, fmaf(-l20, M02, M22));
-    const float id2 = fast_rcp(d2);
-    const bool ok = (d1 > PIVOT_RTOL * M11) && (d2 > PIVOT_RTOL * M22);
-    {
-        const float b0 = hsum(bq0), b1 = hsum(bq1), b2 = hsum(bq2);
-        const float y1 = fmaf(-l10, b0, b1);
-        const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
-        const float z0 = b0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
-        sq[2] = z2; sq[1] = fmaf(-l21, z2, z1); sq[0] = fmaf(-l20, sq[2], fmaf(-l10, sq[1], z0));
-        ll = fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
-    }
-    {
-        const float b0 = hsum(bu0), b1 = hsum(bu1), b2 = hsum(bu2);
-        const float y1 = fmaf(-l10, b0, b1);
-        const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
-        const float z0 = b0 * kc.inv_m00, z1 = y1 * id1, z2 = y2 * id2;
-        su[2] = z2; su[1] = fmaf(-l21, z2, z1); su[0] = fmaf(-l20, su[2], fmaf(-l10, su[1], z0));
-        ll += fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
-    }
-    ll *= -0.5f;                          // -1/2 sum_S b_S . s_S                        (Eq. 6)
-    return ok;
-}
-
-// Gradient terms (Eq. 17 with s held fixed): g_theta = - sum_f w_f (da_f/dtheta) sum_S s_{S,c} r_{S,f}.
-template <int NF>
-__device__ __forceinline__ void pixel_grad(const PixelIn<NF> &in, const float2 (&ad)[NPAIR], const float2 (&as)[NPAIR],
-                                           const float2 (&dG)[NPAIR], const KConst &kc, const float (&sq)[3],
-                                           const float (&su)[3], float &g_bd, float &g_td, float &g_bs) {
-    // q_f  = sum_S s_{S,dust} r_{S,f},  qs_f = sum_S s_{S,sync} r_{S,f},  r = d - A s, expanded so that the
-    // residual itself is never stored.
-    const float2 *w2 = reinterpret_cast<const float2 *>(kc.w);
-    const float2 *lnd2 = reinterpret_cast<const float2 *>(kc.lnd);
-    const float2 *lnsw2 = reinterpret_cast<const float2 *>(kc.lnsw);
-    const float2 sqd = dup2(sq[1]), sud = dup2(su[1]), sqs = dup2(sq[2]), sus = dup2(su[2]);
-    const float2 nc0 = dup2(-fmaf(sq[1], sq[0], su[1] * su[0]));
-    const float2 nc1 = dup2(-fmaf(sq[1], sq[1], su[1] * su[1]));
-    const float2 nc2 = dup2(-fmaf(sq[1], sq[2], su[1] * su[2]));
-    const float2 ne0 = dup2(-fmaf(sq[2], sq[0], su[2] * su[0]));
-    const float2 ne2 = dup2(-fmaf(sq[2], sq[2], su[2] * su[2]));
-    const float2 z = make_float2(0.f, 0.f);
-    float2 g1 = z, g2 = z, g3 = z;
-#pragma unroll
-    for (int j = 0; j < NPAIR; ++j) {
-        const float2 a = ad[j], s = as[j];
-        const float2 dq = in.dq(j), du = in.du(j);
-        float2 q = fma2(sqd, dq, nc0);
-        q = fma2(sud, du, q);
-        q = fma2(nc1, a, q);
-        q = fma2(nc2, s, q);
-        float2 qs = fma2(sqs, dq, ne0);
-        qs = fma2(sus, du, qs);
-        qs = fma2(nc2, a, qs);
-        qs = fma2(ne2, s, qs);
-        const float2 t = mul2(w2[j], mul2(a, q));
-        g1 = fma2(lnd2[j], t, g1);               // d a_d / d beta_d = ln(nu/nu0d) a_d
-        g2 = fma2(dG[j], t, g2);                 // d a_d / d T_d    = (d ln G / dT) a_d
-        g3 = fma2(lnsw2[j], mul2(s, qs), g3);    // d a_s / d beta_s = ln(nu/nu0s) a_s
-    }
-    g_bd = -hsum(g1); g_td = -hsum(g2); g_bs = -hsum(g3);
-}
-
 // ----------------------------------------------------------------------------------------------------------
 // a2 + first level of a3: the fused kernel.  grid = (ntile, ngroup), block = TP threads = 8 warps.
 //
@@ -349,8 +240,9 @@ __device__ __forceinline__ void load_tile_plan(const MapDev *__restrict__ maps, 
 }
 
 // First level of the ordered reduction (a3) for `nent` buffered entries: one thread per (entry, term, segment); a
-// segment is a contiguous run of the rank-ordered terms of one cluster, summed in ascending pixel order in fp64 and
-// stored at the segment's cluster-major slot of the entry's partial row.
+// segment is a contiguous run of the rank-ordered terms of one cluster, summed in fp64 in the fixed chunk order of
+// cs_math.cuh (the same order as the reducer warps of k_like_cell) and stored at the segment's cluster-major slot of
+// the entry's partial row.
 __device__ __forceinline__ void reduce_terms(const float *tbuf, int nent, int tid, const int32_t *meta, const uint16_t *s_desc,
                                              const int32_t *s_slot, const int32_t *s_ent, double *__restrict__ partial, int64_t PS) {
     const int n0 = meta[0], n1 = meta[1], n2 = meta[2], n3 = meta[3];
@@ -362,11 +254,7 @@ __device__ __forceinline__ void reduce_terms(const float *tbuf, int nent, int ti
         const int ls = r - (t == 0 ? 0 : (t == 1 ? c1 : (t == 2 ? c2 : c3)));
         const uint32_t desc = s_desc[t * TP + ls];
         const int start = desc & 0xff, len = (int)(desc >> 8) + 1;
-        const float *term = tbuf + (ent * 4 + t) * TROW + start;
-        double acc = 0.0;
-#pragma unroll 4
-        for (int j = 0; j < len; ++j) acc += (double)term[j];
-        partial[(int64_t)s_ent[ent] * PS + s_slot[t * TP + ls]] = acc;
+        partial[(int64_t)s_ent[ent] * PS + s_slot[t * TP + ls]] = segment_sum(tbuf + (ent * 4 + t) * TROW, start, len);
     }
 }
 
@@ -478,19 +366,10 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
     for (int i = 0; i < grp.count; ++i) {
         const int s = i % NST;
         const float *tb = s_tab[i];
-        float2 ad[NPAIR], Fs[NPAIR];
-        if (live) {   // table rows first: their latency overlaps the wait for the data box
-            float2 Fd[NPAIR], G[NPAIR];
-            load_row(tb + r_fd, Fd);
-            load_row(tb + r_g, G);
-            load_row(tb + r_fs, Fs);
-#pragma unroll
-            for (int j = 0; j < NPAIR; ++j) ad[j] = mul2(Fd[j], G[j]);
-            if (i + 1 < grp.count) {   // next entry's rows on their way to L1 while this entry is computed
-                const float *tn = s_tab[i + 1];
-                prefetch_row(tn + r_fd); prefetch_row(tn + r_g); prefetch_row(tn + r_fs);
-                if (MODE == MODE_GRAD) prefetch_row(tn + r_dg);
-            }
+        if (live && i + 1 < grp.count) {   // next entry's rows on their way to L1 while this entry is computed
+            const float *tn = s_tab[i + 1];
+            prefetch_row(tn + r_fd); prefetch_row(tn + r_g); prefetch_row(tn + r_fs);
+            if (MODE == MODE_GRAD) prefetch_row(tn + r_dg);
         }
         PixelIn<NF> in;
         in.st = wring + s * 2 * NF * 32 + lane;
@@ -507,18 +386,41 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
 
         float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
         if (live) {
-            float sq[3], su[3], ll;
-            const bool ok = pixel_forward<NF>(in, ad, Fs, P.kc, sq, su, ll);
-            if (!ok) {
-                atomicOr(P.err, ERR_SINGULAR);
-                ll = CUDART_INF_F;
+            // the pixel is its own cell: the per-cell and the per-pixel part of cs_math.cuh in one pass over the bands
+            constexpr bool kGrad = (MODE == MODE_GRAD);
+            const float2 *w2 = reinterpret_cast<const float2 *>(P.kc.w);
+            const float2 *lnd2 = reinterpret_cast<const float2 *>(P.kc.lnd);
+            const float2 *lns2 = reinterpret_cast<const float2 *>(P.kc.lns);
+            const float4 *rFd = reinterpret_cast<const float4 *>(tb + r_fd), *rG = reinterpret_cast<const float4 *>(tb + r_g);
+            const float4 *rdG = reinterpret_cast<const float4 *>(tb + r_dg), *rFs = reinterpret_cast<const float4 *>(tb + r_fs);
+            CellSums S;
+            PixSums A;
+            cell_sums_zero(S);
+            pix_sums_zero(A);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 vFd = __ldg(rFd + q), vG = __ldg(rG + q), vFs = __ldg(rFs + q);
+                const float4 vdG = kGrad ? __ldg(rdG + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int j = 2 * q + h;
+                    const float2 Fd = h ? make_float2(vFd.z, vFd.w) : make_float2(vFd.x, vFd.y);
+                    const float2 G = h ? make_float2(vG.z, vG.w) : make_float2(vG.x, vG.y);
+                    const float2 dG = h ? make_float2(vdG.z, vdG.w) : make_float2(vdG.x, vdG.y);
+                    const float2 as = h ? make_float2(vFs.z, vFs.w) : make_float2(vFs.x, vFs.y);
+                    const float2 wd = cell_pair<kGrad>(S, Fd, G, dG, as, w2[j], lnd2[j], lns2[j]);
+                    pix_pair<kGrad>(A, wd, as, dG, w2[j], lnd2[j], lns2[j], in.dq(j), in.du(j));
+                }
             }
+            CellScal C;
+            cell_finish<kGrad>(S, P.kc.inv_m00, C);
+            if (C.bad != 0.f) atomicOr(P.err, ERR_SINGULAR);
+            float sq[3], su[3], ll;
+            pix_solve(A, C, P.kc.inv_m00, sq, su, ll);
             if (MODE == MODE_VALUE) {
                 t3 = ll;
             } else if (MODE == MODE_GRAD) {
-                float2 dG[NPAIR];
-                load_row(tb + r_dg, dG);
-                pixel_grad<NF>(in, ad, Fs, dG, P.kc, sq, su, t0, t1, t2);
+                pix_grad_terms(A, C, sq, su, t0, t1, t2);
                 t3 = ll;
             } else if (MODE == MODE_CMBVAR) {
                 t0 = sq[0]; t1 = su[0]; t2 = sq[0] * sq[0]; t3 = su[0] * su[0];

@@ -115,6 +115,7 @@ struct cs_ctx {
     TConst *d_tc = nullptr;             // device copy of tc (k_tables stages it in shared memory)
     int64_t launches = 0;
     bool tables_built = false;
+    int32_t cell_min_group = CELL_MIN_GROUP;   // CS_CELL_MIN_GROUP overrides (tests run the cell kernel on 1-entry groups)
     bool force_direct = false;          // CS_FORCE_DIRECT=1 in the environment at cs_create: never use the cell kernel (tests)
 };
 
@@ -447,6 +448,8 @@ int cs_create(cs_ctx **out, const cs_model *m) {
     }
     const char *fd = std::getenv("CS_FORCE_DIRECT");
     c->force_direct = fd && fd[0] == '1';
+    const char *mg = std::getenv("CS_CELL_MIN_GROUP");
+    if (mg && std::atoi(mg) >= 1) c->cell_min_group = std::atoi(mg);
     *out = c;
     return CS_OK;
 }
@@ -633,15 +636,20 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     // cell-path configurations first, then the direct ones; stable inside a configuration
     auto key = [&](int32_t e) { return ((int64_t)(c->cfgs[cfg_of[e]].ncell_max > 0 ? 0 : 1) << 32) | (int64_t)cfg_of[e]; };
     std::stable_sort(elist.begin(), elist.end(), [&](int32_t a, int32_t b) { return key(a) < key(b); });
-    std::vector<Group> groups;
-    c->ngroup_cell = 0;
+    // a group runs on the cell kernel when its configuration has a cell plan and it is long enough to amortise that
+    // kernel's per-CTA set-up (plan loading, ring fill); short groups (configuration scans: one entry per
+    // configuration) are ~2x faster on the direct kernel.  Cell-kernel groups come first in the array.
+    std::vector<Group> groups, direct;
     for (int32_t i = 0; i < batch;) {
         int32_t j = i;
         while (j < batch && cfg_of[elist[j]] == cfg_of[elist[i]] && j - i < GROUP_MAX) ++j;
-        groups.push_back(Group{cfg_of[elist[i]], i, j - i, 0});
-        if (c->cfgs[cfg_of[elist[i]]].ncell_max > 0) c->ngroup_cell = (int32_t)groups.size();
+        const Group g{cfg_of[elist[i]], i, j - i, 0};
+        if (c->cfgs[g.cfg].ncell_max > 0 && g.count >= c->cell_min_group) groups.push_back(g);
+        else direct.push_back(g);
         i = j;
     }
+    c->ngroup_cell = (int32_t)groups.size();
+    groups.insert(groups.end(), direct.begin(), direct.end());
     c->ngroup = (int32_t)groups.size();
     int rc;
     std::vector<int32_t> zero_i(batch, 0);
@@ -727,7 +735,7 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
             const int32_t cf = c->cfg_of[el[i]];
             int32_t j = i;
             while (j < nsel && c->cfg_of[el[j]] == cf && j - i < GROUP_MAX) ++j;
-            const bool cellp = c->cfgs[cf].ncell_max > 0;
+            const bool cellp = c->cfgs[cf].ncell_max > 0 && j - i >= c->cell_min_group;
             if (cellp == (pass == 0)) {
                 gr.push_back(Group{cf, i, j - i, 0});
                 if (pass == 0) ++ncell;

@@ -25,6 +25,7 @@
 //                barriers | per-entry meta | segment plan
 #pragma once
 #include "cs_kernels.cuh"
+#include "cs_math.cuh"
 
 namespace cs {
 
@@ -110,18 +111,7 @@ __device__ __forceinline__ void reduce_entry(const float *tbuf, int lane, const 
     for (int r = lane; r < nchunk; r += 32) {
         const uint32_t d = s_cdesc[r];
         const int start = d & 0xff, len = (int)((d >> 8) & 7) + 1, t = (int)(d >> 11);
-        const float *term = tbuf + t * TROW + start;
-        // element (k + lane) mod 8 in step k: consecutive lanes hold consecutive chunks (8 ranks apart), so the rotation
-        // spreads a step's 32 loads over all banks; the order stays a fixed function of the plan
-        float x[CHUNK_LEN];
-#pragma unroll
-        for (int k = 0; k < CHUNK_LEN; ++k) {
-            const int j = (k + lane) & (CHUNK_LEN - 1);
-            x[k] = (j < len) ? term[j] : 0.f;
-        }
-        const double a0 = (double)x[0] + (double)x[4], a1 = (double)x[1] + (double)x[5];
-        const double a2 = (double)x[2] + (double)x[6], a3 = (double)x[3] + (double)x[7];
-        csum[r] = (a0 + a1) + (a2 + a3);
+        csum[r] = chunk_sum(tbuf + t * TROW, start, len);   // cs_math.cuh: the same order as the direct kernel's sums
     }
     __syncwarp();
     for (int r = lane; r < nseg; r += 32) {
@@ -153,20 +143,19 @@ __device__ __forceinline__ void load_cell_rows(const float *tb, const int4 rows,
     }
 }
 
-// One cell (Eq. 2 columns -> weighted columns, M, LDL^T, P) from the entry's four table rows.
+// One cell (Eq. 2 columns -> weighted column, M, LDL^T, P; cs_math.cuh) from the entry's four table rows.
 template <bool GRAD>
 __device__ __forceinline__ void build_cell(const CellRows &R, const KConst &kc, float *__restrict__ out, int32_t *err) {
     const float2 *w2 = reinterpret_cast<const float2 *>(kc.w);
     const float2 *lnd2 = reinterpret_cast<const float2 *>(kc.lnd);
     const float2 *lns2 = reinterpret_cast<const float2 *>(kc.lns);
     const float4 *vFd = R.Fd, *vG = R.G, *vdG = R.dG, *vFs = R.Fs;
-    const float2 z = make_float2(0.f, 0.f);
-    float2 m01 = z, m02 = z, m11 = z, m12 = z, m22 = z;
-    float2 p10 = z, p11 = z, p12 = z, p20 = z, p21 = z, p22 = z, p30 = z, p31 = z, p32 = z;
+    CellSums S;
+    cell_sums_zero(S);
     float4 *o4 = reinterpret_cast<float4 *>(out);
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-        float2 wd[2], ws[2], u2[2];
+        float2 wd[2];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const int j = 2 * q + h;
@@ -174,38 +163,17 @@ __device__ __forceinline__ void build_cell(const CellRows &R, const KConst &kc, 
             const float2 G = h ? make_float2(vG[q].z, vG[q].w) : make_float2(vG[q].x, vG[q].y);
             const float2 dG = h ? make_float2(vdG[q].z, vdG[q].w) : make_float2(vdG[q].x, vdG[q].y);
             const float2 as = h ? make_float2(vFs[q].z, vFs[q].w) : make_float2(vFs[q].x, vFs[q].y);
-            const float2 ad = mul2(Fd, G);                   // a_d = cd (nu/nu0)^beta_d * Planck ratio   (Eq. 2)
-            wd[h] = mul2(w2[j], ad);
-            ws[h] = mul2(w2[j], as);
-            m01 = add2(m01, wd[h]); m02 = add2(m02, ws[h]);
-            m11 = fma2(wd[h], ad, m11); m12 = fma2(wd[h], as, m12); m22 = fma2(ws[h], as, m22);
-            u2[h] = z;
-            if (GRAD) {
-                const float2 u1 = mul2(lnd2[j], wd[h]);      // w da_d/dbeta_d
-                u2[h] = mul2(dG, wd[h]);                     // w da_d/dT_d
-                const float2 u3 = mul2(lns2[j], ws[h]);      // w da_s/dbeta_s
-                p10 = add2(p10, u1); p11 = fma2(u1, ad, p11); p12 = fma2(u1, as, p12);
-                p20 = add2(p20, u2[h]); p21 = fma2(u2[h], ad, p21); p22 = fma2(u2[h], as, p22);
-                p30 = add2(p30, u3); p31 = fma2(u3, ad, p31); p32 = fma2(u3, as, p32);
-            }
+            wd[h] = cell_pair<GRAD>(S, Fd, G, dG, as, w2[j], lnd2[j], lns2[j]);
         }
         o4[q] = make_float4(wd[0].x, wd[0].y, wd[1].x, wd[1].y);
     }
-    // LDL^T of M (m00 = sum_f w_f is a constant of the data set)
-    const float M01 = hsum(m01), M02 = hsum(m02), M11 = hsum(m11), M12 = hsum(m12), M22 = hsum(m22);
-    const float l10 = M01 * kc.inv_m00, l20 = M02 * kc.inv_m00;
-    const float d1 = fmaf(-l10, M01, M11);
-    const float t12 = fmaf(-l10, M02, M12);
-    const float id1 = fast_rcp(d1);
-    const float l21 = t12 * id1;
-    const float d2 = fmaf(-l21, t12, fmaf(-l20, M02, M22));
-    const float id2 = fast_rcp(d2);
-    const bool ok = (d1 > PIVOT_RTOL * M11) && (d2 > PIVOT_RTOL * M22);
-    if (!ok) atomicOr(err, ERR_SINGULAR);
-    o4[4] = make_float4(l10, l20, l21, id1);
-    o4[5] = make_float4(id2, hsum(p10), hsum(p11), hsum(p12));
-    o4[6] = make_float4(hsum(p20), hsum(p21), hsum(p22), hsum(p30));
-    o4[7] = make_float4(hsum(p31), hsum(p32), ok ? 0.f : 1.f, 0.f);
+    CellScal C;
+    cell_finish<GRAD>(S, kc.inv_m00, C);
+    if (C.bad != 0.f) atomicOr(err, ERR_SINGULAR);
+    o4[4] = make_float4(C.l10, C.l20, C.l21, C.id1);
+    o4[5] = make_float4(C.id2, C.P10, C.P11, C.P12);
+    o4[6] = make_float4(C.P20, C.P21, C.P22, C.P30);
+    o4[7] = make_float4(C.P31, C.P32, C.bad, 0.f);
 }
 
 template <int NF, int MODE>
@@ -387,9 +355,8 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         const int sd = i % ND, sc = i % NC, sr = i % NR;
         mbar_wait(&full_c[sc], (uint32_t)((i / NC) & 1));   // the builders waited for full_r[sr]: the rows are there too
         mbar_wait(&full_d[sd], (uint32_t)((i / ND) & 1));
-        const float2 z = make_float2(0.f, 0.f);
-        float2 bq0 = z, bq1 = z, bq2 = z, bu0 = z, bu1 = z, bu2 = z;
-        float2 cq1 = z, cq2 = z, cq3 = z, cu1 = z, cu2 = z, cu3 = z;
+        PixSums A;
+        pix_sums_zero(A);
         float4 S0 = make_float4(0.f, 0.f, 0.f, 0.f), S1 = S0, S2 = S0, S3 = S0;
         if (live) {
             const float *st = ring + sd * STAGE + tid;
@@ -407,60 +374,30 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
                     const float2 dq = make_float2(st[(4 * j + 0) * TP], (2 * j + 1 < NF) ? st[(4 * j + 2) * TP] : 0.f);
                     const float2 du = make_float2(st[(4 * j + 1) * TP], (2 * j + 1 < NF) ? st[(4 * j + 3) * TP] : 0.f);
                     const float2 wd = h ? make_float2(WD.z, WD.w) : make_float2(WD.x, WD.y);
-                    const float2 ws = mul2(w2[j], h ? make_float2(FS.z, FS.w) : make_float2(FS.x, FS.y));
-                    bq0 = fma2(w2[j], dq, bq0); bq1 = fma2(wd, dq, bq1); bq2 = fma2(ws, dq, bq2);
-                    bu0 = fma2(w2[j], du, bu0); bu1 = fma2(wd, du, bu1); bu2 = fma2(ws, du, bu2);
-                    if (kGrad) {
-                        const float2 u2 = mul2(h ? make_float2(DG.z, DG.w) : make_float2(DG.x, DG.y), wd);
-                        const float2 u1 = mul2(lnd2[j], wd), u3 = mul2(lns2[j], ws);
-                        cq1 = fma2(u1, dq, cq1); cq2 = fma2(u2, dq, cq2); cq3 = fma2(u3, dq, cq3);
-                        cu1 = fma2(u1, du, cu1); cu2 = fma2(u2, du, cu2); cu3 = fma2(u3, du, cu3);
-                    }
+                    const float2 fs = h ? make_float2(FS.z, FS.w) : make_float2(FS.x, FS.y);
+                    const float2 dg = h ? make_float2(DG.z, DG.w) : make_float2(DG.x, DG.y);
+                    pix_pair<kGrad>(A, wd, fs, dg, w2[j], lnd2[j], lns2[j], dq, du);   // cs_math.cuh
                 }
             }
             S0 = cell[4]; S1 = cell[5];
             if (kGrad) S2 = cell[6];
             S3 = cell[7];
         }
-        __syncwarp();   // every lane has read its data and cell rows: hand both slots back
+        __syncwarp();   // every lane has read its data and cell rows: hand the slots back
         if (lane == 0) { mbar_arrive(&empty_d[sd]); mbar_arrive(&empty_c[sc]); mbar_arrive(&empty_r[sr]); }
 
         float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
         if (live) {
-            const float l10 = S0.x, l20 = S0.y, l21 = S0.z, id1 = S0.w, id2 = S1.x;
+            CellScal C;
+            C.l10 = S0.x; C.l20 = S0.y; C.l21 = S0.z; C.id1 = S0.w; C.id2 = S1.x;
+            C.P10 = S1.y; C.P11 = S1.z; C.P12 = S1.w; C.P20 = S2.x; C.P21 = S2.y; C.P22 = S2.z; C.P30 = S2.w;
+            C.P31 = S3.x; C.P32 = S3.y; C.bad = S3.z;
             float sq[3], su[3], ll;
-            {
-                const float b0 = hsum(bq0), b1 = hsum(bq1), b2 = hsum(bq2);
-                const float y1 = fmaf(-l10, b0, b1);
-                const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
-                const float z0 = b0 * inv_m00, z1 = y1 * id1, z2 = y2 * id2;
-                sq[2] = z2; sq[1] = fmaf(-l21, z2, z1); sq[0] = fmaf(-l20, sq[2], fmaf(-l10, sq[1], z0));
-                ll = fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
-            }
-            {
-                const float b0 = hsum(bu0), b1 = hsum(bu1), b2 = hsum(bu2);
-                const float y1 = fmaf(-l10, b0, b1);
-                const float y2 = fmaf(-l21, y1, fmaf(-l20, b0, b2));
-                const float z0 = b0 * inv_m00, z1 = y1 * id1, z2 = y2 * id2;
-                su[2] = z2; su[1] = fmaf(-l21, z2, z1); su[0] = fmaf(-l20, su[2], fmaf(-l10, su[1], z0));
-                ll += fmaf(b0, z0, fmaf(y1, z1, y2 * z2));
-            }
-            ll *= -0.5f;                              // -1/2 sum_S b_S . s_S                    (Eq. 6)
-            if (S3.z != 0.f) ll = CUDART_INF_F;       // non-positive pivot in this cell's M
+            pix_solve(A, C, inv_m00, sq, su, ll);
             if (MODE == MODE_VALUE) {
                 t3 = ll;
             } else if (MODE == MODE_GRAD) {
-                // g_theta = - sum_S s_{S,c} ( c_{S,theta} - P_theta . s_S )                      (Eq. 17)
-                const float P10 = S1.y, P11 = S1.z, P12 = S1.w, P20 = S2.x, P21 = S2.y, P22 = S2.z, P30 = S2.w, P31 = S3.x, P32 = S3.y;
-                const float eq1 = fmaf(-P12, sq[2], fmaf(-P11, sq[1], fmaf(-P10, sq[0], hsum(cq1))));
-                const float eu1 = fmaf(-P12, su[2], fmaf(-P11, su[1], fmaf(-P10, su[0], hsum(cu1))));
-                const float eq2 = fmaf(-P22, sq[2], fmaf(-P21, sq[1], fmaf(-P20, sq[0], hsum(cq2))));
-                const float eu2 = fmaf(-P22, su[2], fmaf(-P21, su[1], fmaf(-P20, su[0], hsum(cu2))));
-                const float eq3 = fmaf(-P32, sq[2], fmaf(-P31, sq[1], fmaf(-P30, sq[0], hsum(cq3))));
-                const float eu3 = fmaf(-P32, su[2], fmaf(-P31, su[1], fmaf(-P30, su[0], hsum(cu3))));
-                t0 = -fmaf(sq[1], eq1, su[1] * eu1);
-                t1 = -fmaf(sq[1], eq2, su[1] * eu2);
-                t2 = -fmaf(sq[2], eq3, su[2] * eu3);
+                pix_grad_terms(A, C, sq, su, t0, t1, t2);
                 t3 = ll;
             } else if (MODE == MODE_CMBVAR) {
                 t0 = sq[0]; t1 = su[0]; t2 = sq[0] * sq[0]; t3 = su[0] * su[0];

@@ -25,6 +25,7 @@ def torch_cuda():
 def path(request, monkeypatch):
     """Both forms of the fused kernel: 'cell' (k_like_cell where the plan allows it) and 'direct' (k_like forced)."""
     monkeypatch.setenv("CS_FORCE_DIRECT", "1" if request.param == "direct" else "0")
+    monkeypatch.setenv("CS_CELL_MIN_GROUP", "1")     # the library's default sends groups of < 12 entries to the direct kernel
     return request.param
 
 
@@ -475,6 +476,38 @@ def test_full_size_c5_nside128_sampled(torch_cuda):
     w = gen.make_config(4)
     assert w.batch == 256 and w.npix == 196608
     _sampled_full_size(w, w.params_jittered(seed=18), 6, 24)
+
+
+def test_kernel_forms_agree_bit_for_bit(torch_cuda, monkeypatch):
+    """The cell form and the direct form run the same arithmetic in the same order (csrc/cs_math.cuh): nll, gradient,
+    maps and the CMB variance are bitwise equal, which is what lets the library pick the form per group without
+    giving up batch invariance."""
+    import torch
+    w = _masked(gen.make_config(3, nside=32, batch=9, ndata=3))
+    params = w.params_jittered(seed=27)
+    out = {}
+    for form, env in (("cell", {"CS_FORCE_DIRECT": "0", "CS_CELL_MIN_GROUP": "1"}), ("direct", {"CS_FORCE_DIRECT": "1"})):
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        ctx, _ = make_ctx(w)
+        nll, grad = gpu_eval(ctx, params)
+        nll_v, _ = gpu_eval(ctx, params, want_grad=False)
+        smaps = gpu_maps(ctx, params)
+        var = torch.zeros(w.batch * w.nregion, dtype=torch.float64, device="cuda")
+        ctx.cmb_variance(var)
+        torch.cuda.synchronize()
+        out[form] = (nll, grad, nll_v, smaps, var.cpu().numpy())
+        ctx.close()
+    for a, b in zip(out["cell"], out["direct"]):
+        assert np.array_equal(a, b)
+
+
+def test_default_kernel_choice_mixes_both_forms(torch_cuda):
+    """Library defaults (no overrides): long groups on the cell kernel, short ones on the direct kernel, in one batch."""
+    w = gen.make_config(3, nside=32, batch=40, ndata=30)     # configuration 0: 30 entries, configuration 1: 10 entries
+    assert sorted(np.bincount(w.cfg_of).tolist()) == [10, 30]
+    _parity(w, w.params_jittered(seed=26), maps=False)
+    _parity(w, w.params_jittered(seed=26), entries=[0, 29, 30, 39])
 
 
 def test_full_size_c3_scan_sampled(torch_cuda):
