@@ -38,6 +38,8 @@ struct LikeParams {
     const Group *groups;
     const int32_t *elist;
     const int32_t *data_of;
+    const int32_t *skip;       // [batch] or null: entries with a non-zero flag are left out (line-search trials of
+                               // entries that already accepted a step); their outputs keep their previous values
     const int64_t *tab_off;    // [batch] first table row of entry
     const float *tab;
     double *partial;
@@ -133,13 +135,14 @@ __device__ __forceinline__ double exp_pow(double y) {
 __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const int64_t *__restrict__ param_off,
                                                 const int64_t *__restrict__ tab_off, const int32_t *__restrict__ cfg_of,
                                                 const CfgDev *__restrict__ cfgs, float *__restrict__ tab, int32_t batch,
-                                                int32_t *err, const TConst *__restrict__ tcg) {
+                                                int32_t *err, const TConst *__restrict__ tcg, const int32_t *__restrict__ skip) {
     __shared__ TConst tc;
     for (int i = threadIdx.x; i < (int)(sizeof(TConst) / 8); i += blockDim.x)
         reinterpret_cast<double *>(&tc)[i] = reinterpret_cast<const double *>(tcg)[i];
     __syncthreads();
     const int nfreq = tc.nfreq;
     for (int e = blockIdx.y; e < batch; e += gridDim.y) {
+        if (skip && skip[e] != 0) continue;
         const CfgDev *cp = cfgs + cfg_of[e];
         const int K0 = cp->K[0], K1 = cp->K[1], ktot = cp->ktot;
         const int id = blockIdx.x * blockDim.x + threadIdx.x;
@@ -277,6 +280,32 @@ __device__ __forceinline__ void tma_box_g2s(void *dst, const CUtensorMap *map, i
         : "memory");
 }
 
+// Per-entry arrays of a group in shared memory (table base, first data row, entry id).  With a skip mask the kept
+// entries are compacted in order; s_cnt[0] + s_cnt[1] is their number once the caller has synchronised the CTA.
+// Called by all threads of the CTA (contains a __syncthreads).
+static_assert(GROUP_MAX <= 64, "two warps compact a group");
+__device__ __forceinline__ void load_group(const LikeParams &P, const Group &grp, int nrows, int tid, const float **s_tab,
+                                           int32_t *s_drow, int32_t *s_ent, int32_t *s_cnt) {
+    int e = 0, pos = 0;
+    bool keep = false;
+    if (tid < 64) {
+        if (tid < grp.count) {
+            e = P.elist[grp.start + tid];
+            keep = !(P.skip && P.skip[e] != 0);
+        }
+        const unsigned b = __ballot_sync(0xffffffffu, keep);
+        pos = __popc(b & ((1u << (tid & 31)) - 1u));
+        if ((tid & 31) == 0) s_cnt[tid >> 5] = __popc(b);
+    }
+    __syncthreads();
+    if (keep) {
+        if (tid >= 32) pos += s_cnt[0];
+        s_ent[pos] = e;
+        s_drow[pos] = P.data_of[e] * nrows;
+        s_tab[pos] = P.tab + P.tab_off[e] * NROW;
+    }
+}
+
 template <int NF, int MODE>
 __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensorMap tmap, const LikeParams P) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -325,12 +354,7 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
     }
     const bool live = (k0 >= 0) && (k1 >= 0) && (k2 >= 0);
     if (kReduce) load_tile_plan<MODE>(P.maps, cfg, tile, tid, s_desc, s_slot, meta);
-    if (tid < grp.count) {
-        const int e = P.elist[grp.start + tid];
-        s_ent[tid] = e;
-        s_drow[tid] = P.data_of[e] * nrows;
-        s_tab[tid] = P.tab + P.tab_off[e] * NROW;
-    }
+    load_group(P, grp, nrows, tid, s_tab, s_drow, s_ent, meta + 12);
     float *wring = ring + warp * NST * 2 * NF * 32;
     uint64_t *wbar = bars + warp * NST;
     if (lane == 0) {
@@ -344,6 +368,7 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
             for (int r = nrows; r < 2 * NF; ++r) wring[(s * 2 * NF + r) * 32 + lane] = 0.f;
     }
     __syncthreads();
+    const int count = meta[12] + meta[13];   // entries of the group that are not skipped
 
     const int px0 = tile * TP + warp * 32;   // first pixel of this warp
     const bool warp_has_pixels = (int64_t)px0 < npix;
@@ -357,16 +382,16 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
         tma_box_g2s(wring + s * 2 * NF * 32, &tmap, px0, s_drow[i], &wbar[s], policy);
     };
     if (P.use_bulk && warp_has_pixels && lane == 0)
-        for (int i = 0; i < NST && i < grp.count; ++i) issue(i);
+        for (int i = 0; i < NST && i < count; ++i) issue(i);
 
     // row offsets (in floats) of this pixel's table rows inside an entry's table block
     const int r_fd = k0 * NROW, r_g = (cfg.K[0] + k1) * NROW, r_dg = (cfg.K[0] + cfg.K[1] + k1) * NROW,
               r_fs = (cfg.K[0] + 2 * cfg.K[1] + k2) * NROW;
 
-    for (int i = 0; i < grp.count; ++i) {
+    for (int i = 0; i < count; ++i) {
         const int s = i % NST;
         const float *tb = s_tab[i];
-        if (live && i + 1 < grp.count) {   // next entry's rows on their way to L1 while this entry is computed
+        if (live && i + 1 < count) {   // next entry's rows on their way to L1 while this entry is computed
             const float *tn = s_tab[i + 1];
             prefetch_row(tn + r_fd); prefetch_row(tn + r_g); prefetch_row(tn + r_fs);
             if (MODE == MODE_GRAD) prefetch_row(tn + r_dg);
@@ -436,13 +461,13 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
         }
         if (warp_has_pixels && P.use_bulk) {
             __syncwarp();   // every lane is done reading stage s: refill it with the entry NST ahead
-            if (lane == 0 && i + NST < grp.count) issue(i + NST);
+            if (lane == 0 && i + NST < count) issue(i + NST);
         }
         if (kReduce) {
             float *tm = sterm + (((i / EC) & 1) * EC + (i % EC)) * 4 * TROW;
             if (MODE != MODE_VALUE) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
             tm[so3] = t3;
-            if ((i % EC) == EC - 1 || i == grp.count - 1) {
+            if ((i % EC) == EC - 1 || i == count - 1) {
                 __syncthreads();
                 const int i0 = i - (i % EC), nent = (i % EC) + 1;
                 reduce_terms(sterm + ((i / EC) & 1) * EC * 4 * TROW, nent, tid, meta, s_desc, s_slot, s_ent + i0, P.partial, P.PS);
@@ -463,8 +488,9 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
 __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
                                                const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
                                                const int64_t *__restrict__ param_off, int32_t nregion, int32_t want_grad,
-                                               double *__restrict__ nll, double *__restrict__ grad) {
+                                               double *__restrict__ nll, double *__restrict__ grad, const int32_t *__restrict__ skip) {
     const int e = blockIdx.y, lane = threadIdx.x & 31;
+    if (skip && skip[e] != 0) return;
     const CfgDev *c = cfgs + cfg_of[e];
     const int K0 = c->K[0], K1 = c->K[1], ktot = want_grad ? c->ktot : 0;
     const int kpad = (ktot + 31) & ~31;

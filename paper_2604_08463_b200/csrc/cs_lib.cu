@@ -114,6 +114,7 @@ struct cs_ctx {
     int32_t *d_err = nullptr;
     TConst *d_tc = nullptr;             // device copy of tc (k_tables stages it in shared memory)
     int64_t launches = 0;
+    const int32_t *skip = nullptr;      // set by cs_optimize around line-search trials: entries that already accepted
     bool tables_built = false;
     int32_t cell_min_group = CELL_MIN_GROUP;   // CS_CELL_MIN_GROUP overrides (tests run the cell kernel on 1-entry groups)
     bool force_direct = false;          // CS_FORCE_DIRECT=1 in the environment at cs_create: never use the cell kernel (tests)
@@ -373,6 +374,7 @@ LikeParams base_params(cs_ctx *c) {
     P.groups = c->d_groups;
     P.elist = c->d_elist;
     P.data_of = c->d_data_of;
+    P.skip = c->skip;
     P.tab_off = c->d_tab_off;
     P.tab = c->d_tab;
     P.partial = c->d_partial;
@@ -682,7 +684,7 @@ int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
     cudaStream_t st = (cudaStream_t)stream;
     dim3 block(256);
     dim3 grid((4 * c->ktot_max + 255) / 256, std::min(c->batch, 65535));
-    k_tables<<<grid, block, 0, st>>>(params, c->d_param_off, c->d_tab_off, c->d_cfg_of, c->d_cfgs, c->d_tab, c->batch, c->d_err, c->d_tc);
+    k_tables<<<grid, block, 0, st>>>(params, c->d_param_off, c->d_tab_off, c->d_cfg_of, c->d_cfgs, c->d_tab, c->batch, c->d_err, c->d_tc, c->skip);
     c->launches++;
     CK(cudaGetLastError());
     c->tables_built = true;
@@ -695,7 +697,8 @@ static int merge_launch(cs_ctx *c, double *nll, double *grad, cudaStream_t st) {
         const int nout = (grad ? ((c->ktot_max + 31) & ~31) : 0) + 32 * c->nregion;   // virtual threads, see k_merge
         dim3 grid((nout + 255) / 256, nb);
         k_merge<<<grid, 256, 0, st>>>(c->d_partial + (int64_t)e0 * c->PS, c->PS, c->d_maps, c->d_cfgs, c->d_cfg_of + e0,
-                                     c->d_param_off + e0, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad);
+                                     c->d_param_off + e0, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad,
+                                     c->skip ? c->skip + e0 : nullptr);
         c->launches++;
     }
     CK(cudaGetLastError());
@@ -782,6 +785,27 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
     if (rc) return rc;
     if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || !(opt->ls_noise >= 0) || c->batch > 65535) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
+    // the legacy default stream cannot be captured into a graph: fork onto an internal stream and join at the end
+    cudaStream_t caller = st;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    const bool forked = (st == nullptr || st == cudaStreamLegacy);
+    if (forked) {
+        if (!c->comp_stream) CK(cudaStreamCreateWithFlags(&c->comp_stream, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&ev_fork, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&ev_join, cudaEventDisableTiming));
+        CK(cudaEventRecord(ev_fork, caller));
+        CK(cudaStreamWaitEvent(c->comp_stream, ev_fork, 0));
+        st = c->comp_stream;
+    }
+    struct Join {   // runs on every return path
+        bool on; cudaStream_t from, to; cudaEvent_t a, b;
+        ~Join() {
+            if (!on) return;
+            cudaEventRecord(b, from);
+            cudaStreamWaitEvent(to, b, 0);
+            cudaEventDestroy(a); cudaEventDestroy(b);
+        }
+    } join{forked, st, caller, ev_fork, ev_join};
     if (!c->opt.y) {
         if ((rc = opt_alloc(c->opt, c->nparam, c->batch, c->nregion, &c->opt_bytes))) return rc == 1 ? CS_ENOMEM : CS_ECUDA;
     }
@@ -789,18 +813,56 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
     OptHyper hy{opt->lr, opt->beta1, opt->beta2, opt->eps, opt->ls_c1, opt->safe_lo, opt->safe_hi, opt->ls_noise, opt->ls_max};
     OptWork &w = c->opt;
     opt_init(w, sh, params, lower, upper, st); c->launches += 1;
-    for (int it = 0; it < opt->iters; ++it) {
+    // one iteration of Alg. 1; nothing in it depends on the host (the iteration counter lives on the device)
+    auto iteration = [&]() -> int {
+        int r;
         // value + gradient at the current point x
-        if ((rc = cs_build_sed_tables(c, w.x, st))) return rc;
-        if ((rc = cs_spectral_like_grad(c, w.nll_reg, w.grad, st))) return rc;
-        opt_direction(w, sh, hy, it, st); c->launches += 1;
+        if ((r = cs_build_sed_tables(c, w.x, st))) return r;
+        if ((r = cs_spectral_like_grad(c, w.nll_reg, w.grad, st))) return r;
+        opt_direction(w, sh, hy, st); c->launches += 1;
         for (int ls = 0; ls < opt->ls_max; ++ls) {
             opt_trial_point(w, sh, st); c->launches += 1;
-            if ((rc = cs_build_sed_tables(c, w.xt, st))) return rc;
-            if ((rc = cs_spectral_like_grad(c, w.nll_reg_t, nullptr, st))) return rc;
+            c->skip = w.accepted;   // entries that already accepted a step sit this trial out
+            r = cs_build_sed_tables(c, w.xt, st);
+            if (!r) r = cs_spectral_like_grad(c, w.nll_reg_t, nullptr, st);
+            c->skip = nullptr;
+            if (r) return r;
             opt_ls_update(w, sh, hy, st); c->launches += 1;
         }
         opt_commit(w, sh, st); c->launches += 1;
+        return CS_OK;
+    };
+    // The body is captured once into a CUDA graph and replayed: a step of a small batch is launch-bound (config 2:
+    // ~30 kernels of a few microseconds each).  If the caller's stream is itself being captured, or the fused-kernel
+    // timer is on, the kernels are enqueued directly.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    cudaStreamIsCapturing(st, &cap);
+    bool replayed = false;
+    if (opt->iters > 1 && cap == cudaStreamCaptureStatusNone && !c->prof_on) {
+        if (opt->iters > 0 && (rc = iteration())) return rc;     // first iteration directly: sets function attributes, warms up
+        const int64_t l0 = c->launches;
+        cudaGraph_t graph = nullptr;
+        cudaGraphExec_t exec = nullptr;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            const int r = iteration();
+            const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+            if (r == CS_OK && ce == cudaSuccess && graph && cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess) {
+                const int64_t per_iter = c->launches - l0;
+                for (int it = 1; it < opt->iters; ++it) CK(cudaGraphLaunch(exec, st));
+                c->launches = l0 + per_iter * (opt->iters - 1);
+                replayed = true;
+            }
+            if (exec) cudaGraphExecDestroy(exec);
+            if (graph) cudaGraphDestroy(graph);
+            if (!replayed) c->launches = l0;
+        }
+        if (!replayed) cudaGetLastError();
+        if (!replayed)
+            for (int it = 1; it < opt->iters; ++it)
+                if ((rc = iteration())) return rc;
+    } else {
+        for (int it = 0; it < opt->iters; ++it)
+            if ((rc = iteration())) return rc;
     }
     // final objective at the result
     if ((rc = cs_build_sed_tables(c, w.x, st))) return rc;

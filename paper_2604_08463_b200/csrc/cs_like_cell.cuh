@@ -215,18 +215,15 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         for (int s = 0; s < NR; ++s) { mbar_init(&full_r[s], 1); mbar_init(&empty_r[s], CELL_CAP / 32 + TP / 32); }   // one builder group + consumers
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (tid < grp.count) {
-        const int e = P.elist[grp.start + tid];
-        s_ent[tid] = e;
-        s_drow[tid] = P.data_of[e] * nrows;
-        s_tab[tid] = P.tab + P.tab_off[e] * NROW;
-    }
+    load_group(P, grp, nrows, tid, s_tab, s_drow, s_ent, meta + 12);
     if (kReduce && tid < TP) load_chunk_plan<MODE>(P.maps, cfg, tile, tid, s_cdesc, s_sdesc, s_slot, meta);
     if (NF > 15 && P.nfreq < NF) {   // generic path: rows beyond nfreq are never copied; they must read as zero
         for (int s = 0; s < ND; ++s)
             for (int r = nrows * TP + tid; r < STAGE; r += CELL_THREADS) ring[s * STAGE + r] = 0.f;
     }
     __syncthreads();
+    const int count = meta[12] + meta[13];   // entries of the group that are not skipped
+    if (count == 0) return;
 
     if (warp == CELL_THREADS / 32 - 1) {
         // ---------------- loader warp ----------------
@@ -251,7 +248,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         };
         const uint64_t policy = P.evict_first ? policy_evict_first() : policy_evict_normal();
         fetch(0);
-        for (int i = 0; i < grp.count; ++i) {
+        for (int i = 0; i < count; ++i) {
             const int sr = i % NR, s = i % ND;
             mbar_wait_relaxed(&empty_r[sr], (uint32_t)(((i / NR) & 1) ^ 1), 250);
             float *dst = rowbuf + sr * ROW_CAP * RSTRIDE;
@@ -262,7 +259,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&full_r[sr]);
-            if (i + 1 < grp.count) fetch(i + 1);   // in flight while lane 0 waits for a data slot
+            if (i + 1 < count) fetch(i + 1);   // in flight while lane 0 waits for a data slot
             if (P.use_bulk) {
                 if (lane == 0) {
                     mbar_wait_relaxed(&empty_d[s], (uint32_t)(((i / ND) & 1) ^ 1), 250);
@@ -289,7 +286,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         // reducer warp r owns term-ring slot r and the entries i = r (mod NT)
         static_assert(NRED / 32 == NT, "one reducer warp per term-ring slot");
         const int s = warp - (TP + NBUILD) / 32;
-        for (int i = s; i < grp.count; i += NT) {
+        for (int i = s; i < count; i += NT) {
             terms_wait(s);
             reduce_entry(sterm + s * 4 * TROW, lane, meta, s_cdesc, s_sdesc, s_slot, csum + s * CHUNK_CAP,
                          P.partial + (int64_t)s_ent[i] * P.PS);
@@ -304,7 +301,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         const int c0 = cfg.cellptr[tile], ncell = cfg.cellptr[tile + 1] - c0;
         int4 rows = make_int4(0, 0, 0, 0);
         if (c < ncell) rows = *reinterpret_cast<const int4 *>(cfg.cellrows + 4 * (int64_t)(c0 + c));
-        for (int i = g; i < grp.count; i += NBG) {
+        for (int i = g; i < count; i += NBG) {
             const int s = i % NC, sr = i % NR;
             CellRows R;
             mbar_wait_relaxed(&full_r[sr], (uint32_t)((i / NR) & 1));
@@ -351,7 +348,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
     const float2 *lns2 = reinterpret_cast<const float2 *>(P.kc.lns);
     const float inv_m00 = P.kc.inv_m00;
 
-    for (int i = 0; i < grp.count; ++i) {
+    for (int i = 0; i < count; ++i) {
         const int sd = i % ND, sc = i % NC, sr = i % NR;
         mbar_wait(&full_c[sc], (uint32_t)((i / NC) & 1));   // the builders waited for full_r[sr]: the rows are there too
         mbar_wait(&full_d[sd], (uint32_t)((i / ND) & 1));

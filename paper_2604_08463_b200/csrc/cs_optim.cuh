@@ -25,6 +25,7 @@ struct OptWork {
     double *L0 = nullptr, *gd = nullptr, *amax = nullptr, *alpha = nullptr, *alpha_acc = nullptr, *cscale = nullptr;
     long long *ilim = nullptr;
     int32_t *accepted = nullptr;
+    int32_t *iter = nullptr;   // device-side iteration counter (the loop body is replayed as a CUDA graph)
 };
 
 struct OptShape {
@@ -41,7 +42,7 @@ struct OptHyper {
 inline void opt_free(OptWork &w) {
     cudaFree(w.y); cudaFree(w.x); cudaFree(w.xt); cudaFree(w.dir); cudaFree(w.m); cudaFree(w.v); cudaFree(w.grad);
     cudaFree(w.pivot); cudaFree(w.nll_reg); cudaFree(w.nll_reg_t); cudaFree(w.L0); cudaFree(w.gd); cudaFree(w.amax);
-    cudaFree(w.alpha); cudaFree(w.alpha_acc); cudaFree(w.cscale); cudaFree(w.ilim); cudaFree(w.accepted);
+    cudaFree(w.alpha); cudaFree(w.alpha_acc); cudaFree(w.cscale); cudaFree(w.ilim); cudaFree(w.accepted); cudaFree(w.iter);
     w = OptWork();
 }
 
@@ -67,6 +68,7 @@ inline int opt_alloc(OptWork &w, int64_t nparam, int32_t batch, int32_t nregion,
     ok &= cudaMalloc((void **)&w.cscale, nb) == cudaSuccess;
     ok &= cudaMalloc((void **)&w.ilim, (size_t)batch * sizeof(long long)) == cudaSuccess;
     ok &= cudaMalloc((void **)&w.accepted, (size_t)batch * sizeof(int32_t)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.iter, sizeof(int32_t)) == cudaSuccess;
     if (!ok) { opt_free(w); return 1; }
     *bytes = (int64_t)(7 * np + nparam + 2 * nb * nregion + 7 * nb + (size_t)batch * 4);
     return 0;
@@ -108,6 +110,7 @@ __device__ __forceinline__ void block_argbest(double &val, long long &idx, bool 
 // A1 (L509-L513): map the start into [0,1], set the pivots, clear the AdaBelief moments.
 __global__ void k_opt_init(OptWork w, int64_t nparam, const double *params, int32_t batch) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) *w.iter = 0;
     if (i < batch) w.cscale[i] = 1.0;
     if (i >= nparam) return;
     const double l = w.lo[i], u = w.hi[i];
@@ -120,7 +123,8 @@ __global__ void k_opt_init(OptWork w, int64_t nparam, const double *params, int3
 }
 
 // Alg. 1 lines 3-17 for one entry per CTA.
-__global__ void __launch_bounds__(OPT_THREADS) k_opt_direction(OptWork w, OptShape sh, OptHyper hy, int32_t iter) {
+__global__ void __launch_bounds__(OPT_THREADS) k_opt_direction(OptWork w, OptShape sh, OptHyper hy) {
+    const int32_t iter = *w.iter;
     __shared__ double shv[OPT_THREADS];
     __shared__ long long shi[OPT_THREADS];
     const int e = blockIdx.x, tid = threadIdx.x;
@@ -221,6 +225,7 @@ __global__ void k_opt_ls(OptWork w, OptShape sh, OptHyper hy) {
 // lines 19-25: move, pin the limiting parameter if the step reached alpha_max
 __global__ void k_opt_commit(OptWork w, OptShape sh) {
     const int e = blockIdx.y;
+    if (blockIdx.x == 0 && e == 0 && threadIdx.x == 0) *w.iter += 1;   // k_opt_direction of this iteration is done
     const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= sh.param_off[e + 1]) return;
     const double a = w.accepted[e] ? w.alpha_acc[e] : 0.0;
@@ -250,8 +255,8 @@ inline void opt_init(OptWork &w, const OptShape &sh, const double *params, const
     const int64_t n = sh.nparam > sh.batch ? sh.nparam : sh.batch;
     k_opt_init<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w, sh.nparam, params, sh.batch);
 }
-inline void opt_direction(OptWork &w, const OptShape &sh, const OptHyper &hy, int iter, cudaStream_t st) {
-    k_opt_direction<<<sh.batch, OPT_THREADS, 0, st>>>(w, sh, hy, iter);
+inline void opt_direction(OptWork &w, const OptShape &sh, const OptHyper &hy, cudaStream_t st) {
+    k_opt_direction<<<sh.batch, OPT_THREADS, 0, st>>>(w, sh, hy);
 }
 inline void opt_trial_point(OptWork &w, const OptShape &sh, cudaStream_t st) {
     dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
