@@ -91,7 +91,10 @@ CS_API int cs_destroy(cs_ctx *ctx);
  * beta_s) (host [ncfg,3]).  A cluster id of -1 in any of a configuration's three maps masks the pixel for that
  * configuration (L211).  region_idx (any, [npix], values < nregion) or NULL with nregion = 1 splits nll by sky
  * region (L269).  Validates -1 <= id < K bit-exactly (CS_EINDEX otherwise, context unchanged), copies the maps
- * (the caller may free them) and builds the per-tile segment plan of the ordered cluster reduction. */
+ * (the caller may free them) and builds the per-tile segment plan of the ordered cluster reduction and, per
+ * configuration, the per-tile cell plan (distinct cluster triples) of the cell form of the fused kernel.
+ * Environment, read at cs_create (tests): CS_FORCE_DIRECT=1 never uses the cell form; CS_CELL_MIN_GROUP=n sets the
+ * shortest group of entries that runs on it (default 12).  Both forms give the same bits. */
 CS_API int cs_set_clusters(cs_ctx *ctx, int32_t nmap, const int32_t *maps, const int32_t *Kmap,
                     int32_t ncfg, const int32_t *cfg_maps, const uint8_t *region_idx, int32_t nregion);
 
@@ -127,7 +130,10 @@ CS_API int cs_cmb_variance(cs_ctx *ctx, double *var, void *stream);
 
 /* a5: device-resident fixed-budget AdaTopK (Alg. 1) on every entry independently; calls only
  * cs_build_sed_tables and cs_spectral_like_grad.  params dev in: start, out: result; lower/upper dev, same layout;
- * nll_final dev [batch] (summed over regions) or NULL.  No host synchronisation. */
+ * nll_final dev [batch] (summed over regions) or NULL.  No host synchronisation.  The iteration body is captured
+ * into a CUDA graph and replayed unless `stream` is itself being captured; on the legacy default stream the work is
+ * forked onto an internal stream and joined back before the call returns (still asynchronous to the host).
+ * Line-search trials skip the entries that have already accepted a step. */
 CS_API int cs_optimize(cs_ctx *ctx, double *params, const double *lower, const double *upper, const cs_opt *opt,
                 double *nll_final, void *stream);
 CS_API void cs_opt_defaults(cs_opt *opt);

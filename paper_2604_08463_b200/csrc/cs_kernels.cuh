@@ -327,8 +327,6 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
     const int64_t p = (int64_t)tile * TP + tid;
     const int nrows = 2 * P.nfreq;
     constexpr bool kReduce = (MODE != MODE_MAPS);
-    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;   // value-only: only the ll / region term is reduced
-
     int k0 = -1, k1 = -1, k2 = -1;
     // float offset of this pixel's slot in each term row: its rank in the tile's (cluster, pixel) order of the
     // reducing map, or the dump slot TP when the pixel has no cluster there
