@@ -77,9 +77,9 @@ typedef struct cs_opt {
     double beta1, beta2, eps;
     double ls_c1;       /* Armijo constant */
     double safe_lo, safe_hi; /* dynamic rescale range for |g_proj| (A4, L541) */
-    double ls_noise;    /* Armijo slack, relative to |L|: accept when L_trial <= L + ls_c1 a g.d + ls_noise |L|.  The
-                           per-pixel likelihood is fp32, so differences of the objective below ~3e-8 |L| are evaluation
-                           noise; 0 = strict decrease of the computed objective (R13) */
+    double ls_noise;    /* Armijo slack, relative to |L|: accept when L_trial <= L + ls_c1 a g.d + ls_noise |L|, with
+                           L = 1/2 chi^2 of the GLS residual (cs_spectral_misfit), whose fp32 evaluation noise is about
+                           1e-6 relative; 0 = strict decrease of the computed objective (R13) */
 } cs_opt;
 
 /* Create a context for `model`.  Allocates only small constant tables.  *out is NULL on failure. */
@@ -118,6 +118,13 @@ CS_API int cs_build_sed_tables(cs_ctx *ctx, const double *params, void *stream);
  * built.  nll dev [batch*nregion] fp64; grad dev fp64 (parameter layout) or NULL for value only.
  * Results are bitwise reproducible and independent of how entries are grouped into batches. */
 CS_API int cs_spectral_like_grad(cs_ctx *ctx, double *nll, double *grad, void *stream);
+
+/* chi^2 of the GLS residual per entry and region, chi2 dev [batch*nregion] fp64:
+ *     chi2 = sum_p sum_S sum_f Ninv_f (d_S - A s_S)_f^2  =  2 nll + d^T N^-1 d            (Eq. 3 at the GLS solution, L66)
+ * for the tables last built.  It differs from 2 nll by a parameter-independent constant but is evaluated from the
+ * residual itself, so small changes of the objective are resolved (nll = -1/2 b.s carries the fp32 rounding of a number
+ * ~1e5 times larger); cs_optimize runs its line search on it. */
+CS_API int cs_spectral_misfit(cs_ctx *ctx, double *chi2, void *stream);
 
 /* a4 (Eq. 5/8): GLS component maps s dev [nsel, 3, 2, npix] fp32 (cmb, dust@nu0d, sync@nu0s; Q,U) for entries
  * `entries` (host [nsel]) or all entries in order when entries == NULL (then nsel must equal batch).  Masked

@@ -13,7 +13,7 @@ OK, EINVAL, EINDEX, EDOMAIN, ESINGULAR, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5, -
 UNITS_KCMB, UNITS_LITERAL = 0, 1
 
 EXPORTS = ["cs_create", "cs_destroy", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
-           "cs_build_sed_tables", "cs_spectral_like_grad", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
+           "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
            "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
 
@@ -61,6 +61,7 @@ def lib():
         "cs_param_offsets": (C.c_int, [vp, vp]),
         "cs_build_sed_tables": (C.c_int, [vp, vp, vp]),
         "cs_spectral_like_grad": (C.c_int, [vp, vp, vp, vp]),
+        "cs_spectral_misfit": (C.c_int, [vp, vp, vp]),
         "cs_component_maps": (C.c_int, [vp, i32, vp, vp, vp]),
         "cs_cmb_variance": (C.c_int, [vp, vp, vp]),
         "cs_optimize": (C.c_int, [vp, vp, vp, vp, C.POINTER(CsOpt), vp, vp]),
@@ -185,6 +186,9 @@ class Context:
 
     def spectral_like_grad(self, nll, grad=None, stream=None):
         _chk(lib().cs_spectral_like_grad(self._h, _ptr(nll), _ptr(grad), _stream(stream)), "cs_spectral_like_grad")
+
+    def spectral_misfit(self, chi2, stream=None):
+        _chk(lib().cs_spectral_misfit(self._h, _ptr(chi2), _stream(stream)), "cs_spectral_misfit")
 
     def component_maps(self, s, entries=None, stream=None):
         if entries is None:

@@ -82,6 +82,7 @@ struct KConst {
     float lnd[NROW];   // ln(nu_f/nu0d)
     float lnsw[NROW];  // ln(nu_f/nu0s) * w_f
     float lns[NROW];   // ln(nu_f/nu0s)
+    float invw[NROW];  // 1 / w_f (0 beyond nfreq)
     float inv_m00;     // 1 / sum_f w_f
     float m00;
 };

@@ -23,6 +23,11 @@ constexpr int MODE_VALUE = 0;   // ll only (line search)
 constexpr int MODE_GRAD = 1;    // ll + three gradient terms
 constexpr int MODE_MAPS = 2;    // component maps
 constexpr int MODE_CMBVAR = 3;  // sums for the CMB-variance metric (Eq. 10)
+constexpr int MODE_CHI2 = 4;    // chi^2 of the GLS residual per region (accurate objective differences for the line search)
+template <int MODE>
+struct ModeTraits {
+    static constexpr bool region_only = (MODE == MODE_VALUE || MODE == MODE_CHI2);   // only term 3 is reduced
+};
 
 constexpr int NST = 2;   // stages of each warp's data ring (both in flight while the warp computes)
 constexpr int EC = 4;    // entries buffered between reduce phases
@@ -225,7 +230,7 @@ constexpr int TROW = TP + 4;   // floats per term row: TP ranks + a dump slot fo
 template <int MODE>
 __device__ __forceinline__ void load_tile_plan(const MapDev *__restrict__ maps, const CfgDev &cfg, int tile, int tid,
                                                uint16_t *s_desc, int32_t *s_slot, int32_t *meta) {
-    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;
+    constexpr int T0 = ModeTraits<MODE>::region_only ? 3 : 0;
     if (tid < 4) {
         const int t = tid;
         const int mi = (MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t];
@@ -341,7 +346,7 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
                 const int r = P.maps[m3].rank[p];
                 so0 = 0 * TROW + r; so1 = 1 * TROW + r; so2 = 2 * TROW + r; so3 = 3 * TROW + r;
             } else {
-                if (MODE != MODE_VALUE) {
+                if (!ModeTraits<MODE>::region_only) {
                     if (k0 >= 0) so0 = 0 * TROW + P.maps[cfg.map[0]].rank[p];
                     if (k1 >= 0) so1 = 1 * TROW + P.maps[cfg.map[1]].rank[p];
                     if (k2 >= 0) so2 = 2 * TROW + P.maps[cfg.map[2]].rank[p];
@@ -442,6 +447,26 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
             pix_solve(A, C, P.kc.inv_m00, sq, su, ll);
             if (MODE == MODE_VALUE) {
                 t3 = ll;
+            } else if (MODE == MODE_CHI2) {
+                const float2 *iw2 = reinterpret_cast<const float2 *>(P.kc.invw);
+                ChiCoef K;
+                chi_coef(sq, su, K);
+                ChiSums X;
+                X.q = X.u = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 vFd = __ldg(rFd + q), vG = __ldg(rG + q), vFs = __ldg(rFs + q);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int j = 2 * q + h;
+                        const float2 Fd = h ? make_float2(vFd.z, vFd.w) : make_float2(vFd.x, vFd.y);
+                        const float2 G = h ? make_float2(vG.z, vG.w) : make_float2(vG.x, vG.y);
+                        const float2 as = h ? make_float2(vFs.z, vFs.w) : make_float2(vFs.x, vFs.y);
+                        const float2 wd = mul2(w2[j], mul2(Fd, G));   // as in cell_pair
+                        pix_chi2_pair(X, K, wd, as, w2[j], iw2[j], in.dq(j), in.du(j));
+                    }
+                }
+                t3 = (C.bad != 0.f) ? CUDART_INF_F : hsum(X.q) + hsum(X.u);
             } else if (MODE == MODE_GRAD) {
                 pix_grad_terms(A, C, sq, su, t0, t1, t2);
                 t3 = ll;
@@ -463,7 +488,7 @@ __global__ void __launch_bounds__(TP, 2) k_like(const __grid_constant__ CUtensor
         }
         if (kReduce) {
             float *tm = sterm + (((i / EC) & 1) * EC + (i % EC)) * 4 * TROW;
-            if (MODE != MODE_VALUE) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
+            if (!ModeTraits<MODE>::region_only) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
             tm[so3] = t3;
             if ((i % EC) == EC - 1 || i == count - 1) {
                 __syncthreads();

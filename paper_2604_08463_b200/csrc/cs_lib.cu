@@ -593,6 +593,7 @@ int cs_set_data(cs_ctx *c, int32_t ndata, const float *d, const float *ninv) {
         c->kc.lnd[f] = (float)c->tc.lnd[f];
         c->kc.lnsw[f] = (float)(c->tc.lns[f] * (double)w[f]);
         c->kc.lns[f] = (float)c->tc.lns[f];
+        c->kc.invw[f] = 1.0f / w[f];
         m00f += w[f];
     }
     (void)m00f;
@@ -716,6 +717,16 @@ int cs_spectral_like_grad(cs_ctx *c, double *nll, double *grad, void *stream) {
     return merge_launch(c, nll, grad, st);
 }
 
+int cs_spectral_misfit(cs_ctx *c, double *chi2, void *stream) {
+    int rc = ready(c);
+    if (rc) return rc;
+    if (!chi2 || !c->tables_built) return CS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    LikeParams P = base_params(c);
+    if ((rc = launch_like<MODE_CHI2>(c, P, 0, c->ngroup, c->ngroup_cell, st))) return rc;
+    return merge_launch(c, chi2, nullptr, st);
+}
+
 int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s, void *stream) {
     int rc = ready(c);
     if (rc) return rc;
@@ -776,7 +787,7 @@ void cs_opt_defaults(cs_opt *o) {
     if (!o) return;
     o->iters = 200; o->ls_max = 8;
     o->lr = 0.02; o->beta1 = 0.9; o->beta2 = 0.999; o->eps = 1e-16;
-    o->ls_c1 = 1e-4; o->safe_lo = 1e-15; o->safe_hi = 1e15; o->ls_noise = 3e-8;
+    o->ls_c1 = 1e-4; o->safe_lo = 1e-15; o->safe_hi = 1e15; o->ls_noise = 1e-6;
 }
 
 int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *upper, const cs_opt *opt, double *nll_final,
@@ -813,6 +824,10 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
     OptHyper hy{opt->lr, opt->beta1, opt->beta2, opt->eps, opt->ls_c1, opt->safe_lo, opt->safe_hi, opt->ls_noise, opt->ls_max};
     OptWork &w = c->opt;
     opt_init(w, sh, params, lower, upper, st); c->launches += 1;
+    // the line search compares 1/2 chi^2 of the GLS residual (cs_spectral_misfit): its value at the start
+    if ((rc = cs_build_sed_tables(c, w.x, st))) return rc;
+    if ((rc = cs_spectral_misfit(c, w.nll_reg_t, st))) return rc;
+    opt_set_L(w, sh, st); c->launches += 1;
     // one iteration of Alg. 1; nothing in it depends on the host (the iteration counter lives on the device)
     auto iteration = [&]() -> int {
         int r;
@@ -824,7 +839,7 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
             opt_trial_point(w, sh, st); c->launches += 1;
             c->skip = w.accepted;   // entries that already accepted a step sit this trial out
             r = cs_build_sed_tables(c, w.xt, st);
-            if (!r) r = cs_spectral_like_grad(c, w.nll_reg_t, nullptr, st);
+            if (!r) r = cs_spectral_misfit(c, w.nll_reg_t, st);
             c->skip = nullptr;
             if (r) return r;
             opt_ls_update(w, sh, hy, st); c->launches += 1;

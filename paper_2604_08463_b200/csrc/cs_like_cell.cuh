@@ -77,7 +77,7 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
 template <int MODE>
 __device__ __forceinline__ void load_chunk_plan(const MapDev *__restrict__ maps, const CfgDev &cfg, int tile, int tid,
                                                 uint16_t *s_cdesc, uint16_t *s_sdesc, int32_t *s_slot, int32_t *meta) {
-    constexpr int T0 = (MODE == MODE_VALUE) ? 3 : 0;
+    constexpr int T0 = ModeTraits<MODE>::region_only ? 3 : 0;
     int sbase = 0, cbase = 0;
 #pragma unroll
     for (int t = T0; t < 4; ++t) {
@@ -355,6 +355,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
         PixSums A;
         pix_sums_zero(A);
         float4 S0 = make_float4(0.f, 0.f, 0.f, 0.f), S1 = S0, S2 = S0, S3 = S0;
+        float chi = 0.f;
         if (live) {
             const float *st = ring + sd * STAGE + tid;
             const float4 *cell = reinterpret_cast<const float4 *>(cells + (sc * CELL_CAP + cid) * CSTRIDE);
@@ -379,6 +380,32 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
             S0 = cell[4]; S1 = cell[5];
             if (kGrad) S2 = cell[6];
             S3 = cell[7];
+            if (MODE == MODE_CHI2) {   // second pass over the bands while the stages are still held: chi^2 of the residual
+                CellScal C;
+                C.l10 = S0.x; C.l20 = S0.y; C.l21 = S0.z; C.id1 = S0.w; C.id2 = S1.x; C.bad = S3.z;
+                C.P10 = C.P11 = C.P12 = C.P20 = C.P21 = C.P22 = C.P30 = C.P31 = C.P32 = 0.f;
+                float sq[3], su[3], ll;
+                pix_solve(A, C, inv_m00, sq, su, ll);
+                const float2 *iw2 = reinterpret_cast<const float2 *>(P.kc.invw);
+                ChiCoef K;
+                chi_coef(sq, su, K);
+                ChiSums X;
+                X.q = X.u = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 WD = cell[q], FS = rfs[q];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int j = 2 * q + h;
+                        const float2 dq = make_float2(st[(4 * j + 0) * TP], (2 * j + 1 < NF) ? st[(4 * j + 2) * TP] : 0.f);
+                        const float2 du = make_float2(st[(4 * j + 1) * TP], (2 * j + 1 < NF) ? st[(4 * j + 3) * TP] : 0.f);
+                        const float2 wd = h ? make_float2(WD.z, WD.w) : make_float2(WD.x, WD.y);
+                        const float2 fs = h ? make_float2(FS.z, FS.w) : make_float2(FS.x, FS.y);
+                        pix_chi2_pair(X, K, wd, fs, w2[j], iw2[j], dq, du);
+                    }
+                }
+                chi = (C.bad != 0.f) ? CUDART_INF_F : hsum(X.q) + hsum(X.u);
+            }
         }
         __syncwarp();   // every lane has read its data and cell rows: hand the slots back
         if (lane == 0) { mbar_arrive(&empty_d[sd]); mbar_arrive(&empty_c[sc]); mbar_arrive(&empty_r[sr]); }
@@ -390,9 +417,11 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
             C.P10 = S1.y; C.P11 = S1.z; C.P12 = S1.w; C.P20 = S2.x; C.P21 = S2.y; C.P22 = S2.z; C.P30 = S2.w;
             C.P31 = S3.x; C.P32 = S3.y; C.bad = S3.z;
             float sq[3], su[3], ll;
-            pix_solve(A, C, inv_m00, sq, su, ll);
+            if (MODE != MODE_CHI2) pix_solve(A, C, inv_m00, sq, su, ll);
             if (MODE == MODE_VALUE) {
                 t3 = ll;
+            } else if (MODE == MODE_CHI2) {
+                t3 = chi;
             } else if (MODE == MODE_GRAD) {
                 pix_grad_terms(A, C, sq, su, t0, t1, t2);
                 t3 = ll;
@@ -412,7 +441,7 @@ __global__ void __launch_bounds__(CELL_THREADS, 1) k_like_cell(const __grid_cons
             const int st = i % NT;
             mbar_wait(&empty_t[st], (uint32_t)(((i / NT) & 1) ^ 1));
             float *tm = sterm + st * 4 * TROW;
-            if (MODE != MODE_VALUE) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
+            if (!ModeTraits<MODE>::region_only) { tm[so0] = t0; tm[so1] = t1; tm[so2] = t2; }
             tm[so3] = t3;
             terms_arrive(st);
         }

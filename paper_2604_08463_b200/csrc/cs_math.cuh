@@ -136,6 +136,28 @@ __device__ __forceinline__ void pix_grad_terms(const PixSums &A, const CellScal 
     g_bs = -fmaf(sq[2], eq3, su[2] * eu3);
 }
 
+// chi^2 of the pixel's GLS residual, a second pass over the bands once s is known: r_S = d_S - A s_S,
+// chi2 = sum_S sum_f w_f r_{S,f}^2 = 2 nll + d^T N^-1 d.  Unlike -1/2 b.s (a difference of large numbers once the
+// parameter-independent d^T N^-1 d is taken out) it resolves small changes of the objective: the line search runs on it.
+struct ChiSums {
+    float2 q, u;
+};
+struct ChiCoef {   // -s_{S,c} duplicated into both lanes
+    float2 q0, q1, q2, u0, u1, u2;
+};
+__device__ __forceinline__ void chi_coef(const float (&sq)[3], const float (&su)[3], ChiCoef &K) {
+    K.q0 = dup2(-sq[0]); K.q1 = dup2(-sq[1]); K.q2 = dup2(-sq[2]);
+    K.u0 = dup2(-su[0]); K.u1 = dup2(-su[1]); K.u2 = dup2(-su[2]);
+}
+// wd = w a_d of the pixel's cell (a_d is recovered as wd / w), fs = a_s
+__device__ __forceinline__ void pix_chi2_pair(ChiSums &X, const ChiCoef &K, float2 wd, float2 fs, float2 w, float2 invw, float2 dq, float2 du) {
+    const float2 ad = mul2(wd, invw);
+    const float2 rq = fma2(K.q2, fs, fma2(K.q1, ad, add2(dq, K.q0)));
+    const float2 ru = fma2(K.u2, fs, fma2(K.u1, ad, add2(du, K.u0)));
+    X.q = fma2(mul2(w, rq), rq, X.q);
+    X.u = fma2(mul2(w, ru), ru, X.u);
+}
+
 // ---- ordered fp64 sums of the rank-ordered term rows (a3, first level) --------------------------------------------
 // Sum of a chunk of <= CHUNK_LEN consecutive ranks: elements are taken in an order rotated by the chunk's position
 // (bank spreading for the reducer warps; a fixed function of the plan) and combined as (x0+x4)+(x1+x5) | (x2+x6)+(x3+x7).

@@ -22,6 +22,7 @@ struct OptWork {
     const double *lo = nullptr, *hi = nullptr;
     int8_t *pivot = nullptr;
     double *nll_reg = nullptr, *nll_reg_t = nullptr;
+    double *Lcur = nullptr, *Lt_acc = nullptr;   // 1/2 chi^2 at the current point / at the accepted trial point
     double *L0 = nullptr, *gd = nullptr, *amax = nullptr, *alpha = nullptr, *alpha_acc = nullptr, *cscale = nullptr;
     long long *ilim = nullptr;
     int32_t *accepted = nullptr;
@@ -42,7 +43,7 @@ struct OptHyper {
 inline void opt_free(OptWork &w) {
     cudaFree(w.y); cudaFree(w.x); cudaFree(w.xt); cudaFree(w.dir); cudaFree(w.m); cudaFree(w.v); cudaFree(w.grad);
     cudaFree(w.pivot); cudaFree(w.nll_reg); cudaFree(w.nll_reg_t); cudaFree(w.L0); cudaFree(w.gd); cudaFree(w.amax);
-    cudaFree(w.alpha); cudaFree(w.alpha_acc); cudaFree(w.cscale); cudaFree(w.ilim); cudaFree(w.accepted); cudaFree(w.iter);
+    cudaFree(w.alpha); cudaFree(w.alpha_acc); cudaFree(w.cscale); cudaFree(w.ilim); cudaFree(w.accepted); cudaFree(w.iter); cudaFree(w.Lcur); cudaFree(w.Lt_acc);
     w = OptWork();
 }
 
@@ -69,6 +70,8 @@ inline int opt_alloc(OptWork &w, int64_t nparam, int32_t batch, int32_t nregion,
     ok &= cudaMalloc((void **)&w.ilim, (size_t)batch * sizeof(long long)) == cudaSuccess;
     ok &= cudaMalloc((void **)&w.accepted, (size_t)batch * sizeof(int32_t)) == cudaSuccess;
     ok &= cudaMalloc((void **)&w.iter, sizeof(int32_t)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.Lcur, nb) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.Lt_acc, nb) == cudaSuccess;
     if (!ok) { opt_free(w); return 1; }
     *bytes = (int64_t)(7 * np + nparam + 2 * nb * nregion + 7 * nb + (size_t)batch * 4);
     return 0;
@@ -130,9 +133,8 @@ __global__ void __launch_bounds__(OPT_THREADS) k_opt_direction(OptWork w, OptSha
     const int e = blockIdx.x, tid = threadIdx.x;
     const int64_t o0 = sh.param_off[e], o1 = sh.param_off[e + 1];
     double cscale = w.cscale[e];
-    double L = 0.0;
-    for (int r = 0; r < sh.nregion; ++r) L += w.nll_reg[(int64_t)e * sh.nregion + r];
-    L *= cscale;
+    // the objective the line search compares is 1/2 chi^2 of the GLS residual (= nll + const, evaluated accurately)
+    double L = w.Lcur[e] * cscale;
     // release (A2, K = 0): the bound parameter whose descent direction -g points furthest into the interior
     double best = 0.0;
     long long bi = -1;
@@ -210,13 +212,15 @@ __global__ void k_opt_trial(OptWork w, OptShape sh) {
 __global__ void k_opt_ls(OptWork w, OptShape sh, OptHyper hy) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= sh.batch || w.accepted[e]) return;
-    double Lt = 0.0;
-    for (int r = 0; r < sh.nregion; ++r) Lt += w.nll_reg_t[(int64_t)e * sh.nregion + r];
-    Lt *= w.cscale[e];
+    double half_chi2 = 0.0;   // nll_reg_t holds chi^2 per region at the trial point
+    for (int r = 0; r < sh.nregion; ++r) half_chi2 += w.nll_reg_t[(int64_t)e * sh.nregion + r];
+    half_chi2 *= 0.5;
+    const double Lt = half_chi2 * w.cscale[e];
     const double a = w.alpha[e];
     if (Lt <= w.L0[e] + hy.c1 * a * w.gd[e] + hy.ls_noise * fabs(w.L0[e])) {   // false for NaN / +inf
         w.accepted[e] = 1;
         w.alpha_acc[e] = a;
+        w.Lt_acc[e] = half_chi2;
     } else {
         w.alpha[e] = 0.5 * a;
     }
@@ -226,6 +230,7 @@ __global__ void k_opt_ls(OptWork w, OptShape sh, OptHyper hy) {
 __global__ void k_opt_commit(OptWork w, OptShape sh) {
     const int e = blockIdx.y;
     if (blockIdx.x == 0 && e == 0 && threadIdx.x == 0) *w.iter += 1;   // k_opt_direction of this iteration is done
+    if (blockIdx.x == 0 && threadIdx.x == 0 && w.accepted[e]) w.Lcur[e] = w.Lt_acc[e];
     const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= sh.param_off[e + 1]) return;
     const double a = w.accepted[e] ? w.alpha_acc[e] : 0.0;
@@ -238,6 +243,15 @@ __global__ void k_opt_commit(OptWork w, OptShape sh) {
     }
     w.y[i] = y;
     w.x[i] = w.lo[i] + y * (w.hi[i] - w.lo[i]);
+}
+
+// 1/2 chi^2 at the start point (nll_reg_t holds chi^2 per region there)
+__global__ void k_opt_setL(OptWork w, OptShape sh) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= sh.batch) return;
+    double c2 = 0.0;
+    for (int r = 0; r < sh.nregion; ++r) c2 += w.nll_reg_t[(int64_t)e * sh.nregion + r];
+    w.Lcur[e] = 0.5 * c2;
 }
 
 __global__ void k_opt_finish(OptWork w, OptShape sh, double *params, double *nll_final) {
@@ -264,6 +278,9 @@ inline void opt_trial_point(OptWork &w, const OptShape &sh, cudaStream_t st) {
 }
 inline void opt_ls_update(OptWork &w, const OptShape &sh, const OptHyper &hy, cudaStream_t st) {
     k_opt_ls<<<(sh.batch + 127) / 128, 128, 0, st>>>(w, sh, hy);
+}
+inline void opt_set_L(OptWork &w, const OptShape &sh, cudaStream_t st) {
+    k_opt_setL<<<(sh.batch + 127) / 128, 128, 0, st>>>(w, sh);
 }
 inline void opt_commit(OptWork &w, const OptShape &sh, cudaStream_t st) {
     dim3 grid((sh.ktot_max + 255) / 256, sh.batch);

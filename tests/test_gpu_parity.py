@@ -312,6 +312,47 @@ def test_cmb_variance_matches_oracle_maps(torch_cuda, path):
     ctx.close()
 
 
+def test_misfit_is_chi2_of_the_gls_residual(torch_cuda, path):
+    """cs_spectral_misfit: chi2 = 2 nll + d^T N^-1 d per entry and region (Eq. 3 at the GLS solution), accurate where
+    nll itself is not: on noiseless data at the truth it is ~0 although nll ~ -2e8, and it resolves a 1e-5 step."""
+    import torch
+    for noiseless in (False, True):
+        w = gen.make_config(3, nside=16, batch=6, ndata=2, noiseless=noiseless, cluster_truth=True)
+        params = w.params_jittered(seed=28, scale=0.2)
+        ctx, _ = make_ctx(w)
+        p = torch.from_numpy(params).cuda()
+        chi2 = torch.full((w.batch * w.nregion,), float("nan"), dtype=torch.float64, device="cuda")
+        ctx.build_sed_tables(p)
+        ctx.spectral_misfit(chi2)
+        torch.cuda.synchronize()
+        chi2 = chi2.cpu().numpy().reshape(w.batch, w.nregion)
+        for e in range(w.batch):
+            ref = oracle_entry(w, params, e)
+            d = w.data()[int(w.data_of[e])].astype(np.float64)
+            for r in range(w.nregion):
+                sel = w.region_idx == r
+                dNd = float(np.einsum("f,fsp,fsp->", w.ninv.astype(np.float64), d[:, :, sel], d[:, :, sel]))
+                want = 2.0 * ref["nll"][r] + dNd
+                assert abs(chi2[e, r] - want) <= 2e-5 * abs(want) + 2e-9 * dNd, (noiseless, e, r, chi2[e, r], want)
+        ctx.close()
+    # noiseless, at the truth: chi2 vanishes to fp32 accuracy of the residual, far below the rounding of nll
+    w = gen.make_config(1, nside=16, K=(20, 4, 6), noiseless=True, cluster_truth=True)
+    truth = np.concatenate(w.truth["per_cluster"])
+    ctx, _ = make_ctx(w)
+    d = w.data()[0].astype(np.float64)
+    dNd = float(np.einsum("f,fsp,fsp->", w.ninv.astype(np.float64), d, d))
+    vals = []
+    for x in (truth, truth + 1e-5):
+        p = torch.from_numpy(x).cuda()
+        c2 = torch.zeros(1, dtype=torch.float64, device="cuda")
+        ctx.build_sed_tables(p)
+        ctx.spectral_misfit(c2)
+        torch.cuda.synchronize()
+        vals.append(c2.item())
+    assert 0.0 <= vals[0] < 1e-9 * dNd and vals[1] > vals[0]
+    ctx.close()
+
+
 def test_eval_host_equals_device_path(torch_cuda, path):
     """cs_eval_host (host buffers in and out, chunked upload overlapped with compute) is bitwise the device path."""
     import torch
