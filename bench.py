@@ -275,13 +275,16 @@ def main():
                 "traffic": None, "kernel": "k_like_cell<15,GRAD> (fused per-pixel kernel, cell form)", "kernel_ms": k_avg_ms, "kernel_share_of_step": k_ms / ms if ms else None,
                 "peak_source": peak_src, "frac_of_8TBps_nominal": achieved / 8000.0,
                 "algorithmic_bytes_per_launch": alg_bytes}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full capture
+    # (profiles/r01_v4i_k_like_cell.md); only quoted when the capture was taken on this workload and batch
+    traffic_file = os.path.join(ROOT, "profiles", "r01_v4i_traffic.csv")
     if os.path.exists(traffic_file):
         try:
+            import csv
             with open(traffic_file) as fh:
-                tj = json.load(fh)
-            if tj.get("workload") == args.workload and tj.get("batch") == w.batch:
-                roofline["traffic"] = tj["dram_bytes_per_launch"]
+                for row in csv.DictReader(fh):
+                    if row["workload"] == args.workload and int(row["batch"]) == w.batch:
+                        roofline["traffic"] = int(row["dram_bytes_per_launch"])
         except Exception:
             pass
 
