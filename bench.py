@@ -296,6 +296,33 @@ def main():
                       "step": "cs_build_sed_tables + cs_spectral_like_grad(value+grad)", "datagen_s": round(t_gen, 1)},
            "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches)}
 
+    # ---- end to end through the C ABI with host buffers (H2D of d and params, D2H of nll and grad inside); every
+    #      rank runs it on its own batch, the time is the max over ranks
+    if not args.no_e2e:
+        d_pin = d_host.pin_memory()
+        p_pin = torch.from_numpy(params).pin_memory()
+        nll_pin = torch.zeros(w.batch * w.nregion, dtype=torch.float64).pin_memory()
+        grad_pin = torch.zeros(params.shape[0], dtype=torch.float64).pin_memory()
+        ninv_h = np.ascontiguousarray(w.ninv)
+        n_e2e = max(1, min(args.steps, 3))
+        ctx.eval_host(d_pin, ninv_h, p_pin, nll_pin, grad_pin)       # warm-up (allocates the staging buffer)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            ctx.eval_host(d_pin, ninv_h, p_pin, nll_pin, grad_pin)
+        torch.cuda.synchronize()
+        dt_t = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(dt_t, op=dist.ReduceOp.MAX)
+        dt = float(dt_t.item())
+        same = bool(np.array_equal(nll_pin.numpy(), nll.cpu().numpy()))
+        out["e2e"] = {"value": pe_step * world * n_e2e / dt, "unit": UNIT,
+                      "h2d_bytes_per_step": int(d_pin.numel() * 4 + p_pin.numel() * 8) * world,
+                      "d2h_bytes_per_step": int(nll_pin.numel() * 8 + grad_pin.numel() * 8) * world,
+                      "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e, "bitwise_equal_to_device_path": same}
+        ctx.set_data(d_dev, w.ninv)
+        del d_pin
+
     if rank == 0 and world == 1:
         # ---- parity sample + CPU baseline: the oracle on the first entries of the same workload
         if not args.no_cpu:
@@ -312,27 +339,6 @@ def main():
                                    "sample": f"first {n} entries x {w.npix} pixels of the same workload"}
             out["parity"] = {"entries": n, "max_rel_err_nll": e_nll, "max_grad_err_over_T2_bound": e_g,
                              "pass": bool(e_nll <= 1e-5 and e_g <= 1.0)}
-        # ---- end to end through the C ABI with host buffers (H2D of d and params, D2H of nll and grad inside)
-        if not args.no_e2e:
-            d_pin = d_host.pin_memory()
-            p_pin = torch.from_numpy(params).pin_memory()
-            nll_pin = torch.zeros(w.batch * w.nregion, dtype=torch.float64).pin_memory()
-            grad_pin = torch.zeros(params.shape[0], dtype=torch.float64).pin_memory()
-            ninv_h = np.ascontiguousarray(w.ninv)
-            n_e2e = max(1, min(args.steps, 3))
-            ctx.eval_host(d_pin, ninv_h, p_pin, nll_pin, grad_pin)       # warm-up (allocates the staging buffer)
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            for _ in range(n_e2e):
-                ctx.eval_host(d_pin, ninv_h, p_pin, nll_pin, grad_pin)
-            torch.cuda.synchronize()
-            dt = time.perf_counter() - t0
-            same = bool(np.array_equal(nll_pin.numpy(), nll.cpu().numpy()))
-            out["e2e"] = {"value": pe_step * n_e2e / dt, "unit": UNIT,
-                          "h2d_bytes_per_step": int(d_pin.numel() * 4 + p_pin.numel() * 8),
-                          "d2h_bytes_per_step": int(nll_pin.numel() * 8 + grad_pin.numel() * 8),
-                          "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e, "bitwise_equal_to_device_path": same}
-            ctx.set_data(d_dev, w.ninv)
         # ---- extras: component maps throughput on a subset
         if not args.no_extras:
             nsel = min(w.batch, 64)
@@ -382,8 +388,6 @@ def main():
             out["extras"].update({"c2_optimize_200_iters_ms": 1e3 * min(times), "c2_final_nll": float(nf.item()),
                                   "c2_like_grad_call_us": 1e3 * e0.elapsed_time(e1) / 20})
             c2.close()
-    elif world > 1:
-        out["e2e"] = None
     if rank == 0:
         print(json.dumps(out), flush=True)
     if dist is not None:
