@@ -40,7 +40,8 @@ extern "C" {
 #define CS_EINVAL     -1   /* bad argument / call order */
 #define CS_EINDEX     -2   /* a cluster id or region id is out of range (checked bit-exactly, nothing computed) */
 #define CS_EDOMAIN    -3   /* device error bit: T_d <= 0 or a non-finite parameter seen by cs_build_sed_tables */
-#define CS_ESINGULAR  -4   /* device error bit: a pixel's M = A^T N^-1 A had a non-positive pivot; that nll = +inf */
+#define CS_ESINGULAR  -4   /* device error bit: a pivot of the LDL^T of some pixel's M = A^T N^-1 A was not above 1e-6 of its
+                              diagonal entry (covers non-positive); that entry's nll = +inf, its gradient is undefined */
 #define CS_ECUDA      -5   /* a CUDA runtime call failed */
 #define CS_ENOMEM     -6   /* allocation failed */
 
@@ -48,6 +49,20 @@ extern "C" {
 #define CS_UNITS_LITERAL 1 /* Eq. 2 as printed (brightness-temperature units), no unit factor */
 
 #define CS_MAX_NFREQ 16
+
+/* Context options (cs_set_option).  They replace nothing in the results' meaning: every combination evaluates the same
+ * sums; what changes is the pixel order in which they are streamed and reduced, hence the last bits. */
+#define CS_OPT_LAYOUT        1 /* CS_LAYOUT_*; set before cs_set_clusters */
+#define CS_OPT_FORM          2 /* CS_FORM_*; set before cs_set_batch */
+#define CS_OPT_MIN_FILL      3 /* CS_LAYOUT_AUTO: smallest fill fraction live pixels / (tiles * 512) of a configuration's
+                                  sorted layout for which it is taken (default 0.85); set before cs_set_clusters */
+#define CS_OPT_COPY_LIMIT_MB 4 /* most device memory [MiB] the private sorted copies of a batch may take; 0 (default) =
+                                  70 % of the memory free when cs_set_batch runs.  Beyond it cs_set_batch returns CS_ENOMEM. */
+#define CS_LAYOUT_AUTO    0 /* sorted layout for configurations whose tiles fill well, in place for the others */
+#define CS_LAYOUT_INPLACE 1 /* never copy: stream the caller's d in its own pixel order (direct kernel only) */
+#define CS_LAYOUT_SORTED  2 /* sorted layout for every configuration */
+#define CS_FORM_AUTO      0 /* sorted-cell kernel on sorted configurations, direct kernel on the others */
+#define CS_FORM_DIRECT    1 /* direct kernel everywhere, on whatever layout each configuration has (same bits) */
 
 #if defined(__GNUC__)
 #define CS_API __attribute__((visibility("default")))
@@ -86,24 +101,35 @@ typedef struct cs_opt {
 CS_API int cs_create(cs_ctx **out, const cs_model *model);
 CS_API int cs_destroy(cs_ctx *ctx);
 
+/* Sets a context option (CS_OPT_*).  CS_EINVAL for an unknown key, a bad value, or a call after the step that reads it. */
+CS_API int cs_set_option(cs_ctx *ctx, int32_t key, double value);
+
 /* Patch model: `maps` holds nmap cluster maps [nmap, npix] int32 (any); Kmap[nmap] (host) their
  * cluster counts; a clustering configuration c is a triple cfg_maps[c] = (map for beta_d, map for T_d, map for
  * beta_s) (host [ncfg,3]).  A cluster id of -1 in any of a configuration's three maps masks the pixel for that
  * configuration (L211).  region_idx (any, [npix], values < nregion) or NULL with nregion = 1 splits nll by sky
  * region (L269).  Validates -1 <= id < K bit-exactly (CS_EINDEX otherwise, context unchanged), copies the maps
  * (the caller may free them) and builds the per-tile segment plan of the ordered cluster reduction and, per
- * configuration, the per-tile cell plan (distinct cluster triples) of the cell form of the fused kernel.
- * Environment, read at cs_create (tests): CS_FORCE_DIRECT=1 never uses the cell form; CS_CELL_MIN_GROUP=n sets the
- * shortest group of entries that runs on it (default 12).  Both forms give the same bits. */
+ * configuration, its layout (CS_OPT_LAYOUT): in place, or sorted by cell = (k0, k1, k2, region) with cells padded to an
+ * even number of positions, for which every (configuration, data set) pair of a batch later gets a private copy of
+ * its data (cs_set_batch / cs_set_data), streamed by the sorted-cell kernel.  Which kernel runs is a property of the
+ * configuration and the options, never of how entries are grouped into batches. */
 CS_API int cs_set_clusters(cs_ctx *ctx, int32_t nmap, const int32_t *maps, const int32_t *Kmap,
                     int32_t ncfg, const int32_t *cfg_maps, const uint8_t *region_idx, int32_t nregion);
 
+/* Layout taken for configuration cfg: *sorted = 1 / 0, *ntile = its 512-position tiles, *fill = live pixels / (ntile * 512)
+ * (any output may be NULL). */
+CS_API int cs_layout_info(cs_ctx *ctx, int32_t cfg, int32_t *sorted, int32_t *ntile, double *fill);
+
 /* Data (Eq. 1): d dev [ndata, nfreq, 2, npix] fp32 (Q then U per band, pixel fastest), borrowed;
- * ninv any [nfreq] fp32 = 1/sigma_f^2, the same for Q, U and every pixel (L219), copied. */
+ * ninv any [nfreq] fp32 = 1/sigma_f^2, the same for Q, U and every pixel (L219), copied.  When a batch is set, the
+ * private copies of its sorted configurations are gathered here (synchronous): call again after changing d in place.
+ * A data_of beyond ndata in the current batch gives CS_EINVAL and leaves the context unchanged. */
 CS_API int cs_set_data(cs_ctx *ctx, int32_t ndata, const float *d, const float *ninv);
 
 /* Batch: entry e evaluates configuration cfg_of[e] on data set data_of[e] (both host [batch]).  Allocates the
- * SED tables and the reduction workspace for this batch (the only allocation outside cs_create/cs_set_clusters). */
+ * SED tables, the reduction workspace and the private sorted copies for this batch (the only allocation outside
+ * cs_create/cs_set_clusters) and, when the data are set, gathers the copies (synchronous). */
 CS_API int cs_set_batch(cs_ctx *ctx, int32_t batch, const int32_t *cfg_of, const int32_t *data_of);
 
 /* off host [batch+1] int64: parameter offsets of the current batch. */
@@ -127,17 +153,20 @@ CS_API int cs_spectral_like_grad(cs_ctx *ctx, double *nll, double *grad, void *s
 CS_API int cs_spectral_misfit(cs_ctx *ctx, double *chi2, void *stream);
 
 /* a4 (Eq. 5/8): GLS component maps s dev [nsel, 3, 2, npix] fp32 (cmb, dust@nu0d, sync@nu0s; Q,U) for entries
- * `entries` (host [nsel]) or all entries in order when entries == NULL (then nsel must equal batch).  Masked
- * pixels are written as 0. */
+ * `entries` (host [nsel], read during the call) or all entries in order when entries == NULL (then nsel must equal
+ * batch).  Masked pixels are written as 0.  Asynchronous on `stream` like the other hot-path calls (the selection
+ * travels through a pinned staging ring; nothing is allocated and the stream is not synchronised). */
 CS_API int cs_component_maps(cs_ctx *ctx, int32_t nsel, const int32_t *entries, float *s, void *stream);
 
 /* f1 (Eq. 10): per entry and region, variance over unmasked pixels of the reconstructed CMB map, Q and U
  * summed: var dev [batch*nregion] fp64, computed without writing the maps. */
 CS_API int cs_cmb_variance(cs_ctx *ctx, double *var, void *stream);
 
-/* a5: device-resident fixed-budget AdaTopK (Alg. 1) on every entry independently; calls only
- * cs_build_sed_tables and cs_spectral_like_grad.  params dev in: start, out: result; lower/upper dev, same layout;
- * nll_final dev [batch] (summed over regions) or NULL.  No host synchronisation.  The iteration body is captured
+/* a5: device-resident fixed-budget AdaTopK (Alg. 1) on every entry independently.  It calls cs_build_sed_tables,
+ * cs_spectral_like_grad (value + gradient, once per iteration) and cs_spectral_misfit (the objective of the line-search
+ * trials: 1/2 chi^2 = nll + const, R13 -- a deviation from north_star's "only the first two").
+ * params dev in: start, out: result; lower/upper dev, same layout; nll_final dev [batch] (summed over regions) or
+ * NULL.  batch <= 65535 (CS_EINVAL beyond).  No host synchronisation.  The iteration body is captured
  * into a CUDA graph and replayed unless `stream` is itself being captured; on the legacy default stream the work is
  * forked onto an internal stream and joined back before the call returns (still asynchronous to the host).
  * Line-search trials skip the entries that have already accepted a step. */

@@ -11,8 +11,11 @@ from . import build as _build
 
 OK, EINVAL, EINDEX, EDOMAIN, ESINGULAR, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5, -6
 UNITS_KCMB, UNITS_LITERAL = 0, 1
+OPT_LAYOUT, OPT_FORM, OPT_MIN_FILL, OPT_COPY_LIMIT_MB = 1, 2, 3, 4
+LAYOUT_AUTO, LAYOUT_INPLACE, LAYOUT_SORTED = 0, 1, 2
+FORM_AUTO, FORM_DIRECT = 0, 1
 
-EXPORTS = ["cs_create", "cs_destroy", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
+EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
            "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
            "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
@@ -55,6 +58,8 @@ def lib():
     sig = {
         "cs_create": (C.c_int, [C.POINTER(vp), C.POINTER(CsModel)]),
         "cs_destroy": (C.c_int, [vp]),
+        "cs_set_option": (C.c_int, [vp, i32, C.c_double]),
+        "cs_layout_info": (C.c_int, [vp, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(C.c_double)]),
         "cs_set_clusters": (C.c_int, [vp, i32, vp, vp, i32, vp, vp, i32]),
         "cs_set_data": (C.c_int, [vp, i32, vp, vp]),
         "cs_set_batch": (C.c_int, [vp, i32, vp, vp]),
@@ -97,16 +102,34 @@ def _hp(a):
     return None if a is None else a.ctypes.data_as(C.c_void_p)
 
 
-def _ptr(t):
-    """Raw pointer of a torch tensor (device or host), a numpy array, an int, or None."""
+_NP_OF = {"float64": np.float64, "float32": np.float32, "int32": np.int32, "uint8": np.uint8}
+
+
+def _ptr(t, dtype=None, device=None, numel=None, what="argument"):
+    """Raw pointer of a torch tensor (device or host), a numpy array, an int, or None.  The C ABI takes untyped
+    pointers: dtype ("float64", ...), device ("cuda" / "cpu") and the least element count are checked here."""
     if t is None:
         return None
-    if isinstance(t, np.ndarray):
-        assert t.flags["C_CONTIGUOUS"]
-        return t.ctypes.data_as(C.c_void_p)
     if isinstance(t, int):
         return C.c_void_p(t)
-    assert t.is_contiguous()
+    if isinstance(t, np.ndarray):
+        if not t.flags["C_CONTIGUOUS"]:
+            raise ValueError(f"{what}: array must be C-contiguous")
+        if dtype is not None and t.dtype != _NP_OF[dtype]:
+            raise TypeError(f"{what}: expected {dtype}, got {t.dtype}")
+        if device == "cuda":
+            raise TypeError(f"{what}: expected a CUDA tensor, got a numpy array")
+        if numel is not None and t.size < numel:
+            raise ValueError(f"{what}: {t.size} elements, need {numel}")
+        return t.ctypes.data_as(C.c_void_p)
+    if not t.is_contiguous():
+        raise ValueError(f"{what}: tensor must be contiguous")
+    if dtype is not None and str(t.dtype) != "torch." + dtype:
+        raise TypeError(f"{what}: expected {dtype}, got {t.dtype}")
+    if device is not None and t.device.type != device:
+        raise TypeError(f"{what}: expected a {device} tensor, got {t.device}")
+    if numel is not None and t.numel() < numel:
+        raise ValueError(f"{what}: {t.numel()} elements, need {numel}")
     return C.c_void_p(t.data_ptr())
 
 
@@ -130,7 +153,7 @@ def opt_defaults(**kw) -> CsOpt:
 class Context:
     """Owns a cs_ctx*.  Methods mirror the C calls one to one (cs_<name> -> <name>)."""
 
-    def __init__(self, freqs_ghz, npix, nu0_dust=353.0, nu0_sync=23.0, t_cmb=2.7255, units=UNITS_KCMB):
+    def __init__(self, freqs_ghz, npix, nu0_dust=353.0, nu0_sync=23.0, t_cmb=2.7255, units=UNITS_KCMB, options=None):
         self._freqs = np.ascontiguousarray(freqs_ghz, dtype=np.float64)
         m = CsModel(len(self._freqs), self._freqs.ctypes.data_as(C.POINTER(C.c_double)), float(nu0_dust),
                     float(nu0_sync), float(t_cmb), int(units), int(npix))
@@ -139,7 +162,10 @@ class Context:
         self.batch = 0
         self.nregion = 1
         self._keep = {}
+        self.nparam = 0
         _chk(lib().cs_create(C.byref(self._h), C.byref(m)), "cs_create")
+        for key, value in (options or {}).items():
+            self.set_option(key, value)
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
@@ -152,13 +178,25 @@ class Context:
         except Exception:
             pass
 
+    def set_option(self, key, value):
+        """key: OPT_* or one of "layout", "form", "min_fill", "copy_limit_mb"."""
+        names = {"layout": OPT_LAYOUT, "form": OPT_FORM, "min_fill": OPT_MIN_FILL, "copy_limit_mb": OPT_COPY_LIMIT_MB}
+        _chk(lib().cs_set_option(self._h, int(names.get(key, key)), float(value)), "cs_set_option")
+
+    def layout_info(self, cfg):
+        """(sorted, ntile, fill) of configuration cfg."""
+        so, nt, fill = C.c_int32(), C.c_int32(), C.c_double()
+        _chk(lib().cs_layout_info(self._h, int(cfg), C.byref(so), C.byref(nt), C.byref(fill)), "cs_layout_info")
+        return bool(so.value), nt.value, fill.value
+
     def set_clusters(self, maps, Kmap, cfg_maps, region_idx=None, nregion=1):
         """maps: int32 [nmap,npix] (torch device tensor or numpy); Kmap, cfg_maps: host arrays."""
         Kmap = np.ascontiguousarray(Kmap, dtype=np.int32)
         cfg_maps = np.ascontiguousarray(cfg_maps, dtype=np.int32).reshape(-1, 3)
         nmap = int(Kmap.shape[0])
-        _chk(lib().cs_set_clusters(self._h, nmap, _ptr(maps), _hp(Kmap), int(cfg_maps.shape[0]), _hp(cfg_maps),
-                                   _ptr(region_idx), int(nregion)), "cs_set_clusters")
+        _chk(lib().cs_set_clusters(self._h, nmap, _ptr(maps, "int32", numel=nmap * self.npix, what="maps"), _hp(Kmap),
+                                   int(cfg_maps.shape[0]), _hp(cfg_maps),
+                                   _ptr(region_idx, "uint8", numel=self.npix, what="region_idx"), int(nregion)), "cs_set_clusters")
         self.nregion = int(nregion)
         self.batch = 0
 
@@ -167,7 +205,8 @@ class Context:
         ndata = int(d.shape[0])
         if isinstance(ninv, np.ndarray):
             ninv = np.ascontiguousarray(ninv, dtype=np.float32)
-        _chk(lib().cs_set_data(self._h, ndata, _ptr(d), _ptr(ninv)), "cs_set_data")
+        _chk(lib().cs_set_data(self._h, ndata, _ptr(d, "float32", "cuda", ndata * self.nfreq * 2 * self.npix, "d"),
+                               _ptr(ninv, "float32", numel=self.nfreq, what="ninv")), "cs_set_data")
         self._keep["d"] = d
 
     def set_batch(self, cfg_of, data_of):
@@ -175,6 +214,7 @@ class Context:
         data_of = np.ascontiguousarray(data_of, dtype=np.int32)
         _chk(lib().cs_set_batch(self._h, int(cfg_of.shape[0]), _hp(cfg_of), _hp(data_of)), "cs_set_batch")
         self.batch = int(cfg_of.shape[0])
+        self.nparam = int(self.param_offsets()[-1])
 
     def param_offsets(self):
         off = np.empty(self.batch + 1, dtype=np.int64)
@@ -182,13 +222,16 @@ class Context:
         return off
 
     def build_sed_tables(self, params, stream=None):
-        _chk(lib().cs_build_sed_tables(self._h, _ptr(params), _stream(stream)), "cs_build_sed_tables")
+        _chk(lib().cs_build_sed_tables(self._h, _ptr(params, "float64", "cuda", self.nparam, "params"), _stream(stream)),
+             "cs_build_sed_tables")
 
     def spectral_like_grad(self, nll, grad=None, stream=None):
-        _chk(lib().cs_spectral_like_grad(self._h, _ptr(nll), _ptr(grad), _stream(stream)), "cs_spectral_like_grad")
+        _chk(lib().cs_spectral_like_grad(self._h, _ptr(nll, "float64", "cuda", self.batch * self.nregion, "nll"),
+                                         _ptr(grad, "float64", "cuda", self.nparam, "grad"), _stream(stream)), "cs_spectral_like_grad")
 
     def spectral_misfit(self, chi2, stream=None):
-        _chk(lib().cs_spectral_misfit(self._h, _ptr(chi2), _stream(stream)), "cs_spectral_misfit")
+        _chk(lib().cs_spectral_misfit(self._h, _ptr(chi2, "float64", "cuda", self.batch * self.nregion, "chi2"), _stream(stream)),
+             "cs_spectral_misfit")
 
     def component_maps(self, s, entries=None, stream=None):
         if entries is None:
@@ -196,21 +239,28 @@ class Context:
         else:
             entries = np.ascontiguousarray(entries, dtype=np.int32)
             nsel, ep = int(entries.shape[0]), _hp(entries)
-        _chk(lib().cs_component_maps(self._h, nsel, ep, _ptr(s), _stream(stream)), "cs_component_maps")
+        _chk(lib().cs_component_maps(self._h, nsel, ep, _ptr(s, "float32", "cuda", nsel * 6 * self.npix, "s"), _stream(stream)),
+             "cs_component_maps")
 
     def cmb_variance(self, var, stream=None):
-        _chk(lib().cs_cmb_variance(self._h, _ptr(var), _stream(stream)), "cs_cmb_variance")
+        _chk(lib().cs_cmb_variance(self._h, _ptr(var, "float64", "cuda", self.batch * self.nregion, "var"), _stream(stream)),
+             "cs_cmb_variance")
 
     def optimize(self, params, lower, upper, opt=None, nll_final=None, stream=None):
         opt = opt or opt_defaults()
-        _chk(lib().cs_optimize(self._h, _ptr(params), _ptr(lower), _ptr(upper), C.byref(opt), _ptr(nll_final),
-                               _stream(stream)), "cs_optimize")
+        n = self.nparam
+        _chk(lib().cs_optimize(self._h, _ptr(params, "float64", "cuda", n, "params"), _ptr(lower, "float64", "cuda", n, "lower"),
+                               _ptr(upper, "float64", "cuda", n, "upper"), C.byref(opt),
+                               _ptr(nll_final, "float64", "cuda", self.batch, "nll_final"), _stream(stream)), "cs_optimize")
 
     def eval_host(self, d_host, ninv_host, params_host, nll_host, grad_host=None):
         """Host buffers in, host buffers out (numpy arrays or pinned torch CPU tensors)."""
         ndata = int(d_host.shape[0])
-        _chk(lib().cs_eval_host(self._h, ndata, _ptr(d_host), _ptr(ninv_host), _ptr(params_host), _ptr(nll_host),
-                                _ptr(grad_host)), "cs_eval_host")
+        _chk(lib().cs_eval_host(self._h, ndata, _ptr(d_host, "float32", "cpu", ndata * self.nfreq * 2 * self.npix, "d_host"),
+                                _ptr(ninv_host, "float32", "cpu", self.nfreq, "ninv_host"),
+                                _ptr(params_host, "float64", "cpu", self.nparam, "params_host"),
+                                _ptr(nll_host, "float64", "cpu", self.batch * self.nregion, "nll_host"),
+                                _ptr(grad_host, "float64", "cpu", self.nparam, "grad_host")), "cs_eval_host")
 
     def check(self, stream=None):
         return lib().cs_check(self._h, _stream(stream))

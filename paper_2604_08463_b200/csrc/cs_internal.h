@@ -1,36 +1,41 @@
 // cs_internal.h -- host/device shared declarations of libcs (not part of the public ABI).
 //
+// Position space.  Every configuration owns a *layout*: an order of its pixels cut into tiles of TPX positions.
+//   in-place layout  position = pixel (the caller's order, HEALPix RING at the boundary); data are read from the caller's d
+//   sorted layout    pixels sorted by cell = (k0, k1, k2, region), every cell padded to an even number of positions, tiles
+//                    broken early when they would hold more than CELL_CAP cells; masked pixels are left out.  Every
+//                    (configuration, data set) pair of the batch gets a private copy of its data in this order
+//                    (k_relayout, once per cs_set_batch / cs_set_data), so that the two positions (2t, 2t+1) of a thread
+//                    always share their cell and the stream of a tile is one contiguous block in HBM.
 // Data layout in HBM:
-//   d        [ndata][nfreq][2][npix] fp32   borrowed from the caller, streamed once per pixel-eval
+//   d        [ndata][nfreq][2][npix] fp32   borrowed from the caller
+//   dcopy    per (cfg, data) pair [ntile][2 halves][2*nfreq rows][256] fp32   private, sorted layout only
 //   tab      per entry e a block of (K0 + 2*K1 + K2) rows x 16 fp32:
 //              rows [0,K0)            Fd'[k][f] = cd[f] * (nu_f/nu0d)^beta_d[k]
 //              rows [K0,K0+K1)        G  [k][f] = expm1(x0)/expm1(x_f),  x = h nu / (k_B T_d[k])
 //              rows [K0+K1,K0+2K1)    dlnG[k][f] = d ln G / d T_d
 //              rows [K0+2K1, ..+K2)   Fs'[k][f] = cs[f] * (nu_f/nu0s)^beta_s[k]
-//   partial  [batch][PS] fp64   per-tile, per-segment ordered partial sums (written by k_like, read by k_merge)
+//   partial  [batch][PS] fp64   per-tile, per-segment ordered partial sums (written by the fused kernels, read by k_merge)
 //            The slot of a segment inside its term's block is cluster-major (all segments of cluster 0 in ascending
 //            tile order, then cluster 1, ...), so that the merge reads every cluster's partials contiguously.
-//   plan     per cluster map: idx int32[npix], rank u8[ntile*TP], segptr int32[ntile+1], segdesc u16[nseg],
-//            segslot int32[nseg], ksegptr int32[K+1]
-//   cells    per clustering configuration (cell path only): the distinct (k0,k1,k2) triples of every tile in order of
-//            first appearance: cellid u8[ntile*TP] (0xFF = masked pixel), cellptr int32[ntile+1],
-//            rowlist int32[nrow] = the distinct table rows a tile's cells read (rowptr int32[ntile+1]),
-//            cellrows int32[ncell][4] = slots of the cell's rows (Fd', G, dlnG, Fs') in its tile's row list
+//   plan     per term map in position space: idx int32[ntile*TPX], rank u16[ntile*TPX], segptr int32[ntile+1],
+//            segdesc u16[nseg], segslot int32[nseg], ksegptr int32[K+1], chunkptr int32[ntile+1], segcfirst u16[nseg]
 #pragma once
 #include <stdint.h>
 
 namespace cs {
 
-constexpr int TP = 256;        // pixels per tile == threads per CTA of the fused kernel
-constexpr int SEG_MAX = 32;    // longest ordered chain summed by one thread in the reduce phase
+constexpr int TPX = 512;       // positions per tile
+constexpr int NCONS = 256;     // consumer threads of a fused kernel: thread t owns positions 2t and 2t+1 of the tile
+constexpr int HALF = 256;      // a tile is staged as two halves of 256 positions (the widest TMA box)
+constexpr int SEG_MAX = 32;    // longest run of ranks summed as one segment
+constexpr int CHUNK_LEN = 8;   // ranks per chunk (SEG_MAX / CHUNK_LEN <= 4 chunks per segment)
 constexpr int NROW = 16;       // floats per table row (nfreq padded to 16 -> 64-byte rows)
-constexpr int GROUP_MAX = 64;  // entries of one configuration handled by one CTA (per tile)
-constexpr int CELL_MIN_GROUP = 12;   // shortest group (entries of one configuration) worth the cell kernel's set-up
-constexpr int CELL_CAP = 96;   // cell path: most distinct cluster triples a tile may hold (else the direct kernel runs)
-constexpr int CHUNK_LEN = 8;   // cell kernel reduce: ranks summed by one lane in one step (SEG_MAX / CHUNK_LEN <= 4)
-constexpr int CHUNK_CAP = 416; // cell kernel reduce: most chunks (and segments) of the four terms of one tile
-constexpr int ROW_CAP = 128;   // cell path: most distinct table rows the cells of one tile may read
-constexpr int CSTRIDE = 36;    // floats per cell row in shared memory: 16 column values + 16 scalars + 4 pad (= 4 mod 32 banks)
+constexpr int CELL_CAP = 32;   // sorted layout: most cells per tile (one builder lane per cell)
+constexpr int CROW = 100;      // floats per cell row in shared memory: 5 columns x 16 + 16 scalars + 4 pad (= 4 mod 32 banks)
+constexpr int SC_CHUNK_CAP = 4 * (TPX / CHUNK_LEN + CELL_CAP);   // sorted layout: most chunks of the four terms of a tile
+constexpr int SC_SEG_CAP = 4 * (TPX / SEG_MAX + CELL_CAP);       // and most segments
+constexpr int NORANK = 0xFFFF; // rank of a position that does not take part in a term's reduction
 
 // A pivot of the LDL^T factorisation of M = A^T N^-1 A counts as non-positive (CS_ESINGULAR) when it is below this
 // fraction of its diagonal entry: below it an fp32 solve carries no correct digit (R11).
@@ -39,12 +44,12 @@ constexpr float PIVOT_RTOL = 1e-6f;
 constexpr int ERR_DOMAIN = 1;
 constexpr int ERR_SINGULAR = 2;
 
-// One cluster map (or the region pseudo-map) as the kernels see it.
+// One term map (a cluster map or the region pseudo-map) in the position space of one layout.
 struct MapDev {
-    const int32_t *idx;       // [npix] cluster id, -1 = masked
-    const uint8_t *rank;      // [ntile*TP] position of the pixel in its tile's (cluster id, pixel) order
+    const int32_t *idx;       // [ntile*TPX] cluster id of the position, -1 = masked / beyond the sky
+    const uint16_t *rank;     // [ntile*TPX] position in its tile's (cluster id, position) order, NORANK = none
     const int32_t *segptr;    // [ntile+1] first segment of each tile (map-local numbering)
-    const uint16_t *segdesc;  // [nseg] start (8 bits) | (len-1) << 8
+    const uint16_t *segdesc;  // [nseg] start rank (9 bits) | (len-1) << 9
     const int32_t *segslot;   // [nseg] cluster-major slot of the segment inside its term's block of a partial row
     const int32_t *ksegptr;   // [K+1] CSR cluster -> slots [ksegptr[k], ksegptr[k+1])
     const int32_t *chunkptr;  // [ntile+1] running count of <= CHUNK_LEN-rank chunks (each segment is cut into 1..4 of them)
@@ -53,34 +58,36 @@ struct MapDev {
     int32_t nseg;
 };
 
-// One clustering configuration: maps for (beta_d, T_d, beta_s, region) and where each term's partials live.
+// One clustering configuration: term maps for (beta_d, T_d, beta_s, region) in its layout and where each term's
+// partials live.
 struct CfgDev {
-    int32_t map[4];
+    int32_t map[4];       // term maps in the position space of this configuration's layout
     int32_t segbase[4];   // offset of term t inside a partial row (t = 0,1,2 gradient terms, 3 = ll / region)
+    int32_t rmap[4];      // the same four maps in pixel space (in-place layout; component maps are written in pixel order)
     int32_t K[3];
     int32_t ktot;
-    // cell plan (null / 0 when the configuration runs on the direct kernel)
-    const uint8_t *cellid;     // [ntile*TP]
-    const int32_t *cellptr;    // [ntile+1]
-    const int32_t *cellrows;   // [ncell][4] tile-local row slots (Fd', G, dlnG, Fs') into the tile's row list
-    const int32_t *rowptr;     // [ntile+1]
-    const int32_t *rowlist;    // [nrow] distinct table rows (of an entry's table block) the tile's cells read
-    int32_t ncell_max;         // most cells in one tile; 0 = direct path
+    int32_t ntile;        // tiles of this configuration's layout
+    int32_t sorted;       // 1: sorted layout with private data copies, 0: in place
+    int32_t ntile_ring;   // tiles of the in-place layout
     int32_t pad;
+    // sorted layout only
+    const uint8_t *cellid;     // [ntile*NCONS] tile-local cell of each thread (position pair)
+    const int32_t *cellptr;    // [ntile+1] first cell of each tile
+    const int32_t *cellrows;   // [ncell][4] table rows (Fd', G, dlnG, Fs') of the cell inside an entry's table block
+    const int32_t *pospix;     // [ntile*TPX] pixel of each position, -1 = pad
 };
 
-struct Group {
-    int32_t cfg;
-    int32_t start;   // into elist
-    int32_t count;
-    int32_t pad;
+// A run of work for a fused kernel: `count` entries (elist[estart .. estart+count)) of configuration cfg on each of its
+// ntile tiles = ntile*count units in (tile-major, entry-minor) order; ustart = units of the runs before this one.
+struct Run {
+    int32_t cfg, estart, count, ntile;
+    int64_t ustart;
 };
 
-// Constants of the fused kernel, passed by value (constant bank).
+// Constants of the fused kernels, passed by value (constant bank).
 struct KConst {
     float w[NROW];     // Ninv per band, 0 beyond nfreq
     float lnd[NROW];   // ln(nu_f/nu0d)
-    float lnsw[NROW];  // ln(nu_f/nu0s) * w_f
     float lns[NROW];   // ln(nu_f/nu0s)
     float invw[NROW];  // 1 / w_f (0 beyond nfreq)
     float inv_m00;     // 1 / sum_f w_f

@@ -1,17 +1,20 @@
-// cs_lib.cu -- C ABI of libcs (include/cs.h): context, reduction plan, launches.  No CPU compute path exists:
-// every arithmetic step of the hot path runs in the kernels of cs_kernels.cuh; the host code below only
-// validates, builds index structures once per clustering and launches.
+// cs_lib.cu -- C ABI of libcs (include/cs.h): context, layouts and reduction plans, launches.  No CPU compute path
+// exists: every arithmetic step of the hot path runs in the kernels of cs_tables.cuh / cs_like_sc.cuh /
+// cs_like_direct.cuh / cs_optim.cuh; the host code below only validates, builds index structures once per clustering
+// and launches.
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <new>
 #include <vector>
 
 #include "../../include/cs.h"
-#include "cs_kernels.cuh"
-#include "cs_like_cell.cuh"
+#include "cs_tables.cuh"
+#include "cs_like_sc.cuh"
+#include "cs_like_direct.cuh"
 #include "cs_optim.cuh"
 
 using namespace cs;
@@ -22,28 +25,33 @@ using namespace cs;
         if (err__ != cudaSuccess) return CS_ECUDA; \
     } while (0)
 
+// No exception may cross the C ABI: host-side plan building allocates std::vectors.
+#define CS_GUARD_BEGIN try {
+#define CS_GUARD_END                                  \
+    }                                                 \
+    catch (const std::bad_alloc &) { return CS_ENOMEM; } \
+    catch (...) { return CS_EINVAL; }
+
 namespace {
 
 struct MapHost {
     int32_t K = 0, nseg = 0;
     int32_t *idx = nullptr;
-    uint8_t *rank = nullptr;
+    uint16_t *rank = nullptr;
     int32_t *segptr = nullptr;
     uint16_t *segdesc = nullptr;
     int32_t *segslot = nullptr;
     int32_t *ksegptr = nullptr;
     int32_t *chunkptr = nullptr;
     uint16_t *segcfirst = nullptr;
-    std::vector<int32_t> h_chunkptr, h_segptr;   // host copies: per-tile counts decide a configuration's kernel
 };
 
-// Device arrays of one configuration's cell plan (empty when it runs on the direct kernel).
-struct CellHost {
+// Device arrays of one configuration's sorted layout (empty when it stays in place).
+struct SortedHost {
     uint8_t *cellid = nullptr;
     int32_t *cellptr = nullptr;
     int32_t *cellrows = nullptr;
-    int32_t *rowptr = nullptr;
-    int32_t *rowlist = nullptr;
+    int32_t *pospix = nullptr;
 };
 
 template <typename T>
@@ -63,17 +71,22 @@ struct cs_ctx {
     // model
     int32_t nfreq = 0, units = 0;
     int64_t npix = 0;
-    int32_t ntile = 0;
+    int32_t ntile_ring = 0;
+    int32_t nsm = 1;
     double freqs[NROW] = {0};
     double nu0d = 0, nu0s = 0, tcmb = 0;
     TConst tc;
     KConst kc;
     bool have_ninv = false;
+    // options (cs_set_option)
+    int32_t opt_layout = CS_LAYOUT_AUTO, opt_form = CS_FORM_AUTO;
+    double opt_min_fill = 0.85;
+    int64_t opt_copy_limit = 0;         // bytes, 0 = 70 % of the free device memory when the batch is set
     // clusters
     int32_t nmap = 0, ncfg = 0, nregion = 1;
-    std::vector<MapHost> maps;          // nmap + 1 (last = region pseudo-map)
+    std::vector<MapHost> maps;          // nmap pixel-space maps, the region pseudo-map, then 4 per sorted configuration
     std::vector<CfgDev> cfgs;
-    std::vector<CellHost> cellplans;    // ncfg
+    std::vector<SortedHost> sorted;     // ncfg
     std::vector<int32_t> npix_live;     // [ncfg*nregion]
     MapDev *d_maps = nullptr;
     CfgDev *d_cfgs = nullptr;
@@ -82,20 +95,32 @@ struct cs_ctx {
     // data
     const float *d = nullptr;
     int32_t ndata = 0;
-    CUtensorMap tmap;                   // d as [ndata*2*nfreq, npix], box [2*nfreq, 32]   (direct kernel: one box per warp)
-    CUtensorMap tmap_cta;               // same tensor, box [2*nfreq, TP]                  (cell kernel: one box per CTA)
+    CUtensorMap tmap;                   // d as [ndata*2*nfreq, npix], box [2*nfreq, 256]
     bool have_tmap = false;
     // batch
-    int32_t batch = 0, ngroup = 0, ngroup_cell = 0, ktot_max = 0;   // groups [0, ngroup_cell) run on the cell kernel
+    int32_t batch = 0, ktot_max = 0;
+    int32_t nrun_sc = 0, nrun_dir = 0;  // d_runs = [sorted-cell runs | direct runs]
+    int64_t W_sc = 0, W_dir = 0;
     int64_t nparam = 0, nrows = 0, PS = 0;
-    std::vector<int32_t> cfg_of, data_of;
-    std::vector<int64_t> param_off;
-    int32_t *d_cfg_of = nullptr, *d_data_of = nullptr, *d_elist = nullptr, *d_sel_elist = nullptr;
-    int64_t *d_param_off = nullptr, *d_tab_off = nullptr;
-    Group *d_groups = nullptr, *d_sel_groups = nullptr;
-    float *d_tab = nullptr;
+    std::vector<int32_t> cfg_of, data_of, elist;
+    std::vector<int64_t> param_off, copy_off;
+    std::vector<Run> runs;
+    std::vector<CopyJob> jobs;          // private copies of the sorted layout, ordered by data set
+    int32_t *d_cfg_of = nullptr, *d_data_of = nullptr, *d_elist = nullptr;
+    int64_t *d_param_off = nullptr, *d_tab_off = nullptr, *d_copy_off = nullptr;
+    Run *d_runs = nullptr;
+    CopyJob *d_jobs = nullptr;
+    float *d_tab = nullptr, *d_copy = nullptr;
     double *d_partial = nullptr;
-    int64_t batch_bytes = 0;
+    int64_t batch_bytes = 0, copy_bytes = 0;
+    int32_t job_ntile_max = 0;
+    // selections of cs_component_maps: small pinned staging ring, so that the call stays asynchronous
+    static constexpr int SEL_RING = 4;
+    int32_t *h_sel = nullptr;           // pinned [SEL_RING][sel_cap] ints (entry list, then runs)
+    int32_t *d_sel = nullptr;           // device  [SEL_RING][sel_cap]
+    int64_t sel_cap = 0;
+    cudaEvent_t sel_ev[SEL_RING] = {nullptr, nullptr, nullptr, nullptr};
+    int64_t sel_n = 0;
     // optimizer workspace
     OptWork opt;
     int64_t opt_bytes = 0;
@@ -103,9 +128,11 @@ struct cs_ctx {
     float *d_stage = nullptr;
     int64_t stage_bytes = 0;
     double *d_hparams = nullptr, *d_hnll = nullptr, *d_hgrad = nullptr;
+    Run *d_hruns = nullptr;
+    int64_t hruns_cap = 0;
     int64_t hbuf_bytes = 0;
     cudaStream_t copy_stream = nullptr, comp_stream = nullptr;
-    // optional timing of the fused kernel (cs_profile): ring of event pairs recorded around every k_like launch
+    // optional timing of the fused kernel (cs_profile): ring of event pairs recorded around every gradient-mode launch
     static constexpr int PROF_RING = 512;
     bool prof_on = false;
     std::vector<cudaEvent_t> prof_ev;   // 2*PROF_RING
@@ -116,8 +143,6 @@ struct cs_ctx {
     int64_t launches = 0;
     const int32_t *skip = nullptr;      // set by cs_optimize around line-search trials: entries that already accepted
     bool tables_built = false;
-    int32_t cell_min_group = CELL_MIN_GROUP;   // CS_CELL_MIN_GROUP overrides (tests run the cell kernel on 1-entry groups)
-    bool force_direct = false;          // CS_FORCE_DIRECT=1 in the environment at cs_create: never use the cell kernel (tests)
 };
 
 namespace {
@@ -128,8 +153,8 @@ void free_clusters(cs_ctx *c) {
         cudaFree(m.chunkptr); cudaFree(m.segcfirst);
     }
     c->maps.clear();
-    for (auto &p : c->cellplans) { cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); cudaFree(p.rowptr); cudaFree(p.rowlist); }
-    c->cellplans.clear();
+    for (auto &p : c->sorted) { cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); cudaFree(p.pospix); }
+    c->sorted.clear();
     cudaFree(c->d_maps); cudaFree(c->d_cfgs); cudaFree(c->d_npix_live);
     c->d_maps = nullptr; c->d_cfgs = nullptr; c->d_npix_live = nullptr;
     c->cfgs.clear();
@@ -143,18 +168,21 @@ void free_opt(cs_ctx *c) {
 }
 
 void free_batch(cs_ctx *c) {
-    cudaFree(c->d_cfg_of); cudaFree(c->d_data_of); cudaFree(c->d_elist); cudaFree(c->d_sel_elist);
-    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_groups); cudaFree(c->d_sel_groups);
-    cudaFree(c->d_tab); cudaFree(c->d_partial);
-    c->d_cfg_of = c->d_data_of = c->d_elist = c->d_sel_elist = nullptr;
-    c->d_param_off = c->d_tab_off = nullptr;
-    c->d_groups = c->d_sel_groups = nullptr;
-    c->d_tab = nullptr; c->d_partial = nullptr;
-    c->batch = 0; c->ngroup = 0; c->batch_bytes = 0;
+    cudaFree(c->d_cfg_of); cudaFree(c->d_data_of); cudaFree(c->d_elist);
+    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_copy_off); cudaFree(c->d_runs); cudaFree(c->d_jobs);
+    cudaFree(c->d_tab); cudaFree(c->d_partial); cudaFree(c->d_copy);
+    c->d_cfg_of = c->d_data_of = c->d_elist = nullptr;
+    c->d_param_off = c->d_tab_off = c->d_copy_off = nullptr;
+    c->d_runs = nullptr; c->d_jobs = nullptr;
+    c->d_tab = nullptr; c->d_partial = nullptr; c->d_copy = nullptr;
+    c->batch = 0; c->nrun_sc = c->nrun_dir = 0; c->batch_bytes = 0; c->copy_bytes = 0;
     c->tables_built = false;
-    cudaFree(c->d_hparams); cudaFree(c->d_hnll); cudaFree(c->d_hgrad);
-    c->d_hparams = c->d_hnll = c->d_hgrad = nullptr;
+    cudaFree(c->d_hparams); cudaFree(c->d_hnll); cudaFree(c->d_hgrad); cudaFree(c->d_hruns);
+    c->d_hparams = c->d_hnll = c->d_hgrad = nullptr; c->d_hruns = nullptr; c->hruns_cap = 0;
     c->hbuf_bytes = 0;
+    if (c->h_sel) cudaFreeHost(c->h_sel);
+    cudaFree(c->d_sel);
+    c->h_sel = nullptr; c->d_sel = nullptr; c->sel_cap = 0;
     free_opt(c);
 }
 
@@ -165,10 +193,10 @@ double krj2kcmb(double nu_ghz, double tcmb, double hk) {
     return em1 * em1 / (x * x * std::exp(x));
 }
 
-// Reduction plan of one cluster map: per tile the rank of every pixel in the (cluster, pixel) order, that order cut
-// into segments of <= SEG_MAX pixels of one cluster, plus the CSR cluster -> segments.
-int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, MapHost *out, int64_t *bytes) {
-    std::vector<uint8_t> rank((size_t)ntile * TP, 0);
+// Reduction plan of one term map in position space: per tile the rank of every position in the (cluster, position)
+// order, that order cut into segments of <= SEG_MAX positions of one cluster, plus the CSR cluster -> segments.
+int build_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, MapHost *out, int64_t *bytes) {
+    std::vector<uint16_t> rank((size_t)ntile * TPX, (uint16_t)NORANK);
     std::vector<int32_t> segptr(ntile + 1, 0);
     std::vector<uint16_t> segdesc;
     std::vector<int32_t> segcluster;
@@ -179,36 +207,36 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     std::vector<int32_t> chunkptr(ntile + 1, 0);
     std::vector<uint16_t> segcfirst;
     int32_t nchunk = 0;
-    tmp.reserve(TP);
+    tmp.reserve(TPX);
     for (int32_t t = 0; t < ntile; ++t) {
         tmp.clear();
-        const int64_t p0 = (int64_t)t * TP;
-        const int nv = (int)std::min<int64_t>(TP, npix - p0);
+        const int64_t p0 = (int64_t)t * TPX;
+        const int nv = (int)std::min<int64_t>(TPX, npos - p0);
         for (int j = 0; j < nv; ++j)
             if (idx[p0 + j] >= 0) tmp.emplace_back(idx[p0 + j], j);
         std::sort(tmp.begin(), tmp.end());
         segptr[t] = (int32_t)segdesc.size();
-        // segments of this tile, longest first: the lanes of a warp of the reduce phase then walk runs of similar length
+        // segments of this tile, longest first: the threads of the reduce phase then walk runs of similar length
         tseg.clear();
         size_t i = 0;
         while (i < tmp.size()) {
             size_t j = i;
             while (j < tmp.size() && tmp[j].first == tmp[i].first && j - i < (size_t)SEG_MAX) ++j;
-            tseg.push_back({(uint16_t)(i | ((j - i - 1) << 8)), tmp[i].first});
+            tseg.push_back({(uint16_t)(i | ((j - i - 1) << 9)), tmp[i].first});
             i = j;
         }
         std::stable_sort(tseg.begin(), tseg.end(), [](const std::pair<uint16_t, int32_t> &a, const std::pair<uint16_t, int32_t> &b) {
-            return (a.first >> 8) > (b.first >> 8);
+            return (a.first >> 9) > (b.first >> 9);
         });
         chunkptr[t] = nchunk;
         int32_t local = 0;
         for (auto &sg : tseg) {
             segdesc.push_back(sg.first); segcluster.push_back(sg.second);
             segcfirst.push_back((uint16_t)local);
-            local += ((sg.first >> 8) + 1 + CHUNK_LEN - 1) / CHUNK_LEN;
+            local += ((sg.first >> 9) + 1 + CHUNK_LEN - 1) / CHUNK_LEN;
         }
         nchunk += local;
-        for (size_t q = 0; q < tmp.size(); ++q) rank[p0 + tmp[q].second] = (uint8_t)q;
+        for (size_t q = 0; q < tmp.size(); ++q) rank[p0 + tmp[q].second] = (uint16_t)q;
     }
     segptr[ntile] = (int32_t)segdesc.size();
     chunkptr[ntile] = nchunk;
@@ -219,7 +247,8 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     for (int32_t k = 0; k < K; ++k) ksegptr[k + 1] += ksegptr[k];
     std::vector<int32_t> fill(ksegptr.begin(), ksegptr.end() - 1);
     for (int32_t s = 0; s < nseg; ++s) segslot[s] = fill[segcluster[s]]++;
-    std::vector<int32_t> idxv(idx, idx + npix);
+    std::vector<int32_t> idxv((size_t)ntile * TPX, -1);
+    std::copy(idx, idx + npos, idxv.begin());
     out->K = K; out->nseg = nseg;
     int rc;
     if ((rc = dev_upload(&out->idx, idxv, bytes))) return rc;
@@ -230,69 +259,92 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npix, int32_t ntile, M
     if ((rc = dev_upload(&out->ksegptr, ksegptr, bytes))) return rc;
     if ((rc = dev_upload(&out->chunkptr, chunkptr, bytes))) return rc;
     if ((rc = dev_upload(&out->segcfirst, segcfirst, bytes))) return rc;
-    out->h_chunkptr = chunkptr; out->h_segptr = segptr;
     return CS_OK;
 }
 
-// Cell plan of one configuration: per tile the distinct (k0,k1,k2) triples in order of first appearance, as table-row
-// indices of an entry's table block.  Returns 1 (and uploads nothing) when some tile holds more than CELL_CAP cells:
-// that configuration then runs on the direct kernel.
-int build_cell_plan(const int32_t *i0, const int32_t *i1, const int32_t *i2, const int32_t K[3], int64_t npix, int32_t ntile,
-                    CellHost *out, int32_t *ncell_max, int64_t *bytes) {
-    std::vector<uint8_t> cellid((size_t)ntile * TP, 0xFF);
-    std::vector<int32_t> cellptr(ntile + 1, 0);
-    std::vector<int32_t> rows, rowlist, rowptr(ntile + 1, 0);
-    rows.reserve((size_t)ntile * 64 * 4);
-    int32_t mx = 0;
-    for (int32_t t = 0; t < ntile; ++t) {
-        const int64_t p0 = (int64_t)t * TP;
-        const int nv = (int)std::min<int64_t>(TP, npix - p0);
-        const size_t base = rows.size() / 4;
-        cellptr[t] = (int32_t)base;
-        int n = 0, last = -1;
-        for (int j = 0; j < nv; ++j) {
-            const int32_t a = i0[p0 + j], b = i1[p0 + j], d = i2[p0 + j];
-            if (a < 0 || b < 0 || d < 0) continue;
-            const int32_t r0 = a, r1 = K[0] + b, r3 = K[0] + 2 * K[1] + d;
-            int id = -1;
-            if (last >= 0 && rows[4 * (base + last)] == r0 && rows[4 * (base + last) + 1] == r1 && rows[4 * (base + last) + 3] == r3) {
-                id = last;   // consecutive pixels mostly share their cell
-            } else {
-                for (int q = n - 1; q >= 0; --q)
-                    if (rows[4 * (base + q)] == r0 && rows[4 * (base + q) + 1] == r1 && rows[4 * (base + q) + 3] == r3) { id = q; break; }
+// Sorted layout of one configuration (cs_internal.h): the live pixels grouped into cells (k0, k1, k2, region), cells
+// ordered so that neighbours in the order are neighbours on the sky (by the first pixel of their beta_d cluster, then
+// by their own first pixel), every cell padded to an even number of positions, tiles closed early when they would
+// hold more than CELL_CAP cells.  Fills the position-space arrays; returns the fill fraction live / (ntile * TPX).
+struct SortedPlan {
+    std::vector<int32_t> pospix, idx[4], cellptr, cellrows;
+    std::vector<uint8_t> cellid;
+    int32_t ntile = 0;
+    double fill = 0.0;
+};
+void plan_sorted(const int32_t *i0, const int32_t *i1, const int32_t *i2, const int32_t *reg, const int32_t K[3], int64_t npix,
+                 SortedPlan &sp) {
+    struct Px { int32_t a, b, c, r, p; };
+    std::vector<Px> px;
+    px.reserve((size_t)npix);
+    for (int64_t p = 0; p < npix; ++p)
+        if (i0[p] >= 0 && i1[p] >= 0 && i2[p] >= 0) px.push_back(Px{i0[p], i1[p], i2[p], reg[p], (int32_t)p});
+    std::sort(px.begin(), px.end(), [](const Px &x, const Px &y) {
+        if (x.a != y.a) return x.a < y.a;
+        if (x.b != y.b) return x.b < y.b;
+        if (x.c != y.c) return x.c < y.c;
+        if (x.r != y.r) return x.r < y.r;
+        return x.p < y.p;
+    });
+    struct Cell { int32_t first, count, kmin, a, minp; };
+    std::vector<Cell> cells;
+    std::vector<int32_t> kmin(K[0], INT32_MAX);
+    for (size_t i = 0; i < px.size();) {
+        size_t j = i;
+        while (j < px.size() && px[j].a == px[i].a && px[j].b == px[i].b && px[j].c == px[i].c && px[j].r == px[i].r) ++j;
+        cells.push_back(Cell{(int32_t)i, (int32_t)(j - i), 0, px[i].a, px[i].p});
+        kmin[px[i].a] = std::min(kmin[px[i].a], px[i].p);
+        i = j;
+    }
+    for (auto &ce : cells) ce.kmin = kmin[ce.a];
+    std::sort(cells.begin(), cells.end(), [](const Cell &x, const Cell &y) {
+        if (x.kmin != y.kmin) return x.kmin < y.kmin;
+        if (x.a != y.a) return x.a < y.a;
+        return x.minp < y.minp;
+    });
+    sp.pospix.clear(); sp.cellid.clear(); sp.cellptr.assign(1, 0); sp.cellrows.clear();
+    for (int t = 0; t < 4; ++t) sp.idx[t].clear();
+    int pos = 0, ncell = 0;   // inside the current tile
+    Px last{0, 0, 0, 0, -1};
+    auto put = [&](const Px &q, int32_t pix) {
+        sp.pospix.push_back(pix);
+        sp.idx[0].push_back(q.a); sp.idx[1].push_back(q.b); sp.idx[2].push_back(q.c); sp.idx[3].push_back(q.r);
+        if (pos & 1) sp.cellid.push_back((uint8_t)(ncell - 1));
+        ++pos;
+    };
+    auto close_tile = [&]() {
+        while (pos < TPX) put(last, -1);   // trailing pads belong to the tile's last cell
+        sp.cellptr.push_back((int32_t)(sp.cellrows.size() / 4));
+        pos = 0; ncell = 0;
+    };
+    for (const Cell &ce : cells) {
+        int32_t done = 0;
+        const int32_t padded = ce.count + (ce.count & 1);
+        while (done < padded) {
+            if (pos == TPX || ncell == CELL_CAP) close_tile();
+            const int32_t take = std::min(padded - done, TPX - pos);
+            const Px &q0 = px[ce.first];
+            ++ncell;
+            sp.cellrows.push_back(q0.a); sp.cellrows.push_back(K[0] + q0.b); sp.cellrows.push_back(K[0] + K[1] + q0.b);
+            sp.cellrows.push_back(K[0] + 2 * K[1] + q0.c);
+            last = q0;
+            for (int32_t j = 0; j < take; ++j) {
+                const int32_t src = done + j;
+                put(q0, src < ce.count ? px[ce.first + src].p : -1);
             }
-            if (id < 0) {
-                if (n == CELL_CAP) return 1;
-                id = n++;
-                rows.push_back(r0); rows.push_back(r1); rows.push_back(K[0] + K[1] + b); rows.push_back(r3);
-            }
-            cellid[p0 + j] = (uint8_t)id;
-            last = id;
-        }
-        mx = std::max(mx, n);
-        // the tile's distinct table rows; cells keep slots into this list (the loader stages the list per entry)
-        rowptr[t] = (int32_t)rowlist.size();
-        const size_t r0 = rowlist.size();
-        for (size_t q = 4 * base; q < rows.size(); ++q) {
-            size_t f = r0;
-            while (f < rowlist.size() && rowlist[f] != rows[q]) ++f;
-            if (f == rowlist.size()) {
-                if (rowlist.size() - r0 == (size_t)ROW_CAP) return 1;
-                rowlist.push_back(rows[q]);
-            }
-            rows[q] = (int32_t)(f - r0);
+            done += take;
         }
     }
-    rowptr[ntile] = (int32_t)rowlist.size();
-    cellptr[ntile] = (int32_t)(rows.size() / 4);
-    *ncell_max = mx;
-    int rc;
-    if ((rc = dev_upload(&out->cellid, cellid, bytes))) return rc;
-    if ((rc = dev_upload(&out->cellptr, cellptr, bytes))) return rc;
-    if ((rc = dev_upload(&out->cellrows, rows, bytes))) return rc;
-    if ((rc = dev_upload(&out->rowptr, rowptr, bytes))) return rc;
-    if ((rc = dev_upload(&out->rowlist, rowlist, bytes))) return rc;
-    return CS_OK;
+    if (pos > 0 || sp.cellptr.size() == 1) {
+        if (ncell == 0) {   // no live pixel at all: one dummy cell reading the first table rows, all pads
+            sp.cellrows.push_back(0); sp.cellrows.push_back(K[0]); sp.cellrows.push_back(K[0] + K[1]); sp.cellrows.push_back(K[0] + 2 * K[1]);
+            ncell = 1;
+            last = Px{0, 0, 0, 0, -1};
+        }
+        close_tile();
+    }
+    sp.ntile = (int32_t)sp.cellptr.size() - 1;
+    sp.fill = (double)px.size() / ((double)sp.ntile * TPX);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -300,12 +352,12 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 // TMA descriptor of d viewed as a 2-D fp32 tensor [ndata*2*nfreq rows, npix]; one box = all rows of one data set for
-// 32 consecutive pixels.  Only possible when rows are 16-byte aligned; otherwise the kernels use plain loads.
-int make_tmap(cs_ctx *c) {
-    c->have_tmap = false;
-    std::memset(&c->tmap, 0, sizeof(c->tmap));
-    std::memset(&c->tmap_cta, 0, sizeof(c->tmap_cta));
-    if ((c->npix % 4) != 0 || (((uintptr_t)c->d) % 16) != 0) return CS_OK;
+// 256 consecutive pixels (half a tile).  Only possible when rows are 16-byte aligned; otherwise the loader warp uses
+// plain loads.
+int make_tmap(cs_ctx *c, const float *d, int32_t ndata, CUtensorMap *tm, bool *have) {
+    *have = false;
+    std::memset(tm, 0, sizeof(*tm));
+    if ((c->npix % 4) != 0 || (((uintptr_t)d) % 16) != 0) return CS_OK;
     static EncodeTiledFn enc = nullptr;
     if (!enc) {
         void *fn = nullptr;
@@ -313,65 +365,86 @@ int make_tmap(cs_ctx *c) {
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return CS_ECUDA;
         enc = (EncodeTiledFn)fn;
     }
-    const cuuint64_t dims[2] = {(cuuint64_t)c->npix, (cuuint64_t)c->ndata * 2 * c->nfreq};
+    const cuuint64_t dims[2] = {(cuuint64_t)c->npix, (cuuint64_t)ndata * 2 * c->nfreq};
     const cuuint64_t strides[1] = {(cuuint64_t)c->npix * 4};
-    const cuuint32_t box[2] = {32, (cuuint32_t)(2 * c->nfreq)}, es[2] = {1, 1};
-    if (enc(&c->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)c->d, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    const cuuint32_t box[2] = {(cuuint32_t)HALF, (cuuint32_t)(2 * c->nfreq)}, es[2] = {1, 1};
+    if (enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)d, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return CS_ECUDA;
-    const cuuint32_t box_cta[2] = {(cuuint32_t)TP, (cuuint32_t)(2 * c->nfreq)};
-    if (enc(&c->tmap_cta, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)c->d, dims, strides, box_cta, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return CS_ECUDA;
-    c->have_tmap = true;
+    *have = true;
     return CS_OK;
 }
 
-// Launches the fused kernel over the groups [g0, g1) of P.groups; groups below `ncell` (cell path) run on
-// k_like_cell, the rest on the direct kernel k_like.  grid.y is limited to 65535: launch in slabs of groups.
+// The dynamic shared memory limit is a per-device function attribute: set for every instantiation when a context is
+// created on a device (a context is bound to the device current at cs_create).
 template <int NF, int MODE>
-int launch_like_t(cs_ctx *c, const LikeParams &P, int g0, int g1, int ncell, cudaStream_t st) {
-    static bool configured = false;
-    constexpr size_t smem = like_smem_bytes<NF>(), smem_cell = cell_smem_bytes<NF>();
-    if (!configured) {
-        CK(cudaFuncSetAttribute(k_like<NF, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(cudaFuncSetAttribute(k_like_cell<NF, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cell));
-        configured = true;
-    }
+cudaError_t configure_mode() {
+    cudaError_t e = cudaFuncSetAttribute(k_like_direct<NF, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)direct_smem_bytes<NF>());
+    if (e != cudaSuccess) return e;
+    if (MODE != MODE_MAPS) e = cudaFuncSetAttribute(k_like_sc<NF, MODE == MODE_MAPS ? MODE_VALUE : MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc_smem_bytes<NF>());
+    return e;
+}
+template <int NF>
+cudaError_t configure_nf() {
+    cudaError_t e;
+    if ((e = configure_mode<NF, MODE_VALUE>()) != cudaSuccess) return e;
+    if ((e = configure_mode<NF, MODE_GRAD>()) != cudaSuccess) return e;
+    if ((e = configure_mode<NF, MODE_MAPS>()) != cudaSuccess) return e;
+    if ((e = configure_mode<NF, MODE_CMBVAR>()) != cudaSuccess) return e;
+    return configure_mode<NF, MODE_CHI2>();
+}
+
+// Launches the fused kernels over nrun_sc sorted-cell runs followed by nrun_dir direct runs at `runs`.
+template <int NF, int MODE>
+int launch_like_t(cs_ctx *c, const LikeParams &P0, const Run *runs, int nrun_sc, int64_t W_sc, int nrun_dir, int64_t W_dir, cudaStream_t st) {
     const bool prof = c->prof_on && MODE == MODE_GRAD;
     for (int pass = 0; pass < 2; ++pass) {
-        const int a = pass == 0 ? g0 : std::max(g0, ncell), b = pass == 0 ? std::min(g1, ncell) : g1;
-        for (int g = a; g < b; g += 65535) {
-            LikeParams Q = P;
-            Q.groups = P.groups + g;
-            dim3 grid(c->ntile, std::min(65535, b - g));
-            if (prof) cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING)], st);
-            if (pass == 0) k_like_cell<NF, MODE><<<grid, CELL_THREADS, smem_cell, st>>>(c->tmap_cta, Q);
-            else k_like<NF, MODE><<<grid, TP, smem, st>>>(c->tmap, Q);
-            if (prof) { cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING) + 1], st); c->prof_n++; }
-            c->launches++;
+        const int nrun = pass == 0 ? nrun_sc : nrun_dir;
+        const int64_t W = pass == 0 ? W_sc : W_dir;
+        if (nrun == 0 || W == 0) continue;
+        LikeParams P = P0;
+        P.runs = runs + (pass == 0 ? 0 : nrun_sc);
+        P.nrun = nrun;
+        P.W = W;
+        const int grid = (int)std::min<int64_t>(W, c->nsm);
+        if (prof) cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING)], st);
+        if (pass == 0) {
+            if (MODE == MODE_MAPS) return CS_EINVAL;
+            k_like_sc<NF, MODE == MODE_MAPS ? MODE_VALUE : MODE><<<grid, SC_THREADS, sc_smem_bytes<NF>(), st>>>(P);
+        } else {
+            k_like_direct<NF, MODE><<<grid, DR_THREADS, direct_smem_bytes<NF>(), st>>>(c->tmap, P);
         }
+        if (prof) { cudaEventRecord(c->prof_ev[2 * (c->prof_n % cs_ctx::PROF_RING) + 1], st); c->prof_n++; }
+        c->launches++;
     }
     CK(cudaGetLastError());
     return CS_OK;
 }
 
 template <int MODE>
-int launch_like(cs_ctx *c, const LikeParams &P, int g0, int g1, int ncell, cudaStream_t st) {
-    if (c->nfreq == 15) return launch_like_t<15, MODE>(c, P, g0, g1, ncell, st);
-    return launch_like_t<16, MODE>(c, P, g0, g1, ncell, st);
+int launch_like(cs_ctx *c, const LikeParams &P, const Run *runs, int nrun_sc, int64_t W_sc, int nrun_dir, int64_t W_dir, cudaStream_t st) {
+    if (c->nfreq == 15) return launch_like_t<15, MODE>(c, P, runs, nrun_sc, W_sc, nrun_dir, W_dir, st);
+    return launch_like_t<16, MODE>(c, P, runs, nrun_sc, W_sc, nrun_dir, W_dir, st);
+}
+template <int MODE>
+int launch_batch(cs_ctx *c, const LikeParams &P, cudaStream_t st) {
+    return launch_like<MODE>(c, P, c->d_runs, c->nrun_sc, c->W_sc, c->nrun_dir, c->W_dir, st);
 }
 
 LikeParams base_params(cs_ctx *c) {
     LikeParams P;
+    std::memset(&P, 0, sizeof(P));
     P.d = c->d;
     P.npix = c->npix;
     P.nfreq = c->nfreq;
-    P.use_bulk = c->have_tmap ? 1 : 0;
-    P.evict_first = ((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4 > (int64_t)96 << 20) ? 1 : 0;
+    P.use_tma = c->have_tmap ? 1 : 0;
+    const int64_t stream_bytes = std::max<int64_t>((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4, c->copy_bytes);
+    P.evict_first = (stream_bytes > (int64_t)96 << 20) ? 1 : 0;
+    P.ring_maps = 0;
+    P.dcopy = c->d_copy;
+    P.copy_off = c->d_copy_off;
     P.maps = c->d_maps;
     P.cfgs = c->d_cfgs;
-    P.groups = c->d_groups;
     P.elist = c->d_elist;
     P.data_of = c->d_data_of;
     P.skip = c->skip;
@@ -390,12 +463,60 @@ int ready(cs_ctx *c) {
     return CS_OK;
 }
 
+// Gathers the private copies [j0, j1) of the sorted layout from the caller's data (k_relayout).
+int relayout(cs_ctx *c, const float *d, int64_t j0, int64_t j1, cudaStream_t st) {
+    for (int64_t j = j0; j < j1; j += 65535) {
+        const int nj = (int)std::min<int64_t>(65535, j1 - j);
+        dim3 grid(c->job_ntile_max, nj);
+        k_relayout<<<grid, TPX, 0, st>>>(d, c->npix, 2 * c->nfreq, c->d_cfgs, c->d_jobs + j, c->d_copy);
+        c->launches++;
+    }
+    CK(cudaGetLastError());
+    return CS_OK;
+}
+
+int set_data_impl(cs_ctx *c, int32_t ndata, const float *d, const float *ninv, bool do_relayout) {
+    if (!c || ndata <= 0 || !d || !ninv) return CS_EINVAL;
+    for (int e = 0; e < c->batch; ++e)   // validate against the current batch before anything is changed
+        if (c->data_of[e] >= ndata) return CS_EINVAL;
+    float w[NROW] = {0};
+    CK(cudaMemcpy(w, ninv, sizeof(float) * c->nfreq, cudaMemcpyDefault));
+    double m00 = 0;
+    for (int f = 0; f < c->nfreq; ++f) {
+        if (!(w[f] > 0.f) || !std::isfinite(w[f])) return CS_EINVAL;
+        m00 += (double)w[f];
+    }
+    CUtensorMap tm;
+    bool have = false;
+    int rc = make_tmap(c, d, ndata, &tm, &have);
+    if (rc) return rc;
+    std::memset(&c->kc, 0, sizeof(c->kc));
+    for (int f = 0; f < c->nfreq; ++f) {
+        c->kc.w[f] = w[f];
+        c->kc.lnd[f] = (float)c->tc.lnd[f];
+        c->kc.lns[f] = (float)c->tc.lns[f];
+        c->kc.invw[f] = 1.0f / w[f];
+    }
+    c->kc.m00 = (float)m00;
+    c->kc.inv_m00 = (float)(1.0 / m00);
+    c->d = d;
+    c->ndata = ndata;
+    c->have_ninv = true;
+    c->tmap = tm;
+    c->have_tmap = have;
+    if (do_relayout && c->batch > 0 && !c->jobs.empty()) {
+        if ((rc = relayout(c, d, 0, (int64_t)c->jobs.size(), nullptr))) return rc;
+        CK(cudaDeviceSynchronize());
+    }
+    return CS_OK;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------------------
 extern "C" {
 
-int cs_version(void) { return 1; }
+int cs_version(void) { return 2; }
 
 const char *cs_strerror(int code) {
     switch (code) {
@@ -413,7 +534,7 @@ const char *cs_strerror(int code) {
 int cs_create(cs_ctx **out, const cs_model *m) {
     if (!out) return CS_EINVAL;
     *out = nullptr;
-    if (!m || !m->freqs_ghz || m->nfreq < 3 || m->nfreq > CS_MAX_NFREQ || m->npix <= 0 || m->npix > (int64_t)TP * 0x7fffff00)
+    if (!m || !m->freqs_ghz || m->nfreq < 3 || m->nfreq > CS_MAX_NFREQ || m->npix <= 0 || m->npix > (int64_t)0x7fff0000)
         return CS_EINVAL;
     if (!(m->nu0_dust_ghz > 0) || !(m->nu0_sync_ghz > 0) || !(m->t_cmb_k > 0)) return CS_EINVAL;
     if (m->units != CS_UNITS_KCMB && m->units != CS_UNITS_LITERAL) return CS_EINVAL;
@@ -422,7 +543,7 @@ int cs_create(cs_ctx **out, const cs_model *m) {
     cs_ctx *c = new (std::nothrow) cs_ctx();
     if (!c) return CS_ENOMEM;
     c->nfreq = m->nfreq; c->units = m->units; c->npix = m->npix;
-    c->ntile = (int32_t)((m->npix + TP - 1) / TP);
+    c->ntile_ring = (int32_t)((m->npix + TPX - 1) / TPX);
     c->nu0d = m->nu0_dust_ghz; c->nu0s = m->nu0_sync_ghz; c->tcmb = m->t_cmb_k;
     // exact SI constants (R3)
     const double hk = 6.62607015e-34 * 1e9 / 1.380649e-23;
@@ -441,17 +562,18 @@ int cs_create(cs_ctx **out, const cs_model *m) {
         c->tc.cd[f] = (nu / c->nu0d) * ud;   // (nu/nu0)^(beta_d+1) = (nu/nu0) * (nu/nu0)^beta_d
         c->tc.cs[f] = us;
     }
-    if (cudaMalloc((void **)&c->d_err, sizeof(int32_t)) != cudaSuccess || cudaMemset(c->d_err, 0, sizeof(int32_t)) != cudaSuccess ||
-        cudaMalloc((void **)&c->d_tc, sizeof(TConst)) != cudaSuccess ||
-        cudaMemcpy(c->d_tc, &c->tc, sizeof(TConst), cudaMemcpyHostToDevice) != cudaSuccess) {
+    int dev = 0, nsm = 0;
+    bool ok = cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0;
+    ok = ok && configure_nf<15>() == cudaSuccess && configure_nf<16>() == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&c->d_err, sizeof(int32_t)) == cudaSuccess && cudaMemset(c->d_err, 0, sizeof(int32_t)) == cudaSuccess &&
+         cudaMalloc((void **)&c->d_tc, sizeof(TConst)) == cudaSuccess &&
+         cudaMemcpy(c->d_tc, &c->tc, sizeof(TConst), cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) {
         cudaFree(c->d_err); cudaFree(c->d_tc);
         delete c;
         return CS_ECUDA;
     }
-    const char *fd = std::getenv("CS_FORCE_DIRECT");
-    c->force_direct = fd && fd[0] == '1';
-    const char *mg = std::getenv("CS_CELL_MIN_GROUP");
-    if (mg && std::atoi(mg) >= 1) c->cell_min_group = std::atoi(mg);
+    c->nsm = nsm;
     *out = c;
     return CS_OK;
 }
@@ -467,14 +589,42 @@ int cs_destroy(cs_ctx *c) {
     cudaFree(c->d_err);
     cudaFree(c->d_tc);
     for (auto &e : c->prof_ev) cudaEventDestroy(e);
+    for (auto &e : c->sel_ev) if (e) cudaEventDestroy(e);
     delete c;
     return CS_OK;
+}
+
+int cs_set_option(cs_ctx *c, int32_t key, double value) {
+    if (!c || !std::isfinite(value)) return CS_EINVAL;
+    switch (key) {
+        case CS_OPT_LAYOUT:
+            if (value != CS_LAYOUT_AUTO && value != CS_LAYOUT_INPLACE && value != CS_LAYOUT_SORTED) return CS_EINVAL;
+            if (!c->maps.empty()) return CS_EINVAL;   // decided when the clusters are set
+            c->opt_layout = (int32_t)value;
+            return CS_OK;
+        case CS_OPT_FORM:
+            if (value != CS_FORM_AUTO && value != CS_FORM_DIRECT) return CS_EINVAL;
+            if (c->batch > 0) return CS_EINVAL;       // decided when the batch is set
+            c->opt_form = (int32_t)value;
+            return CS_OK;
+        case CS_OPT_MIN_FILL:
+            if (!(value >= 0.0 && value <= 1.0) || !c->maps.empty()) return CS_EINVAL;
+            c->opt_min_fill = value;
+            return CS_OK;
+        case CS_OPT_COPY_LIMIT_MB:
+            if (value < 0) return CS_EINVAL;
+            c->opt_copy_limit = (int64_t)(value * 1048576.0);
+            return CS_OK;
+        default:
+            return CS_EINVAL;
+    }
 }
 
 int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t *Kmap, int32_t ncfg,
                     const int32_t *cfg_maps, const uint8_t *region_idx, int32_t nregion) {
     if (!c || nmap <= 0 || !maps || !Kmap || ncfg <= 0 || !cfg_maps || nregion < 1 || nregion > 255) return CS_EINVAL;
     if (nregion > 1 && !region_idx) return CS_EINVAL;
+    CS_GUARD_BEGIN
     const int64_t npix = c->npix;
     for (int32_t m = 0; m < nmap; ++m)
         if (Kmap[m] <= 0) return CS_EINVAL;
@@ -505,69 +655,68 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     c->maps.resize(nmap + 1);
     int rc;
     for (int32_t m = 0; m < nmap; ++m)
-        if ((rc = build_map_plan(h.data() + (size_t)m * npix, Kmap[m], npix, c->ntile, &c->maps[m], &c->cluster_bytes))) {
+        if ((rc = build_map_plan(h.data() + (size_t)m * npix, Kmap[m], npix, c->ntile_ring, &c->maps[m], &c->cluster_bytes))) {
             free_clusters(c);
             return rc;
         }
-    if ((rc = build_map_plan(reg.data(), nregion, npix, c->ntile, &c->maps[nmap], &c->cluster_bytes))) {
+    if ((rc = build_map_plan(reg.data(), nregion, npix, c->ntile_ring, &c->maps[nmap], &c->cluster_bytes))) {
         free_clusters(c);
         return rc;
     }
     c->nmap = nmap; c->ncfg = ncfg; c->nregion = nregion;
-    std::vector<MapDev> md(nmap + 1);
-    for (int32_t m = 0; m <= nmap; ++m) {
-        const MapHost &s = c->maps[m];
-        md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.segslot, s.ksegptr, s.chunkptr, s.segcfirst, s.K, s.nseg};
-    }
     c->cfgs.resize(ncfg);
-    c->cellplans.resize(ncfg);
+    c->sorted.resize(ncfg);
     c->npix_live.assign((size_t)ncfg * nregion, 0);
+    SortedPlan sp;
     for (int32_t i = 0; i < ncfg; ++i) {
         CfgDev &cf = c->cfgs[i];
-        int32_t off = 0;
+        std::memset(&cf, 0, sizeof(cf));
         for (int t = 0; t < 4; ++t) {
-            cf.map[t] = t < 3 ? cfg_maps[i * 3 + t] : nmap;
-            cf.segbase[t] = off;
-            off += c->maps[cf.map[t]].nseg;
-            if (t < 3) cf.K[t] = Kmap[cf.map[t]];
+            cf.rmap[t] = t < 3 ? cfg_maps[i * 3 + t] : nmap;
+            cf.map[t] = cf.rmap[t];
+            if (t < 3) cf.K[t] = Kmap[cf.rmap[t]];
         }
         cf.ktot = cf.K[0] + cf.K[1] + cf.K[2];
-        const int32_t *a = h.data() + (size_t)cf.map[0] * npix, *b = h.data() + (size_t)cf.map[1] * npix,
-                      *d = h.data() + (size_t)cf.map[2] * npix;
+        cf.ntile = cf.ntile_ring = c->ntile_ring;
+        const int32_t *a = h.data() + (size_t)cf.rmap[0] * npix, *b = h.data() + (size_t)cf.rmap[1] * npix,
+                      *d = h.data() + (size_t)cf.rmap[2] * npix;
         for (int64_t p = 0; p < npix; ++p)
             if (a[p] >= 0 && b[p] >= 0 && d[p] >= 0) c->npix_live[(size_t)i * nregion + reg[p]]++;
-        // cell plan; a configuration with a tile of more than CELL_CAP distinct triples stays on the direct kernel
-        cf.cellid = nullptr; cf.cellptr = nullptr; cf.cellrows = nullptr; cf.rowptr = nullptr; cf.rowlist = nullptr;
-        cf.ncell_max = 0; cf.pad = 0;
-        if (!c->force_direct) {
-            int32_t mx = 0;
-            rc = build_cell_plan(a, b, d, cf.K, npix, c->ntile, &c->cellplans[i], &mx, &c->cluster_bytes);
-            if (rc < 0) { free_clusters(c); return rc; }
-            if (rc == 0) {   // the reducer warps' plan must fit too
-                for (int32_t t = 0; t < c->ntile && rc == 0; ++t) {
-                    int32_t nc = 0, ns = 0;
-                    for (int q = 0; q < 4; ++q) {
-                        const MapHost &mh = c->maps[cf.map[q]];
-                        nc += mh.h_chunkptr[t + 1] - mh.h_chunkptr[t];
-                        ns += mh.h_segptr[t + 1] - mh.h_segptr[t];
+        // sorted layout: taken when the option asks for it, or (auto) when its tiles come out well filled -- small
+        // cells (K ~ npix) would mostly stream padding
+        if (c->opt_layout != CS_LAYOUT_INPLACE) {
+            plan_sorted(a, b, d, reg.data(), cf.K, npix, sp);
+            if (c->opt_layout == CS_LAYOUT_SORTED || sp.fill >= c->opt_min_fill) {
+                SortedHost &sh = c->sorted[i];
+                if ((rc = dev_upload(&sh.cellid, sp.cellid, &c->cluster_bytes)) || (rc = dev_upload(&sh.cellptr, sp.cellptr, &c->cluster_bytes)) ||
+                    (rc = dev_upload(&sh.cellrows, sp.cellrows, &c->cluster_bytes)) || (rc = dev_upload(&sh.pospix, sp.pospix, &c->cluster_bytes))) {
+                    free_clusters(c);
+                    return rc;
+                }
+                const int64_t npos = (int64_t)sp.ntile * TPX;
+                for (int t = 0; t < 4; ++t) {
+                    c->maps.emplace_back();
+                    if ((rc = build_map_plan(sp.idx[t].data(), t < 3 ? cf.K[t] : nregion, npos, sp.ntile, &c->maps.back(), &c->cluster_bytes))) {
+                        free_clusters(c);
+                        return rc;
                     }
-                    // CMBVAR reduces all four terms over the region map
-                    const MapHost &mr = c->maps[cf.map[3]];
-                    nc = std::max(nc, 4 * (mr.h_chunkptr[t + 1] - mr.h_chunkptr[t]));
-                    if (nc > CHUNK_CAP || ns > CHUNK_CAP) rc = 1;
+                    cf.map[t] = (int32_t)c->maps.size() - 1;
                 }
-                if (rc == 1) {
-                    cudaFree(c->cellplans[i].cellid); cudaFree(c->cellplans[i].cellptr); cudaFree(c->cellplans[i].cellrows);
-                    cudaFree(c->cellplans[i].rowptr); cudaFree(c->cellplans[i].rowlist);
-                    c->cellplans[i] = CellHost();
-                }
-            }
-            if (rc == 0) {
-                cf.cellid = c->cellplans[i].cellid; cf.cellptr = c->cellplans[i].cellptr; cf.cellrows = c->cellplans[i].cellrows;
-                cf.rowptr = c->cellplans[i].rowptr; cf.rowlist = c->cellplans[i].rowlist;
-                cf.ncell_max = std::max(mx, 1);
+                cf.sorted = 1;
+                cf.ntile = sp.ntile;
+                cf.cellid = sh.cellid; cf.cellptr = sh.cellptr; cf.cellrows = sh.cellrows; cf.pospix = sh.pospix;
             }
         }
+        int32_t off = 0;
+        for (int t = 0; t < 4; ++t) {
+            cf.segbase[t] = off;
+            off += c->maps[cf.map[t]].nseg;
+        }
+    }
+    std::vector<MapDev> md(c->maps.size());
+    for (size_t m = 0; m < c->maps.size(); ++m) {
+        const MapHost &s = c->maps[m];
+        md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.segslot, s.ksegptr, s.chunkptr, s.segcfirst, s.K, s.nseg};
     }
     if ((rc = dev_upload(&c->d_maps, md, &c->cluster_bytes)) || (rc = dev_upload(&c->d_cfgs, c->cfgs, &c->cluster_bytes)) ||
         (rc = dev_upload(&c->d_npix_live, c->npix_live, &c->cluster_bytes))) {
@@ -575,39 +724,21 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
         return rc;
     }
     return CS_OK;
+    CS_GUARD_END
 }
 
-int cs_set_data(cs_ctx *c, int32_t ndata, const float *d, const float *ninv) {
-    if (!c || ndata <= 0 || !d || !ninv) return CS_EINVAL;
-    float w[NROW] = {0};
-    CK(cudaMemcpy(w, ninv, sizeof(float) * c->nfreq, cudaMemcpyDefault));
-    double m00 = 0;
-    for (int f = 0; f < c->nfreq; ++f) {
-        if (!(w[f] > 0.f) || !std::isfinite(w[f])) return CS_EINVAL;
-        m00 += (double)w[f];
-    }
-    std::memset(&c->kc, 0, sizeof(c->kc));
-    float m00f = 0.f;
-    for (int f = 0; f < c->nfreq; ++f) {
-        c->kc.w[f] = w[f];
-        c->kc.lnd[f] = (float)c->tc.lnd[f];
-        c->kc.lnsw[f] = (float)(c->tc.lns[f] * (double)w[f]);
-        c->kc.lns[f] = (float)c->tc.lns[f];
-        c->kc.invw[f] = 1.0f / w[f];
-        m00f += w[f];
-    }
-    (void)m00f;
-    c->kc.m00 = (float)m00;
-    c->kc.inv_m00 = (float)(1.0 / m00);
-    c->d = d;
-    c->ndata = ndata;
-    c->have_ninv = true;
-    int rc = make_tmap(c);
-    if (rc) return rc;
-    for (int e = 0; e < c->batch; ++e)
-        if (c->data_of[e] >= ndata) return CS_EINVAL;
+int cs_layout_info(cs_ctx *c, int32_t cfg, int32_t *sorted, int32_t *ntile, double *fill) {
+    if (!c || cfg < 0 || cfg >= c->ncfg) return CS_EINVAL;
+    const CfgDev &cf = c->cfgs[cfg];
+    int64_t live = 0;
+    for (int r = 0; r < c->nregion; ++r) live += c->npix_live[(size_t)cfg * c->nregion + r];
+    if (sorted) *sorted = cf.sorted;
+    if (ntile) *ntile = cf.ntile;
+    if (fill) *fill = (double)live / ((double)cf.ntile * TPX);
     return CS_OK;
 }
+
+int cs_set_data(cs_ctx *c, int32_t ndata, const float *d, const float *ninv) { return set_data_impl(c, ndata, d, ninv, true); }
 
 int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t *data_of) {
     if (!c || c->maps.empty() || batch <= 0 || !cfg_of || !data_of) return CS_EINVAL;
@@ -615,63 +746,110 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         if (cfg_of[e] < 0 || cfg_of[e] >= c->ncfg || data_of[e] < 0) return CS_EINVAL;
         if (c->d && data_of[e] >= c->ndata) return CS_EINVAL;
     }
+    CS_GUARD_BEGIN
     cudaDeviceSynchronize();
     free_batch(c);
     c->cfg_of.assign(cfg_of, cfg_of + batch);
     c->data_of.assign(data_of, data_of + batch);
     c->param_off.assign(batch + 1, 0);
     std::vector<int64_t> tab_off(batch);
-    int64_t rows = 0, PS = 4 * (int64_t)c->maps[c->nmap].nseg;
+    const int32_t nseg_reg = c->maps[c->nmap].nseg;
+    int64_t rows = 0, PS = 4 * (int64_t)nseg_reg;
     int32_t kmax = 0;
     for (int32_t e = 0; e < batch; ++e) {
         const CfgDev &cf = c->cfgs[cfg_of[e]];
         c->param_off[e + 1] = c->param_off[e] + cf.ktot;
         tab_off[e] = rows;
         rows += cf.K[0] + 2 * (int64_t)cf.K[1] + cf.K[2];
-        PS = std::max<int64_t>(PS, (int64_t)cf.segbase[3] + c->maps[c->nmap].nseg);
+        const int64_t nreg = c->maps[cf.map[3]].nseg;
+        PS = std::max<int64_t>(PS, std::max<int64_t>((int64_t)cf.segbase[3] + nreg, 4 * nreg));
         kmax = std::max(kmax, cf.ktot);
     }
     c->nparam = c->param_off[batch];
     c->nrows = rows; c->PS = PS; c->ktot_max = kmax;
-    // entries grouped by configuration (stable), cut into groups of <= GROUP_MAX
-    std::vector<int32_t> elist(batch);
-    for (int32_t e = 0; e < batch; ++e) elist[e] = e;
-    // cell-path configurations first, then the direct ones; stable inside a configuration
-    auto key = [&](int32_t e) { return ((int64_t)(c->cfgs[cfg_of[e]].ncell_max > 0 ? 0 : 1) << 32) | (int64_t)cfg_of[e]; };
-    std::stable_sort(elist.begin(), elist.end(), [&](int32_t a, int32_t b) { return key(a) < key(b); });
-    // a group runs on the cell kernel when its configuration has a cell plan and it is long enough to amortise that
-    // kernel's per-CTA set-up (plan loading, ring fill); short groups (configuration scans: one entry per
-    // configuration) are ~2x faster on the direct kernel.  Cell-kernel groups come first in the array.
-    std::vector<Group> groups, direct;
+    // entries ordered by (kernel form, configuration), stable; a run = all entries of one configuration
+    const bool force_direct = c->opt_form == CS_FORM_DIRECT;
+    c->elist.resize(batch);
+    for (int32_t e = 0; e < batch; ++e) c->elist[e] = e;
+    auto is_sc = [&](int32_t e) { return c->cfgs[cfg_of[e]].sorted && !force_direct; };
+    auto key = [&](int32_t e) { return ((int64_t)(is_sc(e) ? 0 : 1) << 32) | (int64_t)cfg_of[e]; };
+    std::stable_sort(c->elist.begin(), c->elist.end(), [&](int32_t a, int32_t b) { return key(a) < key(b); });
+    c->runs.clear();
+    c->nrun_sc = c->nrun_dir = 0;
+    c->W_sc = c->W_dir = 0;
     for (int32_t i = 0; i < batch;) {
         int32_t j = i;
-        while (j < batch && cfg_of[elist[j]] == cfg_of[elist[i]] && j - i < GROUP_MAX) ++j;
-        const Group g{cfg_of[elist[i]], i, j - i, 0};
-        if (c->cfgs[g.cfg].ncell_max > 0 && g.count >= c->cell_min_group) groups.push_back(g);
-        else direct.push_back(g);
+        while (j < batch && cfg_of[c->elist[j]] == cfg_of[c->elist[i]]) ++j;
+        const CfgDev &cf = c->cfgs[cfg_of[c->elist[i]]];
+        const bool sc = is_sc(c->elist[i]);
+        Run r{cfg_of[c->elist[i]], i, j - i, cf.ntile, sc ? c->W_sc : c->W_dir};
+        const int64_t units = (int64_t)cf.ntile * (j - i);
+        if (sc) { c->W_sc += units; c->nrun_sc++; } else { c->W_dir += units; c->nrun_dir++; }
+        c->runs.push_back(r);
         i = j;
     }
-    c->ngroup_cell = (int32_t)groups.size();
-    groups.insert(groups.end(), direct.begin(), direct.end());
-    c->ngroup = (int32_t)groups.size();
+    // private copies of the sorted layout: one per (configuration, data set) pair, ordered by data set
+    c->jobs.clear();
+    c->copy_off.assign(batch, -1);
+    c->job_ntile_max = 0;
+    int64_t copy_floats = 0;
+    {
+        std::map<std::pair<int32_t, int32_t>, int64_t> seen;   // (data, cfg) -> offset
+        std::vector<std::pair<int32_t, int32_t>> order;
+        for (int32_t e = 0; e < batch; ++e)
+            if (c->cfgs[cfg_of[e]].sorted) {
+                const auto k = std::make_pair(data_of[e], cfg_of[e]);
+                if (seen.emplace(k, 0).second) order.push_back(k);
+            }
+        std::sort(order.begin(), order.end());
+        for (const auto &k : order) {
+            const CfgDev &cf = c->cfgs[k.second];
+            seen[k] = copy_floats;
+            c->jobs.push_back(CopyJob{k.second, k.first, copy_floats});
+            copy_floats += (int64_t)cf.ntile * 2 * c->nfreq * TPX;
+            c->job_ntile_max = std::max(c->job_ntile_max, cf.ntile);
+        }
+        for (int32_t e = 0; e < batch; ++e)
+            if (c->cfgs[cfg_of[e]].sorted) c->copy_off[e] = seen[std::make_pair(data_of[e], cfg_of[e])];
+    }
+    const int64_t copy_bytes = copy_floats * 4;
+    if (copy_bytes > 0) {
+        int64_t limit = c->opt_copy_limit;
+        if (limit == 0) {
+            size_t fr = 0, tot = 0;
+            CK(cudaMemGetInfo(&fr, &tot));
+            limit = (int64_t)(0.7 * (double)fr);
+        }
+        if (copy_bytes > limit) { free_batch(c); return CS_ENOMEM; }
+    }
     int rc;
-    std::vector<int32_t> zero_i(batch, 0);
-    std::vector<Group> zero_g(batch, Group{0, 0, 0, 0});
     if ((rc = dev_upload(&c->d_cfg_of, c->cfg_of, &c->batch_bytes)) || (rc = dev_upload(&c->d_data_of, c->data_of, &c->batch_bytes)) ||
-        (rc = dev_upload(&c->d_elist, elist, &c->batch_bytes)) || (rc = dev_upload(&c->d_sel_elist, zero_i, &c->batch_bytes)) ||
+        (rc = dev_upload(&c->d_elist, c->elist, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_param_off, c->param_off, &c->batch_bytes)) || (rc = dev_upload(&c->d_tab_off, tab_off, &c->batch_bytes)) ||
-        (rc = dev_upload(&c->d_groups, groups, &c->batch_bytes)) || (rc = dev_upload(&c->d_sel_groups, zero_g, &c->batch_bytes))) {
+        (rc = dev_upload(&c->d_copy_off, c->copy_off, &c->batch_bytes)) || (rc = dev_upload(&c->d_runs, c->runs, &c->batch_bytes)) ||
+        (rc = dev_upload(&c->d_jobs, c->jobs, &c->batch_bytes))) {
         free_batch(c);
         return rc;
     }
     const size_t tab_bytes = (size_t)rows * NROW * sizeof(float), part_bytes = (size_t)batch * PS * sizeof(double);
-    if (cudaMalloc((void **)&c->d_tab, tab_bytes) != cudaSuccess || cudaMalloc((void **)&c->d_partial, part_bytes) != cudaSuccess) {
+    c->sel_cap = (((int64_t)batch * (1 + (int64_t)(sizeof(Run) / 4)) + 8) + 3) & ~(int64_t)3;   // slots stay 16-byte aligned
+    if (cudaMalloc((void **)&c->d_tab, tab_bytes) != cudaSuccess || cudaMalloc((void **)&c->d_partial, part_bytes) != cudaSuccess ||
+        (copy_bytes > 0 && cudaMalloc((void **)&c->d_copy, (size_t)copy_bytes) != cudaSuccess) ||
+        cudaMalloc((void **)&c->d_sel, (size_t)(cs_ctx::SEL_RING * c->sel_cap * 4)) != cudaSuccess ||
+        cudaMallocHost((void **)&c->h_sel, (size_t)(cs_ctx::SEL_RING * c->sel_cap * 4)) != cudaSuccess) {
+        cudaGetLastError();
         free_batch(c);
         return CS_ENOMEM;
     }
-    c->batch_bytes += (int64_t)(tab_bytes + part_bytes);
+    c->batch_bytes += (int64_t)(tab_bytes + part_bytes) + copy_bytes + cs_ctx::SEL_RING * c->sel_cap * 4;
+    c->copy_bytes = copy_bytes;
     c->batch = batch;
+    if (c->d && !c->jobs.empty()) {
+        if ((rc = relayout(c, c->d, 0, (int64_t)c->jobs.size(), nullptr))) { free_batch(c); return rc; }
+        CK(cudaDeviceSynchronize());
+    }
     return CS_OK;
+    CS_GUARD_END
 }
 
 int cs_param_offsets(cs_ctx *c, int64_t *off) {
@@ -712,7 +890,7 @@ int cs_spectral_like_grad(cs_ctx *c, double *nll, double *grad, void *stream) {
     if (!nll || !c->tables_built) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     LikeParams P = base_params(c);
-    rc = grad ? launch_like<MODE_GRAD>(c, P, 0, c->ngroup, c->ngroup_cell, st) : launch_like<MODE_VALUE>(c, P, 0, c->ngroup, c->ngroup_cell, st);
+    rc = grad ? launch_batch<MODE_GRAD>(c, P, st) : launch_batch<MODE_VALUE>(c, P, st);
     if (rc) return rc;
     return merge_launch(c, nll, grad, st);
 }
@@ -723,7 +901,7 @@ int cs_spectral_misfit(cs_ctx *c, double *chi2, void *stream) {
     if (!chi2 || !c->tables_built) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     LikeParams P = base_params(c);
-    if ((rc = launch_like<MODE_CHI2>(c, P, 0, c->ngroup, c->ngroup_cell, st))) return rc;
+    if ((rc = launch_batch<MODE_CHI2>(c, P, st))) return rc;
     return merge_launch(c, chi2, nullptr, st);
 }
 
@@ -733,39 +911,40 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
     if (!s || !c->tables_built || nsel <= 0 || nsel > c->batch) return CS_EINVAL;
     if (!entries && nsel != c->batch) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    std::vector<int32_t> el(nsel);
-    std::vector<Group> gr;
-    gr.reserve(nsel);
+    // The selection (entry list, then its runs = stretches of consecutive selected entries of one configuration) goes
+    // through a small ring of pinned staging slots, so that the call never synchronises the caller's stream; a slot is
+    // reused only after the copy that read it has completed.
+    const int slot = (int)(c->sel_n % cs_ctx::SEL_RING);
+    if (!c->sel_ev[slot]) CK(cudaEventCreateWithFlags(&c->sel_ev[slot], cudaEventDisableTiming));
+    else CK(cudaEventSynchronize(c->sel_ev[slot]));
+    int32_t *hs = c->h_sel + slot * c->sel_cap, *ds = c->d_sel + slot * c->sel_cap;
     for (int32_t i = 0; i < nsel; ++i) {
         const int32_t e = entries ? entries[i] : i;
         if (e < 0 || e >= c->batch) return CS_EINVAL;
-        el[i] = e;
+        hs[i] = e;
     }
-    // groups = runs of consecutive selected entries of one configuration (a group's start is its first output slot);
-    // cell-path groups first
-    int32_t ncell = 0;
-    for (int pass = 0; pass < 2; ++pass)
-        for (int32_t i = 0; i < nsel;) {
-            const int32_t cf = c->cfg_of[el[i]];
-            int32_t j = i;
-            while (j < nsel && c->cfg_of[el[j]] == cf && j - i < GROUP_MAX) ++j;
-            const bool cellp = c->cfgs[cf].ncell_max > 0 && j - i >= c->cell_min_group;
-            if (cellp == (pass == 0)) {
-                gr.push_back(Group{cf, i, j - i, 0});
-                if (pass == 0) ++ncell;
-            }
-            i = j;
-        }
-    const int32_t ngr = (int32_t)gr.size();
-    // small synchronous uploads: map output is not on the optimizer's hot path
-    CK(cudaStreamSynchronize(st));
-    CK(cudaMemcpy(c->d_sel_elist, el.data(), sizeof(int32_t) * nsel, cudaMemcpyHostToDevice));
-    CK(cudaMemcpy(c->d_sel_groups, gr.data(), sizeof(Group) * ngr, cudaMemcpyHostToDevice));
+    const int64_t roff = ((int64_t)nsel + 1) & ~(int64_t)1;   // runs start 8-byte aligned
+    Run *hr = reinterpret_cast<Run *>(hs + roff);
+    int32_t nrun = 0;
+    int64_t W = 0;
+    for (int32_t i = 0; i < nsel;) {
+        const int32_t cf = c->cfg_of[hs[i]];
+        int32_t j = i;
+        while (j < nsel && c->cfg_of[hs[j]] == cf) ++j;
+        hr[nrun++] = Run{cf, i, j - i, c->ntile_ring, W};
+        W += (int64_t)c->ntile_ring * (j - i);
+        i = j;
+    }
+    const size_t bytes = (size_t)roff * 4 + (size_t)nrun * sizeof(Run);
+    CK(cudaMemcpyAsync(ds, hs, bytes, cudaMemcpyHostToDevice, st));
+    CK(cudaEventRecord(c->sel_ev[slot], st));
+    c->sel_n++;
     LikeParams P = base_params(c);
-    P.groups = c->d_sel_groups;
-    P.elist = c->d_sel_elist;
+    P.elist = ds;
     P.maps_out = s;
-    return launch_like<MODE_MAPS>(c, P, 0, ngr, ncell, st);
+    P.ring_maps = 1;
+    P.evict_first = ((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4 > (int64_t)96 << 20) ? 1 : 0;
+    return launch_like<MODE_MAPS>(c, P, reinterpret_cast<const Run *>(ds + roff), 0, 0, nrun, W, st);
 }
 
 int cs_cmb_variance(cs_ctx *c, double *var, void *stream) {
@@ -774,7 +953,7 @@ int cs_cmb_variance(cs_ctx *c, double *var, void *stream) {
     if (!var || !c->tables_built) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     LikeParams P = base_params(c);
-    if ((rc = launch_like<MODE_CMBVAR>(c, P, 0, c->ngroup, c->ngroup_cell, st))) return rc;
+    if ((rc = launch_batch<MODE_CMBVAR>(c, P, st))) return rc;
     const int n = c->batch * c->nregion;
     k_cmbvar<<<(n + 127) / 128, 128, 0, st>>>(c->d_partial, c->PS, c->d_maps, c->d_cfgs, c->d_cfg_of, c->d_npix_live,
                                              c->nregion, c->batch, var);
@@ -854,7 +1033,7 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
     cudaStreamIsCapturing(st, &cap);
     bool replayed = false;
     if (opt->iters > 1 && cap == cudaStreamCaptureStatusNone && !c->prof_on) {
-        if (opt->iters > 0 && (rc = iteration())) return rc;     // first iteration directly: sets function attributes, warms up
+        if (opt->iters > 0 && (rc = iteration())) return rc;     // first iteration directly: warms up
         const int64_t l0 = c->launches;
         cudaGraph_t graph = nullptr;
         cudaGraphExec_t exec = nullptr;
@@ -892,6 +1071,7 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
     if (!c || c->batch <= 0 || c->maps.empty() || !d_host || !ninv_host || !params_host || !nll_host || ndata <= 0) return CS_EINVAL;
     for (int32_t e = 0; e < c->batch; ++e)
         if (c->data_of[e] >= ndata || (e > 0 && c->data_of[e] < c->data_of[e - 1])) return CS_EINVAL;
+    CS_GUARD_BEGIN
     const int64_t per = (int64_t)c->nfreq * 2 * c->npix;
     const int64_t need = per * ndata * (int64_t)sizeof(float);
     if (c->stage_bytes < need) {
@@ -909,40 +1089,68 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
     }
     if (!c->copy_stream) CK(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
     if (!c->comp_stream) CK(cudaStreamCreateWithFlags(&c->comp_stream, cudaStreamNonBlocking));
-    int rc = cs_set_data(c, ndata, c->d_stage, ninv_host);   // the staged copy becomes the context's data
+    int rc = set_data_impl(c, ndata, c->d_stage, ninv_host, false);   // the staged copy becomes the context's data
     if (rc) return rc;
     cudaStream_t cp = c->copy_stream, cm = c->comp_stream;
     // parameters and tables on the compute stream while the first data chunk is in flight on the copy stream
     CK(cudaMemcpyAsync(c->d_hparams, params_host, sizeof(double) * c->nparam, cudaMemcpyHostToDevice, cm));
     if ((rc = cs_build_sed_tables(c, c->d_hparams, cm))) return rc;
-    // upload in chunks of data sets; after each chunk, launch (on the compute stream, behind an event) the groups
-    // whose data are resident, so that the next chunk's copy overlaps their kernels.
-    std::vector<Group> groups(c->ngroup);
-    std::vector<int32_t> elist(c->batch);
-    CK(cudaMemcpy(groups.data(), c->d_groups, sizeof(Group) * c->ngroup, cudaMemcpyDeviceToHost));
-    CK(cudaMemcpy(elist.data(), c->d_elist, sizeof(int32_t) * c->batch, cudaMemcpyDeviceToHost));
-    std::vector<int32_t> gmax(c->ngroup, 0);
-    for (int g = 0; g < c->ngroup; ++g)
-        for (int i = 0; i < groups[g].count; ++i) gmax[g] = std::max(gmax[g], c->data_of[elist[groups[g].start + i]]);
-    std::vector<char> done(c->ngroup, 0);
+    // Upload in chunks of data sets; after each chunk, on the compute stream and behind an event: gather the private
+    // copies of the data sets that arrived, then run the entries whose data are resident, so that the next chunk's
+    // copy overlaps their kernels.  data_of is non-decreasing, so inside every run the entries of a chunk are a
+    // contiguous stretch.
     const int64_t chunk_sets = std::max<int64_t>(1, (int64_t)(128ll << 20) / (per * 4));
+    const int64_t nchunk = (ndata + chunk_sets - 1) / chunk_sets;
+    const int64_t nrun_all = (int64_t)c->runs.size();
+    if (c->hruns_cap < nchunk * nrun_all) {
+        cudaFree(c->d_hruns);
+        c->d_hruns = nullptr; c->hruns_cap = 0;
+        if (cudaMalloc((void **)&c->d_hruns, sizeof(Run) * (size_t)(nchunk * nrun_all)) != cudaSuccess) return CS_ENOMEM;
+        c->hruns_cap = nchunk * nrun_all;
+    }
+    std::vector<Run> hr((size_t)(nchunk * nrun_all));
+    std::vector<int32_t> cnt_sc(nchunk, 0), cnt_dir(nchunk, 0);
+    std::vector<int64_t> Wsc(nchunk, 0), Wdir(nchunk, 0);
+    for (int64_t ch = 0; ch < nchunk; ++ch) {
+        const int64_t n0 = ch * chunk_sets, n1 = std::min<int64_t>(ndata, n0 + chunk_sets);
+        Run *out = hr.data() + ch * nrun_all;
+        for (int pass = 0; pass < 2; ++pass)
+            for (int64_t r = 0; r < nrun_all; ++r) {
+                const Run &run = c->runs[r];
+                const bool sc = r < c->nrun_sc;
+                if (sc != (pass == 0)) continue;
+                int32_t a = run.estart, b = run.estart + run.count;
+                while (a < b && c->data_of[c->elist[a]] < n0) ++a;
+                int32_t e2 = a;
+                while (e2 < b && c->data_of[c->elist[e2]] < n1) ++e2;
+                if (e2 == a) continue;
+                int64_t &W = sc ? Wsc[ch] : Wdir[ch];
+                out[cnt_sc[ch] + cnt_dir[ch]] = Run{run.cfg, a, e2 - a, run.ntile, W};
+                W += (int64_t)run.ntile * (e2 - a);
+                (sc ? cnt_sc[ch] : cnt_dir[ch])++;
+            }
+    }
+    CK(cudaMemcpyAsync(c->d_hruns, hr.data(), sizeof(Run) * hr.size(), cudaMemcpyHostToDevice, cm));
     LikeParams P = base_params(c);
     std::vector<cudaEvent_t> evs;
     rc = CS_OK;
-    for (int64_t n0 = 0; n0 < ndata && rc == CS_OK; n0 += chunk_sets) {
-        const int64_t n1 = std::min<int64_t>(ndata, n0 + chunk_sets);
+    size_t j0 = 0;
+    for (int64_t ch = 0; ch < nchunk && rc == CS_OK; ++ch) {
+        const int64_t n0 = ch * chunk_sets, n1 = std::min<int64_t>(ndata, n0 + chunk_sets);
         cudaEvent_t ev;
         if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { rc = CS_ECUDA; break; }
         evs.push_back(ev);
         if (cudaMemcpyAsync(c->d_stage + n0 * per, d_host + n0 * per, (size_t)((n1 - n0) * per) * sizeof(float),
                             cudaMemcpyHostToDevice, cp) != cudaSuccess ||
             cudaEventRecord(ev, cp) != cudaSuccess || cudaStreamWaitEvent(cm, ev, 0) != cudaSuccess) { rc = CS_ECUDA; break; }
-        for (int g = 0; g < c->ngroup && rc == CS_OK;) {
-            if (done[g] || gmax[g] >= n1) { ++g; continue; }
-            int h = g;
-            while (h < c->ngroup && !done[h] && gmax[h] < n1) { done[h] = 1; ++h; }
-            rc = grad_host ? launch_like<MODE_GRAD>(c, P, g, h, c->ngroup_cell, cm) : launch_like<MODE_VALUE>(c, P, g, h, c->ngroup_cell, cm);
-            g = h;
+        size_t j1 = j0;
+        while (j1 < c->jobs.size() && c->jobs[j1].data < n1) ++j1;
+        if (j1 > j0) rc = relayout(c, c->d_stage, (int64_t)j0, (int64_t)j1, cm);
+        j0 = j1;
+        if (rc == CS_OK && cnt_sc[ch] + cnt_dir[ch] > 0) {
+            const Run *dr = c->d_hruns + ch * nrun_all;
+            rc = grad_host ? launch_like<MODE_GRAD>(c, P, dr, cnt_sc[ch], Wsc[ch], cnt_dir[ch], Wdir[ch], cm)
+                           : launch_like<MODE_VALUE>(c, P, dr, cnt_sc[ch], Wsc[ch], cnt_dir[ch], Wdir[ch], cm);
         }
     }
     if (rc == CS_OK) rc = merge_launch(c, c->d_hnll, grad_host ? c->d_hgrad : nullptr, cm);
@@ -951,6 +1159,7 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
     if (cudaStreamSynchronize(cp) != cudaSuccess || cudaStreamSynchronize(cm) != cudaSuccess) rc = rc ? rc : CS_ECUDA;
     for (cudaEvent_t ev : evs) cudaEventDestroy(ev);
     return rc;
+    CS_GUARD_END
 }
 
 int cs_check(cs_ctx *c, void *stream) {

@@ -1,0 +1,372 @@
+// cs_like_sc.cuh -- k_like_sc: the fused per-pixel kernel (a2 + first level of a3, f1) on the sorted layout.
+//
+// Everything in Eq. 5/6/17 that depends on the parameters depends on the pixel only through its cluster triple
+// (k0,k1,k2): the weighted columns N^-1 a_d, N^-1 a_s and their derivatives, the matrix M = A^T N^-1 A,
+// its LDL^T factors and the nine contractions P_{theta,c} = sum_f w_f (da_f/dtheta) A_{f,c}.  Pixels with the same
+// triple (and region) form a *cell*.  In the sorted layout (cs_internal.h) the pixels of a cell are consecutive and every
+// consumer thread owns two positions of one cell, so per entry a builder lane evaluates the per-cell part once per cell
+// of the tile, and a pixel-eval is left with
+//
+//     b_S  = A^T N^-1 d_S                        (3 dots per Stokes)            Eq. 5
+//     c_S  = (dA/dtheta)^T N^-1 d_S              (3 dots per Stokes)
+//     s_S  = M^-1 b_S  via the cell's LDL^T ;   ll = -1/2 sum_S b_S . s_S       Eq. 5, 6
+//     g_th = - sum_S s_{S,c(th)} ( c_{S,th} - sum_c P_{th,c} s_{S,c} )          Eq. 17 with r = d - A s expanded
+//
+// evaluated for the thread's two pixels at once: 12 packed FFMA2 per band whose coefficient operand is a per-cell
+// scalar (broadcast operand form), data read as one LDS.64 per band and Stokes parameter.
+//
+// Persistent grid: one CTA per SM, each walking a contiguous, equal share of all (tile, entry) units (cs_pipe.cuh).
+// CTA = 12 warps (so that a thread may hold up to 168 registers), warp-specialised; every hand-over is an mbarrier full/empty pair or a hardware named barrier, no
+// CTA-wide barrier after the prologue:
+//   warps 0-7    consumers: positions (2t, 2t+1) of the 512-position tile per thread, one entry after the other
+//   warps 8-9    reducers : first level of the ordered fp64 reduction (a3) of the pair sums the consumers leave behind;
+//                           warp r owns term-ring slot r and the entries n = r (mod 2)
+//   warp  10     builder  : lane c builds cell c of the tile for the next entry (five weighted columns, LDL^T, P)
+//   warp  11     loader   : one 60-KB bulk copy per entry into the data ring
+// shared memory: data ring [ND][2 halves][2*NF][256] | cell tables [NC][CELL_CAP][CROW] | term ring [NT][4][256] fp64 |
+//                reducer plans | barriers
+#pragma once
+#include "cs_pipe.cuh"
+#include "cs_math.cuh"
+
+namespace cs {
+
+constexpr int SC_ND = 3;        // data ring depth (2 for the generic band count, whose stages are 16 bands tall)
+template <int NF>
+struct ScDepth { static constexpr int value = (NF == 15) ? SC_ND : 2; };
+constexpr int SC_NC = 2;        // cell-table ring depth
+constexpr int SC_NBW = 1;       // builder warps (warp b takes the entries n = b mod SC_NBW; SC_NC is a multiple of it)
+constexpr int SC_NT = 2;        // term ring depth = reducer warps
+constexpr int SC_THREADS = NCONS + (SC_NT + SC_NBW + 1) * 32;   // 384
+constexpr int SC_WARP_RED = NCONS / 32, SC_WARP_BUILD = SC_WARP_RED + SC_NT, SC_WARP_LOAD = SC_WARP_BUILD + SC_NBW;
+constexpr int SC_PLAN_BYTES = SC_CHUNK_CAP * 2 + SC_SEG_CAP * 2 + SC_SEG_CAP * 4 + 16;   // one reducer warp's plan
+
+template <int NF>
+constexpr size_t sc_smem_bytes() {
+    return (size_t)ScDepth<NF>::value * 2 * NF * TPX * 4   // data ring
+           + (size_t)SC_NC * CELL_CAP * CROW * 4       // cell tables
+           + (size_t)SC_NT * 4 * NCONS * 8             // term ring (fp64 pair sums)
+           + (size_t)SC_NT * SC_PLAN_BYTES             // reducer plans (one copy per reducer warp)
+           + (2 * ScDepth<NF>::value + 2 * SC_NC + SC_NT) * 8   // mbarriers
+           + 16;
+}
+
+// Reducer plan of a tile: every (term, cluster) segment of <= SEG_MAX rank-ordered terms is cut into 1..4 chunks of
+// <= CHUNK_LEN ranks.  In the sorted layout all starts and lengths are even; the plan is kept in pairs:
+// s_cdesc[chunk] = first pair (8 bits) | (pairs-1) << 8 | term << 10;
+// s_sdesc[segment] = first pair (8 bits) | (chunks-1) << 8 | term << 10; s_slot[segment] = slot in the entry's partial row.
+template <int MODE>
+__device__ __forceinline__ void sc_load_plan(const MapDev *__restrict__ maps, const CfgDev &cfg, int tile, int lane,
+                                             uint16_t *s_cdesc, uint16_t *s_sdesc, int32_t *s_slot, int32_t *meta) {
+    constexpr int T0 = ModeTraits<MODE>::region_only ? 3 : 0;
+    int sbase = 0, cbase = 0;
+#pragma unroll
+    for (int t = T0; t < 4; ++t) {
+        const MapDev m = maps[(MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t]];
+        const int s0 = m.segptr[tile], ns = m.segptr[tile + 1] - s0;
+        const int nc = m.chunkptr[tile + 1] - m.chunkptr[tile];
+        for (int i = lane; i < ns; i += 32) {
+            const uint32_t desc = m.segdesc[s0 + i];
+            const int start = desc & 0x1ff, len = (int)(desc >> 9) + 1;
+            const int first = cbase + m.segcfirst[s0 + i], cnt = (len + CHUNK_LEN - 1) / CHUNK_LEN;
+            s_sdesc[sbase + i] = (uint16_t)((start >> 1) | ((cnt - 1) << 8) | (t << 10));
+            s_slot[sbase + i] = ((MODE == MODE_CMBVAR) ? t * m.nseg : cfg.segbase[t]) + m.segslot[s0 + i];
+            for (int q = 0; q < cnt; ++q) {
+                const int l = min(CHUNK_LEN, len - CHUNK_LEN * q);
+                s_cdesc[first + q] = (uint16_t)(((start + CHUNK_LEN * q) >> 1) | ((l / 2 - 1) << 8) | (t << 10));
+            }
+        }
+        sbase += ns; cbase += nc;
+    }
+    if (lane == 0) { meta[0] = cbase; meta[1] = sbase; }
+    __syncwarp();
+}
+
+// First level of the ordered reduction (a3) of one entry by a reducer warp, in fp64 and in a fixed order:
+// step 1, one lane per chunk: (y0 + y1) + (y2 + y3) over the chunk's <= 4 pair sums (cs_math.cuh: chunk_tree), left in
+// place of the chunk's first pair sum; step 2, one lane per segment: the segment's chunk sums left to right, stored at
+// the segment's cluster-major slot of the entry's partial row.  Two chunks / segments per lane and round are in flight.
+__device__ __forceinline__ double sc_chunk(const double *tbuf, uint32_t d, int &at) {
+    const int p0 = d & 0xff, np = (int)((d >> 8) & 3) + 1, t = (int)(d >> 10);
+    at = t * NCONS + p0;
+    const double *y = tbuf + at;
+    const double y0 = y[0], y1 = np > 1 ? y[1] : 0.0, y2 = np > 2 ? y[2] : 0.0, y3 = np > 3 ? y[3] : 0.0;
+    return chunk_tree(y0, y1, y2, y3);
+}
+__device__ __forceinline__ double sc_segment(const double *tbuf, uint32_t d) {
+    const int p0 = d & 0xff, cnt = (int)((d >> 8) & 3) + 1, t = (int)(d >> 10);
+    const double *y = tbuf + t * NCONS + p0;
+    double acc = y[0];
+    if (cnt > 1) acc += y[CHUNK_LEN / 2];
+    if (cnt > 2) acc += y[CHUNK_LEN];
+    if (cnt > 3) acc += y[3 * CHUNK_LEN / 2];
+    return acc;
+}
+__device__ __forceinline__ void sc_reduce_entry(double *tbuf, int lane, const int32_t *meta, const uint16_t *s_cdesc,
+                                                const uint16_t *s_sdesc, const int32_t *s_slot, double *__restrict__ prow) {
+    const int nchunk = meta[0], nseg = meta[1];
+    for (int r = lane; r < nchunk; r += 64) {
+        int a0, a1 = 0;
+        const bool two = r + 32 < nchunk;
+        const uint32_t d0 = s_cdesc[r], d1 = two ? s_cdesc[r + 32] : 0u;
+        const double c0 = sc_chunk(tbuf, d0, a0);
+        double c1 = 0.0;
+        if (two) c1 = sc_chunk(tbuf, d1, a1);
+        tbuf[a0] = c0;
+        if (two) tbuf[a1] = c1;
+    }
+    __syncwarp();
+    for (int r = lane; r < nseg; r += 64) {
+        const bool two = r + 32 < nseg;
+        const uint32_t d0 = s_sdesc[r], d1 = two ? s_sdesc[r + 32] : 0u;
+        const int slot0 = s_slot[r], slot1 = two ? s_slot[r + 32] : 0;
+        const double v0 = sc_segment(tbuf, d0);
+        double v1 = 0.0;
+        if (two) v1 = sc_segment(tbuf, d1);
+        prow[slot0] = v0;
+        if (two) prow[slot1] = v1;
+    }
+    __syncwarp();
+}
+
+// One cell (Eq. 2 columns -> five weighted columns, M, LDL^T, P; cs_math.cuh) from the entry's four table rows.
+// Cell row (floats): [0,16) w a_d | [16,32) w da_d/dbeta_d | [32,48) w da_d/dT_d | [48,64) w a_s | [64,80) w da_s/dbeta_s |
+// [80,96) l10 l20 l21 1/d1 | 1/d2 P10 P11 P12 | P20 P21 P22 P30 | P31 P32 bad -
+template <int NF, bool GRAD>
+__device__ __forceinline__ void sc_build_cell(const float4 (&Fd)[4], const float4 (&G)[4], const float4 (&dG)[4], const float4 (&Fs)[4],
+                                              const KConst &kc, float *__restrict__ out, int32_t *err) {
+    CellSums<float> S;
+    cell_sums_zero(S);
+    float4 *o4 = reinterpret_cast<float4 *>(out);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float vFd[4] = {Fd[q].x, Fd[q].y, Fd[q].z, Fd[q].w}, vG[4] = {G[q].x, G[q].y, G[q].z, G[q].w};
+        const float vdG[4] = {dG[q].x, dG[q].y, dG[q].z, dG[q].w}, vFs[4] = {Fs[q].x, Fs[q].y, Fs[q].z, Fs[q].w};
+        float wd[4] = {0.f, 0.f, 0.f, 0.f}, u1[4] = {0.f, 0.f, 0.f, 0.f}, u2[4] = {0.f, 0.f, 0.f, 0.f}, ws[4] = {0.f, 0.f, 0.f, 0.f},
+              u3[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            const int f = 4 * q + h;
+            if (f < NF) {   // bands beyond nfreq carry w = 0 and zero table entries: their columns come out as zero
+                CellCols<float> C;
+                cell_band<GRAD>(S, C, vFd[h], vG[h], vdG[h], vFs[h], kc.w[f], kc.lnd[f], kc.lns[f]);
+                wd[h] = C.wd; u1[h] = C.u1; u2[h] = C.u2; ws[h] = C.ws; u3[h] = C.u3;
+            }
+        }
+        o4[q] = make_float4(wd[0], wd[1], wd[2], wd[3]);
+        o4[12 + q] = make_float4(ws[0], ws[1], ws[2], ws[3]);
+        if (GRAD) {
+            o4[4 + q] = make_float4(u1[0], u1[1], u1[2], u1[3]);
+            o4[8 + q] = make_float4(u2[0], u2[1], u2[2], u2[3]);
+            o4[16 + q] = make_float4(u3[0], u3[1], u3[2], u3[3]);
+        }
+    }
+    CellScal<float> C;
+    cell_finish<GRAD>(S, kc.inv_m00, C);
+    if (C.bad != 0.f) atomicOr(err, ERR_SINGULAR);
+    o4[20] = make_float4(C.l10, C.l20, C.l21, C.id1);
+    o4[21] = make_float4(C.id2, C.P10, C.P11, C.P12);
+    o4[22] = make_float4(C.P20, C.P21, C.P22, C.P30);
+    o4[23] = make_float4(C.P31, C.P32, C.bad, 0.f);
+}
+
+template <int NF, int MODE>
+__global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int STAGE = 2 * NF * TPX;   // floats per data stage
+    constexpr int ND = ScDepth<NF>::value, NC = SC_NC, NT = SC_NT;
+    constexpr bool kGrad = ModeTraits<MODE>::grad;
+    float *ring = reinterpret_cast<float *>(smem_raw);
+    float *cells = ring + ND * STAGE;
+    double *sterm = reinterpret_cast<double *>(cells + NC * CELL_CAP * CROW);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sterm + NT * 4 * NCONS);
+    uint64_t *full_d = bars, *empty_d = bars + ND, *full_c = bars + 2 * ND, *empty_c = bars + 2 * ND + NC;
+    uint64_t *empty_t = bars + 2 * ND + 2 * NC;
+    unsigned char *plans = reinterpret_cast<unsigned char *>(empty_t + NT);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    // ---------------- prologue (all threads) ----------------
+    if (tid == 0) {
+        for (int s = 0; s < ND; ++s) { mbar_init(&full_d[s], 1); mbar_init(&empty_d[s], NCONS / 32); }
+        for (int s = 0; s < NC; ++s) { mbar_init(&full_c[s], 1); mbar_init(&empty_c[s], NCONS / 32); }
+        for (int s = 0; s < NT; ++s) mbar_init(&empty_t[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (NF * 2 != 2 * P.nfreq) {   // generic band count: rows beyond nfreq are never copied; they must read as zero
+        for (int i = tid; i < ND * STAGE; i += SC_THREADS) ring[i] = 0.f;
+    }
+    __syncthreads();
+
+    if (warp == SC_WARP_LOAD) {
+        loader_loop<NF, ND>(nullptr, P, ring, full_d, empty_d, lane);
+        return;
+    }
+    Walk w;
+    walk_init(w, P);
+    int n = 0;   // live entries so far (ring slots and barrier phases follow it)
+
+    if (warp >= SC_WARP_BUILD) {
+        // ---------------- builder warps: lane c builds cell c of the current tile; warp b takes the entries n = b (mod SC_NBW)
+        const int mine = warp - SC_WARP_BUILD;
+        while (walk_next(w, P)) {
+            const CfgDev *cf = P.cfgs + w.run.cfg;
+            const int c0 = __ldg(cf->cellptr + w.tile), ncell = __ldg(cf->cellptr + w.tile + 1) - c0;
+            int4 rows = make_int4(0, 0, 0, 0);
+            if (lane < ncell) rows = __ldg(reinterpret_cast<const int4 *>(cf->cellrows) + c0 + lane);
+            for (int k = w.k; k < w.kend; ++k) {
+                const int e = __ldg(P.elist + w.run.estart + k);
+                if (P.skip && __ldg(P.skip + e) != 0) continue;
+                const int s = n % NC;
+                if (SC_NBW > 1 && n % SC_NBW != mine) { ++n; continue; }
+                float4 Fd[4], G[4], dG[4], Fs[4];
+                if (lane < ncell) {
+                    const float *tb = P.tab + __ldg(P.tab_off + e) * NROW;
+                    const float4 *rFd = reinterpret_cast<const float4 *>(tb + (int64_t)rows.x * NROW);
+                    const float4 *rG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.y * NROW);
+                    const float4 *rdG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.z * NROW);
+                    const float4 *rFs = reinterpret_cast<const float4 *>(tb + (int64_t)rows.w * NROW);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        Fd[q] = __ldg(rFd + q); G[q] = __ldg(rG + q); Fs[q] = __ldg(rFs + q);
+                        dG[q] = kGrad ? __ldg(rdG + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                }
+                mbar_wait_relaxed(&empty_c[s], (uint32_t)(((n / NC) & 1) ^ 1));
+                if (lane < ncell) sc_build_cell<NF, kGrad>(Fd, G, dG, Fs, P.kc, cells + (s * CELL_CAP + lane) * CROW, P.err);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&full_c[s]);
+                ++n;
+            }
+        }
+        return;
+    }
+    if (warp >= SC_WARP_RED) {
+        // ---------------- reducer warps: first level of a3; warp r takes the entries n = r (mod NT) ----------------
+        const int mine = warp - SC_WARP_RED;
+        unsigned char *pl = plans + mine * SC_PLAN_BYTES;   // this warp's own copy of the tile's plan
+        int32_t *s_slot = reinterpret_cast<int32_t *>(pl);
+        int32_t *meta = s_slot + SC_SEG_CAP;
+        uint16_t *s_cdesc = reinterpret_cast<uint16_t *>(meta + 4);
+        uint16_t *s_sdesc = s_cdesc + SC_CHUNK_CAP;
+        while (walk_next(w, P)) {
+            const CfgDev cf = P.cfgs[w.run.cfg];
+            sc_load_plan<MODE>(P.maps, cf, w.tile, lane, s_cdesc, s_sdesc, s_slot, meta);
+            for (int k = w.k; k < w.kend; ++k) {
+                const int e = __ldg(P.elist + w.run.estart + k);
+                if (P.skip && __ldg(P.skip + e) != 0) continue;
+                const int s = n % NT;
+                if (s != mine) { ++n; continue; }
+                named_sync(1 + s, NCONS + 32);
+                sc_reduce_entry(sterm + s * 4 * NCONS, lane, meta, s_cdesc, s_sdesc, s_slot, P.partial + (int64_t)e * P.PS);
+                if (lane == 0) mbar_arrive(&empty_t[s]);
+                ++n;
+            }
+        }
+        return;
+    }
+
+    // ---------------- consumers ----------------
+    const float *st0 = ring + (tid >> 7) * (2 * NF * HALF) + ((2 * tid) & (HALF - 1));
+    const KConst &kc = P.kc;
+    while (walk_next(w, P)) {
+        const CfgDev *cf = P.cfgs + w.run.cfg;
+        const int cell = __ldg(cf->cellid + (int64_t)w.tile * NCONS + tid);
+        // slot of this thread's pair sums in each term row: half the rank of its first position
+        int so0 = 0, so1 = 0, so2 = 0, so3 = 0;
+        {
+            const int64_t pos = (int64_t)w.tile * TPX + 2 * tid;
+            const int m3 = cf->map[3];
+            if (MODE == MODE_CMBVAR) {
+                const int r = __ldg(P.maps[m3].rank + pos) >> 1;
+                so0 = r; so1 = NCONS + r; so2 = 2 * NCONS + r; so3 = 3 * NCONS + r;
+            } else {
+                if (kGrad) {
+                    so0 = __ldg(P.maps[cf->map[0]].rank + pos) >> 1;
+                    so1 = NCONS + (__ldg(P.maps[cf->map[1]].rank + pos) >> 1);
+                    so2 = 2 * NCONS + (__ldg(P.maps[cf->map[2]].rank + pos) >> 1);
+                }
+                so3 = 3 * NCONS + (__ldg(P.maps[m3].rank + pos) >> 1);
+            }
+        }
+        for (int k = w.k; k < w.kend; ++k) {
+            const int e = __ldg(P.elist + w.run.estart + k);
+            if (P.skip && __ldg(P.skip + e) != 0) continue;
+            const int sd = n % ND, sc = n % NC, stt = n % NT;
+            const float4 *crow = reinterpret_cast<const float4 *>(cells + (sc * CELL_CAP + cell) * CROW);
+            const float *st = st0 + sd * STAGE;
+            mbar_wait(&full_c[sc], (uint32_t)((n / NC) & 1));
+            mbar_wait(&full_d[sd], (uint32_t)((n / ND) & 1));
+            PixSums A;
+            pix_sums_zero(A);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 WD = crow[q], WS = crow[12 + q];
+                float4 U1 = make_float4(0.f, 0.f, 0.f, 0.f), U2 = U1, U3 = U1;
+                if (kGrad) { U1 = crow[4 + q]; U2 = crow[8 + q]; U3 = crow[16 + q]; }
+                const float wd[4] = {WD.x, WD.y, WD.z, WD.w}, ws[4] = {WS.x, WS.y, WS.z, WS.w};
+                const float u1[4] = {U1.x, U1.y, U1.z, U1.w}, u2[4] = {U2.x, U2.y, U2.z, U2.w}, u3[4] = {U3.x, U3.y, U3.z, U3.w};
+#pragma unroll
+                for (int h = 0; h < 4; ++h) {
+                    const int f = 4 * q + h;
+                    if (f < NF) {
+                        const float2 dq = *reinterpret_cast<const float2 *>(st + (2 * f) * HALF);
+                        const float2 du = *reinterpret_cast<const float2 *>(st + (2 * f + 1) * HALF);
+                        CellCols<float> C;
+                        C.wd = wd[h]; C.u1 = u1[h]; C.u2 = u2[h]; C.ws = ws[h]; C.u3 = u3[h];
+                        pix_band<kGrad>(A, C, kc.w[f], dq, du);
+                    }
+                }
+            }
+            const float4 S0 = crow[20], S1 = crow[21], S3 = crow[23];
+            float4 S2 = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (kGrad) S2 = crow[22];
+            CellScal<float> C;
+            C.l10 = S0.x; C.l20 = S0.y; C.l21 = S0.z; C.id1 = S0.w; C.id2 = S1.x;
+            C.P10 = S1.y; C.P11 = S1.z; C.P12 = S1.w; C.P20 = S2.x; C.P21 = S2.y; C.P22 = S2.z; C.P30 = S2.w;
+            C.P31 = S3.x; C.P32 = S3.y; C.bad = S3.z;
+            float2 sq[3], su[3], ll;
+            float2 t0 = make_float2(0.f, 0.f), t1 = t0, t2 = t0, t3 = t0;
+            if (MODE == MODE_CHI2) {   // second pass over the bands while the stages are still held: chi^2 of the residual
+                pix_solve(A, C, kc.inv_m00, sq, su, ll);
+                float2 xq = make_float2(0.f, 0.f), xu = xq;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 WD = crow[q], WS = crow[12 + q];
+                    const float wd[4] = {WD.x, WD.y, WD.z, WD.w}, ws[4] = {WS.x, WS.y, WS.z, WS.w};
+#pragma unroll
+                    for (int h = 0; h < 4; ++h) {
+                        const int f = 4 * q + h;
+                        if (f < NF) {
+                            const float2 dq = *reinterpret_cast<const float2 *>(st + (2 * f) * HALF);
+                            const float2 du = *reinterpret_cast<const float2 *>(st + (2 * f + 1) * HALF);
+                            pix_chi2_band(xq, xu, sq, su, wd[h], ws[h], kc.w[f], kc.invw[f], dq, du);
+                        }
+                    }
+                }
+                t3 = sel_inf(C.bad, add_(xq, xu));
+            }
+            __syncwarp();   // every lane has read its data and cell rows: hand the slots back
+            if (lane == 0) { mbar_arrive(&empty_d[sd]); mbar_arrive(&empty_c[sc]); }
+            if (MODE != MODE_CHI2) pix_solve(A, C, kc.inv_m00, sq, su, ll);
+            if (MODE == MODE_VALUE) {
+                t3 = ll;
+            } else if (MODE == MODE_GRAD) {
+                pix_grad_terms(A, C, sq, su, t0, t1, t2);
+                t3 = ll;
+            } else if (MODE == MODE_CMBVAR) {
+                t0 = sq[0]; t1 = su[0]; t2 = mul_(sq[0], sq[0]); t3 = mul_(su[0], su[0]);
+            }
+            mbar_wait(&empty_t[stt], (uint32_t)(((n / NT) & 1) ^ 1));
+            double *tm = sterm + stt * 4 * NCONS;
+            if (!ModeTraits<MODE>::region_only) {
+                tm[so0] = pair_sum(t0.x, t0.y); tm[so1] = pair_sum(t1.x, t1.y); tm[so2] = pair_sum(t2.x, t2.y);
+            }
+            tm[so3] = pair_sum(t3.x, t3.y);
+            named_arrive(1 + stt, NCONS + 32);
+            ++n;
+        }
+    }
+}
+
+}  // namespace cs

@@ -1,0 +1,176 @@
+// cs_tables.cuh -- the small kernels around the fused ones.
+//
+//   k_tables    a1  SED factor tables, fp64 math -> fp32 rows                     (Eq. 2)
+//   k_merge     a3  second level: fixed-order sum of per-tile partials onto clusters and regions
+//   k_cmbvar    f1  variance of the CMB map from the region-reduced sums          (Eq. 10)
+//   k_relayout      gathers a data set into the sorted layout of one configuration (cs_internal.h), once per
+//                   (configuration, data set) pair of a batch
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include "cs_internal.h"
+
+namespace cs {
+
+// ----------------------------------------------------------------------------------------------------------
+// a1: SED factor tables.  One thread per (entry, parameter, band quad).  fp64 -> fp32.
+// ----------------------------------------------------------------------------------------------------------
+// exp(y) in fp64 for the power-law rows: y = k ln2 + r, |r| <= ln2/2, degree-11 Taylor polynomial (truncation
+// 6e-15 relative, far below the fp32 rounding of the stored value), scaled by 2^k through the exponent field.
+// Arguments outside the range where 2^k is a normal number take the library routine.
+__device__ __forceinline__ double exp_pow(double y) {
+    if (!(fabs(y) < 700.0)) return exp(y);
+    const double kf = rint(y * 1.4426950408889634074);
+    double r = fma(-kf, 6.93147180369123816490e-01, y);
+    r = fma(-kf, 1.90821492927058770002e-10, r);
+    double p = 1.0 / 39916800.0;
+    p = fma(p, r, 1.0 / 3628800.0); p = fma(p, r, 1.0 / 362880.0); p = fma(p, r, 1.0 / 40320.0);
+    p = fma(p, r, 1.0 / 5040.0);    p = fma(p, r, 1.0 / 720.0);    p = fma(p, r, 1.0 / 120.0);
+    p = fma(p, r, 1.0 / 24.0);      p = fma(p, r, 1.0 / 6.0);      p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);             p = fma(p, r, 1.0);
+    return p * __hiloint2double(((int)kf + 1023) << 20, 0);
+}
+
+// One thread per (entry, parameter, band quad): four table values, one 16-byte store.  The band constants come from a
+// shared-memory copy (indexed by the thread's quad: a constant-bank read would serialise).
+// grid = (ceil(4 * ktot_max / 256), batch), block = 256.
+__global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const int64_t *__restrict__ param_off,
+                                                const int64_t *__restrict__ tab_off, const int32_t *__restrict__ cfg_of,
+                                                const CfgDev *__restrict__ cfgs, float *__restrict__ tab, int32_t batch,
+                                                int32_t *err, const TConst *__restrict__ tcg, const int32_t *__restrict__ skip) {
+    __shared__ TConst tc;
+    for (int i = threadIdx.x; i < (int)(sizeof(TConst) / 8); i += blockDim.x)
+        reinterpret_cast<double *>(&tc)[i] = reinterpret_cast<const double *>(tcg)[i];
+    __syncthreads();
+    const int nfreq = tc.nfreq;
+    for (int e = blockIdx.y; e < batch; e += gridDim.y) {
+        if (skip && skip[e] != 0) continue;
+        const CfgDev *cp = cfgs + cfg_of[e];
+        const int K0 = cp->K[0], K1 = cp->K[1], ktot = cp->ktot;
+        const int id = blockIdx.x * blockDim.x + threadIdx.x;
+        const int j = id >> 2, f0 = (id & 3) * 4;
+        if (j >= ktot) continue;
+        const double x = params[param_off[e] + j];
+        float *row0 = tab + tab_off[e] * NROW;
+        bool bad = !isfinite(x);
+        float v[4];
+        if (j < K0) {
+            // dust power-law factor with the band constant folded in: cd[f] * (nu_f/nu0d)^beta_d
+#pragma unroll
+            for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cd[f0 + i] * exp_pow(x * tc.lnd[f0 + i])) : 0.f;
+            *reinterpret_cast<float4 *>(row0 + (int64_t)j * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+        } else if (j < K0 + K1) {
+            // Planck ratio G = expm1(x0)/expm1(x) and d ln G / dT = (1/T) [ x/(1-e^-x) - x0/(1-e^-x0) ]
+            bad = bad || !(x > 0.0);
+            const int k = j - K0;
+            float dg[4];
+            const double x0 = tc.hk * tc.nu0d / x, e0 = expm1(x0), h0 = x0 / (-expm1(-x0));
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                v[i] = 0.f; dg[i] = 0.f;
+                if (f0 + i < nfreq) {
+                    const double xf = tc.hk * tc.nu[f0 + i] / x;
+                    v[i] = (float)(e0 / expm1(xf));
+                    dg[i] = (float)((xf / (-expm1(-xf)) - h0) / x);
+                }
+            }
+            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + K1 + k) * NROW + f0) = make_float4(dg[0], dg[1], dg[2], dg[3]);
+        } else {
+            const int k = j - K0 - K1;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cs[f0 + i] * exp_pow(x * tc.lns[f0 + i])) : 0.f;
+            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + 2 * K1 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+        }
+        if (bad && f0 == 0) atomicOr(err, ERR_DOMAIN);
+    }
+}
+
+// ----------------------------------------------------------------------------------------------------------
+// a3 second level: grad[e][j] / nll[e][r] = fixed-order (ascending tile) sum over the segments of cluster j / region r,
+// which are contiguous in the partial row.
+// want_grad = 0: only the region outputs.
+// ----------------------------------------------------------------------------------------------------------
+// Cluster outputs (short slot ranges): one thread each, slots added in ascending order.  Region outputs (one slot per
+// tile): one warp each, lane l adds the slots a+l, a+l+32, ... in ascending order and the 32 lane sums are combined by a
+// fixed xor-shuffle tree.  Both orders are fixed, so the result is bitwise reproducible.
+// Virtual thread index v: [0, ktot) clusters, [ktot_pad + 32 r, +32) region r.  grid = (ceil(nvirt_max/256), batch).
+__global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
+                                               const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
+                                               const int64_t *__restrict__ param_off, int32_t nregion, int32_t want_grad,
+                                               double *__restrict__ nll, double *__restrict__ grad, const int32_t *__restrict__ skip) {
+    const int e = blockIdx.y, lane = threadIdx.x & 31;
+    if (skip && skip[e] != 0) return;
+    const CfgDev *c = cfgs + cfg_of[e];
+    const int K0 = c->K[0], K1 = c->K[1], ktot = want_grad ? c->ktot : 0;
+    const int kpad = (ktot + 31) & ~31;
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    const double *erow = partial + (int64_t)e * PS;
+    if (v < ktot) {
+        int t, k;
+        if (v < K0) { t = 0; k = v; }
+        else if (v < K0 + K1) { t = 1; k = v - K0; }
+        else { t = 2; k = v - K0 - K1; }
+        const int32_t *ksegptr = maps[c->map[t]].ksegptr;
+        const double *row = erow + c->segbase[t];
+        const int a = ksegptr[k], b = ksegptr[k + 1];
+        double acc = 0.0;
+#pragma unroll 4
+        for (int q = a; q < b; ++q) acc += row[q];
+        grad[param_off[e] + v] = acc;
+    } else if (v >= kpad && (v - kpad) >> 5 < nregion) {
+        const int r = (v - kpad) >> 5;
+        const int32_t *ksegptr = maps[c->map[3]].ksegptr;
+        const double *row = erow + c->segbase[3];
+        const int a = ksegptr[r], b = ksegptr[r + 1];
+        double acc = 0.0;
+#pragma unroll 4
+        for (int q = a + lane; q < b; q += 32) acc += row[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) nll[(int64_t)e * nregion + r] = acc;
+    }
+}
+
+// f1 (Eq. 10): variance of the CMB map per entry and region from the four region-reduced sums.
+__global__ void __launch_bounds__(128) k_cmbvar(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
+                                                const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
+                                                const int32_t *__restrict__ npix_live, int32_t nregion, int32_t batch,
+                                                double *__restrict__ var) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= batch * nregion) return;
+    const int e = i / nregion, r = i - e * nregion;
+    const MapDev *m = maps + cfgs[cfg_of[e]].map[3];
+    const int32_t *ksegptr = m->ksegptr;
+    const int32_t nseg = m->nseg;
+    double s[4];
+    for (int t = 0; t < 4; ++t) {
+        const double *row = partial + (int64_t)e * PS + (int64_t)t * nseg;
+        double acc = 0.0;
+        for (int q = ksegptr[r]; q < ksegptr[r + 1]; ++q) acc += row[q];
+        s[t] = acc;
+    }
+    const double n = (double)npix_live[cfg_of[e] * nregion + r];
+    var[i] = n > 0 ? (s[2] / n - (s[0] / n) * (s[0] / n)) + (s[3] / n - (s[1] / n) * (s[1] / n)) : 0.0;
+}
+
+// Private copy of one data set in the sorted layout of one configuration: copy[tile][half][row][x] =
+// d[data][row][pospix[tile*TPX + half*256 + x]], zero at pad positions.  grid = (ntile, pairs), block = TPX.
+struct CopyJob {
+    int32_t cfg, data;
+    int64_t off;   // float offset of the copy inside dcopy
+};
+__global__ void __launch_bounds__(TPX) k_relayout(const float *__restrict__ d, int64_t npix, int32_t nrows, const CfgDev *__restrict__ cfgs,
+                                                  const CopyJob *__restrict__ jobs, float *__restrict__ dcopy) {
+    const CopyJob job = jobs[blockIdx.y];
+    const CfgDev *cf = cfgs + job.cfg;
+    const int tile = blockIdx.x;
+    if (tile >= cf->ntile) return;
+    const int x = threadIdx.x;
+    const int32_t pix = cf->pospix[(int64_t)tile * TPX + x];
+    const float *src = d + (int64_t)job.data * nrows * npix + (pix >= 0 ? pix : 0);
+    float *dst = dcopy + job.off + (int64_t)tile * nrows * TPX + (x >> 8) * nrows * HALF + (x & (HALF - 1));
+    for (int r = 0; r < nrows; ++r) dst[r * HALF] = (pix >= 0) ? __ldg(src + (int64_t)r * npix) : 0.f;
+}
+
+}  // namespace cs

@@ -7,11 +7,20 @@ import gen
 import oracle
 
 
-def make_ctx(w, d_dev=None, device="cuda:0", units=0):
+# Context options applied by new_ctx / make_ctx; the `path` fixture of the GPU tests switches them so that every parity
+# case runs on the sorted layout (sorted-cell kernel) and in place (direct kernel).
+CTX_OPTIONS = {}
+
+
+def new_ctx(freqs, npix, units=0, options=None):
+    import paper_2604_08463_b200 as cs
+    return cs.Context(freqs, npix, units=units, options=CTX_OPTIONS if options is None else options)
+
+
+def make_ctx(w, d_dev=None, device="cuda:0", units=0, options=None):
     """Context with the workload's clusters, data and batch set.  Returns (ctx, d_dev)."""
     import torch
-    import paper_2604_08463_b200 as cs
-    ctx = cs.Context(w.freqs, w.npix, units=units)
+    ctx = new_ctx(w.freqs, w.npix, units=units, options=options)
     ctx.set_clusters(w.maps, w.Kmap, w.cfg_maps, w.region_idx, w.nregion)
     if d_dev is None:
         d_dev = torch.from_numpy(w.data()).to(device)

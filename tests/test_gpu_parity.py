@@ -9,7 +9,8 @@ import pytest
 
 import gen
 import oracle
-from helpers import make_ctx, gpu_eval, gpu_maps, oracle_entry, check_T1, check_T2, check_T3
+import helpers
+from helpers import make_ctx, new_ctx, gpu_eval, gpu_maps, oracle_entry, check_T1, check_T2, check_T3
 
 pytestmark = pytest.mark.gpu
 
@@ -21,11 +22,12 @@ def torch_cuda():
     return torch
 
 
-@pytest.fixture(params=["cell", "direct"])
+@pytest.fixture(params=["sorted", "inplace"])
 def path(request, monkeypatch):
-    """Both forms of the fused kernel: 'cell' (k_like_cell where the plan allows it) and 'direct' (k_like forced)."""
-    monkeypatch.setenv("CS_FORCE_DIRECT", "1" if request.param == "direct" else "0")
-    monkeypatch.setenv("CS_CELL_MIN_GROUP", "1")     # the library's default sends groups of < 12 entries to the direct kernel
+    """Both layouts and kernels: 'sorted' (private cell-sorted copies, k_like_sc, forced for every configuration) and
+    'inplace' (the caller's pixel order, k_like_direct)."""
+    import paper_2604_08463_b200 as cs
+    monkeypatch.setattr(helpers, "CTX_OPTIONS", {"layout": cs.LAYOUT_SORTED if request.param == "sorted" else cs.LAYOUT_INPLACE})
     return request.param
 
 
@@ -138,7 +140,7 @@ def test_generic_band_count_and_literal_units(torch_cuda, path):
     ninv = np.ascontiguousarray(w.ninv[sel])
     params = w.params_jittered(seed=8)
     for units in (cs.UNITS_KCMB, cs.UNITS_LITERAL):
-        ctx = cs.Context(freqs, w.npix, units=units)
+        ctx = new_ctx(freqs, w.npix, units=units)
         ctx.set_clusters(w.maps, w.Kmap, w.cfg_maps)
         dd = torch.from_numpy(d).cuda()
         ctx.set_data(dd, ninv)
@@ -279,7 +281,7 @@ def test_singular_system_is_flagged(torch_cuda, path):
     freqs = np.array([100.0, 100.0, 100.0])
     d = np.ascontiguousarray(w.data()[:, [6, 6, 6]])
     ninv = np.ascontiguousarray(w.ninv[[6, 6, 6]])
-    ctx = cs.Context(freqs, w.npix)
+    ctx = new_ctx(freqs, w.npix)
     ctx.set_clusters(w.maps, w.Kmap, w.cfg_maps)
     ctx.set_data(torch.from_numpy(d).cuda(), ninv)
     ctx.set_batch(w.cfg_of, w.data_of)
@@ -519,36 +521,44 @@ def test_full_size_c5_nside128_sampled(torch_cuda):
     _sampled_full_size(w, w.params_jittered(seed=18), 6, 24)
 
 
-def test_kernel_forms_agree_bit_for_bit(torch_cuda, monkeypatch):
-    """The cell form and the direct form run the same arithmetic in the same order (csrc/cs_math.cuh): nll, gradient,
-    maps and the CMB variance are bitwise equal, which is what lets the library pick the form per group without
-    giving up batch invariance."""
+def test_kernel_forms_agree_bit_for_bit(torch_cuda):
+    """The sorted-cell kernel and the direct kernel run the same arithmetic in the same order on the same layout
+    (csrc/cs_math.cuh): nll, gradient, the value-only nll, chi^2 and the CMB variance are bitwise equal.  (Which kernel
+    runs is a property of the configuration, so batch invariance never depended on this; the equality is a check of
+    the warp-specialised kernel's hand-overs against the plain one.)"""
     import torch
+    import paper_2604_08463_b200 as cs
     w = _masked(gen.make_config(3, nside=32, batch=9, ndata=3))
     params = w.params_jittered(seed=27)
     out = {}
-    for form, env in (("cell", {"CS_FORCE_DIRECT": "0", "CS_CELL_MIN_GROUP": "1"}), ("direct", {"CS_FORCE_DIRECT": "1"})):
-        for k, v in env.items():
-            monkeypatch.setenv(k, v)
-        ctx, _ = make_ctx(w)
+    for form in (cs.FORM_AUTO, cs.FORM_DIRECT):
+        ctx, _ = make_ctx(w, options={"layout": cs.LAYOUT_SORTED, "form": form})
+        assert all(ctx.layout_info(c)[0] for c in range(w.cfg_maps.shape[0]))
         nll, grad = gpu_eval(ctx, params)
         nll_v, _ = gpu_eval(ctx, params, want_grad=False)
-        smaps = gpu_maps(ctx, params)
         var = torch.zeros(w.batch * w.nregion, dtype=torch.float64, device="cuda")
+        chi2 = torch.zeros(w.batch * w.nregion, dtype=torch.float64, device="cuda")
         ctx.cmb_variance(var)
+        ctx.spectral_misfit(chi2)
         torch.cuda.synchronize()
-        out[form] = (nll, grad, nll_v, smaps, var.cpu().numpy())
+        out[form] = (nll, grad, nll_v, var.cpu().numpy(), chi2.cpu().numpy())
         ctx.close()
-    for a, b in zip(out["cell"], out["direct"]):
+    for a, b in zip(out[cs.FORM_AUTO], out[cs.FORM_DIRECT]):
         assert np.array_equal(a, b)
 
 
-def test_default_kernel_choice_mixes_both_forms(torch_cuda):
-    """Library defaults (no overrides): long groups on the cell kernel, short ones on the direct kernel, in one batch."""
-    w = gen.make_config(3, nside=32, batch=40, ndata=30)     # configuration 0: 30 entries, configuration 1: 10 entries
-    assert sorted(np.bincount(w.cfg_of).tolist()) == [10, 30]
+def test_default_layout_choice_mixes_both_kernels(torch_cuda):
+    """Library defaults (CS_LAYOUT_AUTO): configurations whose sorted tiles fill well stream private sorted copies
+    through the sorted-cell kernel, the others stay in place on the direct kernel -- both in one batch."""
+    w = gen.make_config(2, batch=24)     # K from (10,1,1) to (1000,500,500) on one shared data set
+    ctx, _ = make_ctx(w, options={})
+    kinds = {ctx.layout_info(c)[0] for c in range(w.cfg_maps.shape[0])}
+    ctx.close()
+    assert kinds == {True, False}
+    helpers_opts = helpers.CTX_OPTIONS
+    assert helpers_opts == {}
     _parity(w, w.params_jittered(seed=26), maps=False)
-    _parity(w, w.params_jittered(seed=26), entries=[0, 29, 30, 39])
+    _parity(w, w.params_jittered(seed=26), entries=[0, 11, 23])
 
 
 def test_full_size_c3_scan_sampled(torch_cuda):
