@@ -33,8 +33,9 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
-    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
-    cmd = [_nvcc()] + flags + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"] + os.environ.get("CS_NVCC_EXTRA", "").split()
+    out = os.environ.get("CS_LIB_OUT", LIB)
+    cmd = [_nvcc()] + flags + ["-o", out] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     log = res.stdout + res.stderr
     with open(os.path.join(_HERE, "build.log"), "w") as fh:

@@ -84,6 +84,14 @@ struct Run {
     int64_t ustart;
 };
 
+// What the roles of a fused kernel need to know about the entry at position i of the launch's entry list, in one
+// 16-byte load whose address does not depend on another load (a dependent global load costs a microsecond under a
+// saturated HBM stream).
+struct PosInfo {
+    int64_t tab_row;   // first table row of the entry
+    int64_t src;       // sorted configuration: float offset of the entry's private copy inside dcopy; else its data set
+};
+
 // Constants of the fused kernels, passed by value (constant bank).
 struct KConst {
     float w[NROW];     // Ninv per band, 0 beyond nfreq

@@ -103,11 +103,13 @@ struct cs_ctx {
     int64_t W_sc = 0, W_dir = 0;
     int64_t nparam = 0, nrows = 0, PS = 0;
     std::vector<int32_t> cfg_of, data_of, elist;
-    std::vector<int64_t> param_off, copy_off;
+    std::vector<int64_t> param_off, copy_off, tab_off;
+    std::vector<PosInfo> pinfo;         // per position of elist
     std::vector<Run> runs;
     std::vector<CopyJob> jobs;          // private copies of the sorted layout, ordered by data set
     int32_t *d_cfg_of = nullptr, *d_data_of = nullptr, *d_elist = nullptr;
-    int64_t *d_param_off = nullptr, *d_tab_off = nullptr, *d_copy_off = nullptr;
+    int64_t *d_param_off = nullptr, *d_tab_off = nullptr;
+    PosInfo *d_pinfo = nullptr;
     Run *d_runs = nullptr;
     CopyJob *d_jobs = nullptr;
     float *d_tab = nullptr, *d_copy = nullptr;
@@ -169,10 +171,10 @@ void free_opt(cs_ctx *c) {
 
 void free_batch(cs_ctx *c) {
     cudaFree(c->d_cfg_of); cudaFree(c->d_data_of); cudaFree(c->d_elist);
-    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_copy_off); cudaFree(c->d_runs); cudaFree(c->d_jobs);
+    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
     cudaFree(c->d_tab); cudaFree(c->d_partial); cudaFree(c->d_copy);
     c->d_cfg_of = c->d_data_of = c->d_elist = nullptr;
-    c->d_param_off = c->d_tab_off = c->d_copy_off = nullptr;
+    c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr;
     c->d_runs = nullptr; c->d_jobs = nullptr;
     c->d_tab = nullptr; c->d_partial = nullptr; c->d_copy = nullptr;
     c->batch = 0; c->nrun_sc = c->nrun_dir = 0; c->batch_bytes = 0; c->copy_bytes = 0;
@@ -442,13 +444,11 @@ LikeParams base_params(cs_ctx *c) {
     P.evict_first = (stream_bytes > (int64_t)96 << 20) ? 1 : 0;
     P.ring_maps = 0;
     P.dcopy = c->d_copy;
-    P.copy_off = c->d_copy_off;
+    P.pinfo = c->d_pinfo;
     P.maps = c->d_maps;
     P.cfgs = c->d_cfgs;
     P.elist = c->d_elist;
-    P.data_of = c->d_data_of;
     P.skip = c->skip;
-    P.tab_off = c->d_tab_off;
     P.tab = c->d_tab;
     P.partial = c->d_partial;
     P.PS = c->PS;
@@ -752,7 +752,8 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     c->cfg_of.assign(cfg_of, cfg_of + batch);
     c->data_of.assign(data_of, data_of + batch);
     c->param_off.assign(batch + 1, 0);
-    std::vector<int64_t> tab_off(batch);
+    std::vector<int64_t> &tab_off = c->tab_off;
+    tab_off.assign(batch, 0);
     const int32_t nseg_reg = c->maps[c->nmap].nseg;
     int64_t rows = 0, PS = 4 * (int64_t)nseg_reg;
     int32_t kmax = 0;
@@ -812,6 +813,11 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         for (int32_t e = 0; e < batch; ++e)
             if (c->cfgs[cfg_of[e]].sorted) c->copy_off[e] = seen[std::make_pair(data_of[e], cfg_of[e])];
     }
+    c->pinfo.resize(batch);
+    for (int32_t i = 0; i < batch; ++i) {
+        const int32_t e = c->elist[i];
+        c->pinfo[i] = PosInfo{tab_off[e], c->cfgs[cfg_of[e]].sorted ? c->copy_off[e] : (int64_t)data_of[e]};
+    }
     const int64_t copy_bytes = copy_floats * 4;
     if (copy_bytes > 0) {
         int64_t limit = c->opt_copy_limit;
@@ -826,13 +832,13 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     if ((rc = dev_upload(&c->d_cfg_of, c->cfg_of, &c->batch_bytes)) || (rc = dev_upload(&c->d_data_of, c->data_of, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_elist, c->elist, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_param_off, c->param_off, &c->batch_bytes)) || (rc = dev_upload(&c->d_tab_off, tab_off, &c->batch_bytes)) ||
-        (rc = dev_upload(&c->d_copy_off, c->copy_off, &c->batch_bytes)) || (rc = dev_upload(&c->d_runs, c->runs, &c->batch_bytes)) ||
+        (rc = dev_upload(&c->d_pinfo, c->pinfo, &c->batch_bytes)) || (rc = dev_upload(&c->d_runs, c->runs, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_jobs, c->jobs, &c->batch_bytes))) {
         free_batch(c);
         return rc;
     }
     const size_t tab_bytes = (size_t)rows * NROW * sizeof(float), part_bytes = (size_t)batch * PS * sizeof(double);
-    c->sel_cap = (((int64_t)batch * (1 + (int64_t)(sizeof(Run) / 4)) + 8) + 3) & ~(int64_t)3;   // slots stay 16-byte aligned
+    c->sel_cap = (((int64_t)batch * (1 + (int64_t)((sizeof(Run) + sizeof(PosInfo)) / 4)) + 16) + 3) & ~(int64_t)3;   // slots stay 16-byte aligned
     if (cudaMalloc((void **)&c->d_tab, tab_bytes) != cudaSuccess || cudaMalloc((void **)&c->d_partial, part_bytes) != cudaSuccess ||
         (copy_bytes > 0 && cudaMalloc((void **)&c->d_copy, (size_t)copy_bytes) != cudaSuccess) ||
         cudaMalloc((void **)&c->d_sel, (size_t)(cs_ctx::SEL_RING * c->sel_cap * 4)) != cudaSuccess ||
@@ -923,7 +929,10 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
         if (e < 0 || e >= c->batch) return CS_EINVAL;
         hs[i] = e;
     }
-    const int64_t roff = ((int64_t)nsel + 1) & ~(int64_t)1;   // runs start 8-byte aligned
+    const int64_t poff = ((int64_t)nsel + 3) & ~(int64_t)3;   // position info starts 16-byte aligned, the runs follow it
+    PosInfo *hp = reinterpret_cast<PosInfo *>(hs + poff);
+    for (int32_t i = 0; i < nsel; ++i) hp[i] = PosInfo{c->tab_off[hs[i]], (int64_t)c->data_of[hs[i]]};
+    const int64_t roff = poff + (int64_t)nsel * (int64_t)(sizeof(PosInfo) / 4);
     Run *hr = reinterpret_cast<Run *>(hs + roff);
     int32_t nrun = 0;
     int64_t W = 0;
@@ -941,6 +950,7 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
     c->sel_n++;
     LikeParams P = base_params(c);
     P.elist = ds;
+    P.pinfo = reinterpret_cast<const PosInfo *>(ds + poff);
     P.maps_out = s;
     P.ring_maps = 1;
     P.evict_first = ((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4 > (int64_t)96 << 20) ? 1 : 0;

@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(DR_THREADS, 1) k_like_direct(const __grid_cons
             const int e = __ldg(P.elist + w.run.estart + k);
             if (P.skip && __ldg(P.skip + e) != 0) continue;
             const int sd = n % ND;
-            const float *tb = P.tab + __ldg(P.tab_off + e) * NROW;
+            const float *tb = P.tab + __ldg(&P.pinfo[w.run.estart + k].tab_row) * NROW;
             const float *st = st0 + sd * STAGE;
             mbar_wait(&full_d[sd], (uint32_t)((n / ND) & 1));
             const float4 *aFd = reinterpret_cast<const float4 *>(tb + rA_fd), *aG = reinterpret_cast<const float4 *>(tb + rA_g);

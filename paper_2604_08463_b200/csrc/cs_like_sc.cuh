@@ -16,13 +16,16 @@
 // scalar (broadcast operand form), data read as one LDS.64 per band and Stokes parameter.
 //
 // Persistent grid: one CTA per SM, each walking a contiguous, equal share of all (tile, entry) units (cs_pipe.cuh).
-// CTA = 12 warps (so that a thread may hold up to 168 registers), warp-specialised; every hand-over is an mbarrier full/empty pair or a hardware named barrier, no
+// CTA = 13 warps (128 registers per thread), warp-specialised; every hand-over is an mbarrier full/empty pair or a hardware named barrier, no
 // CTA-wide barrier after the prologue:
 //   warps 0-7    consumers: positions (2t, 2t+1) of the 512-position tile per thread, one entry after the other
 //   warps 8-9    reducers : first level of the ordered fp64 reduction (a3) of the pair sums the consumers leave behind;
 //                           warp r owns term-ring slot r and the entries n = r (mod 2)
-//   warp  10     builder  : lane c builds cell c of the tile for the next entry (five weighted columns, LDL^T, P)
-//   warp  11     loader   : one 60-KB bulk copy per entry into the data ring
+//   warps 10-11  builders : lane c builds cell c of the tile (five weighted columns, LDL^T, P); warp b owns cell-table
+//                           slot b and the entries n = b (mod 2).  Two of them, because under a saturated HBM stream the
+//                           L2 round trip of a cell's four table rows takes about as long as a whole entry
+//   warp  12     loader   : one 60-KB bulk copy per entry into the data ring (two stages: measured, a deeper ring
+//                           adds nothing once the consumers release a stage as soon as it is read)
 // shared memory: data ring [ND][2 halves][2*NF][256] | cell tables [NC][CELL_CAP][CROW] | term ring [NT][4][256] fp64 |
 //                reducer plans | barriers
 #pragma once
@@ -31,13 +34,19 @@
 
 namespace cs {
 
-constexpr int SC_ND = 3;        // data ring depth (2 for the generic band count, whose stages are 16 bands tall)
+#ifndef CS_SC_ND
+#define CS_SC_ND 2
+#endif
+#ifndef CS_SC_NBW
+#define CS_SC_NBW 2
+#endif
+constexpr int SC_ND = CS_SC_ND; // data ring depth 
 template <int NF>
-struct ScDepth { static constexpr int value = (NF == 15) ? SC_ND : 2; };
+struct ScDepth { static constexpr int value = SC_ND; };
 constexpr int SC_NC = 2;        // cell-table ring depth
-constexpr int SC_NBW = 1;       // builder warps (warp b takes the entries n = b mod SC_NBW; SC_NC is a multiple of it)
+constexpr int SC_NBW = CS_SC_NBW; // builder warps (warp b takes the entries n = b mod SC_NBW; SC_NC is a multiple of it)
 constexpr int SC_NT = 2;        // term ring depth = reducer warps
-constexpr int SC_THREADS = NCONS + (SC_NT + SC_NBW + 1) * 32;   // 384
+constexpr int SC_THREADS = NCONS + (SC_NT + SC_NBW + 1) * 32;   // 416
 constexpr int SC_WARP_RED = NCONS / 32, SC_WARP_BUILD = SC_WARP_RED + SC_NT, SC_WARP_LOAD = SC_WARP_BUILD + SC_NBW;
 constexpr int SC_PLAN_BYTES = SC_CHUNK_CAP * 2 + SC_SEG_CAP * 2 + SC_SEG_CAP * 4 + 16;   // one reducer warp's plan
 
@@ -215,13 +224,13 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
             int4 rows = make_int4(0, 0, 0, 0);
             if (lane < ncell) rows = __ldg(reinterpret_cast<const int4 *>(cf->cellrows) + c0 + lane);
             for (int k = w.k; k < w.kend; ++k) {
-                const int e = __ldg(P.elist + w.run.estart + k);
-                if (P.skip && __ldg(P.skip + e) != 0) continue;
+                const int64_t tab_row = __ldg(&P.pinfo[w.run.estart + k].tab_row);
+                if (P.skip && __ldg(P.skip + __ldg(P.elist + w.run.estart + k)) != 0) continue;
                 const int s = n % NC;
                 if (SC_NBW > 1 && n % SC_NBW != mine) { ++n; continue; }
                 float4 Fd[4], G[4], dG[4], Fs[4];
                 if (lane < ncell) {
-                    const float *tb = P.tab + __ldg(P.tab_off + e) * NROW;
+                    const float *tb = P.tab + tab_row * NROW;
                     const float4 *rFd = reinterpret_cast<const float4 *>(tb + (int64_t)rows.x * NROW);
                     const float4 *rG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.y * NROW);
                     const float4 *rdG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.z * NROW);
@@ -232,7 +241,7 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
                         dG[q] = kGrad ? __ldg(rdG + q) : make_float4(0.f, 0.f, 0.f, 0.f);
                     }
                 }
-                mbar_wait_relaxed(&empty_c[s], (uint32_t)(((n / NC) & 1) ^ 1));
+                mbar_wait(&empty_c[s], (uint32_t)(((n / NC) & 1) ^ 1));
                 if (lane < ncell) sc_build_cell<NF, kGrad>(Fd, G, dG, Fs, P.kc, cells + (s * CELL_CAP + lane) * CROW, P.err);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&full_c[s]);

@@ -29,18 +29,16 @@ struct LikeParams {
     int32_t evict_first;       // 1: the stream is much larger than L2 and read once -> L2 evict-first policy
     int32_t ring_maps;         // 1: use the pixel-space maps (rmap) and the caller's d whatever the layout (MODE_MAPS)
     const float *dcopy;        // private sorted copies
-    const int64_t *copy_off;   // [batch] float offset of the entry's copy inside dcopy (sorted configurations)
+    const PosInfo *pinfo;      // [entries of the launch's list] table block and data source of the entry at each position
     const MapDev *maps;
     const CfgDev *cfgs;
     const Run *runs;
     int32_t nrun;
-    int32_t out_base;          // MODE_MAPS: runs[r].estart - out_base + k = output slot
+    int32_t pad0;
     int64_t W;                 // total units of the launch
     const int32_t *elist;
-    const int32_t *data_of;
     const int32_t *skip;       // [batch] or null: entries with a non-zero flag are left out (line-search trials of
                                // entries that already accepted a step); their outputs keep their previous values
-    const int64_t *tab_off;    // [batch] first table row of entry
     const float *tab;
     double *partial;
     int64_t PS;                // doubles per partial row
@@ -164,6 +162,35 @@ __device__ __forceinline__ bool walk_next(Walk &w, const LikeParams &P) {
     return true;
 }
 
+// The same walk entry by entry, with the skipped entries left out: e = next live entry, newpiece = it starts a new
+// (run, tile) piece.  Lets a role look one entry ahead (the builder loads the next entry's table rows early).
+struct EntryWalk {
+    Walk w;
+    int k;
+    bool open;
+};
+__device__ __forceinline__ void entry_init(EntryWalk &it, const LikeParams &P) {
+    walk_init(it.w, P);
+    it.k = 0;
+    it.open = false;
+}
+__device__ __forceinline__ bool entry_next(EntryWalk &it, const LikeParams &P, int &e, int &pos, bool &newpiece) {
+    newpiece = false;
+    while (true) {
+        if (!it.open || it.k >= it.w.kend) {
+            if (!walk_next(it.w, P)) return false;
+            it.k = it.w.k;
+            it.open = true;
+            newpiece = true;
+        }
+        while (it.k < it.w.kend) {
+            pos = it.w.run.estart + it.k++;
+            e = __ldg(P.elist + pos);
+            if (!(P.skip && __ldg(P.skip + e) != 0)) return true;
+        }
+    }
+}
+
 // ----------------------------------------------------------------------------------------------------------
 // Loader warp: streams one stage per live entry into the data ring.  A stage holds the tile as two halves of
 // [2*nfreq rows][256 positions] fp32.  Sorted layout: one contiguous bulk copy from the entry's private copy.
@@ -183,34 +210,34 @@ __device__ __forceinline__ void loader_loop(const CUtensorMap *tmap, const LikeP
         const CfgDev *cf = P.cfgs + w.run.cfg;
         const bool sorted = cf->sorted && !P.ring_maps;
         for (int k = w.k; k < w.kend; ++k) {
-            const int e = __ldg(P.elist + w.run.estart + k);
-            if (P.skip && __ldg(P.skip + e) != 0) continue;
+            const int64_t srcinfo = __ldg(&P.pinfo[w.run.estart + k].src);
+            if (P.skip && __ldg(P.skip + __ldg(P.elist + w.run.estart + k)) != 0) continue;
             const int s = n % ND;
             float *dst = ring + s * STAGE;
             if (sorted) {
                 if (lane == 0) {
-                    mbar_wait_relaxed(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1), 200);
+                    mbar_wait(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1));
                     const uint32_t bytes = (uint32_t)nrows * TPX * 4u;
                     mbar_expect_tx(&full_d[s], bytes);
                     if (NF * 2 == nrows) {
-                        bulk_g2s(dst, P.dcopy + __ldg(P.copy_off + e) + (int64_t)w.tile * nrows * TPX, bytes, &full_d[s], policy);
+                        bulk_g2s(dst, P.dcopy + srcinfo + (int64_t)w.tile * nrows * TPX, bytes, &full_d[s], policy);
                     } else {   // generic band count: the stage keeps 2*NF rows per half, the copy only 2*nfreq
-                        const float *src = P.dcopy + __ldg(P.copy_off + e) + (int64_t)w.tile * nrows * TPX;
+                        const float *src = P.dcopy + srcinfo + (int64_t)w.tile * nrows * TPX;
                         bulk_g2s(dst, src, bytes / 2, &full_d[s], policy);
                         bulk_g2s(dst + NF * 2 * HALF, src + nrows * HALF, bytes / 2, &full_d[s], policy);
                     }
                 }
             } else if (P.use_tma) {
                 if (lane == 0) {
-                    mbar_wait_relaxed(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1), 200);
+                    mbar_wait(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1));
                     mbar_expect_tx(&full_d[s], (uint32_t)nrows * TPX * 4u);
-                    const int y = __ldg(P.data_of + e) * nrows;
+                    const int y = (int)srcinfo * nrows;
                     tma_box_g2s(dst, tmap, w.tile * TPX, y, &full_d[s], policy);
                     tma_box_g2s(dst + NF * 2 * HALF, tmap, w.tile * TPX + HALF, y, &full_d[s], policy);
                 }
             } else {   // rows of d not 16-byte aligned: plain loads by the whole warp
-                mbar_wait_relaxed(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1), 200);
-                const int64_t row0 = (int64_t)__ldg(P.data_of + e) * nrows;
+                mbar_wait(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1));
+                const int64_t row0 = srcinfo * nrows;
                 for (int h = 0; h < 2; ++h)
                     for (int r = 0; r < nrows; ++r)
                         for (int x = lane; x < HALF; x += 32) {
