@@ -21,7 +21,10 @@
  * elimination with partial pivoting, sums over pixels are accumulated in long double in pixel order.
  * Parity pins (tests/test_oracle_pins.py): a(nu0)=1, RJ limit, W A = I (Eq. 11), normal equations,
  * noiseless recovery, nfreq = ncomp reduction, central finite differences, chi^2 statistics, brute-force
- * grid argmin, Ninv scaling, K=(1,1,1) vs per-pixel gradients.
+ * grid argmin, Ninv scaling, K=(1,1,1) vs per-pixel gradients.  The tolerance scales absg / gscale (every T2
+ * bound of the GPU tests is built from them) are pinned too: one pixel's gs against a numpy restatement of its
+ * definition, absg == |grad| when every pixel is its own cluster, both as sums of the per-pixel terms over a
+ * cluster's pixels, the closed form of gscale on noiseless data at the truth, and their scalings.
  */
 #include <math.h>
 #include <stdint.h>

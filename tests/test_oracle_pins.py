@@ -320,3 +320,125 @@ def test_brute_force_grid_recovers_truth():
     dNd = np.sum(ninv.astype(np.float64)[:, None, None] * d.astype(np.float64) ** 2)
     assert abs(vals[5, 5, 5] + 0.5 * dNd) < 1e-3                    # chi^2 ~ 0 (fp32 rounding of d only)
     assert np.sort(vals.ravel())[1] - vals[5, 5, 5] > 1.0           # unique, well separated minimum
+
+
+# ----------------------------------------------------------------------------- tolerance scales absg / gscale (T2)
+# Every gradient bound of the GPU parity tests is built from these two oracle outputs (tests/helpers.py check_T2), so
+# a mistake in them would silently loosen every gradient check.  They are pinned to things other than themselves.
+
+def _dA_numpy(freqs, bd, Td, bs, h=1e-6):
+    """d a_d/d beta_d, d a_d/d T_d, d a_s/d beta_s [F] by central differences of gen's independent forward model."""
+    ad_p, _ = gen.mixing_columns(freqs, bd + h, Td, bs)
+    ad_m, _ = gen.mixing_columns(freqs, bd - h, Td, bs)
+    at_p, _ = gen.mixing_columns(freqs, bd, Td + h, bs)
+    at_m, _ = gen.mixing_columns(freqs, bd, Td - h, bs)
+    _, as_p = gen.mixing_columns(freqs, bd, Td, bs + h)
+    _, as_m = gen.mixing_columns(freqs, bd, Td, bs - h)
+    return np.stack([(ad_p - ad_m) / (2 * h), (at_p - at_m) / (2 * h), (as_p - as_m) / (2 * h)])
+
+
+def test_gscale_of_one_pixel_against_a_numpy_restatement(model, c1):
+    """gs_theta = sum_S |s_{S,c(theta)}| sum_f w_f |d_{S,f}| |da_f/dtheta|, restated with numpy
+    from the definition: GLS solution by lstsq on gen's forward model, derivatives by central differences."""
+    d, idx, K = _entry(c1)
+    w = c1.ninv.astype(np.float64)
+    comp_of = (1, 1, 2)
+    for p, (bd, Td, bs) in ((3, (1.54, 20.0, -3.0)), (200, (1.7, 17.5, -2.8)), (767, (1.2, 31.0, -3.4))):
+        dq, du = d[:, 0, p].astype(np.float64), d[:, 1, p].astype(np.float64)
+        r = oracle.pixel(model, w, dq, du, bd, Td, bs)
+        a_d, a_s = gen.mixing_columns(c1.freqs, bd, Td, bs)
+        A = np.stack([np.ones_like(a_d), a_d, a_s], axis=1)
+        sw = np.sqrt(w)
+        s = np.stack([np.linalg.lstsq(A * sw[:, None], x * sw, rcond=None)[0] for x in (dq, du)], axis=1)   # [3, 2]
+        dA = _dA_numpy(c1.freqs, bd, Td, bs)
+        for t in range(3):
+            want = sum(abs(s[comp_of[t], S]) * np.sum(w * np.abs(x) * np.abs(dA[t])) for S, x in enumerate((dq, du)))
+            assert abs(r["gs"][t] - want) <= 2e-7 * want, (p, t, r["gs"][t], want)
+            # and the gradient term itself, from the same restatement (Eq. 17, factor 1)
+            g = -sum(s[comp_of[t], S] * np.sum(w * (x - A @ s[:, S]) * dA[t]) for S, x in enumerate((dq, du)))
+            assert abs(r["g"][t] - g) <= 2e-6 * want
+
+
+def test_absg_equals_abs_grad_when_every_pixel_is_its_own_cluster(model, c1):
+    d, _, _ = _entry(c1)
+    npix = c1.npix
+    idx = np.tile(np.arange(npix, dtype=np.int32), (3, 1))
+    params = np.concatenate([1.54 + 0.05 * np.sin(np.arange(npix)), 20.0 + np.cos(np.arange(npix)),
+                             -3.0 + 0.05 * np.sin(0.3 * np.arange(npix))])
+    r = oracle.nll_grad(model, d, c1.ninv, idx, [npix] * 3, params, want_tol=True)
+    assert r["rc"] == 0
+    assert np.array_equal(r["absg"], np.abs(r["grad"]))
+    # per cluster = per pixel here: gscale is the one-pixel quantity pinned above
+    w = c1.ninv.astype(np.float64)
+    for p in (0, 411):
+        one = oracle.pixel(model, w, d[:, 0, p].astype(np.float64), d[:, 1, p].astype(np.float64),
+                           params[p], params[npix + p], params[2 * npix + p])
+        assert np.allclose([r["gscale"][p], r["gscale"][npix + p], r["gscale"][2 * npix + p]], one["gs"], rtol=1e-14)
+
+
+def test_absg_and_gscale_are_sums_over_the_clusters_pixels(model, c1):
+    """absg_k = sum_{p in k} |g_p| and gscale_k = sum_{p in k} gs_p with the per-pixel terms of the K = npix run;
+    hence absg >= |grad| (triangle inequality), with equality only without cancellation."""
+    d, idx, K = _entry(c1)
+    params = c1.params_jittered(seed=4)
+    r = oracle.nll_grad(model, d, c1.ninv, idx, K, params, want_tol=True)
+    npix = c1.npix
+    own = np.tile(np.arange(npix, dtype=np.int32), (3, 1))
+    pp = np.concatenate([params[:K[0]][idx[0]], params[K[0]:K[0] + K[1]][idx[1]], params[K[0] + K[1]:][idx[2]]])
+    rp = oracle.nll_grad(model, d, c1.ninv, own, [npix] * 3, pp, want_tol=True)
+    o = 0
+    for t in range(3):
+        gp, sp = rp["grad"][t * npix:(t + 1) * npix], rp["gscale"][t * npix:(t + 1) * npix]
+        want_a = np.bincount(idx[t], weights=np.abs(gp), minlength=K[t])
+        want_s = np.bincount(idx[t], weights=sp, minlength=K[t])
+        assert np.allclose(r["absg"][o:o + K[t]], want_a, rtol=1e-12)
+        assert np.allclose(r["gscale"][o:o + K[t]], want_s, rtol=1e-12)
+        o += K[t]
+    assert np.all(r["absg"] >= np.abs(r["grad"]) * (1 - 1e-12))
+    assert np.all(r["gscale"] > 0)
+
+
+def test_gscale_closed_form_on_noiseless_data_at_the_truth():
+    """Noiseless cluster-constant sky at its true parameters: s = s*, d = A s*, the gradient vanishes but
+    gscale_k = sum_{p in k} sum_S |s*_c| sum_f w_f |(A s*)_f| |da_f/dtheta| is a closed form of the inputs."""
+    w = gen.make_config(0, noiseless=True, cluster_truth=True)
+    model = oracle.Model(w.freqs)
+    d, idx, K = _entry(w)
+    truth = np.concatenate(w.truth["per_cluster"])
+    r = oracle.nll_grad(model, d, w.ninv, idx, K, truth, want_tol=True)
+    assert r["rc"] == 0
+    wf = w.ninv.astype(np.float64)
+    comp_of = (1, 1, 2)
+    s = w.truth["s"]                                             # [3, 2, npix]
+    gs = np.zeros((3, w.npix))
+    for p in range(w.npix):
+        dA = _dA_numpy(w.freqs, w.truth["beta_d"][p], w.truth["T_d"][p], w.truth["beta_s"][p])
+        for t in range(3):
+            gs[t, p] = sum(abs(s[comp_of[t], S, p]) * np.sum(wf * np.abs(d[:, S, p].astype(np.float64)) * np.abs(dA[t]))
+                           for S in range(2))
+    o = 0
+    for t in range(3):
+        want = np.bincount(idx[t], weights=gs[t], minlength=K[t])
+        assert np.allclose(r["gscale"][o:o + K[t]], want, rtol=5e-6)     # fp32 rounding of d moves s by ~1e-7
+        o += K[t]
+    # the gradient is zero to the rounding of the fp32 data, many orders below the scale
+    assert np.all(np.abs(r["grad"]) <= 1e-5 * r["gscale"])
+
+
+def test_tolerance_scales_follow_the_scalings_of_the_gradient(model, c1):
+    """Ninv -> c Ninv scales grad, absg and gscale by c; relabelling clusters permutes all three alike."""
+    d, idx, K = _entry(c1)
+    params = c1.params_jittered(seed=5)
+    r1 = oracle.nll_grad(model, d, c1.ninv, idx, K, params, want_tol=True)
+    r4 = oracle.nll_grad(model, d, (4.0 * c1.ninv).astype(np.float32), idx, K, params, want_tol=True)
+    for key in ("grad", "absg", "gscale"):
+        assert np.allclose(r4[key], 4.0 * r1[key], rtol=1e-13)
+    perm = np.array([2, 0, 3, 1], dtype=np.int32)               # new label of old cluster k of the beta_d map
+    idx2 = idx.copy()
+    idx2[0] = perm[idx[0]]
+    p2 = params.copy()
+    p2[:K[0]][perm] = params[:K[0]]
+    r2 = oracle.nll_grad(model, d, c1.ninv, idx2, K, p2, want_tol=True)
+    for key in ("grad", "absg", "gscale"):
+        assert np.allclose(r2[key][:K[0]][perm], r1[key][:K[0]], rtol=1e-13)
+        assert np.allclose(r2[key][K[0]:], r1[key][K[0]:], rtol=1e-13)
