@@ -62,3 +62,62 @@ def test_recovers_known_optimum_on_noiseless_cluster_constant_sky():
     dd = d.astype(np.float64)
     dNd = float(np.einsum("f,fsp,fsp->", w.ninv.astype(np.float64), dd, dd))
     assert L + 0.5 * dNd < 1e-3 * abs(hist[0] + 0.5 * dNd)      # misfit reduced by > 1000x towards the noiseless optimum 0
+
+
+def _box_problem(n=40, seed=78):
+    """Separable quadratic on [0,1]^n whose targets are all inside the box, started with every parameter ON a bound."""
+    g = gen.rng_for("misc", seed)
+    c = 1.0 + 9.0 * g.random(n)
+    t = g.uniform(0.2, 0.8, n)
+
+    def fun(x, want_grad):
+        return 0.5 * float(np.sum(c * (x - t) ** 2)), (c * (x - t) if want_grad else None)
+    x0 = np.where(np.arange(n) % 2 == 0, 0.0, 1.0)
+    return fun, x0, t
+
+
+def test_topk_zero_releases_exactly_one_bound_per_iteration():
+    # A3 (L535): "K=0 (single-parameter release per iteration, matching the classical TNC strategy)"
+    fun, x0, t = _box_problem()
+    rel = []
+    adatopk(fun, x0, np.zeros_like(x0), np.ones_like(x0), iters=25, released=rel)
+    assert rel == [1] * 25
+
+
+def test_topk_one_releases_every_bound_pushed_inwards_at_once():
+    # A3 (L531): "K=1.0 (all constraints released simultaneously)"; every start value sits on the wrong side of its target
+    fun, x0, t = _box_problem()
+    rel = []
+    x, L = adatopk(fun, x0, np.zeros_like(x0), np.ones_like(x0), iters=400, lr=0.05, topk=1.0, released=rel)
+    assert rel[0] == len(x0) and sum(rel[1:]) == 0
+    assert np.max(np.abs(x - t)) < 5e-3
+
+
+def test_topk_fraction_releases_floor_of_the_fraction_of_the_bound_set():
+    # n = max(1, floor(topk * n_bound)); the bound set shrinks as parameters are released
+    fun, x0, t = _box_problem(n=40)
+    rel = []
+    adatopk(fun, x0, np.zeros_like(x0), np.ones_like(x0), iters=6, topk=0.25, released=rel)
+    nb, want = 40, []
+    for _ in range(6):
+        n = max(1, int(np.floor(0.25 * nb)))
+        want.append(n)
+        nb -= n
+    assert rel == want                                   # 10, 7, 5, 4, 3, 2
+    # and the released ones are those with the largest scores: after one iteration the 10 largest c_i |x0_i - t_i| are free
+    hist = []
+    x1, _ = adatopk(fun, x0, np.zeros_like(x0), np.ones_like(x0), iters=1, topk=0.25, history=hist)
+    moved = np.flatnonzero(x1 != x0)
+    c_t = np.abs(fun(x0, True)[1])
+    assert set(moved.tolist()) == set(np.argsort(c_t)[::-1][:10].tolist())
+
+
+def test_topk_keeps_bounds_and_monotonicity():
+    fun, x0, t = _box_problem(n=30, seed=79)
+    t[:5] = [1.4, -0.3, 1.2, -0.1, 1.6]                  # minima beyond the box: those parameters must stay / end pinned
+    for topk in (0.0, 0.3, 1.0):
+        hist = []
+        x, L = adatopk(fun, x0, np.zeros_like(x0), np.ones_like(x0), iters=500, lr=0.05, topk=topk, history=hist)
+        assert np.all(x >= 0.0) and np.all(x <= 1.0)
+        assert all(b <= a for a, b in zip(hist, hist[1:]))
+        assert np.max(np.abs(x - np.clip(t, 0, 1))) < 5e-3, topk
