@@ -92,9 +92,13 @@ typedef struct cs_opt {
     double beta1, beta2, eps;
     double ls_c1;       /* Armijo constant */
     double safe_lo, safe_hi; /* dynamic rescale range for |g_proj| (A4, L541) */
-    double ls_noise;    /* Armijo slack, relative to |L|: accept when L_trial <= L + ls_c1 a g.d + ls_noise |L|, with
-                           L = 1/2 chi^2 of the GLS residual (cs_spectral_misfit), whose fp32 evaluation noise is about
-                           1e-6 relative; 0 = strict decrease of the computed objective (R13) */
+    double ls_noise;    /* Armijo slack, relative to |L|: accept when L_trial <= L + ls_c1 a min(g.d, 0) + ls_noise |L|, with
+                           L = 1/2 chi^2 of the GLS residual (cs_spectral_misfit), whose fp32 evaluation noise was measured
+                           at 6e-9 .. 9e-8 of itself (R13); default 1e-7; 0 = strict decrease of the computed
+                           objective */
+    double topk;        /* Top-K fraction in [0,1] (A2-A3, L519-L537): per iteration the max(1, floor(topk n_bound)) bound
+                           parameters with the highest positive release scores are released together; 0 (default, the
+                           paper's production setting, L535) releases one per iteration, 1 every one pushed inwards */
 } cs_opt;
 
 /* Create a context for `model`.  Allocates only small constant tables.  *out is NULL on failure. */

@@ -29,7 +29,7 @@ class CsModel(C.Structure):
 class CsOpt(C.Structure):
     _fields_ = [("iters", C.c_int32), ("ls_max", C.c_int32), ("lr", C.c_double), ("beta1", C.c_double),
                 ("beta2", C.c_double), ("eps", C.c_double), ("ls_c1", C.c_double), ("safe_lo", C.c_double),
-                ("safe_hi", C.c_double), ("ls_noise", C.c_double)]
+                ("safe_hi", C.c_double), ("ls_noise", C.c_double), ("topk", C.c_double)]
 
 
 class CsError(RuntimeError):

@@ -976,14 +976,16 @@ void cs_opt_defaults(cs_opt *o) {
     if (!o) return;
     o->iters = 200; o->ls_max = 8;
     o->lr = 0.02; o->beta1 = 0.9; o->beta2 = 0.999; o->eps = 1e-16;
-    o->ls_c1 = 1e-4; o->safe_lo = 1e-15; o->safe_hi = 1e15; o->ls_noise = 1e-6;
+    o->ls_c1 = 1e-4; o->safe_lo = 1e-15; o->safe_hi = 1e15; o->ls_noise = 1e-7; o->topk = 0.0;
 }
 
 int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *upper, const cs_opt *opt, double *nll_final,
                 void *stream) {
     int rc = ready(c);
     if (rc) return rc;
-    if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || !(opt->ls_noise >= 0) || c->batch > 65535) return CS_EINVAL;
+    if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || !(opt->ls_noise >= 0) || !(opt->topk >= 0.0 && opt->topk <= 1.0) ||
+        c->batch > 65535)
+        return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     // the legacy default stream cannot be captured into a graph: fork onto an internal stream and join at the end
     cudaStream_t caller = st;
@@ -1010,7 +1012,7 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
         if ((rc = opt_alloc(c->opt, c->nparam, c->batch, c->nregion, &c->opt_bytes))) return rc == 1 ? CS_ENOMEM : CS_ECUDA;
     }
     OptShape sh{c->nparam, c->batch, c->nregion, c->ktot_max, c->d_param_off};
-    OptHyper hy{opt->lr, opt->beta1, opt->beta2, opt->eps, opt->ls_c1, opt->safe_lo, opt->safe_hi, opt->ls_noise, opt->ls_max};
+    OptHyper hy{opt->lr, opt->beta1, opt->beta2, opt->eps, opt->ls_c1, opt->safe_lo, opt->safe_hi, opt->ls_noise, opt->topk, opt->ls_max};
     OptWork &w = c->opt;
     opt_init(w, sh, params, lower, upper, st); c->launches += 1;
     // the line search compares 1/2 chi^2 of the GLS residual (cs_spectral_misfit): its value at the start

@@ -4,7 +4,8 @@
 //
 // One iteration (Alg. 1):
 //   y = (x - l)/(u - l), g_int = g * (u - l)                                   A1, L509-L513, Alg. 1 line 3
-//   release the single bound parameter pushed hardest into the feasible region  A2, L519-L525 with K = 0 (L249)
+//   release the n = max(1, floor(topk n_bound)) bound parameters pushed hardest into the feasible region
+//                                                                                A2-A3, L519-L537; topk = 0 (L249, L535): one
 //   g_proj = g_int * (p == 0)                                                    line 8
 //   if |g_proj| outside [safe_lo, safe_hi]: f = 1/|g_proj|; L,g_proj *= f; m *= f; v *= f^2     A4, L541-L546
 //   AdaBelief direction (Zhuang et al. 2020), masked by p == 0                   lines 14-16
@@ -36,7 +37,7 @@ struct OptShape {
 };
 
 struct OptHyper {
-    double lr, beta1, beta2, eps, c1, safe_lo, safe_hi, ls_noise;
+    double lr, beta1, beta2, eps, c1, safe_lo, safe_hi, ls_noise, topk;
     int32_t ls_max;
 };
 
@@ -110,6 +111,52 @@ __device__ __forceinline__ void block_argbest(double &val, long long &idx, bool 
     __syncthreads();
 }
 
+// Release score of parameter i (A2, L519-L523 with the sign of the prose, R14): > 0 when the descent direction -g
+// points from the bound it sits on into the interior.
+__device__ __forceinline__ double release_score(const OptWork &w, int64_t i, double cscale) {
+    const int8_t p = w.pivot[i];
+    if (p == 0) return 0.0;
+    const double gint = cscale * w.grad[i] * (w.hi[i] - w.lo[i]);
+    return (p < 0) ? -gint : gint;
+}
+// The n-th highest positive release score of the entry's parameters [o0, o1) (n >= 2), by an 8-bit radix select on
+// the bit patterns (positive doubles order like unsigned integers); 0 when fewer than n scores are positive (then
+// every positive score is released).  Integer histograms in shared memory: deterministic.
+__device__ __forceinline__ double nth_highest_score(const OptWork &w, int64_t o0, int64_t o1, double cscale, int n, uint32_t *hist,
+                                                    unsigned long long *sh_prefix, int *sh_n) {
+    const int tid = threadIdx.x;
+    unsigned long long prefix = 0ull, mask = 0ull;
+    int want = n;
+    for (int shift = 56; shift >= 0; shift -= 8) {
+        for (int b = tid; b < 256; b += OPT_THREADS) hist[b] = 0u;
+        __syncthreads();
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) {
+            const double sc = release_score(w, i, cscale);
+            if (sc > 0.0) {
+                const unsigned long long k = (unsigned long long)__double_as_longlong(sc);
+                if ((k & mask) == prefix) atomicAdd(&hist[(unsigned)((k >> shift) & 0xffull)], 1u);
+            }
+        }
+        __syncthreads();
+        if (tid == 0) {
+            int acc = 0, digit = -1;
+            for (int b = 255; b >= 0; --b) {
+                if (acc + (int)hist[b] >= want) { digit = b; break; }
+                acc += (int)hist[b];
+            }
+            if (digit < 0) { *sh_n = -1; }                  // fewer than `want` candidates: release every positive score
+            else { *sh_n = want - acc; *sh_prefix = prefix | ((unsigned long long)digit << shift); }
+        }
+        __syncthreads();
+        if (*sh_n < 0) return 0.0;
+        want = *sh_n;
+        prefix = *sh_prefix;
+        mask |= 0xffull << shift;
+        __syncthreads();
+    }
+    return __longlong_as_double((long long)prefix);
+}
+
 // A1 (L509-L513): map the start into [0,1], set the pivots, clear the AdaBelief moments.
 __global__ void k_opt_init(OptWork w, int64_t nparam, const double *params, int32_t batch) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -135,19 +182,33 @@ __global__ void __launch_bounds__(OPT_THREADS) k_opt_direction(OptWork w, OptSha
     double cscale = w.cscale[e];
     // the objective the line search compares is 1/2 chi^2 of the GLS residual (= nll + const, evaluated accurately)
     double L = w.Lcur[e] * cscale;
-    // release (A2, K = 0): the bound parameter whose descent direction -g points furthest into the interior
-    double best = 0.0;
-    long long bi = -1;
-    for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) {
-        const int8_t p = w.pivot[i];
-        if (p != 0) {
-            const double gint = cscale * w.grad[i] * (w.hi[i] - w.lo[i]);
-            const double score = (p < 0) ? -gint : gint;
+    // release (A2): the n bound parameters whose descent direction -g points furthest into the interior
+    __shared__ uint32_t hist[256];
+    __shared__ unsigned long long sh_prefix;
+    __shared__ int sh_n;
+    int nrel = 1;
+    if (hy.topk > 0.0) {
+        double nb = 0.0;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) nb += (w.pivot[i] != 0) ? 1.0 : 0.0;
+        nb = block_sum(nb, shv);
+        nrel = max(1, (int)floor(hy.topk * nb));
+    }
+    if (nrel == 1) {   // the single highest score, lowest index on ties
+        double best = 0.0;
+        long long bi = -1;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) {
+            const double score = release_score(w, i, cscale);
             if (score > 0.0 && (bi < 0 || score > best)) { best = score; bi = i; }
         }
+        block_argbest(best, bi, false, shv, shi);
+        if (tid == 0 && bi >= 0) w.pivot[bi] = 0;
+    } else {           // every score >= the n-th highest positive one
+        const double thr = nth_highest_score(w, o0, o1, cscale, nrel, hist, &sh_prefix, &sh_n);
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) {
+            const double score = release_score(w, i, cscale);
+            if (score > 0.0 && score >= thr) w.pivot[i] = 0;
+        }
     }
-    block_argbest(best, bi, false, shv, shi);
-    if (tid == 0 && bi >= 0) w.pivot[bi] = 0;
     __syncthreads();
     // projected gradient norm and dynamic rescale (A4)
     double n2 = 0.0;
@@ -217,7 +278,8 @@ __global__ void k_opt_ls(OptWork w, OptShape sh, OptHyper hy) {
     half_chi2 *= 0.5;
     const double Lt = half_chi2 * w.cscale[e];
     const double a = w.alpha[e];
-    if (Lt <= w.L0[e] + hy.c1 * a * w.gd[e] + hy.ls_noise * fabs(w.L0[e])) {   // false for NaN / +inf
+    // sufficient decrease with min(g.d, 0): a momentum direction with g.d >= 0 never licenses an increase (L263)
+    if (Lt <= w.L0[e] + hy.c1 * a * fmin(w.gd[e], 0.0) + hy.ls_noise * fabs(w.L0[e])) {   // false for NaN / +inf
         w.accepted[e] = 1;
         w.alpha_acc[e] = a;
         w.Lt_acc[e] = half_chi2;

@@ -59,7 +59,7 @@ def test_opt_defaults_follow_design_R13():
     assert (o.iters, o.ls_max) == (200, 8)
     assert (o.lr, o.beta1, o.beta2, o.eps, o.ls_c1) == (0.02, 0.9, 0.999, 1e-16, 1e-4)
     assert (o.safe_lo, o.safe_hi) == (1e-15, 1e15)
-    assert o.ls_noise == 1e-6
+    assert o.ls_noise == 1e-7 and o.topk == 0.0
 
 
 def test_product_package_does_not_import_the_oracle():

@@ -11,6 +11,7 @@ import gen
 import oracle
 import helpers
 from helpers import make_ctx, new_ctx, gpu_eval, gpu_maps, oracle_entry, check_T1, check_T2, check_T3
+from oracle.adatopk import adatopk
 
 pytestmark = pytest.mark.gpu
 
@@ -384,51 +385,116 @@ def _bounds(w):
     return lo, hi
 
 
-def test_optimizer_recovers_truth_on_noiseless_cluster_constant_sky(torch_cuda, path):
-    """a5 / R13: 200 AdaTopK iterations from (1.54, 20, -3) on a sky whose truth is constant per cluster
-    (PAPER.md:L287), against the fp64 reference of the same reading (oracle/adatopk.py): bounds are never violated,
-    the objective ends as low as the reference's up to the fp32 evaluation noise, and the truth is recovered as well
-    as the reference recovers it (trajectories are not unique, R12: parameters are compared with the truth, not with
-    each other)."""
-    import torch
-    import paper_2604_08463_b200 as cs
-    from oracle.adatopk import adatopk
-    w = gen.make_config(1, nside=16, K=(60, 8, 12), noiseless=True, cluster_truth=True)
-    ctx, _ = make_ctx(w)
-    lo, hi = _bounds(w)
-    p = torch.from_numpy(w.params_const()).cuda()
-    nll0, _ = gpu_eval(ctx, w.params_const())
-    nf = torch.zeros(w.batch, dtype=torch.float64, device="cuda")
-    ctx.optimize(p, torch.from_numpy(lo).cuda(), torch.from_numpy(hi).cuda(), cs.opt_defaults(iters=200), nf)
-    torch.cuda.synchronize()
-    assert ctx.check() == 0
-    x = p.cpu().numpy()
-    assert np.all(x >= lo) and np.all(x <= hi)
-    assert nf.item() < nll0[0, 0]
-    # the fp64 reference of the same algorithm on the same inputs
+def _opt_problem(w):
+    """The fp64 reference's objective on entry 0 of w, and d^T N^-1 d / 2 (nll + it = 1/2 chi^2, the misfit)."""
     model, K = oracle.Model(w.freqs), w.K_of_cfg(0)
     d0, idx = w.data()[0], w.maps[w.cfg_maps[0]]
 
     def fun(xx, want_grad):
         r = oracle.nll_grad(model, d0, w.ninv, idx, K, xx, want_grad=want_grad)
         return r["nll"][0], r["grad"]
+    dd = d0.astype(np.float64)
+    return fun, 0.5 * float(np.einsum("f,fsp,fsp->", w.ninv.astype(np.float64), dd, dd)), K
+
+
+def _gpu_optimize(ctx, w, lo, hi, **opt):
+    import torch
+    import paper_2604_08463_b200 as cs
+    p = torch.from_numpy(w.params_const()).cuda()
+    nf = torch.zeros(w.batch, dtype=torch.float64, device="cuda")
+    ctx.optimize(p, torch.from_numpy(lo).cuda(), torch.from_numpy(hi).cuda(), cs.opt_defaults(**opt), nf)
+    torch.cuda.synchronize()
+    assert ctx.check() == 0
+    return p.cpu().numpy(), nf.cpu().numpy()
+
+
+def test_optimizer_recovers_truth_on_noiseless_cluster_constant_sky(torch_cuda, path):
+    """a5 / R13: 200 AdaTopK iterations from (1.54, 20, -3) on a sky whose truth is constant per cluster
+    (PAPER.md:L287), against the fp64 reference of the same reading (oracle/adatopk.py).
+    Measured on this sky (nside 16, K = (60, 8, 12); R13): the fp64 reference itself ends
+    1.80e-3 / 7.09e-2 K / 2.25e-4 from the truth (max abs per block) -- the survey's scratch figures
+    1e-3 / 5e-2 K / 1e-3 came from a different sky and do not hold for beta_d and T_d even in fp64 -- and the GPU ends
+    1.80e-3 / 7.10e-2 K / 2.31e-4 from it.  The thresholds below are those with a 2x margin: absolute
+    4e-3 / 0.15 K / 5e-4, and no further from the truth than the reference by more than 1e-5 / 3e-4 K / 2e-5."""
+    w = gen.make_config(1, nside=16, K=(60, 8, 12), noiseless=True, cluster_truth=True)
+    ctx, _ = make_ctx(w)
+    lo, hi = _bounds(w)
+    nll0, _ = gpu_eval(ctx, w.params_const())
+    x, nf = _gpu_optimize(ctx, w, lo, hi, iters=200)
+    assert np.all(x >= lo) and np.all(x <= hi)
+    assert nf[0] < nll0[0, 0]
+    # the fp64 reference of the same algorithm on the same inputs
+    fun, half_dNd, K = _opt_problem(w)
     hist = []
     x_ref, L_ref = adatopk(fun, w.params_const(), lo, hi, iters=200, history=hist)
     assert all(b <= a for a, b in zip(hist, hist[1:]))                 # reference: monotone (L263)
     truth = np.concatenate(w.truth["per_cluster"])
     blocks = [slice(0, K[0]), slice(K[0], K[0] + K[1]), slice(K[0] + K[1], None)]
-    for sl, floor in zip(blocks, (1e-3, 5e-2, 1e-3)):
+    for sl, absolute, excess in zip(blocks, (4e-3, 0.15, 5e-4), (1e-5, 3e-4, 2e-5)):
         e_gpu, e_ref = np.abs(x - truth)[sl].max(), np.abs(x_ref - truth)[sl].max()
-        assert e_ref < 4 * floor                                        # the reading itself converges
-        assert e_gpu <= 2.0 * e_ref + floor, (e_gpu, e_ref)
-    # objective: the oracle evaluated at the GPU's result is as low as the reference's end point, within the fp32
-    # evaluation noise of the line search (3e-8 |L|, cs_opt.ls_noise)
-    L_at_gpu = fun(x, False)[0]
-    assert L_at_gpu <= L_ref + 3e-8 * abs(L_ref), (L_at_gpu, L_ref)
+        assert e_gpu < absolute and e_ref < absolute, (e_gpu, e_ref)
+        assert e_gpu <= e_ref + excess, (e_gpu, e_ref)
+    # objective: the misfit 1/2 chi^2 = nll + d^T N^-1 d / 2, evaluated by the oracle at the GPU's result, has come
+    # down from 1.2e4 to the reference's 7.6e-2 within 1 % (measured 0.2 %)
+    m_gpu, m_ref = fun(x, False)[0] + half_dNd, L_ref + half_dNd
+    assert abs(m_gpu - m_ref) <= 1e-2 * m_ref, (m_gpu, m_ref)
     # the reported final objective is the objective at the returned parameters (T1 against the oracle)
     nll1, _ = gpu_eval(ctx, x)
-    assert nll1[0, 0] == nf.item()
-    assert abs(L_at_gpu - nf.item()) <= 1e-5 * abs(L_at_gpu)
+    assert nll1[0, 0] == nf[0]
+    assert abs(fun(x, False)[0] - nf[0]) <= 1e-5 * abs(nf[0])
+    ctx.close()
+
+
+@pytest.mark.parametrize("noiseless", [False, True])
+def test_optimizer_follows_the_fp64_reference_trajectory(torch_cuda, path, noiseless):
+    """a5: the objective after 1, 10, 50 and 200 iterations against the history of oracle/adatopk.py on the same
+    inputs.  Compared on the misfit 1/2 chi^2 = nll + d^T N^-1 d / 2 (the part of nll that depends on the parameters;
+    nll itself agrees to 1e-7 trivially because the constant dominates it), evaluated by the oracle at the GPU's
+    iterate.  Measured: noisy sky <= 1.6e-6 relative at every checkpoint; noiseless sky 2.6e-5 up to iteration 50,
+    2.2e-3 at iteration 200, where the misfit has fallen by five orders of magnitude."""
+    w = gen.make_config(1, nside=16, K=(60, 8, 12), noiseless=noiseless, cluster_truth=True)
+    ctx, _ = make_ctx(w)
+    lo, hi = _bounds(w)
+    fun, half_dNd, K = _opt_problem(w)
+    hist = []
+    _, L_ref = adatopk(fun, w.params_const(), lo, hi, iters=200, history=hist)
+    hist.append(L_ref)                                                   # hist[k] = objective after k iterations
+    tol = {1: 1e-5, 10: 1e-4, 50: 1e-4, 200: 1e-2} if noiseless else {1: 1e-5, 10: 1e-5, 50: 1e-5, 200: 1e-5}
+    for k in (1, 10, 50, 200):
+        x, nf = _gpu_optimize(ctx, w, lo, hi, iters=k)
+        m_gpu, m_ref = fun(x, False)[0] + half_dNd, hist[k] + half_dNd
+        assert abs(m_gpu - m_ref) <= tol[k] * m_ref, (k, m_gpu, m_ref)
+        assert abs(nf[0] - hist[k]) <= 1e-7 * abs(hist[k]), (k, nf[0], hist[k])
+    ctx.close()
+
+
+def test_optimizer_topk_release_matches_the_reference(torch_cuda, path):
+    """f4(i), A2-A3: with a Top-K fraction the GPU driver releases the same number of bound parameters per iteration
+    as the reference and ends at the same objective.  Start with every T_d on its lower bound and every beta_s on its
+    upper bound, so that releases are what the first iterations are about."""
+    w = gen.make_config(1, nside=16, K=(60, 8, 12), cluster_truth=True)
+    ctx, _ = make_ctx(w)
+    lo, hi = _bounds(w)
+    fun, half_dNd, K = _opt_problem(w)
+    import torch
+    import paper_2604_08463_b200 as cs
+    x0 = w.params_const()
+    x0[K[0]:K[0] + K[1]] = lo[K[0]:K[0] + K[1]]
+    x0[K[0] + K[1]:] = hi[K[0] + K[1]:]
+    for topk in (0.0, 0.5, 1.0):
+        for iters in (1, 3, 40):
+            rel = []
+            x_ref, L_ref = adatopk(fun, x0, lo, hi, iters=iters, topk=topk, released=rel)
+            p = torch.from_numpy(x0).cuda()
+            nf = torch.zeros(1, dtype=torch.float64, device="cuda")
+            ctx.optimize(p, torch.from_numpy(lo).cuda(), torch.from_numpy(hi).cuda(), cs.opt_defaults(iters=iters, topk=topk), nf)
+            torch.cuda.synchronize()
+            x = p.cpu().numpy()
+            assert np.all(x >= lo) and np.all(x <= hi)
+            if iters <= 3:      # which parameters have left their bound: the same set as in the reference
+                assert np.array_equal(x != x0, x_ref != x0), (topk, iters, rel)
+            m_gpu, m_ref = fun(x, False)[0] + half_dNd, L_ref + half_dNd
+            assert abs(m_gpu - m_ref) <= 1e-4 * m_ref, (topk, iters, m_gpu, m_ref)
     ctx.close()
 
 
@@ -451,7 +517,8 @@ def test_optimizer_batch_is_independent_and_monotone(torch_cuda, path):
         res[iters] = (p.cpu().numpy(), nf.cpu().numpy())
         assert np.all(res[iters][0] >= lo) and np.all(res[iters][0] <= hi)
     nll0, _ = gpu_eval(ctx, w.params_const())
-    slack = 3e-8 * np.abs(nll0.sum(axis=1)) * 40          # at most ls_noise |L| per accepted step
+    # every accepted step may exceed strict decrease by at most the documented slack ls_noise |L|, L = 1/2 chi^2 <= |nll|
+    slack = cs.opt_defaults().ls_noise * np.abs(nll0.sum(axis=1)) * 35
     assert np.all(res[5][1] <= nll0.sum(axis=1)) and np.all(res[40][1] <= res[5][1] + slack)
     off = w.param_offsets()
     for e in (0, 3):
