@@ -55,7 +55,8 @@ extern "C" {
 #define CS_OPT_LAYOUT        1 /* CS_LAYOUT_*; set before cs_set_clusters */
 #define CS_OPT_FORM          2 /* CS_FORM_*; set before cs_set_batch */
 #define CS_OPT_MIN_FILL      3 /* CS_LAYOUT_AUTO: smallest fill fraction live pixels / (tiles * 512) of a configuration's
-                                  sorted layout for which it is taken (default 0.85); set before cs_set_clusters */
+                                  sorted layout for which it is taken (default 0.45: below it the padding
+                                  costs more than the direct kernel); set before cs_set_clusters */
 #define CS_OPT_COPY_LIMIT_MB 4 /* most device memory [MiB] the private sorted copies of a batch may take; 0 (default) =
                                   70 % of the memory free when cs_set_batch runs.  Beyond it cs_set_batch returns CS_ENOMEM. */
 #define CS_LAYOUT_AUTO    0 /* sorted layout for configurations whose tiles fill well, in place for the others */
@@ -161,6 +162,18 @@ CS_API int cs_spectral_misfit(cs_ctx *ctx, double *chi2, void *stream);
  * batch).  Masked pixels are written as 0.  Asynchronous on `stream` like the other hot-path calls (the selection
  * travels through a pinned staging ring; nothing is allocated and the stream is not synchronised). */
 CS_API int cs_component_maps(cs_ctx *ctx, int32_t nsel, const int32_t *entries, float *s, void *stream);
+
+/* f3, the cell-compressed likelihood (PAPER.md:L95 patch model, L80 Eq. 6): pixels with the same cluster triple share
+ * A, so their part of Eq. 6 is tr(M^-1 A^T T A) with the parameter-independent second moments
+ * T = N^-1 (sum_{p,S} d_S d_S^T) N^-1 of the cell.  cs_cell_moments builds T (fp64) for every (configuration, data set)
+ * pair of the current batch from the current data -- call it once after cs_set_data / cs_set_batch, and again when the
+ * data change; it allocates its workspace on the first call.  cs_spectral_like_grad_cells then evaluates nll and grad
+ * (same meaning, layout and tolerances as cs_spectral_like_grad) for the tables last built, from T alone, in fp64: one
+ * 15 x 15 contraction per cell instead of one pass over every pixel.  It pays when cells hold more than ~8 pixels
+ * (a clustering scan over coarse configurations) and is slower than the per-pixel path at K ~ npix.
+ * Requirements: nfreq <= 15 and every configuration of the batch on the sorted layout (CS_EINVAL otherwise). */
+CS_API int cs_cell_moments(cs_ctx *ctx, void *stream);
+CS_API int cs_spectral_like_grad_cells(cs_ctx *ctx, double *nll, double *grad, void *stream);
 
 /* f1 (Eq. 10): per entry and region, variance over unmasked pixels of the reconstructed CMB map, Q and U
  * summed: var dev [batch*nregion] fp64, computed without writing the maps. */

@@ -16,7 +16,7 @@ LAYOUT_AUTO, LAYOUT_INPLACE, LAYOUT_SORTED = 0, 1, 2
 FORM_AUTO, FORM_DIRECT = 0, 1
 
 EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
-           "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
+           "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_cell_moments", "cs_spectral_like_grad_cells", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
            "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
 
@@ -67,6 +67,8 @@ def lib():
         "cs_build_sed_tables": (C.c_int, [vp, vp, vp]),
         "cs_spectral_like_grad": (C.c_int, [vp, vp, vp, vp]),
         "cs_spectral_misfit": (C.c_int, [vp, vp, vp]),
+        "cs_cell_moments": (C.c_int, [vp, vp]),
+        "cs_spectral_like_grad_cells": (C.c_int, [vp, vp, vp, vp]),
         "cs_component_maps": (C.c_int, [vp, i32, vp, vp, vp]),
         "cs_cmb_variance": (C.c_int, [vp, vp, vp]),
         "cs_optimize": (C.c_int, [vp, vp, vp, vp, C.POINTER(CsOpt), vp, vp]),
@@ -232,6 +234,14 @@ class Context:
     def spectral_misfit(self, chi2, stream=None):
         _chk(lib().cs_spectral_misfit(self._h, _ptr(chi2, "float64", "cuda", self.batch * self.nregion, "chi2"), _stream(stream)),
              "cs_spectral_misfit")
+
+    def cell_moments(self, stream=None):
+        _chk(lib().cs_cell_moments(self._h, _stream(stream)), "cs_cell_moments")
+
+    def spectral_like_grad_cells(self, nll, grad=None, stream=None):
+        _chk(lib().cs_spectral_like_grad_cells(self._h, _ptr(nll, "float64", "cuda", self.batch * self.nregion, "nll"),
+                                               _ptr(grad, "float64", "cuda", self.nparam, "grad"), _stream(stream)),
+             "cs_spectral_like_grad_cells")
 
     def component_maps(self, s, entries=None, stream=None):
         if entries is None:

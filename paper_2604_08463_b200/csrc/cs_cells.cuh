@@ -1,0 +1,211 @@
+// cs_cells.cuh -- f3: the cell-compressed likelihood (PAPER.md:L95 patch model, L80 Eq. 6).
+//
+// All pixels of a cell (same cluster triple and region) share A, so their contribution to Eq. 6 depends on the data
+// only through the cell's second moments:
+//
+//     sum_{p in cell} sum_S b_S^T M^-1 b_S  =  tr( M^-1 A^T T A ),        T = N^-1 (sum_{p,S} d_S d_S^T) N^-1   [F x F]
+//
+// T is independent of the parameters: k_cc_moments builds it once per (configuration, data set) pair, in fp64, from
+// the caller's data.  A likelihood + gradient evaluation then costs one F x F contraction per cell instead of one
+// pass over every pixel (k_like_cc, fp64; one thread per (entry, cell)):
+//
+//     u_i  = T a_i   (a_0 = 1, a_1 = a_d, a_2 = a_s) ;   B = A^T T A ;   nll_cell = -1/2 tr(M^-1 B)
+//     g_th = X[j,:] . P_th  -  M^-1[j,:] . (U^T a'_th) ,   X = M^-1 B M^-1 ,  P_th = A^T N^-1 a'_th ,  j = column of th
+//
+// which is Eq. 17 summed over the cell's pixels with s = M^-1 A^T N^-1 d written out.  The per-cell
+// terms are then summed onto clusters and regions in ascending cell order (k_cc_reduce, fp64, deterministic).
+// Cells are the tile-cells of the configuration's sorted layout (a cell that straddles a tile boundary counts twice,
+// which changes nothing in the sums).  Pays when cells hold more than ~8 pixels (960 B of moments against 120 B per
+// pixel); useless at K ~ npix.
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include "cs_internal.h"
+
+namespace cs {
+
+constexpr int CC_NMOM = NROW * (NROW - 1) / 2;   // 120 = 15 * 16 / 2 unique entries of a symmetric 15 x 15 (generic nfreq <= 16: 136 would be needed; see CC_MAXF)
+constexpr int CC_MAXF = 15;                      // f3 is built for nfreq <= 15 (the LiteBIRD-like band set)
+__host__ __device__ __forceinline__ int cc_idx(int f, int g) {   // packed upper triangle of a 15 x 15 symmetric matrix, f <= g
+    return f * CC_MAXF - (f * (f - 1)) / 2 + (g - f);
+}
+
+// Global (per configuration) cell list of the sorted layout.
+struct CellsDev {
+    const int32_t *cellpos;    // [ncell] first position of the cell (global position index = tile * TPX + offset)
+    const int32_t *celllen;    // [ncell] positions it covers (pads included)
+    const int32_t *cellrows;   // [ncell][4] table rows (Fd', G, dlnG, Fs') = CfgDev::cellrows
+    const int32_t *cellreg;    // [ncell] region
+    const int32_t *kptr[4];    // CSR cluster (t = 0..2) / region (t = 3) -> cells: [K_t + 1]
+    const int32_t *klist[4];   // [ncell] cells of each cluster in ascending order
+    int32_t ncell;
+    int32_t pad;
+};
+
+struct MomJob {
+    int32_t cfg, data;
+    int64_t off;   // double offset of the pair's moments [CC_NMOM][ncell] inside the moments buffer
+};
+
+// Second moments of one (configuration, data set) pair: one warp per cell, lane l owns the unique (f,g) pairs l, l+32,
+// l+64, l+96.  The cell's pixels are staged 32 at a time in shared memory (row stride 33: lanes reading different
+// bands hit different banks).  grid = (ceil(ncell_max / 4), pairs), block = 128.
+__global__ void __launch_bounds__(128) k_cc_moments(const float *__restrict__ d, int64_t npix, int32_t nfreq, const CfgDev *__restrict__ cfgs,
+                                                    const CellsDev *__restrict__ cells, const MomJob *__restrict__ jobs,
+                                                    const float *__restrict__ w, double *__restrict__ mom) {
+    __shared__ float sd[4][2 * CC_MAXF][33];
+    const MomJob job = jobs[blockIdx.y];
+    const CellsDev *cl = cells + job.cfg;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int c = blockIdx.x * 4 + warp;
+    if (c >= cl->ncell) return;
+    const int32_t *pospix = cfgs[job.cfg].pospix;
+    const int pos0 = cl->cellpos[c], len = cl->celllen[c];
+    const float *dd = d + (int64_t)job.data * 2 * nfreq * npix;
+    int pf[4], pg[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {   // unpack the lane's pairs
+        int idx = lane + 32 * q, f = 0;
+        pf[q] = pg[q] = -1;
+        if (idx < CC_NMOM) {
+            while (idx >= CC_MAXF - f) { idx -= CC_MAXF - f; ++f; }
+            pf[q] = f; pg[q] = f + idx;
+            if (pg[q] >= nfreq) pf[q] = pg[q] = -1;
+        }
+    }
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int j0 = 0; j0 < len; j0 += 32) {
+        const int j = j0 + lane;
+        const int pix = (j < len) ? pospix[pos0 + j] : -1;
+        for (int r = 0; r < 2 * nfreq; ++r) sd[warp][r][lane] = (pix >= 0) ? __ldg(dd + (int64_t)r * npix + pix) : 0.f;
+        __syncwarp();
+        const int n = min(32, len - j0);
+        for (int x = 0; x < n; ++x) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (pf[q] >= 0) {
+                    acc[q] = fma((double)sd[warp][2 * pf[q]][x], (double)sd[warp][2 * pg[q]][x], acc[q]);           // Q
+                    acc[q] = fma((double)sd[warp][2 * pf[q] + 1][x], (double)sd[warp][2 * pg[q] + 1][x], acc[q]);   // U
+                }
+        }
+        __syncwarp();
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int idx = lane + 32 * q;
+        if (idx < CC_NMOM)
+            mom[job.off + (int64_t)idx * cl->ncell + c] = (pf[q] >= 0) ? (double)w[pf[q]] * (double)w[pg[q]] * acc[q] : 0.0;
+    }
+}
+
+// One (entry, cell): nll term and the three gradient terms from the cell's moments, in fp64.
+// grid = (ceil(ncell_max / 128), batch), block = 128.  out[e] = [4][ncell_max] (ll, g_beta_d, g_T_d, g_beta_s).
+__global__ void __launch_bounds__(128) k_like_cc(const CfgDev *__restrict__ cfgs, const CellsDev *__restrict__ cells,
+                                                 const int32_t *__restrict__ cfg_of, const int64_t *__restrict__ mom_off,
+                                                 const int64_t *__restrict__ tab_off, const float *__restrict__ tab,
+                                                 const double *__restrict__ mom, KConst kc, int32_t nfreq, int32_t want_grad,
+                                                 double *__restrict__ out, int64_t out_stride, int32_t *err) {
+    const int e = blockIdx.y;
+    const CellsDev *cl = cells + cfg_of[e];
+    const int ncell = cl->ncell;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    const int4 rows = __ldg(reinterpret_cast<const int4 *>(cl->cellrows) + c);
+    const float *tb = tab + tab_off[e] * NROW;
+    const float *rFd = tb + (int64_t)rows.x * NROW, *rG = tb + (int64_t)rows.y * NROW, *rdG = tb + (int64_t)rows.z * NROW,
+                *rFs = tb + (int64_t)rows.w * NROW;
+    double a1[CC_MAXF], a2[CC_MAXF];
+    float dg[CC_MAXF];
+    // M = A^T N^-1 A and P_th = A^T N^-1 a'_th from the columns (the table values are the fp32 ones the per-pixel path uses)
+    double m00 = 0, m01 = 0, m02 = 0, m11 = 0, m12 = 0, m22 = 0;
+    double p1[3] = {0, 0, 0}, p2[3] = {0, 0, 0}, p3[3] = {0, 0, 0};
+#pragma unroll
+    for (int f = 0; f < CC_MAXF; ++f) {
+        a1[f] = 0.0; a2[f] = 0.0; dg[f] = 0.f;
+        if (f < nfreq) {
+            a1[f] = (double)__ldg(rFd + f) * (double)__ldg(rG + f);
+            a2[f] = (double)__ldg(rFs + f);
+            dg[f] = __ldg(rdG + f);
+            const double wf = (double)kc.w[f], wd = wf * a1[f], ws = wf * a2[f];
+            m00 += wf; m01 += wd; m02 += ws; m11 += wd * a1[f]; m12 += wd * a2[f]; m22 += ws * a2[f];
+            const double u1 = (double)kc.lnd[f] * wd, u2 = (double)dg[f] * wd, u3 = (double)kc.lns[f] * ws;
+            p1[0] += u1; p1[1] += u1 * a1[f]; p1[2] += u1 * a2[f];
+            p2[0] += u2; p2[1] += u2 * a1[f]; p2[2] += u2 * a2[f];
+            p3[0] += u3; p3[1] += u3 * a1[f]; p3[2] += u3 * a2[f];
+        }
+    }
+    // B = A^T T A and V_th = U^T a'_th, row by row of T (u_i[f] = sum_g T_fg a_i[g] is never stored)
+    const double *T = mom + mom_off[e] + c;
+    double b00 = 0, b01 = 0, b02 = 0, b11 = 0, b12 = 0, b22 = 0;
+    double v1[3] = {0, 0, 0}, v2[3] = {0, 0, 0}, v3[3] = {0, 0, 0};
+#pragma unroll
+    for (int f = 0; f < CC_MAXF; ++f) {
+        double u0 = 0, u1 = 0, u2 = 0;
+#pragma unroll
+        for (int g = 0; g < CC_MAXF; ++g) {
+            const double t = __ldg(T + (int64_t)(f <= g ? cc_idx(f, g) : cc_idx(g, f)) * ncell);
+            u0 += t; u1 = fma(t, a1[g], u1); u2 = fma(t, a2[g], u2);
+        }
+        b00 += u0; b01 += u1; b02 += u2;
+        b11 = fma(a1[f], u1, b11); b12 = fma(a1[f], u2, b12); b22 = fma(a2[f], u2, b22);
+        const double d1 = (double)kc.lnd[f] * a1[f], d2 = (double)dg[f] * a1[f], d3 = (double)kc.lns[f] * a2[f];
+        v1[0] = fma(d1, u0, v1[0]); v1[1] = fma(d1, u1, v1[1]); v1[2] = fma(d1, u2, v1[2]);
+        v2[0] = fma(d2, u0, v2[0]); v2[1] = fma(d2, u1, v2[1]); v2[2] = fma(d2, u2, v2[2]);
+        v3[0] = fma(d3, u0, v3[0]); v3[1] = fma(d3, u1, v3[1]); v3[2] = fma(d3, u2, v3[2]);
+    }
+    // M^-1 by cofactors (3 x 3 symmetric positive definite; cond ~ 5, R11)
+    const double c00 = m11 * m22 - m12 * m12, c01 = m02 * m12 - m01 * m22, c02 = m01 * m12 - m02 * m11;
+    const double c11 = m00 * m22 - m02 * m02, c12 = m01 * m02 - m00 * m12, c22 = m00 * m11 - m01 * m01;
+    const double det = m00 * c00 + m01 * c01 + m02 * c02;
+    const bool bad = !(det > 1e-12 * m00 * m11 * m22);
+    if (bad) atomicOr(err, ERR_SINGULAR);
+    const double id = 1.0 / det;
+    const double i00 = c00 * id, i01 = c01 * id, i02 = c02 * id, i11 = c11 * id, i12 = c12 * id, i22 = c22 * id;
+    // tr(M^-1 B)
+    const double tr = i00 * b00 + i11 * b11 + i22 * b22 + 2.0 * (i01 * b01 + i02 * b02 + i12 * b12);
+    double *o = out + (int64_t)e * out_stride + c;
+    const int64_t cs_ = out_stride / 4;
+    o[0] = bad ? CUDART_INF : -0.5 * tr;
+    if (want_grad) {
+        // X = M^-1 B M^-1: rows 1 (dust) and 2 (synchrotron) are all the gradient needs
+        const double y10 = i01 * b00 + i11 * b01 + i12 * b02, y11 = i01 * b01 + i11 * b11 + i12 * b12, y12 = i01 * b02 + i11 * b12 + i12 * b22;
+        const double y20 = i02 * b00 + i12 * b01 + i22 * b02, y21 = i02 * b01 + i12 * b11 + i22 * b12, y22 = i02 * b02 + i12 * b12 + i22 * b22;
+        const double x10 = y10 * i00 + y11 * i01 + y12 * i02, x11 = y10 * i01 + y11 * i11 + y12 * i12, x12 = y10 * i02 + y11 * i12 + y12 * i22;
+        const double x20 = y20 * i00 + y21 * i01 + y22 * i02, x21 = y20 * i01 + y21 * i11 + y22 * i12, x22 = y20 * i02 + y21 * i12 + y22 * i22;
+        o[cs_] = (x10 * p1[0] + x11 * p1[1] + x12 * p1[2]) - (i01 * v1[0] + i11 * v1[1] + i12 * v1[2]);
+        o[2 * cs_] = (x10 * p2[0] + x11 * p2[1] + x12 * p2[2]) - (i01 * v2[0] + i11 * v2[1] + i12 * v2[2]);
+        o[3 * cs_] = (x20 * p3[0] + x21 * p3[1] + x22 * p3[2]) - (i02 * v3[0] + i12 * v3[1] + i22 * v3[2]);
+    }
+}
+
+// Ordered sums of the per-cell terms onto clusters (grad) and regions (nll): thread = one output of one entry,
+// cells in ascending order.  grid = (ceil((ktot_max + nregion) / 128), batch), block = 128.
+__global__ void __launch_bounds__(128) k_cc_reduce(const CfgDev *__restrict__ cfgs, const CellsDev *__restrict__ cells,
+                                                   const int32_t *__restrict__ cfg_of, const int64_t *__restrict__ param_off,
+                                                   const double *__restrict__ out, int64_t out_stride, int32_t nregion,
+                                                   int32_t want_grad, double *__restrict__ nll, double *__restrict__ grad) {
+    const int e = blockIdx.y;
+    const CfgDev *cf = cfgs + cfg_of[e];
+    const CellsDev *cl = cells + cfg_of[e];
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    const double *o = out + (int64_t)e * out_stride;
+    const int64_t cs_ = out_stride / 4;
+    const int ktot = want_grad ? cf->ktot : 0;
+    int t, k;
+    if (v < ktot) {
+        if (v < cf->K[0]) { t = 0; k = v; }
+        else if (v < cf->K[0] + cf->K[1]) { t = 1; k = v - cf->K[0]; }
+        else { t = 2; k = v - cf->K[0] - cf->K[1]; }
+    } else if (v - ktot < nregion) {
+        t = 3; k = v - ktot;
+    } else {
+        return;
+    }
+    const double *src = o + (t == 3 ? 0 : (int64_t)(t + 1) * cs_);
+    double acc = 0.0;
+    for (int q = cl->kptr[t][k]; q < cl->kptr[t][k + 1]; ++q) acc += src[cl->klist[t][q]];
+    if (t == 3) nll[(int64_t)e * nregion + k] = acc;
+    else grad[param_off[e] + v] = acc;
+}
+
+}  // namespace cs

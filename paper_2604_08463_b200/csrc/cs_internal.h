@@ -31,7 +31,7 @@ constexpr int HALF = 256;      // a tile is staged as two halves of 256 position
 constexpr int SEG_MAX = 32;    // longest run of ranks summed as one segment
 constexpr int CHUNK_LEN = 8;   // ranks per chunk (SEG_MAX / CHUNK_LEN <= 4 chunks per segment)
 constexpr int NROW = 16;       // floats per table row (nfreq padded to 16 -> 64-byte rows)
-constexpr int CELL_CAP = 32;   // sorted layout: most cells per tile (one builder lane per cell)
+constexpr int CELL_CAP = 64;   // sorted layout: most cells per tile (a builder lane builds cells lane and lane + 32)
 constexpr int CROW = 100;      // floats per cell row in shared memory: 5 columns x 16 + 16 scalars + 4 pad (= 4 mod 32 banks)
 constexpr int SC_CHUNK_CAP = 4 * (TPX / CHUNK_LEN + CELL_CAP);   // sorted layout: most chunks of the four terms of a tile
 constexpr int SC_SEG_CAP = 4 * (TPX / SEG_MAX + CELL_CAP);       // and most segments

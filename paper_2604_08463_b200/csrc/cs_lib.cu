@@ -16,6 +16,7 @@
 #include "cs_like_sc.cuh"
 #include "cs_like_direct.cuh"
 #include "cs_optim.cuh"
+#include "cs_cells.cuh"
 
 using namespace cs;
 
@@ -54,6 +55,13 @@ struct SortedHost {
     int32_t *pospix = nullptr;
 };
 
+// Device arrays of one configuration's global cell list (f3; sorted configurations only).
+struct CellsHost {
+    int32_t *cellpos = nullptr, *celllen = nullptr, *cellreg = nullptr;
+    int32_t *kptr[4] = {nullptr, nullptr, nullptr, nullptr}, *klist[4] = {nullptr, nullptr, nullptr, nullptr};
+    int32_t ncell = 0;
+};
+
 template <typename T>
 int dev_upload(T **dst, const std::vector<T> &src, int64_t *bytes) {
     *dst = nullptr;
@@ -80,13 +88,16 @@ struct cs_ctx {
     bool have_ninv = false;
     // options (cs_set_option)
     int32_t opt_layout = CS_LAYOUT_AUTO, opt_form = CS_FORM_AUTO;
-    double opt_min_fill = 0.85;
+    double opt_min_fill = 0.45;
     int64_t opt_copy_limit = 0;         // bytes, 0 = 70 % of the free device memory when the batch is set
     // clusters
     int32_t nmap = 0, ncfg = 0, nregion = 1;
     std::vector<MapHost> maps;          // nmap pixel-space maps, the region pseudo-map, then 4 per sorted configuration
     std::vector<CfgDev> cfgs;
     std::vector<SortedHost> sorted;     // ncfg
+    std::vector<CellsHost> cellsh;      // ncfg
+    CellsDev *d_cells = nullptr;
+    int32_t ncell_max = 0;
     std::vector<int32_t> npix_live;     // [ncfg*nregion]
     MapDev *d_maps = nullptr;
     CfgDev *d_cfgs = nullptr;
@@ -123,6 +134,13 @@ struct cs_ctx {
     int64_t sel_cap = 0;
     cudaEvent_t sel_ev[SEL_RING] = {nullptr, nullptr, nullptr, nullptr};
     int64_t sel_n = 0;
+    // f3 workspace (cs_cell_moments)
+    double *d_mom = nullptr, *d_ccout = nullptr;
+    int64_t *d_mom_off = nullptr;
+    MomJob *d_momjobs = nullptr;
+    float *d_w = nullptr;
+    int64_t cc_bytes = 0, cc_out_stride = 0;
+    bool have_moments = false;
     // optimizer workspace
     OptWork opt;
     int64_t opt_bytes = 0;
@@ -157,6 +175,14 @@ void free_clusters(cs_ctx *c) {
     c->maps.clear();
     for (auto &p : c->sorted) { cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); cudaFree(p.pospix); }
     c->sorted.clear();
+    for (auto &p : c->cellsh) {
+        cudaFree(p.cellpos); cudaFree(p.celllen); cudaFree(p.cellreg);
+        for (int t = 0; t < 4; ++t) { cudaFree(p.kptr[t]); cudaFree(p.klist[t]); }
+    }
+    c->cellsh.clear();
+    cudaFree(c->d_cells);
+    c->d_cells = nullptr;
+    c->ncell_max = 0;
     cudaFree(c->d_maps); cudaFree(c->d_cfgs); cudaFree(c->d_npix_live);
     c->d_maps = nullptr; c->d_cfgs = nullptr; c->d_npix_live = nullptr;
     c->cfgs.clear();
@@ -182,6 +208,9 @@ void free_batch(cs_ctx *c) {
     cudaFree(c->d_hparams); cudaFree(c->d_hnll); cudaFree(c->d_hgrad); cudaFree(c->d_hruns);
     c->d_hparams = c->d_hnll = c->d_hgrad = nullptr; c->d_hruns = nullptr; c->hruns_cap = 0;
     c->hbuf_bytes = 0;
+    cudaFree(c->d_mom); cudaFree(c->d_ccout); cudaFree(c->d_mom_off); cudaFree(c->d_momjobs); cudaFree(c->d_w);
+    c->d_mom = c->d_ccout = nullptr; c->d_mom_off = nullptr; c->d_momjobs = nullptr; c->d_w = nullptr;
+    c->cc_bytes = 0; c->have_moments = false;
     if (c->h_sel) cudaFreeHost(c->h_sel);
     cudaFree(c->d_sel);
     c->h_sel = nullptr; c->d_sel = nullptr; c->sel_cap = 0;
@@ -270,6 +299,7 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, M
 // hold more than CELL_CAP cells.  Fills the position-space arrays; returns the fill fraction live / (ntile * TPX).
 struct SortedPlan {
     std::vector<int32_t> pospix, idx[4], cellptr, cellrows;
+    std::vector<int32_t> cellpos, celllen, cellkey[4];   // per tile-cell: first position, live + odd-pad positions, ids
     std::vector<uint8_t> cellid;
     int32_t ntile = 0;
     double fill = 0.0;
@@ -305,6 +335,8 @@ void plan_sorted(const int32_t *i0, const int32_t *i1, const int32_t *i2, const 
         return x.minp < y.minp;
     });
     sp.pospix.clear(); sp.cellid.clear(); sp.cellptr.assign(1, 0); sp.cellrows.clear();
+    sp.cellpos.clear(); sp.celllen.clear();
+    for (int t = 0; t < 4; ++t) sp.cellkey[t].clear();
     for (int t = 0; t < 4; ++t) sp.idx[t].clear();
     int pos = 0, ncell = 0;   // inside the current tile
     Px last{0, 0, 0, 0, -1};
@@ -329,6 +361,8 @@ void plan_sorted(const int32_t *i0, const int32_t *i1, const int32_t *i2, const 
             ++ncell;
             sp.cellrows.push_back(q0.a); sp.cellrows.push_back(K[0] + q0.b); sp.cellrows.push_back(K[0] + K[1] + q0.b);
             sp.cellrows.push_back(K[0] + 2 * K[1] + q0.c);
+            sp.cellpos.push_back((int32_t)sp.pospix.size()); sp.celllen.push_back(take);
+            sp.cellkey[0].push_back(q0.a); sp.cellkey[1].push_back(q0.b); sp.cellkey[2].push_back(q0.c); sp.cellkey[3].push_back(q0.r);
             last = q0;
             for (int32_t j = 0; j < take; ++j) {
                 const int32_t src = done + j;
@@ -340,6 +374,8 @@ void plan_sorted(const int32_t *i0, const int32_t *i1, const int32_t *i2, const 
     if (pos > 0 || sp.cellptr.size() == 1) {
         if (ncell == 0) {   // no live pixel at all: one dummy cell reading the first table rows, all pads
             sp.cellrows.push_back(0); sp.cellrows.push_back(K[0]); sp.cellrows.push_back(K[0] + K[1]); sp.cellrows.push_back(K[0] + 2 * K[1]);
+            sp.cellpos.push_back((int32_t)sp.pospix.size()); sp.celllen.push_back(0);
+            for (int t = 0; t < 4; ++t) sp.cellkey[t].push_back(0);
             ncell = 1;
             last = Px{0, 0, 0, 0, -1};
         }
@@ -502,6 +538,7 @@ int set_data_impl(cs_ctx *c, int32_t ndata, const float *d, const float *ninv, b
     c->d = d;
     c->ndata = ndata;
     c->have_ninv = true;
+    c->have_moments = false;   // f3 moments belong to the previous data
     c->tmap = tm;
     c->have_tmap = have;
     if (do_relayout && c->batch > 0 && !c->jobs.empty()) {
@@ -666,6 +703,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     c->nmap = nmap; c->ncfg = ncfg; c->nregion = nregion;
     c->cfgs.resize(ncfg);
     c->sorted.resize(ncfg);
+    c->cellsh.resize(ncfg);
     c->npix_live.assign((size_t)ncfg * nregion, 0);
     SortedPlan sp;
     for (int32_t i = 0; i < ncfg; ++i) {
@@ -702,6 +740,28 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
                     }
                     cf.map[t] = (int32_t)c->maps.size() - 1;
                 }
+                {   // global cell list for the cell-compressed likelihood (f3)
+                    CellsHost &ch = c->cellsh[i];
+                    ch.ncell = (int32_t)sp.cellpos.size();
+                    c->ncell_max = std::max(c->ncell_max, ch.ncell);
+                    if ((rc = dev_upload(&ch.cellpos, sp.cellpos, &c->cluster_bytes)) || (rc = dev_upload(&ch.celllen, sp.celllen, &c->cluster_bytes)) ||
+                        (rc = dev_upload(&ch.cellreg, sp.cellkey[3], &c->cluster_bytes))) {
+                        free_clusters(c);
+                        return rc;
+                    }
+                    for (int t = 0; t < 4; ++t) {
+                        const int32_t Kt = t < 3 ? cf.K[t] : nregion;
+                        std::vector<int32_t> kp(Kt + 1, 0), kl(ch.ncell);
+                        for (int32_t q = 0; q < ch.ncell; ++q) kp[sp.cellkey[t][q] + 1]++;
+                        for (int32_t k = 0; k < Kt; ++k) kp[k + 1] += kp[k];
+                        std::vector<int32_t> fill(kp.begin(), kp.end() - 1);
+                        for (int32_t q = 0; q < ch.ncell; ++q) kl[fill[sp.cellkey[t][q]]++] = q;
+                        if ((rc = dev_upload(&ch.kptr[t], kp, &c->cluster_bytes)) || (rc = dev_upload(&ch.klist[t], kl, &c->cluster_bytes))) {
+                            free_clusters(c);
+                            return rc;
+                        }
+                    }
+                }
                 cf.sorted = 1;
                 cf.ntile = sp.ntile;
                 cf.cellid = sh.cellid; cf.cellptr = sh.cellptr; cf.cellrows = sh.cellrows; cf.pospix = sh.pospix;
@@ -718,7 +778,16 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
         const MapHost &s = c->maps[m];
         md[m] = MapDev{s.idx, s.rank, s.segptr, s.segdesc, s.segslot, s.ksegptr, s.chunkptr, s.segcfirst, s.K, s.nseg};
     }
+    std::vector<CellsDev> cd(ncfg);
+    for (int32_t i = 0; i < ncfg; ++i) {
+        const CellsHost &ch = c->cellsh[i];
+        std::memset(&cd[i], 0, sizeof(CellsDev));
+        cd[i].cellpos = ch.cellpos; cd[i].celllen = ch.celllen; cd[i].cellrows = c->sorted[i].cellrows; cd[i].cellreg = ch.cellreg;
+        for (int t = 0; t < 4; ++t) { cd[i].kptr[t] = ch.kptr[t]; cd[i].klist[t] = ch.klist[t]; }
+        cd[i].ncell = ch.ncell;
+    }
     if ((rc = dev_upload(&c->d_maps, md, &c->cluster_bytes)) || (rc = dev_upload(&c->d_cfgs, c->cfgs, &c->cluster_bytes)) ||
+        (rc = dev_upload(&c->d_cells, cd, &c->cluster_bytes)) ||
         (rc = dev_upload(&c->d_npix_live, c->npix_live, &c->cluster_bytes))) {
         free_clusters(c);
         return rc;
@@ -955,6 +1024,69 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
     P.ring_maps = 1;
     P.evict_first = ((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4 > (int64_t)96 << 20) ? 1 : 0;
     return launch_like<MODE_MAPS>(c, P, reinterpret_cast<const Run *>(ds + roff), 0, 0, nrun, W, st);
+}
+
+int cs_cell_moments(cs_ctx *c, void *stream) {
+    int rc = ready(c);
+    if (rc) return rc;
+    if (c->nfreq > CC_MAXF) return CS_EINVAL;
+    for (int32_t e = 0; e < c->batch; ++e)
+        if (!c->cfgs[c->cfg_of[e]].sorted) return CS_EINVAL;   // f3 needs the cell list of the sorted layout
+    CS_GUARD_BEGIN
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!c->d_mom) {   // workspace: moments of every (configuration, data set) pair, per-cell terms, offsets
+        std::vector<MomJob> mj(c->jobs.size());
+        std::map<std::pair<int32_t, int32_t>, int64_t> off;
+        int64_t n = 0;
+        for (size_t j = 0; j < c->jobs.size(); ++j) {
+            mj[j] = MomJob{c->jobs[j].cfg, c->jobs[j].data, n};
+            off[std::make_pair(c->jobs[j].data, c->jobs[j].cfg)] = n;
+            n += (int64_t)CC_NMOM * c->cellsh[c->jobs[j].cfg].ncell;
+        }
+        std::vector<int64_t> mo(c->batch);
+        for (int32_t e = 0; e < c->batch; ++e) mo[e] = off[std::make_pair(c->data_of[e], c->cfg_of[e])];
+        c->cc_out_stride = 4 * (int64_t)((c->ncell_max + 31) & ~31);
+        const size_t out_bytes = (size_t)c->batch * c->cc_out_stride * sizeof(double);
+        int64_t b = 0;
+        if ((rc = dev_upload(&c->d_momjobs, mj, &b)) || (rc = dev_upload(&c->d_mom_off, mo, &b))) return rc;
+        if (cudaMalloc((void **)&c->d_mom, (size_t)std::max<int64_t>(n, 1) * sizeof(double)) != cudaSuccess ||
+            cudaMalloc((void **)&c->d_ccout, out_bytes) != cudaSuccess || cudaMalloc((void **)&c->d_w, NROW * sizeof(float)) != cudaSuccess) {
+            cudaGetLastError();
+            return CS_ENOMEM;
+        }
+        c->cc_bytes = b + n * (int64_t)sizeof(double) + (int64_t)out_bytes + NROW * 4;
+        c->batch_bytes += c->cc_bytes;
+    }
+    CK(cudaMemcpyAsync(c->d_w, c->kc.w, NROW * sizeof(float), cudaMemcpyHostToDevice, st));
+    for (size_t j = 0; j < c->jobs.size(); j += 65535) {
+        const int nj = (int)std::min<size_t>(65535, c->jobs.size() - j);
+        dim3 grid((c->ncell_max + 3) / 4, nj);
+        k_cc_moments<<<grid, 128, 0, st>>>(c->d, c->npix, c->nfreq, c->d_cfgs, c->d_cells, c->d_momjobs + j, c->d_w, c->d_mom);
+        c->launches++;
+    }
+    CK(cudaGetLastError());
+    c->have_moments = true;
+    return CS_OK;
+    CS_GUARD_END
+}
+
+int cs_spectral_like_grad_cells(cs_ctx *c, double *nll, double *grad, void *stream) {
+    int rc = ready(c);
+    if (rc) return rc;
+    if (!nll || !c->tables_built || !c->have_moments) return CS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int e0 = 0; e0 < c->batch; e0 += 65535) {
+        const int nb = std::min(65535, c->batch - e0);
+        dim3 g1((c->ncell_max + 127) / 128, nb);
+        k_like_cc<<<g1, 128, 0, st>>>(c->d_cfgs, c->d_cells, c->d_cfg_of + e0, c->d_mom_off + e0, c->d_tab_off + e0, c->d_tab, c->d_mom, c->kc,
+                                      c->nfreq, grad ? 1 : 0, c->d_ccout + (int64_t)e0 * c->cc_out_stride, c->cc_out_stride, c->d_err);
+        dim3 g2(((grad ? c->ktot_max : 0) + c->nregion + 127) / 128, nb);
+        k_cc_reduce<<<g2, 128, 0, st>>>(c->d_cfgs, c->d_cells, c->d_cfg_of + e0, c->d_param_off + e0, c->d_ccout + (int64_t)e0 * c->cc_out_stride,
+                                        c->cc_out_stride, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad);
+        c->launches += 2;
+    }
+    CK(cudaGetLastError());
+    return CS_OK;
 }
 
 int cs_cmb_variance(cs_ctx *c, double *var, void *stream) {

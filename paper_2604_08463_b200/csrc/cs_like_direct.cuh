@@ -18,13 +18,14 @@
 
 namespace cs {
 
-constexpr int DR_ND = 3;                 // data ring depth (2 for the generic band count)
+constexpr int DR_ND = 2;                 // data ring depth (deeper adds nothing, cs_like_sc.cuh; the rest of the SM's
+                                         // 228 KB stays L1, which the table rows of the next entry are prefetched into)
 constexpr int DR_EC = 2;                 // entries buffered between reduce phases
 constexpr int DR_THREADS = NCONS + 32;   // 288
 constexpr int TROW = TPX + 4;            // floats per term row: TPX ranks + a dump slot for positions without a rank
 
 template <int NF>
-struct DirectDepth { static constexpr int value = (NF == 15) ? DR_ND : 2; };
+struct DirectDepth { static constexpr int value = DR_ND; };
 
 template <int NF>
 constexpr size_t direct_smem_bytes() {
@@ -133,6 +134,11 @@ __global__ void __launch_bounds__(DR_THREADS, 1) k_like_direct(const __grid_cons
             const int sd = n % ND;
             const float *tb = P.tab + __ldg(&P.pinfo[w.run.estart + k].tab_row) * NROW;
             const float *st = st0 + sd * STAGE;
+            if (k + 1 < w.kend) {   // the next entry's rows on their way to L1 while this entry is computed
+                const float *tn = P.tab + __ldg(&P.pinfo[w.run.estart + k + 1].tab_row) * NROW;
+                if (liveA) { prefetch_row(tn + rA_fd); prefetch_row(tn + rA_g); prefetch_row(tn + rA_fs); if (kGrad) prefetch_row(tn + rA_dg); }
+                if (liveB) { prefetch_row(tn + rB_fd); prefetch_row(tn + rB_g); prefetch_row(tn + rB_fs); if (kGrad) prefetch_row(tn + rB_dg); }
+            }
             mbar_wait(&full_d[sd], (uint32_t)((n / ND) & 1));
             const float4 *aFd = reinterpret_cast<const float4 *>(tb + rA_fd), *aG = reinterpret_cast<const float4 *>(tb + rA_g);
             const float4 *adG = reinterpret_cast<const float4 *>(tb + rA_dg), *aFs = reinterpret_cast<const float4 *>(tb + rA_fs);

@@ -16,15 +16,16 @@
 // scalar (broadcast operand form), data read as one LDS.64 per band and Stokes parameter.
 //
 // Persistent grid: one CTA per SM, each walking a contiguous, equal share of all (tile, entry) units (cs_pipe.cuh).
-// CTA = 13 warps (128 registers per thread), warp-specialised; every hand-over is an mbarrier full/empty pair or a hardware named barrier, no
+// CTA = 14 warps (128 registers per thread), warp-specialised; every hand-over is an mbarrier full/empty pair or a hardware named barrier, no
 // CTA-wide barrier after the prologue:
 //   warps 0-7    consumers: positions (2t, 2t+1) of the 512-position tile per thread, one entry after the other
 //   warps 8-9    reducers : first level of the ordered fp64 reduction (a3) of the pair sums the consumers leave behind;
 //                           warp r owns term-ring slot r and the entries n = r (mod 2)
-//   warps 10-11  builders : lane c builds cell c of the tile (five weighted columns, LDL^T, P); warp b owns cell-table
-//                           slot b and the entries n = b (mod 2).  Two of them, because under a saturated HBM stream the
-//                           L2 round trip of a cell's four table rows takes about as long as a whole entry
-//   warp  12     loader   : one 60-KB bulk copy per entry into the data ring (two stages: measured, a deeper ring
+//   warps 10-12  builders : lane c builds the cells c and c + 32 of the tile (five weighted columns, LDL^T, P); warp b
+//                           owns cell-table slot b and the entries n = b (mod 3).  Three of them, and each prefetches the
+//                           rows of its next entry to L1, because under a saturated HBM stream the L2 round trip of a
+//                           cell's four table rows takes about as long as a whole entry
+//   warp  13     loader   : one 60-KB bulk copy per entry into the data ring (two stages: measured, a deeper ring
 //                           adds nothing once the consumers release a stage as soon as it is read)
 // shared memory: data ring [ND][2 halves][2*NF][256] | cell tables [NC][CELL_CAP][CROW] | term ring [NT][4][256] fp64 |
 //                reducer plans | barriers
@@ -38,15 +39,15 @@ namespace cs {
 #define CS_SC_ND 2
 #endif
 #ifndef CS_SC_NBW
-#define CS_SC_NBW 2
+#define CS_SC_NBW 3
 #endif
 constexpr int SC_ND = CS_SC_ND; // data ring depth 
 template <int NF>
 struct ScDepth { static constexpr int value = SC_ND; };
-constexpr int SC_NC = 2;        // cell-table ring depth
+constexpr int SC_NC = CS_SC_NBW; // cell-table ring depth = builder warps
 constexpr int SC_NBW = CS_SC_NBW; // builder warps (warp b takes the entries n = b mod SC_NBW; SC_NC is a multiple of it)
 constexpr int SC_NT = 2;        // term ring depth = reducer warps
-constexpr int SC_THREADS = NCONS + (SC_NT + SC_NBW + 1) * 32;   // 416
+constexpr int SC_THREADS = NCONS + (SC_NT + SC_NBW + 1) * 32;   // 448
 constexpr int SC_WARP_RED = NCONS / 32, SC_WARP_BUILD = SC_WARP_RED + SC_NT, SC_WARP_LOAD = SC_WARP_BUILD + SC_NBW;
 constexpr int SC_PLAN_BYTES = SC_CHUNK_CAP * 2 + SC_SEG_CAP * 2 + SC_SEG_CAP * 4 + 16;   // one reducer warp's plan
 
@@ -216,33 +217,54 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
     int n = 0;   // live entries so far (ring slots and barrier phases follow it)
 
     if (warp >= SC_WARP_BUILD) {
-        // ---------------- builder warps: lane c builds cell c of the current tile; warp b takes the entries n = b (mod SC_NBW)
+        // ---------------- builder warps: lane c builds the cells c and c + 32 of the current tile; warp b takes the
+        // entries n = b (mod SC_NBW)
+        static_assert(CELL_CAP == 64, "two cells per builder lane");
         const int mine = warp - SC_WARP_BUILD;
         while (walk_next(w, P)) {
             const CfgDev *cf = P.cfgs + w.run.cfg;
             const int c0 = __ldg(cf->cellptr + w.tile), ncell = __ldg(cf->cellptr + w.tile + 1) - c0;
-            int4 rows = make_int4(0, 0, 0, 0);
-            if (lane < ncell) rows = __ldg(reinterpret_cast<const int4 *>(cf->cellrows) + c0 + lane);
+            const int4 rows0 = (lane < ncell) ? __ldg(reinterpret_cast<const int4 *>(cf->cellrows) + c0 + lane) : make_int4(0, 0, 0, 0);
+            const int4 rows1 = (lane + 32 < ncell) ? __ldg(reinterpret_cast<const int4 *>(cf->cellrows) + c0 + lane + 32) : make_int4(0, 0, 0, 0);
             for (int k = w.k; k < w.kend; ++k) {
                 const int64_t tab_row = __ldg(&P.pinfo[w.run.estart + k].tab_row);
                 if (P.skip && __ldg(P.skip + __ldg(P.elist + w.run.estart + k)) != 0) continue;
                 const int s = n % NC;
                 if (SC_NBW > 1 && n % SC_NBW != mine) { ++n; continue; }
-                float4 Fd[4], G[4], dG[4], Fs[4];
-                if (lane < ncell) {
-                    const float *tb = P.tab + tab_row * NROW;
-                    const float4 *rFd = reinterpret_cast<const float4 *>(tb + (int64_t)rows.x * NROW);
-                    const float4 *rG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.y * NROW);
-                    const float4 *rdG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.z * NROW);
-                    const float4 *rFs = reinterpret_cast<const float4 *>(tb + (int64_t)rows.w * NROW);
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        Fd[q] = __ldg(rFd + q); G[q] = __ldg(rG + q); Fs[q] = __ldg(rFs + q);
-                        dG[q] = kGrad ? __ldg(rdG + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+                const float *tb = P.tab + tab_row * NROW;
+                const int nh = ncell > 32 ? 2 : 1;   // warp-uniform: most tiles hold fewer than 32 cells
+                if (k + SC_NBW < w.kend) {   // this warp's next entry: its rows on their way to L1
+                    const float *tn = P.tab + __ldg(&P.pinfo[w.run.estart + k + SC_NBW].tab_row) * NROW;
+                    if (lane < ncell) {
+                        prefetch_row(tn + (int64_t)rows0.x * NROW); prefetch_row(tn + (int64_t)rows0.y * NROW);
+                        prefetch_row(tn + (int64_t)rows0.w * NROW);
+                        if (kGrad) prefetch_row(tn + (int64_t)rows0.z * NROW);
+                    }
+                    if (lane + 32 < ncell) {
+                        prefetch_row(tn + (int64_t)rows1.x * NROW); prefetch_row(tn + (int64_t)rows1.y * NROW);
+                        prefetch_row(tn + (int64_t)rows1.w * NROW);
+                        if (kGrad) prefetch_row(tn + (int64_t)rows1.z * NROW);
                     }
                 }
-                mbar_wait(&empty_c[s], (uint32_t)(((n / NC) & 1) ^ 1));
-                if (lane < ncell) sc_build_cell<NF, kGrad>(Fd, G, dG, Fs, P.kc, cells + (s * CELL_CAP + lane) * CROW, P.err);
+#pragma unroll 1
+                for (int h = 0; h < nh; ++h) {
+                    const int4 rows = h ? rows1 : rows0;
+                    const int c = lane + 32 * h;
+                    float4 Fd[4], G[4], dG[4], Fs[4];
+                    if (c < ncell) {
+                        const float4 *rFd = reinterpret_cast<const float4 *>(tb + (int64_t)rows.x * NROW);
+                        const float4 *rG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.y * NROW);
+                        const float4 *rdG = reinterpret_cast<const float4 *>(tb + (int64_t)rows.z * NROW);
+                        const float4 *rFs = reinterpret_cast<const float4 *>(tb + (int64_t)rows.w * NROW);
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            Fd[q] = __ldg(rFd + q); G[q] = __ldg(rG + q); Fs[q] = __ldg(rFs + q);
+                            dG[q] = kGrad ? __ldg(rdG + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+                        }
+                    }
+                    if (h == 0) mbar_wait(&empty_c[s], (uint32_t)(((n / NC) & 1) ^ 1));
+                    if (c < ncell) sc_build_cell<NF, kGrad>(Fd, G, dG, Fs, P.kc, cells + (s * CELL_CAP + c) * CROW, P.err);
+                }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&full_c[s]);
                 ++n;

@@ -616,16 +616,22 @@ def test_kernel_forms_agree_bit_for_bit(torch_cuda):
 
 def test_default_layout_choice_mixes_both_kernels(torch_cuda):
     """Library defaults (CS_LAYOUT_AUTO): configurations whose sorted tiles fill well stream private sorted copies
-    through the sorted-cell kernel, the others stay in place on the direct kernel -- both in one batch."""
-    w = gen.make_config(2, batch=24)     # K from (10,1,1) to (1000,500,500) on one shared data set
+    through the sorted-cell kernel; one whose cells are single pixels (K = npix for beta_d, the paper's own optimum,
+    Table 2) would mostly stream padding and stays in place on the direct kernel -- both in one batch."""
+    w = gen.make_config(2, batch=6)     # six configurations of the scan on one shared data set
+    nmap, ncfg = w.maps.shape[0], w.cfg_maps.shape[0]
+    maps = np.concatenate([w.maps, np.arange(w.npix, dtype=np.int32)[None]])
+    cfg_maps = np.concatenate([w.cfg_maps, [[nmap, w.cfg_maps[0][1], w.cfg_maps[0][2]]]]).astype(np.int32)
+    w = dataclasses.replace(w, maps=maps, Kmap=np.concatenate([w.Kmap, [w.npix]]).astype(np.int32), cfg_maps=cfg_maps,
+                            cfg_of=np.concatenate([w.cfg_of, [ncfg, ncfg]]).astype(np.int32),
+                            data_of=np.concatenate([w.data_of, [0, 0]]).astype(np.int32))
     ctx, _ = make_ctx(w, options={})
-    kinds = {ctx.layout_info(c)[0] for c in range(w.cfg_maps.shape[0])}
+    kinds = [ctx.layout_info(c)[0] for c in range(w.cfg_maps.shape[0])]
     ctx.close()
-    assert kinds == {True, False}
-    helpers_opts = helpers.CTX_OPTIONS
-    assert helpers_opts == {}
+    assert kinds == [True] * ncfg + [False]
+    assert helpers.CTX_OPTIONS == {}
     _parity(w, w.params_jittered(seed=26), maps=False)
-    _parity(w, w.params_jittered(seed=26), entries=[0, 11, 23])
+    _parity(w, w.params_jittered(seed=26), entries=[0, 5, 7])
 
 
 def test_full_size_c3_scan_sampled(torch_cuda):
@@ -633,3 +639,99 @@ def test_full_size_c3_scan_sampled(torch_cuda):
     w = gen.make_config(2)
     assert w.batch == 1024 and w.maps.shape[0] == 32
     _sampled_full_size(w, w.params_jittered(seed=19), 10, 25)
+
+
+# ----------------------------------------------------------------------------- f3: cell-compressed likelihood
+
+def _cells_eval(ctx, params, want_grad=True):
+    import torch
+    p = torch.from_numpy(np.ascontiguousarray(params, dtype=np.float64)).cuda()
+    nll = torch.full((ctx.batch * ctx.nregion,), float("nan"), dtype=torch.float64, device="cuda")
+    grad = torch.full_like(p, float("nan")) if want_grad else None
+    ctx.build_sed_tables(p)
+    ctx.spectral_like_grad_cells(nll, grad)
+    torch.cuda.synchronize()
+    return nll.cpu().numpy().reshape(ctx.batch, ctx.nregion), (grad.cpu().numpy() if want_grad else None)
+
+
+def _cells_parity(w, params, entries=None):
+    """cs_cell_moments + cs_spectral_like_grad_cells against the oracle (T1, T2) and against the per-pixel path."""
+    import paper_2604_08463_b200 as cs
+    ctx, _ = make_ctx(w, options={"layout": cs.LAYOUT_SORTED})
+    ctx.cell_moments()
+    nll, grad = _cells_eval(ctx, params)
+    assert ctx.check() == 0
+    nll_v, _ = _cells_eval(ctx, params, want_grad=False)
+    assert np.array_equal(nll_v, nll)
+    nll_pp, grad_pp = gpu_eval(ctx, params)
+    assert np.all(np.abs(nll - nll_pp) <= 1e-6 * np.abs(nll_pp))
+    off = w.param_offsets()
+    for e in (range(w.batch) if entries is None else entries):
+        ref = oracle_entry(w, params, e)
+        assert ref["rc"] == 0
+        check_T1(nll[e], ref["nll"])
+        check_T2(grad[off[e]:off[e + 1]], ref, w.K_of_cfg(int(w.cfg_of[e])))
+    ctx.close()
+
+
+def test_cells_c1_and_c2(torch_cuda):
+    w = gen.make_config(0)
+    _cells_parity(w, w.params_jittered(seed=1))
+    _cells_parity(w, w.params_const())
+    w = gen.make_config(1)
+    _cells_parity(w, w.params_jittered(seed=2))
+
+
+def test_cells_clustering_scan_subset(torch_cuda):
+    """The workload f3 is for: many configurations (K from (10,1,1) to (1000,500,500)) on one shared data set."""
+    w = gen.make_config(2, batch=24)
+    _cells_parity(w, w.params_jittered(seed=3))
+
+
+def test_cells_regions_masks_and_several_data_sets(torch_cuda):
+    w = _masked(gen.make_config(3, nside=32, batch=12, ndata=3))
+    _cells_parity(w, w.params_jittered(seed=4))
+
+
+def test_cells_moments_follow_the_data(torch_cuda):
+    """cs_set_data invalidates the moments (CS_EINVAL until cs_cell_moments is called again); Ninv -> 4 Ninv scales
+    nll and grad by 4 exactly (powers of two go through every product unchanged)."""
+    import torch
+    import paper_2604_08463_b200 as cs
+    w = gen.make_config(0)
+    params = w.params_jittered(seed=13)
+    ctx, d = make_ctx(w, options={"layout": cs.LAYOUT_SORTED})
+    ctx.cell_moments()
+    nll, grad = _cells_eval(ctx, params)
+    ctx.set_data(d, (4.0 * w.ninv).astype(np.float32))
+    with pytest.raises(cs.CsError) as ei:
+        _cells_eval(ctx, params)
+    assert ei.value.code == cs.EINVAL
+    ctx.cell_moments()
+    nll4, grad4 = _cells_eval(ctx, params)
+    assert np.array_equal(nll4, 4.0 * nll) and np.array_equal(grad4, 4.0 * grad)
+    ctx.close()
+    # an in-place configuration has no cell list
+    ctx, _ = make_ctx(w, options={"layout": cs.LAYOUT_INPLACE})
+    with pytest.raises(cs.CsError) as ei:
+        ctx.cell_moments()
+    assert ei.value.code == cs.EINVAL
+    ctx.close()
+
+
+def test_cells_full_size_c3_scan_sampled(torch_cuda):
+    """configs[2] at full size through f3: 1024 configurations on one shared data set, a seeded sample against the oracle."""
+    w = gen.make_config(2)
+    params = w.params_jittered(seed=19)
+    ctx, _ = make_ctx(w)
+    assert all(ctx.layout_info(c)[0] for c in range(0, 1024, 37))
+    ctx.cell_moments()
+    nll, grad = _cells_eval(ctx, params)
+    assert ctx.check() == 0 and np.isfinite(nll).all() and np.isfinite(grad).all()
+    off = w.param_offsets()
+    data = w.data()
+    for e in sorted(set(gen.rng_for("misc", 31).integers(0, w.batch, 10).tolist()) | {0, w.batch - 1}):
+        ref = oracle_entry(w, params, e, data=data)
+        check_T1(nll[e], ref["nll"])
+        check_T2(grad[off[e]:off[e + 1]], ref, w.K_of_cfg(int(w.cfg_of[e])))
+    ctx.close()
