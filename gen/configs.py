@@ -42,6 +42,33 @@ def cluster_map(vecs: np.ndarray, param: int, K: int, region_idx=None, nregion: 
     return lab, off
 
 
+def irregular_mask(vecs: np.ndarray, seed: int = 0, ndisc: int = 40, frac_pix: float = 0.03) -> np.ndarray:
+    """bool [npix], True = masked: a Planck-like irregular mask made of a band of random width along the equator
+    ("Galactic plane" with a ragged edge), `ndisc` point-source discs of random radius (0.5 .. 6 degrees) and isolated
+    random pixels.  Stands in for the Planck GAL / point-source masks, which are not available
+    here; its purpose is a mask with no structure in RING order."""
+    g = sky.rng_for("mask", seed)
+    npix = vecs.shape[0]
+    lon = np.arctan2(vecs[:, 1], vecs[:, 0])
+    edge = np.deg2rad(8.0 + 6.0 * np.sin(3.0 * lon + g.uniform(0, 2 * np.pi)) + 3.0 * np.sin(11.0 * lon + g.uniform(0, 2 * np.pi)))
+    m = np.abs(np.arcsin(vecs[:, 2])) < edge
+    centres = g.standard_normal((ndisc, 3))
+    centres /= np.linalg.norm(centres, axis=1, keepdims=True)
+    radii = np.deg2rad(g.uniform(0.5, 6.0, ndisc))
+    for c, r in zip(centres, radii):
+        m |= vecs @ c > np.cos(r)
+    m |= g.random(npix) < frac_pix
+    return m
+
+
+def multires_maps(nside: int, nside_patch=(16, 4, 8)):
+    """Multi-resolution super-pixel patches (Table 3): one NESTED super-pixel map per spectral
+    parameter.  Returns (maps int32 [3, npix], K [3])."""
+    from .healpix import superpixel_map_ring
+    maps = np.stack([superpixel_map_ring(nside, min(int(n), nside)) for n in nside_patch])
+    return np.ascontiguousarray(maps.astype(np.int32)), [12 * min(int(n), nside) ** 2 for n in nside_patch]
+
+
 def c3_grid(seed: int = 3) -> np.ndarray:
     """The 16 x 8 x 8 = 1024 clustering grid of configs[2], in a seeded shuffled order; rows (K_bd, K_Td, K_bs)."""
     kbd = [int(round(10 ** (1 + 2 * i / 15))) for i in range(16)]
@@ -125,14 +152,16 @@ def _base(nside: int):
 
 
 def make_config(idx: int, *, nside=None, batch=None, ndata=None, K=None, noiseless=False,
-                cluster_truth=False, sky_seed: int = 1) -> Workload:
+                cluster_truth=False, sky_seed: int = 1, multires=None, holes=None) -> Workload:
     """BASELINE.json configs[idx] (idx 0..4), optionally scaled down (nside / batch / ndata) for tests.
 
     0: tiny sky nside 8, K=(4,2,3).   1: nside 64, K=(500,50,100), one entry.
     2: nside 64 clustering scan, 1024 configurations from 32 distinct maps, one shared noise realisation.
     3: nside 64, 3 latitude regions, 64 configurations x 100 noise realisations.
     4: nside 128, K=(2000,200,400), 256 noise realisations (batch sweep {1,16,64,256} = prefixes).
-    `cluster_truth=True` makes the truth constant per cluster of configuration 0."""
+    `cluster_truth=True` makes the truth constant per cluster of configuration 0.
+    `multires=(n0, n1, n2)` (configs 0, 1, 4) replaces the K-means maps by NESTED super-pixel maps at those resolutions
+    (Table 3); `holes=seed` masks an irregular, Planck-like set of pixels (-1 in all three maps)."""
     defaults = {0: (8, (4, 2, 3)), 1: (64, (500, 50, 100)), 2: (64, None), 3: (64, None), 4: (128, (2000, 200, 400))}
     nside = nside or defaults[idx][0]
     K = K or defaults[idx][1]
@@ -140,9 +169,13 @@ def make_config(idx: int, *, nside=None, batch=None, ndata=None, K=None, noisele
     region_idx, nregion = None, 1
     if idx in (0, 1, 4):
         maps, Kmap = [], []
-        for prm in range(3):
-            m, kt = cluster_map(vecs, prm, int(K[prm]))
-            maps.append(m); Kmap.append(kt)
+        if multires is not None:
+            mm, Kmap = multires_maps(nside, multires)
+            maps = [mm[0], mm[1], mm[2]]
+        else:
+            for prm in range(3):
+                m, kt = cluster_map(vecs, prm, int(K[prm]))
+                maps.append(m); Kmap.append(kt)
         cfg_maps = np.array([[0, 1, 2]], dtype=np.int32)
         nd = ndata or (256 if idx == 4 else 1)
         B = batch or nd
@@ -183,6 +216,8 @@ def make_config(idx: int, *, nside=None, batch=None, ndata=None, K=None, noisele
             name = "C4"
     maps = np.ascontiguousarray(np.stack(maps).astype(np.int32))
     Kmap = np.array(Kmap, dtype=np.int32)
+    if holes is not None:
+        maps[:, irregular_mask(vecs, int(holes))] = -1
     if cluster_truth:
         tm = maps[cfg_maps[0]]
         truth = sky.draw_truth(npix, sky_seed, tm, [int(Kmap[m]) for m in cfg_maps[0]])

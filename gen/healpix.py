@@ -60,3 +60,52 @@ def pix2vec_ring(nside: int) -> np.ndarray:
     z, phi = pix2zphi_ring(nside)
     st = np.sqrt(np.maximum(0.0, 1.0 - z * z))
     return np.stack([st * np.cos(phi), st * np.sin(phi), z], axis=1)
+
+
+def zphi2pix_nest(nside: int, z: np.ndarray, phi: np.ndarray) -> np.ndarray:
+    """NESTED pixel index at resolution `nside` of the directions (z, phi), restated from the published scheme
+    (Gorski et al. 2005): the sphere is twelve base faces, each an nside x nside grid whose cell (ix, iy) has the index
+    face * nside^2 + bit-interleave(ix, iy).  Used to build multi-resolution super-pixel patches (Table 3,
+    L328-L334): the NESTED index at a coarse nside is a partition into compact equal-area patches."""
+    n = int(nside)
+    assert n >= 1 and (n & (n - 1)) == 0, "NESTED needs a power-of-two nside"
+    z = np.asarray(z, dtype=np.float64)
+    za = np.abs(z)
+    tt = np.mod(np.asarray(phi, dtype=np.float64), 2.0 * np.pi) / (0.5 * np.pi)      # [0, 4)
+    face = np.empty(z.shape, dtype=np.int64)
+    ix = np.empty(z.shape, dtype=np.int64)
+    iy = np.empty(z.shape, dtype=np.int64)
+    eq = za <= 2.0 / 3.0
+    # equatorial belt
+    t1 = n * (0.5 + tt[eq])
+    t2 = n * z[eq] * 0.75
+    jp = np.floor(t1 - t2).astype(np.int64)         # ascending edge line
+    jm = np.floor(t1 + t2).astype(np.int64)         # descending edge line
+    ifp, ifm = jp // n, jm // n
+    face[eq] = np.where(ifp == ifm, (ifp & 3) + 4, np.where(ifp < ifm, ifp & 3, (ifm & 3) + 8))
+    ix[eq] = jm & (n - 1)
+    iy[eq] = n - (jp & (n - 1)) - 1
+    # polar caps
+    po = ~eq
+    ntt = np.minimum(3, np.floor(tt[po]).astype(np.int64))
+    tp = tt[po] - ntt
+    tmp = n * np.sqrt(3.0 * (1.0 - za[po]))
+    jp = np.minimum(n - 1, np.floor(tp * tmp).astype(np.int64))
+    jm = np.minimum(n - 1, np.floor((1.0 - tp) * tmp).astype(np.int64))
+    north = z[po] >= 0
+    face[po] = np.where(north, ntt, ntt + 8)
+    ix[po] = np.where(north, n - jm - 1, jp)
+    iy[po] = np.where(north, n - jp - 1, jm)
+    # interleave the bits of ix (even positions) and iy (odd positions)
+    idx = np.zeros(z.shape, dtype=np.int64)
+    for b in range(max(1, n.bit_length() - 1)):
+        idx |= ((ix >> b) & 1) << (2 * b)
+        idx |= ((iy >> b) & 1) << (2 * b + 1)
+    return face * n * n + idx
+
+
+def superpixel_map_ring(nside: int, nside_patch: int) -> np.ndarray:
+    """int32 [npix]: for every RING pixel of the nside map, the NESTED index of the nside_patch super-pixel that holds
+    its centre (`multires_clusters` of the paper, L607: a fixed baseline tiling with K = 12 nside_patch^2 patches)."""
+    z, phi = pix2zphi_ring(nside)
+    return zphi2pix_nest(nside_patch, z, phi).astype(np.int32)

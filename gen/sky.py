@@ -14,7 +14,7 @@ NU0_SYNC_GHZ = 23.0
 T_CMB_K = 2.7255
 _H_OVER_K = 6.62607015e-34 / 1.380649e-23 * 1e9      # K per GHz
 
-_PURPOSE = {"sky": 1, "noise": 2, "kmeans": 3, "shuffle": 4, "params": 5, "misc": 6}
+_PURPOSE = {"sky": 1, "noise": 2, "kmeans": 3, "shuffle": 4, "params": 5, "misc": 6, "mask": 7}
 
 
 def rng_for(purpose: str, index: int = 0) -> np.random.Generator:

@@ -163,6 +163,16 @@ CS_API int cs_spectral_misfit(cs_ctx *ctx, double *chi2, void *stream);
  * travels through a pinned staging ring; nothing is allocated and the stream is not synchronised). */
 CS_API int cs_component_maps(cs_ctx *ctx, int32_t nsel, const int32_t *entries, float *s, void *stream);
 
+/* Map level of the residual estimates of Eq. 14-15: cmb dev [nsel, 2, npix] fp32 =
+ * [W_e d_j]_CMB, the CMB row (Q, U) of the map-making operator W = (A^T N^-1 A)^-1 A^T N^-1 of entry entries[i]
+ * (its configuration and the parameters the tables were last built with) applied to data set j = data_sel[i] of the
+ * current data -- any data set, not only the entry's own.  With d_j the noise-free foreground-only maps d_fg it is
+ * the systematic residual [W d_fg]_CMB of Eq. 15; the statistical residual of Eq. 14 is the caller's difference
+ * (s_hat_CMB - s_CMB^true) - [W d_fg]_CMB.  entries == NULL takes all entries in order; data_sel host [nsel], required.
+ * Masked pixels are written as 0.  Asynchronous like cs_component_maps.  (The spectra C_l of those maps are out of
+ * scope: they need spherical-harmonic transforms.) */
+CS_API int cs_cmb_residual_maps(cs_ctx *ctx, int32_t nsel, const int32_t *entries, const int32_t *data_sel, float *cmb, void *stream);
+
 /* f3, the cell-compressed likelihood (PAPER.md:L95 patch model, L80 Eq. 6): pixels with the same cluster triple share
  * A, so their part of Eq. 6 is tr(M^-1 A^T T A) with the parameter-independent second moments
  * T = N^-1 (sum_{p,S} d_S d_S^T) N^-1 of the cell.  cs_cell_moments builds T (fp64) for every (configuration, data set)

@@ -16,7 +16,7 @@ LAYOUT_AUTO, LAYOUT_INPLACE, LAYOUT_SORTED = 0, 1, 2
 FORM_AUTO, FORM_DIRECT = 0, 1
 
 EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
-           "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_cell_moments", "cs_spectral_like_grad_cells", "cs_component_maps", "cs_cmb_variance", "cs_optimize",
+           "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_cell_moments", "cs_spectral_like_grad_cells", "cs_component_maps", "cs_cmb_residual_maps", "cs_cmb_variance", "cs_optimize",
            "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
 
@@ -70,6 +70,7 @@ def lib():
         "cs_cell_moments": (C.c_int, [vp, vp]),
         "cs_spectral_like_grad_cells": (C.c_int, [vp, vp, vp, vp]),
         "cs_component_maps": (C.c_int, [vp, i32, vp, vp, vp]),
+        "cs_cmb_residual_maps": (C.c_int, [vp, i32, vp, vp, vp, vp]),
         "cs_cmb_variance": (C.c_int, [vp, vp, vp]),
         "cs_optimize": (C.c_int, [vp, vp, vp, vp, C.POINTER(CsOpt), vp, vp]),
         "cs_opt_defaults": (None, [C.POINTER(CsOpt)]),
@@ -251,6 +252,18 @@ class Context:
             nsel, ep = int(entries.shape[0]), _hp(entries)
         _chk(lib().cs_component_maps(self._h, nsel, ep, _ptr(s, "float32", "cuda", nsel * 6 * self.npix, "s"), _stream(stream)),
              "cs_component_maps")
+
+    def cmb_residual_maps(self, cmb, data_sel, entries=None, stream=None):
+        """cmb: float32 device [nsel,2,npix]; data_sel: data set each selected entry's W is applied to."""
+        data_sel = np.ascontiguousarray(data_sel, dtype=np.int32)
+        nsel = int(data_sel.shape[0])
+        ep = None
+        if entries is not None:
+            entries = np.ascontiguousarray(entries, dtype=np.int32)
+            assert entries.shape[0] == nsel
+            ep = _hp(entries)
+        _chk(lib().cs_cmb_residual_maps(self._h, nsel, ep, _hp(data_sel), _ptr(cmb, "float32", "cuda", nsel * 2 * self.npix, "cmb"),
+                                        _stream(stream)), "cs_cmb_residual_maps")
 
     def cmb_variance(self, var, stream=None):
         _chk(lib().cs_cmb_variance(self._h, _ptr(var, "float64", "cuda", self.batch * self.nregion, "var"), _stream(stream)),

@@ -980,15 +980,16 @@ int cs_spectral_misfit(cs_ctx *c, double *chi2, void *stream) {
     return merge_launch(c, chi2, nullptr, st);
 }
 
-int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s, void *stream) {
+// a4 and the map level of f4(ii): W(params of entry e) applied to data set data_sel[i] (or the entry's own), `planes`
+// output planes per selected entry.
+static int maps_impl(cs_ctx *c, int32_t nsel, const int32_t *entries, const int32_t *data_sel, int32_t planes, float *s, cudaStream_t st) {
     int rc = ready(c);
     if (rc) return rc;
     if (!s || !c->tables_built || nsel <= 0 || nsel > c->batch) return CS_EINVAL;
     if (!entries && nsel != c->batch) return CS_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    // The selection (entry list, then its runs = stretches of consecutive selected entries of one configuration) goes
-    // through a small ring of pinned staging slots, so that the call never synchronises the caller's stream; a slot is
-    // reused only after the copy that read it has completed.
+    // The selection (entry list, per-position info, then its runs = stretches of consecutive selected entries of one
+    // configuration) goes through a small ring of pinned staging slots, so that the call never synchronises the
+    // caller's stream; a slot is reused only after the copy that read it has completed.
     const int slot = (int)(c->sel_n % cs_ctx::SEL_RING);
     if (!c->sel_ev[slot]) CK(cudaEventCreateWithFlags(&c->sel_ev[slot], cudaEventDisableTiming));
     else CK(cudaEventSynchronize(c->sel_ev[slot]));
@@ -996,11 +997,12 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
     for (int32_t i = 0; i < nsel; ++i) {
         const int32_t e = entries ? entries[i] : i;
         if (e < 0 || e >= c->batch) return CS_EINVAL;
+        if (data_sel && (data_sel[i] < 0 || data_sel[i] >= c->ndata)) return CS_EINVAL;
         hs[i] = e;
     }
     const int64_t poff = ((int64_t)nsel + 3) & ~(int64_t)3;   // position info starts 16-byte aligned, the runs follow it
     PosInfo *hp = reinterpret_cast<PosInfo *>(hs + poff);
-    for (int32_t i = 0; i < nsel; ++i) hp[i] = PosInfo{c->tab_off[hs[i]], (int64_t)c->data_of[hs[i]]};
+    for (int32_t i = 0; i < nsel; ++i) hp[i] = PosInfo{c->tab_off[hs[i]], (int64_t)(data_sel ? data_sel[i] : c->data_of[hs[i]])};
     const int64_t roff = poff + (int64_t)nsel * (int64_t)(sizeof(PosInfo) / 4);
     Run *hr = reinterpret_cast<Run *>(hs + roff);
     int32_t nrun = 0;
@@ -1021,9 +1023,19 @@ int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s,
     P.elist = ds;
     P.pinfo = reinterpret_cast<const PosInfo *>(ds + poff);
     P.maps_out = s;
+    P.maps_planes = planes;
     P.ring_maps = 1;
     P.evict_first = ((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4 > (int64_t)96 << 20) ? 1 : 0;
     return launch_like<MODE_MAPS>(c, P, reinterpret_cast<const Run *>(ds + roff), 0, 0, nrun, W, st);
+}
+
+int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s, void *stream) {
+    return maps_impl(c, nsel, entries, nullptr, 6, s, (cudaStream_t)stream);
+}
+
+int cs_cmb_residual_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, const int32_t *data_sel, float *cmb, void *stream) {
+    if (!data_sel) return CS_EINVAL;
+    return maps_impl(c, nsel, entries, data_sel, 2, cmb, (cudaStream_t)stream);
 }
 
 int cs_cell_moments(cs_ctx *c, void *stream) {

@@ -198,11 +198,12 @@ __global__ void __launch_bounds__(DR_THREADS, 1) k_like_direct(const __grid_cons
             } else if (MODE == MODE_CMBVAR) {
                 t0 = sq[0]; t1 = su[0]; t2 = mul_(sq[0], sq[0]); t3 = mul_(su[0], su[0]);
             } else if (MODE == MODE_MAPS) {
-                float *o = P.maps_out + (int64_t)(w.run.estart + k) * 6 * P.npix + posA;
+                float *o = P.maps_out + (int64_t)(w.run.estart + k) * P.maps_planes * P.npix + posA;
                 const float2 v[6] = {sq[0], su[0], sq[1], su[1], sq[2], su[2]};
                 const bool vec = inB && ((P.npix & 1) == 0) && ((reinterpret_cast<uintptr_t>(P.maps_out) & 7) == 0);
 #pragma unroll
                 for (int c = 0; c < 6; ++c) {
+                    if (c >= P.maps_planes) break;
                     const float a = liveA ? v[c].x : 0.f, b = liveB ? v[c].y : 0.f;
                     if (vec) {
                         *reinterpret_cast<float2 *>(o + c * P.npix) = make_float2(a, b);

@@ -34,7 +34,7 @@ struct LikeParams {
     const CfgDev *cfgs;
     const Run *runs;
     int32_t nrun;
-    int32_t pad0;
+    int32_t maps_planes;       // MODE_MAPS: 6 = all components (cmb, dust, sync) x (Q, U); 2 = the CMB component only
     int64_t W;                 // total units of the launch
     const int32_t *elist;
     const int32_t *skip;       // [batch] or null: entries with a non-zero flag are left out (line-search trials of

@@ -90,3 +90,42 @@ def test_workloads_shapes():
 def test_forward_model_is_unit_normalised():
     a_d, a_s = gen.mixing_columns([353.0, 23.0], 1.6, 19.0, -3.1)
     assert abs(a_d[0] - 1.0) < 1e-14 and abs(a_s[1] - 1.0) < 1e-14
+
+
+def test_nested_superpixels_are_equal_area_compact_patches():
+    """zphi2pix_nest (Gorski et al. 2005, restated): at a coarse nside the NESTED index partitions the pixel centres
+    of a fine map into 12 nside_patch^2 patches of exactly (nside / nside_patch)^2 pixels each -- true only if faces,
+    (ix, iy) and the bit interleave are all right -- and every patch is compact (its pixels lie within ~1.5 patch
+    diagonals of their mean direction)."""
+    for nside, npatch in ((8, 1), (16, 2), (32, 4), (64, 16), (64, 64)):
+        m = gen.superpixel_map_ring(nside, npatch)
+        counts = np.bincount(m, minlength=12 * npatch * npatch)
+        assert counts.shape[0] == 12 * npatch * npatch and np.all(counts == (nside // npatch) ** 2)
+    nside, npatch = 32, 4
+    m = gen.superpixel_map_ring(nside, npatch)
+    v = gen.pix2vec_ring(nside)
+    size = np.sqrt(4 * np.pi / (12 * npatch * npatch))           # angular size of a patch
+    for k in (0, 17, 100, 191):
+        vk = v[m == k]
+        c = vk.mean(axis=0)
+        c /= np.linalg.norm(c)
+        assert np.arccos(np.clip(vk @ c, -1, 1)).max() < 1.5 * size
+    # at the map's own resolution the NESTED index is a permutation of the RING index with the known fixed points
+    # of nside 1: pixel p of RING order is pixel p of NESTED order
+    assert np.array_equal(gen.superpixel_map_ring(1, 1), np.arange(12))
+
+
+def test_irregular_mask_and_multires_workload():
+    w = gen.make_config(1, nside=16, multires=(8, 2, 4), holes=3)
+    assert w.K_of_cfg(0) == [768, 48, 192]
+    masked = (w.maps < 0).any(axis=0)
+    assert np.array_equal(masked, (w.maps < 0).all(axis=0))         # a hole masks all three maps
+    frac = masked.mean()
+    assert 0.1 < frac < 0.5
+    # no structure in RING order: masked runs of many different lengths, including single pixels
+    edges = np.flatnonzero(np.diff(masked.astype(np.int8)))
+    runs = np.diff(edges)
+    assert len(np.unique(runs)) > 8 and runs.min() == 1
+    # same seed, same mask; another seed, another mask
+    assert np.array_equal(masked, (gen.make_config(1, nside=16, multires=(8, 2, 4), holes=3).maps < 0).any(axis=0))
+    assert not np.array_equal(masked, (gen.make_config(1, nside=16, multires=(8, 2, 4), holes=4).maps < 0).any(axis=0))

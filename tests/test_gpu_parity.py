@@ -735,3 +735,58 @@ def test_cells_full_size_c3_scan_sampled(torch_cuda):
         check_T1(nll[e], ref["nll"])
         check_T2(grad[off[e]:off[e + 1]], ref, w.K_of_cfg(int(w.cfg_of[e])))
     ctx.close()
+
+
+# ----------------------------------------------------------------------------- f4: second workload, residual maps
+
+def test_multires_superpixel_patches_with_an_irregular_mask(torch_cuda, path):
+    """f4(iii): NESTED super-pixel patches (Table 3) instead of K-means clusters, under a
+    Planck-like irregular mask (ragged equatorial band, point-source discs, isolated pixels): nothing in the kernels
+    may depend on K-means compactness or on RING-contiguous regions."""
+    w = gen.make_config(1, nside=32, multires=(8, 2, 4), holes=5, ndata=2)
+    assert w.K_of_cfg(0) == [768, 48, 192]
+    _parity(w, w.params_jittered(seed=31))
+    w = gen.make_config(1, nside=32, multires=(32, 1, 16), holes=6)       # beta_d per pixel, one T_d patch per base face
+    _parity(w, w.params_jittered(seed=32))
+
+
+def test_cmb_residual_maps_are_W_applied_to_another_data_set(torch_cuda, path):
+    """f4(ii), map level of Eq. 14-15: [W_e d_fg]_CMB with d_fg the noise-free foreground-only maps, against the
+    oracle's maps of the same parameters on d_fg (T3); applied to the entry's own data it is the CMB plane of
+    cs_component_maps, bit for bit."""
+    import torch
+    w = _masked(gen.make_config(3, nside=16, batch=4, ndata=2))
+    fg = dict(w.truth)
+    fg["s"] = w.truth["s"].copy()
+    fg["s"][0] = 0.0                                                       # no CMB
+    d_fg = gen.synthesize(fg, w.freqs, None)                               # no noise
+    data = np.ascontiguousarray(np.concatenate([w.data(), d_fg]))          # data set 2 = d_fg
+    w = dataclasses.replace(w, _d=data, ndata=3)
+    params = w.params_jittered(seed=33)
+    ctx, _ = make_ctx(w)
+    p = torch.from_numpy(params).cuda()
+    ctx.build_sed_tables(p)
+    ent = np.array([0, 1, 3], dtype=np.int32)
+    out = torch.full((3, 2, w.npix), float("nan"), dtype=torch.float32, device="cuda")
+    ctx.cmb_residual_maps(out, np.array([2, 2, 2], dtype=np.int32), ent)
+    own = torch.full((3, 2, w.npix), float("nan"), dtype=torch.float32, device="cuda")
+    ctx.cmb_residual_maps(own, w.data_of[ent], ent)
+    smaps = torch.full((3, 3, 2, w.npix), float("nan"), dtype=torch.float32, device="cuda")
+    ctx.component_maps(smaps, ent)
+    torch.cuda.synchronize()
+    assert np.array_equal(own.cpu().numpy(), smaps.cpu().numpy()[:, 0])
+    out = out.cpu().numpy()
+    off = w.param_offsets()
+    model = oracle.Model(w.freqs)
+    for i, e in enumerate(ent):
+        c = int(w.cfg_of[e])
+        ref = oracle.nll_grad(model, d_fg[0], w.ninv, w.maps[w.cfg_maps[c]], w.K_of_cfg(c), params[off[e]:off[e + 1]],
+                              region=w.region_idx, nregion=w.nregion, want_grad=False, want_maps=True)["maps"][0]
+        ds = out[i].astype(np.float64) - ref
+        # the leakage of foregrounds into the CMB map is a small difference of large terms: compare against the scale of
+        # the foreground maps it is made from (T3 on the three components together)
+        scale = np.abs(d_fg[0]).max()
+        assert np.abs(ds).max() <= 1e-5 * scale, (np.abs(ds).max(), scale)
+        masked = (w.maps[w.cfg_maps[c]] < 0).any(axis=0)
+        assert np.all(out[i][:, masked] == 0.0)
+    ctx.close()
