@@ -9,12 +9,25 @@ its label (labels are never compacted).  K larger than the number of pixels: one
 import numpy as np
 
 
-def _assign(vecs: np.ndarray, cent: np.ndarray, chunk: int = 16384) -> np.ndarray:
+def _assign(vecs: np.ndarray, cent: np.ndarray, chunk: int = 8192) -> np.ndarray:
+    """argmax_k n_p . c_k, ties to the lowest id.  The dot product is written out as (x cx + y cy) + z cz, every
+    operation rounded once (no BLAS, no FMA): region problems are seeded from pixel centres, whose symmetries produce
+    exactly tied dot products, so the result must not depend on how a library associates the three terms."""
     out = np.empty(vecs.shape[0], dtype=np.int32)
-    ct = np.ascontiguousarray(cent.T)
+    cx, cy, cz = (np.ascontiguousarray(cent[:, i])[None, :] for i in range(3))
     for s in range(0, vecs.shape[0], chunk):
-        out[s:s + chunk] = np.argmax(vecs[s:s + chunk] @ ct, axis=1)
+        v = vecs[s:s + chunk]
+        dots = (v[:, 0:1] * cx + v[:, 1:2] * cy) + v[:, 2:3] * cz
+        out[s:s + chunk] = np.argmax(dots, axis=1)
     return out
+
+
+def initial_centroids(vecs: np.ndarray, K: int, rng: np.random.Generator, seed_from_pixels: bool = False) -> np.ndarray:
+    """The seeded start of a K-means problem ([K,3] fp64): uniform on the sphere, or K distinct random pixels."""
+    if seed_from_pixels:
+        return vecs[rng.choice(vecs.shape[0], size=K, replace=False)].copy()
+    g = rng.standard_normal((K, 3))
+    return g / np.linalg.norm(g, axis=1, keepdims=True)
 
 
 def spherical_kmeans(vecs: np.ndarray, K: int, rng: np.random.Generator, iters: int = 10,
@@ -25,11 +38,7 @@ def spherical_kmeans(vecs: np.ndarray, K: int, rng: np.random.Generator, iters: 
         return np.arange(n, dtype=np.int32)
     if K == 1:
         return np.zeros(n, dtype=np.int32)
-    if seed_from_pixels:
-        cent = vecs[rng.choice(n, size=K, replace=False)].copy()
-    else:
-        g = rng.standard_normal((K, 3))
-        cent = g / np.linalg.norm(g, axis=1, keepdims=True)
+    cent = initial_centroids(vecs, K, rng, seed_from_pixels)
     lab = _assign(vecs, cent)
     for _ in range(iters):
         sums = np.zeros((K, 3))

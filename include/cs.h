@@ -207,6 +207,18 @@ CS_API void cs_opt_defaults(cs_opt *opt);
 CS_API int cs_eval_host(cs_ctx *ctx, int32_t ndata, const float *d_host, const float *ninv_host, const double *params_host,
                  double *nll_host, double *grad_host);
 
+/* f2, batched spherical K-means patching, the step before the path; needs no context.
+ * nprob independent problems on the same pixel set: vecs dev [npix,3] fp64 unit vectors of the pixel centres; problem j
+ * has K[j] patches (host [nprob]) and, when prob_region != NULL and prob_region[j] >= 0, only the pixels with
+ * region[p] == prob_region[j] (region dev [npix] uint8) take part.  cent dev [sum_j K[j], 3] fp64: in = the initial
+ * centroids (the caller draws them), out = the final ones.  Runs one assignment, then `iters` Lloyd iterations
+ * (centroid = renormalised mean of its pixels, an empty patch keeps its centroid; assignment = largest dot product in
+ * fp64, ties to the lowest id).  labels dev [nprob, npix] int32: patch id in [0, K[j]), or -1 outside the problem's
+ * region.  The arithmetic is fixed operation by operation (csrc/cs_kmeans.cuh), so labels are reproducible bit for
+ * bit.  Asynchronous on `stream`. */
+CS_API int cs_spherical_kmeans(int64_t npix, const double *vecs, const uint8_t *region, int32_t nprob, const int32_t *K,
+                        const int32_t *prob_region, double *cent, int32_t iters, int32_t *labels, void *stream);
+
 /* Synchronises `stream`, returns and clears the sticky device error bits: CS_OK, CS_EDOMAIN or CS_ESINGULAR. */
 CS_API int cs_check(cs_ctx *ctx, void *stream);
 CS_API const char *cs_strerror(int code);

@@ -17,7 +17,7 @@ FORM_AUTO, FORM_DIRECT = 0, 1
 
 EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
            "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_cell_moments", "cs_spectral_like_grad_cells", "cs_component_maps", "cs_cmb_residual_maps", "cs_cmb_variance", "cs_optimize",
-           "cs_opt_defaults", "cs_eval_host", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
+           "cs_opt_defaults", "cs_eval_host", "cs_spherical_kmeans", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
 
 
@@ -75,6 +75,7 @@ def lib():
         "cs_optimize": (C.c_int, [vp, vp, vp, vp, C.POINTER(CsOpt), vp, vp]),
         "cs_opt_defaults": (None, [C.POINTER(CsOpt)]),
         "cs_eval_host": (C.c_int, [vp, i32, vp, vp, vp, vp, vp]),
+        "cs_spherical_kmeans": (C.c_int, [i64, vp, vp, i32, vp, vp, vp, i32, vp, vp]),
         "cs_check": (C.c_int, [vp, vp]),
         "cs_profile": (C.c_int, [vp, C.c_int]),
         "cs_profile_read": (C.c_int, [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
@@ -151,6 +152,18 @@ def opt_defaults(**kw) -> CsOpt:
     for k, v in kw.items():
         setattr(o, k, v)
     return o
+
+
+def spherical_kmeans(vecs, K, cent, labels, iters=10, region=None, prob_region=None, stream=None):
+    """cs_spherical_kmeans: vecs float64 cuda [npix,3]; K host int32 [nprob]; cent float64 cuda [sum K,3] (in: initial,
+    out: final); labels int32 cuda [nprob,npix]; region uint8 cuda [npix] and prob_region host [nprob] or None."""
+    K = np.ascontiguousarray(K, dtype=np.int32)
+    nprob, npix = int(K.shape[0]), int(vecs.shape[0])
+    if prob_region is not None:
+        prob_region = np.ascontiguousarray(prob_region, dtype=np.int32)
+    _chk(lib().cs_spherical_kmeans(npix, _ptr(vecs, "float64", "cuda", 3 * npix, "vecs"), _ptr(region, "uint8", "cuda", npix, "region"),
+                                   nprob, _hp(K), _hp(prob_region), _ptr(cent, "float64", "cuda", 3 * int(K.sum()), "cent"), int(iters),
+                                   _ptr(labels, "int32", "cuda", nprob * npix, "labels"), _stream(stream)), "cs_spherical_kmeans")
 
 
 class Context:

@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libcs.so")
 SOURCES = ["cs_lib.cu"]
-HEADERS = ["cs_cells.cuh", "cs_pipe.cuh", "cs_tables.cuh", "cs_like_sc.cuh", "cs_like_direct.cuh", "cs_math.cuh", "cs_optim.cuh", "cs_internal.h", os.path.join("..", "..", "include", "cs.h")]
+HEADERS = ["cs_kmeans.cuh", "cs_cells.cuh", "cs_pipe.cuh", "cs_tables.cuh", "cs_like_sc.cuh", "cs_like_direct.cuh", "cs_math.cuh", "cs_optim.cuh", "cs_internal.h", os.path.join("..", "..", "include", "cs.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
               "-Xcompiler", "-fPIC,-O2,-fvisibility=hidden", "-Xptxas", "-v", "--use_fast_math=false"]
 

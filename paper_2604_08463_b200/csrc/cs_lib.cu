@@ -17,6 +17,7 @@
 #include "cs_like_direct.cuh"
 #include "cs_optim.cuh"
 #include "cs_cells.cuh"
+#include "cs_kmeans.cuh"
 
 using namespace cs;
 
@@ -1315,6 +1316,38 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
     if (cudaStreamSynchronize(cp) != cudaSuccess || cudaStreamSynchronize(cm) != cudaSuccess) rc = rc ? rc : CS_ECUDA;
     for (cudaEvent_t ev : evs) cudaEventDestroy(ev);
     return rc;
+    CS_GUARD_END
+}
+
+int cs_spherical_kmeans(int64_t npix, const double *vecs, const uint8_t *region, int32_t nprob, const int32_t *K,
+                        const int32_t *prob_region, double *cent, int32_t iters, int32_t *labels, void *stream) {
+    if (npix <= 0 || !vecs || nprob <= 0 || nprob > 65535 || !K || !cent || iters < 0 || !labels) return CS_EINVAL;
+    CS_GUARD_BEGIN
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<KmProb> pr(nprob);
+    int64_t off = 0;
+    int32_t kmax = 0;
+    for (int32_t j = 0; j < nprob; ++j) {
+        if (K[j] < 1) return CS_EINVAL;
+        const int32_t reg = prob_region ? prob_region[j] : -1;
+        if (reg >= 0 && !region) return CS_EINVAL;
+        pr[j] = KmProb{K[j], reg, off};
+        off += K[j];
+        kmax = std::max(kmax, K[j]);
+    }
+    KmProb *d_pr = nullptr;
+    if (cudaMallocAsync((void **)&d_pr, sizeof(KmProb) * nprob, st) != cudaSuccess) return CS_ENOMEM;
+    // pageable host memory: the copy has left the host buffer when cudaMemcpyAsync returns
+    if (cudaMemcpyAsync(d_pr, pr.data(), sizeof(KmProb) * nprob, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaFreeAsync(d_pr, st); return CS_ECUDA; }
+    const dim3 ga((unsigned)((npix + 255) / 256), nprob), gu((kmax + 127) / 128, nprob);
+    k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
+    for (int32_t it = 0; it < iters; ++it) {
+        k_km_update<<<gu, 128, 0, st>>>(vecs, npix, d_pr, labels, cent);
+        k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
+    }
+    const cudaError_t ce = cudaGetLastError();
+    cudaFreeAsync(d_pr, st);
+    return ce == cudaSuccess ? CS_OK : CS_ECUDA;
     CS_GUARD_END
 }
 
