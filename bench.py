@@ -231,8 +231,9 @@ def time_hot_path(ctx, w, params, steps, warmup, dev, stream, barrier=None):
             "launches": launches, "nll": nll, "grad": grad, "p_dev": p_dev, "t0": t0, "t1": t1}
 
 
-def extra_workload(cs, name, batch, steps, dev, stream, peak):
-    """One short run of another BASELINE configuration for `extras`."""
+def extra_workload(cs, name, batch, steps, dev, stream, peak, prefixes=None):
+    """Short runs of another BASELINE configuration for `extras`: the whole batch, or (prefixes) its first b entries for
+    every b in `prefixes` on the same context and data (the batch sweep of config 5).  Returns {key: result}."""
     import torch
     t0 = time.time()
     w, desc = make_workload(name, batch)
@@ -242,27 +243,103 @@ def extra_workload(cs, name, batch, steps, dev, stream, peak):
     ctx = cs.Context(w.freqs, w.npix)
     ctx.set_clusters(w.maps, w.Kmap, w.cfg_maps, w.region_idx, w.nregion)
     ctx.set_data(d_dev, w.ninv)
-    ctx.set_batch(w.cfg_of, w.data_of)
     torch.cuda.synchronize()
     t_setup = time.time() - t0
-    r = time_hot_path(ctx, w, w.params_jittered(seed=7), steps, 3, dev, stream)
-    pe = float(w.batch) * w.npix
-    ms_step = r["ms"] / steps
-    sorted_cfgs = sum(1 for c in np.unique(w.cfg_of) if ctx.layout_info(int(c))[0])
-    distinct_data = len({(int(c), int(d)) for c, d in zip(w.cfg_of, w.data_of)}) if sorted_cfgs else len(np.unique(w.data_of))
-    out = {"workload": desc, "batch": w.batch, "npix": w.npix, "steps": steps, "ms_per_step": ms_step,
-           "pixel_evals_per_s": pe / (ms_step * 1e-3), "fused_kernel_ms_per_step": r["kernel_ms_per_step"],
-           "kernel": kernel_name(ctx, w, w.nfreq),
-           # d-stream accounting (120 B per pixel-eval); meaningful where every entry streams its own data
-           "roofline_frac_of_measured_peak": BYTES_PER_PIXEL_EVAL * pe / (r["kernel_ms_per_step"] * 1e-3) / 1e9 / peak
-           if r["kernel_ms_per_step"] > 0 else None,
-           "configurations_sorted": sorted_cfgs, "configurations": int(len(np.unique(w.cfg_of))),
-           "streams_read_per_step": distinct_data, "workspace_GB": ctx.workspace_bytes() / 1e9,
-           "datagen_s": round(t_gen, 1), "setup_s": round(t_setup, 1)}
+    res = {}
+    params_all = w.params_jittered(seed=7)
+    off = w.param_offsets()
+    for b in (prefixes or [w.batch]):
+        import dataclasses
+        wb = dataclasses.replace(w, cfg_of=w.cfg_of[:b], data_of=w.data_of[:b])
+        t0 = time.time()
+        ctx.set_batch(wb.cfg_of, wb.data_of)
+        torch.cuda.synchronize()
+        t_batch = time.time() - t0
+        r = time_hot_path(ctx, wb, params_all[:off[b]], steps, 3, dev, stream)
+        pe = float(b) * w.npix
+        ms_step = r["ms"] / steps
+        sorted_cfgs = sum(1 for c in np.unique(wb.cfg_of) if ctx.layout_info(int(c))[0])
+        streams = len({(int(c), int(d)) for c, d in zip(wb.cfg_of, wb.data_of)}) if sorted_cfgs else len(np.unique(wb.data_of))
+        res[b] = {"workload": desc if b == w.batch else f"{desc}: first {b} entries", "batch": b, "npix": w.npix, "steps": steps,
+                  "ms_per_step": ms_step, "pixel_evals_per_s": pe / (ms_step * 1e-3),
+                  "fused_kernel_ms_per_step": r["kernel_ms_per_step"], "kernel": kernel_name(ctx, wb, w.nfreq),
+                  # d-stream accounting (120 B per pixel-eval): every entry streams its own (private) data
+                  "roofline_frac_of_measured_peak": BYTES_PER_PIXEL_EVAL * pe / (r["kernel_ms_per_step"] * 1e-3) / 1e9 / peak
+                  if r["kernel_ms_per_step"] > 0 else None,
+                  "configurations_sorted": sorted_cfgs, "configurations": int(len(np.unique(wb.cfg_of))),
+                  "streams_read_per_step": streams, "workspace_GB": ctx.workspace_bytes() / 1e9,
+                  "datagen_s": round(t_gen, 1), "set_clusters_and_data_s": round(t_setup, 1), "set_batch_s": round(t_batch, 3)}
+    ctx.close()
+    del d_dev
+    torch.cuda.empty_cache()
+    return res
+
+
+def extra_cells(cs, name, batch, steps, dev, stream):
+    """f3 on a workload: cs_cell_moments once, then steps of tables + cs_spectral_like_grad_cells.  Reported under its
+    own metric: pixel-evals-equivalent/s = batch x npix / step time (no pixel is touched in the step)."""
+    import torch
+    w, desc = make_workload(name, batch)
+    d_dev = torch.from_numpy(w.data()).to(dev)
+    ctx = cs.Context(w.freqs, w.npix, options={"layout": cs.LAYOUT_SORTED})
+    ctx.set_clusters(w.maps, w.Kmap, w.cfg_maps, w.region_idx, w.nregion)
+    ctx.set_data(d_dev, w.ninv)
+    ctx.set_batch(w.cfg_of, w.data_of)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    ctx.cell_moments(stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    mom_ms = e0.elapsed_time(e1)
+    p_dev = torch.from_numpy(w.params_jittered(seed=7)).to(dev)
+    nll = torch.zeros(w.batch * w.nregion, dtype=torch.float64, device=dev)
+    grad = torch.zeros_like(p_dev)
+    for _ in range(3):
+        ctx.build_sed_tables(p_dev, stream)
+        ctx.spectral_like_grad_cells(nll, grad, stream)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        ctx.build_sed_tables(p_dev, stream)
+        ctx.spectral_like_grad_cells(nll, grad, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    nll_pp = torch.zeros_like(nll)
+    ctx.spectral_like_grad(nll_pp, None, stream)
+    torch.cuda.synchronize()
+    rel = float(((nll - nll_pp).abs() / nll_pp.abs()).max().item())
+    out = {"metric": "f3 cell-compressed likelihood: pixel-evals-equivalent/s (batch x npix / step time)",
+           "workload": desc, "batch": w.batch, "ms_per_step": ms, "pixel_evals_equivalent_per_s": w.batch * w.npix / (ms * 1e-3),
+           "cell_moments_ms_once": mom_ms, "max_rel_diff_nll_vs_per_pixel_path": rel, "workspace_GB": ctx.workspace_bytes() / 1e9}
     ctx.close()
     del d_dev
     torch.cuda.empty_cache()
     return out
+
+
+def extra_kmeans(cs, dev):
+    """f2: the 32 distinct cluster maps of the C3 scan (nside 64, K = 1 .. 1000, 10 Lloyd iterations) in one batched call."""
+    import torch
+    from gen import kmeans as gk
+    vecs = gen.pix2vec_ring(64)
+    specs = sorted({(prm, int(k[prm])) for k in gen.c3_grid() for prm in range(3)})
+    probs = [(prm, K) for prm, K in specs if 1 < K < vecs.shape[0]]
+    cent0 = np.concatenate([gk.initial_centroids(vecs, K, gen.rng_for("kmeans", (prm * 1_000_003 + K) * 16)) for prm, K in probs])
+    v_d = torch.from_numpy(vecs).to(dev)
+    lab = torch.zeros((len(probs), vecs.shape[0]), dtype=torch.int32, device=dev)
+    Ks = [K for _, K in probs]
+    times = []
+    for _ in range(2):
+        cent = torch.from_numpy(cent0.copy()).to(dev)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        cs.spherical_kmeans(v_d, Ks, cent, lab, iters=10)
+        torch.cuda.synchronize()
+        times.append(time.perf_counter() - t0)
+    return {"workload": f"{len(probs)} K-means problems of the C3 scan, nside 64, K = {min(Ks)} .. {max(Ks)}, 10 Lloyd iterations",
+            "ms": 1e3 * min(times), "dot_products_per_s": 11 * vecs.shape[0] * float(sum(Ks)) / min(times)}
 
 
 def relaunch_multi_gpu(args):
@@ -531,11 +608,18 @@ def main():
                                    "pixel_evals_per_s": w2.npix / (e0.elapsed_time(e1) / 20 * 1e-3)}
             c2.close()
             del d2
-            for nm, b in (("c3", 0), ("c4", 0), ("c5", 1), ("c5", 16), ("c5", 64), ("c5", 256)):
-                key = nm if nm != "c5" else f"c5_batch{b}"
+            for nm, prefixes in (("c3", None), ("c4", None), ("c5", [1, 16, 64, 256])):
                 try:
-                    out["extras"][key] = extra_workload(cs, nm, b, 5, dev, stream, peak)
+                    for b, res in extra_workload(cs, nm, 0, 5, dev, stream, peak, prefixes).items():
+                        out["extras"][nm if prefixes is None else f"{nm}_batch{b}"] = res
                 except Exception as exc:   # a failed extra must not lose the headline line
+                    out["extras"][nm] = {"error": repr(exc)}
+            for key, fn in (("f3_cells_c3", lambda: extra_cells(cs, "c3", 0, 5, dev, stream)),
+                            ("f3_cells_c3h", lambda: extra_cells(cs, "c3h", 256, 5, dev, stream)),
+                            ("f2_kmeans", lambda: extra_kmeans(cs, dev))):
+                try:
+                    out["extras"][key] = fn()
+                except Exception as exc:
                     out["extras"][key] = {"error": repr(exc)}
     if rank == 0:
         print(json.dumps(out), flush=True)

@@ -22,10 +22,24 @@ def latitude_regions(vecs: np.ndarray) -> np.ndarray:
     return reg
 
 
+_MAP_CACHE = {}
+
+
 def cluster_map(vecs: np.ndarray, param: int, K: int, region_idx=None, nregion: int = 1, iters: int = 10):
     """One cluster map for spectral parameter `param` (0,1,2) with K patches (per region when regions are
     given: independent K-means per region, ids concatenated region after region, K capped at the region's
-    pixel count).  Returns (labels int32 [npix], K_total)."""
+    pixel count).  Returns (labels int32 [npix], K_total).  Seeded, hence cached per process."""
+    key = (vecs.shape[0], float(vecs[vecs.shape[0] // 3, 0]), int(param), int(K), int(nregion),
+           None if region_idx is None else hash(np.asarray(region_idx).tobytes()), int(iters))
+    if key not in _MAP_CACHE:
+        lab, kt = _cluster_map(vecs, param, K, region_idx, nregion, iters)
+        lab.setflags(write=False)
+        _MAP_CACHE[key] = (lab, kt)
+    lab, kt = _MAP_CACHE[key]
+    return lab.copy(), kt
+
+
+def _cluster_map(vecs: np.ndarray, param: int, K: int, region_idx, nregion: int, iters: int):
     npix = vecs.shape[0]
     if region_idx is None or nregion == 1:
         g = sky.rng_for("kmeans", (param * 1_000_003 + K) * 16)
