@@ -229,6 +229,16 @@ CS_API const char *cs_strerror(int code);
 CS_API int cs_profile(cs_ctx *ctx, int enable);
 CS_API int cs_profile_read(cs_ctx *ctx, double *total_ms, int64_t *count);
 
+/* The parameter-independent constants the table and fused kernels are given, computed on the host once per context
+ * (cs_create) or data set (cs_set_data); any output may be NULL.  Host [nfreq] each:
+ *   cd[f]  = (nu_f/nu0d) u(nu_f)/u(nu0d)   dust band constant: (nu/nu0)^(beta_d+1) = (nu/nu0) (nu/nu0)^beta_d times the
+ *                                           K_RJ -> K_CMB factor u = (e^x-1)^2 / (x^2 e^x), x = h nu / (k T_cmb)   (Eq. 2, R1-R2)
+ *   cs[f]  = u(nu_f)/u(nu0s)               synchrotron band constant (1 in CS_UNITS_LITERAL, like the u ratio of cd)
+ *   lnd[f] = ln(nu_f/nu0d), lns[f] = ln(nu_f/nu0s)   the log-derivatives of the two power laws
+ *   *inv_sum_w = 1 / sum_f Ninv_f (fp32 as the kernels use it; 0 before cs_set_data).
+ * For tests: they are compared with the oracle's own evaluation of the same expressions. */
+CS_API int cs_model_constants(cs_ctx *ctx, double *cd, double *cs, double *lnd, double *lns, double *inv_sum_w);
+
 /* Introspection used by the bench and the tests. */
 CS_API int64_t cs_workspace_bytes(cs_ctx *ctx);      /* device bytes currently held by the context */
 CS_API int64_t cs_kernel_launches(cs_ctx *ctx);      /* kernels launched by this context so far */

@@ -15,7 +15,7 @@ OPT_LAYOUT, OPT_FORM, OPT_MIN_FILL, OPT_COPY_LIMIT_MB = 1, 2, 3, 4
 LAYOUT_AUTO, LAYOUT_INPLACE, LAYOUT_SORTED = 0, 1, 2
 FORM_AUTO, FORM_DIRECT = 0, 1
 
-EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
+EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_model_constants", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
            "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_cell_moments", "cs_spectral_like_grad_cells", "cs_component_maps", "cs_cmb_residual_maps", "cs_cmb_variance", "cs_optimize",
            "cs_opt_defaults", "cs_eval_host", "cs_spherical_kmeans", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
@@ -60,6 +60,7 @@ def lib():
         "cs_destroy": (C.c_int, [vp]),
         "cs_set_option": (C.c_int, [vp, i32, C.c_double]),
         "cs_layout_info": (C.c_int, [vp, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(C.c_double)]),
+        "cs_model_constants": (C.c_int, [vp, vp, vp, vp, vp, C.POINTER(C.c_double)]),
         "cs_set_clusters": (C.c_int, [vp, i32, vp, vp, i32, vp, vp, i32]),
         "cs_set_data": (C.c_int, [vp, i32, vp, vp]),
         "cs_set_batch": (C.c_int, [vp, i32, vp, vp]),
@@ -204,6 +205,15 @@ class Context:
         so, nt, fill = C.c_int32(), C.c_int32(), C.c_double()
         _chk(lib().cs_layout_info(self._h, int(cfg), C.byref(so), C.byref(nt), C.byref(fill)), "cs_layout_info")
         return bool(so.value), nt.value, fill.value
+
+    def model_constants(self):
+        """dict(cd, cs, lnd, lns [nfreq], inv_sum_w): the host-computed constants the kernels are given."""
+        arr = {k: np.empty(self.nfreq) for k in ("cd", "cs", "lnd", "lns")}
+        inv = C.c_double()
+        _chk(lib().cs_model_constants(self._h, _hp(arr["cd"]), _hp(arr["cs"]), _hp(arr["lnd"]), _hp(arr["lns"]), C.byref(inv)),
+             "cs_model_constants")
+        arr["inv_sum_w"] = inv.value
+        return arr
 
     def set_clusters(self, maps, Kmap, cfg_maps, region_idx=None, nregion=1):
         """maps: int32 [nmap,npix] (torch device tensor or numpy); Kmap, cfg_maps: host arrays."""

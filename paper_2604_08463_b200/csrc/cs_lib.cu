@@ -121,6 +121,7 @@ struct cs_ctx {
     std::vector<CopyJob> jobs;          // private copies of the sorted layout, ordered by data set
     int32_t *d_cfg_of = nullptr, *d_data_of = nullptr, *d_elist = nullptr;
     int64_t *d_param_off = nullptr, *d_tab_off = nullptr;
+    TabEntry *d_tabent = nullptr;
     PosInfo *d_pinfo = nullptr;
     Run *d_runs = nullptr;
     CopyJob *d_jobs = nullptr;
@@ -198,10 +199,10 @@ void free_opt(cs_ctx *c) {
 
 void free_batch(cs_ctx *c) {
     cudaFree(c->d_cfg_of); cudaFree(c->d_data_of); cudaFree(c->d_elist);
-    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
+    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_tabent); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
     cudaFree(c->d_tab); cudaFree(c->d_partial); cudaFree(c->d_copy);
     c->d_cfg_of = c->d_data_of = c->d_elist = nullptr;
-    c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr;
+    c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr; c->d_tabent = nullptr;
     c->d_runs = nullptr; c->d_jobs = nullptr;
     c->d_tab = nullptr; c->d_partial = nullptr; c->d_copy = nullptr;
     c->batch = 0; c->nrun_sc = c->nrun_dir = 0; c->batch_bytes = 0; c->copy_bytes = 0;
@@ -632,6 +633,18 @@ int cs_destroy(cs_ctx *c) {
     return CS_OK;
 }
 
+int cs_model_constants(cs_ctx *c, double *cd, double *cs_, double *lnd, double *lns, double *inv_sum_w) {
+    if (!c) return CS_EINVAL;
+    for (int f = 0; f < c->nfreq; ++f) {
+        if (cd) cd[f] = c->tc.cd[f];
+        if (cs_) cs_[f] = c->tc.cs[f];
+        if (lnd) lnd[f] = c->tc.lnd[f];
+        if (lns) lns[f] = c->tc.lns[f];
+    }
+    if (inv_sum_w) *inv_sum_w = c->have_ninv ? (double)c->kc.inv_m00 : 0.0;
+    return CS_OK;
+}
+
 int cs_set_option(cs_ctx *c, int32_t key, double value) {
     if (!c || !std::isfinite(value)) return CS_EINVAL;
     switch (key) {
@@ -898,8 +911,14 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         }
         if (copy_bytes > limit) { free_batch(c); return CS_ENOMEM; }
     }
+    std::vector<TabEntry> tabent(batch);
+    for (int32_t e = 0; e < batch; ++e) {
+        const CfgDev &cf = c->cfgs[cfg_of[e]];
+        tabent[e] = TabEntry{c->param_off[e], tab_off[e], cf.K[0], cf.K[1], cf.ktot, 0};
+    }
     int rc;
-    if ((rc = dev_upload(&c->d_cfg_of, c->cfg_of, &c->batch_bytes)) || (rc = dev_upload(&c->d_data_of, c->data_of, &c->batch_bytes)) ||
+    if ((rc = dev_upload(&c->d_tabent, tabent, &c->batch_bytes)) ||
+        (rc = dev_upload(&c->d_cfg_of, c->cfg_of, &c->batch_bytes)) || (rc = dev_upload(&c->d_data_of, c->data_of, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_elist, c->elist, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_param_off, c->param_off, &c->batch_bytes)) || (rc = dev_upload(&c->d_tab_off, tab_off, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_pinfo, c->pinfo, &c->batch_bytes)) || (rc = dev_upload(&c->d_runs, c->runs, &c->batch_bytes)) ||
@@ -939,7 +958,7 @@ int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
     cudaStream_t st = (cudaStream_t)stream;
     dim3 block(256);
     dim3 grid((4 * c->ktot_max + 255) / 256, std::min(c->batch, 65535));
-    k_tables<<<grid, block, 0, st>>>(params, c->d_param_off, c->d_tab_off, c->d_cfg_of, c->d_cfgs, c->d_tab, c->batch, c->d_err, c->d_tc, c->skip);
+    k_tables<<<grid, block, 0, st>>>(params, c->d_tabent, c->d_tab, c->batch, c->d_err, c->d_tc, c->skip);
     c->launches++;
     CK(cudaGetLastError());
     c->tables_built = true;

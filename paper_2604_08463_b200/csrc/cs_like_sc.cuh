@@ -164,20 +164,25 @@ __device__ __forceinline__ void sc_build_cell(const float4 (&Fd)[4], const float
             }
         }
         o4[q] = make_float4(wd[0], wd[1], wd[2], wd[3]);
-        o4[12 + q] = make_float4(ws[0], ws[1], ws[2], ws[3]);
+        o4[CR_WS + q] = make_float4(ws[0], ws[1], ws[2], ws[3]);
+#ifdef CS_SC_FAT
         if (GRAD) {
             o4[4 + q] = make_float4(u1[0], u1[1], u1[2], u1[3]);
             o4[8 + q] = make_float4(u2[0], u2[1], u2[2], u2[3]);
             o4[16 + q] = make_float4(u3[0], u3[1], u3[2], u3[3]);
         }
+#else
+        if (GRAD) o4[4 + q] = make_float4(u2[0], u2[1], u2[2], u2[3]);   // the other two derivative columns are one multiply
+                                                                         // by a band constant away from w a_d and w a_s
+#endif
     }
     CellScal<float> C;
     cell_finish<GRAD>(S, kc.inv_m00, C);
     if (C.bad != 0.f) atomicOr(err, ERR_SINGULAR);
-    o4[20] = make_float4(C.l10, C.l20, C.l21, C.id1);
-    o4[21] = make_float4(C.id2, C.P10, C.P11, C.P12);
-    o4[22] = make_float4(C.P20, C.P21, C.P22, C.P30);
-    o4[23] = make_float4(C.P31, C.P32, C.bad, 0.f);
+    o4[CR_SC] = make_float4(C.l10, C.l20, C.l21, C.id1);
+    o4[CR_SC + 1] = make_float4(C.id2, C.P10, C.P11, C.P12);
+    o4[CR_SC + 2] = make_float4(C.P20, C.P21, C.P22, C.P30);
+    o4[CR_SC + 3] = make_float4(C.P31, C.P32, C.bad, 0.f);
 }
 
 template <int NF, int MODE>
@@ -332,11 +337,23 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
             pix_sums_zero(A);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const float4 WD = crow[q], WS = crow[12 + q];
+                const float4 WD = crow[q], WS = crow[CR_WS + q];
                 float4 U1 = make_float4(0.f, 0.f, 0.f, 0.f), U2 = U1, U3 = U1;
+#ifdef CS_SC_FAT
                 if (kGrad) { U1 = crow[4 + q]; U2 = crow[8 + q]; U3 = crow[16 + q]; }
+#else
+                if (kGrad) U2 = crow[4 + q];
+#endif
                 const float wd[4] = {WD.x, WD.y, WD.z, WD.w}, ws[4] = {WS.x, WS.y, WS.z, WS.w};
-                const float u1[4] = {U1.x, U1.y, U1.z, U1.w}, u2[4] = {U2.x, U2.y, U2.z, U2.w}, u3[4] = {U3.x, U3.y, U3.z, U3.w};
+                float u1[4] = {U1.x, U1.y, U1.z, U1.w}, u3[4] = {U3.x, U3.y, U3.z, U3.w};
+                const float u2[4] = {U2.x, U2.y, U2.z, U2.w};
+#ifndef CS_SC_FAT
+                if (kGrad) {   // the same products the builder formed for the cell's P sums (cs_math.cuh: cell_band)
+#pragma unroll
+                    for (int h = 0; h < 4; ++h)
+                        if (4 * q + h < NF) { u1[h] = mul_(kc.lnd[4 * q + h], wd[h]); u3[h] = mul_(kc.lns[4 * q + h], ws[h]); }
+                }
+#endif
 #pragma unroll
                 for (int h = 0; h < 4; ++h) {
                     const int f = 4 * q + h;
@@ -349,9 +366,9 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
                     }
                 }
             }
-            const float4 S0 = crow[20], S1 = crow[21], S3 = crow[23];
+            const float4 S0 = crow[CR_SC], S1 = crow[CR_SC + 1], S3 = crow[CR_SC + 3];
             float4 S2 = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (kGrad) S2 = crow[22];
+            if (kGrad) S2 = crow[CR_SC + 2];
             CellScal<float> C;
             C.l10 = S0.x; C.l20 = S0.y; C.l21 = S0.z; C.id1 = S0.w; C.id2 = S1.x;
             C.P10 = S1.y; C.P11 = S1.z; C.P12 = S1.w; C.P20 = S2.x; C.P21 = S2.y; C.P22 = S2.z; C.P30 = S2.w;
@@ -363,7 +380,7 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
                 float2 xq = make_float2(0.f, 0.f), xu = xq;
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const float4 WD = crow[q], WS = crow[12 + q];
+                    const float4 WD = crow[q], WS = crow[CR_WS + q];
                     const float wd[4] = {WD.x, WD.y, WD.z, WD.w}, ws[4] = {WS.x, WS.y, WS.z, WS.w};
 #pragma unroll
                     for (int h = 0; h < 4; ++h) {

@@ -31,13 +31,20 @@ __device__ __forceinline__ double exp_pow(double y) {
     return p * __hiloint2double(((int)kf + 1023) << 20, 0);
 }
 
-// One thread per (entry, parameter, band quad): four table values, one 16-byte store.  The band constants come from a
+// What k_tables needs to know about an entry, in one aligned 32-byte load (no chain of dependent loads through the
+// configuration table).
+struct TabEntry {
+    int64_t param_off;   // first parameter of the entry
+    int64_t tab_row;     // first table row of the entry
+    int32_t K0, K1, ktot, pad;
+};
+
+// One thread per (entry, parameter, band quad): four table values and one 16-byte store.  The band constants come from a
 // shared-memory copy (indexed by the thread's quad: a constant-bank read would serialise).
 // grid = (ceil(4 * ktot_max / 256), batch), block = 256.
-__global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const int64_t *__restrict__ param_off,
-                                                const int64_t *__restrict__ tab_off, const int32_t *__restrict__ cfg_of,
-                                                const CfgDev *__restrict__ cfgs, float *__restrict__ tab, int32_t batch,
-                                                int32_t *err, const TConst *__restrict__ tcg, const int32_t *__restrict__ skip) {
+__global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const TabEntry *__restrict__ ents, float *__restrict__ tab,
+                                                int32_t batch, int32_t *err, const TConst *__restrict__ tcg,
+                                                const int32_t *__restrict__ skip) {
     __shared__ TConst tc;
     for (int i = threadIdx.x; i < (int)(sizeof(TConst) / 8); i += blockDim.x)
         reinterpret_cast<double *>(&tc)[i] = reinterpret_cast<const double *>(tcg)[i];
@@ -45,13 +52,13 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
     const int nfreq = tc.nfreq;
     for (int e = blockIdx.y; e < batch; e += gridDim.y) {
         if (skip && skip[e] != 0) continue;
-        const CfgDev *cp = cfgs + cfg_of[e];
-        const int K0 = cp->K[0], K1 = cp->K[1], ktot = cp->ktot;
+        const TabEntry en = ents[e];
+        const int K0 = en.K0, K1 = en.K1, ktot = en.ktot;
         const int id = blockIdx.x * blockDim.x + threadIdx.x;
         const int j = id >> 2, f0 = (id & 3) * 4;
         if (j >= ktot) continue;
-        const double x = params[param_off[e] + j];
-        float *row0 = tab + tab_off[e] * NROW;
+        const double x = params[en.param_off + j];
+        float *row0 = tab + en.tab_row * NROW;
         bool bad = !isfinite(x);
         float v[4];
         if (j < K0) {

@@ -790,3 +790,48 @@ def test_cmb_residual_maps_are_W_applied_to_another_data_set(torch_cuda, path):
         masked = (w.maps[w.cfg_maps[c]] < 0).any(axis=0)
         assert np.all(out[i][:, masked] == 0.0)
     ctx.close()
+
+
+def test_host_constants_against_the_oracle(torch_cuda):
+    """The parameter-independent constants computed on the host (unit factors, log ratios, 1/sum w) against the
+    oracle's own evaluation: u(nu) from orc_krj2kcmb, and the SED at special parameters, where it reduces to them:
+    a_d(nu; beta_d = 1, T -> inf) -> (nu/nu0d) u(nu)/u(nu0d) = cd(nu) and a_s(nu; beta_s = 0) = cs(nu)."""
+    import paper_2604_08463_b200 as cs
+    w = gen.make_config(0)
+    for units in (cs.UNITS_KCMB, cs.UNITS_LITERAL):
+        ctx, _ = make_ctx(w, units=units, options={})
+        k = ctx.model_constants()
+        m = oracle.Model(w.freqs, units=units)
+        for f, nu in enumerate(w.freqs):
+            ud = oracle.krj2kcmb(nu) / oracle.krj2kcmb(353.0) if units == cs.UNITS_KCMB else 1.0
+            us = oracle.krj2kcmb(nu) / oracle.krj2kcmb(23.0) if units == cs.UNITS_KCMB else 1.0
+            assert abs(k["cd"][f] / ((nu / 353.0) * ud) - 1) < 1e-14 and abs(k["cs"][f] / us - 1) < 1e-14
+            assert abs(k["lnd"][f] - np.log(nu / 353.0)) < 1e-15 and abs(k["lns"][f] - np.log(nu / 23.0)) < 1e-15
+            # through the oracle's SED: synchrotron at beta_s = 0 is the unit factor alone; dust at beta_d = 1 in the
+            # Rayleigh-Jeans limit is (nu/nu0) times the unit factor
+            assert abs(oracle.sed_sync(m, nu, 0.0) / k["cs"][f] - 1) < 1e-13
+            assert abs(oracle.sed_dust(m, nu, 1.0, 1e9) / k["cd"][f] - 1) < 1e-7
+        assert abs(k["inv_sum_w"] * float(np.sum(w.ninv.astype(np.float64))) - 1) < 1e-6
+        ctx.close()
+
+
+def test_two_contexts_on_two_devices(torch_cuda):
+    """A context is bound to the device current at cs_create; the kernels' shared-memory attributes are set per device."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    w = gen.make_config(0)
+    params = w.params_jittered(seed=1)
+    res = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            ctx, _ = make_ctx(w, device=f"cuda:{dev}", options={})
+            p = torch.from_numpy(params).to(f"cuda:{dev}")
+            nll = torch.zeros(1, dtype=torch.float64, device=f"cuda:{dev}")
+            grad = torch.zeros_like(p)
+            ctx.build_sed_tables(p)
+            ctx.spectral_like_grad(nll, grad)
+            torch.cuda.synchronize()
+            res.append((nll.cpu().numpy(), grad.cpu().numpy()))
+            ctx.close()
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
