@@ -25,6 +25,10 @@
 namespace cs {
 
 constexpr int CC_NMOM = NROW * (NROW - 1) / 2;   // 120 = 15 * 16 / 2 unique entries of a symmetric 15 x 15 (generic nfreq <= 16: 136 would be needed; see CC_MAXF)
+#ifndef CS_CC_UNROLL
+#define CS_CC_UNROLL 15
+#endif
+constexpr int CC_UNROLL = CS_CC_UNROLL;           // rows of T in flight per thread in k_like_cc
 constexpr int CC_MAXF = 15;                      // f3 is built for nfreq <= 15 (the LiteBIRD-like band set)
 __host__ __device__ __forceinline__ int cc_idx(int f, int g) {   // packed upper triangle of a 15 x 15 symmetric matrix, f <= g
     return f * CC_MAXF - (f * (f - 1)) / 2 + (g - f);
@@ -105,7 +109,11 @@ __global__ void __launch_bounds__(128) k_like_cc(const CfgDev *__restrict__ cfgs
                                                  const int64_t *__restrict__ tab_off, const float *__restrict__ tab,
                                                  const double *__restrict__ mom, KConst kc, int32_t nfreq, int32_t want_grad,
                                                  double *__restrict__ out, int64_t out_stride, int32_t *err) {
-    const int e = blockIdx.y;
+    // the two non-trivial columns of A live in shared memory (one slot per thread, conflict-free): in registers they
+    // cost 60 of them and the kernel ran at 252 registers, latency-bound
+    __shared__ double a1[CC_MAXF][128], a2[CC_MAXF][128];
+    __shared__ float sdgv[CC_MAXF][128];   // dlnG/dT of the cell's T_d cluster
+    const int e = blockIdx.y, tid = threadIdx.x;
     const CellsDev *cl = cells + cfg_of[e];
     const int ncell = cl->ncell;
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -114,41 +122,43 @@ __global__ void __launch_bounds__(128) k_like_cc(const CfgDev *__restrict__ cfgs
     const float *tb = tab + tab_off[e] * NROW;
     const float *rFd = tb + (int64_t)rows.x * NROW, *rG = tb + (int64_t)rows.y * NROW, *rdG = tb + (int64_t)rows.z * NROW,
                 *rFs = tb + (int64_t)rows.w * NROW;
-    double a1[CC_MAXF], a2[CC_MAXF];
     float dg[CC_MAXF];
     // M = A^T N^-1 A and P_th = A^T N^-1 a'_th from the columns (the table values are the fp32 ones the per-pixel path uses)
     double m00 = 0, m01 = 0, m02 = 0, m11 = 0, m12 = 0, m22 = 0;
     double p1[3] = {0, 0, 0}, p2[3] = {0, 0, 0}, p3[3] = {0, 0, 0};
 #pragma unroll
     for (int f = 0; f < CC_MAXF; ++f) {
-        a1[f] = 0.0; a2[f] = 0.0; dg[f] = 0.f;
+        double x1 = 0.0, x2 = 0.0;
+        dg[f] = 0.f;
         if (f < nfreq) {
-            a1[f] = (double)__ldg(rFd + f) * (double)__ldg(rG + f);
-            a2[f] = (double)__ldg(rFs + f);
+            x1 = (double)__ldg(rFd + f) * (double)__ldg(rG + f);
+            x2 = (double)__ldg(rFs + f);
             dg[f] = __ldg(rdG + f);
-            const double wf = (double)kc.w[f], wd = wf * a1[f], ws = wf * a2[f];
-            m00 += wf; m01 += wd; m02 += ws; m11 += wd * a1[f]; m12 += wd * a2[f]; m22 += ws * a2[f];
+            const double wf = (double)kc.w[f], wd = wf * x1, ws = wf * x2;
+            m00 += wf; m01 += wd; m02 += ws; m11 += wd * x1; m12 += wd * x2; m22 += ws * x2;
             const double u1 = (double)kc.lnd[f] * wd, u2 = (double)dg[f] * wd, u3 = (double)kc.lns[f] * ws;
-            p1[0] += u1; p1[1] += u1 * a1[f]; p1[2] += u1 * a2[f];
-            p2[0] += u2; p2[1] += u2 * a1[f]; p2[2] += u2 * a2[f];
-            p3[0] += u3; p3[1] += u3 * a1[f]; p3[2] += u3 * a2[f];
+            p1[0] += u1; p1[1] += u1 * x1; p1[2] += u1 * x2;
+            p2[0] += u2; p2[1] += u2 * x1; p2[2] += u2 * x2;
+            p3[0] += u3; p3[1] += u3 * x1; p3[2] += u3 * x2;
         }
+        a1[f][tid] = x1; a2[f][tid] = x2; sdgv[f][tid] = dg[f];
     }
     // B = A^T T A and V_th = U^T a'_th, row by row of T (u_i[f] = sum_g T_fg a_i[g] is never stored)
     const double *T = mom + mom_off[e] + c;
     double b00 = 0, b01 = 0, b02 = 0, b11 = 0, b12 = 0, b22 = 0;
     double v1[3] = {0, 0, 0}, v2[3] = {0, 0, 0}, v3[3] = {0, 0, 0};
-#pragma unroll
-    for (int f = 0; f < CC_MAXF; ++f) {
+#pragma unroll CC_UNROLL
+    for (int f = 0; f < CC_MAXF; ++f) {   // CS_CC_UNROLL rows of T at a time: 15 loads in flight per row and thread
         double u0 = 0, u1 = 0, u2 = 0;
 #pragma unroll
         for (int g = 0; g < CC_MAXF; ++g) {
             const double t = __ldg(T + (int64_t)(f <= g ? cc_idx(f, g) : cc_idx(g, f)) * ncell);
-            u0 += t; u1 = fma(t, a1[g], u1); u2 = fma(t, a2[g], u2);
+            u0 += t; u1 = fma(t, a1[g][tid], u1); u2 = fma(t, a2[g][tid], u2);
         }
+        const double x1 = a1[f][tid], x2 = a2[f][tid];
         b00 += u0; b01 += u1; b02 += u2;
-        b11 = fma(a1[f], u1, b11); b12 = fma(a1[f], u2, b12); b22 = fma(a2[f], u2, b22);
-        const double d1 = (double)kc.lnd[f] * a1[f], d2 = (double)dg[f] * a1[f], d3 = (double)kc.lns[f] * a2[f];
+        b11 = fma(x1, u1, b11); b12 = fma(x1, u2, b12); b22 = fma(x2, u2, b22);
+        const double d1 = (double)kc.lnd[f] * x1, d2 = (double)sdgv[f][tid] * x1, d3 = (double)kc.lns[f] * x2;
         v1[0] = fma(d1, u0, v1[0]); v1[1] = fma(d1, u1, v1[1]); v1[2] = fma(d1, u2, v1[2]);
         v2[0] = fma(d2, u0, v2[0]); v2[1] = fma(d2, u1, v2[1]); v2[2] = fma(d2, u2, v2[2]);
         v3[0] = fma(d3, u0, v3[0]); v3[1] = fma(d3, u1, v3[1]); v3[2] = fma(d3, u2, v3[2]);
