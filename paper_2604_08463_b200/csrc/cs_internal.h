@@ -41,6 +41,20 @@ constexpr int CR_WS = 8, CR_SC = 12;    // float4 offsets of the w a_s column an
 #endif
 constexpr int SC_CHUNK_CAP = 4 * (TPX / CHUNK_LEN + CELL_CAP);   // sorted layout: most chunks of the four terms of a tile
 constexpr int SC_SEG_CAP = 4 * (TPX / SEG_MAX + CELL_CAP);       // and most segments
+// Tile header of the sorted layout (one per configuration and tile, variable length, a multiple of 16 bytes; 32-bit words):
+//   [0, HDR_META)                meta, indices HM_*
+//   [HDR_META, +HDR_CONS)        per consumer thread two words: cell | r0 << 8 | r1 << 16 | r2 << 24 ; r3   (r_t = half the rank
+//                                of the thread's first position in the tile's (cluster, position) order of term map t)
+//   [.., + 4 ncell)              table rows (Fd', G, dlnG, Fs') of the tile's cells
+//   [HM_OFF_SLOT, + nseg)        slot of every segment in the entry's partial row (terms 0..3 one after the other)
+//   [HM_OFF_CDESC, ..) u16       chunk descriptors: first pair (8 bits) | (pairs-1) << 8 | term << 10
+//   [HM_OFF_SDESC, ..) u16       segment descriptors: first pair | (chunks-1) << 8 | term << 10
+// The loader warp of k_like_sc fetches it with one bulk copy one tile ahead of the other roles, so that a change of
+// tile costs no chain of dependent global loads (a clustering scan changes tile, and configuration, with every entry).
+constexpr int HDR_META = 16, HDR_CONS = 2 * NCONS;
+constexpr int HM_NCELL = 0, HM_NCHUNK = 1, HM_NSEG = 2, HM_CBASE3 = 3, HM_SBASE3 = 4, HM_NSEGREG = 5, HM_SEGBASE3 = 6,
+              HM_OFF_SLOT = 7, HM_OFF_CDESC = 8, HM_OFF_SDESC = 9;
+constexpr int HDR_CAP_WORDS = HDR_META + HDR_CONS + 4 * CELL_CAP + SC_SEG_CAP + SC_CHUNK_CAP / 2 + SC_SEG_CAP / 2 + 4;   // longest header
 constexpr int NORANK = 0xFFFF; // rank of a position that does not take part in a term's reduction
 
 // A pivot of the LDL^T factorisation of M = A^T N^-1 A counts as non-positive (CS_ESINGULAR) when it is below this
@@ -76,11 +90,14 @@ struct CfgDev {
     int32_t sorted;       // 1: sorted layout with private data copies, 0: in place
     int32_t ntile_ring;   // tiles of the in-place layout
     int32_t pad;
+    const int32_t *kseg[4];    // = maps[map[t]].ksegptr: one load less on k_merge's way to its slots
     // sorted layout only
     const uint8_t *cellid;     // [ntile*NCONS] tile-local cell of each thread (position pair)
     const int32_t *cellptr;    // [ntile+1] first cell of each tile
     const int32_t *cellrows;   // [ncell][4] table rows (Fd', G, dlnG, Fs') of the cell inside an entry's table block
     const int32_t *pospix;     // [ntile*TPX] pixel of each position, -1 = pad
+    const uint32_t *hdr;       // tile headers, one after the other
+    const int32_t *hdrptr;     // [ntile+1] start of each tile's header in units of 16 bytes
 };
 
 // A run of work for a fused kernel: `count` entries (elist[estart .. estart+count)) of configuration cfg on each of its
@@ -88,6 +105,8 @@ struct CfgDev {
 struct Run {
     int32_t cfg, estart, count, ntile;
     int64_t ustart;
+    const uint32_t *hdr;       // = cfgs[cfg].hdr, cfgs[cfg].hdrptr (sorted configurations; the loader's look-ahead reads
+    const int32_t *hdrptr;     //   them from the run it already holds instead of chasing the configuration table)
 };
 
 // What the roles of a fused kernel need to know about the entry at position i of the launch's entry list, in one

@@ -50,6 +50,8 @@ struct MapHost {
 
 // Device arrays of one configuration's sorted layout (empty when it stays in place).
 struct SortedHost {
+    uint32_t *hdr = nullptr;
+    int32_t *hdrptr = nullptr;
     uint8_t *cellid = nullptr;
     int32_t *cellptr = nullptr;
     int32_t *cellrows = nullptr;
@@ -121,7 +123,8 @@ struct cs_ctx {
     std::vector<CopyJob> jobs;          // private copies of the sorted layout, ordered by data set
     int32_t *d_cfg_of = nullptr, *d_data_of = nullptr, *d_elist = nullptr;
     int64_t *d_param_off = nullptr, *d_tab_off = nullptr;
-    TabEntry *d_tabent = nullptr;
+    TabBlock *d_tabblk = nullptr;      // k_tables' work list: 64-parameter blocks of every entry
+    int64_t ntabblk = 0;
     PosInfo *d_pinfo = nullptr;
     Run *d_runs = nullptr;
     CopyJob *d_jobs = nullptr;
@@ -175,7 +178,7 @@ void free_clusters(cs_ctx *c) {
         cudaFree(m.chunkptr); cudaFree(m.segcfirst);
     }
     c->maps.clear();
-    for (auto &p : c->sorted) { cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); cudaFree(p.pospix); }
+    for (auto &p : c->sorted) { cudaFree(p.hdr); cudaFree(p.hdrptr); cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); cudaFree(p.pospix); }
     c->sorted.clear();
     for (auto &p : c->cellsh) {
         cudaFree(p.cellpos); cudaFree(p.celllen); cudaFree(p.cellreg);
@@ -199,10 +202,10 @@ void free_opt(cs_ctx *c) {
 
 void free_batch(cs_ctx *c) {
     cudaFree(c->d_cfg_of); cudaFree(c->d_data_of); cudaFree(c->d_elist);
-    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_tabent); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
+    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_tabblk); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
     cudaFree(c->d_tab); cudaFree(c->d_partial); cudaFree(c->d_copy);
     c->d_cfg_of = c->d_data_of = c->d_elist = nullptr;
-    c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr; c->d_tabent = nullptr;
+    c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr; c->d_tabblk = nullptr; c->ntabblk = 0;
     c->d_runs = nullptr; c->d_jobs = nullptr;
     c->d_tab = nullptr; c->d_partial = nullptr; c->d_copy = nullptr;
     c->batch = 0; c->nrun_sc = c->nrun_dir = 0; c->batch_bytes = 0; c->copy_bytes = 0;
@@ -228,7 +231,11 @@ double krj2kcmb(double nu_ghz, double tcmb, double hk) {
 
 // Reduction plan of one term map in position space: per tile the rank of every position in the (cluster, position)
 // order, that order cut into segments of <= SEG_MAX positions of one cluster, plus the CSR cluster -> segments.
-int build_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, MapHost *out, int64_t *bytes) {
+struct MapPlanHost {   // host copies of what the tile headers of the sorted layout are packed from
+    std::vector<uint16_t> rank, segdesc, segcfirst;
+    std::vector<int32_t> segptr, segslot, chunkptr;
+};
+int build_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, MapHost *out, int64_t *bytes, MapPlanHost *keep = nullptr) {
     std::vector<uint16_t> rank((size_t)ntile * TPX, (uint16_t)NORANK);
     std::vector<int32_t> segptr(ntile + 1, 0);
     std::vector<uint16_t> segdesc;
@@ -292,6 +299,10 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, M
     if ((rc = dev_upload(&out->ksegptr, ksegptr, bytes))) return rc;
     if ((rc = dev_upload(&out->chunkptr, chunkptr, bytes))) return rc;
     if ((rc = dev_upload(&out->segcfirst, segcfirst, bytes))) return rc;
+    if (keep) {
+        keep->rank.swap(rank); keep->segdesc.swap(segdesc); keep->segcfirst.swap(segcfirst);
+        keep->segptr.swap(segptr); keep->segslot.swap(segslot); keep->chunkptr.swap(chunkptr);
+    }
     return CS_OK;
 }
 
@@ -385,6 +396,62 @@ void plan_sorted(const int32_t *i0, const int32_t *i1, const int32_t *i2, const 
     }
     sp.ntile = (int32_t)sp.cellptr.size() - 1;
     sp.fill = (double)px.size() / ((double)sp.ntile * TPX);
+}
+
+// Tile headers of one sorted configuration (cs_internal.h "tile header"): everything the roles of k_like_sc need to
+// know about a tile, packed so that the loader warp fetches it with one bulk copy one tile ahead.
+void pack_tile_headers(const SortedPlan &sp, const MapPlanHost (&mp)[4], const int32_t segbase[4], int32_t nseg_region,
+                       std::vector<int32_t> &hdrptr, std::vector<uint32_t> &blob) {
+    hdrptr.assign(sp.ntile + 1, 0);
+    blob.clear();
+    for (int32_t tile = 0; tile < sp.ntile; ++tile) {
+        const size_t base = blob.size();   // in 32-bit words
+        hdrptr[tile] = (int32_t)(base / 4);
+        const int32_t c0 = sp.cellptr[tile], ncell = sp.cellptr[tile + 1] - c0;
+        int32_t nchunk[4], nseg[4], ctot = 0, stot = 0;
+        for (int t = 0; t < 4; ++t) {
+            nchunk[t] = mp[t].chunkptr[tile + 1] - mp[t].chunkptr[tile];
+            nseg[t] = mp[t].segptr[tile + 1] - mp[t].segptr[tile];
+            ctot += nchunk[t]; stot += nseg[t];
+        }
+        const int32_t off_cells = HDR_META + HDR_CONS;                      // words
+        const int32_t off_slot = off_cells + 4 * ncell;
+        const int32_t off_cdesc = off_slot + stot;                          // u16 arrays, packed two per word
+        const int32_t off_sdesc = off_cdesc + (ctot + 1) / 2;
+        const int32_t total = (off_sdesc + (stot + 1) / 2 + 3) & ~3;        // multiple of 16 bytes
+        blob.resize(base + total, 0u);
+        uint32_t *h = blob.data() + base;
+        h[HM_NCELL] = (uint32_t)ncell; h[HM_NCHUNK] = (uint32_t)ctot; h[HM_NSEG] = (uint32_t)stot;
+        h[HM_CBASE3] = (uint32_t)(ctot - nchunk[3]); h[HM_SBASE3] = (uint32_t)(stot - nseg[3]);
+        h[HM_NSEGREG] = (uint32_t)nseg_region; h[HM_SEGBASE3] = (uint32_t)segbase[3];
+        h[HM_OFF_SLOT] = (uint32_t)off_slot; h[HM_OFF_CDESC] = (uint32_t)off_cdesc; h[HM_OFF_SDESC] = (uint32_t)off_sdesc;
+        for (int tid = 0; tid < NCONS; ++tid) {
+            const size_t pos = (size_t)tile * TPX + 2 * tid;
+            uint32_t r[4];
+            for (int t = 0; t < 4; ++t) r[t] = (uint32_t)(mp[t].rank[pos] >> 1) & 0xffu;
+            h[HDR_META + 2 * tid] = (uint32_t)sp.cellid[(size_t)tile * NCONS + tid] | (r[0] << 8) | (r[1] << 16) | (r[2] << 24);
+            h[HDR_META + 2 * tid + 1] = r[3];
+        }
+        for (int32_t q = 0; q < 4 * ncell; ++q) h[off_cells + q] = (uint32_t)sp.cellrows[(size_t)4 * c0 + q];
+        uint16_t *cdesc = reinterpret_cast<uint16_t *>(h + off_cdesc), *sdesc = reinterpret_cast<uint16_t *>(h + off_sdesc);
+        int32_t sb = 0, cb = 0;
+        for (int t = 0; t < 4; ++t) {   // the same plan sc_load_plan used to assemble per tile in the kernel
+            const int32_t s0 = mp[t].segptr[tile];
+            for (int32_t i = 0; i < nseg[t]; ++i) {
+                const uint32_t desc = mp[t].segdesc[s0 + i];
+                const int start = desc & 0x1ff, len = (int)(desc >> 9) + 1;
+                const int first = cb + mp[t].segcfirst[s0 + i], cnt = (len + CHUNK_LEN - 1) / CHUNK_LEN;
+                sdesc[sb + i] = (uint16_t)((start >> 1) | ((cnt - 1) << 8) | (t << 10));
+                h[off_slot + sb + i] = (uint32_t)(segbase[t] + mp[t].segslot[s0 + i]);
+                for (int q = 0; q < cnt; ++q) {
+                    const int l = std::min(CHUNK_LEN, len - CHUNK_LEN * q);
+                    cdesc[first + q] = (uint16_t)(((start + CHUNK_LEN * q) >> 1) | ((l / 2 - 1) << 8) | (t << 10));
+                }
+            }
+            sb += nseg[t]; cb += nchunk[t];
+        }
+    }
+    hdrptr[sp.ntile] = (int32_t)(blob.size() / 4);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -720,6 +787,9 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     c->cellsh.resize(ncfg);
     c->npix_live.assign((size_t)ncfg * nregion, 0);
     SortedPlan sp;
+    MapPlanHost mplan[4];
+    std::vector<int32_t> hdrptr;
+    std::vector<uint32_t> hdrblob;
     for (int32_t i = 0; i < ncfg; ++i) {
         CfgDev &cf = c->cfgs[i];
         std::memset(&cf, 0, sizeof(cf));
@@ -748,7 +818,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
                 const int64_t npos = (int64_t)sp.ntile * TPX;
                 for (int t = 0; t < 4; ++t) {
                     c->maps.emplace_back();
-                    if ((rc = build_map_plan(sp.idx[t].data(), t < 3 ? cf.K[t] : nregion, npos, sp.ntile, &c->maps.back(), &c->cluster_bytes))) {
+                    if ((rc = build_map_plan(sp.idx[t].data(), t < 3 ? cf.K[t] : nregion, npos, sp.ntile, &c->maps.back(), &c->cluster_bytes, &mplan[t]))) {
                         free_clusters(c);
                         return rc;
                     }
@@ -784,7 +854,17 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
         int32_t off = 0;
         for (int t = 0; t < 4; ++t) {
             cf.segbase[t] = off;
+            cf.kseg[t] = c->maps[cf.map[t]].ksegptr;
             off += c->maps[cf.map[t]].nseg;
+        }
+        if (cf.sorted) {   // tile headers (they hold the slots, hence after segbase)
+            pack_tile_headers(sp, mplan, cf.segbase, c->maps[cf.map[3]].nseg, hdrptr, hdrblob);
+            SortedHost &sh = c->sorted[i];
+            if ((rc = dev_upload(&sh.hdr, hdrblob, &c->cluster_bytes)) || (rc = dev_upload(&sh.hdrptr, hdrptr, &c->cluster_bytes))) {
+                free_clusters(c);
+                return rc;
+            }
+            cf.hdr = sh.hdr; cf.hdrptr = sh.hdrptr;
         }
     }
     std::vector<MapDev> md(c->maps.size());
@@ -866,7 +946,7 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         while (j < batch && cfg_of[c->elist[j]] == cfg_of[c->elist[i]]) ++j;
         const CfgDev &cf = c->cfgs[cfg_of[c->elist[i]]];
         const bool sc = is_sc(c->elist[i]);
-        Run r{cfg_of[c->elist[i]], i, j - i, cf.ntile, sc ? c->W_sc : c->W_dir};
+        Run r{cfg_of[c->elist[i]], i, j - i, cf.ntile, sc ? c->W_sc : c->W_dir, cf.hdr, cf.hdrptr};
         const int64_t units = (int64_t)cf.ntile * (j - i);
         if (sc) { c->W_sc += units; c->nrun_sc++; } else { c->W_dir += units; c->nrun_dir++; }
         c->runs.push_back(r);
@@ -911,13 +991,15 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         }
         if (copy_bytes > limit) { free_batch(c); return CS_ENOMEM; }
     }
-    std::vector<TabEntry> tabent(batch);
+    std::vector<TabBlock> tabblk;
     for (int32_t e = 0; e < batch; ++e) {
         const CfgDev &cf = c->cfgs[cfg_of[e]];
-        tabent[e] = TabEntry{c->param_off[e], tab_off[e], cf.K[0], cf.K[1], cf.ktot, 0};
+        for (int32_t j0 = 0; j0 < cf.ktot; j0 += TAB_ROWS_PER_BLOCK)
+            tabblk.push_back(TabBlock{c->param_off[e], tab_off[e], cf.K[0], cf.K[1], cf.ktot, j0, e, {0, 0, 0}});
     }
+    c->ntabblk = (int64_t)tabblk.size();
     int rc;
-    if ((rc = dev_upload(&c->d_tabent, tabent, &c->batch_bytes)) ||
+    if ((rc = dev_upload(&c->d_tabblk, tabblk, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_cfg_of, c->cfg_of, &c->batch_bytes)) || (rc = dev_upload(&c->d_data_of, c->data_of, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_elist, c->elist, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_param_off, c->param_off, &c->batch_bytes)) || (rc = dev_upload(&c->d_tab_off, tab_off, &c->batch_bytes)) ||
@@ -956,9 +1038,8 @@ int cs_param_offsets(cs_ctx *c, int64_t *off) {
 int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
     if (!c || c->batch <= 0 || !params) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    dim3 block(256);
-    dim3 grid((4 * c->ktot_max + 255) / 256, std::min(c->batch, 65535));
-    k_tables<<<grid, block, 0, st>>>(params, c->d_tabent, c->d_tab, c->batch, c->d_err, c->d_tc, c->skip);
+    if (c->ntabblk > 0)
+        k_tables<<<(unsigned)c->ntabblk, 256, 0, st>>>(params, c->d_tabblk, c->d_tab, c->d_err, c->d_tc, c->skip);
     c->launches++;
     CK(cudaGetLastError());
     c->tables_built = true;
@@ -1031,7 +1112,7 @@ static int maps_impl(cs_ctx *c, int32_t nsel, const int32_t *entries, const int3
         const int32_t cf = c->cfg_of[hs[i]];
         int32_t j = i;
         while (j < nsel && c->cfg_of[hs[j]] == cf) ++j;
-        hr[nrun++] = Run{cf, i, j - i, c->ntile_ring, W};
+        hr[nrun++] = Run{cf, i, j - i, c->ntile_ring, W, nullptr, nullptr};
         W += (int64_t)c->ntile_ring * (j - i);
         i = j;
     }
@@ -1301,7 +1382,7 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
                 while (e2 < b && c->data_of[c->elist[e2]] < n1) ++e2;
                 if (e2 == a) continue;
                 int64_t &W = sc ? Wsc[ch] : Wdir[ch];
-                out[cnt_sc[ch] + cnt_dir[ch]] = Run{run.cfg, a, e2 - a, run.ntile, W};
+                out[cnt_sc[ch] + cnt_dir[ch]] = Run{run.cfg, a, e2 - a, run.ntile, W, run.hdr, run.hdrptr};
                 W += (int64_t)run.ntile * (e2 - a);
                 (sc ? cnt_sc[ch] : cnt_dir[ch])++;
             }

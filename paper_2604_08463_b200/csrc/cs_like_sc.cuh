@@ -26,9 +26,13 @@
 //                           rows of its next entry to L1, because under a saturated HBM stream the L2 round trip of a
 //                           cell's four table rows takes about as long as a whole entry
 //   warp  13     loader   : one 60-KB bulk copy per entry into the data ring (two stages: measured, a deeper ring
-//                           adds nothing once the consumers release a stage as soon as it is read)
+//                           adds nothing once the consumers release a stage as soon as it is read), and one bulk copy
+//                           per tile of the tile's header (cs_internal.h) into the header ring, one tile ahead: what the
+//                           other roles need to know about a tile (cell of every thread, ranks, cell rows, reducer plan)
+//                           is in shared memory before they get there, so a change of tile costs no dependent global
+//                           load -- a clustering scan (config 3) changes tile and configuration with every entry
 // shared memory: data ring [ND][2 halves][2*NF][256] | cell tables [NC][CELL_CAP][CROW] | term ring [NT][4][256] fp64 |
-//                reducer plans | barriers
+//                header ring [NH][HDR_CAP_WORDS] | barriers
 #pragma once
 #include "cs_pipe.cuh"
 #include "cs_math.cuh"
@@ -49,49 +53,27 @@ constexpr int SC_NBW = CS_SC_NBW; // builder warps (warp b takes the entries n =
 constexpr int SC_NT = 2;        // term ring depth = reducer warps
 constexpr int SC_THREADS = NCONS + (SC_NT + SC_NBW + 1) * 32;   // 448
 constexpr int SC_WARP_RED = NCONS / 32, SC_WARP_BUILD = SC_WARP_RED + SC_NT, SC_WARP_LOAD = SC_WARP_BUILD + SC_NBW;
-constexpr int SC_PLAN_BYTES = SC_CHUNK_CAP * 2 + SC_SEG_CAP * 2 + SC_SEG_CAP * 4 + 16;   // one reducer warp's plan
+constexpr int SC_NH = 4;        // header ring depth: the header of tile i+1 is fetched while tile i is worked on, into the
+                                // slot tile i-3 used, which every role has left by then
+constexpr int SC_HDR_USERS = NCONS / 32 + SC_NBW + SC_NT;   // warps that read a header and hand its slot back
 
 template <int NF>
 constexpr size_t sc_smem_bytes() {
     return (size_t)ScDepth<NF>::value * 2 * NF * TPX * 4   // data ring
            + (size_t)SC_NC * CELL_CAP * CROW * 4       // cell tables
            + (size_t)SC_NT * 4 * NCONS * 8             // term ring (fp64 pair sums)
-           + (size_t)SC_NT * SC_PLAN_BYTES             // reducer plans (one copy per reducer warp)
-           + (2 * ScDepth<NF>::value + 2 * SC_NC + SC_NT) * 8   // mbarriers
+           + (size_t)SC_NH * HDR_CAP_WORDS * 4         // header ring
+           + (2 * ScDepth<NF>::value + 2 * SC_NC + SC_NT + 2 * SC_NH) * 8   // mbarriers
            + 16;
 }
 
-// Reducer plan of a tile: every (term, cluster) segment of <= SEG_MAX rank-ordered terms is cut into 1..4 chunks of
-// <= CHUNK_LEN ranks.  In the sorted layout all starts and lengths are even; the plan is kept in pairs:
-// s_cdesc[chunk] = first pair (8 bits) | (pairs-1) << 8 | term << 10;
-// s_sdesc[segment] = first pair (8 bits) | (chunks-1) << 8 | term << 10; s_slot[segment] = slot in the entry's partial row.
-template <int MODE>
-__device__ __forceinline__ void sc_load_plan(const MapDev *__restrict__ maps, const CfgDev &cfg, int tile, int lane,
-                                             uint16_t *s_cdesc, uint16_t *s_sdesc, int32_t *s_slot, int32_t *meta) {
-    constexpr int T0 = ModeTraits<MODE>::region_only ? 3 : 0;
-    int sbase = 0, cbase = 0;
-#pragma unroll
-    for (int t = T0; t < 4; ++t) {
-        const MapDev m = maps[(MODE == MODE_CMBVAR) ? cfg.map[3] : cfg.map[t]];
-        const int s0 = m.segptr[tile], ns = m.segptr[tile + 1] - s0;
-        const int nc = m.chunkptr[tile + 1] - m.chunkptr[tile];
-        for (int i = lane; i < ns; i += 32) {
-            const uint32_t desc = m.segdesc[s0 + i];
-            const int start = desc & 0x1ff, len = (int)(desc >> 9) + 1;
-            const int first = cbase + m.segcfirst[s0 + i], cnt = (len + CHUNK_LEN - 1) / CHUNK_LEN;
-            s_sdesc[sbase + i] = (uint16_t)((start >> 1) | ((cnt - 1) << 8) | (t << 10));
-            s_slot[sbase + i] = ((MODE == MODE_CMBVAR) ? t * m.nseg : cfg.segbase[t]) + m.segslot[s0 + i];
-            for (int q = 0; q < cnt; ++q) {
-                const int l = min(CHUNK_LEN, len - CHUNK_LEN * q);
-                s_cdesc[first + q] = (uint16_t)(((start + CHUNK_LEN * q) >> 1) | ((l / 2 - 1) << 8) | (t << 10));
-            }
-        }
-        sbase += ns; cbase += nc;
-    }
-    if (lane == 0) { meta[0] = cbase; meta[1] = sbase; }
-    __syncwarp();
-}
-
+// Reducer plan of a tile (part of its header): every (term, cluster) segment of <= SEG_MAX rank-ordered terms is cut
+// into 1..4 chunks of <= CHUNK_LEN ranks.  In the sorted layout all starts and lengths are even; the plan is kept in pairs:
+// cdesc[chunk] = first pair (8 bits) | (pairs-1) << 8 | term << 10;
+// sdesc[segment] = first pair (8 bits) | (chunks-1) << 8 | term << 10; slot[segment] = slot in the entry's partial row.
+// Modes that reduce only the region term use the part of the plan that belongs to term 3; MODE_CMBVAR reduces four
+// terms that all follow the region map: term 3's part with the term replaced and the slots re-based.
+//
 // First level of the ordered reduction (a3) of one entry by a reducer warp, in fp64 and in a fixed order:
 // step 1, one lane per chunk: (y0 + y1) + (y2 + y3) over the chunk's <= 4 pair sums (cs_math.cuh: chunk_tree), left in
 // place of the chunk's first pair sum; step 2, one lane per segment: the segment's chunk sums left to right, stored at
@@ -112,13 +94,32 @@ __device__ __forceinline__ double sc_segment(const double *tbuf, uint32_t d) {
     if (cnt > 3) acc += y[3 * CHUNK_LEN / 2];
     return acc;
 }
-__device__ __forceinline__ void sc_reduce_entry(double *tbuf, int lane, const int32_t *meta, const uint16_t *s_cdesc,
-                                                const uint16_t *s_sdesc, const int32_t *s_slot, double *__restrict__ prow) {
-    const int nchunk = meta[0], nseg = meta[1];
+template <int MODE>
+__device__ __forceinline__ void sc_reduce_entry(double *tbuf, int lane, const uint32_t *h, double *__restrict__ prow) {
+    constexpr bool kTerm3 = ModeTraits<MODE>::region_only || MODE == MODE_CMBVAR;
+    constexpr bool kRep = MODE == MODE_CMBVAR;
+    const uint16_t *cdesc = reinterpret_cast<const uint16_t *>(h + h[HM_OFF_CDESC]);
+    const uint16_t *sdesc = reinterpret_cast<const uint16_t *>(h + h[HM_OFF_SDESC]);
+    const int32_t *slot = reinterpret_cast<const int32_t *>(h + h[HM_OFF_SLOT]);
+    const int c_lo = kTerm3 ? (int)h[HM_CBASE3] : 0, s_lo = kTerm3 ? (int)h[HM_SBASE3] : 0;
+    const int ncr = (int)h[HM_NCHUNK] - c_lo, nsr = (int)h[HM_NSEG] - s_lo;
+    const int nsegreg = (int)h[HM_NSEGREG], segbase3 = (int)h[HM_SEGBASE3];
+    auto chunk_desc = [&](int r) -> uint32_t {
+        if (!kRep) return cdesc[c_lo + r];
+        const int rep = r / ncr;
+        return (uint32_t)(cdesc[c_lo + r - rep * ncr] & 0x3ff) | ((uint32_t)rep << 10);
+    };
+    auto seg_desc = [&](int r, int &sl) -> uint32_t {
+        if (!kRep) { sl = slot[s_lo + r]; return sdesc[s_lo + r]; }
+        const int rep = r / nsr, i = r - rep * nsr;
+        sl = rep * nsegreg + (slot[s_lo + i] - segbase3);
+        return (uint32_t)(sdesc[s_lo + i] & 0x3ff) | ((uint32_t)rep << 10);
+    };
+    const int nchunk = (kRep ? 4 : 1) * ncr, nseg = (kRep ? 4 : 1) * nsr;
     for (int r = lane; r < nchunk; r += 64) {
         int a0, a1 = 0;
         const bool two = r + 32 < nchunk;
-        const uint32_t d0 = s_cdesc[r], d1 = two ? s_cdesc[r + 32] : 0u;
+        const uint32_t d0 = chunk_desc(r), d1 = two ? chunk_desc(r + 32) : 0u;
         const double c0 = sc_chunk(tbuf, d0, a0);
         double c1 = 0.0;
         if (two) c1 = sc_chunk(tbuf, d1, a1);
@@ -128,8 +129,8 @@ __device__ __forceinline__ void sc_reduce_entry(double *tbuf, int lane, const in
     __syncwarp();
     for (int r = lane; r < nseg; r += 64) {
         const bool two = r + 32 < nseg;
-        const uint32_t d0 = s_sdesc[r], d1 = two ? s_sdesc[r + 32] : 0u;
-        const int slot0 = s_slot[r], slot1 = two ? s_slot[r + 32] : 0;
+        int slot0 = 0, slot1 = 0;
+        const uint32_t d0 = seg_desc(r, slot0), d1 = two ? seg_desc(r + 32, slot1) : 0u;
         const double v0 = sc_segment(tbuf, d0);
         double v1 = 0.0;
         if (two) v1 = sc_segment(tbuf, d1);
@@ -137,6 +138,64 @@ __device__ __forceinline__ void sc_reduce_entry(double *tbuf, int lane, const in
         if (two) prow[slot1] = v1;
     }
     __syncwarp();
+}
+
+// Loader of the sorted-cell kernel (one lane): walks the CTA's pieces (a tile and a range of entries of one run); for
+// piece i it first sends off the header of piece i+1, then asks for the header range of piece i+2 (a load whose result
+// is not needed before the next round), then streams the entries of piece i into the data ring.
+template <int NF, int ND>
+__device__ __forceinline__ void sc_loader(const LikeParams &P, float *ring, uint32_t *hdr, uint64_t *full_d, uint64_t *empty_d,
+                                          uint64_t *full_h, uint64_t *empty_h) {
+    constexpr int STAGE = 2 * NF * TPX;   // floats per stage
+    const int nrows = 2 * P.nfreq;
+    const uint64_t policy = P.evict_first ? policy_evict_first() : policy_evict_normal();
+    const uint64_t keep = policy_evict_normal();
+    auto hdr_range = [](const Walk &x) { return make_int2(__ldg(x.run.hdrptr + x.tile), __ldg(x.run.hdrptr + x.tile + 1)); };
+    auto send_header = [&](int ip, const Walk &x, int2 hr) {
+        const int s = ip % SC_NH;
+        mbar_wait(&empty_h[s], (uint32_t)(((ip / SC_NH) & 1) ^ 1));
+        const uint32_t bytes = (uint32_t)(hr.y - hr.x) * 16u;
+        mbar_expect_tx(&full_h[s], bytes);
+        bulk_g2s(hdr + s * HDR_CAP_WORDS, x.run.hdr + (int64_t)hr.x * 4, bytes, &full_h[s], keep);
+    };
+    Walk w0, w1, w2;   // pieces i, i+1, i+2
+    walk_init(w0, P);
+    if (!walk_next(w0, P)) return;
+    w1 = w0;
+    bool ok1 = walk_next(w1, P);
+    int2 h1 = make_int2(0, 0);
+    send_header(0, w0, hdr_range(w0));
+    if (ok1) h1 = hdr_range(w1);
+    int n = 0;   // live entries so far
+    for (int ip = 0;; ++ip) {
+        bool ok2 = false;
+        int2 h2 = make_int2(0, 0);
+        if (ok1) {
+            send_header(ip + 1, w1, h1);
+            w2 = w1;
+            ok2 = walk_next(w2, P);
+            if (ok2) h2 = hdr_range(w2);
+        }
+        for (int k = w0.k; k < w0.kend; ++k) {
+            const int64_t srcinfo = __ldg(&P.pinfo[w0.run.estart + k].src);
+            if (P.skip && __ldg(P.skip + __ldg(P.elist + w0.run.estart + k)) != 0) continue;
+            const int s = n % ND;
+            float *dst = ring + s * STAGE;
+            mbar_wait(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1));
+            const uint32_t bytes = (uint32_t)nrows * TPX * 4u;
+            mbar_expect_tx(&full_d[s], bytes);
+            const float *src = P.dcopy + srcinfo + (int64_t)w0.tile * nrows * TPX;
+            if (NF * 2 == nrows) {
+                bulk_g2s(dst, src, bytes, &full_d[s], policy);
+            } else {   // generic band count: the stage keeps 2*NF rows per half, the copy only 2*nfreq
+                bulk_g2s(dst, src, bytes / 2, &full_d[s], policy);
+                bulk_g2s(dst + NF * 2 * HALF, src + nrows * HALF, bytes / 2, &full_d[s], policy);
+            }
+            ++n;
+        }
+        if (!ok1) break;
+        w0 = w1; w1 = w2; ok1 = ok2; h1 = h2;
+    }
 }
 
 // One cell (Eq. 2 columns -> five weighted columns, M, LDL^T, P; cs_math.cuh) from the entry's four table rows.
@@ -194,10 +253,11 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
     float *ring = reinterpret_cast<float *>(smem_raw);
     float *cells = ring + ND * STAGE;
     double *sterm = reinterpret_cast<double *>(cells + NC * CELL_CAP * CROW);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(sterm + NT * 4 * NCONS);
+    uint32_t *hdr = reinterpret_cast<uint32_t *>(sterm + NT * 4 * NCONS);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(hdr + SC_NH * HDR_CAP_WORDS);
     uint64_t *full_d = bars, *empty_d = bars + ND, *full_c = bars + 2 * ND, *empty_c = bars + 2 * ND + NC;
     uint64_t *empty_t = bars + 2 * ND + 2 * NC;
-    unsigned char *plans = reinterpret_cast<unsigned char *>(empty_t + NT);
+    uint64_t *full_h = empty_t + NT, *empty_h = full_h + SC_NH;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
@@ -206,6 +266,7 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
         for (int s = 0; s < ND; ++s) { mbar_init(&full_d[s], 1); mbar_init(&empty_d[s], NCONS / 32); }
         for (int s = 0; s < NC; ++s) { mbar_init(&full_c[s], 1); mbar_init(&empty_c[s], NCONS / 32); }
         for (int s = 0; s < NT; ++s) mbar_init(&empty_t[s], 1);
+        for (int s = 0; s < SC_NH; ++s) { mbar_init(&full_h[s], 1); mbar_init(&empty_h[s], SC_HDR_USERS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (NF * 2 != 2 * P.nfreq) {   // generic band count: rows beyond nfreq are never copied; they must read as zero
@@ -214,23 +275,28 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
     __syncthreads();
 
     if (warp == SC_WARP_LOAD) {
-        loader_loop<NF, ND>(nullptr, P, ring, full_d, empty_d, lane);
+        if (lane == 0) sc_loader<NF, ND>(P, ring, hdr, full_d, empty_d, full_h, empty_h);
         return;
     }
     Walk w;
     walk_init(w, P);
-    int n = 0;   // live entries so far (ring slots and barrier phases follow it)
+    int n = 0;    // live entries so far (ring slots and barrier phases follow it)
+    int ip = 0;   // pieces so far (header ring slot and phase)
 
     if (warp >= SC_WARP_BUILD) {
         // ---------------- builder warps: lane c builds the cells c and c + 32 of the current tile; warp b takes the
         // entries n = b (mod SC_NBW)
         static_assert(CELL_CAP == 64, "two cells per builder lane");
         const int mine = warp - SC_WARP_BUILD;
-        while (walk_next(w, P)) {
-            const CfgDev *cf = P.cfgs + w.run.cfg;
-            const int c0 = __ldg(cf->cellptr + w.tile), ncell = __ldg(cf->cellptr + w.tile + 1) - c0;
-            const int4 rows0 = (lane < ncell) ? __ldg(reinterpret_cast<const int4 *>(cf->cellrows) + c0 + lane) : make_int4(0, 0, 0, 0);
-            const int4 rows1 = (lane + 32 < ncell) ? __ldg(reinterpret_cast<const int4 *>(cf->cellrows) + c0 + lane + 32) : make_int4(0, 0, 0, 0);
+        for (; walk_next(w, P); ++ip) {
+            const uint32_t *hd = hdr + (ip % SC_NH) * HDR_CAP_WORDS;
+            mbar_wait(&full_h[ip % SC_NH], (uint32_t)((ip / SC_NH) & 1));
+            const int ncell = (int)hd[HM_NCELL];
+            const int4 *hrows = reinterpret_cast<const int4 *>(hd + HDR_META + HDR_CONS);
+            const int4 rows0 = (lane < ncell) ? hrows[lane] : make_int4(0, 0, 0, 0);
+            const int4 rows1 = (lane + 32 < ncell) ? hrows[lane + 32] : make_int4(0, 0, 0, 0);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_h[ip % SC_NH]);
             for (int k = w.k; k < w.kend; ++k) {
                 const int64_t tab_row = __ldg(&P.pinfo[w.run.estart + k].tab_row);
                 if (P.skip && __ldg(P.skip + __ldg(P.elist + w.run.estart + k)) != 0) continue;
@@ -280,24 +346,21 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
     if (warp >= SC_WARP_RED) {
         // ---------------- reducer warps: first level of a3; warp r takes the entries n = r (mod NT) ----------------
         const int mine = warp - SC_WARP_RED;
-        unsigned char *pl = plans + mine * SC_PLAN_BYTES;   // this warp's own copy of the tile's plan
-        int32_t *s_slot = reinterpret_cast<int32_t *>(pl);
-        int32_t *meta = s_slot + SC_SEG_CAP;
-        uint16_t *s_cdesc = reinterpret_cast<uint16_t *>(meta + 4);
-        uint16_t *s_sdesc = s_cdesc + SC_CHUNK_CAP;
-        while (walk_next(w, P)) {
-            const CfgDev cf = P.cfgs[w.run.cfg];
-            sc_load_plan<MODE>(P.maps, cf, w.tile, lane, s_cdesc, s_sdesc, s_slot, meta);
+        for (; walk_next(w, P); ++ip) {
+            const uint32_t *h = hdr + (ip % SC_NH) * HDR_CAP_WORDS;   // the tile's plan is used in place
+            mbar_wait(&full_h[ip % SC_NH], (uint32_t)((ip / SC_NH) & 1));
             for (int k = w.k; k < w.kend; ++k) {
                 const int e = __ldg(P.elist + w.run.estart + k);
                 if (P.skip && __ldg(P.skip + e) != 0) continue;
                 const int s = n % NT;
                 if (s != mine) { ++n; continue; }
                 named_sync(1 + s, NCONS + 32);
-                sc_reduce_entry(sterm + s * 4 * NCONS, lane, meta, s_cdesc, s_sdesc, s_slot, P.partial + (int64_t)e * P.PS);
+                sc_reduce_entry<MODE>(sterm + s * 4 * NCONS, lane, h, P.partial + (int64_t)e * P.PS);
                 if (lane == 0) mbar_arrive(&empty_t[s]);
                 ++n;
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty_h[ip % SC_NH]);
         }
         return;
     }
@@ -305,25 +368,19 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
     // ---------------- consumers ----------------
     const float *st0 = ring + (tid >> 7) * (2 * NF * HALF) + ((2 * tid) & (HALF - 1));
     const KConst &kc = P.kc;
-    while (walk_next(w, P)) {
-        const CfgDev *cf = P.cfgs + w.run.cfg;
-        const int cell = __ldg(cf->cellid + (int64_t)w.tile * NCONS + tid);
-        // slot of this thread's pair sums in each term row: half the rank of its first position
-        int so0 = 0, so1 = 0, so2 = 0, so3 = 0;
-        {
-            const int64_t pos = (int64_t)w.tile * TPX + 2 * tid;
-            const int m3 = cf->map[3];
-            if (MODE == MODE_CMBVAR) {
-                const int r = __ldg(P.maps[m3].rank + pos) >> 1;
-                so0 = r; so1 = NCONS + r; so2 = 2 * NCONS + r; so3 = 3 * NCONS + r;
-            } else {
-                if (kGrad) {
-                    so0 = __ldg(P.maps[cf->map[0]].rank + pos) >> 1;
-                    so1 = NCONS + (__ldg(P.maps[cf->map[1]].rank + pos) >> 1);
-                    so2 = 2 * NCONS + (__ldg(P.maps[cf->map[2]].rank + pos) >> 1);
-                }
-                so3 = 3 * NCONS + (__ldg(P.maps[m3].rank + pos) >> 1);
-            }
+    for (; walk_next(w, P); ++ip) {
+        // this thread's cell and the slots of its pair sums in the four term rows (half the rank of its first position)
+        mbar_wait(&full_h[ip % SC_NH], (uint32_t)((ip / SC_NH) & 1));
+        const uint2 ci = reinterpret_cast<const uint2 *>(hdr + (ip % SC_NH) * HDR_CAP_WORDS + HDR_META)[tid];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_h[ip % SC_NH]);
+        const int cell = (int)(ci.x & 0xff);
+        int so0, so1, so2, so3;
+        if (MODE == MODE_CMBVAR) {
+            so0 = (int)ci.y; so1 = NCONS + (int)ci.y; so2 = 2 * NCONS + (int)ci.y; so3 = 3 * NCONS + (int)ci.y;
+        } else {
+            so0 = (int)((ci.x >> 8) & 0xff); so1 = NCONS + (int)((ci.x >> 16) & 0xff); so2 = 2 * NCONS + (int)(ci.x >> 24);
+            so3 = 3 * NCONS + (int)ci.y;
         }
         for (int k = w.k; k < w.kend; ++k) {
             const int e = __ldg(P.elist + w.run.estart + k);

@@ -31,66 +31,83 @@ __device__ __forceinline__ double exp_pow(double y) {
     return p * __hiloint2double(((int)kf + 1023) << 20, 0);
 }
 
-// What k_tables needs to know about an entry, in one aligned 32-byte load (no chain of dependent loads through the
-// configuration table).
-struct TabEntry {
+// 1/a for a normal positive double: MUFU.RCP64H seed (about 20 bits) and two Newton steps (error ~1 ulp, no slow path).
+__device__ __forceinline__ double rcp_pos(double a) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+    double e = fma(-a, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-a, r, 1.0);
+    return fma(r, e, r);
+}
+// expm1(x): for x >= 1/32 the subtraction exp(x) - 1 loses at most five bits of the 6e-15 of exp_pow; smaller (and
+// non-positive or non-finite) arguments take the library routine.
+__device__ __forceinline__ double expm1_pos(double x) { return (x >= 0.03125 && x < 700.0) ? exp_pow(x) - 1.0 : expm1(x); }
+
+// One block of k_tables' work: 64 consecutive parameters [j0, j0 + 64) of entry e, in one aligned 48-byte record
+// (no chain of dependent loads through the configuration table, and no block without work).
+struct TabBlock {
     int64_t param_off;   // first parameter of the entry
     int64_t tab_row;     // first table row of the entry
-    int32_t K0, K1, ktot, pad;
+    int32_t K0, K1, ktot, j0;
+    int32_t e, pad[3];
 };
+constexpr int TAB_ROWS_PER_BLOCK = 64;
 
 // One thread per (entry, parameter, band quad): four table values and one 16-byte store.  The band constants come from a
-// shared-memory copy (indexed by the thread's quad: a constant-bank read would serialise).
-// grid = (ceil(4 * ktot_max / 256), batch), block = 256.
-__global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const TabEntry *__restrict__ ents, float *__restrict__ tab,
-                                                int32_t batch, int32_t *err, const TConst *__restrict__ tcg,
-                                                const int32_t *__restrict__ skip) {
+// shared-memory copy (indexed by the thread's quad: a constant-bank read would serialise); the parameter load is issued
+// before the copy is staged.  grid = number of 64-parameter blocks of the batch, block = 256.
+__global__ void __launch_bounds__(256) k_tables(const double *__restrict__ params, const TabBlock *__restrict__ blocks, float *__restrict__ tab,
+                                                int32_t *err, const TConst *__restrict__ tcg, const int32_t *__restrict__ skip) {
     __shared__ TConst tc;
+    const int4 *bp = reinterpret_cast<const int4 *>(blocks + blockIdx.x);
+    const int4 b0 = __ldg(bp), b1 = __ldg(bp + 1), b2 = __ldg(bp + 2);
+    const int64_t param_off = ((int64_t)(uint32_t)b0.y << 32) | (uint32_t)b0.x, tab_row = ((int64_t)(uint32_t)b0.w << 32) | (uint32_t)b0.z;
+    const int K0 = b1.x, K1 = b1.y, ktot = b1.z, j0 = b1.w, e = b2.x;
+    if (skip && skip[e] != 0) return;
+    const int j = j0 + (threadIdx.x >> 2), f0 = (threadIdx.x & 3) * 4;
+    const bool live = j < ktot;
+    const double x = live ? __ldg(params + param_off + j) : 1.0;
     for (int i = threadIdx.x; i < (int)(sizeof(TConst) / 8); i += blockDim.x)
         reinterpret_cast<double *>(&tc)[i] = reinterpret_cast<const double *>(tcg)[i];
     __syncthreads();
+    if (!live) return;
     const int nfreq = tc.nfreq;
-    for (int e = blockIdx.y; e < batch; e += gridDim.y) {
-        if (skip && skip[e] != 0) continue;
-        const TabEntry en = ents[e];
-        const int K0 = en.K0, K1 = en.K1, ktot = en.ktot;
-        const int id = blockIdx.x * blockDim.x + threadIdx.x;
-        const int j = id >> 2, f0 = (id & 3) * 4;
-        if (j >= ktot) continue;
-        const double x = params[en.param_off + j];
-        float *row0 = tab + en.tab_row * NROW;
-        bool bad = !isfinite(x);
-        float v[4];
-        if (j < K0) {
-            // dust power-law factor with the band constant folded in: cd[f] * (nu_f/nu0d)^beta_d
+    float *row0 = tab + tab_row * NROW;
+    bool bad = !isfinite(x);
+    float v[4];
+    if (j < K0) {
+        // dust power-law factor with the band constant folded in: cd[f] * (nu_f/nu0d)^beta_d
 #pragma unroll
-            for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cd[f0 + i] * exp_pow(x * tc.lnd[f0 + i])) : 0.f;
-            *reinterpret_cast<float4 *>(row0 + (int64_t)j * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
-        } else if (j < K0 + K1) {
-            // Planck ratio G = expm1(x0)/expm1(x) and d ln G / dT = (1/T) [ x/(1-e^-x) - x0/(1-e^-x0) ]
-            bad = bad || !(x > 0.0);
-            const int k = j - K0;
-            float dg[4];
-            const double x0 = tc.hk * tc.nu0d / x, e0 = expm1(x0), h0 = x0 / (-expm1(-x0));
+        for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cd[f0 + i] * exp_pow(x * tc.lnd[f0 + i])) : 0.f;
+        *reinterpret_cast<float4 *>(row0 + (int64_t)j * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+    } else if (j < K0 + K1) {
+        // Planck ratio G = expm1(x0)/expm1(x) and d ln G / dT = (1/T) [ h(x) - h(x0) ],
+        // h(x) = x / (1 - e^-x) = x + x / expm1(x): one expm1 and one reciprocal per band
+        bad = bad || !(x > 0.0);
+        const int k = j - K0;
+        float dg[4];
+        const double inv_t = 1.0 / x;
+        const double x0 = tc.hk * tc.nu0d * inv_t, e0 = expm1_pos(x0), h0 = fma(x0, rcp_pos(e0), x0);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                v[i] = 0.f; dg[i] = 0.f;
-                if (f0 + i < nfreq) {
-                    const double xf = tc.hk * tc.nu[f0 + i] / x;
-                    v[i] = (float)(e0 / expm1(xf));
-                    dg[i] = (float)((xf / (-expm1(-xf)) - h0) / x);
-                }
+        for (int i = 0; i < 4; ++i) {
+            v[i] = 0.f; dg[i] = 0.f;
+            if (f0 + i < nfreq) {
+                const double xf = tc.hk * tc.nu[f0 + i] * inv_t;
+                const double re = rcp_pos(expm1_pos(xf));
+                v[i] = (float)(e0 * re);
+                dg[i] = (float)((fma(xf, re, xf) - h0) * inv_t);
             }
-            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
-            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + K1 + k) * NROW + f0) = make_float4(dg[0], dg[1], dg[2], dg[3]);
-        } else {
-            const int k = j - K0 - K1;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cs[f0 + i] * exp_pow(x * tc.lns[f0 + i])) : 0.f;
-            *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + 2 * K1 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
         }
-        if (bad && f0 == 0) atomicOr(err, ERR_DOMAIN);
+        *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+        *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + K1 + k) * NROW + f0) = make_float4(dg[0], dg[1], dg[2], dg[3]);
+    } else {
+        const int k = j - K0 - K1;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cs[f0 + i] * exp_pow(x * tc.lns[f0 + i])) : 0.f;
+        *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + 2 * K1 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
     }
+    if (bad && f0 == 0) atomicOr(err, ERR_DOMAIN);
 }
 
 // ----------------------------------------------------------------------------------------------------------
@@ -101,6 +118,9 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
 // Cluster outputs (short slot ranges): one thread each, slots added in ascending order.  Region outputs (one slot per
 // tile): one warp each, lane l adds the slots a+l, a+l+32, ... in ascending order and the 32 lane sums are combined by a
 // fixed xor-shuffle tree.  Both orders are fixed, so the result is bitwise reproducible.
+// (Measured alternatives, both slower on every configuration: eight lanes per cluster -- eight times the threads, each
+// with the same chain of pointer loads in front of one or two slots; warp-cooperative sums of the long ranges only --
+// a warp full of T_d clusters then walks them one after the other.)
 // Virtual thread index v: [0, ktot) clusters, [ktot_pad + 32 r, +32) region r.  grid = (ceil(nvirt_max/256), batch).
 __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
                                                const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
@@ -118,18 +138,18 @@ __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partia
         if (v < K0) { t = 0; k = v; }
         else if (v < K0 + K1) { t = 1; k = v - K0; }
         else { t = 2; k = v - K0 - K1; }
-        const int32_t *ksegptr = maps[c->map[t]].ksegptr;
+        const int32_t *ksegptr = c->kseg[t];
         const double *row = erow + c->segbase[t];
-        const int a = ksegptr[k], b = ksegptr[k + 1];
+        const int a = __ldg(ksegptr + k), b = __ldg(ksegptr + k + 1);
         double acc = 0.0;
-#pragma unroll 4
+#pragma unroll 8
         for (int q = a; q < b; ++q) acc += row[q];
         grad[param_off[e] + v] = acc;
     } else if (v >= kpad && (v - kpad) >> 5 < nregion) {
         const int r = (v - kpad) >> 5;
-        const int32_t *ksegptr = maps[c->map[3]].ksegptr;
+        const int32_t *ksegptr = c->kseg[3];
         const double *row = erow + c->segbase[3];
-        const int a = ksegptr[r], b = ksegptr[r + 1];
+        const int a = __ldg(ksegptr + r), b = __ldg(ksegptr + r + 1);
         double acc = 0.0;
 #pragma unroll 4
         for (int q = a + lane; q < b; q += 32) acc += row[q];
