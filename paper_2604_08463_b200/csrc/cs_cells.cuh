@@ -104,16 +104,16 @@ __global__ void __launch_bounds__(128) k_cc_moments(const float *__restrict__ d,
 
 // One (entry, cell): nll term and the three gradient terms from the cell's moments, in fp64.
 // grid = (ceil(ncell_max / 128), batch), block = 128.  out[e] = [4][ncell_max] (ll, g_beta_d, g_T_d, g_beta_s).
-__global__ void __launch_bounds__(128) k_like_cc(const CfgDev *__restrict__ cfgs, const CellsDev *__restrict__ cells,
-                                                 const int32_t *__restrict__ cfg_of, const int64_t *__restrict__ mom_off,
-                                                 const int64_t *__restrict__ tab_off, const float *__restrict__ tab,
-                                                 const double *__restrict__ mom, KConst kc, int32_t nfreq, int32_t want_grad,
-                                                 double *__restrict__ out, int64_t out_stride, int32_t *err) {
-    // the two non-trivial columns of A live in shared memory (one slot per thread, conflict-free): in registers they
-    // cost 60 of them and the kernel ran at 252 registers, latency-bound
-    __shared__ double a1[CC_MAXF][128], a2[CC_MAXF][128];
-    __shared__ float sdgv[CC_MAXF][128];   // dlnG/dT of the cell's T_d cluster
-    const int e = blockIdx.y, tid = threadIdx.x;
+// Every unique moment T_fg is loaded once (coalesced over the cells of a warp) and used for both rows it belongs to:
+// u_i[f] += T_fg a_i[g], u_i[g] += T_fg a_i[f].  The loops are fully unrolled so that u_0, u_1, u_2 and the two
+// non-trivial columns of A (75 doubles) stay in registers; the contractions with u come first, the sums that need only
+// the columns (M, P) after u is dead, which keeps the kernel below 255 registers without spills.
+__global__ void __launch_bounds__(128, 2) k_like_cc(const CfgDev *__restrict__ cfgs, const CellsDev *__restrict__ cells,
+                                                    const int32_t *__restrict__ cfg_of, const int64_t *__restrict__ mom_off,
+                                                    const int64_t *__restrict__ tab_off, const float *__restrict__ tab,
+                                                    const double *__restrict__ mom, KConst kc, int32_t nfreq, int32_t want_grad,
+                                                    double *__restrict__ out, int64_t out_stride, int32_t *err) {
+    const int e = blockIdx.y;
     const CellsDev *cl = cells + cfg_of[e];
     const int ncell = cl->ncell;
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -122,46 +122,81 @@ __global__ void __launch_bounds__(128) k_like_cc(const CfgDev *__restrict__ cfgs
     const float *tb = tab + tab_off[e] * NROW;
     const float *rFd = tb + (int64_t)rows.x * NROW, *rG = tb + (int64_t)rows.y * NROW, *rdG = tb + (int64_t)rows.z * NROW,
                 *rFs = tb + (int64_t)rows.w * NROW;
-    float dg[CC_MAXF];
-    // M = A^T N^-1 A and P_th = A^T N^-1 a'_th from the columns (the table values are the fp32 ones the per-pixel path uses)
+    // the two non-trivial columns of A (the table values are the fp32 ones the per-pixel path uses); zero beyond nfreq
+    double a1[CC_MAXF], a2[CC_MAXF];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 fd = __ldg(reinterpret_cast<const float4 *>(rFd) + q), g = __ldg(reinterpret_cast<const float4 *>(rG) + q),
+                     fs = __ldg(reinterpret_cast<const float4 *>(rFs) + q);
+        const float vfd[4] = {fd.x, fd.y, fd.z, fd.w}, vg[4] = {g.x, g.y, g.z, g.w}, vfs[4] = {fs.x, fs.y, fs.z, fs.w};
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            const int f = 4 * q + h;
+            if (f < CC_MAXF) {
+                a1[f] = (f < nfreq) ? (double)vfd[h] * (double)vg[h] : 0.0;
+                a2[f] = (f < nfreq) ? (double)vfs[h] : 0.0;
+            }
+        }
+    }
+    // u_i = T a_i (a_0 = 1) from the 120 unique moments
+    const double *T = mom + mom_off[e] + c;
+    double u0[CC_MAXF], u1[CC_MAXF], u2[CC_MAXF];
+#pragma unroll
+    for (int f = 0; f < CC_MAXF; ++f) {
+        const double t = __ldg(T + (int64_t)cc_idx(f, f) * ncell);
+        u0[f] = t; u1[f] = t * a1[f]; u2[f] = t * a2[f];
+    }
+#pragma unroll
+    for (int f = 0; f < CC_MAXF; ++f) {
+#pragma unroll
+        for (int g = f + 1; g < CC_MAXF; ++g) {
+            const double t = __ldg(T + (int64_t)cc_idx(f, g) * ncell);
+            u0[f] += t; u0[g] += t;
+            u1[f] = fma(t, a1[g], u1[f]); u1[g] = fma(t, a1[f], u1[g]);
+            u2[f] = fma(t, a2[g], u2[f]); u2[g] = fma(t, a2[f], u2[g]);
+        }
+    }
+    // B = A^T T A and V_th = U^T a'_th
+    double b00 = 0, b01 = 0, b02 = 0, b11 = 0, b12 = 0, b22 = 0;
+    double v1[3] = {0, 0, 0}, v2[3] = {0, 0, 0}, v3[3] = {0, 0, 0};
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 dg4 = __ldg(reinterpret_cast<const float4 *>(rdG) + q);
+        const float vdg[4] = {dg4.x, dg4.y, dg4.z, dg4.w};
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            const int f = 4 * q + h;
+            if (f < CC_MAXF) {
+                const double x1 = a1[f], x2 = a2[f];
+                b00 += u0[f]; b01 += u1[f]; b02 += u2[f];
+                b11 = fma(x1, u1[f], b11); b12 = fma(x1, u2[f], b12); b22 = fma(x2, u2[f], b22);
+                const double d1 = (double)kc.lnd[f] * x1, d2 = (double)vdg[h] * x1, d3 = (double)kc.lns[f] * x2;
+                v1[0] = fma(d1, u0[f], v1[0]); v1[1] = fma(d1, u1[f], v1[1]); v1[2] = fma(d1, u2[f], v1[2]);
+                v2[0] = fma(d2, u0[f], v2[0]); v2[1] = fma(d2, u1[f], v2[1]); v2[2] = fma(d2, u2[f], v2[2]);
+                v3[0] = fma(d3, u0[f], v3[0]); v3[1] = fma(d3, u1[f], v3[1]); v3[2] = fma(d3, u2[f], v3[2]);
+            }
+        }
+    }
+    // M = A^T N^-1 A and P_th = A^T N^-1 a'_th from the columns
     double m00 = 0, m01 = 0, m02 = 0, m11 = 0, m12 = 0, m22 = 0;
     double p1[3] = {0, 0, 0}, p2[3] = {0, 0, 0}, p3[3] = {0, 0, 0};
 #pragma unroll
-    for (int f = 0; f < CC_MAXF; ++f) {
-        double x1 = 0.0, x2 = 0.0;
-        dg[f] = 0.f;
-        if (f < nfreq) {
-            x1 = (double)__ldg(rFd + f) * (double)__ldg(rG + f);
-            x2 = (double)__ldg(rFs + f);
-            dg[f] = __ldg(rdG + f);
-            const double wf = (double)kc.w[f], wd = wf * x1, ws = wf * x2;
-            m00 += wf; m01 += wd; m02 += ws; m11 += wd * x1; m12 += wd * x2; m22 += ws * x2;
-            const double u1 = (double)kc.lnd[f] * wd, u2 = (double)dg[f] * wd, u3 = (double)kc.lns[f] * ws;
-            p1[0] += u1; p1[1] += u1 * x1; p1[2] += u1 * x2;
-            p2[0] += u2; p2[1] += u2 * x1; p2[2] += u2 * x2;
-            p3[0] += u3; p3[1] += u3 * x1; p3[2] += u3 * x2;
-        }
-        a1[f][tid] = x1; a2[f][tid] = x2; sdgv[f][tid] = dg[f];
-    }
-    // B = A^T T A and V_th = U^T a'_th, row by row of T (u_i[f] = sum_g T_fg a_i[g] is never stored)
-    const double *T = mom + mom_off[e] + c;
-    double b00 = 0, b01 = 0, b02 = 0, b11 = 0, b12 = 0, b22 = 0;
-    double v1[3] = {0, 0, 0}, v2[3] = {0, 0, 0}, v3[3] = {0, 0, 0};
-#pragma unroll CC_UNROLL
-    for (int f = 0; f < CC_MAXF; ++f) {   // CS_CC_UNROLL rows of T at a time: 15 loads in flight per row and thread
-        double u0 = 0, u1 = 0, u2 = 0;
+    for (int q = 0; q < 4; ++q) {
+        const float4 dg4 = __ldg(reinterpret_cast<const float4 *>(rdG) + q);
+        const float vdg[4] = {dg4.x, dg4.y, dg4.z, dg4.w};
 #pragma unroll
-        for (int g = 0; g < CC_MAXF; ++g) {
-            const double t = __ldg(T + (int64_t)(f <= g ? cc_idx(f, g) : cc_idx(g, f)) * ncell);
-            u0 += t; u1 = fma(t, a1[g][tid], u1); u2 = fma(t, a2[g][tid], u2);
+        for (int h = 0; h < 4; ++h) {
+            const int f = 4 * q + h;
+            if (f < CC_MAXF) {
+                const double x1 = a1[f], x2 = a2[f];
+                const double wf = (double)kc.w[f], wd = wf * x1, ws = wf * x2;
+                m00 += wf; m01 += wd; m02 += ws; m11 += wd * x1; m12 += wd * x2; m22 += ws * x2;
+                const double q1 = (double)kc.lnd[f] * wd, q2 = (double)vdg[h] * wd, q3 = (double)kc.lns[f] * ws;
+                p1[0] += q1; p1[1] += q1 * x1; p1[2] += q1 * x2;
+                p2[0] += q2; p2[1] += q2 * x1; p2[2] += q2 * x2;
+                p3[0] += q3; p3[1] += q3 * x1; p3[2] += q3 * x2;
+            }
         }
-        const double x1 = a1[f][tid], x2 = a2[f][tid];
-        b00 += u0; b01 += u1; b02 += u2;
-        b11 = fma(x1, u1, b11); b12 = fma(x1, u2, b12); b22 = fma(x2, u2, b22);
-        const double d1 = (double)kc.lnd[f] * x1, d2 = (double)sdgv[f][tid] * x1, d3 = (double)kc.lns[f] * x2;
-        v1[0] = fma(d1, u0, v1[0]); v1[1] = fma(d1, u1, v1[1]); v1[2] = fma(d1, u2, v1[2]);
-        v2[0] = fma(d2, u0, v2[0]); v2[1] = fma(d2, u1, v2[1]); v2[2] = fma(d2, u2, v2[2]);
-        v3[0] = fma(d3, u0, v3[0]); v3[1] = fma(d3, u1, v3[1]); v3[2] = fma(d3, u2, v3[2]);
     }
     // M^-1 by cofactors (3 x 3 symmetric positive definite; cond ~ 5, R11)
     const double c00 = m11 * m22 - m12 * m12, c01 = m02 * m12 - m01 * m22, c02 = m01 * m12 - m02 * m11;
@@ -188,34 +223,75 @@ __global__ void __launch_bounds__(128) k_like_cc(const CfgDev *__restrict__ cfgs
     }
 }
 
-// Ordered sums of the per-cell terms onto clusters (grad) and regions (nll): thread = one output of one entry,
-// cells in ascending order.  grid = (ceil((ktot_max + nregion) / 128), batch), block = 128.
+// Ordered sums of the per-cell terms onto clusters (grad) and regions (nll).  A cluster with at most CC_LONG cells: one
+// thread, cells in ascending order.  Longer lists (every region; the clusters of maps with a handful of patches) are
+// summed by a whole block: thread i adds the cells i, i+128, ... of the list in ascending order, the 32 lane sums of a
+// warp are combined by a fixed xor-shuffle tree and the four warp sums left to right.  Which way a cluster goes depends
+// on its cell count only: deterministic and independent of the batch.
+// grid = (ceil(ktot_max / 128) [cluster blocks, want_grad only] + nregion [region blocks], batch), block = 128.
+constexpr int CC_LONG = 64;
+__device__ __forceinline__ double cc_block_sum(const double *__restrict__ src, const int32_t *__restrict__ list, int a, int b, double *wsum) {
+    double acc = 0.0;
+#pragma unroll 8
+    for (int q = a + (int)threadIdx.x; q < b; q += 128) acc += src[__ldg(list + q)];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    __syncthreads();   // wsum is free again
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    return ((wsum[0] + wsum[1]) + wsum[2]) + wsum[3];
+}
 __global__ void __launch_bounds__(128) k_cc_reduce(const CfgDev *__restrict__ cfgs, const CellsDev *__restrict__ cells,
                                                    const int32_t *__restrict__ cfg_of, const int64_t *__restrict__ param_off,
                                                    const double *__restrict__ out, int64_t out_stride, int32_t nregion,
                                                    int32_t want_grad, double *__restrict__ nll, double *__restrict__ grad) {
+    __shared__ double wsum[4];
+    __shared__ int32_t s_long[128][3];   // (first, end, term) of this block's long clusters, by thread
+    __shared__ int32_t s_who[128], s_nlong;
     const int e = blockIdx.y;
     const CfgDev *cf = cfgs + cfg_of[e];
     const CellsDev *cl = cells + cfg_of[e];
-    const int v = blockIdx.x * blockDim.x + threadIdx.x;
     const double *o = out + (int64_t)e * out_stride;
     const int64_t cs_ = out_stride / 4;
-    const int ktot = want_grad ? cf->ktot : 0;
-    int t, k;
-    if (v < ktot) {
-        if (v < cf->K[0]) { t = 0; k = v; }
-        else if (v < cf->K[0] + cf->K[1]) { t = 1; k = v - cf->K[0]; }
-        else { t = 2; k = v - cf->K[0] - cf->K[1]; }
-    } else if (v - ktot < nregion) {
-        t = 3; k = v - ktot;
+    const int nblk_cluster = (int)gridDim.x - nregion;
+    if ((int)blockIdx.x < nblk_cluster) {
+        const int ktot = cf->ktot;
+        if ((int)(blockIdx.x * blockDim.x) >= ktot) return;   // block-uniform
+        if (threadIdx.x == 0) s_nlong = 0;
+        __syncthreads();
+        const int v = blockIdx.x * blockDim.x + threadIdx.x;
+        const int64_t dst0 = param_off[e] + (int64_t)blockIdx.x * blockDim.x;
+        if (v < ktot) {
+            int t, k;
+            if (v < cf->K[0]) { t = 0; k = v; }
+            else if (v < cf->K[0] + cf->K[1]) { t = 1; k = v - cf->K[0]; }
+            else { t = 2; k = v - cf->K[0] - cf->K[1]; }
+            const int a = __ldg(cl->kptr[t] + k), b = __ldg(cl->kptr[t] + k + 1);
+            if (b - a <= CC_LONG) {
+                const double *src = o + (int64_t)(t + 1) * cs_;
+                const int32_t *list = cl->klist[t];
+                double acc = 0.0;
+#pragma unroll 8
+                for (int q = a; q < b; ++q) acc += src[__ldg(list + q)];
+                grad[dst0 + threadIdx.x] = acc;
+            } else {
+                s_long[threadIdx.x][0] = a; s_long[threadIdx.x][1] = b; s_long[threadIdx.x][2] = t;
+                s_who[atomicAdd(&s_nlong, 1)] = threadIdx.x;
+            }
+        }
+        __syncthreads();
+        const int nlong = s_nlong;
+        for (int i = 0; i < nlong; ++i) {   // in any order: every sum is on its own
+            const int who = s_who[i], t = s_long[who][2];
+            const double tot = cc_block_sum(o + (int64_t)(t + 1) * cs_, cl->klist[t], s_long[who][0], s_long[who][1], wsum);
+            if (threadIdx.x == 0) grad[dst0 + who] = tot;
+        }
     } else {
-        return;
+        const int r = (int)blockIdx.x - nblk_cluster;
+        const int a = __ldg(cl->kptr[3] + r), b = __ldg(cl->kptr[3] + r + 1);
+        const double tot = cc_block_sum(o, cl->klist[3], a, b, wsum);
+        if (threadIdx.x == 0) nll[(int64_t)e * nregion + r] = tot;
     }
-    const double *src = o + (t == 3 ? 0 : (int64_t)(t + 1) * cs_);
-    double acc = 0.0;
-    for (int q = cl->kptr[t][k]; q < cl->kptr[t][k + 1]; ++q) acc += src[cl->klist[t][q]];
-    if (t == 3) nll[(int64_t)e * nregion + k] = acc;
-    else grad[param_off[e] + v] = acc;
 }
 
 }  // namespace cs

@@ -1049,8 +1049,7 @@ int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
 static int merge_launch(cs_ctx *c, double *nll, double *grad, cudaStream_t st) {
     for (int e0 = 0; e0 < c->batch; e0 += 65535) {
         const int nb = std::min(65535, c->batch - e0);
-        const int nout = (grad ? ((c->ktot_max + 31) & ~31) : 0) + 32 * c->nregion;   // virtual threads, see k_merge
-        dim3 grid((nout + 255) / 256, nb);
+        dim3 grid((grad ? (c->ktot_max + 255) / 256 : 0) + c->nregion, nb);   // cluster blocks, then one block per region
         k_merge<<<grid, 256, 0, st>>>(c->d_partial + (int64_t)e0 * c->PS, c->PS, c->d_maps, c->d_cfgs, c->d_cfg_of + e0,
                                      c->d_param_off + e0, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad,
                                      c->skip ? c->skip + e0 : nullptr);
@@ -1193,7 +1192,7 @@ int cs_spectral_like_grad_cells(cs_ctx *c, double *nll, double *grad, void *stre
         dim3 g1((c->ncell_max + 127) / 128, nb);
         k_like_cc<<<g1, 128, 0, st>>>(c->d_cfgs, c->d_cells, c->d_cfg_of + e0, c->d_mom_off + e0, c->d_tab_off + e0, c->d_tab, c->d_mom, c->kc,
                                       c->nfreq, grad ? 1 : 0, c->d_ccout + (int64_t)e0 * c->cc_out_stride, c->cc_out_stride, c->d_err);
-        dim3 g2(((grad ? c->ktot_max : 0) + c->nregion + 127) / 128, nb);
+        dim3 g2((grad ? (c->ktot_max + 127) / 128 : 0) + c->nregion, nb);   // cluster blocks, then one block per region
         k_cc_reduce<<<g2, 128, 0, st>>>(c->d_cfgs, c->d_cells, c->d_cfg_of + e0, c->d_param_off + e0, c->d_ccout + (int64_t)e0 * c->cc_out_stride,
                                         c->cc_out_stride, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad);
         c->launches += 2;

@@ -115,47 +115,83 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
 // which are contiguous in the partial row.
 // want_grad = 0: only the region outputs.
 // ----------------------------------------------------------------------------------------------------------
-// Cluster outputs (short slot ranges): one thread each, slots added in ascending order.  Region outputs (one slot per
-// tile): one warp each, lane l adds the slots a+l, a+l+32, ... in ascending order and the 32 lane sums are combined by a
-// fixed xor-shuffle tree.  Both orders are fixed, so the result is bitwise reproducible.
-// (Measured alternatives, both slower on every configuration: eight lanes per cluster -- eight times the threads, each
-// with the same chain of pointer loads in front of one or two slots; warp-cooperative sums of the long ranges only --
-// a warp full of T_d clusters then walks them one after the other.)
-// Virtual thread index v: [0, ktot) clusters, [ktot_pad + 32 r, +32) region r.  grid = (ceil(nvirt_max/256), batch).
+// Cluster outputs with at most MERGE_LONG slots (nearly all): one thread each, slots added in ascending order.  Longer
+// ranges -- the region outputs (sixteen slots per tile: thousands per entry) and the clusters of a map with a handful
+// of patches (K = 1 in the clustering scan: one cluster owns every slot of its term) -- are summed by a whole block:
+// thread i adds the slots a+i, a+i+256, ... in ascending order, the 32 lane sums of a warp are combined by a fixed
+// xor-shuffle tree and the eight warp sums left to right.  Which way a cluster goes depends on its slot count only, and
+// all orders are fixed, so the result is bitwise reproducible and independent of the batch.
+// (Measured alternatives for the short clusters, both slower on every configuration: eight lanes per cluster -- eight
+// times the threads, each with the same chain of pointer loads in front of one or two slots; warp-cooperative sums from
+// 16 slots on -- a warp full of T_d clusters then walks them one after the other.  One thread per long range was the
+// long pole of the whole kernel: 1536 dependent adds for a K = 1 map, 192 rounds of loads per lane for a region at nside 128.)
+// grid = (ceil(ktot_max / 256) [cluster blocks, want_grad only] + nregion [region blocks], batch), block = 256.
+constexpr int MERGE_LONG = 64;
+__device__ __forceinline__ double merge_block_sum(const double *__restrict__ row, int a, int b, double *wsum) {
+    double acc = 0.0;
+#pragma unroll 8
+    for (int q = a + (int)threadIdx.x; q < b; q += 256) acc += row[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    __syncthreads();   // wsum is free again
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    double tot = wsum[0];
+#pragma unroll
+    for (int i = 1; i < 8; ++i) tot += wsum[i];
+    return tot;
+}
 __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
                                                const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
                                                const int64_t *__restrict__ param_off, int32_t nregion, int32_t want_grad,
                                                double *__restrict__ nll, double *__restrict__ grad, const int32_t *__restrict__ skip) {
-    const int e = blockIdx.y, lane = threadIdx.x & 31;
+    __shared__ double wsum[8];
+    __shared__ int32_t s_long[256][3];   // (a, b, offset of the term's block in the row) of this block's long clusters, by thread
+    __shared__ int32_t s_who[256], s_nlong;
+    const int e = blockIdx.y;
     if (skip && skip[e] != 0) return;
     const CfgDev *c = cfgs + cfg_of[e];
-    const int K0 = c->K[0], K1 = c->K[1], ktot = want_grad ? c->ktot : 0;
-    const int kpad = (ktot + 31) & ~31;
-    const int v = blockIdx.x * blockDim.x + threadIdx.x;
     const double *erow = partial + (int64_t)e * PS;
-    if (v < ktot) {
-        int t, k;
-        if (v < K0) { t = 0; k = v; }
-        else if (v < K0 + K1) { t = 1; k = v - K0; }
-        else { t = 2; k = v - K0 - K1; }
-        const int32_t *ksegptr = c->kseg[t];
-        const double *row = erow + c->segbase[t];
-        const int a = __ldg(ksegptr + k), b = __ldg(ksegptr + k + 1);
-        double acc = 0.0;
+    const int nblk_cluster = (int)gridDim.x - nregion;
+    if ((int)blockIdx.x < nblk_cluster) {
+        const int K0 = c->K[0], K1 = c->K[1], ktot = c->ktot;
+        if ((int)(blockIdx.x * blockDim.x) >= ktot) return;   // block-uniform
+        if (threadIdx.x == 0) s_nlong = 0;
+        __syncthreads();
+        const int v = blockIdx.x * blockDim.x + threadIdx.x;
+        const int64_t dst0 = param_off[e] + (int64_t)blockIdx.x * blockDim.x;
+        if (v < ktot) {
+            int t, k;
+            if (v < K0) { t = 0; k = v; }
+            else if (v < K0 + K1) { t = 1; k = v - K0; }
+            else { t = 2; k = v - K0 - K1; }
+            const int32_t *ksegptr = c->kseg[t];
+            const int base = c->segbase[t];
+            const int a = __ldg(ksegptr + k), b = __ldg(ksegptr + k + 1);
+            if (b - a <= MERGE_LONG) {
+                const double *row = erow + base;
+                double acc = 0.0;
 #pragma unroll 8
-        for (int q = a; q < b; ++q) acc += row[q];
-        grad[param_off[e] + v] = acc;
-    } else if (v >= kpad && (v - kpad) >> 5 < nregion) {
-        const int r = (v - kpad) >> 5;
+                for (int q = a; q < b; ++q) acc += row[q];
+                grad[dst0 + threadIdx.x] = acc;
+            } else {
+                s_long[threadIdx.x][0] = a; s_long[threadIdx.x][1] = b; s_long[threadIdx.x][2] = base;
+                s_who[atomicAdd(&s_nlong, 1)] = threadIdx.x;
+            }
+        }
+        __syncthreads();
+        const int nlong = s_nlong;
+        for (int i = 0; i < nlong; ++i) {   // in any order: every sum is on its own
+            const int who = s_who[i];
+            const double tot = merge_block_sum(erow + s_long[who][2], s_long[who][0], s_long[who][1], wsum);
+            if (threadIdx.x == 0) grad[dst0 + who] = tot;
+        }
+    } else {
+        const int r = (int)blockIdx.x - nblk_cluster;
         const int32_t *ksegptr = c->kseg[3];
-        const double *row = erow + c->segbase[3];
         const int a = __ldg(ksegptr + r), b = __ldg(ksegptr + r + 1);
-        double acc = 0.0;
-#pragma unroll 4
-        for (int q = a + lane; q < b; q += 32) acc += row[q];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if (lane == 0) nll[(int64_t)e * nregion + r] = acc;
+        const double tot = merge_block_sum(erow + c->segbase[3], a, b, wsum);
+        if (threadIdx.x == 0) nll[(int64_t)e * nregion + r] = tot;
     }
 }
 
