@@ -64,6 +64,35 @@ def test_recovers_known_optimum_on_noiseless_cluster_constant_sky():
     assert L + 0.5 * dNd < 1e-3 * abs(hist[0] + 0.5 * dNd)      # misfit reduced by > 1000x towards the noiseless optimum 0
 
 
+def test_reaches_the_bounded_minimum_an_independent_solver_finds():
+    # The result of a5 is the bound-constrained minimiser of the spectral likelihood: scipy's L-BFGS-B (an independent
+    # implementation of bounded minimisation, run to convergence on the same oracle objective) must find the same
+    # minimum, on a noisy sky with tight bounds so that several parameters end pinned ("reaches the same
+    # minimum as scipy L-BFGS-B").
+    from scipy.optimize import minimize
+    w = gen.make_config(0, nside=8, K=(6, 2, 3), cluster_truth=True)
+    model, K = oracle.Model(w.freqs), w.K_of_cfg(0)
+    d, idx = w.data()[0], w.maps[w.cfg_maps[0]]
+
+    def fun(x, want_grad):
+        r = oracle.nll_grad(model, d, w.ninv, idx, K, x, want_grad=want_grad)
+        return r["nll"][0], r["grad"]
+    lo = np.concatenate([np.full(K[0], 1.50), np.full(K[1], 8.0), np.full(K[2], -5.0)])
+    hi = np.concatenate([np.full(K[0], 1.56), np.full(K[1], 40.0), np.full(K[2], -2.95)])   # tight: some minima lie beyond
+    x, L = adatopk(fun, np.clip(w.params_const(), lo, hi), lo, hi, iters=600)
+    res = minimize(lambda z: fun(z, True), np.clip(w.params_const(), lo, hi), jac=True, method="L-BFGS-B",
+                   bounds=list(zip(lo, hi)), options={"maxiter": 2000, "ftol": 1e-15, "gtol": 1e-10, "maxcor": 20})
+    dd = d.astype(np.float64)
+    half_dNd = 0.5 * float(np.einsum("f,fsp,fsp->", w.ninv.astype(np.float64), dd, dd))
+    m_ada, m_ref = L + half_dNd, res.fun + half_dNd          # misfits 1/2 chi^2: the part that depends on the parameters
+    assert abs(m_ada - m_ref) <= 1e-9 * m_ref, (m_ada, m_ref)            # measured 1.6e-12
+    at_bound_ref = (res.x <= lo) | (res.x >= hi)
+    assert at_bound_ref.any()                                 # the test is about active bounds
+    assert np.array_equal((x <= lo) | (x >= hi), at_bound_ref)
+    free = ~at_bound_ref
+    assert np.max(np.abs(x - res.x)[free] / (hi - lo)[free]) < 1e-5   # measured 2e-8
+
+
 def _box_problem(n=40, seed=78):
     """Separable quadratic on [0,1]^n whose targets are all inside the box, started with every parameter ON a bound."""
     g = gen.rng_for("misc", seed)

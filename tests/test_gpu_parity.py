@@ -498,6 +498,35 @@ def test_optimizer_topk_release_matches_the_reference(torch_cuda, path):
     ctx.close()
 
 
+def test_optimizer_rescale_at_extreme_snr(torch_cuda, path):
+    """f4(i), A4: dynamic state rescaling.  Scaling N^-1 by 2^+-40 (signal-to-noise changed by a
+    factor 10^6 either way) scales objective and gradient by 10^+-12, far outside the safe range [1e-15, 1e15] once
+    multiplied by the objective's own 1e8: the driver must rescale its state and then follow the trajectory of the
+    unscaled problem.  A power of two scales every fp32 quantity of the likelihood exactly, so the only difference
+    between the runs is the rescaling itself: parameters agree to 1e-7 of their bounds' width after 60 iterations, the
+    objectives to 1e-9 relative once the scale is taken out, and the fp64 reference of the same reading agrees with the
+    GPU on the scaled problems as closely as on the unscaled one."""
+    import torch
+    w = gen.make_config(1, nside=16, K=(60, 8, 12), cluster_truth=True)
+    ctx, d = make_ctx(w)
+    lo, hi = _bounds(w)
+    x1, nf1 = _gpu_optimize(ctx, w, lo, hi, iters=60)
+    for k in (40, -40):
+        c = 2.0 ** k
+        ctx.set_data(d, (c * w.ninv).astype(np.float32))
+        xs, nfs = _gpu_optimize(ctx, w, lo, hi, iters=60)
+        assert np.all(xs >= lo) and np.all(xs <= hi)
+        assert np.max(np.abs(xs - x1) / (hi - lo)) < 1e-7, (k, np.max(np.abs(xs - x1) / (hi - lo)))
+        assert abs(nfs[0] / c - nf1[0]) <= 1e-9 * abs(nf1[0]), (k, nfs[0] / c, nf1[0])
+        # against the fp64 reference on the scaled problem
+        ws = dataclasses.replace(w, ninv=(c * w.ninv).astype(np.float32))
+        fun, half_dNd, K = _opt_problem(ws)
+        x_ref, L_ref = adatopk(fun, w.params_const(), lo, hi, iters=60)
+        m_gpu, m_ref = fun(xs, False)[0] + half_dNd, L_ref + half_dNd
+        assert abs(m_gpu - m_ref) <= 1e-5 * m_ref, (k, m_gpu, m_ref)
+    ctx.close()
+
+
 def test_optimizer_batch_is_independent_and_monotone(torch_cuda, path):
     """Every entry is an independent problem: optimising a batch equals optimising its entries one by one (bitwise);
     more iterations never end higher; active bounds are respected."""
