@@ -100,7 +100,16 @@ typedef struct cs_opt {
     double topk;        /* Top-K fraction in [0,1] (A2-A3, L519-L537): per iteration the max(1, floor(topk n_bound)) bound
                            parameters with the highest positive release scores are released together; 0 (default, the
                            paper's production setting, L535) releases one per iteration, 1 every one pushed inwards */
+    int32_t method;     /* CS_METHOD_ADATOPK (default; Alg. 1) or CS_METHOD_LBFGS (f4(i); the L-BFGS back-end with
+                           the box handled by the sigmoid reparameterisation x = l + (u - l) sigma(z); two-loop recursion over
+                           `history` pairs, H0 = (s.y / y.y) I, a pair is stored when s.y > 1e-10 |s| |y|, first step and
+                           fall-back -g/|g|, the same backtracking Armijo search from alpha = 1 on 1/2 chi^2 (ls_c1, ls_max,
+                           ls_noise); a start on a bound is moved to 1e-6 of the width inside; lr, beta*, eps, safe_*, topk
+                           are not used; R19) */
+    int32_t history;    /* L-BFGS pairs kept, 1 .. 32 (default 10) */
 } cs_opt;
+#define CS_METHOD_ADATOPK 0
+#define CS_METHOD_LBFGS 1
 
 /* Create a context for `model`.  Allocates only small constant tables.  *out is NULL on failure. */
 CS_API int cs_create(cs_ctx **out, const cs_model *model);
@@ -189,7 +198,8 @@ CS_API int cs_spectral_like_grad_cells(cs_ctx *ctx, double *nll, double *grad, v
  * summed: var dev [batch*nregion] fp64, computed without writing the maps. */
 CS_API int cs_cmb_variance(cs_ctx *ctx, double *var, void *stream);
 
-/* a5: device-resident fixed-budget AdaTopK (Alg. 1) on every entry independently.  It calls cs_build_sed_tables,
+/* a5: device-resident fixed-budget optimizer -- AdaTopK (Alg. 1) or, with opt->method = CS_METHOD_LBFGS, L-BFGS -- on
+ * every entry independently.  It calls cs_build_sed_tables,
  * cs_spectral_like_grad (value + gradient, once per iteration) and cs_spectral_misfit (the objective of the line-search
  * trials: 1/2 chi^2 = nll + const, R13 -- a deviation from north_star's "only the first two").
  * params dev in: start, out: result; lower/upper dev, same layout; nll_final dev [batch] (summed over regions) or

@@ -14,6 +14,7 @@ UNITS_KCMB, UNITS_LITERAL = 0, 1
 OPT_LAYOUT, OPT_FORM, OPT_MIN_FILL, OPT_COPY_LIMIT_MB = 1, 2, 3, 4
 LAYOUT_AUTO, LAYOUT_INPLACE, LAYOUT_SORTED = 0, 1, 2
 FORM_AUTO, FORM_DIRECT = 0, 1
+METHOD_ADATOPK, METHOD_LBFGS = 0, 1
 
 EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_model_constants", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
            "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_cell_moments", "cs_spectral_like_grad_cells", "cs_component_maps", "cs_cmb_residual_maps", "cs_cmb_variance", "cs_optimize",
@@ -29,7 +30,8 @@ class CsModel(C.Structure):
 class CsOpt(C.Structure):
     _fields_ = [("iters", C.c_int32), ("ls_max", C.c_int32), ("lr", C.c_double), ("beta1", C.c_double),
                 ("beta2", C.c_double), ("eps", C.c_double), ("ls_c1", C.c_double), ("safe_lo", C.c_double),
-                ("safe_hi", C.c_double), ("ls_noise", C.c_double), ("topk", C.c_double)]
+                ("safe_hi", C.c_double), ("ls_noise", C.c_double), ("topk", C.c_double), ("method", C.c_int32),
+                ("history", C.c_int32)]
 
 
 class CsError(RuntimeError):

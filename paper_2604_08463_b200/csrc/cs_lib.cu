@@ -1221,6 +1221,7 @@ void cs_opt_defaults(cs_opt *o) {
     o->iters = 200; o->ls_max = 8;
     o->lr = 0.02; o->beta1 = 0.9; o->beta2 = 0.999; o->eps = 1e-16;
     o->ls_c1 = 1e-4; o->safe_lo = 1e-15; o->safe_hi = 1e15; o->ls_noise = 1e-7; o->topk = 0.0;
+    o->method = CS_METHOD_ADATOPK; o->history = 10;
 }
 
 int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *upper, const cs_opt *opt, double *nll_final,
@@ -1230,6 +1231,9 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
     if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || !(opt->ls_noise >= 0) || !(opt->topk >= 0.0 && opt->topk <= 1.0) ||
         c->batch > 65535)
         return CS_EINVAL;
+    const bool lbfgs = opt->method == CS_METHOD_LBFGS;
+    if (opt->method != CS_METHOD_ADATOPK && !lbfgs) return CS_EINVAL;
+    if (lbfgs && (opt->history < 1 || opt->history > LBFGS_HIST_MAX)) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     // the legacy default stream cannot be captured into a graph: fork onto an internal stream and join at the end
     cudaStream_t caller = st;
@@ -1258,7 +1262,13 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
     OptShape sh{c->nparam, c->batch, c->nregion, c->ktot_max, c->d_param_off};
     OptHyper hy{opt->lr, opt->beta1, opt->beta2, opt->eps, opt->ls_c1, opt->safe_lo, opt->safe_hi, opt->ls_noise, opt->topk, opt->ls_max};
     OptWork &w = c->opt;
-    opt_init(w, sh, params, lower, upper, st); c->launches += 1;
+    if (lbfgs) {
+        if (opt_alloc_lbfgs(w, c->nparam, c->batch, opt->history, &c->opt_bytes)) return CS_ENOMEM;
+        lb_init(w, sh, params, lower, upper, 1e-6, st);
+    } else {
+        opt_init(w, sh, params, lower, upper, st);
+    }
+    c->launches += 1;
     // the line search compares 1/2 chi^2 of the GLS residual (cs_spectral_misfit): its value at the start
     if ((rc = cs_build_sed_tables(c, w.x, st))) return rc;
     if ((rc = cs_spectral_misfit(c, w.nll_reg_t, st))) return rc;
@@ -1269,9 +1279,11 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
         // value + gradient at the current point x
         if ((r = cs_build_sed_tables(c, w.x, st))) return r;
         if ((r = cs_spectral_like_grad(c, w.nll_reg, w.grad, st))) return r;
-        opt_direction(w, sh, hy, st); c->launches += 1;
+        if (lbfgs) lb_direction(w, sh, opt->history, 1e-10, st); else opt_direction(w, sh, hy, st);
+        c->launches += 1;
         for (int ls = 0; ls < opt->ls_max; ++ls) {
-            opt_trial_point(w, sh, st); c->launches += 1;
+            if (lbfgs) lb_trial_point(w, sh, st); else opt_trial_point(w, sh, st);
+            c->launches += 1;
             c->skip = w.accepted;   // entries that already accepted a step sit this trial out
             r = cs_build_sed_tables(c, w.xt, st);
             if (!r) r = cs_spectral_misfit(c, w.nll_reg_t, st);
@@ -1279,7 +1291,8 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
             if (r) return r;
             opt_ls_update(w, sh, hy, st); c->launches += 1;
         }
-        opt_commit(w, sh, st); c->launches += 1;
+        if (lbfgs) lb_commit(w, sh, st); else opt_commit(w, sh, st);
+        c->launches += 1;
         return CS_OK;
     };
     // The body is captured once into a CUDA graph and replayed: a step of a small batch is launch-bound (config 2:

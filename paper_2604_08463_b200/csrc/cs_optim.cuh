@@ -28,6 +28,11 @@ struct OptWork {
     long long *ilim = nullptr;
     int32_t *accepted = nullptr;
     int32_t *iter = nullptr;   // device-side iteration counter (the loop body is replayed as a CUDA graph)
+    // L-BFGS back-end (f4(i)): unconstrained variable z, its gradient at the current point, the history ring
+    double *z = nullptr, *gz = nullptr, *S = nullptr, *Y = nullptr;   // S, Y: [hist + 1][nparam] (ring; one slot is scratch)
+    double *sy = nullptr;                                             // [hist + 1][batch] s.yv of each stored pair
+    int32_t *hcount = nullptr, *hhead = nullptr, *moved = nullptr;    // [batch] pairs stored, next slot, last step accepted
+    int32_t hist = 0;                                                 // history slots allocated
 };
 
 struct OptShape {
@@ -45,6 +50,7 @@ inline void opt_free(OptWork &w) {
     cudaFree(w.y); cudaFree(w.x); cudaFree(w.xt); cudaFree(w.dir); cudaFree(w.m); cudaFree(w.v); cudaFree(w.grad);
     cudaFree(w.pivot); cudaFree(w.nll_reg); cudaFree(w.nll_reg_t); cudaFree(w.L0); cudaFree(w.gd); cudaFree(w.amax);
     cudaFree(w.alpha); cudaFree(w.alpha_acc); cudaFree(w.cscale); cudaFree(w.ilim); cudaFree(w.accepted); cudaFree(w.iter); cudaFree(w.Lcur); cudaFree(w.Lt_acc);
+    cudaFree(w.z); cudaFree(w.gz); cudaFree(w.S); cudaFree(w.Y); cudaFree(w.sy); cudaFree(w.hcount); cudaFree(w.hhead); cudaFree(w.moved);
     w = OptWork();
 }
 
@@ -75,6 +81,31 @@ inline int opt_alloc(OptWork &w, int64_t nparam, int32_t batch, int32_t nregion,
     ok &= cudaMalloc((void **)&w.Lt_acc, nb) == cudaSuccess;
     if (!ok) { opt_free(w); return 1; }
     *bytes = (int64_t)(7 * np + nparam + 2 * nb * nregion + 7 * nb + (size_t)batch * 4);
+    return 0;
+}
+
+// workspace of the L-BFGS back-end, allocated on its first use (or when a longer history is asked for)
+inline int opt_alloc_lbfgs(OptWork &w, int64_t nparam, int32_t batch, int32_t hist, int64_t *bytes) {
+    if (w.z && w.hist >= hist) return 0;
+    cudaFree(w.z); cudaFree(w.gz); cudaFree(w.S); cudaFree(w.Y); cudaFree(w.sy); cudaFree(w.hcount); cudaFree(w.hhead); cudaFree(w.moved);
+    w.z = w.gz = w.S = w.Y = w.sy = nullptr; w.hcount = w.hhead = w.moved = nullptr; w.hist = 0;
+    const size_t np = (size_t)(nparam > 0 ? nparam : 1) * sizeof(double);
+    bool ok = true;
+    ok &= cudaMalloc((void **)&w.z, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.gz, np) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.S, np * (hist + 1)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.Y, np * (hist + 1)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.sy, (size_t)batch * (hist + 1) * sizeof(double)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.hcount, (size_t)batch * sizeof(int32_t)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.hhead, (size_t)batch * sizeof(int32_t)) == cudaSuccess;
+    ok &= cudaMalloc((void **)&w.moved, (size_t)batch * sizeof(int32_t)) == cudaSuccess;
+    if (!ok) {
+        cudaFree(w.z); cudaFree(w.gz); cudaFree(w.S); cudaFree(w.Y); cudaFree(w.sy); cudaFree(w.hcount); cudaFree(w.hhead); cudaFree(w.moved);
+        w.z = w.gz = w.S = w.Y = w.sy = nullptr; w.hcount = w.hhead = w.moved = nullptr;
+        return 1;
+    }
+    w.hist = hist;
+    *bytes += (int64_t)(np * (2 + 2 * (size_t)(hist + 1)) + (size_t)batch * ((hist + 1) * 8 + 12));
     return 0;
 }
 
@@ -324,6 +355,158 @@ __global__ void k_opt_finish(OptWork w, OptShape sh, double *params, double *nll
         for (int r = 0; r < sh.nregion; ++r) L += w.nll_reg[i * sh.nregion + r];
         nll_final[i] = L;
     }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// L-BFGS back-end (f4(i); "multiple solvers (L-BFGS, AdaTopK, ...), box constraints via sigmoid
+// reparameterisation"; reading R19 of DESIGN.md; Liu & Nocedal 1989, Nocedal & Wright Alg. 7.4 / 7.5).
+//   x = l + (u - l) sigma(z);  g_z = g_x (u - l) y (1 - y), y = sigma(z);  d = -H g_z by the two-loop recursion over
+//   the stored pairs; backtracking Armijo line search from alpha = 1 on 1/2 chi^2 (the kernels of the AdaTopK line
+//   search); pair (s, yv) = (alpha d, g_z+ - g_z) stored when s.yv > curv_eps |s| |yv|.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int LBFGS_HIST_MAX = 32;
+__device__ __forceinline__ double sigmoid_(double z) { return 0.5 * (1.0 + tanh(0.5 * z)); }
+
+__global__ void k_lb_init(OptWork w, int64_t nparam, const double *params, int32_t batch, double ymin) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) *w.iter = 0;
+    if (i < batch) { w.cscale[i] = 1.0; w.hcount[i] = 0; w.hhead[i] = 0; w.moved[i] = 0; }
+    if (i >= nparam) return;
+    const double l = w.lo[i], u = w.hi[i];
+    double y = (params[i] - l) / (u - l);
+    y = fmin(fmax(y, ymin), 1.0 - ymin);
+    const double z = log(y) - log1p(-y);
+    w.z[i] = z;
+    w.gz[i] = 0.0; w.dir[i] = 0.0;
+    w.x[i] = l + (u - l) * sigmoid_(z);
+}
+
+// One entry per CTA: gradient in z, pair update, two-loop recursion, directional derivative.
+__global__ void __launch_bounds__(OPT_THREADS) k_lb_direction(OptWork w, OptShape sh, int32_t hist, double curv_eps) {
+    __shared__ double shv[OPT_THREADS];
+    __shared__ double s_a[LBFGS_HIST_MAX];
+    const int e = blockIdx.x, tid = threadIdx.x;
+    const int64_t o0 = sh.param_off[e], o1 = sh.param_off[e + 1], np = sh.nparam;
+    const int nslot = hist + 1;   // the new pair is written to the slot after the newest: never one of the <= hist valid ones
+    int count = w.hcount[e], head = w.hhead[e];
+    const bool moved = w.moved[e] != 0;
+    const double a_acc = w.alpha_acc[e];
+    // gradient in z at the current point; the new pair (s, yv) = (alpha d, g_z - g_z of the previous point)
+    double sy = 0.0, ss = 0.0, yy = 0.0, gg = 0.0;
+    for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) {
+        const double y = sigmoid_(w.z[i]);
+        const double g = w.grad[i] * (w.hi[i] - w.lo[i]) * y * (1.0 - y);
+        if (moved) {
+            const double s = a_acc * w.dir[i], yv = g - w.gz[i];
+            w.S[(int64_t)head * np + i] = s;      // written to the next slot; kept only if the curvature test passes
+            w.Y[(int64_t)head * np + i] = yv;
+            sy += s * yv; ss += s * s; yy += yv * yv;
+        }
+        w.gz[i] = g;
+        gg += g * g;
+    }
+    sy = block_sum(sy, shv); ss = block_sum(ss, shv); yy = block_sum(yy, shv); gg = block_sum(gg, shv);
+    if (moved) {
+        if (sy > curv_eps * sqrt(ss) * sqrt(yy)) {
+            if (tid == 0) w.sy[(int64_t)head * sh.batch + e] = sy;
+            head = (head + 1) % nslot;
+            count = min(count + 1, hist);
+        }
+    } else {
+        count = 0;   // the line search found no step (or this is the first iteration): no history
+    }
+    __syncthreads();
+    // two-loop recursion on q = dir (Nocedal & Wright Alg. 7.4), newest pair first
+    for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) w.dir[i] = w.gz[i];
+    __syncthreads();
+    for (int j = 0; j < count; ++j) {
+        const int slot = ((head - 1 - j) % nslot + nslot) % nslot;
+        double sq = 0.0;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) sq += w.S[(int64_t)slot * np + i] * w.dir[i];
+        sq = block_sum(sq, shv);
+        const double a = sq / w.sy[(int64_t)slot * sh.batch + e];
+        if (tid == 0) s_a[j] = a;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) w.dir[i] -= a * w.Y[(int64_t)slot * np + i];
+        __syncthreads();
+    }
+    if (count > 0) {   // H0 = gamma I with the newest pair
+        const int slot = ((head - 1) % nslot + nslot) % nslot;
+        double y2 = 0.0;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) { const double yv = w.Y[(int64_t)slot * np + i]; y2 += yv * yv; }
+        y2 = block_sum(y2, shv);
+        const double gamma = w.sy[(int64_t)slot * sh.batch + e] / y2;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) w.dir[i] *= gamma;
+        __syncthreads();
+    }
+    for (int j = count - 1; j >= 0; --j) {   // oldest pair first
+        const int slot = ((head - 1 - j) % nslot + nslot) % nslot;
+        double yr = 0.0;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) yr += w.Y[(int64_t)slot * np + i] * w.dir[i];
+        yr = block_sum(yr, shv);
+        const double b = yr / w.sy[(int64_t)slot * sh.batch + e];
+        const double a = s_a[j];
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) w.dir[i] += w.S[(int64_t)slot * np + i] * (a - b);
+        __syncthreads();
+    }
+    double gd = 0.0;
+    for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) { const double d = -w.dir[i]; w.dir[i] = d; gd += w.gz[i] * d; }
+    gd = block_sum(gd, shv);
+    const double nrm = sqrt(gg);
+    if (count == 0 || !(gd < 0.0)) {   // no pair yet, or not a descent direction (rounding): unit steepest-descent step
+        count = 0;
+        const double inv = nrm > 0.0 ? 1.0 / nrm : 0.0;
+        for (int64_t i = o0 + tid; i < o1; i += OPT_THREADS) w.dir[i] = -w.gz[i] * inv;
+        gd = -nrm;
+    }
+    if (tid == 0) {
+        w.hcount[e] = count; w.hhead[e] = head;
+        w.L0[e] = w.Lcur[e];
+        w.gd[e] = gd;
+        w.alpha[e] = 1.0;
+        w.alpha_acc[e] = 0.0;
+        w.accepted[e] = 0;
+    }
+}
+
+// trial point x_t = l + (u - l) sigma(z + alpha d); grid = (ceil(ktot_max/256), batch)
+__global__ void k_lb_trial(OptWork w, OptShape sh) {
+    const int e = blockIdx.y;
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= sh.param_off[e + 1]) return;
+    const double a = w.accepted[e] ? w.alpha_acc[e] : w.alpha[e];
+    w.xt[i] = w.lo[i] + (w.hi[i] - w.lo[i]) * sigmoid_(w.z[i] + a * w.dir[i]);
+}
+
+__global__ void k_lb_commit(OptWork w, OptShape sh) {
+    const int e = blockIdx.y;
+    if (blockIdx.x == 0 && e == 0 && threadIdx.x == 0) *w.iter += 1;
+    const bool acc = w.accepted[e] != 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (acc) w.Lcur[e] = w.Lt_acc[e];
+        w.moved[e] = acc ? 1 : 0;
+    }
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= sh.param_off[e + 1] || !acc) return;
+    const double z = w.z[i] + w.alpha_acc[e] * w.dir[i];
+    w.z[i] = z;
+    w.x[i] = w.lo[i] + (w.hi[i] - w.lo[i]) * sigmoid_(z);
+}
+
+inline void lb_init(OptWork &w, const OptShape &sh, const double *params, const double *lo, const double *hi, double ymin, cudaStream_t st) {
+    w.lo = lo; w.hi = hi;
+    const int64_t n = sh.nparam > sh.batch ? sh.nparam : sh.batch;
+    k_lb_init<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(w, sh.nparam, params, sh.batch, ymin);
+}
+inline void lb_direction(OptWork &w, const OptShape &sh, int32_t hist, double curv_eps, cudaStream_t st) {
+    k_lb_direction<<<sh.batch, OPT_THREADS, 0, st>>>(w, sh, hist, curv_eps);
+}
+inline void lb_trial_point(OptWork &w, const OptShape &sh, cudaStream_t st) {
+    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    k_lb_trial<<<grid, 256, 0, st>>>(w, sh);
+}
+inline void lb_commit(OptWork &w, const OptShape &sh, cudaStream_t st) {
+    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    k_lb_commit<<<grid, 256, 0, st>>>(w, sh);
 }
 
 inline void opt_init(OptWork &w, const OptShape &sh, const double *params, const double *lo, const double *hi, cudaStream_t st) {
