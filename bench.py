@@ -594,6 +594,17 @@ def main():
                 c2.optimize(p2, lo, hi, cs.opt_defaults(iters=200), nf, stream)
                 torch.cuda.synchronize()
                 times.append(time.perf_counter() - t0)
+            # the same problem with the L-BFGS back-end (f4(i)), 100 iterations
+            p3 = torch.from_numpy(w2.params_const()).to(dev)
+            nf3 = torch.zeros(1, dtype=torch.float64, device=dev)
+            t_lb = []
+            for _ in range(2):
+                p3.copy_(torch.from_numpy(w2.params_const()).to(dev))
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                c2.optimize(p3, lo, hi, cs.opt_defaults(iters=100, method=cs.METHOD_LBFGS), nf3, stream)
+                torch.cuda.synchronize()
+                t_lb.append(time.perf_counter() - t0)
             n1 = torch.zeros(1, dtype=torch.float64, device=dev)
             g1 = torch.zeros_like(p2)
             e0.record(stream)
@@ -604,6 +615,7 @@ def main():
             torch.cuda.synchronize()
             out["extras"]["c2"] = {"workload": "C2: nside 64, K=(500,50,100), one entry",
                                    "optimize_200_iters_ms": 1e3 * min(times), "final_nll": float(nf.item()),
+                                   "lbfgs_100_iters_ms": 1e3 * min(t_lb), "lbfgs_final_nll": float(nf3.item()),
                                    "like_grad_call_us": 1e3 * e0.elapsed_time(e1) / 20,
                                    "pixel_evals_per_s": w2.npix / (e0.elapsed_time(e1) / 20 * 1e-3)}
             c2.close()

@@ -6,7 +6,7 @@
 //     sum_{p in cell} sum_S b_S^T M^-1 b_S  =  tr( M^-1 A^T T A ),        T = N^-1 (sum_{p,S} d_S d_S^T) N^-1   [F x F]
 //
 // T is independent of the parameters: k_cc_moments builds it once per (configuration, data set) pair, in fp64, from
-// the caller's data.  A likelihood + gradient evaluation then costs one F x F contraction per cell instead of one
+// the pair's private sorted copy of the data.  A likelihood + gradient evaluation then costs one F x F contraction per cell instead of one
 // pass over every pixel (k_like_cc, fp64; one thread per (entry, cell)):
 //
 //     u_i  = T a_i   (a_0 = 1, a_1 = a_d, a_2 = a_s) ;   B = A^T T A ;   nll_cell = -1/2 tr(M^-1 B)
@@ -48,57 +48,63 @@ struct CellsDev {
 
 struct MomJob {
     int32_t cfg, data;
-    int64_t off;   // double offset of the pair's moments [CC_NMOM][ncell] inside the moments buffer
+    int64_t off;        // double offset of the pair's moments [CC_NMOM][ncell] inside the moments buffer
+    int64_t copy_off;   // float offset of the pair's private sorted copy inside dcopy
 };
 
-// Second moments of one (configuration, data set) pair: one warp per cell, lane l owns the unique (f,g) pairs l, l+32,
-// l+64, l+96.  The cell's pixels are staged 32 at a time in shared memory (row stride 33: lanes reading different
-// bands hit different banks).  grid = (ceil(ncell_max / 4), pairs), block = 128.
-__global__ void __launch_bounds__(128) k_cc_moments(const float *__restrict__ d, int64_t npix, int32_t nfreq, const CfgDev *__restrict__ cfgs,
-                                                    const CellsDev *__restrict__ cells, const MomJob *__restrict__ jobs,
-                                                    const float *__restrict__ w, double *__restrict__ mom) {
-    __shared__ float sd[4][2 * CC_MAXF][33];
+// Second moments of one (configuration, data set) pair: T = N^-1 (D_Q D_Q^T + D_U D_U^T) N^-1 with D_S the [nfreq x pixels]
+// block of the cell's data -- a dense contraction over the pixels, the one step of this library that is GEMM-shaped, on
+// the fp64 tensor cores (mma.sync m8n8k4: the fp32 data are promoted exactly, products and sums are fp64).
+// One warp per cell; the 15 bands are two row blocks of 8 (the 16th row is zero), the pixels go through in steps of 4.
+// Lane (r, k) = (lane / 4, lane % 4) holds D[8 b + r][pixel j0 + k] for both row blocks b and both Stokes parameters:
+// that register is its A fragment of block b (row r, column k) and, the matrix being D D^T, also its B fragment
+// (row k, column r) -- no shared memory and no transposition.  The cell's pixels are consecutive positions of the
+// pair's private sorted copy (pads read as zero data), 16 contiguous bytes per row and step.
+// Three accumulator tiles (0,0), (0,1), (1,1) of 8 x 8; lane (r, k) ends with the entries (r, 2k) and (r, 2k + 1) of each.
+// grid = (ceil(ncell_max / 4), pairs), block = 128.
+__device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+__global__ void __launch_bounds__(128) k_cc_moments(const float *__restrict__ dcopy, int32_t nfreq, const CellsDev *__restrict__ cells,
+                                                    const MomJob *__restrict__ jobs, const float *__restrict__ w, double *__restrict__ mom) {
     const MomJob job = jobs[blockIdx.y];
     const CellsDev *cl = cells + job.cfg;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int c = blockIdx.x * 4 + warp;
-    if (c >= cl->ncell) return;
-    const int32_t *pospix = cfgs[job.cfg].pospix;
+    if (c >= cl->ncell) return;   // whole warps: the cell is the warp's
     const int pos0 = cl->cellpos[c], len = cl->celllen[c];
-    const float *dd = d + (int64_t)job.data * 2 * nfreq * npix;
-    int pf[4], pg[4];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {   // unpack the lane's pairs
-        int idx = lane + 32 * q, f = 0;
-        pf[q] = pg[q] = -1;
-        if (idx < CC_NMOM) {
-            while (idx >= CC_MAXF - f) { idx -= CC_MAXF - f; ++f; }
-            pf[q] = f; pg[q] = f + idx;
-            if (pg[q] >= nfreq) pf[q] = pg[q] = -1;
+    const int nrows = 2 * nfreq;
+    const float *dd = dcopy + job.copy_off;
+    const int r = lane >> 2, k = lane & 3;
+    const int f0 = r, f1 = 8 + r;   // the lane's band in the two row blocks
+    const bool has0 = f0 < nfreq, has1 = f1 < nfreq;
+    double c00[2] = {0.0, 0.0}, c01[2] = {0.0, 0.0}, c11[2] = {0.0, 0.0};
+#pragma unroll 2
+    for (int j0 = 0; j0 < len; j0 += 4) {
+        const int j = j0 + k;
+        float q0 = 0.f, u0 = 0.f, q1 = 0.f, u1 = 0.f;
+        if (j < len) {
+            const int pos = pos0 + j, tile = pos / TPX, within = pos - tile * TPX;
+            const float *src = dd + (int64_t)tile * nrows * TPX + (within / HALF) * nrows * HALF + (within % HALF);
+            if (has0) { q0 = __ldg(src + (2 * f0) * HALF); u0 = __ldg(src + (2 * f0 + 1) * HALF); }
+            if (has1) { q1 = __ldg(src + (2 * f1) * HALF); u1 = __ldg(src + (2 * f1 + 1) * HALF); }
         }
+        const double dq0 = (double)q0, du0 = (double)u0, dq1 = (double)q1, du1 = (double)u1;
+        dmma_m8n8k4(c00, dq0, dq0); dmma_m8n8k4(c00, du0, du0);
+        dmma_m8n8k4(c01, dq0, dq1); dmma_m8n8k4(c01, du0, du1);
+        dmma_m8n8k4(c11, dq1, dq1); dmma_m8n8k4(c11, du1, du1);
     }
-    double acc[4] = {0.0, 0.0, 0.0, 0.0};
-    for (int j0 = 0; j0 < len; j0 += 32) {
-        const int j = j0 + lane;
-        const int pix = (j < len) ? pospix[pos0 + j] : -1;
-        for (int r = 0; r < 2 * nfreq; ++r) sd[warp][r][lane] = (pix >= 0) ? __ldg(dd + (int64_t)r * npix + pix) : 0.f;
-        __syncwarp();
-        const int n = min(32, len - j0);
-        for (int x = 0; x < n; ++x) {
+    // the unique entries f <= g < 15 (zero where a band is beyond nfreq), weighted by w_f w_g
+    const int ncell = cl->ncell;
+    double *out = mom + job.off + c;
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
-                if (pf[q] >= 0) {
-                    acc[q] = fma((double)sd[warp][2 * pf[q]][x], (double)sd[warp][2 * pg[q]][x], acc[q]);           // Q
-                    acc[q] = fma((double)sd[warp][2 * pf[q] + 1][x], (double)sd[warp][2 * pg[q] + 1][x], acc[q]);   // U
-                }
-        }
-        __syncwarp();
-    }
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const int idx = lane + 32 * q;
-        if (idx < CC_NMOM)
-            mom[job.off + (int64_t)idx * cl->ncell + c] = (pf[q] >= 0) ? (double)w[pf[q]] * (double)w[pg[q]] * acc[q] : 0.0;
+    for (int i = 0; i < 2; ++i) {
+        const int g0 = 2 * k + i, g1 = 8 + g0;
+        const double wf0 = has0 ? (double)w[f0] : 0.0, wf1 = has1 ? (double)w[f1] : 0.0;
+        const double wg0 = (g0 < nfreq) ? (double)w[g0] : 0.0, wg1 = (g1 < nfreq) ? (double)w[g1] : 0.0;
+        if (f0 <= g0) out[(int64_t)cc_idx(f0, g0) * ncell] = wf0 * wg0 * c00[i];
+        if (g1 < CC_MAXF) out[(int64_t)cc_idx(f0, g1) * ncell] = wf0 * wg1 * c01[i];
+        if (f1 < CC_MAXF && g1 < CC_MAXF && f1 <= g1) out[(int64_t)cc_idx(f1, g1) * ncell] = wf1 * wg1 * c11[i];
     }
 }
 

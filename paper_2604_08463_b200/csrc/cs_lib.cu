@@ -1151,7 +1151,7 @@ int cs_cell_moments(cs_ctx *c, void *stream) {
         std::map<std::pair<int32_t, int32_t>, int64_t> off;
         int64_t n = 0;
         for (size_t j = 0; j < c->jobs.size(); ++j) {
-            mj[j] = MomJob{c->jobs[j].cfg, c->jobs[j].data, n};
+            mj[j] = MomJob{c->jobs[j].cfg, c->jobs[j].data, n, c->jobs[j].off};
             off[std::make_pair(c->jobs[j].data, c->jobs[j].cfg)] = n;
             n += (int64_t)CC_NMOM * c->cellsh[c->jobs[j].cfg].ncell;
         }
@@ -1173,7 +1173,7 @@ int cs_cell_moments(cs_ctx *c, void *stream) {
     for (size_t j = 0; j < c->jobs.size(); j += 65535) {
         const int nj = (int)std::min<size_t>(65535, c->jobs.size() - j);
         dim3 grid((c->ncell_max + 3) / 4, nj);
-        k_cc_moments<<<grid, 128, 0, st>>>(c->d, c->npix, c->nfreq, c->d_cfgs, c->d_cells, c->d_momjobs + j, c->d_w, c->d_mom);
+        k_cc_moments<<<grid, 128, 0, st>>>(c->d_copy, c->nfreq, c->d_cells, c->d_momjobs + j, c->d_w, c->d_mom);
         c->launches++;
     }
     CK(cudaGetLastError());
