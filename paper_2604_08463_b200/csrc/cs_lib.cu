@@ -1451,10 +1451,10 @@ int cs_spherical_kmeans(int64_t npix, const double *vecs, const uint8_t *region,
     if (cudaMallocAsync((void **)&d_pr, sizeof(KmProb) * nprob, st) != cudaSuccess) return CS_ENOMEM;
     // pageable host memory: the copy has left the host buffer when cudaMemcpyAsync returns
     if (cudaMemcpyAsync(d_pr, pr.data(), sizeof(KmProb) * nprob, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaFreeAsync(d_pr, st); return CS_ECUDA; }
-    const dim3 ga((unsigned)((npix + 255) / 256), nprob), gu((kmax + 127) / 128, nprob);
+    const dim3 ga((unsigned)((npix + 255) / 256), nprob), gu((kmax + 7) / 8, nprob);
     k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
     for (int32_t it = 0; it < iters; ++it) {
-        k_km_update<<<gu, 128, 0, st>>>(vecs, npix, d_pr, labels, cent);
+        k_km_update<<<gu, 256, 0, st>>>(vecs, npix, d_pr, labels, cent);
         k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
     }
     const cudaError_t ce = cudaGetLastError();
