@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <stdexcept>
 #include <new>
 #include <vector>
 
@@ -419,6 +420,7 @@ void pack_tile_headers(const SortedPlan &sp, const MapPlanHost (&mp)[4], const i
         const int32_t off_cdesc = off_slot + stot;                          // u16 arrays, packed two per word
         const int32_t off_sdesc = off_cdesc + (ctot + 1) / 2;
         const int32_t total = (off_sdesc + (stot + 1) / 2 + 3) & ~3;        // multiple of 16 bytes
+        if (total > HDR_CAP_WORDS || ncell > CELL_CAP) throw std::length_error("tile header");   // cannot happen: the caps follow from CELL_CAP
         blob.resize(base + total, 0u);
         uint32_t *h = blob.data() + base;
         h[HM_NCELL] = (uint32_t)ncell; h[HM_NCHUNK] = (uint32_t)ctot; h[HM_NSEG] = (uint32_t)stot;

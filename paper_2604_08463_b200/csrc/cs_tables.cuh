@@ -17,18 +17,28 @@ namespace cs {
 // ----------------------------------------------------------------------------------------------------------
 // exp(y) in fp64 for the power-law rows: y = k ln2 + r, |r| <= ln2/2, degree-11 Taylor polynomial (truncation
 // 6e-15 relative, far below the fp32 rounding of the stored value), scaled by 2^k through the exponent field.
-// Arguments outside the range where 2^k is a normal number take the library routine.
+// k comes from the 1.5 * 2^52 shift (no FRND / F2I on the conversion pipe), the coefficients from the constant bank
+// (as 64-bit immediates every one costs two UMOV per use: the kernel is bound by instruction issue), and 2^k is an
+// integer add on the high word of the polynomial's value (it lies in [0.7, 1.42] and the result is a normal number).
+// Arguments outside the range where 2^k is a normal number give +inf / 0 / NaN by selection (what the library routine
+// returns there once rounded to fp32), so that the four values of a thread stay free of branches and interleave.
+__constant__ double EXP_C[12] = {1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0, 1.0 / 40320.0, 1.0 / 5040.0, 1.0 / 720.0,
+                                 1.0 / 120.0,      1.0 / 24.0,      1.0 / 6.0,      0.5,          1.0,          1.0};
+__constant__ double EXP_R[4] = {1.4426950408889634074, 6755399441055744.0, 6.93147180369123816490e-01, 1.90821492927058770002e-10};
 __device__ __forceinline__ double exp_pow(double y) {
-    if (!(fabs(y) < 700.0)) return exp(y);
-    const double kf = rint(y * 1.4426950408889634074);
-    double r = fma(-kf, 6.93147180369123816490e-01, y);
-    r = fma(-kf, 1.90821492927058770002e-10, r);
-    double p = 1.0 / 39916800.0;
-    p = fma(p, r, 1.0 / 3628800.0); p = fma(p, r, 1.0 / 362880.0); p = fma(p, r, 1.0 / 40320.0);
-    p = fma(p, r, 1.0 / 5040.0);    p = fma(p, r, 1.0 / 720.0);    p = fma(p, r, 1.0 / 120.0);
-    p = fma(p, r, 1.0 / 24.0);      p = fma(p, r, 1.0 / 6.0);      p = fma(p, r, 0.5);
-    p = fma(p, r, 1.0);             p = fma(p, r, 1.0);
-    return p * __hiloint2double(((int)kf + 1023) << 20, 0);
+    const bool ok = fabs(y) < 700.0;               // false for NaN
+    const double ys = ok ? y : 0.0;
+    const double t = fma(ys, EXP_R[0], EXP_R[1]);  // the integer nearest to y / ln2 sits in the low word
+    const double kf = t - EXP_R[1];
+    const int k = __double2loint(t);
+    double r = fma(-kf, EXP_R[2], ys);
+    r = fma(-kf, EXP_R[3], r);
+    double p = EXP_C[0];
+#pragma unroll
+    for (int i = 1; i < 12; ++i) p = fma(p, r, EXP_C[i]);
+    const double res = __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+    const double out_of_range = (y > 0.0) ? CUDART_INF : ((y < 0.0) ? 0.0 : y + y);
+    return ok ? res : out_of_range;
 }
 
 // 1/a for a normal positive double: MUFU.RCP64H seed (about 20 bits) and two Newton steps (error ~1 ulp, no slow path).
@@ -44,7 +54,7 @@ __device__ __forceinline__ double rcp_pos(double a) {
 // non-positive or non-finite) arguments take the library routine.
 __device__ __forceinline__ double expm1_pos(double x) { return (x >= 0.03125 && x < 700.0) ? exp_pow(x) - 1.0 : expm1(x); }
 
-// One block of k_tables' work: 64 consecutive parameters [j0, j0 + 64) of entry e, in one aligned 48-byte record
+// One block of k_tables' work: TAB_ROWS_PER_BLOCK consecutive parameters from j0 on of entry e, in one aligned 48-byte record
 // (no chain of dependent loads through the configuration table, and no block without work).
 struct TabBlock {
     int64_t param_off;   // first parameter of the entry
@@ -52,7 +62,8 @@ struct TabBlock {
     int32_t K0, K1, ktot, j0;
     int32_t e, pad[3];
 };
-constexpr int TAB_ROWS_PER_BLOCK = 64;
+constexpr int TAB_SUB = 4;                       // parameters per thread quad
+constexpr int TAB_ROWS_PER_BLOCK = 64 * TAB_SUB;
 
 // One thread per (entry, parameter, band quad): four table values and one 16-byte store.  The band constants come from a
 // shared-memory copy (indexed by the thread's quad: a constant-bank read would serialise); the parameter load is issued
@@ -65,16 +76,26 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
     const int64_t param_off = ((int64_t)(uint32_t)b0.y << 32) | (uint32_t)b0.x, tab_row = ((int64_t)(uint32_t)b0.w << 32) | (uint32_t)b0.z;
     const int K0 = b1.x, K1 = b1.y, ktot = b1.z, j0 = b1.w, e = b2.x;
     if (skip && skip[e] != 0) return;
-    const int j = j0 + (threadIdx.x >> 2), f0 = (threadIdx.x & 3) * 4;
-    const bool live = j < ktot;
-    const double x = live ? __ldg(params + param_off + j) : 1.0;
-    for (int i = threadIdx.x; i < (int)(sizeof(TConst) / 8); i += blockDim.x)
-        reinterpret_cast<double *>(&tc)[i] = reinterpret_cast<const double *>(tcg)[i];
+    const int f0 = (threadIdx.x & 3) * 4;
+    // the block's TAB_SUB x 64 parameters: all loads first (one latency for the block), then the rows one after the other
+    double xs[TAB_SUB];
+#pragma unroll
+    for (int u = 0; u < TAB_SUB; ++u) {
+        const int j = j0 + 64 * u + (threadIdx.x >> 2);
+        xs[u] = (j < ktot) ? __ldg(params + param_off + j) : 1.0;
+    }
+    static_assert(sizeof(TConst) / 8 <= 256, "one word per thread");
+    if (threadIdx.x < (int)(sizeof(TConst) / 8)) reinterpret_cast<double *>(&tc)[threadIdx.x] = __ldg(reinterpret_cast<const double *>(tcg) + threadIdx.x);
     __syncthreads();
-    if (!live) return;
     const int nfreq = tc.nfreq;
     float *row0 = tab + tab_row * NROW;
-    bool bad = !isfinite(x);
+    bool bad = false;
+#pragma unroll
+    for (int u = 0; u < TAB_SUB; ++u) {
+    const int j = j0 + 64 * u + (threadIdx.x >> 2);
+    if (j >= ktot) break;
+    const double x = xs[u];
+    bad = bad || !isfinite(x);
     float v[4];
     if (j < K0) {
         // dust power-law factor with the band constant folded in: cd[f] * (nu_f/nu0d)^beta_d
@@ -106,6 +127,7 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
 #pragma unroll
         for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cs[f0 + i] * exp_pow(x * tc.lns[f0 + i])) : 0.f;
         *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + 2 * K1 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
+    }
     }
     if (bad && f0 == 0) atomicOr(err, ERR_DOMAIN);
 }
