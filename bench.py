@@ -55,6 +55,12 @@ def make_workload(name, batch, rank=0):
     elif name == "c4":
         w = gen.make_config(3, batch=batch or None)
         desc = f"C4: nside 64, 3 latitude regions, 64 configurations x 100 noise realisations ({w.batch} entries, 100 data sets)"
+    elif name == "kmax":
+        # the shape of the paper's own optimum (Table 2: beta_d per pixel, K_Td = 2500, K_bs = 150): every pixel
+        # is its own cell, the configuration stays in place on the direct kernel
+        B = batch or 256
+        w = gen.make_config(1, ndata=B, K=(49152, 2500, 150))
+        desc = f"Kmax: nside 64, K=(npix,2500,150) (beta_d per pixel, PAPER.md Table 2), {B} entries x distinct noise realisations"
     elif name == "c2":
         w = gen.make_config(1)
         desc = "C2: nside 64, K=(500,50,100), one entry"
@@ -620,6 +626,10 @@ def main():
                                    "pixel_evals_per_s": w2.npix / (e0.elapsed_time(e1) / 20 * 1e-3)}
             c2.close()
             del d2
+            try:   # the shape of the paper's own optimum (Table 2): beta_d per pixel, in place on the direct kernel
+                out["extras"]["kmax"] = extra_workload(cs, "kmax", 256, 5, dev, stream, peak, None)[256]
+            except Exception as exc:
+                out["extras"]["kmax"] = {"error": repr(exc)}
             for nm, prefixes in (("c3", None), ("c4", None), ("c5", [1, 16, 64, 256])):
                 try:
                     for b, res in extra_workload(cs, nm, 0, 5, dev, stream, peak, prefixes).items():

@@ -59,11 +59,17 @@ extern "C" {
                                   costs more than the direct kernel); set before cs_set_clusters */
 #define CS_OPT_COPY_LIMIT_MB 4 /* most device memory [MiB] the private sorted copies of a batch may take; 0 (default) =
                                   70 % of the memory free when cs_set_batch runs.  Beyond it cs_set_batch returns CS_ENOMEM. */
+#define CS_OPT_PIXEL_BETA    5 /* CS_PIXBETA_*; set before cs_set_clusters */
 #define CS_LAYOUT_AUTO    0 /* sorted layout for configurations whose tiles fill well, in place for the others */
 #define CS_LAYOUT_INPLACE 1 /* never copy: stream the caller's d in its own pixel order (direct kernel only) */
 #define CS_LAYOUT_SORTED  2 /* sorted layout for every configuration */
 #define CS_FORM_AUTO      0 /* sorted-cell kernel on sorted configurations, direct kernel on the others */
 #define CS_FORM_DIRECT    1 /* direct kernel everywhere, on whatever layout each configuration has (same bits) */
+#define CS_PIXBETA_AUTO   0 /* a configuration that stays in place and whose beta_d map has more patches than half the
+                             pixels (the paper's own optimum fits beta_d per pixel, Table 2) gets no beta_d table rows: the
+                             direct kernel evaluates cd (nu/nu0)^beta_d per pixel with the table kernel's own fp64
+                             arithmetic (same bits), which saves 64 B written and 64 B read per pixel-eval */
+#define CS_PIXBETA_OFF    1 /* always build and gather the beta_d rows */
 
 #if defined(__GNUC__)
 #define CS_API __attribute__((visibility("default")))

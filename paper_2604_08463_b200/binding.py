@@ -11,7 +11,8 @@ from . import build as _build
 
 OK, EINVAL, EINDEX, EDOMAIN, ESINGULAR, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5, -6
 UNITS_KCMB, UNITS_LITERAL = 0, 1
-OPT_LAYOUT, OPT_FORM, OPT_MIN_FILL, OPT_COPY_LIMIT_MB = 1, 2, 3, 4
+OPT_LAYOUT, OPT_FORM, OPT_MIN_FILL, OPT_COPY_LIMIT_MB, OPT_PIXEL_BETA = 1, 2, 3, 4, 5
+PIXBETA_AUTO, PIXBETA_OFF = 0, 1
 LAYOUT_AUTO, LAYOUT_INPLACE, LAYOUT_SORTED = 0, 1, 2
 FORM_AUTO, FORM_DIRECT = 0, 1
 METHOD_ADATOPK, METHOD_LBFGS = 0, 1
@@ -199,7 +200,8 @@ class Context:
 
     def set_option(self, key, value):
         """key: OPT_* or one of "layout", "form", "min_fill", "copy_limit_mb"."""
-        names = {"layout": OPT_LAYOUT, "form": OPT_FORM, "min_fill": OPT_MIN_FILL, "copy_limit_mb": OPT_COPY_LIMIT_MB}
+        names = {"layout": OPT_LAYOUT, "form": OPT_FORM, "min_fill": OPT_MIN_FILL, "copy_limit_mb": OPT_COPY_LIMIT_MB,
+                 "pixel_beta": OPT_PIXEL_BETA}
         _chk(lib().cs_set_option(self._h, int(names.get(key, key)), float(value)), "cs_set_option")
 
     def layout_info(self, cfg):

@@ -89,7 +89,8 @@ struct CfgDev {
     int32_t ntile;        // tiles of this configuration's layout
     int32_t sorted;       // 1: sorted layout with private data copies, 0: in place
     int32_t ntile_ring;   // tiles of the in-place layout
-    int32_t pad;
+    int32_t pixbeta;      // 1: in place with beta_d (nearly) per pixel: no beta_d table rows, the direct kernel evaluates
+                          //    cd (nu/nu0)^beta_d per pixel from a copy of the parameters (k_tables' arithmetic, same bits)
     const int32_t *kseg[4];    // = maps[map[t]].ksegptr: one load less on k_merge's way to its slots
     // sorted layout only
     const uint8_t *cellid;     // [ntile*NCONS] tile-local cell of each thread (position pair)
@@ -115,6 +116,8 @@ struct Run {
 struct PosInfo {
     int64_t tab_row;   // first table row of the entry
     int64_t src;       // sorted configuration: float offset of the entry's private copy inside dcopy; else its data set
+    int64_t param_off; // first parameter of the entry (pixbeta configurations read beta_d from the parameter copy)
+    int64_t pad;
 };
 
 // Constants of the fused kernels, passed by value (constant bank).

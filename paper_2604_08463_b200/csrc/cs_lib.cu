@@ -91,7 +91,7 @@ struct cs_ctx {
     KConst kc;
     bool have_ninv = false;
     // options (cs_set_option)
-    int32_t opt_layout = CS_LAYOUT_AUTO, opt_form = CS_FORM_AUTO;
+    int32_t opt_layout = CS_LAYOUT_AUTO, opt_form = CS_FORM_AUTO, opt_pixbeta = CS_PIXBETA_AUTO;
     double opt_min_fill = 0.45;
     int64_t opt_copy_limit = 0;         // bytes, 0 = 70 % of the free device memory when the batch is set
     // clusters
@@ -130,6 +130,7 @@ struct cs_ctx {
     Run *d_runs = nullptr;
     CopyJob *d_jobs = nullptr;
     float *d_tab = nullptr, *d_copy = nullptr;
+    double *d_pcopy = nullptr;          // the parameters the tables were last built from
     double *d_partial = nullptr;
     int64_t batch_bytes = 0, copy_bytes = 0;
     int32_t job_ntile_max = 0;
@@ -204,7 +205,8 @@ void free_opt(cs_ctx *c) {
 void free_batch(cs_ctx *c) {
     cudaFree(c->d_cfg_of); cudaFree(c->d_data_of); cudaFree(c->d_elist);
     cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_tabblk); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
-    cudaFree(c->d_tab); cudaFree(c->d_partial); cudaFree(c->d_copy);
+    cudaFree(c->d_tab); cudaFree(c->d_partial); cudaFree(c->d_copy); cudaFree(c->d_pcopy);
+    c->d_pcopy = nullptr;
     c->d_cfg_of = c->d_data_of = c->d_elist = nullptr;
     c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr; c->d_tabblk = nullptr; c->ntabblk = 0;
     c->d_runs = nullptr; c->d_jobs = nullptr;
@@ -561,6 +563,11 @@ LikeParams base_params(cs_ctx *c) {
     P.PS = c->PS;
     P.maps_out = nullptr;
     P.err = c->d_err;
+    P.pcopy = c->d_pcopy;
+    for (int f = 0; f < NROW; ++f) {
+        const double l2 = c->tc.lnd[f] * 1.4426950408889634074;   // log2(nu_f/nu0d); 0 beyond nfreq (cd = 0 there)
+        P.cdf[f] = (float)c->tc.cd[f]; P.l2h[f] = (float)l2; P.l2l[f] = (float)(l2 - (double)P.l2h[f]);
+    }
     P.kc = c->kc;
     return P;
 }
@@ -731,6 +738,11 @@ int cs_set_option(cs_ctx *c, int32_t key, double value) {
             if (!(value >= 0.0 && value <= 1.0) || !c->maps.empty()) return CS_EINVAL;
             c->opt_min_fill = value;
             return CS_OK;
+        case CS_OPT_PIXEL_BETA:
+            if (value != CS_PIXBETA_AUTO && value != CS_PIXBETA_OFF) return CS_EINVAL;
+            if (!c->maps.empty()) return CS_EINVAL;   // decided when the clusters are set
+            c->opt_pixbeta = (int32_t)value;
+            return CS_OK;
         case CS_OPT_COPY_LIMIT_MB:
             if (value < 0) return CS_EINVAL;
             c->opt_copy_limit = (int64_t)(value * 1048576.0);
@@ -853,6 +865,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
                 cf.cellid = sh.cellid; cf.cellptr = sh.cellptr; cf.cellrows = sh.cellrows; cf.pospix = sh.pospix;
             }
         }
+        cf.pixbeta = (!cf.sorted && c->opt_pixbeta == CS_PIXBETA_AUTO && 2 * (int64_t)cf.K[0] > npix) ? 1 : 0;
         int32_t off = 0;
         for (int t = 0; t < 4; ++t) {
             cf.segbase[t] = off;
@@ -981,7 +994,7 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     c->pinfo.resize(batch);
     for (int32_t i = 0; i < batch; ++i) {
         const int32_t e = c->elist[i];
-        c->pinfo[i] = PosInfo{tab_off[e], c->cfgs[cfg_of[e]].sorted ? c->copy_off[e] : (int64_t)data_of[e]};
+        c->pinfo[i] = PosInfo{tab_off[e], c->cfgs[cfg_of[e]].sorted ? c->copy_off[e] : (int64_t)data_of[e], c->param_off[e], 0};
     }
     const int64_t copy_bytes = copy_floats * 4;
     if (copy_bytes > 0) {
@@ -997,7 +1010,8 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     for (int32_t e = 0; e < batch; ++e) {
         const CfgDev &cf = c->cfgs[cfg_of[e]];
         for (int32_t j0 = 0; j0 < cf.ktot; j0 += TAB_ROWS_PER_BLOCK)
-            tabblk.push_back(TabBlock{c->param_off[e], tab_off[e], cf.K[0], cf.K[1], cf.ktot, j0, e, {0, 0, 0}});
+            if (!(cf.pixbeta && j0 + TAB_ROWS_PER_BLOCK <= cf.K[0]))   // nothing to build in a block of unused beta_d rows
+            tabblk.push_back(TabBlock{c->param_off[e], tab_off[e], cf.K[0], cf.K[1], cf.ktot, j0, e, cf.pixbeta, {0, 0}});
     }
     c->ntabblk = (int64_t)tabblk.size();
     int rc;
@@ -1013,6 +1027,7 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     const size_t tab_bytes = (size_t)rows * NROW * sizeof(float), part_bytes = (size_t)batch * PS * sizeof(double);
     c->sel_cap = (((int64_t)batch * (1 + (int64_t)((sizeof(Run) + sizeof(PosInfo)) / 4)) + 16) + 3) & ~(int64_t)3;   // slots stay 16-byte aligned
     if (cudaMalloc((void **)&c->d_tab, tab_bytes) != cudaSuccess || cudaMalloc((void **)&c->d_partial, part_bytes) != cudaSuccess ||
+        cudaMalloc((void **)&c->d_pcopy, (size_t)std::max<int64_t>(c->nparam, 1) * sizeof(double)) != cudaSuccess ||
         (copy_bytes > 0 && cudaMalloc((void **)&c->d_copy, (size_t)copy_bytes) != cudaSuccess) ||
         cudaMalloc((void **)&c->d_sel, (size_t)(cs_ctx::SEL_RING * c->sel_cap * 4)) != cudaSuccess ||
         cudaMallocHost((void **)&c->h_sel, (size_t)(cs_ctx::SEL_RING * c->sel_cap * 4)) != cudaSuccess) {
@@ -1020,7 +1035,7 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         free_batch(c);
         return CS_ENOMEM;
     }
-    c->batch_bytes += (int64_t)(tab_bytes + part_bytes) + copy_bytes + cs_ctx::SEL_RING * c->sel_cap * 4;
+    c->batch_bytes += (int64_t)(tab_bytes + part_bytes) + c->nparam * 8 + copy_bytes + cs_ctx::SEL_RING * c->sel_cap * 4;
     c->copy_bytes = copy_bytes;
     c->batch = batch;
     if (c->d && !c->jobs.empty()) {
@@ -1040,6 +1055,8 @@ int cs_param_offsets(cs_ctx *c, int64_t *off) {
 int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
     if (!c || c->batch <= 0 || !params) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
+    // the parameters the tables belong to: read by the per-pixel beta_d path of the direct kernel
+    CK(cudaMemcpyAsync(c->d_pcopy, params, (size_t)c->nparam * sizeof(double), cudaMemcpyDeviceToDevice, st));
     if (c->ntabblk > 0)
         k_tables<<<(unsigned)c->ntabblk, 256, 0, st>>>(params, c->d_tabblk, c->d_tab, c->d_err, c->d_tc, c->skip);
     c->launches++;
@@ -1104,7 +1121,7 @@ static int maps_impl(cs_ctx *c, int32_t nsel, const int32_t *entries, const int3
     }
     const int64_t poff = ((int64_t)nsel + 3) & ~(int64_t)3;   // position info starts 16-byte aligned, the runs follow it
     PosInfo *hp = reinterpret_cast<PosInfo *>(hs + poff);
-    for (int32_t i = 0; i < nsel; ++i) hp[i] = PosInfo{c->tab_off[hs[i]], (int64_t)(data_sel ? data_sel[i] : c->data_of[hs[i]])};
+    for (int32_t i = 0; i < nsel; ++i) hp[i] = PosInfo{c->tab_off[hs[i]], (int64_t)(data_sel ? data_sel[i] : c->data_of[hs[i]]), c->param_off[hs[i]], 0};
     const int64_t roff = poff + (int64_t)nsel * (int64_t)(sizeof(PosInfo) / 4);
     Run *hr = reinterpret_cast<Run *>(hs + roff);
     int32_t nrun = 0;

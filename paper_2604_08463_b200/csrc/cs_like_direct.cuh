@@ -15,6 +15,7 @@
 #pragma once
 #include "cs_pipe.cuh"
 #include "cs_math.cuh"
+#include "cs_tables.cuh"   // powerlaw_value: the per-pixel beta_d path evaluates the table kernel's own expression
 
 namespace cs {
 
@@ -128,16 +129,27 @@ __global__ void __launch_bounds__(DR_THREADS, 1) k_like_direct(const __grid_cons
         const int rB_fd = max(k0B, 0) * NROW, rB_g = (K0 + max(k1B, 0)) * NROW, rB_dg = (K0 + K1 + max(k1B, 0)) * NROW,
                   rB_fs = (K0 + 2 * K1 + max(k2B, 0)) * NROW;
 
+        // beta_d (nearly) per pixel (CfgDev::pixbeta): every beta_d row would be built, written and read for one or two
+        // pixels, 128 B of traffic per pixel-eval next to the 120 B of data; the row's values are evaluated here instead,
+        // from the parameter copy, in compensated fp32 for both pixels at once (cs_tables.cuh: powerlaw_pair_f32)
+        const bool pixbeta = cf->pixbeta != 0;
         for (int k = w.k; k < w.kend; ++k) {
             const int e = __ldg(P.elist + w.run.estart + k);
             if (P.skip && __ldg(P.skip + e) != 0) continue;
             const int sd = n % ND;
             const float *tb = P.tab + __ldg(&P.pinfo[w.run.estart + k].tab_row) * NROW;
             const float *st = st0 + sd * STAGE;
+            float2 bh = make_float2(0.f, 0.f), bl = bh;   // beta_d of the two pixels as float pairs
+            if (pixbeta) {
+                const double *pe = P.pcopy + __ldg(&P.pinfo[w.run.estart + k].param_off);
+                const double betaA = __ldg(pe + max(k0A, 0)), betaB = __ldg(pe + max(k0B, 0));
+                bh = make_float2((float)betaA, (float)betaB);
+                bl = make_float2((float)(betaA - (double)bh.x), (float)(betaB - (double)bh.y));
+            }
             if (k + 1 < w.kend) {   // the next entry's rows on their way to L1 while this entry is computed
                 const float *tn = P.tab + __ldg(&P.pinfo[w.run.estart + k + 1].tab_row) * NROW;
-                if (liveA) { prefetch_row(tn + rA_fd); prefetch_row(tn + rA_g); prefetch_row(tn + rA_fs); if (kGrad) prefetch_row(tn + rA_dg); }
-                if (liveB) { prefetch_row(tn + rB_fd); prefetch_row(tn + rB_g); prefetch_row(tn + rB_fs); if (kGrad) prefetch_row(tn + rB_dg); }
+                if (liveA) { if (!pixbeta) prefetch_row(tn + rA_fd); prefetch_row(tn + rA_g); prefetch_row(tn + rA_fs); if (kGrad) prefetch_row(tn + rA_dg); }
+                if (liveB) { if (!pixbeta) prefetch_row(tn + rB_fd); prefetch_row(tn + rB_g); prefetch_row(tn + rB_fs); if (kGrad) prefetch_row(tn + rB_dg); }
             }
             mbar_wait(&full_d[sd], (uint32_t)((n / ND) & 1));
             const float4 *aFd = reinterpret_cast<const float4 *>(tb + rA_fd), *aG = reinterpret_cast<const float4 *>(tb + rA_g);
@@ -151,8 +163,21 @@ __global__ void __launch_bounds__(DR_THREADS, 1) k_like_direct(const __grid_cons
             float2 wdk[NROW], wsk[NROW];   // kept for the second pass of MODE_CHI2 only
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const float4 xFd = __ldg(aFd + q), xG = __ldg(aG + q), xFs = __ldg(aFs + q);
-                const float4 yFd = __ldg(bFd + q), yG = __ldg(bG + q), yFs = __ldg(bFs + q);
+                float4 xFd, yFd;
+                if (pixbeta) {
+                    float a[4], b[4];
+#pragma unroll
+                    for (int h = 0; h < 4; ++h) {
+                        const int f = 4 * q + h;   // bands beyond nfreq: cdf = 0
+                        const float2 v = powerlaw_pair_f32(P.cdf[f], P.l2h[f], P.l2l[f], bh, bl);
+                        a[h] = v.x; b[h] = v.y;
+                    }
+                    xFd = make_float4(a[0], a[1], a[2], a[3]); yFd = make_float4(b[0], b[1], b[2], b[3]);
+                } else {
+                    xFd = __ldg(aFd + q); yFd = __ldg(bFd + q);
+                }
+                const float4 xG = __ldg(aG + q), xFs = __ldg(aFs + q);
+                const float4 yG = __ldg(bG + q), yFs = __ldg(bFs + q);
                 float4 xdG = make_float4(0.f, 0.f, 0.f, 0.f), ydG = xdG;
                 if (kGrad) { xdG = __ldg(adG + q); ydG = __ldg(bdG + q); }
                 const float2 vFd[4] = {{xFd.x, yFd.x}, {xFd.y, yFd.y}, {xFd.z, yFd.z}, {xFd.w, yFd.w}};

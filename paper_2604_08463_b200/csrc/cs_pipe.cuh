@@ -44,6 +44,8 @@ struct LikeParams {
     int64_t PS;                // doubles per partial row
     float *maps_out;           // MODE_MAPS: [nsel,3,2,npix]
     int32_t *err;
+    const double *pcopy;       // copy of the parameters the tables were built from (per-pixel beta_d path)
+    float cdf[NROW], l2h[NROW], l2l[NROW];   // cd[f] and log2(nu_f/nu0d) as a float pair (per-pixel beta_d path)
     KConst kc;
 };
 

@@ -41,6 +41,35 @@ __device__ __forceinline__ double exp_pow(double y) {
     return ok ? res : out_of_range;
 }
 
+// One value of a power-law row, band constant folded in: c (nu/nu0)^beta = c exp(beta ln(nu/nu0)), rounded to fp32.
+// Written once: k_tables and the direct kernel's per-pixel beta_d path (CfgDev::pixbeta) must give the same bits.
+__device__ __forceinline__ float powerlaw_value(double c, double lnr, double beta) {
+    return (float)__dmul_rn(c, exp_pow(__dmul_rn(beta, lnr)));
+}
+
+// The same value for two pixels at once in fp32, for the direct kernel's per-pixel beta_d path (CfgDev::pixbeta):
+// c 2^(beta L), L = log2(nu/nu0), with beta and L as float pairs (hi, lo) so that the exponent beta L is known to 1e-14:
+// p = bh Lh (rounded), e = fma(bh, Lh, -p) (its error, exact), s = e + bh Ll + bl Lh; k = rint(p); r = (p - k) + s with
+// |r| <= 1/2; 2^r by MUFU.EX2 (at most two units in the last place), 2^k through the exponent field (k clamped to the
+// normal range: beyond it the fp32 table value would be 0 or inf as well).  Relative error <= 2.5e-7 (the table rows
+// are correctly rounded, 6e-8); the fp64 expression above costs the direct kernel, which has eight consumer warps per
+// SM to fill the fp64 pipe with, more than it saves (measured: DESIGN.md section 7).
+__device__ __forceinline__ float2 powerlaw_pair_f32(float ch, float Lh, float Ll, float2 bh, float2 bl) {
+    const float2 p = __fmul2_rn(bh, make_float2(Lh, Lh));
+    const float2 e = __ffma2_rn(bh, make_float2(Lh, Lh), make_float2(-p.x, -p.y));
+    const float2 s = __ffma2_rn(bh, make_float2(Ll, Ll), __ffma2_rn(bl, make_float2(Lh, Lh), e));
+    const float2 magic = make_float2(12582912.f, 12582912.f);
+    const float2 t = __fadd2_rn(p, magic);
+    const float2 kf = __fadd2_rn(t, make_float2(-12582912.f, -12582912.f));
+    const float2 r = __fadd2_rn(__fadd2_rn(p, make_float2(-kf.x, -kf.y)), s);
+    float ex, ey;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(r.x));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ey) : "f"(r.y));
+    const int kx = min(max((int)kf.x, -126), 127), ky = min(max((int)kf.y, -126), 127);
+    const float2 sc = make_float2(__int_as_float((kx + 127) << 23), __int_as_float((ky + 127) << 23));
+    return __fmul2_rn(__fmul2_rn(make_float2(ch, ch), sc), make_float2(ex, ey));
+}
+
 // 1/a for a normal positive double: MUFU.RCP64H seed (about 20 bits) and two Newton steps (error ~1 ulp, no slow path).
 __device__ __forceinline__ double rcp_pos(double a) {
     double r;
@@ -60,7 +89,7 @@ struct TabBlock {
     int64_t param_off;   // first parameter of the entry
     int64_t tab_row;     // first table row of the entry
     int32_t K0, K1, ktot, j0;
-    int32_t e, pad[3];
+    int32_t e, pixbeta, pad[2];   // pixbeta: the beta_d rows of this entry are not built (CfgDev::pixbeta)
 };
 constexpr int TAB_SUB = 4;                       // parameters per thread quad
 constexpr int TAB_ROWS_PER_BLOCK = 64 * TAB_SUB;
@@ -75,6 +104,7 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
     const int4 b0 = __ldg(bp), b1 = __ldg(bp + 1), b2 = __ldg(bp + 2);
     const int64_t param_off = ((int64_t)(uint32_t)b0.y << 32) | (uint32_t)b0.x, tab_row = ((int64_t)(uint32_t)b0.w << 32) | (uint32_t)b0.z;
     const int K0 = b1.x, K1 = b1.y, ktot = b1.z, j0 = b1.w, e = b2.x;
+    const bool pixbeta = b2.y != 0;
     if (skip && skip[e] != 0) return;
     const int f0 = (threadIdx.x & 3) * 4;
     // the block's TAB_SUB x 64 parameters: all loads first (one latency for the block), then the rows one after the other
@@ -98,9 +128,10 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
     bad = bad || !isfinite(x);
     float v[4];
     if (j < K0) {
+        if (pixbeta) continue;   // evaluated per pixel by the direct kernel
         // dust power-law factor with the band constant folded in: cd[f] * (nu_f/nu0d)^beta_d
 #pragma unroll
-        for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cd[f0 + i] * exp_pow(x * tc.lnd[f0 + i])) : 0.f;
+        for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? powerlaw_value(tc.cd[f0 + i], tc.lnd[f0 + i], x) : 0.f;
         *reinterpret_cast<float4 *>(row0 + (int64_t)j * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
     } else if (j < K0 + K1) {
         // Planck ratio G = expm1(x0)/expm1(x) and d ln G / dT = (1/T) [ h(x) - h(x0) ],
@@ -125,7 +156,7 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
     } else {
         const int k = j - K0 - K1;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? (float)(tc.cs[f0 + i] * exp_pow(x * tc.lns[f0 + i])) : 0.f;
+        for (int i = 0; i < 4; ++i) v[i] = (f0 + i < nfreq) ? powerlaw_value(tc.cs[f0 + i], tc.lns[f0 + i], x) : 0.f;
         *reinterpret_cast<float4 *>(row0 + (int64_t)(K0 + 2 * K1 + k) * NROW + f0) = make_float4(v[0], v[1], v[2], v[3]);
     }
     }
