@@ -13,6 +13,7 @@
 // entries the consumers meet at a named barrier and sum the segments (one thread per (entry, term, segment), fp64,
 // the chunk tree of cs_math.cuh) into the partial buffer.  The term buffer is double buffered.
 #pragma once
+#include <type_traits>
 #include "cs_pipe.cuh"
 #include "cs_math.cuh"
 #include "cs_tables.cuh"   // powerlaw_value: the per-pixel beta_d path evaluates the table kernel's own expression
@@ -132,7 +133,10 @@ __global__ void __launch_bounds__(DR_THREADS, 1) k_like_direct(const __grid_cons
         // beta_d (nearly) per pixel (CfgDev::pixbeta): every beta_d row would be built, written and read for one or two
         // pixels, 128 B of traffic per pixel-eval next to the 120 B of data; the row's values are evaluated here instead,
         // from the parameter copy, in compensated fp32 for both pixels at once (cs_tables.cuh: powerlaw_pair_f32)
-        const bool pixbeta = cf->pixbeta != 0;
+        // The entry loop exists twice, with and without that path, so that the ordinary one keeps its registers and
+        // schedule (with the branch inside one loop the component maps ran a quarter slower).
+        auto entry_loop = [&](auto pb) {
+        constexpr bool pixbeta = decltype(pb)::value;
         for (int k = w.k; k < w.kend; ++k) {
             const int e = __ldg(P.elist + w.run.estart + k);
             if (P.skip && __ldg(P.skip + e) != 0) continue;
@@ -256,6 +260,8 @@ __global__ void __launch_bounds__(DR_THREADS, 1) k_like_direct(const __grid_cons
             }
             ++n;
         }
+        };
+        if (cf->pixbeta != 0) entry_loop(std::true_type{}); else entry_loop(std::false_type{});
         if (kReduce && nbuf > 0) {   // the tile changes (or the share ends): flush what is buffered with this tile's plan
             __threadfence_block();
             named_sync(1, NCONS);
