@@ -157,7 +157,10 @@ CS_API int cs_param_offsets(cs_ctx *ctx, int64_t *off);
 
 /* a1 (Eq. 2): per entry, cluster and band the separable SED factors cd*(nu/nu0d)^beta_d, the Planck ratio
  * B-factor G(nu,T_d), its log-derivative dlnG/dT_d and cs*(nu/nu0s)^beta_s, evaluated in fp64 and stored fp32.
- * params dev fp64 (layout above).  Sets the sticky device bit CS_EDOMAIN on T_d <= 0 / non-finite input. */
+ * params dev fp64 (layout above).  Sets the sticky device bit CS_EDOMAIN on T_d <= 0 / non-finite input.
+ * The library keeps its own copy of `params` (made on `stream`): the caller may overwrite them after the call.  For a
+ * configuration that stays in place with beta_d (nearly) per pixel (CS_OPT_PIXEL_BETA) the beta_d rows are not built;
+ * the fused kernel evaluates them per pixel from that copy (relative error <= 2.5e-7 instead of 6e-8; same tolerances). */
 CS_API int cs_build_sed_tables(cs_ctx *ctx, const double *params, void *stream);
 
 /* a2+a3: fused per-pixel likelihood / gradient and the ordered fp64 reduction onto clusters, for the tables last
@@ -190,7 +193,7 @@ CS_API int cs_cmb_residual_maps(cs_ctx *ctx, int32_t nsel, const int32_t *entrie
 
 /* f3, the cell-compressed likelihood (PAPER.md:L95 patch model, L80 Eq. 6): pixels with the same cluster triple share
  * A, so their part of Eq. 6 is tr(M^-1 A^T T A) with the parameter-independent second moments
- * T = N^-1 (sum_{p,S} d_S d_S^T) N^-1 of the cell.  cs_cell_moments builds T (fp64) for every (configuration, data set)
+ * T = N^-1 (sum_{p,S} d_S d_S^T) N^-1 of the cell.  cs_cell_moments builds T (fp64, on the fp64 tensor cores, from the pair's private sorted copy) for every (configuration, data set)
  * pair of the current batch from the current data -- call it once after cs_set_data / cs_set_batch, and again when the
  * data change; it allocates its workspace on the first call.  cs_spectral_like_grad_cells then evaluates nll and grad
  * (same meaning, layout and tolerances as cs_spectral_like_grad) for the tables last built, from T alone, in fp64: one
