@@ -124,8 +124,10 @@ struct cs_ctx {
     std::vector<CopyJob> jobs;          // private copies of the sorted layout, ordered by data set
     int32_t *d_cfg_of = nullptr, *d_data_of = nullptr, *d_elist = nullptr;
     int64_t *d_param_off = nullptr, *d_tab_off = nullptr;
-    TabBlock *d_tabblk = nullptr;      // k_tables' work list: 64-parameter blocks of every entry
+    TabBlock *d_tabblk = nullptr;      // k_tables' work list: blocks of TAB_ROWS_PER_BLOCK parameters of every entry
     int64_t ntabblk = 0;
+    MergeBlock *d_mblk = nullptr;      // k_merge's work list: [region blocks of every entry | cluster blocks of every entry]
+    int64_t nmblk_region = 0, nmblk_all = 0;
     PosInfo *d_pinfo = nullptr;
     Run *d_runs = nullptr;
     CopyJob *d_jobs = nullptr;
@@ -204,11 +206,11 @@ void free_opt(cs_ctx *c) {
 
 void free_batch(cs_ctx *c) {
     cudaFree(c->d_cfg_of); cudaFree(c->d_data_of); cudaFree(c->d_elist);
-    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_tabblk); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
+    cudaFree(c->d_param_off); cudaFree(c->d_tab_off); cudaFree(c->d_tabblk); cudaFree(c->d_mblk); cudaFree(c->d_pinfo); cudaFree(c->d_runs); cudaFree(c->d_jobs);
     cudaFree(c->d_tab); cudaFree(c->d_partial); cudaFree(c->d_copy); cudaFree(c->d_pcopy);
     c->d_pcopy = nullptr;
     c->d_cfg_of = c->d_data_of = c->d_elist = nullptr;
-    c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr; c->d_tabblk = nullptr; c->ntabblk = 0;
+    c->d_param_off = c->d_tab_off = nullptr; c->d_pinfo = nullptr; c->d_tabblk = nullptr; c->ntabblk = 0; c->d_mblk = nullptr; c->nmblk_region = c->nmblk_all = 0;
     c->d_runs = nullptr; c->d_jobs = nullptr;
     c->d_tab = nullptr; c->d_partial = nullptr; c->d_copy = nullptr;
     c->batch = 0; c->nrun_sc = c->nrun_dir = 0; c->batch_bytes = 0; c->copy_bytes = 0;
@@ -1014,8 +1016,15 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
             tabblk.push_back(TabBlock{c->param_off[e], tab_off[e], cf.K[0], cf.K[1], cf.ktot, j0, e, cf.pixbeta, {0, 0}});
     }
     c->ntabblk = (int64_t)tabblk.size();
+    std::vector<MergeBlock> mblk;
+    for (int32_t e = 0; e < batch; ++e)
+        for (int32_t r = 0; r < c->nregion; ++r) mblk.push_back(MergeBlock{e, -(r + 1)});
+    c->nmblk_region = (int64_t)mblk.size();
+    for (int32_t e = 0; e < batch; ++e)
+        for (int32_t b = 0; b * 256 < c->cfgs[cfg_of[e]].ktot; ++b) mblk.push_back(MergeBlock{e, b});
+    c->nmblk_all = (int64_t)mblk.size();
     int rc;
-    if ((rc = dev_upload(&c->d_tabblk, tabblk, &c->batch_bytes)) ||
+    if ((rc = dev_upload(&c->d_tabblk, tabblk, &c->batch_bytes)) || (rc = dev_upload(&c->d_mblk, mblk, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_cfg_of, c->cfg_of, &c->batch_bytes)) || (rc = dev_upload(&c->d_data_of, c->data_of, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_elist, c->elist, &c->batch_bytes)) ||
         (rc = dev_upload(&c->d_param_off, c->param_off, &c->batch_bytes)) || (rc = dev_upload(&c->d_tab_off, tab_off, &c->batch_bytes)) ||
@@ -1066,12 +1075,9 @@ int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
 }
 
 static int merge_launch(cs_ctx *c, double *nll, double *grad, cudaStream_t st) {
-    for (int e0 = 0; e0 < c->batch; e0 += 65535) {
-        const int nb = std::min(65535, c->batch - e0);
-        dim3 grid((grad ? (c->ktot_max + 255) / 256 : 0) + c->nregion, nb);   // cluster blocks, then one block per region
-        k_merge<<<grid, 256, 0, st>>>(c->d_partial + (int64_t)e0 * c->PS, c->PS, c->d_maps, c->d_cfgs, c->d_cfg_of + e0,
-                                     c->d_param_off + e0, c->nregion, grad ? 1 : 0, nll + (int64_t)e0 * c->nregion, grad,
-                                     c->skip ? c->skip + e0 : nullptr);
+    const int64_t nblk = grad ? c->nmblk_all : c->nmblk_region;   // value only: the region blocks at the head of the list
+    if (nblk > 0) {
+        k_merge<<<(unsigned)nblk, 256, 0, st>>>(c->d_partial, c->PS, c->d_cfgs, c->d_cfg_of, c->d_param_off, c->nregion, c->d_mblk, nll, grad, c->skip);
         c->launches++;
     }
     CK(cudaGetLastError());

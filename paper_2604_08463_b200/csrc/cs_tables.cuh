@@ -178,8 +178,14 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
 // times the threads, each with the same chain of pointer loads in front of one or two slots; warp-cooperative sums from
 // 16 slots on -- a warp full of T_d clusters then walks them one after the other.  One thread per long range was the
 // long pole of the whole kernel: 1536 dependent adds for a K = 1 map, 192 rounds of loads per lane for a region at nside 128.)
-// grid = (ceil(ktot_max / 256) [cluster blocks, want_grad only] + nregion [region blocks], batch), block = 256.
+// grid = the batch's work list of blocks (host-built: per entry ceil(ktot / 256) cluster blocks when the gradient is wanted,
+// then one block per region -- entries of one batch own between 12 and 6000 parameters, a 2-D grid sized for the
+// largest left most blocks without work), block = 256.
 constexpr int MERGE_LONG = 64;
+struct MergeBlock {
+    int32_t e;   // entry
+    int32_t b;   // >= 0: cluster block (parameters [256 b, 256 b + 256)); < 0: region -(b + 1)
+};
 __device__ __forceinline__ double merge_block_sum(const double *__restrict__ row, int a, int b, double *wsum) {
     double acc = 0.0;
 #pragma unroll 8
@@ -194,25 +200,24 @@ __device__ __forceinline__ double merge_block_sum(const double *__restrict__ row
     for (int i = 1; i < 8; ++i) tot += wsum[i];
     return tot;
 }
-__global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const MapDev *__restrict__ maps,
-                                               const CfgDev *__restrict__ cfgs, const int32_t *__restrict__ cfg_of,
-                                               const int64_t *__restrict__ param_off, int32_t nregion, int32_t want_grad,
-                                               double *__restrict__ nll, double *__restrict__ grad, const int32_t *__restrict__ skip) {
+__global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partial, int64_t PS, const CfgDev *__restrict__ cfgs,
+                                               const int32_t *__restrict__ cfg_of, const int64_t *__restrict__ param_off, int32_t nregion,
+                                               const MergeBlock *__restrict__ blocks, double *__restrict__ nll, double *__restrict__ grad,
+                                               const int32_t *__restrict__ skip) {
     __shared__ double wsum[8];
     __shared__ int32_t s_long[256][3];   // (a, b, offset of the term's block in the row) of this block's long clusters, by thread
     __shared__ int32_t s_who[256], s_nlong;
-    const int e = blockIdx.y;
+    const MergeBlock mb = blocks[blockIdx.x];
+    const int e = mb.e;
     if (skip && skip[e] != 0) return;
     const CfgDev *c = cfgs + cfg_of[e];
     const double *erow = partial + (int64_t)e * PS;
-    const int nblk_cluster = (int)gridDim.x - nregion;
-    if ((int)blockIdx.x < nblk_cluster) {
+    if (mb.b >= 0) {
         const int K0 = c->K[0], K1 = c->K[1], ktot = c->ktot;
-        if ((int)(blockIdx.x * blockDim.x) >= ktot) return;   // block-uniform
         if (threadIdx.x == 0) s_nlong = 0;
         __syncthreads();
-        const int v = blockIdx.x * blockDim.x + threadIdx.x;
-        const int64_t dst0 = param_off[e] + (int64_t)blockIdx.x * blockDim.x;
+        const int v = mb.b * 256 + threadIdx.x;
+        const int64_t dst0 = param_off[e] + (int64_t)mb.b * 256;
         if (v < ktot) {
             int t, k;
             if (v < K0) { t = 0; k = v; }
@@ -240,7 +245,7 @@ __global__ void __launch_bounds__(256) k_merge(const double *__restrict__ partia
             if (threadIdx.x == 0) grad[dst0 + who] = tot;
         }
     } else {
-        const int r = (int)blockIdx.x - nblk_cluster;
+        const int r = -(mb.b + 1);
         const int32_t *ksegptr = c->kseg[3];
         const int a = __ldg(ksegptr + r), b = __ldg(ksegptr + r + 1);
         const double tot = merge_block_sum(erow + c->segbase[3], a, b, wsum);
