@@ -210,6 +210,20 @@ def test_per_pixel_beta_d_path(torch_cuda):
             assert np.all(dg <= 5e-5 * ref["absg"] + 5e-7 * ref["gscale"]), (dg / (5e-5 * ref["absg"] + 5e-7 * ref["gscale"])).max()
 
 
+def test_random_labels_stress_the_tile_plans(torch_cuda, path):
+    """Cluster maps without any spatial structure (labels drawn at random, independently per map): every tile of the
+    sorted layout holds the most cells it may (64), every term has the most segments and chunks a tile header can
+    carry, cells are one or two pixels; in place the ranks of a tile are spread over all clusters.  Nothing in the
+    kernels may depend on K-means compactness (SURVEY.md 8(f4 iii))."""
+    w = gen.make_config(0, nside=16, batch=2, ndata=2)
+    g = gen.rng_for("misc", 31)
+    for K in ((7, 300, 41), (64, 64, 64), (1500, 3, 2)):
+        maps = np.stack([g.integers(0, k, w.npix).astype(np.int32) for k in K])
+        maps[:, g.random(w.npix) < 0.05] = -1
+        ww = dataclasses.replace(w, maps=maps, Kmap=np.array(K, dtype=np.int32))
+        _parity(ww, ww.params_jittered(seed=17))
+
+
 def test_empty_clusters_give_exact_zero(torch_cuda, path):
     """R9: labels are not compacted; a cluster without pixels gets gradient exactly 0."""
     w = gen.make_config(0)
