@@ -50,6 +50,7 @@ struct MomJob {
     int32_t cfg, data;
     int64_t off;        // double offset of the pair's moments [CC_NMOM][ncell] inside the moments buffer
     int64_t copy_off;   // float offset of the pair's private sorted copy inside dcopy
+    int64_t tstride;    // floats from one tile of the copy to the next
 };
 
 // Second moments of one (configuration, data set) pair: T = N^-1 (D_Q D_Q^T + D_U D_U^T) N^-1 with D_S the [nfreq x pixels]
@@ -85,7 +86,7 @@ __global__ void __launch_bounds__(128) k_cc_moments(const float *__restrict__ dc
         float q0 = 0.f, u0 = 0.f, q1 = 0.f, u1 = 0.f;
         if (j < len) {
             const int pos = pos0 + j, tile = pos / TPX, within = pos - tile * TPX;
-            const float *src = dd + (int64_t)tile * nrows * TPX + (within / HALF) * nrows * HALF + (within % HALF);
+            const float *src = dd + (int64_t)tile * job.tstride + (within / HALF) * nrows * HALF + (within % HALF);
             if (has0) { q0 = __ldg(src + (2 * f0) * HALF); u0 = __ldg(src + (2 * f0 + 1) * HALF); }
             if (has1) { q1 = __ldg(src + (2 * f1) * HALF); u1 = __ldg(src + (2 * f1 + 1) * HALF); }
         }

@@ -9,7 +9,10 @@
 //                    always share their cell and the stream of a tile is one contiguous block in HBM.
 // Data layout in HBM:
 //   d        [ndata][nfreq][2][npix] fp32   borrowed from the caller
-//   dcopy    per (cfg, data) pair [ntile][2 halves][2*nfreq rows][256] fp32   private, sorted layout only
+//   dcopy    per sorted configuration [ntile][pairs of the configuration][2 halves][2*nfreq rows][256] fp32 ("tile-major":
+//            the copies of a configuration's (cfg, data) pairs are interleaved tile by tile, so that a CTA walking the
+//            entries of one tile reads one contiguous stretch -- with one copy after the other every 60-KB block of a
+//            6-GB batch lay in another 2-MB page and the stream ran 6 % slower than on a 1.5-GB batch)   private
 //   tab      per entry e a block of (K0 + 2*K1 + K2) rows x 16 fp32:
 //              rows [0,K0)            Fd'[k][f] = cd[f] * (nu_f/nu0d)^beta_d[k]
 //              rows [K0,K0+K1)        G  [k][f] = expm1(x0)/expm1(x_f),  x = h nu / (k_B T_d[k])
@@ -108,6 +111,7 @@ struct Run {
     int64_t ustart;
     const uint32_t *hdr;       // = cfgs[cfg].hdr, cfgs[cfg].hdrptr (sorted configurations; the loader's look-ahead reads
     const int32_t *hdrptr;     //   them from the run it already holds instead of chasing the configuration table)
+    int64_t tstride;           // floats from one tile of a private copy to the next (sorted configurations)
 };
 
 // What the roles of a fused kernel need to know about the entry at position i of the launch's entry list, in one

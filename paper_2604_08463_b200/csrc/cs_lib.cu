@@ -122,6 +122,7 @@ struct cs_ctx {
     std::vector<PosInfo> pinfo;         // per position of elist
     std::vector<Run> runs;
     std::vector<CopyJob> jobs;          // private copies of the sorted layout, ordered by data set
+    std::vector<int64_t> cfg_tstride;   // [ncfg] floats between consecutive tiles of a configuration's copies in this batch
     int32_t *d_cfg_of = nullptr, *d_data_of = nullptr, *d_elist = nullptr;
     int64_t *d_param_off = nullptr, *d_tab_off = nullptr;
     TabBlock *d_tabblk = nullptr;      // k_tables' work list: blocks of TAB_ROWS_PER_BLOCK parameters of every entry
@@ -963,7 +964,7 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         while (j < batch && cfg_of[c->elist[j]] == cfg_of[c->elist[i]]) ++j;
         const CfgDev &cf = c->cfgs[cfg_of[c->elist[i]]];
         const bool sc = is_sc(c->elist[i]);
-        Run r{cfg_of[c->elist[i]], i, j - i, cf.ntile, sc ? c->W_sc : c->W_dir, cf.hdr, cf.hdrptr};
+        Run r{cfg_of[c->elist[i]], i, j - i, cf.ntile, sc ? c->W_sc : c->W_dir, cf.hdr, cf.hdrptr, 0};   // tstride: below
         const int64_t units = (int64_t)cf.ntile * (j - i);
         if (sc) { c->W_sc += units; c->nrun_sc++; } else { c->W_dir += units; c->nrun_dir++; }
         c->runs.push_back(r);
@@ -971,6 +972,7 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     }
     // private copies of the sorted layout: one per (configuration, data set) pair, ordered by data set
     c->jobs.clear();
+    c->cfg_tstride.assign(c->ncfg, 0);
     c->copy_off.assign(batch, -1);
     c->job_ntile_max = 0;
     int64_t copy_floats = 0;
@@ -983,16 +985,28 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
                 if (seen.emplace(k, 0).second) order.push_back(k);
             }
         std::sort(order.begin(), order.end());
-        for (const auto &k : order) {
+        // tile-major (cs_internal.h): the pairs of a configuration are interleaved tile by tile
+        const int64_t blk = (int64_t)2 * c->nfreq * TPX;   // floats of one tile of one copy
+        std::vector<int32_t> npair(c->ncfg, 0), pidx(order.size(), 0);
+        for (size_t j = 0; j < order.size(); ++j) pidx[j] = npair[order[j].second]++;
+        std::vector<int64_t> cfgbase(c->ncfg, 0);
+        for (int32_t q = 0; q < c->ncfg; ++q) {
+            cfgbase[q] = copy_floats;
+            copy_floats += (int64_t)c->cfgs[q].ntile * npair[q] * blk * (npair[q] > 0 ? 1 : 0);
+            c->cfg_tstride[q] = (int64_t)npair[q] * blk;
+        }
+        for (size_t j = 0; j < order.size(); ++j) {
+            const auto &k = order[j];
             const CfgDev &cf = c->cfgs[k.second];
-            seen[k] = copy_floats;
-            c->jobs.push_back(CopyJob{k.second, k.first, copy_floats});
-            copy_floats += (int64_t)cf.ntile * 2 * c->nfreq * TPX;
+            const int64_t off = cfgbase[k.second] + (int64_t)pidx[j] * blk;
+            seen[k] = off;
+            c->jobs.push_back(CopyJob{k.second, k.first, off, c->cfg_tstride[k.second]});
             c->job_ntile_max = std::max(c->job_ntile_max, cf.ntile);
         }
         for (int32_t e = 0; e < batch; ++e)
             if (c->cfgs[cfg_of[e]].sorted) c->copy_off[e] = seen[std::make_pair(data_of[e], cfg_of[e])];
     }
+    for (Run &r : c->runs) r.tstride = c->cfg_tstride[r.cfg];
     c->pinfo.resize(batch);
     for (int32_t i = 0; i < batch; ++i) {
         const int32_t e = c->elist[i];
@@ -1136,7 +1150,7 @@ static int maps_impl(cs_ctx *c, int32_t nsel, const int32_t *entries, const int3
         const int32_t cf = c->cfg_of[hs[i]];
         int32_t j = i;
         while (j < nsel && c->cfg_of[hs[j]] == cf) ++j;
-        hr[nrun++] = Run{cf, i, j - i, c->ntile_ring, W, nullptr, nullptr};
+        hr[nrun++] = Run{cf, i, j - i, c->ntile_ring, W, nullptr, nullptr, 0};
         W += (int64_t)c->ntile_ring * (j - i);
         i = j;
     }
@@ -1176,7 +1190,7 @@ int cs_cell_moments(cs_ctx *c, void *stream) {
         std::map<std::pair<int32_t, int32_t>, int64_t> off;
         int64_t n = 0;
         for (size_t j = 0; j < c->jobs.size(); ++j) {
-            mj[j] = MomJob{c->jobs[j].cfg, c->jobs[j].data, n, c->jobs[j].off};
+            mj[j] = MomJob{c->jobs[j].cfg, c->jobs[j].data, n, c->jobs[j].off, c->jobs[j].tstride};
             off[std::make_pair(c->jobs[j].data, c->jobs[j].cfg)] = n;
             n += (int64_t)CC_NMOM * c->cellsh[c->jobs[j].cfg].ncell;
         }
@@ -1419,7 +1433,7 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
                 while (e2 < b && c->data_of[c->elist[e2]] < n1) ++e2;
                 if (e2 == a) continue;
                 int64_t &W = sc ? Wsc[ch] : Wdir[ch];
-                out[cnt_sc[ch] + cnt_dir[ch]] = Run{run.cfg, a, e2 - a, run.ntile, W, run.hdr, run.hdrptr};
+                out[cnt_sc[ch] + cnt_dir[ch]] = Run{run.cfg, a, e2 - a, run.ntile, W, run.hdr, run.hdrptr, run.tstride};
                 W += (int64_t)run.ntile * (e2 - a);
                 (sc ? cnt_sc[ch] : cnt_dir[ch])++;
             }

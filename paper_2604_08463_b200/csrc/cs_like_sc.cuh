@@ -184,7 +184,7 @@ __device__ __forceinline__ void sc_loader(const LikeParams &P, float *ring, uint
             mbar_wait(&empty_d[s], (uint32_t)(((n / ND) & 1) ^ 1));
             const uint32_t bytes = (uint32_t)nrows * TPX * 4u;
             mbar_expect_tx(&full_d[s], bytes);
-            const float *src = P.dcopy + srcinfo + (int64_t)w0.tile * nrows * TPX;
+            const float *src = P.dcopy + srcinfo + (int64_t)w0.tile * w0.run.tstride;
             if (NF * 2 == nrows) {
                 bulk_g2s(dst, src, bytes, &full_d[s], policy);
             } else {   // generic band count: the stage keeps 2*NF rows per half, the copy only 2*nfreq

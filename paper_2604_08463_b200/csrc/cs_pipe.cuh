@@ -222,9 +222,9 @@ __device__ __forceinline__ void loader_loop(const CUtensorMap *tmap, const LikeP
                     const uint32_t bytes = (uint32_t)nrows * TPX * 4u;
                     mbar_expect_tx(&full_d[s], bytes);
                     if (NF * 2 == nrows) {
-                        bulk_g2s(dst, P.dcopy + srcinfo + (int64_t)w.tile * nrows * TPX, bytes, &full_d[s], policy);
+                        bulk_g2s(dst, P.dcopy + srcinfo + (int64_t)w.tile * w.run.tstride, bytes, &full_d[s], policy);
                     } else {   // generic band count: the stage keeps 2*NF rows per half, the copy only 2*nfreq
-                        const float *src = P.dcopy + srcinfo + (int64_t)w.tile * nrows * TPX;
+                        const float *src = P.dcopy + srcinfo + (int64_t)w.tile * w.run.tstride;
                         bulk_g2s(dst, src, bytes / 2, &full_d[s], policy);
                         bulk_g2s(dst + NF * 2 * HALF, src + nrows * HALF, bytes / 2, &full_d[s], policy);
                     }

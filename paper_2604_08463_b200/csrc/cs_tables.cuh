@@ -275,11 +275,12 @@ __global__ void __launch_bounds__(128) k_cmbvar(const double *__restrict__ parti
     var[i] = n > 0 ? (s[2] / n - (s[0] / n) * (s[0] / n)) + (s[3] / n - (s[1] / n) * (s[1] / n)) : 0.0;
 }
 
-// Private copy of one data set in the sorted layout of one configuration: copy[tile][half][row][x] =
+// Private copy of one data set in the sorted layout of one configuration: copy[tile (stride job.tstride)][half][row][x] =
 // d[data][row][pospix[tile*TPX + half*256 + x]], zero at pad positions.  grid = (ntile, pairs), block = TPX.
 struct CopyJob {
     int32_t cfg, data;
-    int64_t off;   // float offset of the copy inside dcopy
+    int64_t off;       // float offset of the copy's tile 0 inside dcopy
+    int64_t tstride;   // floats from one tile of the copy to the next (see "tile-major" in cs_internal.h)
 };
 __global__ void __launch_bounds__(TPX) k_relayout(const float *__restrict__ d, int64_t npix, int32_t nrows, const CfgDev *__restrict__ cfgs,
                                                   const CopyJob *__restrict__ jobs, float *__restrict__ dcopy) {
@@ -290,7 +291,7 @@ __global__ void __launch_bounds__(TPX) k_relayout(const float *__restrict__ d, i
     const int x = threadIdx.x;
     const int32_t pix = cf->pospix[(int64_t)tile * TPX + x];
     const float *src = d + (int64_t)job.data * nrows * npix + (pix >= 0 ? pix : 0);
-    float *dst = dcopy + job.off + (int64_t)tile * nrows * TPX + (x >> 8) * nrows * HALF + (x & (HALF - 1));
+    float *dst = dcopy + job.off + (int64_t)tile * job.tstride + (x >> 8) * nrows * HALF + (x & (HALF - 1));
     for (int r = 0; r < nrows; ++r) dst[r * HALF] = (pix >= 0) ? __ldg(src + (int64_t)r * npix) : 0.f;
 }
 
