@@ -77,6 +77,39 @@ int dev_upload(T **dst, const std::vector<T> &src, int64_t *bytes) {
     return CS_OK;
 }
 
+// Device memory of cs_set_clusters: a clustering scan sets a thousand configurations of some thirty arrays each, so the
+// arrays are carved out of 64-MB chunks instead of one cudaMalloc apiece.
+struct Arena {
+    std::vector<void *> chunks;
+    char *cur = nullptr;
+    size_t left = 0;
+    void *alloc(size_t n) {
+        n = (std::max<size_t>(n, 1) + 255) & ~(size_t)255;
+        if (n > left) {
+            const size_t sz = std::max<size_t>(n, (size_t)64 << 20);
+            void *p = nullptr;
+            if (cudaMalloc(&p, sz) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+            chunks.push_back(p);
+            cur = (char *)p; left = sz;
+        }
+        void *r = cur;
+        cur += n; left -= n;
+        return r;
+    }
+    void release() {
+        for (void *p : chunks) cudaFree(p);
+        chunks.clear(); cur = nullptr; left = 0;
+    }
+};
+template <typename T>
+int arena_upload(Arena &ar, T **dst, const std::vector<T> &src, int64_t *bytes) {
+    *dst = (T *)ar.alloc(src.size() * sizeof(T));
+    if (!*dst) return CS_ENOMEM;
+    if (!src.empty() && cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return CS_ECUDA;
+    *bytes += (int64_t)((std::max<size_t>(src.size() * sizeof(T), 1) + 255) & ~(size_t)255);
+    return CS_OK;
+}
+
 }  // namespace
 
 struct cs_ctx {
@@ -107,6 +140,7 @@ struct cs_ctx {
     CfgDev *d_cfgs = nullptr;
     int32_t *d_npix_live = nullptr;
     int64_t cluster_bytes = 0;
+    Arena cl_arena;                     // every device array of cs_set_clusters
     // data
     const float *d = nullptr;
     int32_t ndata = 0;
@@ -178,22 +212,12 @@ struct cs_ctx {
 namespace {
 
 void free_clusters(cs_ctx *c) {
-    for (auto &m : c->maps) {
-        cudaFree(m.idx); cudaFree(m.rank); cudaFree(m.segptr); cudaFree(m.segdesc); cudaFree(m.segslot); cudaFree(m.ksegptr);
-        cudaFree(m.chunkptr); cudaFree(m.segcfirst);
-    }
+    c->cl_arena.release();   // every device array of the maps, the sorted layouts, the cell lists and the tables of them
     c->maps.clear();
-    for (auto &p : c->sorted) { cudaFree(p.hdr); cudaFree(p.hdrptr); cudaFree(p.cellid); cudaFree(p.cellptr); cudaFree(p.cellrows); cudaFree(p.pospix); }
     c->sorted.clear();
-    for (auto &p : c->cellsh) {
-        cudaFree(p.cellpos); cudaFree(p.celllen); cudaFree(p.cellreg);
-        for (int t = 0; t < 4; ++t) { cudaFree(p.kptr[t]); cudaFree(p.klist[t]); }
-    }
     c->cellsh.clear();
-    cudaFree(c->d_cells);
     c->d_cells = nullptr;
     c->ncell_max = 0;
-    cudaFree(c->d_maps); cudaFree(c->d_cfgs); cudaFree(c->d_npix_live);
     c->d_maps = nullptr; c->d_cfgs = nullptr; c->d_npix_live = nullptr;
     c->cfgs.clear();
     c->nmap = c->ncfg = 0;
@@ -241,7 +265,7 @@ struct MapPlanHost {   // host copies of what the tile headers of the sorted lay
     std::vector<uint16_t> rank, segdesc, segcfirst;
     std::vector<int32_t> segptr, segslot, chunkptr;
 };
-int build_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, MapHost *out, int64_t *bytes, MapPlanHost *keep = nullptr) {
+int build_map_plan(Arena &ar, const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, MapHost *out, int64_t *bytes, MapPlanHost *keep = nullptr) {
     std::vector<uint16_t> rank((size_t)ntile * TPX, (uint16_t)NORANK);
     std::vector<int32_t> segptr(ntile + 1, 0);
     std::vector<uint16_t> segdesc;
@@ -297,14 +321,14 @@ int build_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, M
     std::copy(idx, idx + npos, idxv.begin());
     out->K = K; out->nseg = nseg;
     int rc;
-    if ((rc = dev_upload(&out->idx, idxv, bytes))) return rc;
-    if ((rc = dev_upload(&out->rank, rank, bytes))) return rc;
-    if ((rc = dev_upload(&out->segptr, segptr, bytes))) return rc;
-    if ((rc = dev_upload(&out->segdesc, segdesc, bytes))) return rc;
-    if ((rc = dev_upload(&out->segslot, segslot, bytes))) return rc;
-    if ((rc = dev_upload(&out->ksegptr, ksegptr, bytes))) return rc;
-    if ((rc = dev_upload(&out->chunkptr, chunkptr, bytes))) return rc;
-    if ((rc = dev_upload(&out->segcfirst, segcfirst, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->idx, idxv, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->rank, rank, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segptr, segptr, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segdesc, segdesc, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segslot, segslot, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->ksegptr, ksegptr, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->chunkptr, chunkptr, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segcfirst, segcfirst, bytes))) return rc;
     if (keep) {
         keep->rank.swap(rank); keep->segdesc.swap(segdesc); keep->segcfirst.swap(segcfirst);
         keep->segptr.swap(segptr); keep->segslot.swap(segslot); keep->chunkptr.swap(chunkptr);
@@ -790,11 +814,11 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     c->maps.resize(nmap + 1);
     int rc;
     for (int32_t m = 0; m < nmap; ++m)
-        if ((rc = build_map_plan(h.data() + (size_t)m * npix, Kmap[m], npix, c->ntile_ring, &c->maps[m], &c->cluster_bytes))) {
+        if ((rc = build_map_plan(c->cl_arena, h.data() + (size_t)m * npix, Kmap[m], npix, c->ntile_ring, &c->maps[m], &c->cluster_bytes))) {
             free_clusters(c);
             return rc;
         }
-    if ((rc = build_map_plan(reg.data(), nregion, npix, c->ntile_ring, &c->maps[nmap], &c->cluster_bytes))) {
+    if ((rc = build_map_plan(c->cl_arena, reg.data(), nregion, npix, c->ntile_ring, &c->maps[nmap], &c->cluster_bytes))) {
         free_clusters(c);
         return rc;
     }
@@ -827,15 +851,15 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
             plan_sorted(a, b, d, reg.data(), cf.K, npix, sp);
             if (c->opt_layout == CS_LAYOUT_SORTED || sp.fill >= c->opt_min_fill) {
                 SortedHost &sh = c->sorted[i];
-                if ((rc = dev_upload(&sh.cellid, sp.cellid, &c->cluster_bytes)) || (rc = dev_upload(&sh.cellptr, sp.cellptr, &c->cluster_bytes)) ||
-                    (rc = dev_upload(&sh.cellrows, sp.cellrows, &c->cluster_bytes)) || (rc = dev_upload(&sh.pospix, sp.pospix, &c->cluster_bytes))) {
+                if ((rc = arena_upload(c->cl_arena, &sh.cellid, sp.cellid, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.cellptr, sp.cellptr, &c->cluster_bytes)) ||
+                    (rc = arena_upload(c->cl_arena, &sh.cellrows, sp.cellrows, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.pospix, sp.pospix, &c->cluster_bytes))) {
                     free_clusters(c);
                     return rc;
                 }
                 const int64_t npos = (int64_t)sp.ntile * TPX;
                 for (int t = 0; t < 4; ++t) {
                     c->maps.emplace_back();
-                    if ((rc = build_map_plan(sp.idx[t].data(), t < 3 ? cf.K[t] : nregion, npos, sp.ntile, &c->maps.back(), &c->cluster_bytes, &mplan[t]))) {
+                    if ((rc = build_map_plan(c->cl_arena, sp.idx[t].data(), t < 3 ? cf.K[t] : nregion, npos, sp.ntile, &c->maps.back(), &c->cluster_bytes, &mplan[t]))) {
                         free_clusters(c);
                         return rc;
                     }
@@ -845,8 +869,8 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
                     CellsHost &ch = c->cellsh[i];
                     ch.ncell = (int32_t)sp.cellpos.size();
                     c->ncell_max = std::max(c->ncell_max, ch.ncell);
-                    if ((rc = dev_upload(&ch.cellpos, sp.cellpos, &c->cluster_bytes)) || (rc = dev_upload(&ch.celllen, sp.celllen, &c->cluster_bytes)) ||
-                        (rc = dev_upload(&ch.cellreg, sp.cellkey[3], &c->cluster_bytes))) {
+                    if ((rc = arena_upload(c->cl_arena, &ch.cellpos, sp.cellpos, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &ch.celllen, sp.celllen, &c->cluster_bytes)) ||
+                        (rc = arena_upload(c->cl_arena, &ch.cellreg, sp.cellkey[3], &c->cluster_bytes))) {
                         free_clusters(c);
                         return rc;
                     }
@@ -857,7 +881,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
                         for (int32_t k = 0; k < Kt; ++k) kp[k + 1] += kp[k];
                         std::vector<int32_t> fill(kp.begin(), kp.end() - 1);
                         for (int32_t q = 0; q < ch.ncell; ++q) kl[fill[sp.cellkey[t][q]]++] = q;
-                        if ((rc = dev_upload(&ch.kptr[t], kp, &c->cluster_bytes)) || (rc = dev_upload(&ch.klist[t], kl, &c->cluster_bytes))) {
+                        if ((rc = arena_upload(c->cl_arena, &ch.kptr[t], kp, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &ch.klist[t], kl, &c->cluster_bytes))) {
                             free_clusters(c);
                             return rc;
                         }
@@ -878,7 +902,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
         if (cf.sorted) {   // tile headers (they hold the slots, hence after segbase)
             pack_tile_headers(sp, mplan, cf.segbase, c->maps[cf.map[3]].nseg, hdrptr, hdrblob);
             SortedHost &sh = c->sorted[i];
-            if ((rc = dev_upload(&sh.hdr, hdrblob, &c->cluster_bytes)) || (rc = dev_upload(&sh.hdrptr, hdrptr, &c->cluster_bytes))) {
+            if ((rc = arena_upload(c->cl_arena, &sh.hdr, hdrblob, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.hdrptr, hdrptr, &c->cluster_bytes))) {
                 free_clusters(c);
                 return rc;
             }
@@ -898,9 +922,9 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
         for (int t = 0; t < 4; ++t) { cd[i].kptr[t] = ch.kptr[t]; cd[i].klist[t] = ch.klist[t]; }
         cd[i].ncell = ch.ncell;
     }
-    if ((rc = dev_upload(&c->d_maps, md, &c->cluster_bytes)) || (rc = dev_upload(&c->d_cfgs, c->cfgs, &c->cluster_bytes)) ||
-        (rc = dev_upload(&c->d_cells, cd, &c->cluster_bytes)) ||
-        (rc = dev_upload(&c->d_npix_live, c->npix_live, &c->cluster_bytes))) {
+    if ((rc = arena_upload(c->cl_arena, &c->d_maps, md, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &c->d_cfgs, c->cfgs, &c->cluster_bytes)) ||
+        (rc = arena_upload(c->cl_arena, &c->d_cells, cd, &c->cluster_bytes)) ||
+        (rc = arena_upload(c->cl_arena, &c->d_npix_live, c->npix_live, &c->cluster_bytes))) {
         free_clusters(c);
         return rc;
     }
