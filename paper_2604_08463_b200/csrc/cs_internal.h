@@ -35,13 +35,8 @@ constexpr int SEG_MAX = 32;    // longest run of ranks summed as one segment
 constexpr int CHUNK_LEN = 8;   // ranks per chunk (SEG_MAX / CHUNK_LEN <= 4 chunks per segment)
 constexpr int NROW = 16;       // floats per table row (nfreq padded to 16 -> 64-byte rows)
 constexpr int CELL_CAP = 64;   // sorted layout: most cells per tile (a builder lane builds cells lane and lane + 32)
-#ifdef CS_SC_FAT
-constexpr int CROW = 100;      // floats per cell row in shared memory: 5 columns x 16 + 16 scalars + 4 pad (= 4 mod 32 banks)
-constexpr int CR_WS = 12, CR_SC = 20;   // float4 offsets of the w a_s column and of the scalars
-#else
 constexpr int CROW = 68;       // floats per cell row in shared memory: 3 columns x 16 + 16 scalars + 4 pad (= 4 mod 32 banks)
 constexpr int CR_WS = 8, CR_SC = 12;    // float4 offsets of the w a_s column and of the scalars
-#endif
 constexpr int SC_CHUNK_CAP = 4 * (TPX / CHUNK_LEN + CELL_CAP);   // sorted layout: most chunks of the four terms of a tile
 constexpr int SC_SEG_CAP = 4 * (TPX / SEG_MAX + CELL_CAP);       // and most segments
 // Tile header of the sorted layout (one per configuration and tile, variable length, a multiple of 16 bytes; 32-bit words):

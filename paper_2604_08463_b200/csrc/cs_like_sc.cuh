@@ -224,16 +224,8 @@ __device__ __forceinline__ void sc_build_cell(const float4 (&Fd)[4], const float
         }
         o4[q] = make_float4(wd[0], wd[1], wd[2], wd[3]);
         o4[CR_WS + q] = make_float4(ws[0], ws[1], ws[2], ws[3]);
-#ifdef CS_SC_FAT
-        if (GRAD) {
-            o4[4 + q] = make_float4(u1[0], u1[1], u1[2], u1[3]);
-            o4[8 + q] = make_float4(u2[0], u2[1], u2[2], u2[3]);
-            o4[16 + q] = make_float4(u3[0], u3[1], u3[2], u3[3]);
-        }
-#else
         if (GRAD) o4[4 + q] = make_float4(u2[0], u2[1], u2[2], u2[3]);   // the other two derivative columns are one multiply
                                                                          // by a band constant away from w a_d and w a_s
-#endif
     }
     CellScal<float> C;
     cell_finish<GRAD>(S, kc.inv_m00, C);
@@ -396,21 +388,15 @@ __global__ void __launch_bounds__(SC_THREADS, 1) k_like_sc(const LikeParams P) {
             for (int q = 0; q < 4; ++q) {
                 const float4 WD = crow[q], WS = crow[CR_WS + q];
                 float4 U1 = make_float4(0.f, 0.f, 0.f, 0.f), U2 = U1, U3 = U1;
-#ifdef CS_SC_FAT
-                if (kGrad) { U1 = crow[4 + q]; U2 = crow[8 + q]; U3 = crow[16 + q]; }
-#else
                 if (kGrad) U2 = crow[4 + q];
-#endif
                 const float wd[4] = {WD.x, WD.y, WD.z, WD.w}, ws[4] = {WS.x, WS.y, WS.z, WS.w};
                 float u1[4] = {U1.x, U1.y, U1.z, U1.w}, u3[4] = {U3.x, U3.y, U3.z, U3.w};
                 const float u2[4] = {U2.x, U2.y, U2.z, U2.w};
-#ifndef CS_SC_FAT
                 if (kGrad) {   // the same products the builder formed for the cell's P sums (cs_math.cuh: cell_band)
 #pragma unroll
                     for (int h = 0; h < 4; ++h)
                         if (4 * q + h < NF) { u1[h] = mul_(kc.lnd[4 * q + h], wd[h]); u3[h] = mul_(kc.lns[4 * q + h], ws[h]); }
                 }
-#endif
 #pragma unroll
                 for (int h = 0; h < 4; ++h) {
                     const int f = 4 * q + h;

@@ -71,22 +71,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
         "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
 }
-// Wait used by producer roles (loader, builder): they are ahead of the consumers most of the time, so the poll
-// backs off (suspend hint + nanosleep) instead of burning issue slots the consumers need.
-__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity, unsigned sleep_ns = 40) {
-    uint32_t done = 0;
-    while (true) {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(done)
-            : "r"(smem_u32(bar)), "r"(parity), "r"(500u)
-            : "memory");
-        if (done) break;
-        __nanosleep(sleep_ns);
-    }
-}
 // global -> shared bulk copy completing on an mbarrier; dst/src/bytes 16-byte aligned.
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t policy) {
     asm volatile(
@@ -162,35 +146,6 @@ __device__ __forceinline__ bool walk_next(Walk &w, const LikeParams &P) {
     w.kend = (int32_t)((left < (int64_t)(w.run.count - w.k)) ? (int64_t)w.k + left : (int64_t)w.run.count);
     w.u += w.kend - w.k;
     return true;
-}
-
-// The same walk entry by entry, with the skipped entries left out: e = next live entry, newpiece = it starts a new
-// (run, tile) piece.  Lets a role look one entry ahead (the builder loads the next entry's table rows early).
-struct EntryWalk {
-    Walk w;
-    int k;
-    bool open;
-};
-__device__ __forceinline__ void entry_init(EntryWalk &it, const LikeParams &P) {
-    walk_init(it.w, P);
-    it.k = 0;
-    it.open = false;
-}
-__device__ __forceinline__ bool entry_next(EntryWalk &it, const LikeParams &P, int &e, int &pos, bool &newpiece) {
-    newpiece = false;
-    while (true) {
-        if (!it.open || it.k >= it.w.kend) {
-            if (!walk_next(it.w, P)) return false;
-            it.k = it.w.k;
-            it.open = true;
-            newpiece = true;
-        }
-        while (it.k < it.w.kend) {
-            pos = it.w.run.estart + it.k++;
-            e = __ldg(P.elist + pos);
-            if (!(P.skip && __ldg(P.skip + e) != 0)) return true;
-        }
-    }
 }
 
 // ----------------------------------------------------------------------------------------------------------
