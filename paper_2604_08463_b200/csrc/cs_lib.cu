@@ -7,7 +7,9 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <atomic>
 #include <map>
+#include <thread>
 #include <stdexcept>
 #include <new>
 #include <vector>
@@ -261,21 +263,27 @@ double krj2kcmb(double nu_ghz, double tcmb, double hk) {
 
 // Reduction plan of one term map in position space: per tile the rank of every position in the (cluster, position)
 // order, that order cut into segments of <= SEG_MAX positions of one cluster, plus the CSR cluster -> segments.
-struct MapPlanHost {   // host copies of what the tile headers of the sorted layout are packed from
+struct MapPlanHost {   // the reduction plan of one term map on the host: computed (on a worker thread), then uploaded
+    std::vector<int32_t> idx, segptr, segslot, ksegptr, chunkptr;
     std::vector<uint16_t> rank, segdesc, segcfirst;
-    std::vector<int32_t> segptr, segslot, chunkptr;
+    int32_t K = 0, nseg = 0;
 };
-int build_map_plan(Arena &ar, const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, MapHost *out, int64_t *bytes, MapPlanHost *keep = nullptr) {
-    std::vector<uint16_t> rank((size_t)ntile * TPX, (uint16_t)NORANK);
-    std::vector<int32_t> segptr(ntile + 1, 0);
-    std::vector<uint16_t> segdesc;
+void compute_map_plan(const int32_t *idx, int32_t K, int64_t npos, int32_t ntile, MapPlanHost &mp) {
+    std::vector<uint16_t> &rank = mp.rank;
+    rank.assign((size_t)ntile * TPX, (uint16_t)NORANK);
+    std::vector<int32_t> &segptr = mp.segptr;
+    segptr.assign(ntile + 1, 0);
+    std::vector<uint16_t> &segdesc = mp.segdesc;
+    segdesc.clear();
     std::vector<int32_t> segcluster;
     segdesc.reserve((size_t)ntile * 16);
     segcluster.reserve((size_t)ntile * 16);
     std::vector<std::pair<int32_t, int32_t>> tmp;
     std::vector<std::pair<uint16_t, int32_t>> tseg;   // (descriptor, cluster)
-    std::vector<int32_t> chunkptr(ntile + 1, 0);
-    std::vector<uint16_t> segcfirst;
+    std::vector<int32_t> &chunkptr = mp.chunkptr;
+    chunkptr.assign(ntile + 1, 0);
+    std::vector<uint16_t> &segcfirst = mp.segcfirst;
+    segcfirst.clear();
     int32_t nchunk = 0;
     tmp.reserve(TPX);
     for (int32_t t = 0; t < ntile; ++t) {
@@ -312,27 +320,28 @@ int build_map_plan(Arena &ar, const int32_t *idx, int32_t K, int64_t npos, int32
     chunkptr[ntile] = nchunk;
     const int32_t nseg = (int32_t)segdesc.size();
     // cluster-major slots: the segments of cluster k occupy [ksegptr[k], ksegptr[k+1]) in ascending (tile, chunk) order
-    std::vector<int32_t> ksegptr(K + 1, 0), segslot(nseg);
+    std::vector<int32_t> &ksegptr = mp.ksegptr, &segslot = mp.segslot;
+    ksegptr.assign(K + 1, 0);
+    segslot.assign(nseg, 0);
     for (int32_t s = 0; s < nseg; ++s) ksegptr[segcluster[s] + 1]++;
     for (int32_t k = 0; k < K; ++k) ksegptr[k + 1] += ksegptr[k];
     std::vector<int32_t> fill(ksegptr.begin(), ksegptr.end() - 1);
     for (int32_t s = 0; s < nseg; ++s) segslot[s] = fill[segcluster[s]]++;
-    std::vector<int32_t> idxv((size_t)ntile * TPX, -1);
-    std::copy(idx, idx + npos, idxv.begin());
-    out->K = K; out->nseg = nseg;
+    mp.idx.assign((size_t)ntile * TPX, -1);
+    std::copy(idx, idx + npos, mp.idx.begin());
+    mp.K = K; mp.nseg = nseg;
+}
+int upload_map_plan(Arena &ar, const MapPlanHost &mp, MapHost *out, int64_t *bytes) {
+    out->K = mp.K; out->nseg = mp.nseg;
     int rc;
-    if ((rc = arena_upload(ar, &out->idx, idxv, bytes))) return rc;
-    if ((rc = arena_upload(ar, &out->rank, rank, bytes))) return rc;
-    if ((rc = arena_upload(ar, &out->segptr, segptr, bytes))) return rc;
-    if ((rc = arena_upload(ar, &out->segdesc, segdesc, bytes))) return rc;
-    if ((rc = arena_upload(ar, &out->segslot, segslot, bytes))) return rc;
-    if ((rc = arena_upload(ar, &out->ksegptr, ksegptr, bytes))) return rc;
-    if ((rc = arena_upload(ar, &out->chunkptr, chunkptr, bytes))) return rc;
-    if ((rc = arena_upload(ar, &out->segcfirst, segcfirst, bytes))) return rc;
-    if (keep) {
-        keep->rank.swap(rank); keep->segdesc.swap(segdesc); keep->segcfirst.swap(segcfirst);
-        keep->segptr.swap(segptr); keep->segslot.swap(segslot); keep->chunkptr.swap(chunkptr);
-    }
+    if ((rc = arena_upload(ar, &out->idx, mp.idx, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->rank, mp.rank, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segptr, mp.segptr, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segdesc, mp.segdesc, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segslot, mp.segslot, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->ksegptr, mp.ksegptr, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->chunkptr, mp.chunkptr, bytes))) return rc;
+    if ((rc = arena_upload(ar, &out->segcfirst, mp.segcfirst, bytes))) return rc;
     return CS_OK;
 }
 
@@ -484,6 +493,36 @@ void pack_tile_headers(const SortedPlan &sp, const MapPlanHost (&mp)[4], const i
     }
     hdrptr[sp.ntile] = (int32_t)(blob.size() / 4);
 }
+
+// Runs fn(i) for i in [0, n) on the host's threads (plan building is pure host work, independent per map and per
+// configuration: a clustering scan sets a thousand configurations).  Returns false if any call threw.
+template <class F>
+bool parallel_for(int n, F fn) {
+    const int nt = std::max(1, std::min<int>(n, std::min<unsigned>(16u, std::thread::hardware_concurrency())));
+    std::atomic<int> next{0};
+    std::atomic<bool> ok{true};
+    auto work = [&]() {
+        try {
+            for (int i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
+        } catch (...) { ok = false; }
+    };
+    std::vector<std::thread> th;
+    for (int t = 1; t < nt; ++t) th.emplace_back(work);
+    work();
+    for (auto &t : th) t.join();
+    return ok;
+}
+
+// Everything of one configuration that is computed on the host before anything is uploaded.
+struct CfgPlanHost {
+    SortedPlan sp;
+    bool sorted = false;
+    MapPlanHost mp[4];
+    std::vector<int32_t> kp[4], kl[4];
+    std::vector<int32_t> hdrptr;
+    std::vector<uint32_t> hdrblob;
+    std::vector<int32_t> live;   // [nregion]
+};
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -813,24 +852,20 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     free_clusters(c);
     c->maps.resize(nmap + 1);
     int rc;
-    for (int32_t m = 0; m < nmap; ++m)
-        if ((rc = build_map_plan(c->cl_arena, h.data() + (size_t)m * npix, Kmap[m], npix, c->ntile_ring, &c->maps[m], &c->cluster_bytes))) {
-            free_clusters(c);
-            return rc;
-        }
-    if ((rc = build_map_plan(c->cl_arena, reg.data(), nregion, npix, c->ntile_ring, &c->maps[nmap], &c->cluster_bytes))) {
-        free_clusters(c);
-        return rc;
+    {   // pixel-space plans of the nmap cluster maps and of the region pseudo-map
+        std::vector<MapPlanHost> pm(nmap + 1);
+        if (!parallel_for(nmap + 1, [&](int m) {
+                if (m < nmap) compute_map_plan(h.data() + (size_t)m * npix, Kmap[m], npix, c->ntile_ring, pm[m]);
+                else compute_map_plan(reg.data(), nregion, npix, c->ntile_ring, pm[m]);
+            })) { free_clusters(c); return CS_ENOMEM; }
+        for (int32_t m = 0; m <= nmap; ++m)
+            if ((rc = upload_map_plan(c->cl_arena, pm[m], &c->maps[m], &c->cluster_bytes))) { free_clusters(c); return rc; }
     }
     c->nmap = nmap; c->ncfg = ncfg; c->nregion = nregion;
     c->cfgs.resize(ncfg);
     c->sorted.resize(ncfg);
     c->cellsh.resize(ncfg);
     c->npix_live.assign((size_t)ncfg * nregion, 0);
-    SortedPlan sp;
-    MapPlanHost mplan[4];
-    std::vector<int32_t> hdrptr;
-    std::vector<uint32_t> hdrblob;
     for (int32_t i = 0; i < ncfg; ++i) {
         CfgDev &cf = c->cfgs[i];
         std::memset(&cf, 0, sizeof(cf));
@@ -841,72 +876,88 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
         }
         cf.ktot = cf.K[0] + cf.K[1] + cf.K[2];
         cf.ntile = cf.ntile_ring = c->ntile_ring;
-        const int32_t *a = h.data() + (size_t)cf.rmap[0] * npix, *b = h.data() + (size_t)cf.rmap[1] * npix,
-                      *d = h.data() + (size_t)cf.rmap[2] * npix;
-        for (int64_t p = 0; p < npix; ++p)
-            if (a[p] >= 0 && b[p] >= 0 && d[p] >= 0) c->npix_live[(size_t)i * nregion + reg[p]]++;
-        // sorted layout: taken when the option asks for it, or (auto) when its tiles come out well filled -- small
-        // cells (K ~ npix) would mostly stream padding
-        if (c->opt_layout != CS_LAYOUT_INPLACE) {
-            plan_sorted(a, b, d, reg.data(), cf.K, npix, sp);
-            if (c->opt_layout == CS_LAYOUT_SORTED || sp.fill >= c->opt_min_fill) {
+    }
+    // configurations in groups: the host part of a group on all threads (sorted layout, the four position-space plans,
+    // the cell lists, the tile headers), then its uploads in order
+    constexpr int GROUP = 32;
+    std::vector<CfgPlanHost> plans(std::min<int32_t>(GROUP, ncfg));
+    for (int32_t i0 = 0; i0 < ncfg; i0 += GROUP) {
+        const int32_t ng = std::min<int32_t>(GROUP, ncfg - i0);
+        if (!parallel_for(ng, [&](int g) {
+                const int32_t i = i0 + g;
+                const CfgDev &cf = c->cfgs[i];
+                CfgPlanHost &pl = plans[g];
+                const int32_t *a = h.data() + (size_t)cf.rmap[0] * npix, *b = h.data() + (size_t)cf.rmap[1] * npix,
+                              *d = h.data() + (size_t)cf.rmap[2] * npix;
+                pl.live.assign(nregion, 0);
+                for (int64_t p = 0; p < npix; ++p)
+                    if (a[p] >= 0 && b[p] >= 0 && d[p] >= 0) pl.live[reg[p]]++;
+                pl.sorted = false;
+                // sorted layout: taken when the option asks for it, or (auto) when its tiles come out well filled --
+                // small cells (K ~ npix) would mostly stream padding
+                if (c->opt_layout == CS_LAYOUT_INPLACE) return;
+                plan_sorted(a, b, d, reg.data(), cf.K, npix, pl.sp);
+                if (!(c->opt_layout == CS_LAYOUT_SORTED || pl.sp.fill >= c->opt_min_fill)) return;
+                pl.sorted = true;
+                const int64_t npos = (int64_t)pl.sp.ntile * TPX;
+                int32_t segbase[4], off = 0;
+                for (int t = 0; t < 4; ++t) {
+                    compute_map_plan(pl.sp.idx[t].data(), t < 3 ? cf.K[t] : nregion, npos, pl.sp.ntile, pl.mp[t]);
+                    segbase[t] = off;
+                    off += pl.mp[t].nseg;
+                }
+                const int32_t ncell = (int32_t)pl.sp.cellpos.size();   // global cell list (f3): cluster / region -> cells
+                for (int t = 0; t < 4; ++t) {
+                    const int32_t Kt = t < 3 ? cf.K[t] : nregion;
+                    std::vector<int32_t> &kp = pl.kp[t], &kl = pl.kl[t];
+                    kp.assign(Kt + 1, 0); kl.assign(ncell, 0);
+                    for (int32_t q = 0; q < ncell; ++q) kp[pl.sp.cellkey[t][q] + 1]++;
+                    for (int32_t k = 0; k < Kt; ++k) kp[k + 1] += kp[k];
+                    std::vector<int32_t> fill(kp.begin(), kp.end() - 1);
+                    for (int32_t q = 0; q < ncell; ++q) kl[fill[pl.sp.cellkey[t][q]]++] = q;
+                }
+                pack_tile_headers(pl.sp, pl.mp, segbase, pl.mp[3].nseg, pl.hdrptr, pl.hdrblob);   // they hold the slots
+            })) { free_clusters(c); return CS_ENOMEM; }
+        for (int32_t g = 0; g < ng; ++g) {
+            const int32_t i = i0 + g;
+            CfgDev &cf = c->cfgs[i];
+            CfgPlanHost &pl = plans[g];
+            for (int32_t r = 0; r < nregion; ++r) c->npix_live[(size_t)i * nregion + r] = pl.live[r];
+            if (pl.sorted) {
+                const SortedPlan &sp = pl.sp;
                 SortedHost &sh = c->sorted[i];
+                CellsHost &ch = c->cellsh[i];
+                ch.ncell = (int32_t)sp.cellpos.size();
+                c->ncell_max = std::max(c->ncell_max, ch.ncell);
                 if ((rc = arena_upload(c->cl_arena, &sh.cellid, sp.cellid, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.cellptr, sp.cellptr, &c->cluster_bytes)) ||
-                    (rc = arena_upload(c->cl_arena, &sh.cellrows, sp.cellrows, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.pospix, sp.pospix, &c->cluster_bytes))) {
+                    (rc = arena_upload(c->cl_arena, &sh.cellrows, sp.cellrows, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.pospix, sp.pospix, &c->cluster_bytes)) ||
+                    (rc = arena_upload(c->cl_arena, &ch.cellpos, sp.cellpos, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &ch.celllen, sp.celllen, &c->cluster_bytes)) ||
+                    (rc = arena_upload(c->cl_arena, &ch.cellreg, sp.cellkey[3], &c->cluster_bytes)) ||
+                    (rc = arena_upload(c->cl_arena, &sh.hdr, pl.hdrblob, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.hdrptr, pl.hdrptr, &c->cluster_bytes))) {
                     free_clusters(c);
                     return rc;
                 }
-                const int64_t npos = (int64_t)sp.ntile * TPX;
                 for (int t = 0; t < 4; ++t) {
                     c->maps.emplace_back();
-                    if ((rc = build_map_plan(c->cl_arena, sp.idx[t].data(), t < 3 ? cf.K[t] : nregion, npos, sp.ntile, &c->maps.back(), &c->cluster_bytes, &mplan[t]))) {
+                    if ((rc = upload_map_plan(c->cl_arena, pl.mp[t], &c->maps.back(), &c->cluster_bytes)) ||
+                        (rc = arena_upload(c->cl_arena, &ch.kptr[t], pl.kp[t], &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &ch.klist[t], pl.kl[t], &c->cluster_bytes))) {
                         free_clusters(c);
                         return rc;
                     }
                     cf.map[t] = (int32_t)c->maps.size() - 1;
                 }
-                {   // global cell list for the cell-compressed likelihood (f3)
-                    CellsHost &ch = c->cellsh[i];
-                    ch.ncell = (int32_t)sp.cellpos.size();
-                    c->ncell_max = std::max(c->ncell_max, ch.ncell);
-                    if ((rc = arena_upload(c->cl_arena, &ch.cellpos, sp.cellpos, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &ch.celllen, sp.celllen, &c->cluster_bytes)) ||
-                        (rc = arena_upload(c->cl_arena, &ch.cellreg, sp.cellkey[3], &c->cluster_bytes))) {
-                        free_clusters(c);
-                        return rc;
-                    }
-                    for (int t = 0; t < 4; ++t) {
-                        const int32_t Kt = t < 3 ? cf.K[t] : nregion;
-                        std::vector<int32_t> kp(Kt + 1, 0), kl(ch.ncell);
-                        for (int32_t q = 0; q < ch.ncell; ++q) kp[sp.cellkey[t][q] + 1]++;
-                        for (int32_t k = 0; k < Kt; ++k) kp[k + 1] += kp[k];
-                        std::vector<int32_t> fill(kp.begin(), kp.end() - 1);
-                        for (int32_t q = 0; q < ch.ncell; ++q) kl[fill[sp.cellkey[t][q]]++] = q;
-                        if ((rc = arena_upload(c->cl_arena, &ch.kptr[t], kp, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &ch.klist[t], kl, &c->cluster_bytes))) {
-                            free_clusters(c);
-                            return rc;
-                        }
-                    }
-                }
                 cf.sorted = 1;
                 cf.ntile = sp.ntile;
                 cf.cellid = sh.cellid; cf.cellptr = sh.cellptr; cf.cellrows = sh.cellrows; cf.pospix = sh.pospix;
+                cf.hdr = sh.hdr; cf.hdrptr = sh.hdrptr;
             }
-        }
-        cf.pixbeta = (!cf.sorted && c->opt_pixbeta == CS_PIXBETA_AUTO && 2 * (int64_t)cf.K[0] > npix) ? 1 : 0;
-        int32_t off = 0;
-        for (int t = 0; t < 4; ++t) {
-            cf.segbase[t] = off;
-            cf.kseg[t] = c->maps[cf.map[t]].ksegptr;
-            off += c->maps[cf.map[t]].nseg;
-        }
-        if (cf.sorted) {   // tile headers (they hold the slots, hence after segbase)
-            pack_tile_headers(sp, mplan, cf.segbase, c->maps[cf.map[3]].nseg, hdrptr, hdrblob);
-            SortedHost &sh = c->sorted[i];
-            if ((rc = arena_upload(c->cl_arena, &sh.hdr, hdrblob, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &sh.hdrptr, hdrptr, &c->cluster_bytes))) {
-                free_clusters(c);
-                return rc;
+            cf.pixbeta = (!cf.sorted && c->opt_pixbeta == CS_PIXBETA_AUTO && 2 * (int64_t)cf.K[0] > npix) ? 1 : 0;
+            int32_t off = 0;
+            for (int t = 0; t < 4; ++t) {
+                cf.segbase[t] = off;
+                cf.kseg[t] = c->maps[cf.map[t]].ksegptr;
+                off += c->maps[cf.map[t]].nseg;
             }
-            cf.hdr = sh.hdr; cf.hdrptr = sh.hdrptr;
         }
     }
     std::vector<MapDev> md(c->maps.size());
