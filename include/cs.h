@@ -18,7 +18,8 @@
  *     needs d, cluster maps and region_idx to share one pixel order.
  *   - "dev" = pointer to device memory on the current CUDA device; "host" = host memory; "any" = either (copied
  *     with cudaMemcpyDefault during the call).  Borrowed pointers must stay valid and unchanged until replaced.
- *   - every function returns CS_OK (0) or a negative CS_E* code; nothing throws; no global state; a context is
+ *   - every function returns CS_OK (0) or a negative CS_E* code; nothing throws; no global state (but for the fixed
+ *     descriptor table of cs_spherical_kmeans_static); a context is
  *     bound to the CUDA device current at cs_create and must be used from one stream at a time.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Hot-path calls are
  *     asynchronous on it and allocate nothing.
@@ -44,6 +45,7 @@ extern "C" {
                               diagonal entry (covers non-positive); that entry's nll = +inf, its gradient is undefined */
 #define CS_ECUDA      -5   /* a CUDA runtime call failed */
 #define CS_ENOMEM     -6   /* allocation failed */
+#define CS_ELIMIT     -7   /* a size is beyond the fixed capacity of an entry point that allocates nothing */
 
 #define CS_UNITS_KCMB    0 /* dust/synchrotron columns carry the K_RJ -> K_CMB factor u(nu)/u(nu0) (default) */
 #define CS_UNITS_LITERAL 1 /* Eq. 2 as printed (brightness-temperature units), no unit factor */
@@ -237,6 +239,29 @@ CS_API int cs_eval_host(cs_ctx *ctx, int32_t ndata, const float *d_host, const f
  * bit.  Asynchronous on `stream`. */
 CS_API int cs_spherical_kmeans(int64_t npix, const double *vecs, const uint8_t *region, int32_t nprob, const int32_t *K,
                         const int32_t *prob_region, double *cent, int32_t iters, int32_t *labels, void *stream);
+
+/* cs_spherical_kmeans for callers that must not allocate device memory.
+ *
+ * Who needs it: a host program that has given all of device memory to a pool of its own (an inference server, a
+ * framework allocator with a hard cap), so that a cudaMalloc from inside a library can fail at any moment; and a
+ * latency-bound loop that cannot take the device-wide synchronisation an allocation or a free may bring.
+ * cs_spherical_kmeans keeps its per-problem descriptors (patch count, region, centroid offset: 16 bytes a problem) in a
+ * table it allocates and frees on every call.  This entry point runs the same two kernels on the same inputs and gives
+ * the same bits in `cent` and `labels`, but keeps that table in a fixed array that is part of the library image:
+ * CS_KMEANS_STATIC_MAX_PROB descriptors = 16 KiB, held by every GPU that loads libcs.so until the process exits.
+ * It calls no cudaMalloc, cudaFree, stream-ordered allocator or other allocating routine, on the device or the host;
+ * inputs and outputs are the caller's, with the layouts of cs_spherical_kmeans.
+ *
+ *   - nprob > CS_KMEANS_STATIC_MAX_PROB returns CS_ELIMIT and launches nothing; split the problems over several calls.
+ *   - The first call on each device looks up the device address of the table (cudaGetSymbolAddress, with that device
+ *     current, result checked and remembered per device).  Make that first call outside any stream capture.
+ *   - One table serves every call on a device and keeps what the last call wrote.  Nothing in it has to start at zero:
+ *     a call overwrites the nprob descriptors it will read, in stream order, before its first kernel, and reads no others.
+ *     Calls issued to the same stream therefore queue up correctly.  Calls that can overlap on the GPU (different streams
+ *     without an event between them, or different host threads doing so) race on the table: serialise them. */
+#define CS_KMEANS_STATIC_MAX_PROB 1024
+CS_API int cs_spherical_kmeans_static(int64_t npix, const double *vecs, const uint8_t *region, int32_t nprob, const int32_t *K,
+                               const int32_t *prob_region, double *cent, int32_t iters, int32_t *labels, void *stream);
 
 /* Synchronises `stream`, returns and clears the sticky device error bits: CS_OK, CS_EDOMAIN or CS_ESINGULAR. */
 CS_API int cs_check(cs_ctx *ctx, void *stream);

@@ -9,7 +9,8 @@ import numpy as np
 
 from . import build as _build
 
-OK, EINVAL, EINDEX, EDOMAIN, ESINGULAR, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5, -6
+OK, EINVAL, EINDEX, EDOMAIN, ESINGULAR, ECUDA, ENOMEM, ELIMIT = 0, -1, -2, -3, -4, -5, -6, -7
+KMEANS_STATIC_MAX_PROB = 1024
 UNITS_KCMB, UNITS_LITERAL = 0, 1
 OPT_LAYOUT, OPT_FORM, OPT_MIN_FILL, OPT_COPY_LIMIT_MB, OPT_PIXEL_BETA = 1, 2, 3, 4, 5
 PIXBETA_AUTO, PIXBETA_OFF = 0, 1
@@ -19,7 +20,7 @@ METHOD_ADATOPK, METHOD_LBFGS = 0, 1
 
 EXPORTS = ["cs_create", "cs_destroy", "cs_set_option", "cs_layout_info", "cs_model_constants", "cs_set_clusters", "cs_set_data", "cs_set_batch", "cs_param_offsets",
            "cs_build_sed_tables", "cs_spectral_like_grad", "cs_spectral_misfit", "cs_cell_moments", "cs_spectral_like_grad_cells", "cs_component_maps", "cs_cmb_residual_maps", "cs_cmb_variance", "cs_optimize",
-           "cs_opt_defaults", "cs_eval_host", "cs_spherical_kmeans", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
+           "cs_opt_defaults", "cs_eval_host", "cs_spherical_kmeans", "cs_spherical_kmeans_static", "cs_check", "cs_profile", "cs_profile_read", "cs_strerror", "cs_workspace_bytes", "cs_kernel_launches",
            "cs_version"]
 
 
@@ -80,6 +81,7 @@ def lib():
         "cs_opt_defaults": (None, [C.POINTER(CsOpt)]),
         "cs_eval_host": (C.c_int, [vp, i32, vp, vp, vp, vp, vp]),
         "cs_spherical_kmeans": (C.c_int, [i64, vp, vp, i32, vp, vp, vp, i32, vp, vp]),
+        "cs_spherical_kmeans_static": (C.c_int, [i64, vp, vp, i32, vp, vp, vp, i32, vp, vp]),
         "cs_check": (C.c_int, [vp, vp]),
         "cs_profile": (C.c_int, [vp, C.c_int]),
         "cs_profile_read": (C.c_int, [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
@@ -168,6 +170,21 @@ def spherical_kmeans(vecs, K, cent, labels, iters=10, region=None, prob_region=N
     _chk(lib().cs_spherical_kmeans(npix, _ptr(vecs, "float64", "cuda", 3 * npix, "vecs"), _ptr(region, "uint8", "cuda", npix, "region"),
                                    nprob, _hp(K), _hp(prob_region), _ptr(cent, "float64", "cuda", 3 * int(K.sum()), "cent"), int(iters),
                                    _ptr(labels, "int32", "cuda", nprob * npix, "labels"), _stream(stream)), "cs_spherical_kmeans")
+
+
+def spherical_kmeans_static(vecs, K, cent, labels, iters=10, region=None, prob_region=None, stream=None):
+    """cs_spherical_kmeans_static: same arguments and same bits as spherical_kmeans, for a caller that must not allocate
+    device memory (its pool owns the whole GPU, or it cannot afford the synchronisation an allocation may bring).  The
+    library's only scratch, the table of problem descriptors, sits in a fixed 16-KiB device array shared by all calls:
+    at most KMEANS_STATIC_MAX_PROB problems per call (CsError ELIMIT beyond), calls that may overlap on the GPU must be
+    serialised by the caller, and the first call on a device should come before any stream capture."""
+    K = np.ascontiguousarray(K, dtype=np.int32)
+    nprob, npix = int(K.shape[0]), int(vecs.shape[0])
+    if prob_region is not None:
+        prob_region = np.ascontiguousarray(prob_region, dtype=np.int32)
+    _chk(lib().cs_spherical_kmeans_static(npix, _ptr(vecs, "float64", "cuda", 3 * npix, "vecs"), _ptr(region, "uint8", "cuda", npix, "region"),
+                                          nprob, _hp(K), _hp(prob_region), _ptr(cent, "float64", "cuda", 3 * int(K.sum()), "cent"), int(iters),
+                                          _ptr(labels, "int32", "cuda", nprob * npix, "labels"), _stream(stream)), "cs_spherical_kmeans_static")
 
 
 class Context:

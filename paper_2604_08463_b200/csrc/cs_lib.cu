@@ -9,6 +9,7 @@
 #include <cstring>
 #include <atomic>
 #include <map>
+#include <mutex>
 #include <thread>
 #include <stdexcept>
 #include <new>
@@ -708,6 +709,7 @@ const char *cs_strerror(int code) {
         case CS_ESINGULAR: return "singular A^T N^-1 A";
         case CS_ECUDA: return "CUDA runtime error";
         case CS_ENOMEM: return "out of device memory";
+        case CS_ELIMIT: return "size beyond the fixed capacity of a no-allocation entry point";
         default: return "unknown error";
     }
 }
@@ -1621,3 +1623,62 @@ int64_t cs_workspace_bytes(cs_ctx *c) {
 int64_t cs_kernel_launches(cs_ctx *c) { return c ? c->launches : 0; }
 
 }  // extern "C"
+
+// ---- cs_spherical_kmeans_static: the K-means entry point that allocates nothing (include/cs.h) -------------------------
+// The problem descriptors that cs_spherical_kmeans puts in a cudaMallocAsync'ed table live here instead, in the library
+// image: 1024 x 16 B = 16 KiB on every GPU that loads libcs.so, until the process exits.  On the host the name
+// g_km_static_probs is only a handle for the runtime's symbol calls, not an address a kernel can use; the launches
+// below get the device address that km_static_table() looks up.
+static __device__ __align__(256) KmProb g_km_static_probs[CS_KMEANS_STATIC_MAX_PROB];
+
+namespace {
+constexpr int KM_STATIC_MAX_DEV = 64;
+std::mutex g_km_static_mu;
+KmProb *g_km_static_addr[KM_STATIC_MAX_DEV] = {};
+
+// Device address of g_km_static_probs on the current device; asked of the runtime once per device, with that device
+// current, and kept.  Every device has its own copy of the array at its own address.
+int km_static_table(KmProb **out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= KM_STATIC_MAX_DEV) return CS_ECUDA;
+    std::lock_guard<std::mutex> lock(g_km_static_mu);
+    if (!g_km_static_addr[dev]) {
+        void *p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_km_static_probs) != cudaSuccess || !p) return CS_ECUDA;
+        g_km_static_addr[dev] = (KmProb *)p;
+    }
+    *out = g_km_static_addr[dev];
+    return CS_OK;
+}
+}  // namespace
+
+extern "C" int cs_spherical_kmeans_static(int64_t npix, const double *vecs, const uint8_t *region, int32_t nprob, const int32_t *K,
+                                          const int32_t *prob_region, double *cent, int32_t iters, int32_t *labels, void *stream) {
+    if (npix <= 0 || !vecs || nprob <= 0 || !K || !cent || iters < 0 || !labels) return CS_EINVAL;
+    if (nprob > CS_KMEANS_STATIC_MAX_PROB) return CS_ELIMIT;
+    cudaStream_t st = (cudaStream_t)stream;
+    KmProb pr[CS_KMEANS_STATIC_MAX_PROB];   // host staging on the stack: no heap either
+    int64_t off = 0;
+    int32_t kmax = 0;
+    for (int32_t j = 0; j < nprob; ++j) {
+        if (K[j] < 1) return CS_EINVAL;
+        const int32_t reg = prob_region ? prob_region[j] : -1;
+        if (reg >= 0 && !region) return CS_EINVAL;
+        pr[j] = KmProb{K[j], reg, off};
+        off += K[j];
+        kmax = std::max(kmax, K[j]);
+    }
+    KmProb *d_pr = nullptr;
+    const int rc = km_static_table(&d_pr);
+    if (rc != CS_OK) return rc;
+    // Overwrites the descriptors this call reads, in stream order: earlier calls on `st` have finished with the table
+    // by then.  Pageable source: the bytes have left `pr` when cudaMemcpyAsync returns.
+    if (cudaMemcpyAsync(d_pr, pr, sizeof(KmProb) * nprob, cudaMemcpyHostToDevice, st) != cudaSuccess) return CS_ECUDA;
+    const dim3 ga((unsigned)((npix + 255) / 256), nprob), gu((kmax + 7) / 8, nprob);
+    k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
+    for (int32_t it = 0; it < iters; ++it) {
+        k_km_update<<<gu, 256, 0, st>>>(vecs, npix, d_pr, labels, cent);
+        k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
+    }
+    return cudaGetLastError() == cudaSuccess ? CS_OK : CS_ECUDA;
+}
