@@ -88,7 +88,8 @@ struct CfgDev {
     int32_t sorted;       // 1: sorted layout with private data copies, 0: in place
     int32_t ntile_ring;   // tiles of the in-place layout
     int32_t pixbeta;      // 1: in place with beta_d (nearly) per pixel: no beta_d table rows, the direct kernel evaluates
-                          //    cd (nu/nu0)^beta_d per pixel from a copy of the parameters (k_tables' arithmetic, same bits)
+                          //    cd (nu/nu0)^beta_d per pixel from a copy of the parameters in compensated fp32
+                          //    (powerlaw_pair_f32: 2.5e-7 relative, not the bits of a table row)
     const int32_t *kseg[4];    // = maps[map[t]].ksegptr: one load less on k_merge's way to its slots
     // sorted layout only
     const uint8_t *cellid;     // [ntile*NCONS] tile-local cell of each thread (position pair)
@@ -110,7 +111,7 @@ struct Run {
 };
 
 // What the roles of a fused kernel need to know about the entry at position i of the launch's entry list, in one
-// 16-byte load whose address does not depend on another load (a dependent global load costs a microsecond under a
+// 32-byte record (two 16-byte loads) whose address does not depend on another load (a dependent global load costs a microsecond under a
 // saturated HBM stream).
 struct PosInfo {
     int64_t tab_row;   // first table row of the entry

@@ -199,8 +199,9 @@ __device__ __forceinline__ void sc_loader(const LikeParams &P, float *ring, uint
 }
 
 // One cell (Eq. 2 columns -> five weighted columns, M, LDL^T, P; cs_math.cuh) from the entry's four table rows.
-// Cell row (floats): [0,16) w a_d | [16,32) w da_d/dbeta_d | [32,48) w da_d/dT_d | [48,64) w a_s | [64,80) w da_s/dbeta_s |
-// [80,96) l10 l20 l21 1/d1 | 1/d2 P10 P11 P12 | P20 P21 P22 P30 | P31 P32 bad -
+// Cell row (CROW = 68 floats): [0,16) w a_d | [16,32) w da_d/dT_d (gradient modes only) | [32,48) w a_s |
+// [48,64) l10 l20 l21 1/d1 | 1/d2 P10 P11 P12 | P20 P21 P22 P30 | P31 P32 bad - | [64,68) pad.
+// The beta derivatives are not stored: w da_d/dbeta_d = lnd w a_d and w da_s/dbeta_s = lns w a_s.
 template <int NF, bool GRAD>
 __device__ __forceinline__ void sc_build_cell(const float4 (&Fd)[4], const float4 (&G)[4], const float4 (&dG)[4], const float4 (&Fs)[4],
                                               const KConst &kc, float *__restrict__ out, int32_t *err) {

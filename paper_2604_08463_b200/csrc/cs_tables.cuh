@@ -42,7 +42,8 @@ __device__ __forceinline__ double exp_pow(double y) {
 }
 
 // One value of a power-law row, band constant folded in: c (nu/nu0)^beta = c exp(beta ln(nu/nu0)), rounded to fp32.
-// Written once: k_tables and the direct kernel's per-pixel beta_d path (CfgDev::pixbeta) must give the same bits.
+// k_tables' form.  (The direct kernel's per-pixel beta_d path, CfgDev::pixbeta, uses powerlaw_pair_f32 below instead: not
+// the same bits.)
 __device__ __forceinline__ float powerlaw_value(double c, double lnr, double beta) {
     return (float)__dmul_rn(c, exp_pow(__dmul_rn(beta, lnr)));
 }
