@@ -1103,7 +1103,8 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
     for (int32_t e = 0; e < batch; ++e) {
         const CfgDev &cf = c->cfgs[cfg_of[e]];
         for (int32_t j0 = 0; j0 < cf.ktot; j0 += TAB_ROWS_PER_BLOCK)
-            if (!(cf.pixbeta && j0 + TAB_ROWS_PER_BLOCK <= cf.K[0]))   // nothing to build in a block of unused beta_d rows
+            // (a block that lies wholly in the beta_d rows of a pixbeta configuration builds nothing, but still checks
+            // its parameters: CS_EDOMAIN is raised here, whichever kernel evaluates the power law)
             tabblk.push_back(TabBlock{c->param_off[e], tab_off[e], cf.K[0], cf.K[1], cf.ktot, j0, e, cf.pixbeta, {0, 0}});
     }
     c->ntabblk = (int64_t)tabblk.size();

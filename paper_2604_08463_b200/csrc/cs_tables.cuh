@@ -115,6 +115,13 @@ __global__ void __launch_bounds__(256) k_tables(const double *__restrict__ param
         const int j = j0 + 64 * u + (threadIdx.x >> 2);
         xs[u] = (j < ktot) ? __ldg(params + param_off + j) : 1.0;
     }
+    if (pixbeta && j0 + TAB_ROWS_PER_BLOCK <= K0) {   // block-uniform: beta_d rows the direct kernel evaluates per pixel;
+        bool nonfinite = false;                       // nothing to build, only the domain check
+#pragma unroll
+        for (int u = 0; u < TAB_SUB; ++u) nonfinite = nonfinite || !isfinite(xs[u]);
+        if (nonfinite && f0 == 0) atomicOr(err, ERR_DOMAIN);
+        return;
+    }
     static_assert(sizeof(TConst) / 8 <= 256, "one word per thread");
     if (threadIdx.x < (int)(sizeof(TConst) / 8)) reinterpret_cast<double *>(&tc)[threadIdx.x] = __ldg(reinterpret_cast<const double *>(tcg) + threadIdx.x);
     __syncthreads();

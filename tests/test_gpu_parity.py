@@ -316,6 +316,18 @@ def test_error_bits_and_index_validation(torch_cuda):
     p[0] = float("nan")                       # beta_d
     gpu_eval(ctx, p)
     assert ctx.check() == cs.EDOMAIN
+    # beta_d per pixel (no beta_d table rows are built): a non-finite beta_d is still a domain error, wherever it sits
+    wp = gen.make_config(0, nside=16, K=(3072, 40, 9), batch=3, ndata=2)
+    ctxp, _ = make_ctx(wp, options={"layout": cs.LAYOUT_INPLACE})
+    offp = wp.param_offsets()
+    for e, j, bad in ((0, 0, float("nan")), (1, 1500, float("inf")), (2, 3071, float("nan"))):
+        p = wp.params_const()
+        gpu_eval(ctxp, p)
+        assert ctxp.check() == 0
+        p[offp[e] + j] = bad
+        gpu_eval(ctxp, p)
+        assert ctxp.check() == cs.EDOMAIN
+    ctxp.close()
     # out-of-range ids are refused bit-exactly and leave the context usable
     for val in (K[0], -2, 2**31 - 1):
         maps = w.maps.copy()
