@@ -162,9 +162,10 @@ CS_API int cs_param_offsets(cs_ctx *ctx, int64_t *off);
 /* a1 (Eq. 2): per entry, cluster and band the separable SED factors cd*(nu/nu0d)^beta_d, the Planck ratio
  * B-factor G(nu,T_d), its log-derivative dlnG/dT_d and cs*(nu/nu0s)^beta_s, evaluated in fp64 and stored fp32.
  * params dev fp64 (layout above).  Sets the sticky device bit CS_EDOMAIN on T_d <= 0 / non-finite input.
- * The library keeps its own copy of `params` (made on `stream`): the caller may overwrite them after the call.  For a
+ * The later calls read the tables, not `params`: the caller may overwrite them (in stream order) after the call.  For a
  * configuration that stays in place with beta_d (nearly) per pixel (CS_OPT_PIXEL_BETA) the beta_d rows are not built;
- * the fused kernel evaluates them per pixel from that copy (relative error <= 2.5e-7 instead of 6e-8; same tolerances). */
+ * the fused kernel evaluates them per pixel from a copy of `params` that the library makes on `stream` when the batch
+ * holds such a configuration (relative error <= 2.5e-7 instead of 6e-8; same tolerances). */
 CS_API int cs_build_sed_tables(cs_ctx *ctx, const double *params, void *stream);
 
 /* a2+a3: fused per-pixel likelihood / gradient and the ordered fp64 reduction onto clusters, for the tables last

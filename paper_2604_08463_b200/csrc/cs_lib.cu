@@ -171,6 +171,7 @@ struct cs_ctx {
     CopyJob *d_jobs = nullptr;
     float *d_tab = nullptr, *d_copy = nullptr;
     double *d_pcopy = nullptr;          // the parameters the tables were last built from
+    bool any_pixbeta = false;           // some entry of the batch reads d_pcopy (per-pixel beta_d); else it is not filled
     double *d_partial = nullptr;
     int64_t batch_bytes = 0, copy_bytes = 0;
     int32_t job_ntile_max = 0;
@@ -496,23 +497,44 @@ void pack_tile_headers(const SortedPlan &sp, const MapPlanHost (&mp)[4], const i
 }
 
 // Runs fn(i) for i in [0, n) on the host's threads (plan building is pure host work, independent per map and per
-// configuration: a clustering scan sets a thousand configurations).  Returns false if any call threw.
+// configuration: a clustering scan sets a thousand configurations).  Returns CS_OK, or what the first call that threw
+// stands for: CS_ENOMEM (bad_alloc, or a vector asked for more than it can hold) or CS_EINVAL.  A thread that cannot be
+// started is not an error: the calling thread and the ones that did start share the work.
 template <class F>
-bool parallel_for(int n, F fn) {
+int parallel_for(int n, F fn) {
     const int nt = std::max(1, std::min<int>(n, std::min<unsigned>(16u, std::thread::hardware_concurrency())));
     std::atomic<int> next{0};
-    std::atomic<bool> ok{true};
+    std::atomic<int> rc{CS_OK};
     auto work = [&]() {
+        int mine = CS_OK;
         try {
             for (int i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
-        } catch (...) { ok = false; }
+        } catch (const std::bad_alloc &) { mine = CS_ENOMEM; }
+        catch (const std::length_error &) { mine = CS_ENOMEM; }
+        catch (...) { mine = CS_EINVAL; }
+        if (mine != CS_OK) {
+            int expect = CS_OK;
+            rc.compare_exchange_strong(expect, mine);
+            next.store(n);   // the others stop at their next index
+        }
     };
     std::vector<std::thread> th;
-    for (int t = 1; t < nt; ++t) th.emplace_back(work);
+    try {
+        th.reserve(nt);
+        for (int t = 1; t < nt; ++t) th.emplace_back(work);
+    } catch (...) {}
     work();
     for (auto &t : th) t.join();
-    return ok;
+    return rc.load();
 }
+
+// Frees the cluster state of a context on every way out of cs_set_clusters but the successful one, exceptions included:
+// a half-built state (maps and configurations listed, their device tables missing) must not survive the call.
+struct ClustersGuard {
+    cs_ctx *c;
+    bool keep = false;
+    ~ClustersGuard() { if (!keep) free_clusters(c); }
+};
 
 // Everything of one configuration that is computed on the host before anything is uploaded.
 struct CfgPlanHost {
@@ -852,14 +874,15 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     cudaDeviceSynchronize();
     free_batch(c);
     free_clusters(c);
+    ClustersGuard guard{c};
     c->maps.resize(nmap + 1);
     int rc;
     {   // pixel-space plans of the nmap cluster maps and of the region pseudo-map
         std::vector<MapPlanHost> pm(nmap + 1);
-        if (!parallel_for(nmap + 1, [&](int m) {
+        if ((rc = parallel_for(nmap + 1, [&](int m) {
                 if (m < nmap) compute_map_plan(h.data() + (size_t)m * npix, Kmap[m], npix, c->ntile_ring, pm[m]);
                 else compute_map_plan(reg.data(), nregion, npix, c->ntile_ring, pm[m]);
-            })) { free_clusters(c); return CS_ENOMEM; }
+            }))) return rc;
         for (int32_t m = 0; m <= nmap; ++m)
             if ((rc = upload_map_plan(c->cl_arena, pm[m], &c->maps[m], &c->cluster_bytes))) { free_clusters(c); return rc; }
     }
@@ -885,7 +908,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     std::vector<CfgPlanHost> plans(std::min<int32_t>(GROUP, ncfg));
     for (int32_t i0 = 0; i0 < ncfg; i0 += GROUP) {
         const int32_t ng = std::min<int32_t>(GROUP, ncfg - i0);
-        if (!parallel_for(ng, [&](int g) {
+        if ((rc = parallel_for(ng, [&](int g) {
                 const int32_t i = i0 + g;
                 const CfgDev &cf = c->cfgs[i];
                 CfgPlanHost &pl = plans[g];
@@ -919,7 +942,7 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
                     for (int32_t q = 0; q < ncell; ++q) kl[fill[pl.sp.cellkey[t][q]]++] = q;
                 }
                 pack_tile_headers(pl.sp, pl.mp, segbase, pl.mp[3].nseg, pl.hdrptr, pl.hdrblob);   // they hold the slots
-            })) { free_clusters(c); return CS_ENOMEM; }
+            }))) return rc;
         for (int32_t g = 0; g < ng; ++g) {
             const int32_t i = i0 + g;
             CfgDev &cf = c->cfgs[i];
@@ -977,10 +1000,9 @@ int cs_set_clusters(cs_ctx *c, int32_t nmap, const int32_t *maps, const int32_t 
     }
     if ((rc = arena_upload(c->cl_arena, &c->d_maps, md, &c->cluster_bytes)) || (rc = arena_upload(c->cl_arena, &c->d_cfgs, c->cfgs, &c->cluster_bytes)) ||
         (rc = arena_upload(c->cl_arena, &c->d_cells, cd, &c->cluster_bytes)) ||
-        (rc = arena_upload(c->cl_arena, &c->d_npix_live, c->npix_live, &c->cluster_bytes))) {
-        free_clusters(c);
+        (rc = arena_upload(c->cl_arena, &c->d_npix_live, c->npix_live, &c->cluster_bytes)))
         return rc;
-    }
+    guard.keep = true;
     return CS_OK;
     CS_GUARD_END
 }
@@ -1100,8 +1122,10 @@ int cs_set_batch(cs_ctx *c, int32_t batch, const int32_t *cfg_of, const int32_t 
         if (copy_bytes > limit) { free_batch(c); return CS_ENOMEM; }
     }
     std::vector<TabBlock> tabblk;
+    c->any_pixbeta = false;
     for (int32_t e = 0; e < batch; ++e) {
         const CfgDev &cf = c->cfgs[cfg_of[e]];
+        c->any_pixbeta = c->any_pixbeta || cf.pixbeta != 0;
         for (int32_t j0 = 0; j0 < cf.ktot; j0 += TAB_ROWS_PER_BLOCK)
             // (a block that lies wholly in the beta_d rows of a pixbeta configuration builds nothing, but still checks
             // its parameters: CS_EDOMAIN is raised here, whichever kernel evaluates the power law)
@@ -1156,8 +1180,8 @@ int cs_param_offsets(cs_ctx *c, int64_t *off) {
 int cs_build_sed_tables(cs_ctx *c, const double *params, void *stream) {
     if (!c || c->batch <= 0 || !params) return CS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
-    // the parameters the tables belong to: read by the per-pixel beta_d path of the direct kernel
-    CK(cudaMemcpyAsync(c->d_pcopy, params, (size_t)c->nparam * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    // the parameters the tables belong to: read only by the per-pixel beta_d path of the direct kernel
+    if (c->any_pixbeta) CK(cudaMemcpyAsync(c->d_pcopy, params, (size_t)c->nparam * sizeof(double), cudaMemcpyDeviceToDevice, st));
     if (c->ntabblk > 0)
         k_tables<<<(unsigned)c->ntabblk, 256, 0, st>>>(params, c->d_tabblk, c->d_tab, c->d_err, c->d_tc, c->skip);
     c->launches++;
@@ -1206,7 +1230,7 @@ static int maps_impl(cs_ctx *c, int32_t nsel, const int32_t *entries, const int3
     if (!entries && nsel != c->batch) return CS_EINVAL;
     // The selection (entry list, per-position info, then its runs = stretches of consecutive selected entries of one
     // configuration) goes through a small ring of pinned staging slots, so that the call never synchronises the
-    // caller's stream; a slot is reused only after the copy that read it has completed.
+    // caller's stream; a slot (host and device side) is reused only after the kernel that read it has completed.
     const int slot = (int)(c->sel_n % cs_ctx::SEL_RING);
     if (!c->sel_ev[slot]) CK(cudaEventCreateWithFlags(&c->sel_ev[slot], cudaEventDisableTiming));
     else CK(cudaEventSynchronize(c->sel_ev[slot]));
@@ -1234,7 +1258,6 @@ static int maps_impl(cs_ctx *c, int32_t nsel, const int32_t *entries, const int3
     }
     const size_t bytes = (size_t)roff * 4 + (size_t)nrun * sizeof(Run);
     CK(cudaMemcpyAsync(ds, hs, bytes, cudaMemcpyHostToDevice, st));
-    CK(cudaEventRecord(c->sel_ev[slot], st));
     c->sel_n++;
     LikeParams P = base_params(c);
     P.elist = ds;
@@ -1243,7 +1266,10 @@ static int maps_impl(cs_ctx *c, int32_t nsel, const int32_t *entries, const int3
     P.maps_planes = planes;
     P.ring_maps = 1;
     P.evict_first = ((int64_t)c->ndata * c->nfreq * 2 * c->npix * 4 > (int64_t)96 << 20) ? 1 : 0;
-    return launch_like<MODE_MAPS>(c, P, reinterpret_cast<const Run *>(ds + roff), 0, 0, nrun, W, st);
+    rc = launch_like<MODE_MAPS>(c, P, reinterpret_cast<const Run *>(ds + roff), 0, 0, nrun, W, st);
+    // after the launch, not after the copy: the kernel reads the device side of the slot, whichever stream it ran on
+    const cudaError_t ev = cudaEventRecord(c->sel_ev[slot], st);
+    return rc ? rc : (ev == cudaSuccess ? CS_OK : CS_ECUDA);
 }
 
 int cs_component_maps(cs_ctx *c, int32_t nsel, const int32_t *entries, float *s, void *stream) {
@@ -1277,10 +1303,16 @@ int cs_cell_moments(cs_ctx *c, void *stream) {
         c->cc_out_stride = 4 * (int64_t)((c->ncell_max + 31) & ~31);
         const size_t out_bytes = (size_t)c->batch * c->cc_out_stride * sizeof(double);
         int64_t b = 0;
-        if ((rc = dev_upload(&c->d_momjobs, mj, &b)) || (rc = dev_upload(&c->d_mom_off, mo, &b))) return rc;
-        if (cudaMalloc((void **)&c->d_mom, (size_t)std::max<int64_t>(n, 1) * sizeof(double)) != cudaSuccess ||
-            cudaMalloc((void **)&c->d_ccout, out_bytes) != cudaSuccess || cudaMalloc((void **)&c->d_w, NROW * sizeof(float)) != cudaSuccess) {
+        // all five buffers or none: d_mom != nullptr is what marks the workspace as present on the next call
+        auto drop = [&]() {
+            cudaFree(c->d_mom); cudaFree(c->d_ccout); cudaFree(c->d_mom_off); cudaFree(c->d_momjobs); cudaFree(c->d_w);
+            c->d_mom = c->d_ccout = nullptr; c->d_mom_off = nullptr; c->d_momjobs = nullptr; c->d_w = nullptr;
             cudaGetLastError();
+        };
+        if ((rc = dev_upload(&c->d_momjobs, mj, &b)) || (rc = dev_upload(&c->d_mom_off, mo, &b))) { drop(); return rc; }
+        if (cudaMalloc((void **)&c->d_ccout, out_bytes) != cudaSuccess || cudaMalloc((void **)&c->d_w, NROW * sizeof(float)) != cudaSuccess ||
+            cudaMalloc((void **)&c->d_mom, (size_t)std::max<int64_t>(n, 1) * sizeof(double)) != cudaSuccess) {
+            drop();
             return CS_ENOMEM;
         }
         c->cc_bytes = b + n * (int64_t)sizeof(double) + (int64_t)out_bytes + NROW * 4;

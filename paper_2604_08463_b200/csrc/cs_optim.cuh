@@ -33,6 +33,7 @@ struct OptWork {
     double *sy = nullptr;                                             // [hist + 1][batch] s.yv of each stored pair
     int32_t *hcount = nullptr, *hhead = nullptr, *moved = nullptr;    // [batch] pairs stored, next slot, last step accepted
     int32_t hist = 0;                                                 // history slots allocated
+    int64_t lbfgs_bytes = 0;                                          // device bytes of the L-BFGS arrays above
 };
 
 struct OptShape {
@@ -89,6 +90,8 @@ inline int opt_alloc_lbfgs(OptWork &w, int64_t nparam, int32_t batch, int32_t hi
     if (w.z && w.hist >= hist) return 0;
     cudaFree(w.z); cudaFree(w.gz); cudaFree(w.S); cudaFree(w.Y); cudaFree(w.sy); cudaFree(w.hcount); cudaFree(w.hhead); cudaFree(w.moved);
     w.z = w.gz = w.S = w.Y = w.sy = nullptr; w.hcount = w.hhead = w.moved = nullptr; w.hist = 0;
+    *bytes -= w.lbfgs_bytes;   // a longer history replaces the arrays: their bytes are counted once
+    w.lbfgs_bytes = 0;
     const size_t np = (size_t)(nparam > 0 ? nparam : 1) * sizeof(double);
     bool ok = true;
     ok &= cudaMalloc((void **)&w.z, np) == cudaSuccess;
@@ -105,7 +108,8 @@ inline int opt_alloc_lbfgs(OptWork &w, int64_t nparam, int32_t batch, int32_t hi
         return 1;
     }
     w.hist = hist;
-    *bytes += (int64_t)(np * (2 + 2 * (size_t)(hist + 1)) + (size_t)batch * ((hist + 1) * 8 + 12));
+    w.lbfgs_bytes = (int64_t)(np * (2 + 2 * (size_t)(hist + 1)) + (size_t)batch * ((hist + 1) * 8 + 12));
+    *bytes += w.lbfgs_bytes;
     return 0;
 }
 

@@ -655,6 +655,14 @@ def test_lbfgs_backend_batch_is_independent(torch_cuda, path):
     xb, nfb = p.cpu().numpy(), nf.cpu().numpy()
     assert np.all(xb >= lo) and np.all(xb <= hi) and np.all(nfb < nll0.sum(axis=1))
     off = w.param_offsets()
+    # the workspace is counted once: a longer history replaces the ring (S, Y: 2 x nparam, s.y: batch doubles per slot),
+    # a shorter or equal one reuses it
+    ws10 = ctx.workspace_bytes()
+    for hist, grow in ((14, 4), (14, 4), (5, 4)):
+        q = torch.from_numpy(w.params_const()).cuda()
+        ctx.optimize(q, lo_d, hi_d, cs.opt_defaults(iters=2, method=cs.METHOD_LBFGS, history=hist), None)
+        torch.cuda.synchronize()
+        assert ctx.workspace_bytes() - ws10 == grow * 8 * (2 * int(off[-1]) + w.batch)
     for e in (0, 3):
         ctx.set_batch(w.cfg_of[e:e + 1], w.data_of[e:e + 1])
         sl = slice(off[e], off[e + 1])
