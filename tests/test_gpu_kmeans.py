@@ -1,11 +1,14 @@
-"""f2: cs_spherical_kmeans (GPU, batched) against gen/kmeans.py (numpy) -- labels must agree bit for bit (index work).
-The random numbers of the method (the initial centroids) are drawn by gen's seeded generator and passed to both."""
+"""f2: cs_spherical_kmeans (GPU, batched) against the K-means reference oracle/kmeans.py (pinned in
+tests/test_kmeans_oracle.py) -- labels must agree bit for bit (index work).  The random numbers of the method (the
+initial centroids) are drawn by gen's seeded generator and passed to both; that the generator's own maps equal the
+reference's is a CPU test (tests/test_kmeans_oracle.py)."""
 import numpy as np
 import pytest
 
 import gen
 from gen import kmeans as gk
 from gen import sky
+from oracle import kmeans as ok
 
 pytestmark = pytest.mark.gpu
 
@@ -61,10 +64,17 @@ def _gpu_cluster_maps(vecs, specs, region_idx=None, nregion=1, iters=10):
     return out
 
 
+def _oracle_map(vecs, param, K, region_idx=None, nregion=1):
+    def cent0(r, sel):
+        seed = (param * 1_000_003 + K) * 16 + (0 if r is None else r + 1)
+        return gk.initial_centroids(vecs[sel], K, sky.rng_for("kmeans", seed), seed_from_pixels=r is not None)
+    return ok.patch_map(vecs, K, cent0, region_idx, nregion)
+
+
 def _check(vecs, specs, region_idx=None, nregion=1):
     got = _gpu_cluster_maps(vecs, specs, region_idx, nregion)
     for param, K in specs:
-        want, ktot = gen.cluster_map(vecs, param, K, region_idx, nregion)
+        want, ktot = _oracle_map(vecs, param, K, region_idx, nregion)
         lab, k2 = got[(param, K)]
         assert k2 == ktot
         assert np.array_equal(lab, want), (param, K, int((lab != want).sum()))
@@ -109,6 +119,8 @@ def test_kmeans_is_deterministic_and_handles_empty_patches():
         torch.cuda.synchronize()
         outs.append((lab.cpu().numpy(), cent.cpu().numpy()))
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    lab_ref, cent_ref = ok.lloyd(vecs, cent0, iters=10)       # labels and final centroids of the reference, bit for bit
+    assert np.array_equal(outs[0][0][0], lab_ref) and np.array_equal(outs[0][1], cent_ref)
     assert np.allclose(np.linalg.norm(outs[0][1], axis=1), 1.0, atol=1e-15)
     # no iteration: the duplicate loses every tie; one iteration: it was empty during the update and keeps its centroid
     res = {}
