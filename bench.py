@@ -14,7 +14,8 @@ Inputs are seeded and synthetic (gen/); see DESIGN.md "Input recipe".
 and the max over ranks only.
 
 Prints ONE JSON line (rank 0).  Keys beyond the base contract: `roofline`, `cpu_baseline`, `e2e`, `clocks`,
-`gpu_launches`, `parity` (GPU vs oracle on the cpu_baseline sample), `extras` (every other BASELINE configuration).
+`gpu_launches`, `parity` (GPU vs oracle on the cpu_baseline sample), `extras` (every other BASELINE configuration, the
+cell-size sweep, f2, f3) and, as the LAST key, `configs`: one short array per configuration (summary_of).
 """
 import argparse
 import json
@@ -200,6 +201,14 @@ def kernel_name(ctx, w, nfreq):
     return " + ".join(names)
 
 
+def copies_bytes(ctx, w):
+    """Bytes of the private cell-sorted copies of the batch: one per distinct (sorted configuration, data set) pair, its
+    tiles x 512 positions x nfreq x (Q, U) x fp32."""
+    info = {int(c): ctx.layout_info(int(c)) for c in np.unique(w.cfg_of)}
+    pairs = {(int(c), int(d)) for c, d in zip(w.cfg_of, w.data_of) if info[int(c)][0]}
+    return sum(info[c][1] * 512 * w.nfreq * 2 * 4 for c, _ in pairs)
+
+
 def time_hot_path(ctx, w, params, steps, warmup, dev, stream, barrier=None):
     """W warm-up steps, then K timed steps of (tables + likelihood/gradient) with CUDA events on `stream`.
     Returns dict(ms, kernel_ms (fused kernels per step), launches, nll, grad)."""
@@ -272,8 +281,9 @@ def extra_workload(cs, name, batch, steps, dev, stream, peak, prefixes=None):
                   # d-stream accounting (120 B per pixel-eval): every entry streams its own (private) data
                   "roofline_frac_of_measured_peak": BYTES_PER_PIXEL_EVAL * pe / (r["kernel_ms_per_step"] * 1e-3) / 1e9 / peak
                   if r["kernel_ms_per_step"] > 0 else None,
+                  "distinct_data_sets": int(len(np.unique(wb.data_of))),
                   "configurations_sorted": sorted_cfgs, "configurations": int(len(np.unique(wb.cfg_of))),
-                  "streams_read_per_step": streams, "workspace_GB": ctx.workspace_bytes() / 1e9,
+                  "streams_read_per_step": streams, "workspace_GB": ctx.workspace_bytes() / 1e9, "copies_GB": copies_bytes(ctx, wb) / 1e9,
                   "datagen_s": round(t_gen, 1), "set_clusters_and_data_s": round(t_setup, 1), "set_batch_s": round(t_batch, 3)}
     ctx.close()
     del d_dev
@@ -346,6 +356,107 @@ def extra_kmeans(cs, dev):
         times.append(time.perf_counter() - t0)
     return {"workload": f"{len(probs)} K-means problems of the C3 scan, nside 64, K = {min(Ks)} .. {max(Ks)}, 10 Lloyd iterations",
             "ms": 1e3 * min(times), "dot_products_per_s": 11 * vecs.shape[0] * float(sum(Ks)) / min(times)}
+
+
+# K = (K_bd, K_Td, K_bs) of the cell-size sweep: from the paper's own optimum (beta_d per pixel, Table 2) through
+# the upper half of its grid (Table 1: K up to 10000 on regions of ~9800 pixels, i.e. 1-5 pixels per cell on
+# the full nside-64 sky at the same densities) down to the bench configuration.
+SWEEP_K = [(49152, 2500, 150), (25000, 5000, 1500), (12500, 2500, 750), (5000, 1500, 750), (3000, 1000, 600),
+           (2000, 800, 500), (1000, 500, 500), (500, 50, 100)]
+
+
+def extra_cellsweep(cs, dev, stream, peak, ndata=256, steps=5):
+    """Pixel-evals/s against the mean cell size (pixels per distinct cluster triple), nside 64, `ndata` entries with
+    their own noise realisation, on each layout: in place (direct kernel), sorted (sorted-cell kernel) and the
+    library's own choice (CS_OPT_MIN_FILL).  The patch maps come from the library's own K-means (cs_spherical_kmeans,
+    seeded starts from gen): the numpy generator would need minutes for K = 25000."""
+    import dataclasses
+    import torch
+    from gen import kmeans as gk
+    w0 = gen.make_config(1, ndata=ndata)
+    vecs = gen.pix2vec_ring(w0.nside)
+    npix = w0.npix
+    specs = sorted({(prm, int(K[prm])) for K in SWEEP_K for prm in range(3) if 1 < K[prm] < npix})
+    cent0 = np.concatenate([gk.initial_centroids(vecs, K, gen.rng_for("kmeans", (prm * 1_000_003 + K) * 16)) for prm, K in specs])
+    lab = torch.zeros((len(specs), npix), dtype=torch.int32, device=dev)
+    cs.spherical_kmeans(torch.from_numpy(vecs).to(dev), [K for _, K in specs], torch.from_numpy(cent0).to(dev), lab, iters=10)
+    torch.cuda.synchronize()
+    lab = lab.cpu().numpy()
+    maps_of = {s: lab[i] for i, s in enumerate(specs)}
+    d_dev = torch.from_numpy(w0.data()).to(dev)
+    rows = []
+    for K in SWEEP_K:
+        maps = np.stack([np.arange(npix, dtype=np.int32) if K[prm] >= npix else maps_of[(prm, int(K[prm]))] for prm in range(3)])
+        Kmap = np.array([min(k, npix) for k in K], dtype=np.int32)
+        w = dataclasses.replace(w0, maps=np.ascontiguousarray(maps), Kmap=Kmap)
+        params = w.params_jittered(seed=7)
+        ncell = len(np.unique(maps[0].astype(np.int64) * (int(Kmap[1]) * int(Kmap[2])) + maps[1].astype(np.int64) * int(Kmap[2]) + maps[2]))
+        row = {"K": list(K), "pixels_per_cell": npix / ncell}
+        for key, layout in (("inplace", cs.LAYOUT_INPLACE), ("sorted", cs.LAYOUT_SORTED), ("auto", cs.LAYOUT_AUTO)):
+            try:
+                ctx = cs.Context(w.freqs, w.npix, options={"layout": layout})
+                ctx.set_clusters(w.maps, w.Kmap, w.cfg_maps, w.region_idx, w.nregion)
+                ctx.set_data(d_dev, w.ninv)
+                ctx.set_batch(w.cfg_of, w.data_of)
+                r = time_hot_path(ctx, w, params, steps, 3, dev, stream)
+                srt, _, fill = ctx.layout_info(0)
+                row[key] = float(w.batch) * npix / (r["ms"] / steps * 1e-3)
+                if key == "sorted":
+                    row["fill"] = fill
+                    row["copies_GB"] = copies_bytes(ctx, w) / 1e9
+                if key == "auto":
+                    row["auto_kernel"] = "sc" if srt else "direct"
+                ctx.close()
+            except Exception as exc:
+                row[key] = None
+                row[key + "_error"] = repr(exc)
+            torch.cuda.empty_cache()
+        rows.append(row)
+    del d_dev
+    torch.cuda.empty_cache()
+    return {"workload": f"nside 64, {ndata} entries x distinct noise realisations, K swept", "steps": steps, "rows": rows}
+
+
+def _short_kernel(name):
+    return "+".join(k for k, tag in (("sc", "k_like_sc"), ("direct", "k_like_direct")) if tag in (name or ""))
+
+
+def summary_of(out, peak):
+    """Every configuration on one screen, as the LAST key of the line (a record that keeps only the tail of the line
+    still shows it).  Per configuration: [ms per step, G pixel-evals/s, fraction of the measured HBM peak counting the
+    bytes each entry streams (120 B per pixel-eval: every entry reads its own, private or distinct, data), the same
+    fraction counting only the DISTINCT data bytes of the step (the compulsory traffic: for a scan of configurations
+    over shared data the streamed bytes are replicas, not algorithmic bytes), kernel]."""
+    ex = out.get("extras", {})
+    s = {"fmt": "[ms/step, G pixel-evals/s, frac of HBM peak by streamed per-entry bytes, frac by distinct-data bytes, kernel]"}
+    rf = out["roofline"]
+    s["c3h"] = [round(out["ms_per_step"], 4), round(out["value"] / out["n_gpus"] / 1e9, 2), round(rf["frac"], 3), round(rf["frac"], 3), _short_kernel(rf["kernel"])]
+    for key in ("c3", "c4", "kmax", "c5_batch1", "c5_batch16", "c5_batch64", "c5_batch256"):
+        e = ex.get(key)
+        if not e or "error" in e:
+            continue
+        fr = e.get("roofline_frac_of_measured_peak")
+        s[key] = [round(e["ms_per_step"], 4), round(e["pixel_evals_per_s"] / 1e9, 2), None if fr is None else round(fr, 3),
+                  None if fr is None else round(fr * e["distinct_data_sets"] / e["batch"], 4), _short_kernel(e["kernel"])]
+    c2 = ex.get("c2")
+    if c2:
+        s["c2"] = {"like_grad_call_us": round(c2["like_grad_call_us"], 1), "adatopk_200_iters_ms": round(c2["optimize_200_iters_ms"], 2),
+                   "lbfgs_100_iters_ms": round(c2["lbfgs_100_iters_ms"], 2)}
+    sw = ex.get("cellsweep")
+    if sw and "rows" in sw:
+        g = lambda v: None if v is None else round(v / 1e9, 1)
+        s["cellsweep_fmt"] = "[pixels per cell, sorted fill, G pixel-evals/s in place, sorted, auto, auto's kernel]"
+        s["cellsweep"] = [[round(r["pixels_per_cell"], 2), round(r.get("fill") or 0, 3), g(r.get("inplace")), g(r.get("sorted")), g(r.get("auto")),
+                           r.get("auto_kernel")] for r in sw["rows"]]
+    for key in ("f3_cells_c3", "f3_cells_c3h", "f3_cells_c4"):
+        e = ex.get(key)
+        if e and "error" not in e:
+            s[key] = [round(e["ms_per_step"], 4), round(e["pixel_evals_equivalent_per_s"] / 1e9, 1), round(e["workspace_GB"], 2)]
+    if "f2_kmeans" in ex and "ms" in ex["f2_kmeans"]:
+        s["f2_kmeans_ms"] = round(ex["f2_kmeans"]["ms"], 2)
+    if "component_maps_GBps" in ex:
+        s["maps_GBps"] = round(ex["component_maps_GBps"], 0)
+    return s
 
 
 def relaunch_multi_gpu(args):
@@ -467,11 +578,13 @@ def main():
            "dtype": "f32 (fp64 tables and reductions)", "data": "synthetic",
            "config": {"workload": desc, "nside": w.nside, "npix": w.npix, "batch_per_gpu": w.batch, "nfreq": w.nfreq,
                       "l2": "inputs larger than L2 (no flush)" if d_dev.numel() * 4 > 2 * 126e6 else "inputs fit in L2: L2-resident by design of this workload",
-                      "step": "cs_build_sed_tables + cs_spectral_like_grad(value+grad)", "datagen_s": round(t_gen, 1),
-                      "layout": {"sorted_configurations": sum(1 for f in fills if f[0]), "configurations": len(fills),
-                                 "fill": min(f[2] for f in fills),
-                                 "set_batch_s (allocates and gathers the private sorted copies, once per batch)": round(t_batch, 4),
-                                 "workspace_GB": ctx.workspace_bytes() / 1e9}},
+                      "step": "cs_build_sed_tables + cs_spectral_like_grad(value+grad); the fused kernel reads private cell-sorted "
+                              "copies of d made once per data set in cs_set_batch / cs_set_data (relayout_ms_once, outside the "
+                              "timed region; inside it in e2e)",
+                      "datagen_s": round(t_gen, 1), "sorted_configurations": sum(1 for f in fills if f[0]),
+                      "configurations": len(fills), "fill_min": min(f[2] for f in fills),
+                      "relayout_ms_once": round(1e3 * t_batch, 2), "workspace_GB": ctx.workspace_bytes() / 1e9,
+                      "copies_GB": copies_bytes(ctx, w) / 1e9},
            "roofline": roofline, "clocks": clocks, "gpu_launches": int(r["launches"])}
 
     # ---- end to end through the C ABI with host buffers (H2D of d and params, D2H of nll and grad inside); every
@@ -551,9 +664,9 @@ def main():
                     o += kk
             out["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                                    "sample": f"first {n} entries x {w.npix} pixels of the same workload",
-                                   "one_thread": {"value": val1, "cores": cores1,
-                                                  "sample": f"first {n1} entries x {w.npix} pixels"}}
+                                   "value_1thread": val1, "sample_1thread": f"first {n1} entries x {w.npix} pixels, {cores1} thread"}
             out["parity"] = {"entries": n, "max_rel_err_nll": e_nll,
+                             "grad_block_rel_l2_beta_d": blk[0], "grad_block_rel_l2_T_d": blk[1], "grad_block_rel_l2_beta_s": blk[2],
                              "grad_block_rel_l2_unfloored (beta_d, T_d, beta_s): max ||dg||_2 / ||g_ref||_2": blk,
                              "grad_worst_cluster_rel_unfloored: max |dg_k| / |g_ref_k|": worst_cluster,
                              "max_grad_err_over_T2_bound": e_g, "T2_term_binding_at_the_worst_cluster": binds,
@@ -638,12 +751,15 @@ def main():
                     out["extras"][nm] = {"error": repr(exc)}
             for key, fn in (("f3_cells_c3", lambda: extra_cells(cs, "c3", 0, 5, dev, stream)),
                             ("f3_cells_c3h", lambda: extra_cells(cs, "c3h", 256, 5, dev, stream)),
-                            ("f2_kmeans", lambda: extra_kmeans(cs, dev))):
+                            ("f3_cells_c4", lambda: extra_cells(cs, "c4", 0, 5, dev, stream)),
+                            ("f2_kmeans", lambda: extra_kmeans(cs, dev)),
+                            ("cellsweep", lambda: extra_cellsweep(cs, dev, stream, peak))):
                 try:
                     out["extras"][key] = fn()
                 except Exception as exc:
                     out["extras"][key] = {"error": repr(exc)}
     if rank == 0:
+        out["configs"] = summary_of(out, peak)     # last key on purpose
         print(json.dumps(out), flush=True)
     if dist is not None:
         dist.barrier()

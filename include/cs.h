@@ -57,8 +57,9 @@ extern "C" {
 #define CS_OPT_LAYOUT        1 /* CS_LAYOUT_*; set before cs_set_clusters */
 #define CS_OPT_FORM          2 /* CS_FORM_*; set before cs_set_batch */
 #define CS_OPT_MIN_FILL      3 /* CS_LAYOUT_AUTO: smallest fill fraction live pixels / (tiles * 512) of a configuration's
-                                  sorted layout for which it is taken (default 0.45: below it the padding
-                                  costs more than the direct kernel); set before cs_set_clusters */
+                                  sorted layout for which it is taken (default 0.36, the measured crossover: below
+                                  it, about 2.9 pixels per cell, streaming the padding costs more than the direct
+                                  kernel's gathers; bench.py cellsweep); set before cs_set_clusters */
 #define CS_OPT_COPY_LIMIT_MB 4 /* most device memory [MiB] the private sorted copies of a batch may take; 0 (default) =
                                   70 % of the memory free when cs_set_batch runs.  Beyond it cs_set_batch returns CS_ENOMEM. */
 #define CS_OPT_PIXEL_BETA    5 /* CS_PIXBETA_*; set before cs_set_clusters */
@@ -153,7 +154,15 @@ CS_API int cs_set_data(cs_ctx *ctx, int32_t ndata, const float *d, const float *
 
 /* Batch: entry e evaluates configuration cfg_of[e] on data set data_of[e] (both host [batch]).  Allocates the
  * SED tables, the reduction workspace and the private sorted copies for this batch (the only allocation outside
- * cs_create/cs_set_clusters) and, when the data are set, gathers the copies (synchronous). */
+ * cs_create/cs_set_clusters) and, when the data are set, gathers the copies (synchronous).
+ * Memory: every distinct (sorted configuration, data set) pair of the batch holds one private copy of
+ * ntile x 512 positions x nfreq x 2 x 4 B (ntile from cs_layout_info: 61440 B a tile at nfreq 15; 6.0 MB a pair at
+ * nside 64 with well filled tiles, 1 / fill times the data otherwise), within CS_OPT_COPY_LIMIT_MB, else CS_ENOMEM with
+ * the context left as after cs_set_clusters.  A job larger than that -- the paper's 13,824 configurations x 40
+ * realisations on three regions is 552,960 pairs = 3.5 TB of copies -- is walked by the caller in
+ * batches: keep the 40 data sets resident (cs_set_data once), and per batch call cs_set_clusters with a slice of the
+ * configurations (about 500 of them x 40 realisations = 20,000 pairs fill 70 % of a 180-GB B200) and cs_set_batch;
+ * configurations never interact, so results do not depend on the slicing. */
 CS_API int cs_set_batch(cs_ctx *ctx, int32_t batch, const int32_t *cfg_of, const int32_t *data_of);
 
 /* off host [batch+1] int64: parameter offsets of the current batch. */
@@ -217,7 +226,7 @@ CS_API int cs_cmb_variance(cs_ctx *ctx, double *var, void *stream);
  * cs_spectral_like_grad (value + gradient, once per iteration) and cs_spectral_misfit (the objective of the line-search
  * trials: 1/2 chi^2 = nll + const, R13 -- a deviation from north_star's "only the first two").
  * params dev in: start, out: result; lower/upper dev, same layout; nll_final dev [batch] (summed over regions) or
- * NULL.  batch <= 65535 (CS_EINVAL beyond).  No host synchronisation.  The iteration body is captured
+ * NULL.  Any batch size (the per-entry kernels put the entry on grid.x).  No host synchronisation.  The iteration body is captured
  * into a CUDA graph and replayed unless `stream` is itself being captured; on the legacy default stream the work is
  * forked onto an internal stream and joined back before the call returns (still asynchronous to the host).
  * Line-search trials skip the entries that have already accepted a step. */

@@ -128,7 +128,7 @@ struct cs_ctx {
     bool have_ninv = false;
     // options (cs_set_option)
     int32_t opt_layout = CS_LAYOUT_AUTO, opt_form = CS_FORM_AUTO, opt_pixbeta = CS_PIXBETA_AUTO;
-    double opt_min_fill = 0.45;
+    double opt_min_fill = 0.36;         // measured crossover of the two kernels (bench.py cellsweep)
     int64_t opt_copy_limit = 0;         // bytes, 0 = 70 % of the free device memory when the batch is set
     // clusters
     int32_t nmap = 0, ncfg = 0, nregion = 1;
@@ -1377,8 +1377,7 @@ int cs_optimize(cs_ctx *c, double *params, const double *lower, const double *up
                 void *stream) {
     int rc = ready(c);
     if (rc) return rc;
-    if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || !(opt->ls_noise >= 0) || !(opt->topk >= 0.0 && opt->topk <= 1.0) ||
-        c->batch > 65535)
+    if (!params || !lower || !upper || !opt || opt->iters < 0 || opt->ls_max < 1 || !(opt->ls_noise >= 0) || !(opt->topk >= 0.0 && opt->topk <= 1.0))
         return CS_EINVAL;
     const bool lbfgs = opt->method == CS_METHOD_LBFGS;
     if (opt->method != CS_METHOD_ADATOPK && !lbfgs) return CS_EINVAL;
@@ -1582,29 +1581,34 @@ int cs_eval_host(cs_ctx *c, int32_t ndata, const float *d_host, const float *nin
 
 int cs_spherical_kmeans(int64_t npix, const double *vecs, const uint8_t *region, int32_t nprob, const int32_t *K,
                         const int32_t *prob_region, double *cent, int32_t iters, int32_t *labels, void *stream) {
-    if (npix <= 0 || !vecs || nprob <= 0 || nprob > 65535 || !K || !cent || iters < 0 || !labels) return CS_EINVAL;
+    if (npix <= 0 || !vecs || nprob <= 0 || !K || !cent || iters < 0 || !labels) return CS_EINVAL;
     CS_GUARD_BEGIN
     cudaStream_t st = (cudaStream_t)stream;
     std::vector<KmProb> pr(nprob);
     int64_t off = 0;
-    int32_t kmax = 0;
     for (int32_t j = 0; j < nprob; ++j) {
         if (K[j] < 1) return CS_EINVAL;
         const int32_t reg = prob_region ? prob_region[j] : -1;
         if (reg >= 0 && !region) return CS_EINVAL;
         pr[j] = KmProb{K[j], reg, off};
         off += K[j];
-        kmax = std::max(kmax, K[j]);
     }
     KmProb *d_pr = nullptr;
     if (cudaMallocAsync((void **)&d_pr, sizeof(KmProb) * nprob, st) != cudaSuccess) return CS_ENOMEM;
     // pageable host memory: the copy has left the host buffer when cudaMemcpyAsync returns
     if (cudaMemcpyAsync(d_pr, pr.data(), sizeof(KmProb) * nprob, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaFreeAsync(d_pr, st); return CS_ECUDA; }
-    const dim3 ga((unsigned)((npix + 255) / 256), nprob), gu((kmax + 7) / 8, nprob);
-    k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
-    for (int32_t it = 0; it < iters; ++it) {
-        k_km_update<<<gu, 256, 0, st>>>(vecs, npix, d_pr, labels, cent);
-        k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr, cent, labels);
+    // problems are independent: more than 65535 of them (the limit of grid.y) go in slices, one after the other
+    for (int32_t j0 = 0; j0 < nprob; j0 += 65535) {
+        const int32_t nj = std::min<int32_t>(65535, nprob - j0);
+        int32_t kmax_j = 0;
+        for (int32_t j = j0; j < j0 + nj; ++j) kmax_j = std::max(kmax_j, K[j]);
+        const dim3 ga((unsigned)((npix + 255) / 256), nj), gu((kmax_j + 7) / 8, nj);
+        int32_t *lab_j = labels + (int64_t)j0 * npix;
+        k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr + j0, cent, lab_j);
+        for (int32_t it = 0; it < iters; ++it) {
+            k_km_update<<<gu, 256, 0, st>>>(vecs, npix, d_pr + j0, lab_j, cent);
+            k_km_assign<<<ga, 256, 0, st>>>(vecs, npix, region, d_pr + j0, cent, lab_j);
+        }
     }
     const cudaError_t ce = cudaGetLastError();
     cudaFreeAsync(d_pr, st);

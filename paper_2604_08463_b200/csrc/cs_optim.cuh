@@ -294,10 +294,10 @@ __global__ void __launch_bounds__(OPT_THREADS) k_opt_direction(OptWork w, OptSha
     }
 }
 
-// trial point x_t = l + clamp(y + alpha d)(u - l); grid = (ceil(ktot_max/256), batch)
+// trial point x_t = l + clamp(y + alpha d)(u - l); grid = (batch, ceil(ktot_max/256)): the entry on grid.x, which has no 65535 limit
 __global__ void k_opt_trial(OptWork w, OptShape sh) {
-    const int e = blockIdx.y;
-    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int e = blockIdx.x;
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= sh.param_off[e + 1]) return;
     const double a = w.accepted[e] ? w.alpha_acc[e] : w.alpha[e];
     const double y = fmin(fmax(w.y[i] + a * w.dir[i], 0.0), 1.0);
@@ -325,10 +325,10 @@ __global__ void k_opt_ls(OptWork w, OptShape sh, OptHyper hy) {
 
 // lines 19-25: move, pin the limiting parameter if the step reached alpha_max
 __global__ void k_opt_commit(OptWork w, OptShape sh) {
-    const int e = blockIdx.y;
-    if (blockIdx.x == 0 && e == 0 && threadIdx.x == 0) *w.iter += 1;   // k_opt_direction of this iteration is done
-    if (blockIdx.x == 0 && threadIdx.x == 0 && w.accepted[e]) w.Lcur[e] = w.Lt_acc[e];
-    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int e = blockIdx.x;
+    if (blockIdx.y == 0 && e == 0 && threadIdx.x == 0) *w.iter += 1;   // k_opt_direction of this iteration is done
+    if (blockIdx.y == 0 && threadIdx.x == 0 && w.accepted[e]) w.Lcur[e] = w.Lt_acc[e];
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= sh.param_off[e + 1]) return;
     const double a = w.accepted[e] ? w.alpha_acc[e] : 0.0;
     double y = fmin(fmax(w.y[i] + a * w.dir[i], 0.0), 1.0);
@@ -472,24 +472,24 @@ __global__ void __launch_bounds__(OPT_THREADS) k_lb_direction(OptWork w, OptShap
     }
 }
 
-// trial point x_t = l + (u - l) sigma(z + alpha d); grid = (ceil(ktot_max/256), batch)
+// trial point x_t = l + (u - l) sigma(z + alpha d); grid = (batch, ceil(ktot_max/256)): the entry on grid.x, which has no 65535 limit
 __global__ void k_lb_trial(OptWork w, OptShape sh) {
-    const int e = blockIdx.y;
-    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int e = blockIdx.x;
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= sh.param_off[e + 1]) return;
     const double a = w.accepted[e] ? w.alpha_acc[e] : w.alpha[e];
     w.xt[i] = w.lo[i] + (w.hi[i] - w.lo[i]) * sigmoid_(w.z[i] + a * w.dir[i]);
 }
 
 __global__ void k_lb_commit(OptWork w, OptShape sh) {
-    const int e = blockIdx.y;
-    if (blockIdx.x == 0 && e == 0 && threadIdx.x == 0) *w.iter += 1;
+    const int e = blockIdx.x;
+    if (blockIdx.y == 0 && e == 0 && threadIdx.x == 0) *w.iter += 1;
     const bool acc = w.accepted[e] != 0;
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
+    if (blockIdx.y == 0 && threadIdx.x == 0) {
         if (acc) w.Lcur[e] = w.Lt_acc[e];
         w.moved[e] = acc ? 1 : 0;
     }
-    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i = sh.param_off[e] + (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
     if (i >= sh.param_off[e + 1] || !acc) return;
     const double z = w.z[i] + w.alpha_acc[e] * w.dir[i];
     w.z[i] = z;
@@ -505,11 +505,11 @@ inline void lb_direction(OptWork &w, const OptShape &sh, int32_t hist, double cu
     k_lb_direction<<<sh.batch, OPT_THREADS, 0, st>>>(w, sh, hist, curv_eps);
 }
 inline void lb_trial_point(OptWork &w, const OptShape &sh, cudaStream_t st) {
-    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    dim3 grid(sh.batch, (sh.ktot_max + 255) / 256);
     k_lb_trial<<<grid, 256, 0, st>>>(w, sh);
 }
 inline void lb_commit(OptWork &w, const OptShape &sh, cudaStream_t st) {
-    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    dim3 grid(sh.batch, (sh.ktot_max + 255) / 256);
     k_lb_commit<<<grid, 256, 0, st>>>(w, sh);
 }
 
@@ -522,7 +522,7 @@ inline void opt_direction(OptWork &w, const OptShape &sh, const OptHyper &hy, cu
     k_opt_direction<<<sh.batch, OPT_THREADS, 0, st>>>(w, sh, hy);
 }
 inline void opt_trial_point(OptWork &w, const OptShape &sh, cudaStream_t st) {
-    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    dim3 grid(sh.batch, (sh.ktot_max + 255) / 256);
     k_opt_trial<<<grid, 256, 0, st>>>(w, sh);
 }
 inline void opt_ls_update(OptWork &w, const OptShape &sh, const OptHyper &hy, cudaStream_t st) {
@@ -532,7 +532,7 @@ inline void opt_set_L(OptWork &w, const OptShape &sh, cudaStream_t st) {
     k_opt_setL<<<(sh.batch + 127) / 128, 128, 0, st>>>(w, sh);
 }
 inline void opt_commit(OptWork &w, const OptShape &sh, cudaStream_t st) {
-    dim3 grid((sh.ktot_max + 255) / 256, sh.batch);
+    dim3 grid(sh.batch, (sh.ktot_max + 255) / 256);
     k_opt_commit<<<grid, 256, 0, st>>>(w, sh);
 }
 inline void opt_finish(OptWork &w, const OptShape &sh, double *params, double *nll_final, cudaStream_t st) {

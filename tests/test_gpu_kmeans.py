@@ -132,3 +132,20 @@ def test_kmeans_is_deterministic_and_handles_empty_patches():
         res[iters] = (lab.cpu().numpy(), cent.cpu().numpy())
     assert not np.any(res[0][0] == 8) and np.any(res[0][0] == 3) and np.array_equal(res[0][1], cent0)
     assert np.array_equal(res[1][1][8], cent0[8]) and not np.array_equal(res[1][1][3], cent0[3])
+
+
+def test_kmeans_takes_more_than_65535_problems():
+    """Problems beyond the 65535 of grid.y go in slices: here all the same problem, so every row of labels and every
+    block of centroids equals the reference's."""
+    import torch
+    import paper_2604_08463_b200 as cs
+    vecs = gen.pix2vec_ring(4)
+    nprob, K = 65535 + 9, 3
+    c0 = gk.initial_centroids(vecs, K, sky.rng_for("misc", 77))
+    cent = torch.from_numpy(np.tile(c0, (nprob, 1))).cuda()
+    lab = torch.full((nprob, vecs.shape[0]), -7, dtype=torch.int32, device="cuda")
+    cs.spherical_kmeans(torch.from_numpy(vecs).cuda(), np.full(nprob, K, dtype=np.int32), cent, lab, iters=3)
+    torch.cuda.synchronize()
+    lab_ref, cent_ref = ok.lloyd(vecs, c0, iters=3)
+    assert torch.equal(lab, torch.from_numpy(lab_ref).cuda().expand(nprob, -1))
+    assert np.array_equal(cent.cpu().numpy().reshape(nprob, K, 3), np.broadcast_to(cent_ref, (nprob, K, 3)))

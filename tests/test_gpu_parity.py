@@ -1015,3 +1015,61 @@ def test_two_contexts_on_two_devices(torch_cuda):
             res.append((nll.cpu().numpy(), grad.cpu().numpy()))
             ctx.close()
     assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+
+
+def test_copy_limit_gives_enomem_and_leaves_the_context_usable(torch_cuda):
+    """CS_OPT_COPY_LIMIT_MB: a batch whose private sorted copies would not fit is refused with CS_ENOMEM before anything
+    is computed; the same context then takes a smaller batch, or the same one under a larger limit, and gives the bits of
+    a context that never failed."""
+    import paper_2604_08463_b200 as cs
+    w = gen.make_config(1, nside=16, K=(40, 10, 20), ndata=12)      # 12 pairs x 6 tiles x 61440 B = 4.4 MB of copies
+    params = w.params_jittered(seed=3)
+    ref_ctx, d_dev = make_ctx(w, options={"layout": cs.LAYOUT_SORTED})
+    nll_ref, grad_ref = gpu_eval(ref_ctx, params)
+    ref_ctx.close()
+    ctx = new_ctx(w.freqs, w.npix, options={"layout": cs.LAYOUT_SORTED, "copy_limit_mb": 1})
+    ctx.set_clusters(w.maps, w.Kmap, w.cfg_maps, w.region_idx, w.nregion)
+    ctx.set_data(d_dev, w.ninv)
+    with pytest.raises(cs.CsError) as err:
+        ctx.set_batch(w.cfg_of, w.data_of)
+    assert err.value.code == cs.ENOMEM
+    off = w.param_offsets()
+    ctx.set_batch(w.cfg_of[:2], w.data_of[:2])                      # two pairs fit under 1 MiB
+    nll2, grad2 = gpu_eval(ctx, params[:off[2]])
+    assert np.array_equal(nll2, nll_ref[:2]) and np.array_equal(grad2, grad_ref[:off[2]])
+    ctx.set_option("copy_limit_mb", 64)
+    ctx.set_batch(w.cfg_of, w.data_of)
+    nll, grad = gpu_eval(ctx, params)
+    assert np.array_equal(nll, nll_ref) and np.array_equal(grad, grad_ref)
+    assert ctx.check() == 0
+    ctx.close()
+
+
+def test_optimizer_takes_more_than_65535_entries(torch_cuda):
+    """The per-entry optimizer kernels index the entry on grid.x: a batch beyond the 65535 of grid.y runs, and every
+    entry -- all the same problem here -- ends where a batch of one ends, bit for bit."""
+    import torch
+    import paper_2604_08463_b200 as cs
+    B = 65536 + 700
+    w = gen.make_config(0, batch=B)
+    assert w.batch == B and w.ndata == 1
+    ctx, _ = make_ctx(w)
+    lo, hi = _bounds(w)
+    n1 = int(w.param_offsets()[1])
+    for method in (cs.METHOD_ADATOPK, cs.METHOD_LBFGS):
+        p = torch.from_numpy(w.params_const()).cuda()
+        nf = torch.zeros(B, dtype=torch.float64, device="cuda")
+        ctx.optimize(p, torch.from_numpy(lo).cuda(), torch.from_numpy(hi).cuda(), cs.opt_defaults(iters=3, method=method), nf)
+        torch.cuda.synchronize()
+        assert ctx.check() == 0
+        x = p.cpu().numpy().reshape(B, n1)
+        assert np.all(x == x[0]) and np.all(nf.cpu().numpy() == nf[0].item())
+        assert not np.array_equal(x[0], w.params_const()[:n1])
+        ctx.set_batch(w.cfg_of[:1], w.data_of[:1])
+        p1 = torch.from_numpy(w.params_const()[:n1]).cuda()
+        nf1 = torch.zeros(1, dtype=torch.float64, device="cuda")
+        ctx.optimize(p1, torch.from_numpy(lo[:n1]).cuda(), torch.from_numpy(hi[:n1]).cuda(), cs.opt_defaults(iters=3, method=method), nf1)
+        torch.cuda.synchronize()
+        assert np.array_equal(p1.cpu().numpy(), x[0]) and nf1.item() == nf[0].item()
+        ctx.set_batch(w.cfg_of, w.data_of)
+    ctx.close()
